@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched-LM hot path on B200 (contract: see DESIGN.md section 6).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload C4|C2|C3|C5]
+
+One "step" = one pass of the whole hot path (S0..S10: load seeds + targets, the on-device LM loop,
+store) over one batch of synthetic input: ``lm_reset`` + ``lm_run(max_iters)``.  The headline
+workload is BASELINE.json configs[3] (4096 trajectories x 300 waypoints, 7-DoF Panda, 50 LM
+iterations) -- the configuration the north_star's roofline target is quoted on.  Metric:
+waypoint-LM-iterations/s (executed iterations only), whole job.
+
+N > 1 (torchrun): every rank refines its own batch of the same shape (trajectories are
+independent units, no data-path collective) -> weak scaling; time = max over ranks.
+
+`--impl reference` times the fp64 CPU oracle (oracle/) on the host cores on a bounded sample of
+the same workload (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "waypoint_lm_iterations_per_sec"
+UNIT = "waypoint-iterations/s"
+
+# Algorithmic FLOPs per waypoint-iteration (DESIGN.md section 6 / SURVEY.md section 8d; FMA = 2).
+ALG_FLOP = {7: 1459.0, 8: 1762.0}
+# FP32 FMA-pipe peak derived from the guide's unit counts and clocks: 148 SMs x 128 lanes x 2 x f_max
+SM_COUNT, FP32_LANES = 148, 128
+
+
+def load_peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        d["_source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "_source": "fallback"}
+
+
+def alg_bytes_per_waypoint(d: int) -> float:
+    """S0 + S10 traffic per waypoint per run: seeds 4d + target 28 in;
+    q 4d + lambda, |r|, pos, rot 16 + iters/status 4 + mask 8 out."""
+    return 4 * d + 28 + 4 * d + 16 + 4 + 8
+
+
+# ------------------------------------------------------------------ clocks sampler
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.lines, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.FIELDS}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            return self
+        self.thread = threading.Thread(target=lambda: [self.lines.append(ln) for ln in self.proc.stdout], daemon=True)
+        self.thread.start()
+        return self
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=5)
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------ distributed plumbing
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def dist_init(backend: str):
+    import torch.distributed as dist
+    rank, _, world = dist_env()
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, world
+
+
+def dist_barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.barrier()
+
+
+def dist_max_sum(ms: float, units: float, device) -> tuple:
+    """(max over ranks of ms, sum over ranks of units) -- the only cross-rank quantities of the
+    path (trajectories are independent units; there is no data-path collective)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return ms, units
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    u = torch.tensor([units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def rank_seed_offset(rank: int) -> int:
+    """Each rank draws its own batch (weak scaling): the workload seed is offset by 1000 * rank."""
+    return 1000 * rank
+
+
+# ------------------------------------------------------------------ workloads
+
+def make_workload(name: str, fk, B: int | None, n: int | None, rank: int = 0):
+    from paper_2309_09102_b200 import workloads as wl
+    kw = {"seed_offset": rank_seed_offset(rank)}
+    if B:
+        kw["B"] = B
+    if n:
+        kw["n"] = n
+    if name == "C4":
+        return wl.config4(fk, **kw)
+    if name == "C2":
+        return wl.config2(fk, **kw)
+    if name == "C3":
+        return wl.config3(fk, **kw)
+    if name == "C5":
+        kw.setdefault("B", 4096)
+        kw.setdefault("n", 300)
+        return wl.config5(fk, **kw)
+    raise SystemExit(f"unknown workload {name}")
+
+
+def workload_desc(w) -> dict:
+    return {"workload": f"{w.name}: {w.B} trajectories x {w.n} waypoints, {w.chain.dof}-DoF {w.chain.name}, "
+                        f"tol={w.tol:g}, max_iters={w.max_iters}, lambda0={w.lambda0:g}",
+            "B": w.B, "n": w.n, "dof": int(w.chain.dof), "max_iters": w.max_iters, "tol": w.tol}
+
+
+# ------------------------------------------------------------------ CPU oracle legs
+
+def time_oracle(w, n_traj: int, steps: int = 1, warmup: int = 0) -> dict:
+    """The oracle as it stands, on the host cores, on the first n_traj trajectories of w."""
+    from oracle import lm_oracle as orc
+    sub = w.subset(slice(0, min(n_traj, w.B)))
+    prm = orc.Params(lambda0=sub.lambda0, tol=sub.tol)
+    tp, tq, s = sub.target_pos.astype(np.float64), sub.target_quat.astype(np.float64), sub.seeds.astype(np.float64)
+    times, executed = [], 0
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        st = orc.lm_run(sub.chain, prm, tp, tq, s, sub.max_iters)
+        dt = time.perf_counter() - t0
+        if i >= warmup:
+            times.append(dt)
+            executed += st.executed
+    total = float(sum(times))
+    return {"value": executed / total, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "sample": f"first {sub.B} of {w.B} trajectories ({sub.W} waypoints, {executed // max(steps, 1)} "
+                      f"waypoint-iterations per step), fp64, OpenMP over waypoints",
+            "seconds": total, "ms_per_step": 1e3 * total / max(steps, 1), "traj_per_s": sub.B * steps / total}
+
+
+def run_reference(args) -> None:
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    from oracle import lm_oracle as orc
+    from paper_2309_09102_b200 import workloads as wl
+    chain = wl.random_chain_8dof(3) if args.workload == "C3" else wl.panda_chain()
+    n_traj = args.ref_traj or 64
+    # only the sampled trajectories are generated (the generators are per-trajectory independent
+    # in distribution, the sample is a prefix of a smaller batch of the same recipe)
+    w = make_workload(args.workload, lambda q: orc.fk(chain, q), n_traj, args.n)
+    r = time_oracle(w, n_traj, steps=args.steps, warmup=min(args.warmup, 1))
+    full = workload_desc(w)
+    full["workload"] += f" [oracle timed on a {n_traj}-trajectory sample of the {args.B or 4096}-trajectory workload]"
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": 0,
+            "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": r["ms_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": full,
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------ GPU legs
+
+def run_gpu(args) -> None:
+    import torch
+    from paper_2309_09102_b200 import build as lm_build, lm
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the batched-LM path has no CPU fallback)")
+    if not os.path.exists(lm_build.LIB_PATH):
+        lm_build.build()
+    torch.cuda.set_device(local_rank)
+    device = torch.device("cuda", local_rank)
+    if world > 1:
+        dist_init("nccl")
+
+    from paper_2309_09102_b200 import workloads as wl
+    chain = wl.random_chain_8dof(3) if args.workload == "C3" else wl.panda_chain()
+    fk = lm.device_fk(chain, device=str(device))
+    w = make_workload(args.workload, fk, args.B, args.n, rank)
+    d = int(chain.dof)
+    prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol)
+    stream = torch.cuda.Stream(device=device)
+    solver = lm.Solver(chain, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, device=str(device), stream=stream)
+    if args.block:
+        solver.set_launch(args.block)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)  # > 126 MB L2
+
+    def one_step():
+        solver.reset()
+        solver.run(w.max_iters)
+
+    with torch.cuda.stream(stream):
+        for _ in range(max(args.warmup, 3)):
+            flush.zero_()
+            one_step()
+        stream.synchronize()
+        iters_per_step, conv_traj = solver.fetch_totals()
+
+        # ---- device-timed steps: CUDA events on the launching stream, L2 flushed between steps
+        sampler = ClockSampler(local_rank).start()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        dist_barrier()
+        torch.cuda.synchronize(device)
+        launches0 = lm.lm_launch_count()
+        wall0 = time.perf_counter()
+        for a, b in evs:
+            flush.zero_()
+            a.record(stream)
+            one_step()
+            b.record(stream)
+        torch.cuda.synchronize(device)
+        wall = time.perf_counter() - wall0
+        launches = lm.lm_launch_count() - launches0
+        dist_barrier()
+        clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = float(sum(step_ms))
+    units = float(iters_per_step) * args.steps
+    total_ms_all, units_all = dist_max_sum(total_ms, units, device)
+    value = units_all / (total_ms_all * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: lm_init (H2D) + lm_run + lm_fetch (D2H)
+    e2e = measure_e2e(lm, torch, chain, w, prm, device, max(1, min(args.steps, 5)))
+    e2e_ms_all, e2e_units_all = dist_max_sum(e2e["ms_total"], e2e["units"], device)
+    e2e_value = e2e_units_all / (e2e_ms_all * 1e-3)
+
+    if rank != 0:
+        return
+    peaks = load_peaks()
+    ms_kernel = total_ms / args.steps  # the step IS one launch of lm_iterate_kernel
+    flop = ALG_FLOP.get(d, 1459.0 * d / 7.0) * iters_per_step
+    peak_tf = SM_COUNT * FP32_LANES * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    achieved_tf = flop / (ms_kernel * 1e-3) / 1e12
+    hbm_bytes = alg_bytes_per_waypoint(d) * w.W
+    roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": achieved_tf / peak_tf, "traffic": None,
+                "kernel": f"lm_iterate_kernel<{d}>", "kernel_ms": ms_kernel,
+                "alg_flop_per_waypoint_iteration": ALG_FLOP.get(d),
+                "peak_how": f"derived: {SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz "
+                            f"(sm_max_mhz {peaks['_source']})",
+                "hbm": {"alg_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / (ms_kernel * 1e-3) / 1e9,
+                        "peak_gbs": peaks["hbm_gbs"], "frac": hbm_bytes / (ms_kernel * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                        "peak_source": peaks["_source"]}}
+    ref_traj = min(args.ref_traj or 256, w.B)
+    cpu = time_oracle(make_workload(args.workload, fk, ref_traj, w.n), ref_traj)
+    cfg = workload_desc(w)
+    cfg.update({"parallelism": f"dp{world} (independent batches, no collective)", "l2": "flushed between steps (256 MiB write)",
+                "block_threads": args.block or 128})
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms_all / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
+            "trajectories_per_sec": w.B * world * args.steps / (total_ms_all * 1e-3),
+            "converged_trajectories_per_step": conv_traj,
+            "waypoint_iterations_per_step": iters_per_step, "wall_s_timed_region": wall,
+            "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
+                    "ms_per_step": e2e_ms_all / e2e["steps"], "how": "lm_init(LM_MEM_HOST, pinned) + lm_run + lm_fetch(host q, |r|, iters, status)"},
+            "roofline": roofline,
+            "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}}
+    print(json.dumps(line))
+
+
+def measure_e2e(lm, torch, chain, w, prm, device, steps: int) -> dict:
+    """The call a user with host data makes: pinned host inputs -> lm_init (H2D copies inside) ->
+    lm_run -> lm_fetch into pinned host outputs (D2H inside), all inside the timed region."""
+    d, W = int(chain.dof), w.W
+    stream = torch.cuda.Stream(device=device)
+    soa = lambda x: torch.from_numpy(np.ascontiguousarray(np.asarray(x, np.float32).T)).pin_memory()
+    tp, tq, seeds = soa(w.target_pos), soa(w.target_quat), soa(w.seeds)
+    nbytes = lm.lm_workspace_bytes(d, w.B, w.n, 0, lm.LM_MEM_HOST)
+    ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+    ws_ptr = (ws.data_ptr() + 255) // 256 * 256
+    cchain, keep = lm.make_chain(chain)
+    q_out = torch.empty((d, W), dtype=torch.float32).pin_memory()
+    res = torch.empty(W, dtype=torch.float32).pin_memory()
+    its = torch.empty(W, dtype=torch.int32).pin_memory()
+    sts = torch.empty(W, dtype=torch.int32).pin_memory()
+    h2d = 4 * W * (d + 3 + 4)
+    d2h = 4 * W * (d + 3)
+    times, units = [], 0
+
+    def once():
+        pb = lm.LmProblem(w.B, w.n, tp.data_ptr(), tq.data_ptr(), 0, seeds.data_ptr(), lm.LM_MEM_HOST, ws_ptr, nbytes)
+        ctx = lm.lm_init(cchain, pb, prm, int(stream.cuda_stream))
+        lm.lm_run(ctx, w.max_iters)
+        st = lm.LmStats(res.data_ptr(), None, None, None, its.data_ptr(), None, sts.data_ptr(), None, None, 0, 0)
+        lm.lm_fetch(ctx, q_out.data_ptr(), st)  # synchronises the stream
+        lm.lm_free(ctx)
+        return int(st.total_waypoint_iters)
+
+    once()
+    once()
+    dist_barrier()
+    torch.cuda.synchronize(device)
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        units += once()
+        times.append(time.perf_counter() - t0)
+    dist_barrier()
+    return {"ms_total": 1e3 * float(sum(times)), "units": float(units), "steps": steps, "h2d": h2d, "d2h": d2h}
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="C4", choices=["C4", "C2", "C3", "C5"])
+    ap.add_argument("--B", type=int, default=None, help="trajectories (default: the config's)")
+    ap.add_argument("--n", type=int, default=None, help="waypoints per trajectory")
+    ap.add_argument("--block", type=int, default=0, help="threads per block override")
+    ap.add_argument("--ref-traj", type=int, default=0,
+                    help="trajectories in the oracle's timed sample (default 256 for cpu_baseline, 64 per step for --impl reference)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

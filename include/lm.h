@@ -1,0 +1,163 @@
+/*
+ * lm.h -- C ABI of the B200-native batched Levenberg-Marquardt pose refinement
+ *         (the trajectory optimiser's pose-error phase of CppFlow, arxiv 2309.09102, sec. III-C).
+ *
+ * Problem: given FK(q): R^d -> SE(3), a target path Y = [y_1..y_n], y_i in
+ * SE(3), and a seed trajectory xi = [q_1..q_n], q_i in R^d, refine xi so that FK(q_i) = y_i.
+ * The pose residual of waypoint i depends on q_i only, so the damped normal
+ * equations (J^T J + lambda I) delta = -J^T r are block diagonal with one d x d block per
+ * waypoint; this library solves B*n such blocks per LM iteration on one GPU, with the
+ * accept/reject decision and the lambda update taken per waypoint on the device.
+ *
+ * One LM iteration of one waypoint (readings R1-R11):
+ *   J = geometric Jacobian at q (world frame, flange point)
+ *   delta = -(J^T J + lambda I)^-1 J^T r   (fp32 Cholesky + refinement)
+ *   q+ = clamp(q + delta, q_lo, q_hi)
+ *   r+ = [w_pos (p(q+) - p_t) ; w_rot Log(R(q+) R_t^T)^vee],  F+ = |r+|^2 PAPER.md:L45-47, L115-117
+ *   if F+ < F: accept, lambda = max(lambda / nu_down, lambda_min)        (paper silent: DESIGN R5)
+ *   else     : reject, lambda = min(lambda * nu_up,  lambda_max)
+ * A waypoint is frozen once sqrt(F) < tol (DESIGN R7); tol = 0 never freezes.
+ *
+ * Conventions
+ *   - All functions return 0 (LM_OK) or a negative lm_status; nothing throws across the ABI.
+ *   - "device" pointers are CUDA device memory owned by the CALLER (e.g. torch tensors) and are
+ *     borrowed until lm_free(); they must be 16-byte aligned.  "host" pointers are plain host
+ *     memory read during the call only (pinned memory makes the copies asynchronous).
+ *   - Device arrays are structure-of-arrays over the waypoint index w = b*n + i (b = trajectory,
+ *     i = timestep):  x[k][w]  is stored at  x[k*W + w],  W = B*n.
+ *   - lm_step / lm_run / lm_fk only enqueue work on the stream given to lm_init; lm_fetch
+ *     synchronises that stream.  There is no CPU fallback: without a CUDA device every entry
+ *     point that needs one returns LM_ECUDA.
+ */
+#ifndef LM_B200_H
+#define LM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LM_MAX_DOF 8
+#define LM_MAX_ITERS 64 /* accept_mask is 64 bits wide */
+
+typedef enum {
+    LM_OK = 0,
+    LM_EINVAL = -1, /* null pointer, dof outside 1..8, B*n == 0, misaligned pointer, lo > hi, max_iters > 64 ... */
+    LM_ENOMEM = -2, /* workspace smaller than lm_workspace_bytes() */
+    LM_ECUDA = -3   /* a CUDA runtime call failed; lm_strerror() gives cudaGetErrorString */
+} lm_status;
+
+typedef struct lm_ctx lm_ctx; /* opaque, library-owned (host memory); lm_free() releases it */
+
+/* Serial kinematic chain, HOST memory, copied by lm_init.  Modified-DH (Craig) rows (DESIGN R1):
+ *   A_j = Rot_x(alpha_{j-1}) Trans_x(a_{j-1}) Rot_z(theta_j) Trans_z(d_j),
+ * revolute: theta_j = theta_off_j + q_j;  prismatic: d_j = d_off_j + q_j.  Base frame = world. */
+typedef struct {
+    int32_t dof;               /* d, 1..8 */
+    const uint8_t *joint_type; /* [d] 0 = revolute, 1 = prismatic */
+    const double *dh;          /* [d][4] a_{j-1} (m), alpha_{j-1} (rad), d_j (m), theta_off_j (rad) */
+    const double *q_lo, *q_hi; /* [d] joint limits (rad | m) */
+    double tool[7];            /* fixed flange transform after joint d: xyz (m) + unit quaternion w,x,y,z */
+} lm_chain;
+
+#define LM_MEM_DEVICE 0
+#define LM_MEM_HOST 1
+
+typedef struct {
+    int64_t B, n;             /* trajectories, waypoints per trajectory */
+    const float *target_pos;  /* [3][Wt] metres; Wt = B*n, or n if shared_targets */
+    const float *target_quat; /* [4][Wt] quaternion w,x,y,z (re-normalised on load, sign free: DESIGN R11) */
+    int32_t shared_targets;   /* 1: all B trajectories track the same path (K candidates of one Y) */
+    const float *seeds;       /* [d][B*n] seed joint values; should lie inside the joint limits */
+    int32_t memory;           /* LM_MEM_DEVICE: the three arrays above are device memory, borrowed until lm_free.
+                                 LM_MEM_HOST: host memory, copied into the workspace by lm_init (async on the stream
+                                 if pinned); the host arrays may be reused once the stream has passed the copies. */
+    void *workspace;          /* DEVICE scratch, caller-allocated, >= lm_workspace_bytes(), 256-byte aligned */
+    size_t workspace_bytes;
+} lm_problem;
+
+/* LM constants.  The paper gives none (DESIGN R5); lm_default_params() fills the documented defaults. */
+typedef struct {
+    float lambda0;        /* initial damping, 1e-3 (BASELINE.json configs[0]) */
+    float nu_up, nu_down; /* Marquardt factors, 10 and 10 */
+    float lambda_min;     /* 1e-4: below ~3e-5 the fp32 pivot of the self-motion direction is noise (DESIGN R5) */
+    float lambda_max;     /* 1e7 */
+    float tol;            /* freeze when sqrt(F) < tol; 0 = run a fixed number of iterations (DESIGN R7/R8) */
+    float w_pos, w_rot;   /* residual weights, 1 and 1 (DESIGN R2b) */
+    int32_t refine_steps; /* iterative-refinement steps on the fp32 Cholesky solve, 0..2 (default 1, DESIGN R4) */
+    int32_t fast_sincos;  /* 0 = accurate sincosf (default); 1 = MUFU __sincosf */
+} lm_params;
+
+/* lm_fetch outputs.  Every pointer is nullable; each may be DEVICE or HOST memory (detected). */
+typedef struct {
+    float *res_norm;           /* [W] sqrt(F) at the current q */
+    float *pos_err, *rot_err;  /* [W] |p - p_t| (m) and geodesic angle (rad), unweighted */
+    float *lambda;             /* [W] current lambda */
+    int32_t *iters;            /* [W] iterations executed (accepted + rejected) */
+    uint64_t *accept_mask;     /* [W] bit k = iteration k accepted */
+    uint32_t *status;          /* [W] LM_ST_* bits */
+    uint8_t *traj_converged;   /* [B] 1 iff every waypoint of the trajectory is frozen */
+    int32_t *traj_iters;       /* [B] max over the trajectory's waypoints of iters */
+    int64_t total_waypoint_iters; /* OUT: sum of iters over all waypoints -- numerator of the throughput metric */
+    int64_t converged_trajectories; /* OUT */
+} lm_stats;
+
+#define LM_ST_FROZEN 1u    /* sqrt(F) < tol */
+#define LM_ST_MAXITER 2u   /* stopped by the iteration limit, not frozen */
+#define LM_ST_BREAKDOWN 4u /* a Cholesky pivot <= 0 or a non-finite step was seen (treated as a rejected step) */
+#define LM_ST_NONFINITE 8u /* a non-finite trial cost was seen (rejected) */
+#define LM_ST_CLAMPED 16u  /* an accepted step was clamped to a joint limit */
+
+/* Device scratch needed for (dof, B, n); `memory` as in lm_problem (host inputs are staged in the workspace). */
+size_t lm_workspace_bytes(int32_t dof, int64_t B, int64_t n, int32_t shared_targets, int32_t memory);
+
+int lm_default_params(lm_params *out);
+
+/* Validate, copy the chain, bind buffers; state := seeds, lambda := lambda0, iters := 0.
+ * cuda_stream: a cudaStream_t (NULL = default stream).  Enqueues at most the host->device copies. */
+int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *problem, const lm_params *params,
+            void *cuda_stream);
+
+/* Exactly one LM iteration for every waypoint that is not frozen and has iters < 64.  Async. */
+int lm_step(lm_ctx *ctx);
+
+/* On-device loop: every waypoint iterates until frozen or until its iters == max_iters (<= 64,
+ * counted from lm_init / lm_reset / lm_set_state).  ONE kernel launch, no host round trip.  Async.
+ * lm_run(N) and N calls of lm_step give bit-identical results. */
+int lm_run(lm_ctx *ctx, int32_t max_iters);
+
+/* Synchronise the stream and copy out the current state.  q_out: [d][W] device or host, nullable. */
+int lm_fetch(lm_ctx *ctx, float *q_out, lm_stats *stats_out);
+
+/* Restart from the seeds given to lm_init (state := seeds, lambda := lambda0, iters := 0).  Host-only, no launch. */
+int lm_reset(lm_ctx *ctx);
+
+/* Inject a state: q [d][W] and lambda [W] (device or host, lambda nullable = lambda0); iters, mask, status := 0.
+ * Used for warm restarts and teacher-forced tests.  Async copies on the stream. */
+int lm_set_state(lm_ctx *ctx, const float *q, const float *lambda);
+
+/* Debug trace (device pointers, nullable, borrowed): every executed iteration overwrites
+ * trial_q [d][W] = q+ and trial_F [2][W] = (F before, F+ of the trial). */
+int lm_set_trace(lm_ctx *ctx, float *trial_q, float *trial_F);
+
+/* Launch geometry override for tuning and bit-stability tests: threads per block (multiple of 32, <= 256; 0 = default). */
+int lm_set_launch(lm_ctx *ctx, int32_t block_threads);
+
+/* Forward kinematics on the device with the context's chain (S1 of the hot path):
+ * q [d][count] -> pos [3][count], rot [9][count] (row-major R, SoA).  Device pointers.  Async. */
+int lm_fk(lm_ctx *ctx, const float *q, int64_t count, float *pos, float *rot);
+
+void lm_free(lm_ctx *ctx);
+
+/* Static string for a status code; for LM_ECUDA the last CUDA error string seen by this thread. */
+const char *lm_strerror(int code);
+
+/* Kernels launched by this library in this process so far (bench.py's gpu_launches). */
+int64_t lm_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LM_B200_H */

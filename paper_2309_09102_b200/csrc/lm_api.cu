@@ -1,0 +1,408 @@
+// lm_api.cu -- C ABI of include/lm.h: validation, workspace carving, launches.  No torch types,
+// no CPU compute path: every step of the hot path runs in the kernels of lm_kernels.cuh.
+#include "../../include/lm.h"
+#include "lm_kernels.cuh"
+
+#include <atomic>
+#include <climits>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace lmk;
+
+namespace {
+
+thread_local char g_cuda_err[256] = "no CUDA error recorded";
+std::atomic<long long> g_launches{0};
+
+int cuda_fail(cudaError_t e) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    return LM_ECUDA;
+}
+#define LM_CUDA(x)                                 \
+    do {                                           \
+        cudaError_t e_ = (x);                      \
+        if (e_ != cudaSuccess) return cuda_fail(e_); \
+    } while (0)
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+struct Layout { // byte offsets into the workspace
+    size_t q, lam, res, perr, rerr, its, mask, ui, us, conv, titers, totals, s_seeds, s_tp, s_tq, total;
+};
+
+Layout make_layout(int dof, int64_t B, int64_t n, int shared, int memory) {
+    const size_t W = (size_t)B * (size_t)n, Wt = shared ? (size_t)n : W;
+    Layout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+    L.q = take(4 * W * dof);
+    L.lam = take(4 * W);
+    L.res = take(4 * W);
+    L.perr = take(4 * W);
+    L.rerr = take(4 * W);
+    L.its = take(4 * W);
+    L.mask = take(8 * W);
+    L.ui = take(4 * W); // unpacked iters / status for host destinations of lm_fetch
+    L.us = take(4 * W);
+    L.conv = take((size_t)B);
+    L.titers = take(4 * (size_t)B);
+    L.totals = take(16);
+    if (memory == LM_MEM_HOST) {
+        L.s_seeds = take(4 * W * dof);
+        L.s_tp = take(4 * Wt * 3);
+        L.s_tq = take(4 * Wt * 4);
+    }
+    L.total = off;
+    return L;
+}
+
+float round_inward(double x, bool lower) { // fp32 value inside [lo, hi] of the fp64 limits
+    float f = (float)x;
+    if (lower && (double)f < x) f = nextafterf(f, INFINITY);
+    if (!lower && (double)f > x) f = nextafterf(f, -INFINITY);
+    return f;
+}
+
+} // namespace
+
+struct lm_ctx {
+    int dof;
+    int64_t B, n, W;
+    int shared;
+    KArgs args; // template for every launch
+    Layout lay;
+    char *ws;
+    cudaStream_t stream;
+    bool fresh;
+    int block;
+    bool fast;
+};
+
+extern "C" {
+
+size_t lm_workspace_bytes(int32_t dof, int64_t B, int64_t n, int32_t shared_targets, int32_t memory) {
+    if (dof < 1 || dof > LM_MAX_DOF || B <= 0 || n <= 0) return 0;
+    return make_layout(dof, B, n, shared_targets, memory).total;
+}
+
+int lm_default_params(lm_params *out) {
+    if (!out) return LM_EINVAL;
+    out->lambda0 = 1e-3f;
+    out->nu_up = 10.f;
+    out->nu_down = 10.f;
+    out->lambda_min = 1e-4f;
+    out->lambda_max = 1e7f;
+    out->tol = 0.f;
+    out->w_pos = 1.f;
+    out->w_rot = 1.f;
+    out->refine_steps = 1;
+    out->fast_sincos = 0;
+    return LM_OK;
+}
+
+int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_params *prm, void *cuda_stream) {
+    if (!out) return LM_EINVAL;
+    *out = nullptr;
+    if (!chain || !pb || !prm) return LM_EINVAL;
+    const int d = chain->dof;
+    if (d < 1 || d > LM_MAX_DOF) return LM_EINVAL;
+    if (!chain->joint_type || !chain->dh || !chain->q_lo || !chain->q_hi) return LM_EINVAL;
+    if (pb->B <= 0 || pb->n <= 0 || pb->n > INT32_MAX) return LM_EINVAL;
+    if (!pb->target_pos || !pb->target_quat || !pb->seeds || !pb->workspace) return LM_EINVAL;
+    if (pb->memory != LM_MEM_DEVICE && pb->memory != LM_MEM_HOST) return LM_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(pb->workspace) & 255u) != 0) return LM_EINVAL;
+    if (pb->memory == LM_MEM_DEVICE && !(aligned16(pb->target_pos) && aligned16(pb->target_quat) && aligned16(pb->seeds)))
+        return LM_EINVAL;
+    if (!(prm->lambda0 > 0.f) || !(prm->nu_up > 1.f) || !(prm->nu_down > 1.f) || !(prm->lambda_min > 0.f) ||
+        !(prm->lambda_max >= prm->lambda_min) || !(prm->tol >= 0.f) || !(prm->w_pos > 0.f) || !(prm->w_rot > 0.f) ||
+        prm->refine_steps < 0 || prm->refine_steps > 2)
+        return LM_EINVAL;
+    for (int j = 0; j < d; ++j) {
+        if (!(chain->q_lo[j] <= chain->q_hi[j])) return LM_EINVAL;
+        if (chain->joint_type[j] > 1) return LM_EINVAL;
+    }
+    const double *tq = chain->tool + 3;
+    const double tn = std::sqrt(tq[0] * tq[0] + tq[1] * tq[1] + tq[2] * tq[2] + tq[3] * tq[3]);
+    if (!(tn > 0.0)) return LM_EINVAL;
+
+    const Layout lay = make_layout(d, pb->B, pb->n, pb->shared_targets, pb->memory);
+    if (pb->workspace_bytes < lay.total) return LM_ENOMEM;
+
+    lm_ctx *c = new (std::nothrow) lm_ctx();
+    if (!c) return LM_ENOMEM;
+    c->dof = d; c->B = pb->B; c->n = pb->n; c->W = pb->B * pb->n; c->shared = pb->shared_targets ? 1 : 0;
+    c->lay = lay; c->ws = static_cast<char *>(pb->workspace);
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->fresh = true; c->block = 128; c->fast = prm->fast_sincos != 0;
+
+    KArgs &a = c->args;
+    std::memset(&a, 0, sizeof(a));
+    KChain &k = a.ch;
+    for (int j = 0; j < d; ++j) {
+        const double aj = chain->dh[4 * j + 0], al = chain->dh[4 * j + 1], dj = chain->dh[4 * j + 2], th = chain->dh[4 * j + 3];
+        // exact 0 / +-1 for the quarter-turn twists every standard DH table uses
+        double ca = std::cos(al), sa = std::sin(al);
+        if (std::fabs(ca) < 1e-15) ca = 0.0;
+        if (std::fabs(sa) < 1e-15) sa = 0.0;
+        k.ca[j] = (float)ca; k.sa[j] = (float)sa; k.a[j] = (float)aj; k.d[j] = (float)dj;
+        k.toff[j] = (float)th; k.cth[j] = (float)std::cos(th); k.sth[j] = (float)std::sin(th);
+        k.lo[j] = round_inward(chain->q_lo[j], true);
+        k.hi[j] = round_inward(chain->q_hi[j], false);
+        if (k.lo[j] > k.hi[j]) k.lo[j] = k.hi[j] = (float)chain->q_lo[j];
+        if (chain->joint_type[j]) k.prismatic_mask |= 1u << j;
+    }
+    {
+        const double w = tq[0] / tn, x = tq[1] / tn, y = tq[2] / tn, z = tq[3] / tn;
+        const double R[9] = {1 - 2 * (y * y + z * z), 2 * (x * y - w * z), 2 * (x * z + w * y),
+                             2 * (x * y + w * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w * x),
+                             2 * (x * z - w * y), 2 * (y * z + w * x), 1 - 2 * (x * x + y * y)};
+        bool ident = true;
+        for (int i = 0; i < 9; ++i) {
+            k.tool_R[i] = (float)R[i];
+            if (std::fabs(R[i] - ((i % 4 == 0) ? 1.0 : 0.0)) > 0.0) ident = false;
+        }
+        k.tool_has_rot = ident ? 0u : 1u;
+        for (int i = 0; i < 3; ++i) k.tool_p[i] = (float)chain->tool[i];
+    }
+    a.lambda0 = prm->lambda0; a.nu_up = prm->nu_up; a.inv_nu_down = (float)(1.0 / (double)prm->nu_down);
+    a.lambda_min = prm->lambda_min; a.lambda_max = prm->lambda_max; a.tol2 = prm->tol * prm->tol;
+    a.w_pos = prm->w_pos; a.w_rot = prm->w_rot;
+    a.inv_w_pos = (float)(1.0 / (double)prm->w_pos); a.inv_w_rot = (float)(1.0 / (double)prm->w_rot);
+    a.weighted = (prm->w_pos != 1.f || prm->w_rot != 1.f) ? 1 : 0;
+    a.refine = prm->refine_steps;
+    a.W = c->W; a.n = (int32_t)c->n; a.shared_targets = c->shared;
+    a.q = reinterpret_cast<float *>(c->ws + lay.q);
+    a.lam = reinterpret_cast<float *>(c->ws + lay.lam);
+    a.res = reinterpret_cast<float *>(c->ws + lay.res);
+    a.perr = reinterpret_cast<float *>(c->ws + lay.perr);
+    a.rerr = reinterpret_cast<float *>(c->ws + lay.rerr);
+    a.its = reinterpret_cast<uint32_t *>(c->ws + lay.its);
+    a.mask = reinterpret_cast<unsigned long long *>(c->ws + lay.mask);
+
+    if (pb->memory == LM_MEM_HOST) {
+        const size_t W = (size_t)c->W, Wt = c->shared ? (size_t)c->n : W;
+        float *s = reinterpret_cast<float *>(c->ws + lay.s_seeds);
+        float *tp = reinterpret_cast<float *>(c->ws + lay.s_tp);
+        float *tqd = reinterpret_cast<float *>(c->ws + lay.s_tq);
+        cudaError_t e = cudaMemcpyAsync(s, pb->seeds, 4 * W * d, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(tp, pb->target_pos, 4 * Wt * 3, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(tqd, pb->target_quat, 4 * Wt * 4, cudaMemcpyHostToDevice, c->stream);
+        if (e != cudaSuccess) { delete c; return cuda_fail(e); }
+        a.seeds = s; a.tp = tp; a.tq = tqd;
+    } else {
+        a.seeds = pb->seeds; a.tp = pb->target_pos; a.tq = pb->target_quat;
+    }
+    *out = c;
+    return LM_OK;
+}
+
+} // extern "C"
+
+namespace {
+
+template <int D>
+cudaError_t launch_iterate_d(lm_ctx *c, const KArgs &a) {
+    const unsigned grid = (unsigned)((c->W + c->block - 1) / c->block);
+    if (c->fast) lm_iterate_kernel<D, true><<<grid, c->block, 0, c->stream>>>(a);
+    else lm_iterate_kernel<D, false><<<grid, c->block, 0, c->stream>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_iterate(lm_ctx *c, const KArgs &a) {
+    g_launches.fetch_add(1);
+    switch (c->dof) {
+    case 1: return launch_iterate_d<1>(c, a);
+    case 2: return launch_iterate_d<2>(c, a);
+    case 3: return launch_iterate_d<3>(c, a);
+    case 4: return launch_iterate_d<4>(c, a);
+    case 5: return launch_iterate_d<5>(c, a);
+    case 6: return launch_iterate_d<6>(c, a);
+    case 7: return launch_iterate_d<7>(c, a);
+    default: return launch_iterate_d<8>(c, a);
+    }
+}
+
+template <int D>
+cudaError_t launch_fk_d(lm_ctx *c, const KFkArgs &a) {
+    const unsigned grid = (unsigned)((a.count + 127) / 128);
+    if (c->fast) lm_fk_kernel<D, true><<<grid, 128, 0, c->stream>>>(a);
+    else lm_fk_kernel<D, false><<<grid, 128, 0, c->stream>>>(a);
+    return cudaGetLastError();
+}
+
+int iterate(lm_ctx *c, int max_total, int at_most) {
+    KArgs a = c->args;
+    a.fresh = c->fresh ? 1 : 0;
+    a.max_total = max_total;
+    a.at_most = at_most;
+    cudaError_t e = launch_iterate(c, a);
+    if (e != cudaSuccess) return cuda_fail(e);
+    c->fresh = false;
+    return LM_OK;
+}
+
+// copy `bytes` from a device workspace array to a device-or-host destination (UVA decides)
+cudaError_t copy_out(void *dst, const void *src, size_t bytes, cudaStream_t s) {
+    if (!dst) return cudaSuccess;
+    return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, s);
+}
+
+__global__ void lm_unpack_kernel(const uint32_t *__restrict__ its, int64_t W, int32_t *__restrict__ iters,
+                                 uint32_t *__restrict__ status) {
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= W) return;
+    const uint32_t pk = its[w];
+    if (iters) iters[w] = (int32_t)(pk & 0xffu);
+    if (status) status[w] = pk >> 8;
+}
+
+__global__ void lm_fill_state_kernel(float *__restrict__ lam, uint32_t *__restrict__ its,
+                                     unsigned long long *__restrict__ mask, int64_t W, float lambda0, int set_lam) {
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= W) return;
+    if (set_lam) lam[w] = lambda0;
+    its[w] = 0u;
+    mask[w] = 0ull;
+}
+
+} // namespace
+
+extern "C" {
+
+int lm_step(lm_ctx *c) {
+    if (!c) return LM_EINVAL;
+    return iterate(c, LM_MAX_ITERS, 1);
+}
+
+int lm_run(lm_ctx *c, int32_t max_iters) {
+    if (!c || max_iters < 0 || max_iters > LM_MAX_ITERS) return LM_EINVAL;
+    return iterate(c, max_iters, INT_MAX);
+}
+
+int lm_reset(lm_ctx *c) {
+    if (!c) return LM_EINVAL;
+    c->fresh = true;
+    return LM_OK;
+}
+
+int lm_set_trace(lm_ctx *c, float *trial_q, float *trial_F) {
+    if (!c || ((trial_q == nullptr) != (trial_F == nullptr))) return LM_EINVAL;
+    c->args.trace_q = trial_q;
+    c->args.trace_F = trial_F;
+    return LM_OK;
+}
+
+int lm_set_launch(lm_ctx *c, int32_t block_threads) {
+    if (!c) return LM_EINVAL;
+    if (block_threads == 0) block_threads = 128;
+    if (block_threads < 32 || block_threads > 256 || (block_threads % 32) != 0) return LM_EINVAL;
+    c->block = block_threads;
+    return LM_OK;
+}
+
+int lm_set_state(lm_ctx *c, const float *q, const float *lambda) {
+    if (!c || !q) return LM_EINVAL;
+    const size_t W = (size_t)c->W;
+    LM_CUDA(cudaMemcpyAsync(c->args.q, q, 4 * W * c->dof, cudaMemcpyDefault, c->stream));
+    if (lambda) LM_CUDA(cudaMemcpyAsync(c->args.lam, lambda, 4 * W, cudaMemcpyDefault, c->stream));
+    const unsigned grid = (unsigned)((W + 255) / 256);
+    g_launches.fetch_add(1);
+    lm_fill_state_kernel<<<grid, 256, 0, c->stream>>>(c->args.lam, c->args.its, c->args.mask, c->W,
+                                                      c->args.lambda0, lambda ? 0 : 1);
+    LM_CUDA(cudaGetLastError());
+    c->fresh = false;
+    return LM_OK;
+}
+
+int lm_fk(lm_ctx *c, const float *q, int64_t count, float *pos, float *rot) {
+    if (!c || !q || !pos || !rot || count <= 0) return LM_EINVAL;
+    if (!(aligned16(q) && aligned16(pos) && aligned16(rot))) return LM_EINVAL;
+    KFkArgs a;
+    a.ch = c->args.ch; a.count = count; a.q = q; a.pos = pos; a.rot = rot;
+    g_launches.fetch_add(1);
+    cudaError_t e;
+    switch (c->dof) {
+    case 1: e = launch_fk_d<1>(c, a); break;
+    case 2: e = launch_fk_d<2>(c, a); break;
+    case 3: e = launch_fk_d<3>(c, a); break;
+    case 4: e = launch_fk_d<4>(c, a); break;
+    case 5: e = launch_fk_d<5>(c, a); break;
+    case 6: e = launch_fk_d<6>(c, a); break;
+    case 7: e = launch_fk_d<7>(c, a); break;
+    default: e = launch_fk_d<8>(c, a); break;
+    }
+    if (e != cudaSuccess) return cuda_fail(e);
+    return LM_OK;
+}
+
+int lm_fetch(lm_ctx *c, float *q_out, lm_stats *s) {
+    if (!c) return LM_EINVAL;
+    const size_t W = (size_t)c->W;
+    const KArgs &a = c->args;
+    if (c->fresh) { // nothing has run yet: materialise the initial state so that fetch is well defined
+        int rc = iterate(c, 0, 0);
+        if (rc != LM_OK) return rc;
+    }
+    LM_CUDA(copy_out(q_out, a.q, 4 * W * c->dof, c->stream));
+    if (s) {
+        LM_CUDA(copy_out(s->res_norm, a.res, 4 * W, c->stream));
+        LM_CUDA(copy_out(s->pos_err, a.perr, 4 * W, c->stream));
+        LM_CUDA(copy_out(s->rot_err, a.rerr, 4 * W, c->stream));
+        LM_CUDA(copy_out(s->lambda, a.lam, 4 * W, c->stream));
+        LM_CUDA(copy_out(s->accept_mask, a.mask, 8 * W, c->stream));
+        uint8_t *conv = reinterpret_cast<uint8_t *>(c->ws + c->lay.conv);
+        int32_t *tit = reinterpret_cast<int32_t *>(c->ws + c->lay.titers);
+        unsigned long long *tot = reinterpret_cast<unsigned long long *>(c->ws + c->lay.totals);
+        LM_CUDA(cudaMemsetAsync(tot, 0, 16, c->stream));
+        const int64_t threads = c->B * 32;
+        g_launches.fetch_add(1);
+        lm_traj_stats_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, c->stream>>>(a.its, c->B, (int32_t)c->n, conv, tit, tot);
+        LM_CUDA(cudaGetLastError());
+        LM_CUDA(copy_out(s->traj_converged, conv, (size_t)c->B, c->stream));
+        LM_CUDA(copy_out(s->traj_iters, tit, 4 * (size_t)c->B, c->stream));
+        if (s->iters || s->status) {
+            // unpack iters | status << 8 into the caller's arrays; host destinations go through scratch
+            cudaPointerAttributes pa;
+            int32_t *di = s->iters;
+            uint32_t *ds = s->status;
+            bool host_i = false, host_s = false;
+            if (di) { LM_CUDA(cudaPointerGetAttributes(&pa, di)); host_i = (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged); }
+            if (ds) { LM_CUDA(cudaPointerGetAttributes(&pa, ds)); host_s = (pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged); }
+            int32_t *ki = di ? (host_i ? reinterpret_cast<int32_t *>(c->ws + c->lay.ui) : di) : nullptr;
+            uint32_t *ks = ds ? (host_s ? reinterpret_cast<uint32_t *>(c->ws + c->lay.us) : ds) : nullptr;
+            g_launches.fetch_add(1);
+            lm_unpack_kernel<<<(unsigned)((W + 255) / 256), 256, 0, c->stream>>>(a.its, c->W, ki, ks);
+            LM_CUDA(cudaGetLastError());
+            if (host_i) LM_CUDA(cudaMemcpyAsync(di, ki, 4 * W, cudaMemcpyDeviceToHost, c->stream));
+            if (host_s) LM_CUDA(cudaMemcpyAsync(ds, ks, 4 * W, cudaMemcpyDeviceToHost, c->stream));
+        }
+        unsigned long long h[2] = {0, 0};
+        LM_CUDA(cudaMemcpyAsync(h, tot, 16, cudaMemcpyDeviceToHost, c->stream));
+        LM_CUDA(cudaStreamSynchronize(c->stream));
+        s->total_waypoint_iters = (int64_t)h[0];
+        s->converged_trajectories = (int64_t)h[1];
+        return LM_OK;
+    }
+    LM_CUDA(cudaStreamSynchronize(c->stream));
+    return LM_OK;
+}
+
+void lm_free(lm_ctx *c) { delete c; }
+
+const char *lm_strerror(int code) {
+    switch (code) {
+    case LM_OK: return "ok";
+    case LM_EINVAL: return "invalid argument";
+    case LM_ENOMEM: return "workspace too small or out of host memory";
+    case LM_ECUDA: return g_cuda_err;
+    default: return "unknown lm_status";
+    }
+}
+
+int64_t lm_launch_count(void) { return g_launches.load(); }
+
+} // extern "C"

@@ -1,0 +1,325 @@
+// lm_device.cuh -- per-waypoint device arithmetic of the batched LM pose refinement (sm_100a).
+//
+// One THREAD owns one waypoint block: its d x d damped normal equations are independent of every
+// other waypoint (block-diagonal Jacobian), so all state lives in registers and all
+// loops over joints are unrolled at compile time (template parameter D).  Every floating-point
+// operation is written as an explicit round-to-nearest intrinsic (fmaf / __fmul_rn / __fadd_rn):
+// the compiler may neither contract nor reassociate them, so a waypoint's bits do not depend on
+// which kernel, launch geometry or batch it is evaluated in (bit-stability).
+//
+// Step names S1..S9 follow DESIGN.md section 2.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lmk {
+
+constexpr int MAX_DOF = 8;
+
+// Chain constants, fp32, passed by value inside the kernel parameter block (constant bank:
+// operands are read as c[0][..] without occupying registers).
+struct KChain {
+    float ca[MAX_DOF], sa[MAX_DOF];   // cos / sin alpha_{j-1}
+    float a[MAX_DOF], d[MAX_DOF];     // a_{j-1}, d_j offset
+    float toff[MAX_DOF];              // theta offset (revolute)
+    float cth[MAX_DOF], sth[MAX_DOF]; // cos / sin of the fixed theta (prismatic)
+    float lo[MAX_DOF], hi[MAX_DOF];   // joint limits, rounded inward to fp32
+    float tool_p[3];
+    float tool_R[9];                  // row-major
+    uint32_t prismatic_mask;          // bit j: joint j prismatic
+    uint32_t tool_has_rot;            // tool rotation != identity
+};
+
+__device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+
+// sin and cos of x for |x| < ~1e4 (joint angles are bounded by the joint limits).
+// Cody-Waite reduction by pi/2 in three parts, then the classic single-precision minimax
+// polynomials on [-pi/4, pi/4]; max error ~1 ulp.  FAST: the MUFU approximations (abs err ~5e-7).
+template <bool FAST>
+__device__ __forceinline__ void sincos_(float x, float &s, float &c) {
+    if (FAST) {
+        __sincosf(x, &s, &c);
+        return;
+    }
+    const float magic = 12582912.0f;                     // 1.5 * 2^23: rounds to nearest integer
+    float t = fma_(x, 0.636619772f, magic);              // x * 2/pi
+    int qd = __float_as_int(t);                          // quadrant in the low mantissa bits
+    float j = sub(t, magic);
+    float r = fma_(j, -1.57079601e+00f, x);
+    r = fma_(j, -3.13916473e-07f, r);
+    r = fma_(j, -5.39030253e-15f, r);
+    float r2 = mul(r, r);
+    float ps = fma_(r2, -1.9515295891e-4f, 8.3321608736e-3f);
+    ps = fma_(ps, r2, -1.6666654611e-1f);
+    float sn = fma_(mul(r, r2), ps, r);
+    float pc = fma_(r2, 2.443315711809948e-5f, -1.388731625493765e-3f);
+    pc = fma_(pc, r2, 4.166664568298827e-2f);
+    pc = fma_(pc, r2, -0.5f);
+    float cs = fma_(pc, r2, 1.0f);
+    float s0 = (qd & 1) ? cs : sn;
+    float c0 = (qd & 1) ? sn : cs;
+    s = __int_as_float(__float_as_int(s0) ^ ((qd & 2) << 30));
+    c = __int_as_float(__float_as_int(c0) ^ (((qd + 1) & 2) << 30));
+}
+
+// theta = atan2(s, c) for s >= 0, theta in [0, pi].  Odd polynomial on [0, 1] (rel. err 1e-7,
+// coefficients: csrc/gen_atan_coeffs.py) + the usual octant reflections.
+__device__ __forceinline__ float atan2_pos(float s, float c) {
+    float ac = fabsf(c);
+    float mx = fmaxf(s, ac), mn = fminf(s, ac);
+    float t = __fdiv_rn(mn, fmaxf(mx, 1e-37f));
+    float t2 = mul(t, t);
+    float p = fma_(t2, 2.622244181e-03f, -1.513253432e-02f);
+    p = fma_(p, t2, 4.112185538e-02f);
+    p = fma_(p, t2, -7.366705686e-02f);
+    p = fma_(p, t2, 1.057393178e-01f);
+    p = fma_(p, t2, -1.418597549e-01f);
+    p = fma_(p, t2, 1.999039650e-01f);
+    p = fma_(p, t2, -3.333298564e-01f);
+    float at = fma_(mul(p, t2), t, t);
+    float th = (s > ac) ? sub(1.57079632679f, at) : at;
+    return (c < 0.0f) ? sub(3.14159265359f, th) : th;
+}
+
+// Pose of one waypoint: everything the LM iteration needs from FK.
+template <int D>
+struct Pose {
+    float Jv[D][3]; // linear part of Jacobian column j   (S3)
+    float Jw[D][3]; // angular part = joint axis z_j (0 for prismatic)
+    float r[6];     // residual (S2)
+    float F;        // r . r
+};
+
+// S1 + S2 + S3: serial-chain FK (modified DH, DESIGN R1), pose residual against the target
+// (p_t, R_t given as COLUMNS Rt[k] = k-th column), geometric Jacobian from the retained joint axes.
+//   A_j = Rot_x(alpha) Trans_x(a) Rot_z(theta) Trans_z(d);  frame columns X, Y, Z and origin o.
+template <int D, bool FAST>
+__device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D], const float (&pt)[3],
+                                          const float (&Rt)[3][3], float w_pos, float w_rot,
+                                          bool weighted, Pose<D> &P, float *p_out, float (*R_out)[3]) {
+    float X[3] = {1.f, 0.f, 0.f}, Y[3] = {0.f, 1.f, 0.f}, Z[3] = {0.f, 0.f, 1.f}, o[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        const bool pris = (ch.prismatic_mask >> j) & 1u; // warp-uniform (constant bank)
+        float s, c, dj;
+        if (!pris) {
+            sincos_<FAST>(add(q[j], ch.toff[j]), s, c);
+            dj = ch.d[j];
+        } else {
+            s = ch.sth[j];
+            c = ch.cth[j];
+            dj = add(ch.d[j], q[j]);
+        }
+        const float ca = ch.ca[j], sa = ch.sa[j], aj = ch.a[j];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            float y1 = fma_(sa, Z[i], mul(ca, Y[i]));   // Rot_x: Y' =  ca Y + sa Z
+            float z1 = fma_(ca, Z[i], mul(-sa, Y[i]));  //        Z' = -sa Y + ca Z
+            float o1 = fma_(aj, X[i], o[i]);            // Trans_x(a)
+            float x2 = fma_(s, y1, mul(c, X[i]));       // Rot_z: X'' =  c X + s Y'
+            float y2 = fma_(c, y1, mul(-s, X[i]));      //        Y'' = -s X + c Y'
+            o[i] = fma_(dj, z1, o1);                    // Trans_z(d)
+            X[i] = x2; Y[i] = y2; Z[i] = z1;
+            P.Jw[j][i] = z1;                            // joint axis z_j
+            P.Jv[j][i] = o[i];                          // frame origin o_j (turned into J_v below)
+        }
+    }
+    // flange: p = o + R tool_p ;  R_ee = R R_tool
+    float p[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+        p[i] = fma_(Z[i], ch.tool_p[2], fma_(Y[i], ch.tool_p[1], fma_(X[i], ch.tool_p[0], o[i])));
+    if (ch.tool_has_rot) { // warp-uniform
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            float x = X[i], y = Y[i], z = Z[i];
+            X[i] = fma_(z, ch.tool_R[6], fma_(y, ch.tool_R[3], mul(x, ch.tool_R[0])));
+            Y[i] = fma_(z, ch.tool_R[7], fma_(y, ch.tool_R[4], mul(x, ch.tool_R[1])));
+            Z[i] = fma_(z, ch.tool_R[8], fma_(y, ch.tool_R[5], mul(x, ch.tool_R[2])));
+        }
+    }
+    if (p_out) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            p_out[i] = p[i];
+            R_out[i][0] = X[i]; R_out[i][1] = Y[i]; R_out[i][2] = Z[i];
+        }
+    }
+
+    // S2: E = R_ee R_t^T = sum_k a_k b_k^T (a_k, b_k = k-th columns);
+    //     vee(antisym E) = 1/2 sum_k b_k x a_k,  tr E = sum_k a_k . b_k          (DESIGN R2)
+    float v[3], tr;
+    {
+        const float *A0 = X, *A1 = Y, *A2 = Z;
+        const float *B0 = Rt[0], *B1 = Rt[1], *B2 = Rt[2];
+#define LM_CROSS_ACC(i, i1, i2)                                                                       \
+    v[i] = fma_(B2[i1], A2[i2], fma_(-B2[i2], A2[i1],                                                 \
+           fma_(B1[i1], A1[i2], fma_(-B1[i2], A1[i1], fma_(B0[i1], A0[i2], mul(-B0[i2], A0[i1]))))));
+        LM_CROSS_ACC(0, 1, 2)
+        LM_CROSS_ACC(1, 2, 0)
+        LM_CROSS_ACC(2, 0, 1)
+#undef LM_CROSS_ACC
+        tr = fma_(A2[2], B2[2], fma_(A2[1], B2[1], fma_(A2[0], B2[0],
+             fma_(A1[2], B1[2], fma_(A1[1], B1[1], fma_(A1[0], B1[0],
+             fma_(A0[2], B0[2], fma_(A0[1], B0[1], mul(A0[0], B0[0])))))))));
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) v[i] = mul(0.5f, v[i]);
+    const float cth = fma_(0.5f, tr, -0.5f);
+    const float s2 = fma_(v[2], v[2], fma_(v[1], v[1], mul(v[0], v[0])));
+    const float sn = __fsqrt_rn(s2);
+    float scale;
+    if (sn < 1e-4f && cth > 0.f) {
+        scale = fma_(s2, 0.166666667f, 1.0f);          // theta/s = 1 + s^2/6
+    } else {
+        scale = __fdiv_rn(atan2_pos(sn, cth), fmaxf(sn, 1e-37f));
+    }
+    float w[3] = {mul(scale, v[0]), mul(scale, v[1]), mul(scale, v[2])};
+    if (sn < 1e-4f && cth <= 0.f) {
+        // theta within 1e-4 of pi (never reached by the documented workloads): axis from the
+        // symmetric part E_ii = c + (1 - c) a_i^2, signs from E_mi + E_im and from v.
+        float E[3][3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int k = 0; k < 3; ++k)
+                E[i][k] = fma_(Z[i], Rt[2][k], fma_(Y[i], Rt[1][k], mul(X[i], Rt[0][k])));
+        const float inv = __fdiv_rn(1.0f, sub(1.0f, cth));
+        float ax[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) ax[i] = __fsqrt_rn(fmaxf(mul(sub(E[i][i], cth), inv), 0.f));
+        int m = 0;
+        if (ax[1] > ax[m]) m = 1;
+        if (ax[2] > ax[m]) m = 2;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            float sym = (m == 0) ? add(E[0][i], E[i][0]) : (m == 1) ? add(E[1][i], E[i][1]) : add(E[2][i], E[i][2]);
+            if (i != m && sym < 0.f) ax[i] = -ax[i];
+        }
+        const float dt = fma_(ax[2], v[2], fma_(ax[1], v[1], mul(ax[0], v[0])));
+        const float th = (dt < 0.f) ? -atan2_pos(sn, cth) : atan2_pos(sn, cth);
+#pragma unroll
+        for (int i = 0; i < 3; ++i) w[i] = mul(th, ax[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        float rp = sub(p[i], pt[i]);
+        P.r[i] = weighted ? mul(w_pos, rp) : rp;
+        P.r[3 + i] = weighted ? mul(w_rot, w[i]) : w[i];
+    }
+    P.F = fma_(P.r[5], P.r[5], fma_(P.r[4], P.r[4], fma_(P.r[3], P.r[3],
+          fma_(P.r[2], P.r[2], fma_(P.r[1], P.r[1], mul(P.r[0], P.r[0]))))));
+
+    // S3: geometric Jacobian (DESIGN R3): revolute [z x (p - o); z], prismatic [z; 0]
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        const bool pris = (ch.prismatic_mask >> j) & 1u;
+        if (!pris) {
+            float e0 = sub(p[0], P.Jv[j][0]), e1 = sub(p[1], P.Jv[j][1]), e2 = sub(p[2], P.Jv[j][2]);
+            float z0 = P.Jw[j][0], z1 = P.Jw[j][1], z2 = P.Jw[j][2];
+            P.Jv[j][0] = fma_(z1, e2, mul(-z2, e1));
+            P.Jv[j][1] = fma_(z2, e0, mul(-z0, e2));
+            P.Jv[j][2] = fma_(z0, e1, mul(-z1, e0));
+        } else {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { P.Jv[j][i] = P.Jw[j][i]; P.Jw[j][i] = 0.f; }
+        }
+        if (weighted) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { P.Jv[j][i] = mul(w_pos, P.Jv[j][i]); P.Jw[j][i] = mul(w_rot, P.Jw[j][i]); }
+        }
+    }
+}
+
+// 6-term dot products of Jacobian columns (rows 0..2 linear, 3..5 angular)
+template <int D>
+__device__ __forceinline__ float coldot(const Pose<D> &P, int i, int j) {
+    return fma_(P.Jw[i][2], P.Jw[j][2], fma_(P.Jw[i][1], P.Jw[j][1], fma_(P.Jw[i][0], P.Jw[j][0],
+           fma_(P.Jv[i][2], P.Jv[j][2], fma_(P.Jv[i][1], P.Jv[j][1], mul(P.Jv[i][0], P.Jv[j][0]))))));
+}
+template <int D>
+__device__ __forceinline__ float colvec(const Pose<D> &P, int i, const float (&t)[6]) {
+    return fma_(P.Jw[i][2], t[5], fma_(P.Jw[i][1], t[4], fma_(P.Jw[i][0], t[3],
+           fma_(P.Jv[i][2], t[2], fma_(P.Jv[i][1], t[1], mul(P.Jv[i][0], t[0]))))));
+}
+
+// x = (L L^T)^-1 b with L's strictly-lower part in L and 1/diag in invd
+template <int D>
+__device__ __forceinline__ void chol_solve(const float (&L)[D][D], const float (&invd)[D],
+                                           const float (&b)[D], float (&x)[D]) {
+    float y[D];
+#pragma unroll
+    for (int i = 0; i < D; ++i) {
+        float s = b[i];
+#pragma unroll
+        for (int j = 0; j < i; ++j) s = fma_(-L[i][j], y[j], s);
+        y[i] = mul(s, invd[i]);
+    }
+#pragma unroll
+    for (int i = D - 1; i >= 0; --i) {
+        float s = y[i];
+#pragma unroll
+        for (int j = i + 1; j < D; ++j) s = fma_(-L[j][i], x[j], s);
+        x[i] = mul(s, invd[i]);
+    }
+}
+
+// S4 + S5: A = J^T J + lambda I, g = J^T r, in-register Cholesky A = L L^T, delta = -A^-1 g,
+// then `refine` steps of iterative refinement with the semi-normal residual
+//   rho = -J^T (r + J delta) - lambda delta,  delta += A^-1 rho                     (DESIGN R4)
+// which removes the 1/lambda amplification of fp32 rounding along the self-motion direction.
+// Returns false on a non-positive pivot or a non-finite step (=> the iteration is a reject).
+template <int D>
+__device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine, float (&delta)[D]) {
+    float L[D][D], invd[D], g[D];
+#pragma unroll
+    for (int i = 0; i < D; ++i) {
+#pragma unroll
+        for (int j = 0; j <= i; ++j) L[i][j] = coldot<D>(P, i, j);
+        L[i][i] = add(L[i][i], lam);
+        g[i] = -colvec<D>(P, i, P.r);
+    }
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < D; ++k) {
+        const float piv = L[k][k];
+        ok = ok && (piv > 0.f);
+        const float id = rsqrtf(piv);
+        invd[k] = id;
+#pragma unroll
+        for (int i = k + 1; i < D; ++i) L[i][k] = mul(L[i][k], id);
+#pragma unroll
+        for (int j = k + 1; j < D; ++j)
+#pragma unroll
+            for (int i = j; i < D; ++i) L[i][j] = fma_(-L[i][k], L[j][k], L[i][j]);
+    }
+    chol_solve<D>(L, invd, g, delta);
+    for (int it = 0; it < refine; ++it) {
+        float t[6], rho[D], e[D];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            float sv = P.r[k], sw = P.r[3 + k];
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                sv = fma_(P.Jv[j][k], delta[j], sv);
+                sw = fma_(P.Jw[j][k], delta[j], sw);
+            }
+            t[k] = sv;
+            t[3 + k] = sw;
+        }
+#pragma unroll
+        for (int i = 0; i < D; ++i) rho[i] = -fma_(lam, delta[i], colvec<D>(P, i, t));
+        chol_solve<D>(L, invd, rho, e);
+#pragma unroll
+        for (int i = 0; i < D; ++i) delta[i] = add(delta[i], e[i]);
+    }
+    float asum = 0.f;
+#pragma unroll
+    for (int i = 0; i < D; ++i) asum = add(asum, fabsf(delta[i]));
+    return ok && (asum < 1e30f);
+}
+
+} // namespace lmk

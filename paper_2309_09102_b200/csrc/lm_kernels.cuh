@@ -1,0 +1,209 @@
+// lm_kernels.cuh -- the kernels of the batched LM hot path (sm_100a).
+//
+//   lm_iterate_kernel<D, FAST>  S0..S10: load -> [Jacobian -> normal equations -> Cholesky ->
+//                               trial -> FK + residual -> accept / lambda -> freeze]* -> store.
+//                               One thread per waypoint block, the whole iteration loop on the
+//                               device, state in registers; lm_step and lm_run are the same
+//                               kernel with different iteration limits.
+//   lm_fk_kernel<D, FAST>       S1 only (targets for synthetic workloads, FK parity tests).
+//   lm_traj_stats_kernel        per-trajectory converged flag / iteration count (integer only).
+#pragma once
+#include "lm_device.cuh"
+
+namespace lmk {
+
+struct KArgs {
+    KChain ch;
+    float lambda0, nu_up, inv_nu_down, lambda_min, lambda_max, tol2;
+    float w_pos, w_rot, inv_w_pos, inv_w_rot;
+    int32_t weighted, refine;
+    int64_t W;              // waypoint blocks
+    int32_t n;              // waypoints per trajectory
+    int32_t shared_targets; // target index = w % n
+    int32_t fresh;          // 1: state := (seeds, lambda0, 0 iters) instead of reading the state arrays
+    int32_t max_total;      // stop when iters == max_total
+    int32_t at_most;        // and after this many iterations in this launch
+    const float *tp, *tq, *seeds;
+    float *q, *lam, *res, *perr, *rerr; // state / outputs, SoA [.][W]
+    uint32_t *its;                      // iters | status << 8
+    unsigned long long *mask;
+    float *trace_q, *trace_F;           // nullable debug trace
+};
+
+__device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z, float (&Rt)[3][3]) {
+    // DESIGN R11: re-normalise, then the textbook conversion; Rt[k] = k-th COLUMN of R_t
+    const float n2 = fma_(z, z, fma_(y, y, fma_(x, x, mul(w, w))));
+    const float inv = __fdiv_rn(1.0f, __fsqrt_rn(n2));
+    w = mul(w, inv); x = mul(x, inv); y = mul(y, inv); z = mul(z, inv);
+    const float xx = mul(x, x), yy = mul(y, y), zz = mul(z, z);
+    const float xy = mul(x, y), xz = mul(x, z), yz = mul(y, z);
+    const float wx = mul(w, x), wy = mul(w, y), wz = mul(w, z);
+    Rt[0][0] = fma_(-2.f, add(yy, zz), 1.f); Rt[1][0] = mul(2.f, sub(xy, wz));        Rt[2][0] = mul(2.f, add(xz, wy));
+    Rt[0][1] = mul(2.f, add(xy, wz));        Rt[1][1] = fma_(-2.f, add(xx, zz), 1.f); Rt[2][1] = mul(2.f, sub(yz, wx));
+    Rt[0][2] = mul(2.f, sub(xz, wy));        Rt[1][2] = mul(2.f, add(yz, wx));        Rt[2][2] = fma_(-2.f, add(xx, yy), 1.f);
+}
+
+template <int D, bool FAST>
+__global__ void __launch_bounds__(256) lm_iterate_kernel(const __grid_constant__ KArgs A) {
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = w < A.W;
+    const int64_t wc = live ? w : A.W - 1; // tail lanes shadow the last waypoint, never store
+    const int64_t W = A.W;
+
+    // ---- S0 load (SoA: consecutive lanes read consecutive 4-byte words => 128-byte lines)
+    float q[D];
+    float lam;
+    uint32_t k, st;
+    unsigned long long mask;
+    if (A.fresh) {
+#pragma unroll
+        for (int j = 0; j < D; ++j) q[j] = __ldg(A.seeds + (int64_t)j * W + wc);
+        lam = A.lambda0; k = 0; st = 0; mask = 0ull;
+    } else {
+#pragma unroll
+        for (int j = 0; j < D; ++j) q[j] = A.q[(int64_t)j * W + wc];
+        lam = A.lam[wc];
+        const uint32_t pk = A.its[wc];
+        k = pk & 0xffu;
+        st = (pk >> 8) & ~(1u | 2u); // FROZEN / MAXITER are re-derived below
+        mask = A.mask[wc];
+    }
+    float pt[3], Rt[3][3];
+    {
+        const int64_t Wt = A.shared_targets ? (int64_t)A.n : W;
+        const int64_t wt = A.shared_targets ? (wc % A.n) : wc;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) pt[i] = __ldg(A.tp + (int64_t)i * Wt + wt);
+        quat_to_cols(__ldg(A.tq + wt), __ldg(A.tq + Wt + wt), __ldg(A.tq + 2 * Wt + wt), __ldg(A.tq + 3 * Wt + wt), Rt);
+    }
+    const bool weighted = A.weighted != 0;
+
+    Pose<D> cur;
+    eval_pose<D, FAST>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, weighted, cur, nullptr, nullptr);
+
+    // ---- S3..S9: the LM loop, entirely on the device.  A lane is `active` while it is not
+    // frozen and has iterations left; the warp leaves the loop when no lane is active.
+    uint32_t done = 0;
+    while (true) {
+        const bool active = (k < (uint32_t)A.max_total) && (done < (uint32_t)A.at_most) && !(cur.F < A.tol2);
+        if (!__any_sync(0xffffffffu, active)) break;
+
+        float delta[D];
+        const bool ok = lm_delta<D>(cur, lam, A.refine, delta);     // S4, S5
+        float qt[D];
+        bool clamped = false;
+#pragma unroll
+        for (int j = 0; j < D; ++j) {                               // S6 (DESIGN R6)
+            const float t = add(q[j], delta[j]);
+            qt[j] = fminf(fmaxf(t, A.ch.lo[j]), A.ch.hi[j]);
+            clamped = clamped || (qt[j] != t);
+        }
+        Pose<D> tri;
+        eval_pose<D, FAST>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, weighted, tri, nullptr, nullptr); // S7
+
+        if (A.trace_q != nullptr && active && live) {
+#pragma unroll
+            for (int j = 0; j < D; ++j) A.trace_q[(int64_t)j * W + w] = qt[j];
+            A.trace_F[w] = cur.F;
+            A.trace_F[W + w] = tri.F;
+        }
+
+        // S8 (DESIGN R5): strict decrease accepts; NaN / inf trial cost compares false => reject
+        const bool accept = active && ok && (tri.F < cur.F);
+        if (active) {
+            if (!ok) st |= 4u;
+            if (!(fabsf(tri.F) < 3.0e38f)) st |= 8u;
+            if (accept && clamped) st |= 16u;
+            const float lam_acc = fmaxf(mul(lam, A.inv_nu_down), A.lambda_min);
+            const float lam_rej = fminf(mul(lam, A.nu_up), A.lambda_max);
+            lam = accept ? lam_acc : lam_rej;
+            if (accept) mask |= 1ull << k;
+            ++k;
+            ++done;
+        }
+        if (accept) {
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                q[j] = qt[j];
+#pragma unroll
+                for (int i = 0; i < 3; ++i) { cur.Jv[j][i] = tri.Jv[j][i]; cur.Jw[j][i] = tri.Jw[j][i]; }
+            }
+#pragma unroll
+            for (int i = 0; i < 6; ++i) cur.r[i] = tri.r[i];
+            cur.F = tri.F;
+        }
+    }
+
+    // ---- S10 store
+    if (!live) return;
+    const bool frozen = cur.F < A.tol2;
+    if (frozen) st |= 1u;
+    else if (k >= (uint32_t)A.max_total) st |= 2u;
+#pragma unroll
+    for (int j = 0; j < D; ++j) A.q[(int64_t)j * W + w] = q[j];
+    A.lam[w] = lam;
+    A.its[w] = k | (st << 8);
+    A.mask[w] = mask;
+    A.res[w] = __fsqrt_rn(cur.F);
+    A.perr[w] = mul(__fsqrt_rn(fma_(cur.r[2], cur.r[2], fma_(cur.r[1], cur.r[1], mul(cur.r[0], cur.r[0])))), A.inv_w_pos);
+    A.rerr[w] = mul(__fsqrt_rn(fma_(cur.r[5], cur.r[5], fma_(cur.r[4], cur.r[4], mul(cur.r[3], cur.r[3])))), A.inv_w_rot);
+}
+
+struct KFkArgs {
+    KChain ch;
+    int64_t count;
+    const float *q;
+    float *pos, *rot;
+};
+
+template <int D, bool FAST>
+__global__ void __launch_bounds__(256) lm_fk_kernel(const __grid_constant__ KFkArgs A) {
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= A.count) return;
+    float q[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) q[j] = __ldg(A.q + (int64_t)j * A.count + w);
+    const float pt[3] = {0.f, 0.f, 0.f};
+    const float Rt[3][3] = {{1.f, 0.f, 0.f}, {0.f, 1.f, 0.f}, {0.f, 0.f, 1.f}};
+    Pose<D> P;
+    float p[3], R[3][3];
+    eval_pose<D, FAST>(A.ch, q, pt, Rt, 1.f, 1.f, false, P, p, R);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        A.pos[(int64_t)i * A.count + w] = p[i];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) A.rot[(int64_t)(3 * i + c) * A.count + w] = R[i][c];
+    }
+}
+
+// One warp per trajectory: converged = AND of frozen bits, iters = MAX, total = SUM (integers only,
+// so the atomics below cannot disturb bit-stability).
+__global__ void lm_traj_stats_kernel(const uint32_t *__restrict__ its, int64_t B, int32_t n,
+                                     uint8_t *__restrict__ conv, int32_t *__restrict__ titers,
+                                     unsigned long long *__restrict__ totals) {
+    const int64_t b = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (b >= B) return;
+    uint32_t all = 1u, mx = 0u;
+    unsigned long long sum = 0ull;
+    for (int i = lane; i < n; i += 32) {
+        const uint32_t pk = its[b * n + i];
+        all &= (pk >> 8) & 1u;
+        mx = max(mx, pk & 0xffu);
+        sum += pk & 0xffu;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        all &= __shfl_xor_sync(0xffffffffu, all, o);
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    }
+    if (lane == 0) {
+        conv[b] = (uint8_t)all;
+        titers[b] = (int32_t)mx;
+        atomicAdd(totals, sum);
+        if (all) atomicAdd(totals + 1, 1ull);
+    }
+}
+
+} // namespace lmk

@@ -1,0 +1,333 @@
+"""Thin ctypes binding of include/lm.h (liblm_b200.so): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels.  PyTorch is used for device
+memory (``torch.empty(..., device="cuda")``) and the stream handle, nothing else.  There is no
+CPU fallback: if the library has not been built (``python -m paper_2309_09102_b200.build``) or
+no CUDA device is present, the calls raise.
+
+The functions ``lm_*`` mirror the C entry points one to one; ``Solver`` bundles the buffers of
+one problem (it owns the torch tensors the library borrows).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+from .build import LIB_PATH
+
+LM_MAX_DOF = 8
+LM_MAX_ITERS = 64
+LM_OK, LM_EINVAL, LM_ENOMEM, LM_ECUDA = 0, -1, -2, -3
+LM_MEM_DEVICE, LM_MEM_HOST = 0, 1
+LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1, 2, 4, 8, 16
+
+# every symbol include/lm.h declares (checked by tests/test_abi.py)
+SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_run", "lm_fetch",
+           "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_launch", "lm_fk", "lm_free",
+           "lm_strerror", "lm_launch_count")
+
+
+class LmChain(C.Structure):
+    _fields_ = [("dof", C.c_int32), ("joint_type", C.POINTER(C.c_uint8)), ("dh", C.POINTER(C.c_double)),
+                ("q_lo", C.POINTER(C.c_double)), ("q_hi", C.POINTER(C.c_double)), ("tool", C.c_double * 7)]
+
+
+class LmProblem(C.Structure):
+    _fields_ = [("B", C.c_int64), ("n", C.c_int64), ("target_pos", C.c_void_p), ("target_quat", C.c_void_p),
+                ("shared_targets", C.c_int32), ("seeds", C.c_void_p), ("memory", C.c_int32),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+class LmParams(C.Structure):
+    _fields_ = [("lambda0", C.c_float), ("nu_up", C.c_float), ("nu_down", C.c_float),
+                ("lambda_min", C.c_float), ("lambda_max", C.c_float), ("tol", C.c_float),
+                ("w_pos", C.c_float), ("w_rot", C.c_float), ("refine_steps", C.c_int32),
+                ("fast_sincos", C.c_int32)]
+
+
+class LmStats(C.Structure):
+    _fields_ = [("res_norm", C.c_void_p), ("pos_err", C.c_void_p), ("rot_err", C.c_void_p),
+                ("lambda_", C.c_void_p), ("iters", C.c_void_p), ("accept_mask", C.c_void_p),
+                ("status", C.c_void_p), ("traj_converged", C.c_void_p), ("traj_iters", C.c_void_p),
+                ("total_waypoint_iters", C.c_int64), ("converged_trajectories", C.c_int64)]
+
+
+class LmError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {lm_strerror(code)} ({code})")
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load liblm_b200.so; fails loudly if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2309_09102_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.lm_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.c_int32, C.c_int32]
+        L.lm_workspace_bytes.restype = C.c_size_t
+        L.lm_default_params.argtypes = [C.POINTER(LmParams)]
+        L.lm_init.argtypes = [C.POINTER(C.c_void_p), C.POINTER(LmChain), C.POINTER(LmProblem),
+                              C.POINTER(LmParams), C.c_void_p]
+        L.lm_step.argtypes = [C.c_void_p]
+        L.lm_run.argtypes = [C.c_void_p, C.c_int32]
+        L.lm_fetch.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(LmStats)]
+        L.lm_reset.argtypes = [C.c_void_p]
+        L.lm_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lm_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lm_set_launch.argtypes = [C.c_void_p, C.c_int32]
+        L.lm_fk.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+        L.lm_free.argtypes = [C.c_void_p]
+        L.lm_free.restype = None
+        L.lm_strerror.argtypes = [C.c_int]
+        L.lm_strerror.restype = C.c_char_p
+        L.lm_launch_count.restype = C.c_int64
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != LM_OK:
+        raise LmError(rc, where)
+
+
+# ------------------------------------------------------------------ 1:1 wrappers
+
+def lm_strerror(code: int) -> str:
+    return lib().lm_strerror(int(code)).decode()
+
+
+def lm_launch_count() -> int:
+    return int(lib().lm_launch_count())
+
+
+def lm_workspace_bytes(dof: int, B: int, n: int, shared_targets: int = 0, memory: int = LM_MEM_DEVICE) -> int:
+    return int(lib().lm_workspace_bytes(dof, B, n, shared_targets, memory))
+
+
+def lm_default_params(**overrides) -> LmParams:
+    p = LmParams()
+    _check(lib().lm_default_params(C.byref(p)), "lm_default_params")
+    for k, v in overrides.items():
+        if not hasattr(p, k):
+            raise AttributeError(k)
+        setattr(p, k, v)
+    return p
+
+
+def make_chain(chain) -> tuple:
+    """Marshal a workloads.Chain-like object into an LmChain (returns the struct and the arrays it
+    points to, which must outlive the lm_init call)."""
+    d = int(chain.dof)
+    jt = np.ascontiguousarray(np.asarray(chain.joint_type), dtype=np.uint8)
+    dh = np.ascontiguousarray(np.stack([chain.a, chain.alpha, chain.d, chain.theta], axis=1), dtype=np.float64)
+    lo = np.ascontiguousarray(chain.q_lo, dtype=np.float64)
+    hi = np.ascontiguousarray(chain.q_hi, dtype=np.float64)
+    c = LmChain()
+    c.dof = d
+    c.joint_type = jt.ctypes.data_as(C.POINTER(C.c_uint8))
+    c.dh = dh.ctypes.data_as(C.POINTER(C.c_double))
+    c.q_lo = lo.ctypes.data_as(C.POINTER(C.c_double))
+    c.q_hi = hi.ctypes.data_as(C.POINTER(C.c_double))
+    for i, v in enumerate(np.asarray(chain.tool, dtype=np.float64)):
+        c.tool[i] = float(v)
+    return c, (jt, dh, lo, hi)
+
+
+def lm_init(chain: LmChain, problem: LmProblem, params: LmParams, cuda_stream: int = 0) -> int:
+    ctx = C.c_void_p()
+    _check(lib().lm_init(C.byref(ctx), C.byref(chain), C.byref(problem), C.byref(params),
+                         C.c_void_p(cuda_stream)), "lm_init")
+    return ctx.value
+
+
+def lm_step(ctx: int) -> None:
+    _check(lib().lm_step(ctx), "lm_step")
+
+
+def lm_run(ctx: int, max_iters: int) -> None:
+    _check(lib().lm_run(ctx, int(max_iters)), "lm_run")
+
+
+def lm_reset(ctx: int) -> None:
+    _check(lib().lm_reset(ctx), "lm_reset")
+
+
+def lm_fetch(ctx: int, q_out_ptr: Optional[int], stats: Optional[LmStats]) -> None:
+    _check(lib().lm_fetch(ctx, q_out_ptr, C.byref(stats) if stats is not None else None), "lm_fetch")
+
+
+def lm_set_state(ctx: int, q_ptr: int, lambda_ptr: Optional[int]) -> None:
+    _check(lib().lm_set_state(ctx, q_ptr, lambda_ptr), "lm_set_state")
+
+
+def lm_set_trace(ctx: int, trial_q_ptr: Optional[int], trial_F_ptr: Optional[int]) -> None:
+    _check(lib().lm_set_trace(ctx, trial_q_ptr, trial_F_ptr), "lm_set_trace")
+
+
+def lm_set_launch(ctx: int, block_threads: int) -> None:
+    _check(lib().lm_set_launch(ctx, int(block_threads)), "lm_set_launch")
+
+
+def lm_fk(ctx: int, q_ptr: int, count: int, pos_ptr: int, rot_ptr: int) -> None:
+    _check(lib().lm_fk(ctx, q_ptr, int(count), pos_ptr, rot_ptr), "lm_fk")
+
+
+def lm_free(ctx: int) -> None:
+    lib().lm_free(ctx)
+
+
+# ------------------------------------------------------------------ buffer bundle
+
+class Solver:
+    """Owns the torch device tensors of one problem and the lm_ctx that borrows them.
+
+    ``target_pos [W,3]``, ``target_quat [W,4]`` (``[n,.]`` when shared), ``seeds [W,d]`` are
+    waypoint-major numpy arrays (as produced by ``workloads``); they are transposed to the
+    library's SoA layout here.  ``host_inputs=True`` hands the library pinned HOST arrays instead
+    (LM_MEM_HOST: the host->device copies happen inside lm_init).
+    """
+
+    def __init__(self, chain, B: int, n: int, target_pos, target_quat, seeds, params: Optional[LmParams] = None,
+                 shared_targets: bool = False, host_inputs: bool = False, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the batched-LM path has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.chain, self.B, self.n, self.W, self.d = chain, int(B), int(n), int(B) * int(n), int(chain.dof)
+        self.params = params if params is not None else lm_default_params()
+        self.shared = bool(shared_targets)
+        self.host_inputs = bool(host_inputs)
+        self.stream = stream
+        self._ctx = None
+        Wt = self.n if self.shared else self.W
+        assert np.shape(target_pos) == (Wt, 3) and np.shape(target_quat) == (Wt, 4) and np.shape(seeds) == (self.W, self.d)
+
+        def soa(x):
+            t = torch.from_numpy(np.ascontiguousarray(np.asarray(x, dtype=np.float32).T))
+            return t.pin_memory() if self.host_inputs else t.to(self.device)
+
+        with torch.cuda.device(self.device):
+            self.tp, self.tq, self.seeds = soa(target_pos), soa(target_quat), soa(seeds)
+            mem = LM_MEM_HOST if self.host_inputs else LM_MEM_DEVICE
+            nbytes = lm_workspace_bytes(self.d, self.B, self.n, int(self.shared), mem)
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            ws_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+            self._cchain, self._keep = make_chain(chain)
+            pb = LmProblem(self.B, self.n, self.tp.data_ptr(), self.tq.data_ptr(), int(self.shared),
+                           self.seeds.data_ptr(), mem, ws_ptr, nbytes)
+            s = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self._stream_handle = int(s.cuda_stream)
+            self._ctx = lm_init(self._cchain, pb, self.params, self._stream_handle)
+
+    # -- the hot path
+    def step(self) -> None:
+        lm_step(self._ctx)
+
+    def run(self, max_iters: int) -> None:
+        lm_run(self._ctx, max_iters)
+
+    def reset(self) -> None:
+        lm_reset(self._ctx)
+
+    def set_launch(self, block_threads: int) -> None:
+        lm_set_launch(self._ctx, block_threads)
+
+    def set_state(self, q, lam=None) -> None:
+        """q [W,d], lam [W] numpy (waypoint-major)."""
+        torch = self.torch
+        self._q_in = torch.from_numpy(np.ascontiguousarray(np.asarray(q, dtype=np.float32).T)).to(self.device)
+        self._lam_in = None if lam is None else torch.from_numpy(np.ascontiguousarray(lam, dtype=np.float32)).to(self.device)
+        lm_set_state(self._ctx, self._q_in.data_ptr(), None if lam is None else self._lam_in.data_ptr())
+
+    def enable_trace(self) -> None:
+        torch = self.torch
+        self.trace_q = torch.full((self.d, self.W), float("nan"), dtype=torch.float32, device=self.device)
+        self.trace_F = torch.full((2, self.W), float("nan"), dtype=torch.float32, device=self.device)
+        lm_set_trace(self._ctx, self.trace_q.data_ptr(), self.trace_F.data_ptr())
+
+    def fetch(self, host: bool = True) -> dict:
+        """lm_fetch into fresh buffers; returns numpy arrays (host=True: the library writes pinned
+        host memory directly; host=False: device tensors copied back by torch afterwards)."""
+        torch = self.torch
+        W, B, d = self.W, self.B, self.d
+
+        def buf(shape, dtype):
+            if host:
+                return torch.empty(shape, dtype=dtype).pin_memory()
+            return torch.empty(shape, dtype=dtype, device=self.device)
+
+        out = {"q": buf((d, W), torch.float32), "res_norm": buf((W,), torch.float32),
+               "pos_err": buf((W,), torch.float32), "rot_err": buf((W,), torch.float32),
+               "lam": buf((W,), torch.float32), "iters": buf((W,), torch.int32),
+               "mask": buf((W,), torch.int64), "status": buf((W,), torch.int32),
+               "traj_converged": buf((B,), torch.uint8), "traj_iters": buf((B,), torch.int32)}
+        st = LmStats(out["res_norm"].data_ptr(), out["pos_err"].data_ptr(), out["rot_err"].data_ptr(),
+                     out["lam"].data_ptr(), out["iters"].data_ptr(), out["mask"].data_ptr(),
+                     out["status"].data_ptr(), out["traj_converged"].data_ptr(), out["traj_iters"].data_ptr(), 0, 0)
+        lm_fetch(self._ctx, out["q"].data_ptr(), st)
+        res = {k: v.cpu().numpy() for k, v in out.items()}
+        res["q"] = np.ascontiguousarray(res["q"].T)
+        res["mask"] = res["mask"].view(np.uint64)
+        res["status"] = res["status"].view(np.uint32)
+        res["total_waypoint_iters"] = int(st.total_waypoint_iters)
+        res["converged_trajectories"] = int(st.converged_trajectories)
+        if getattr(self, "trace_q", None) is not None:
+            res["trial_q"] = np.ascontiguousarray(self.trace_q.cpu().numpy().T)
+            tf = self.trace_F.cpu().numpy()
+            res["F_before"], res["F_trial"] = tf[0], tf[1]
+        return res
+
+    def fetch_totals(self) -> tuple:
+        """lm_fetch of the two scalar totals only (synchronises the stream)."""
+        st = LmStats()
+        lm_fetch(self._ctx, None, st)
+        return int(st.total_waypoint_iters), int(st.converged_trajectories)
+
+    def fk(self, q) -> tuple:
+        """Device FK of q [count, d] -> (pos [count,3], R [count,3,3]) float64 numpy."""
+        torch = self.torch
+        q = np.asarray(q, dtype=np.float32)
+        count = q.shape[0]
+        qd = torch.from_numpy(np.ascontiguousarray(q.T)).to(self.device)
+        pos = torch.empty((3, count), dtype=torch.float32, device=self.device)
+        rot = torch.empty((9, count), dtype=torch.float32, device=self.device)
+        lm_fk(self._ctx, qd.data_ptr(), count, pos.data_ptr(), rot.data_ptr())
+        torch.cuda.synchronize(self.device)
+        return (pos.cpu().numpy().T.astype(np.float64),
+                rot.cpu().numpy().T.reshape(count, 3, 3).astype(np.float64))
+
+    def close(self) -> None:
+        if self._ctx is not None:
+            self.torch.cuda.synchronize(self.device)
+            lm_free(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def device_fk(chain, device: str = "cuda:0"):
+    """An ``fk`` callable for workloads.*: FK on the GPU through lm_fk (S1 of the hot path)."""
+    dummy = Solver(chain, 1, 1, np.zeros((1, 3), np.float32), np.array([[1, 0, 0, 0]], np.float32),
+                   np.zeros((1, chain.dof), np.float32), device=device)
+
+    def fk(q):
+        q = np.asarray(q, dtype=np.float64)
+        flat = q.reshape(-1, chain.dof)
+        pos, R = dummy.fk(flat)
+        return pos.reshape(q.shape[:-1] + (3,)), R.reshape(q.shape[:-1] + (3, 3))
+
+    return fk

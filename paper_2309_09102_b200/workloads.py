@@ -159,39 +159,39 @@ def _from_truth(name, chain, truth, sigma, rng, fk: FkFn, tol, max_iters, lambda
                     lambda0=lambda0, truth=flat)
 
 
-def config1(fk: FkFn) -> Workload:
+def config1(fk: FkFn, seed_offset: int = 0) -> Workload:
     """BASELINE.json configs[0]: 1 x 50, Panda, 3 sinusoids amp 0.3, seeds N(0, 0.05), 20 iters."""
-    rng = np.random.default_rng(1)
+    rng = np.random.default_rng(1 + seed_offset)
     ch = panda_chain()
     return _from_truth("C1", ch, smooth_joint_paths(ch, 1, 50, 3, 0.3, rng), 0.05, rng, fk, 0.0, 20)
 
 
-def config2(fk: FkFn, B: int = 512, n: int = 300) -> Workload:
+def config2(fk: FkFn, B: int = 512, n: int = 300, seed_offset: int = 0) -> Workload:
     """configs[1]: 512 x 300, Panda, 5 sinusoids amp 0.5, seeds N(0, 0.1), tol 1e-5, <= 50 iters."""
-    rng = np.random.default_rng(2)
+    rng = np.random.default_rng(2 + seed_offset)
     ch = panda_chain()
     return _from_truth("C2", ch, smooth_joint_paths(ch, B, n, 5, 0.5, rng), 0.1, rng, fk, 1e-5, 50)
 
 
-def config3(fk: FkFn, B: int = 2048, n: int = 300) -> Workload:
+def config3(fk: FkFn, B: int = 2048, n: int = 300, seed_offset: int = 0) -> Workload:
     """configs[2]: 2048 x 300, 8-DoF chain with one prismatic joint, seeds N(0, 0.15)."""
     ch = random_chain_8dof(3)
-    rng = np.random.default_rng(4)
+    rng = np.random.default_rng(4 + seed_offset)
     return _from_truth("C3", ch, smooth_joint_paths(ch, B, n, 5, 0.5, rng), 0.15, rng, fk, 1e-5, 50)
 
 
-def config5(fk: FkFn, B: int, n: int) -> Workload:
+def config5(fk: FkFn, B: int, n: int, seed_offset: int = 0) -> Workload:
     """configs[4] sweep point: B x n, Panda, paths as config 2, fixed 20 iterations."""
-    rng = np.random.default_rng(6)
+    rng = np.random.default_rng(6 + seed_offset)
     ch = panda_chain()
     return _from_truth(f"C5_{B}x{n}", ch, smooth_joint_paths(ch, B, n, 5, 0.5, rng), 0.1, rng, fk, 0.0, 20)
 
 
-def config4(fk: FkFn, B: int = 4096, n: int = 300) -> Workload:
+def config4(fk: FkFn, B: int = 4096, n: int = 300, seed_offset: int = 0) -> Workload:
     """configs[3]: 4096 x 300, Panda; SE(3) lines / circles (radius U[0.1, 0.3] m), orientation
     slerp over <= 90 deg; seeds = anchor configuration + N(0, 0.2) at every waypoint; 50 iters.
     Reachability of the far end of a path is NOT guaranteed -- that is the workload."""
-    rng = np.random.default_rng(5)
+    rng = np.random.default_rng(5 + seed_offset)
     ch = panda_chain()
     d = ch.dof
     mid = 0.5 * (ch.q_lo + ch.q_hi)

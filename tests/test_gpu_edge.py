@@ -1,0 +1,226 @@
+"""Bit-stability (P11), edge cases and API behaviour of the CUDA path -- needs a B200."""
+import numpy as np
+import pytest
+
+from oracle import lm_oracle as orc
+from paper_2309_09102_b200 import workloads as wl
+
+import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+KEYS = ("q", "res_norm", "pos_err", "rot_err", "lam", "iters", "mask", "status")
+
+
+@pytest.fixture(scope="module")
+def lm():
+    from paper_2309_09102_b200 import build, lm as _lm
+    build.build()
+    return _lm
+
+
+def same_bits(a, b, keys=KEYS, sl=None):
+    for k in keys:
+        x, y = a[k], b[k]
+        if sl is not None:
+            y = y[sl]
+        assert np.array_equal(x.view(np.uint32) if x.dtype == np.float32 else x,
+                              y.view(np.uint32) if y.dtype == np.float32 else y), k
+
+
+@pytest.fixture(scope="module")
+def w_small():
+    return wl.config2(H.oracle_fk(wl.panda_chain()), B=7, n=101)  # W = 707: ragged tail
+
+
+def test_bitwise_repeatable_and_launch_geometry_independent(lm, w_small):
+    ref = H.run_gpu(w_small)
+    same_bits(H.run_gpu(w_small), ref)
+    for block in (32, 64, 96, 256):
+        s = H.make_solver(w_small)
+        s.set_launch(block)
+        s.run(w_small.max_iters)
+        same_bits(s.fetch(), ref)
+        s.close()
+
+
+def test_bits_independent_of_batch_composition(lm, w_small):
+    ref = H.run_gpu(w_small)
+    sub = w_small.subset(slice(2, 5))
+    same_bits(H.run_gpu(sub), ref, sl=slice(2 * w_small.n, 5 * w_small.n))
+    # a single waypoint on its own
+    i = 3 * w_small.n + 17
+    one = wl.Workload("one", w_small.chain, 1, 1, w_small.target_pos[i:i + 1], w_small.target_quat[i:i + 1],
+                      w_small.seeds[i:i + 1], w_small.tol, w_small.max_iters)
+    same_bits(H.run_gpu(one), ref, sl=slice(i, i + 1))
+
+
+@pytest.mark.parametrize("cfg", ["tol", "fixed"])
+def test_run_equals_repeated_steps(lm, w_small, cfg):
+    w = w_small if cfg == "tol" else wl.Workload("f", w_small.chain, w_small.B, w_small.n, w_small.target_pos,
+                                                 w_small.target_quat, w_small.seeds, 0.0, 9)
+    N = 9
+    ref = H.run_gpu(w, max_iters=N)
+    s = H.make_solver(w)
+    for _ in range(N):
+        s.step()
+    got = s.fetch()
+    s.close()
+    same_bits(got, ref, keys=("q", "res_norm", "lam", "iters", "mask"))
+    assert np.array_equal(got["status"] & 1, ref["status"] & 1)
+    # resumed run: run(4) then run(9) == run(9); reset restarts from the seeds
+    s = H.make_solver(w)
+    s.run(4)
+    mid = s.fetch()
+    assert mid["iters"].max() <= 4
+    s.run(N)
+    same_bits(s.fetch(), ref)
+    s.reset()
+    s.run(N)
+    same_bits(s.fetch(), ref)
+    s.close()
+
+
+def test_shared_targets_host_inputs_and_device_fetch(lm):
+    ch = wl.panda_chain()
+    w1 = wl.config2(H.oracle_fk(ch), B=1, n=77)
+    B = 5
+    rng = np.random.default_rng(7)
+    seeds = np.clip(np.tile(w1.seeds, (B, 1)) + rng.normal(size=(B * 77, 7)).astype(np.float32) * 0.02,
+                    ch.q_lo.astype(np.float32) + 1e-6, ch.q_hi.astype(np.float32) - 1e-6).astype(np.float32)
+    tiled = wl.Workload("tiled", ch, B, 77, np.tile(w1.target_pos, (B, 1)), np.tile(w1.target_quat, (B, 1)), seeds,
+                        w1.tol, w1.max_iters)
+    ref = H.run_gpu(tiled)
+    prm = lm.lm_default_params(lambda0=tiled.lambda0, tol=tiled.tol)
+    s = lm.Solver(ch, B, 77, w1.target_pos, w1.target_quat, seeds, params=prm, shared_targets=True)
+    s.run(tiled.max_iters)
+    same_bits(s.fetch(), ref)
+    same_bits(s.fetch(host=False), ref)   # lm_fetch into device buffers
+    s.close()
+    same_bits(H.run_gpu(tiled, host_inputs=True), ref)  # LM_MEM_HOST: pinned host inputs
+    s = lm.Solver(ch, B, 77, w1.target_pos, w1.target_quat, seeds, params=prm, shared_targets=True, host_inputs=True)
+    s.run(tiled.max_iters)
+    same_bits(s.fetch(), ref)
+    s.close()
+
+
+@pytest.mark.parametrize("W", [1, 31, 33, 129])
+def test_ragged_sizes(lm, W):
+    w = wl.config2(H.oracle_fk(wl.panda_chain()), B=1, n=W)
+    g, o = H.run_gpu(w), H.run_oracle(w)
+    assert np.abs(g["q"] - o.q).max() <= H.TOL_Q and np.all((g["status"] & 1) == 1)
+    assert g["total_waypoint_iters"] == g["iters"].sum()
+
+
+def test_zero_iterations_and_already_converged(lm, w_small):
+    g = H.run_gpu(w_small, max_iters=0)
+    assert np.array_equal(g["q"], w_small.seeds) and np.all(g["iters"] == 0) and np.all(g["mask"] == 0)
+    assert np.all(g["lam"] == np.float32(w_small.lambda0))
+    o = H.run_oracle(w_small, max_iters=0)
+    assert np.abs(g["res_norm"] - o.res_norm).max() < 1e-6
+    # fetch before any run is the same thing
+    s = H.make_solver(w_small)
+    g2 = s.fetch()
+    s.close()
+    same_bits(g2, g)
+    # seeds that already meet tol: frozen at once, zero iterations
+    ch = w_small.chain
+    q = np.clip(w_small.truth, ch.q_lo, ch.q_hi).astype(np.float32)
+    p, R = orc.fk(ch, q.astype(np.float64))
+    at = wl.Workload("at", ch, w_small.B, w_small.n, p.astype(np.float32), wl._R_to_quat_wxyz(R).astype(np.float32),
+                     q, 1e-5, 50)
+    g = H.run_gpu(at)
+    assert np.all(g["iters"] == 0) and np.all(g["status"] == 1) and np.array_equal(g["q"], q)
+    assert g["converged_trajectories"] == at.B
+
+
+def test_weights_match_oracle(lm):
+    w = wl.config2(H.oracle_fk(wl.panda_chain()), B=4, n=64)
+    w = wl.Workload(w.name, w.chain, w.B, w.n, w.target_pos, w.target_quat, w.seeds, 0.0, 8)
+    g = H.run_gpu(w, w_pos=2.0, w_rot=0.5)
+    o = H.run_oracle(w, w_pos=2.0, w_rot=0.5)
+    assert np.abs(g["q"] - o.q).max() <= H.TOL_Q
+    assert np.abs(g["pos_err"] - o.pos_err).max() < 1e-6 and np.abs(g["rot_err"] - o.rot_err).max() < 1e-6
+    g1 = H.run_gpu(w)
+    assert np.abs(g1["q"] - g["q"]).max() > 1e-6  # the weights do change the iteration
+
+
+def test_bad_inputs_do_not_poison_neighbours(lm, w_small):
+    ref = H.run_gpu(w_small)
+    seeds = w_small.seeds.copy()
+    bad = [5, 64, 300]
+    seeds[5, 2] = np.nan
+    seeds[64, :] = np.inf
+    tq = w_small.target_quat.copy()
+    tp = w_small.target_pos.copy()
+    tp[300] = [5.0, 5.0, 5.0]  # far outside the workspace: unreachable
+    w = wl.Workload("bad", w_small.chain, w_small.B, w_small.n, tp, tq, seeds, w_small.tol, 20)
+    g = H.run_gpu(w)
+    ok = np.ones(w.W, bool)
+    ok[bad] = False
+    refc = H.run_gpu(wl.Workload("r", w.chain, w.B, w.n, w_small.target_pos, w_small.target_quat, w_small.seeds, w.tol, 20))
+    for k in ("q", "iters", "mask"):
+        assert np.array_equal(g[k][ok], refc[k][ok]), k
+    assert np.all(g["status"][[5, 64]] & (lm.LM_ST_BREAKDOWN | lm.LM_ST_NONFINITE))
+    assert not np.any(g["status"][[5, 64]] & lm.LM_ST_FROZEN) and np.all(g["mask"][[5, 64]] == 0)
+    assert np.all(g["iters"][[5, 64]] == 20)
+    # unreachable target: finite, inside the limits, not converged, hits the iteration limit
+    assert np.all(np.isfinite(g["q"][300])) and g["status"][300] & lm.LM_ST_MAXITER
+    assert np.all(g["q"][300] >= w.chain.q_lo.astype(np.float32)) and np.all(g["q"][300] <= w.chain.q_hi.astype(np.float32))
+    assert g["res_norm"][300] > 1.0
+    assert ref["q"].shape == g["q"].shape
+
+
+def test_joint_limit_clamp(lm):
+    """targets reachable only outside a narrowed limit => q stays on the limit."""
+    ch = wl.panda_chain()
+    w = wl.config2(H.oracle_fk(ch), B=2, n=50)
+    narrow = wl.panda_chain()
+    narrow.q_hi = np.minimum(narrow.q_hi, w.truth.max(axis=0) - 0.05)
+    narrow.q_lo = np.maximum(narrow.q_lo, w.truth.min(axis=0) + 0.05)
+    seeds = np.clip(w.seeds, narrow.q_lo.astype(np.float32) + 1e-6, narrow.q_hi.astype(np.float32) - 1e-6)
+    wn = wl.Workload("narrow", narrow, w.B, w.n, w.target_pos, w.target_quat, seeds, 0.0, 12)
+    g, o = H.run_gpu(wn), H.run_oracle(wn)
+    assert np.all(g["q"] >= narrow.q_lo.astype(np.float32)) and np.all(g["q"] <= narrow.q_hi.astype(np.float32))
+    assert np.any(g["status"] & lm.LM_ST_CLAMPED)
+    # the clamped problem is non-smooth; the bulk still follows the oracle
+    dq = np.abs(g["q"] - o.q).max(axis=1)
+    assert np.median(dq) < 1e-5 and np.mean(dq <= H.TOL_Q) > 0.9
+
+
+@pytest.mark.parametrize("d", [1, 2, 3, 4, 5, 6])
+def test_low_dof_chains(lm, d):
+    rng = np.random.default_rng(40 + d)
+    ch = wl.Chain(f"gen{d}", d, (rng.random(d) < 0.25).astype(np.int32), rng.uniform(-0.3, 0.3, d),
+                  rng.choice([0.0, np.pi / 2, -np.pi / 2, 0.7], d), rng.uniform(0.0, 0.3, d), rng.uniform(-1, 1, d),
+                  np.full(d, -2.0), np.full(d, 2.0), np.array([0.05, 0.0, 0.1, 1, 0, 0, 0.0]))
+    truth = rng.uniform(-1.0, 1.0, size=(1, 90, d))
+    w = wl._from_truth("low", ch, truth, 0.05, rng, H.oracle_fk(ch), 0.0, 10)
+    g, o = H.run_gpu(w), H.run_oracle(w)
+    assert np.array_equal(g["iters"], o.iters)
+    # under-actuated chains (d < 6) sit at a least-squares point; lambda_min keeps it well conditioned
+    assert np.abs(g["q"] - o.q).max() <= H.TOL_Q
+    assert np.abs(g["res_norm"] - o.res_norm).max() <= 1e-5
+
+
+def test_solver_variants(lm, w_small):
+    o = H.run_oracle(w_small)
+    for kw in (dict(refine_steps=0), dict(refine_steps=2), dict(fast_sincos=1)):
+        g = H.run_gpu(w_small, **kw)
+        dq = np.abs(g["q"] - o.q).max(axis=1)
+        assert np.all((g["status"] & 1) == 1)
+        assert np.percentile(dq, 99) <= (H.TOL_Q if "fast_sincos" not in kw else 5e-4), kw
+
+
+def test_api_errors_on_device(lm, w_small):
+    s = H.make_solver(w_small)
+    with pytest.raises(lm.LmError):
+        lm.lm_run(s._ctx, 65)
+    with pytest.raises(lm.LmError):
+        lm.lm_set_launch(s._ctx, 40)
+    with pytest.raises(lm.LmError):
+        lm.lm_fk(s._ctx, 0, 10, 0, 0)
+    n0 = lm.lm_launch_count()
+    s.run(3)
+    assert lm.lm_launch_count() == n0 + 1   # the whole LM loop is ONE launch
+    s.close()
