@@ -20,7 +20,6 @@ from __future__ import annotations
 import argparse
 import json
 import os
-import subprocess
 import sys
 import threading
 import time
@@ -58,49 +57,52 @@ def alg_bytes_per_waypoint(d: int) -> float:
 # ------------------------------------------------------------------ clocks sampler
 
 class ClockSampler:
-    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-              "clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons sampled through NVML every 10 ms while the timed region runs
+    (the same counters `nvidia-smi --query-gpu=clocks.sm,clocks_event_reasons.*` prints)."""
+    REASONS = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
 
     def __init__(self, index: int):
-        self.index, self.lines, self.proc, self.thread = index, [], None, None
+        self.index, self.sm, self.bits, self.power = index, [], [], []
+        self.stop_flag, self.thread, self.err, self.sm_max = threading.Event(), None, None, None
+
+    def _loop(self, h, nv):
+        while not self.stop_flag.is_set():
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                self.bits.append(nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                                 if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons")
+                                 else nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+            except Exception as e:  # noqa: BLE001
+                self.err = repr(e)
+                return
+            time.sleep(0.01)
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
-                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-        except OSError:
-            return self
-        self.thread = threading.Thread(target=lambda: [self.lines.append(ln) for ln in self.proc.stdout], daemon=True)
-        self.thread.start()
+            import pynvml as nv
+            nv.nvmlInit()
+            idx = self.index
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            if vis and all(x.strip().isdigit() for x in vis.split(",")):
+                idx = int(vis.split(",")[self.index])
+            h = nv.nvmlDeviceGetHandleByIndex(idx)
+            self.sm_max = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            self.thread = threading.Thread(target=self._loop, args=(h, nv), daemon=True)
+            self.thread.start()
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
         return self
 
     def stop(self) -> dict:
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-        self.thread.join(timeout=5)
-        sm, mx, reasons = [], [], set()
-        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for ln in self.lines:
-            f = [x.strip() for x in ln.split(",")]
-            if len(f) < 7:
-                continue
-            try:
-                sm.append(float(f[0]))
-                mx.append(float(f[1]))
-            except ValueError:
-                continue
-            for nm, v in zip(names, f[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(nm)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": float(max(mx)) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+        self.stop_flag.set()
+        if self.thread is not None:
+            self.thread.join(timeout=2)
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "samples": 0, "reasons": [], "error": self.err}
+        reasons = sorted(n for n, b in self.REASONS.items() if any(x & b for x in self.bits))
+        return {"sm_mhz": float(np.median(self.sm)), "sm_min_mhz": float(min(self.sm)), "sm_max_mhz": float(self.sm_max),
+                "power_w_max": float(max(self.power)), "samples": len(self.sm), "reasons": reasons}
 
 
 # ------------------------------------------------------------------ distributed plumbing
@@ -202,7 +204,7 @@ def run_reference(args) -> None:
     from oracle import lm_oracle as orc
     from paper_2309_09102_b200 import workloads as wl
     chain = wl.random_chain_8dof(3) if args.workload == "C3" else wl.panda_chain()
-    n_traj = args.ref_traj or 64
+    n_traj = args.ref_traj or 16
     # only the sampled trajectories are generated (the generators are per-trajectory independent
     # in distribution, the sample is a prefix of a smaller batch of the same recipe)
     w = make_workload(args.workload, lambda q: orc.fk(chain, q), n_traj, args.n)
@@ -364,7 +366,7 @@ def measure_e2e(lm, torch, chain, w, prm, device, steps: int) -> dict:
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C4", "C2", "C3", "C5"])
@@ -372,7 +374,7 @@ def main() -> None:
     ap.add_argument("--n", type=int, default=None, help="waypoints per trajectory")
     ap.add_argument("--block", type=int, default=0, help="threads per block override")
     ap.add_argument("--ref-traj", type=int, default=0,
-                    help="trajectories in the oracle's timed sample (default 256 for cpu_baseline, 64 per step for --impl reference)")
+                    help="trajectories in the oracle's timed sample (default 256 for cpu_baseline, 16 per step for --impl reference)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

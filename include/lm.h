@@ -142,8 +142,16 @@ int lm_set_state(lm_ctx *ctx, const float *q, const float *lambda);
  * trial_q [d][W] = q+ and trial_F [2][W] = (F before, F+ of the trial). */
 int lm_set_trace(lm_ctx *ctx, float *trial_q, float *trial_F);
 
-/* Launch geometry override for tuning and bit-stability tests: threads per block (multiple of 32, <= 256; 0 = default). */
-int lm_set_launch(lm_ctx *ctx, int32_t block_threads);
+/* Tuning / test knobs.  LM_OPT_BLOCK_THREADS: threads per block (multiple of 32, <= 256; 0 = default 128).
+ * LM_OPT_GENERIC_KERNEL: 1 = run the generic kernel even if the chain's structure matches a
+ * specialised one (the two return the same values).  Results never depend on either. */
+#define LM_OPT_BLOCK_THREADS 1
+#define LM_OPT_GENERIC_KERNEL 2
+int lm_set_option(lm_ctx *ctx, int32_t option, int32_t value);
+
+/* Name of the LM kernel variant this context launches: "panda7", "rand8" (compile-time chain
+ * structure, csrc/lm_specs.cuh) or "generic".  Static string. */
+const char *lm_kernel_name(lm_ctx *ctx);
 
 /* Forward kinematics on the device with the context's chain (S1 of the hot path):
  * q [d][count] -> pos [3][count], rot [9][count] (row-major R, SoA).  Device pointers.  Async. */

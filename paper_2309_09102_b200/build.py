@@ -13,12 +13,15 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _ROOT = os.path.dirname(_HERE)
 LIB_PATH = os.path.join(_HERE, "liblm_b200.so")
-SOURCES = [os.path.join(_CSRC, "lm_api.cu")]
-DEPS = SOURCES + [os.path.join(_CSRC, "lm_kernels.cuh"), os.path.join(_CSRC, "lm_device.cuh"),
-                  os.path.join(_ROOT, "include", "lm.h")]
+SOURCES = [os.path.join(_CSRC, f) for f in ("lm_api.cu", "lm_inst_specs.cu", "lm_inst_generic_lo.cu",
+                                            "lm_inst_generic_hi.cu")]
+DEPS = SOURCES + [os.path.join(_CSRC, f) for f in ("lm_kernels.cuh", "lm_device.cuh", "lm_specs.cuh", "lm_launch.h")] \
+    + [os.path.join(_ROOT, "include", "lm.h")]
 
+# -ftz / -prec-div / -prec-sqrt only affect sqrtf(), rsqrtf() and '/' (MUFU forms); every other
+# floating-point operation in the kernels is an explicit round-to-nearest intrinsic.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
+              "-ftz=true", "-prec-div=false", "-prec-sqrt=false", "-Xcompiler", "-fPIC"]
 
 
 def nvcc() -> str:
@@ -36,15 +39,34 @@ def is_stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile each translation unit (in parallel) and link liblm_b200.so."""
     if not (force or is_stale()):
         return LIB_PATH
-    tmp = LIB_PATH + f".tmp{os.getpid()}"
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
-    res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout)
+    from concurrent.futures import ThreadPoolExecutor
+    objdir = os.path.join(_HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+
+    def compile_one(src):
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + f".{os.getpid()}.o")
+        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+        res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+        if res.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout)
+        return obj, res.stdout
+
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+        results = list(ex.map(compile_one, SOURCES))
     if verbose:
-        print(res.stdout)
+        for _, out in results:
+            print(out)
+    tmp = LIB_PATH + f".tmp{os.getpid()}"
+    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static", "-o", tmp] \
+        + [o for o, _ in results]
+    res = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    for o, _ in results:
+        os.remove(o)
+    if res.returncode != 0:
+        raise RuntimeError("link failed:\n" + " ".join(cmd) + "\n" + res.stdout)
     os.replace(tmp, LIB_PATH)
     return LIB_PATH
 

@@ -1,7 +1,7 @@
 // lm_api.cu -- C ABI of include/lm.h: validation, workspace carving, launches.  No torch types,
 // no CPU compute path: every step of the hot path runs in the kernels of lm_kernels.cuh.
 #include "../../include/lm.h"
-#include "lm_kernels.cuh"
+#include "lm_launch.h"
 
 #include <atomic>
 #include <climits>
@@ -67,6 +67,36 @@ float round_inward(double x, bool lower) { // fp32 value inside [lo, hi] of the 
     return f;
 }
 
+// Structure of a run-time chain in the canonical form of lm_specs.cuh (prismatic joints carry
+// the d0 / t0 bits: neither offset is used on that path).
+ChainSpec chain_signature(int d, const KChain &k) {
+    ChainSpec s{false, d, 0, 0, 0, 0, 0, 0, 0, k.tool_has_rot != 0, 0};
+    for (int j = 0; j < d; ++j) {
+        const uint32_t b = 1u << j;
+        const bool pris = (k.prismatic_mask & b) != 0;
+        if (pris) s.pris |= b;
+        if (k.ca[j] == 1.f && k.sa[j] == 0.f) s.al0 |= b;
+        if (k.ca[j] == 0.f && k.sa[j] == 1.f) s.alp |= b;
+        if (k.ca[j] == 0.f && k.sa[j] == -1.f) s.aln |= b;
+        if (k.a[j] == 0.f) s.a0 |= b;
+        if (k.d[j] == 0.f || pris) s.d0 |= b;
+        if (k.toff[j] == 0.f || pris) s.t0 |= b;
+    }
+    for (int i = 0; i < 3; ++i)
+        if (k.tool_p[i] == 0.f) s.tp0 |= 1u << i;
+    return s;
+}
+
+int match_spec(const ChainSpec &s) {
+    for (int id = 1; id < SPEC_COUNT; ++id) {
+        const ChainSpec *r = registered_spec(id);
+        if (r && r->dof == s.dof && r->pris == s.pris && r->al0 == s.al0 && r->alp == s.alp && r->aln == s.aln &&
+            r->a0 == s.a0 && r->d0 == s.d0 && r->t0 == s.t0 && r->tool_rot == s.tool_rot && r->tp0 == s.tp0)
+            return id;
+    }
+    return SPEC_GENERIC;
+}
+
 } // namespace
 
 struct lm_ctx {
@@ -80,6 +110,8 @@ struct lm_ctx {
     bool fresh;
     int block;
     bool fast;
+    int spec_id;     // structure-matched specialised kernel (lm_specs.cuh) or SPEC_GENERIC
+    bool use_generic; // LM_OPT_GENERIC_KERNEL
 };
 
 extern "C" {
@@ -168,6 +200,8 @@ int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_
         k.tool_has_rot = ident ? 0u : 1u;
         for (int i = 0; i < 3; ++i) k.tool_p[i] = (float)chain->tool[i];
     }
+    c->spec_id = match_spec(chain_signature(d, k));
+    c->use_generic = false;
     a.lambda0 = prm->lambda0; a.nu_up = prm->nu_up; a.inv_nu_down = (float)(1.0 / (double)prm->nu_down);
     a.lambda_min = prm->lambda_min; a.lambda_max = prm->lambda_max; a.tol2 = prm->tol * prm->tol;
     a.w_pos = prm->w_pos; a.w_rot = prm->w_rot;
@@ -204,34 +238,14 @@ int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_
 
 namespace {
 
-template <int D>
-cudaError_t launch_iterate_d(lm_ctx *c, const KArgs &a) {
-    const unsigned grid = (unsigned)((c->W + c->block - 1) / c->block);
-    if (c->fast) lm_iterate_kernel<D, true><<<grid, c->block, 0, c->stream>>>(a);
-    else lm_iterate_kernel<D, false><<<grid, c->block, 0, c->stream>>>(a);
-    return cudaGetLastError();
-}
-
 cudaError_t launch_iterate(lm_ctx *c, const KArgs &a) {
     g_launches.fetch_add(1);
-    switch (c->dof) {
-    case 1: return launch_iterate_d<1>(c, a);
-    case 2: return launch_iterate_d<2>(c, a);
-    case 3: return launch_iterate_d<3>(c, a);
-    case 4: return launch_iterate_d<4>(c, a);
-    case 5: return launch_iterate_d<5>(c, a);
-    case 6: return launch_iterate_d<6>(c, a);
-    case 7: return launch_iterate_d<7>(c, a);
-    default: return launch_iterate_d<8>(c, a);
-    }
-}
-
-template <int D>
-cudaError_t launch_fk_d(lm_ctx *c, const KFkArgs &a) {
-    const unsigned grid = (unsigned)((a.count + 127) / 128);
-    if (c->fast) lm_fk_kernel<D, true><<<grid, 128, 0, c->stream>>>(a);
-    else lm_fk_kernel<D, false><<<grid, 128, 0, c->stream>>>(a);
-    return cudaGetLastError();
+    const unsigned grid = (unsigned)((c->W + c->block - 1) / c->block);
+    const bool weighted = a.weighted != 0;
+    if (c->spec_id != SPEC_GENERIC && !c->use_generic)
+        return launch_iterate_spec(c->spec_id, c->fast, weighted, grid, c->block, c->stream, a);
+    return c->dof <= 4 ? launch_iterate_generic_lo(c->dof, c->fast, weighted, grid, c->block, c->stream, a)
+                       : launch_iterate_generic_hi(c->dof, c->fast, weighted, grid, c->block, c->stream, a);
 }
 
 int iterate(lm_ctx *c, int max_total, int at_most) {
@@ -249,6 +263,36 @@ int iterate(lm_ctx *c, int max_total, int at_most) {
 cudaError_t copy_out(void *dst, const void *src, size_t bytes, cudaStream_t s) {
     if (!dst) return cudaSuccess;
     return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, s);
+}
+
+// One warp per trajectory: converged = AND of frozen bits, iters = MAX, total = SUM (integers only,
+// so the atomics below cannot disturb bit-stability).
+__global__ void lm_traj_stats_kernel(const uint32_t *__restrict__ its, int64_t B, int32_t n,
+                                     uint8_t *__restrict__ conv, int32_t *__restrict__ titers,
+                                     unsigned long long *__restrict__ totals) {
+    const int64_t b = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (b >= B) return;
+    uint32_t all = 1u, mx = 0u;
+    unsigned long long sum = 0ull;
+    for (int i = lane; i < n; i += 32) {
+        const uint32_t pk = its[b * n + i];
+        all &= (pk >> 8) & 1u;
+        mx = max(mx, pk & 0xffu);
+        sum += pk & 0xffu;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        all &= __shfl_xor_sync(0xffffffffu, all, o);
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    }
+    if (lane == 0) {
+        conv[b] = (uint8_t)all;
+        titers[b] = (int32_t)mx;
+        atomicAdd(totals, sum);
+        if (all) atomicAdd(totals + 1, 1ull);
+    }
 }
 
 __global__ void lm_unpack_kernel(const uint32_t *__restrict__ its, int64_t W, int32_t *__restrict__ iters,
@@ -296,12 +340,25 @@ int lm_set_trace(lm_ctx *c, float *trial_q, float *trial_F) {
     return LM_OK;
 }
 
-int lm_set_launch(lm_ctx *c, int32_t block_threads) {
+int lm_set_option(lm_ctx *c, int32_t option, int32_t value) {
     if (!c) return LM_EINVAL;
-    if (block_threads == 0) block_threads = 128;
-    if (block_threads < 32 || block_threads > 256 || (block_threads % 32) != 0) return LM_EINVAL;
-    c->block = block_threads;
-    return LM_OK;
+    switch (option) {
+    case LM_OPT_BLOCK_THREADS:
+        if (value == 0) value = 128;
+        if (value < 32 || value > 256 || (value % 32) != 0) return LM_EINVAL;
+        c->block = value;
+        return LM_OK;
+    case LM_OPT_GENERIC_KERNEL:
+        c->use_generic = value != 0;
+        return LM_OK;
+    default:
+        return LM_EINVAL;
+    }
+}
+
+const char *lm_kernel_name(lm_ctx *c) {
+    if (!c) return "";
+    return (c->spec_id != SPEC_GENERIC && !c->use_generic) ? spec_name(c->spec_id) : "generic";
 }
 
 int lm_set_state(lm_ctx *c, const float *q, const float *lambda) {
@@ -324,17 +381,10 @@ int lm_fk(lm_ctx *c, const float *q, int64_t count, float *pos, float *rot) {
     KFkArgs a;
     a.ch = c->args.ch; a.count = count; a.q = q; a.pos = pos; a.rot = rot;
     g_launches.fetch_add(1);
-    cudaError_t e;
-    switch (c->dof) {
-    case 1: e = launch_fk_d<1>(c, a); break;
-    case 2: e = launch_fk_d<2>(c, a); break;
-    case 3: e = launch_fk_d<3>(c, a); break;
-    case 4: e = launch_fk_d<4>(c, a); break;
-    case 5: e = launch_fk_d<5>(c, a); break;
-    case 6: e = launch_fk_d<6>(c, a); break;
-    case 7: e = launch_fk_d<7>(c, a); break;
-    default: e = launch_fk_d<8>(c, a); break;
-    }
+    const unsigned grid = (unsigned)((count + 127) / 128);
+    cudaError_t e = (c->spec_id != SPEC_GENERIC && !c->use_generic)
+                        ? launch_fk_spec(c->spec_id, c->fast, grid, 128, c->stream, a)
+                        : launch_fk_generic(c->dof, c->fast, grid, 128, c->stream, a);
     if (e != cudaSuccess) return cuda_fail(e);
     return LM_OK;
 }

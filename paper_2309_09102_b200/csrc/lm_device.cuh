@@ -2,10 +2,16 @@
 //
 // One THREAD owns one waypoint block: its d x d damped normal equations are independent of every
 // other waypoint (block-diagonal Jacobian), so all state lives in registers and all
-// loops over joints are unrolled at compile time (template parameter D).  Every floating-point
-// operation is written as an explicit round-to-nearest intrinsic (fmaf / __fmul_rn / __fadd_rn):
-// the compiler may neither contract nor reassociate them, so a waypoint's bits do not depend on
-// which kernel, launch geometry or batch it is evaluated in (bit-stability).
+// loops over joints are unrolled at compile time.  Every floating-point operation is written as
+// an explicit round-to-nearest intrinsic (fmaf / __fmul_rn / __fadd_rn): the compiler may neither
+// contract nor reassociate them, so a waypoint's bits do not depend on which kernel, launch
+// geometry or batch it is evaluated in (bit-stability).
+//
+// The STRUCTURE of the kinematic chain (which joints are prismatic, which link twists are 0 or
+// +-pi/2, which link offsets vanish) is a compile-time ChainSpec: for a registered robot the
+// multiplications by 0 / +-1, the offset adds and every warp-uniform branch disappear from the
+// instruction stream.  Skipping a term that is exactly zero (or multiplying by exactly +-1)
+// leaves every result unchanged, so a specialised kernel returns the same values as the generic one.
 //
 // Step names S1..S9 follow DESIGN.md section 2.
 #pragma once
@@ -16,8 +22,7 @@ namespace lmk {
 
 constexpr int MAX_DOF = 8;
 
-// Chain constants, fp32, passed by value inside the kernel parameter block (constant bank:
-// operands are read as c[0][..] without occupying registers).
+// Chain constants, fp32, passed by value inside the kernel parameter block (constant bank).
 struct KChain {
     float ca[MAX_DOF], sa[MAX_DOF];   // cos / sin alpha_{j-1}
     float a[MAX_DOF], d[MAX_DOF];     // a_{j-1}, d_j offset
@@ -29,6 +34,24 @@ struct KChain {
     uint32_t prismatic_mask;          // bit j: joint j prismatic
     uint32_t tool_has_rot;            // tool rotation != identity
 };
+
+// Compile-time structure of a chain.  generic = true: everything is decided at run time from
+// KChain (warp-uniform branches).  Otherwise the masks say, per joint j (bit j):
+struct ChainSpec {
+    bool generic;
+    int dof;
+    uint32_t pris; // prismatic
+    uint32_t al0;  // alpha == 0
+    uint32_t alp;  // alpha == +pi/2  (ca = 0, sa = +1)
+    uint32_t aln;  // alpha == -pi/2  (ca = 0, sa = -1)
+    uint32_t a0;   // a == 0
+    uint32_t d0;   // d offset == 0
+    uint32_t t0;   // theta offset == 0
+    bool tool_rot; // tool rotation != identity
+    uint32_t tp0;  // bit i: tool_p[i] == 0
+};
+
+__host__ __device__ constexpr ChainSpec generic_spec(int d) { return ChainSpec{true, d, 0, 0, 0, 0, 0, 0, 0, true, 0}; }
 
 __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
 __device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
@@ -70,7 +93,7 @@ __device__ __forceinline__ void sincos_(float x, float &s, float &c) {
 __device__ __forceinline__ float atan2_pos(float s, float c) {
     float ac = fabsf(c);
     float mx = fmaxf(s, ac), mn = fminf(s, ac);
-    float t = __fdiv_rn(mn, fmaxf(mx, 1e-37f));
+    float t = __fdividef(mn, fmaxf(mx, 1e-30f));
     float t2 = mul(t, t);
     float p = fma_(t2, 2.622244181e-03f, -1.513253432e-02f);
     p = fma_(p, t2, 4.112185538e-02f);
@@ -93,46 +116,109 @@ struct Pose {
     float F;        // r . r
 };
 
+// w = Log(E)^vee for theta within 1e-4 of pi (rare: never reached by the documented workloads).
+// Axis from the symmetric part E_ii = c + (1 - c) a_i^2, signs from E_mi + E_im and from v.
+__device__ __forceinline__ void log_near_pi(const float (&X)[3], const float (&Y)[3], const float (&Z)[3],
+                                            const float (&Rt)[3][3], const float (&v)[3], float cth, float theta,
+                                            float (&w)[3]) {
+    float E[3][3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+            E[i][k] = fma_(Z[i], Rt[2][k], fma_(Y[i], Rt[1][k], mul(X[i], Rt[0][k])));
+    const float inv = __fdividef(1.0f, sub(1.0f, cth));
+    float ax[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) ax[i] = sqrtf(fmaxf(mul(sub(E[i][i], cth), inv), 0.f));
+    int m = 0;
+    float amax = ax[0];
+    if (ax[1] > amax) { amax = ax[1]; m = 1; }
+    if (ax[2] > amax) { m = 2; }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const float sym = (m == 0) ? add(E[0][i], E[i][0]) : (m == 1) ? add(E[1][i], E[i][1]) : add(E[2][i], E[i][2]);
+        if (i != m && sym < 0.f) ax[i] = -ax[i];
+    }
+    const float dt = fma_(ax[2], v[2], fma_(ax[1], v[1], mul(ax[0], v[0])));
+    const float th = (dt < 0.f) ? -theta : theta;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) w[i] = mul(th, ax[i]);
+}
+
 // S1 + S2 + S3: serial-chain FK (modified DH, DESIGN R1), pose residual against the target
 // (p_t, R_t given as COLUMNS Rt[k] = k-th column), geometric Jacobian from the retained joint axes.
 //   A_j = Rot_x(alpha) Trans_x(a) Rot_z(theta) Trans_z(d);  frame columns X, Y, Z and origin o.
-template <int D, bool FAST>
+template <int D, bool FAST, bool WEIGHTED, typename SpecT>
 __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D], const float (&pt)[3],
                                           const float (&Rt)[3][3], float w_pos, float w_rot,
-                                          bool weighted, Pose<D> &P, float *p_out, float (*R_out)[3]) {
-    float X[3] = {1.f, 0.f, 0.f}, Y[3] = {0.f, 1.f, 0.f}, Z[3] = {0.f, 0.f, 1.f}, o[3] = {0.f, 0.f, 0.f};
+                                          Pose<D> &P, float *p_out, float (*R_out)[3]) {
+    constexpr ChainSpec S = SpecT::spec;
+    float X[3], Y[3], Z[3], o[3];
 #pragma unroll
     for (int j = 0; j < D; ++j) {
-        const bool pris = (ch.prismatic_mask >> j) & 1u; // warp-uniform (constant bank)
-        float s, c, dj;
+        const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
+        const bool al0 = !S.generic && ((S.al0 >> j) & 1u), alp = !S.generic && ((S.alp >> j) & 1u),
+                   aln = !S.generic && ((S.aln >> j) & 1u);
+        const bool a_zero = !S.generic && ((S.a0 >> j) & 1u), d_zero = !S.generic && ((S.d0 >> j) & 1u) && !pris,
+                   t_zero = !S.generic && ((S.t0 >> j) & 1u);
+        float s, c, dj = 0.f;
         if (!pris) {
-            sincos_<FAST>(add(q[j], ch.toff[j]), s, c);
-            dj = ch.d[j];
+            sincos_<FAST>(t_zero ? q[j] : add(q[j], ch.toff[j]), s, c);
+            if (!d_zero) dj = ch.d[j];
         } else {
             s = ch.sth[j];
             c = ch.cth[j];
             dj = add(ch.d[j], q[j]);
         }
         const float ca = ch.ca[j], sa = ch.sa[j], aj = ch.a[j];
+        if (j == 0) {
+            // base frame = identity: Y' = (0, ca, sa), Z' = (0, -sa, ca), o' = (a, 0, 0)
+            float y1[3], z1[3];
+            y1[0] = 0.f; z1[0] = 0.f;
+            if (al0)      { y1[1] = 1.f; y1[2] = 0.f;  z1[1] = 0.f;  z1[2] = 1.f; }
+            else if (alp) { y1[1] = 0.f; y1[2] = 1.f;  z1[1] = -1.f; z1[2] = 0.f; }
+            else if (aln) { y1[1] = 0.f; y1[2] = -1.f; z1[1] = 1.f;  z1[2] = 0.f; }
+            else          { y1[1] = ca;  y1[2] = sa;   z1[1] = -sa;  z1[2] = ca; }
+            X[0] = c;  X[1] = (al0 ? s : (alp || aln) ? 0.f : mul(s, y1[1]));  X[2] = (al0 ? 0.f : alp ? s : aln ? -s : mul(s, y1[2]));
+            Y[0] = -s; Y[1] = (al0 ? c : (alp || aln) ? 0.f : mul(c, y1[1]));  Y[2] = (al0 ? 0.f : alp ? c : aln ? -c : mul(c, y1[2]));
+            o[0] = a_zero ? 0.f : aj;
+            o[1] = (d_zero || al0) ? 0.f : mul(dj, z1[1]);
+            o[2] = d_zero ? 0.f : (al0 ? dj : (alp || aln) ? 0.f : mul(dj, z1[2]));
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { Z[i] = z1[i]; P.Jw[j][i] = z1[i]; P.Jv[j][i] = o[i]; }
+            continue;
+        }
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-            float y1 = fma_(sa, Z[i], mul(ca, Y[i]));   // Rot_x: Y' =  ca Y + sa Z
-            float z1 = fma_(ca, Z[i], mul(-sa, Y[i]));  //        Z' = -sa Y + ca Z
-            float o1 = fma_(aj, X[i], o[i]);            // Trans_x(a)
-            float x2 = fma_(s, y1, mul(c, X[i]));       // Rot_z: X'' =  c X + s Y'
-            float y2 = fma_(c, y1, mul(-s, X[i]));      //        Y'' = -s X + c Y'
-            o[i] = fma_(dj, z1, o1);                    // Trans_z(d)
+            float y1, z1;
+            if (al0)      { y1 = Y[i];  z1 = Z[i]; }                       // Rot_x(0)
+            else if (alp) { y1 = Z[i];  z1 = -Y[i]; }                      // Rot_x(+pi/2)
+            else if (aln) { y1 = -Z[i]; z1 = Y[i]; }                       // Rot_x(-pi/2)
+            else {
+                y1 = fma_(sa, Z[i], mul(ca, Y[i]));                         // Y' =  ca Y + sa Z
+                z1 = fma_(ca, Z[i], mul(-sa, Y[i]));                        // Z' = -sa Y + ca Z
+            }
+            const float o1 = a_zero ? o[i] : fma_(aj, X[i], o[i]);          // Trans_x(a)
+            const float x2 = fma_(s, y1, mul(c, X[i]));                     // Rot_z: X'' =  c X + s Y'
+            const float y2 = fma_(c, y1, mul(-s, X[i]));                    //        Y'' = -s X + c Y'
+            o[i] = d_zero ? o1 : fma_(dj, z1, o1);                          // Trans_z(d)
             X[i] = x2; Y[i] = y2; Z[i] = z1;
-            P.Jw[j][i] = z1;                            // joint axis z_j
-            P.Jv[j][i] = o[i];                          // frame origin o_j (turned into J_v below)
+            P.Jw[j][i] = z1;                                                // joint axis z_j
+            P.Jv[j][i] = o[i];                                              // frame origin o_j (-> J_v below)
         }
     }
     // flange: p = o + R tool_p ;  R_ee = R R_tool
     float p[3];
 #pragma unroll
-    for (int i = 0; i < 3; ++i)
-        p[i] = fma_(Z[i], ch.tool_p[2], fma_(Y[i], ch.tool_p[1], fma_(X[i], ch.tool_p[0], o[i])));
-    if (ch.tool_has_rot) { // warp-uniform
+    for (int i = 0; i < 3; ++i) {
+        float t = o[i];
+        if (S.generic || !(S.tp0 & 1u)) t = fma_(X[i], ch.tool_p[0], t);
+        if (S.generic || !(S.tp0 & 2u)) t = fma_(Y[i], ch.tool_p[1], t);
+        if (S.generic || !(S.tp0 & 4u)) t = fma_(Z[i], ch.tool_p[2], t);
+        p[i] = t;
+    }
+    if (S.generic ? (ch.tool_has_rot != 0) : S.tool_rot) {
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             float x = X[i], y = Y[i], z = Z[i];
@@ -170,45 +256,17 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
     for (int i = 0; i < 3; ++i) v[i] = mul(0.5f, v[i]);
     const float cth = fma_(0.5f, tr, -0.5f);
     const float s2 = fma_(v[2], v[2], fma_(v[1], v[1], mul(v[0], v[0])));
-    const float sn = __fsqrt_rn(s2);
-    float scale;
-    if (sn < 1e-4f && cth > 0.f) {
-        scale = fma_(s2, 0.166666667f, 1.0f);          // theta/s = 1 + s^2/6
-    } else {
-        scale = __fdiv_rn(atan2_pos(sn, cth), fmaxf(sn, 1e-37f));
-    }
+    const float sn = sqrtf(s2);
+    const float theta = atan2_pos(sn, cth);
+    // theta / s; the small-angle series 1 + s^2/6 takes over below s = 1e-4
+    const float scale = (sn < 1e-4f) ? fma_(s2, 0.166666667f, 1.0f) : __fdividef(theta, sn);
     float w[3] = {mul(scale, v[0]), mul(scale, v[1]), mul(scale, v[2])};
-    if (sn < 1e-4f && cth <= 0.f) {
-        // theta within 1e-4 of pi (never reached by the documented workloads): axis from the
-        // symmetric part E_ii = c + (1 - c) a_i^2, signs from E_mi + E_im and from v.
-        float E[3][3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-#pragma unroll
-            for (int k = 0; k < 3; ++k)
-                E[i][k] = fma_(Z[i], Rt[2][k], fma_(Y[i], Rt[1][k], mul(X[i], Rt[0][k])));
-        const float inv = __fdiv_rn(1.0f, sub(1.0f, cth));
-        float ax[3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) ax[i] = __fsqrt_rn(fmaxf(mul(sub(E[i][i], cth), inv), 0.f));
-        int m = 0;
-        if (ax[1] > ax[m]) m = 1;
-        if (ax[2] > ax[m]) m = 2;
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            float sym = (m == 0) ? add(E[0][i], E[i][0]) : (m == 1) ? add(E[1][i], E[i][1]) : add(E[2][i], E[i][2]);
-            if (i != m && sym < 0.f) ax[i] = -ax[i];
-        }
-        const float dt = fma_(ax[2], v[2], fma_(ax[1], v[1], mul(ax[0], v[0])));
-        const float th = (dt < 0.f) ? -atan2_pos(sn, cth) : atan2_pos(sn, cth);
-#pragma unroll
-        for (int i = 0; i < 3; ++i) w[i] = mul(th, ax[i]);
-    }
+    if (sn < 1e-4f && cth <= 0.f) log_near_pi(X, Y, Z, Rt, v, cth, theta, w);
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
-        float rp = sub(p[i], pt[i]);
-        P.r[i] = weighted ? mul(w_pos, rp) : rp;
-        P.r[3 + i] = weighted ? mul(w_rot, w[i]) : w[i];
+        const float rp = sub(p[i], pt[i]);
+        P.r[i] = WEIGHTED ? mul(w_pos, rp) : rp;
+        P.r[3 + i] = WEIGHTED ? mul(w_rot, w[i]) : w[i];
     }
     P.F = fma_(P.r[5], P.r[5], fma_(P.r[4], P.r[4], fma_(P.r[3], P.r[3],
           fma_(P.r[2], P.r[2], fma_(P.r[1], P.r[1], mul(P.r[0], P.r[0]))))));
@@ -216,10 +274,10 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
     // S3: geometric Jacobian (DESIGN R3): revolute [z x (p - o); z], prismatic [z; 0]
 #pragma unroll
     for (int j = 0; j < D; ++j) {
-        const bool pris = (ch.prismatic_mask >> j) & 1u;
+        const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
         if (!pris) {
-            float e0 = sub(p[0], P.Jv[j][0]), e1 = sub(p[1], P.Jv[j][1]), e2 = sub(p[2], P.Jv[j][2]);
-            float z0 = P.Jw[j][0], z1 = P.Jw[j][1], z2 = P.Jw[j][2];
+            const float e0 = sub(p[0], P.Jv[j][0]), e1 = sub(p[1], P.Jv[j][1]), e2 = sub(p[2], P.Jv[j][2]);
+            const float z0 = P.Jw[j][0], z1 = P.Jw[j][1], z2 = P.Jw[j][2];
             P.Jv[j][0] = fma_(z1, e2, mul(-z2, e1));
             P.Jv[j][1] = fma_(z2, e0, mul(-z0, e2));
             P.Jv[j][2] = fma_(z0, e1, mul(-z1, e0));
@@ -227,7 +285,7 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
 #pragma unroll
             for (int i = 0; i < 3; ++i) { P.Jv[j][i] = P.Jw[j][i]; P.Jw[j][i] = 0.f; }
         }
-        if (weighted) {
+        if (WEIGHTED) {
 #pragma unroll
             for (int i = 0; i < 3; ++i) { P.Jv[j][i] = mul(w_pos, P.Jv[j][i]); P.Jw[j][i] = mul(w_rot, P.Jw[j][i]); }
         }
@@ -278,8 +336,9 @@ __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine
 #pragma unroll
     for (int i = 0; i < D; ++i) {
 #pragma unroll
-        for (int j = 0; j <= i; ++j) L[i][j] = coldot<D>(P, i, j);
-        L[i][i] = add(L[i][i], lam);
+        for (int j = 0; j < i; ++j) L[i][j] = coldot<D>(P, i, j);
+        L[i][i] = fma_(P.Jw[i][2], P.Jw[i][2], fma_(P.Jw[i][1], P.Jw[i][1], fma_(P.Jw[i][0], P.Jw[i][0],
+                  fma_(P.Jv[i][2], P.Jv[i][2], fma_(P.Jv[i][1], P.Jv[i][1], fma_(P.Jv[i][0], P.Jv[i][0], lam))))));
         g[i] = -colvec<D>(P, i, P.r);
     }
     bool ok = true;
@@ -287,7 +346,7 @@ __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine
     for (int k = 0; k < D; ++k) {
         const float piv = L[k][k];
         ok = ok && (piv > 0.f);
-        const float id = rsqrtf(piv);
+        const float id = rsqrtf(piv);   // MUFU.RSQ (built with -ftz=true); pivots are >= ~lambda_min
         invd[k] = id;
 #pragma unroll
         for (int i = k + 1; i < D; ++i) L[i][k] = mul(L[i][k], id);

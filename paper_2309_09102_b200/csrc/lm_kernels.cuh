@@ -33,7 +33,7 @@ struct KArgs {
 __device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z, float (&Rt)[3][3]) {
     // DESIGN R11: re-normalise, then the textbook conversion; Rt[k] = k-th COLUMN of R_t
     const float n2 = fma_(z, z, fma_(y, y, fma_(x, x, mul(w, w))));
-    const float inv = __fdiv_rn(1.0f, __fsqrt_rn(n2));
+    const float inv = rsqrtf(n2);
     w = mul(w, inv); x = mul(x, inv); y = mul(y, inv); z = mul(z, inv);
     const float xx = mul(x, x), yy = mul(y, y), zz = mul(z, z);
     const float xy = mul(x, y), xz = mul(x, z), yz = mul(y, z);
@@ -43,7 +43,7 @@ __device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z,
     Rt[0][2] = mul(2.f, sub(xz, wy));        Rt[1][2] = mul(2.f, add(yz, wx));        Rt[2][2] = fma_(-2.f, add(xx, yy), 1.f);
 }
 
-template <int D, bool FAST>
+template <int D, bool FAST, bool WEIGHTED, typename SpecT>
 __global__ void __launch_bounds__(256) lm_iterate_kernel(const __grid_constant__ KArgs A) {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = w < A.W;
@@ -76,10 +76,8 @@ __global__ void __launch_bounds__(256) lm_iterate_kernel(const __grid_constant__
         for (int i = 0; i < 3; ++i) pt[i] = __ldg(A.tp + (int64_t)i * Wt + wt);
         quat_to_cols(__ldg(A.tq + wt), __ldg(A.tq + Wt + wt), __ldg(A.tq + 2 * Wt + wt), __ldg(A.tq + 3 * Wt + wt), Rt);
     }
-    const bool weighted = A.weighted != 0;
-
     Pose<D> cur;
-    eval_pose<D, FAST>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, weighted, cur, nullptr, nullptr);
+    eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, cur, nullptr, nullptr);
 
     // ---- S3..S9: the LM loop, entirely on the device.  A lane is `active` while it is not
     // frozen and has iterations left; the warp leaves the loop when no lane is active.
@@ -99,7 +97,7 @@ __global__ void __launch_bounds__(256) lm_iterate_kernel(const __grid_constant__
             clamped = clamped || (qt[j] != t);
         }
         Pose<D> tri;
-        eval_pose<D, FAST>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, weighted, tri, nullptr, nullptr); // S7
+        eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, tri, nullptr, nullptr); // S7
 
         if (A.trace_q != nullptr && active && live) {
 #pragma unroll
@@ -144,9 +142,9 @@ __global__ void __launch_bounds__(256) lm_iterate_kernel(const __grid_constant__
     A.lam[w] = lam;
     A.its[w] = k | (st << 8);
     A.mask[w] = mask;
-    A.res[w] = __fsqrt_rn(cur.F);
-    A.perr[w] = mul(__fsqrt_rn(fma_(cur.r[2], cur.r[2], fma_(cur.r[1], cur.r[1], mul(cur.r[0], cur.r[0])))), A.inv_w_pos);
-    A.rerr[w] = mul(__fsqrt_rn(fma_(cur.r[5], cur.r[5], fma_(cur.r[4], cur.r[4], mul(cur.r[3], cur.r[3])))), A.inv_w_rot);
+    A.res[w] = sqrtf(cur.F);
+    A.perr[w] = mul(sqrtf(fma_(cur.r[2], cur.r[2], fma_(cur.r[1], cur.r[1], mul(cur.r[0], cur.r[0])))), A.inv_w_pos);
+    A.rerr[w] = mul(sqrtf(fma_(cur.r[5], cur.r[5], fma_(cur.r[4], cur.r[4], mul(cur.r[3], cur.r[3])))), A.inv_w_rot);
 }
 
 struct KFkArgs {
@@ -156,7 +154,7 @@ struct KFkArgs {
     float *pos, *rot;
 };
 
-template <int D, bool FAST>
+template <int D, bool FAST, typename SpecT>
 __global__ void __launch_bounds__(256) lm_fk_kernel(const __grid_constant__ KFkArgs A) {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (w >= A.count) return;
@@ -167,7 +165,7 @@ __global__ void __launch_bounds__(256) lm_fk_kernel(const __grid_constant__ KFkA
     const float Rt[3][3] = {{1.f, 0.f, 0.f}, {0.f, 1.f, 0.f}, {0.f, 0.f, 1.f}};
     Pose<D> P;
     float p[3], R[3][3];
-    eval_pose<D, FAST>(A.ch, q, pt, Rt, 1.f, 1.f, false, P, p, R);
+    eval_pose<D, FAST, false, SpecT>(A.ch, q, pt, Rt, 1.f, 1.f, P, p, R);
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         A.pos[(int64_t)i * A.count + w] = p[i];
@@ -176,34 +174,7 @@ __global__ void __launch_bounds__(256) lm_fk_kernel(const __grid_constant__ KFkA
     }
 }
 
-// One warp per trajectory: converged = AND of frozen bits, iters = MAX, total = SUM (integers only,
-// so the atomics below cannot disturb bit-stability).
-__global__ void lm_traj_stats_kernel(const uint32_t *__restrict__ its, int64_t B, int32_t n,
-                                     uint8_t *__restrict__ conv, int32_t *__restrict__ titers,
-                                     unsigned long long *__restrict__ totals) {
-    const int64_t b = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
-    if (b >= B) return;
-    uint32_t all = 1u, mx = 0u;
-    unsigned long long sum = 0ull;
-    for (int i = lane; i < n; i += 32) {
-        const uint32_t pk = its[b * n + i];
-        all &= (pk >> 8) & 1u;
-        mx = max(mx, pk & 0xffu);
-        sum += pk & 0xffu;
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        all &= __shfl_xor_sync(0xffffffffu, all, o);
-        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-        sum += __shfl_xor_sync(0xffffffffu, sum, o);
-    }
-    if (lane == 0) {
-        conv[b] = (uint8_t)all;
-        titers[b] = (int32_t)mx;
-        atomicAdd(totals, sum);
-        if (all) atomicAdd(totals + 1, 1ull);
-    }
-}
+template <int D>
+struct GenericSpec { static constexpr ChainSpec spec = generic_spec(D); };
 
 } // namespace lmk

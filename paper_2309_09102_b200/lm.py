@@ -22,11 +22,12 @@ LM_MAX_DOF = 8
 LM_MAX_ITERS = 64
 LM_OK, LM_EINVAL, LM_ENOMEM, LM_ECUDA = 0, -1, -2, -3
 LM_MEM_DEVICE, LM_MEM_HOST = 0, 1
+LM_OPT_BLOCK_THREADS, LM_OPT_GENERIC_KERNEL = 1, 2
 LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1, 2, 4, 8, 16
 
 # every symbol include/lm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_run", "lm_fetch",
-           "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_launch", "lm_fk", "lm_free",
+           "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_option", "lm_kernel_name", "lm_fk", "lm_free",
            "lm_strerror", "lm_launch_count")
 
 
@@ -83,7 +84,9 @@ def lib() -> C.CDLL:
         L.lm_reset.argtypes = [C.c_void_p]
         L.lm_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.lm_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
-        L.lm_set_launch.argtypes = [C.c_void_p, C.c_int32]
+        L.lm_set_option.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        L.lm_kernel_name.argtypes = [C.c_void_p]
+        L.lm_kernel_name.restype = C.c_char_p
         L.lm_fk.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
         L.lm_free.argtypes = [C.c_void_p]
         L.lm_free.restype = None
@@ -173,8 +176,12 @@ def lm_set_trace(ctx: int, trial_q_ptr: Optional[int], trial_F_ptr: Optional[int
     _check(lib().lm_set_trace(ctx, trial_q_ptr, trial_F_ptr), "lm_set_trace")
 
 
-def lm_set_launch(ctx: int, block_threads: int) -> None:
-    _check(lib().lm_set_launch(ctx, int(block_threads)), "lm_set_launch")
+def lm_set_option(ctx: int, option: int, value: int) -> None:
+    _check(lib().lm_set_option(ctx, int(option), int(value)), "lm_set_option")
+
+
+def lm_kernel_name(ctx: int) -> str:
+    return lib().lm_kernel_name(ctx).decode()
 
 
 def lm_fk(ctx: int, q_ptr: int, count: int, pos_ptr: int, rot_ptr: int) -> None:
@@ -240,7 +247,14 @@ class Solver:
         lm_reset(self._ctx)
 
     def set_launch(self, block_threads: int) -> None:
-        lm_set_launch(self._ctx, block_threads)
+        lm_set_option(self._ctx, LM_OPT_BLOCK_THREADS, block_threads)
+
+    def use_generic_kernel(self, on: bool = True) -> None:
+        lm_set_option(self._ctx, LM_OPT_GENERIC_KERNEL, int(on))
+
+    @property
+    def kernel_name(self) -> str:
+        return lm_kernel_name(self._ctx)
 
     def set_state(self, q, lam=None) -> None:
         """q [W,d], lam [W] numpy (waypoint-major)."""

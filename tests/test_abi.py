@@ -95,7 +95,12 @@ def test_init_validation_without_gpu(L):
     rc, ctx = init()
     assert rc == lm.LM_OK and ctx.value
     assert L.lm_run(ctx, 65) == lm.LM_EINVAL and L.lm_run(ctx, -1) == lm.LM_EINVAL
-    assert L.lm_set_launch(ctx, 48) == lm.LM_EINVAL and L.lm_set_launch(ctx, 64) == lm.LM_OK
+    assert L.lm_set_option(ctx, lm.LM_OPT_BLOCK_THREADS, 48) == lm.LM_EINVAL
+    assert L.lm_set_option(ctx, lm.LM_OPT_BLOCK_THREADS, 64) == lm.LM_OK
+    assert L.lm_set_option(ctx, 77, 1) == lm.LM_EINVAL
+    # the Panda table's structure is registered: a specialised kernel is selected at lm_init
+    assert L.lm_kernel_name(ctx) == b"panda7"
+    assert L.lm_set_option(ctx, lm.LM_OPT_GENERIC_KERNEL, 1) == lm.LM_OK and L.lm_kernel_name(ctx) == b"generic"
     L.lm_free(ctx)
 
 

@@ -217,10 +217,44 @@ def test_api_errors_on_device(lm, w_small):
     with pytest.raises(lm.LmError):
         lm.lm_run(s._ctx, 65)
     with pytest.raises(lm.LmError):
-        lm.lm_set_launch(s._ctx, 40)
+        lm.lm_set_option(s._ctx, lm.LM_OPT_BLOCK_THREADS, 40)
+    with pytest.raises(lm.LmError):
+        lm.lm_set_option(s._ctx, 99, 1)
     with pytest.raises(lm.LmError):
         lm.lm_fk(s._ctx, 0, 10, 0, 0)
     n0 = lm.lm_launch_count()
     s.run(3)
     assert lm.lm_launch_count() == n0 + 1   # the whole LM loop is ONE launch
     s.close()
+
+
+def test_specialised_kernels_equal_generic(lm):
+    """Chains whose structure is registered in csrc/lm_specs.cuh run a compile-time specialised
+    kernel; it must return the generic kernel's values (only multiplications by exact 0 / +-1 and
+    additions of exact 0 are removed; the sign of a zero may differ, nothing else)."""
+    cases = [("panda7", wl.config2(H.oracle_fk(wl.panda_chain()), B=5, n=131)),
+             ("rand8", wl.config3(H.oracle_fk(wl.random_chain_8dof(3)), B=5, n=131)),
+             ("panda7", wl.config4(H.oracle_fk(wl.panda_chain()), B=5, n=131))]
+    for name, w in cases:
+        s = H.make_solver(w)
+        assert s.kernel_name == name
+        s.run(w.max_iters)
+        a = s.fetch()
+        s.use_generic_kernel(True)
+        assert s.kernel_name == "generic"
+        s.reset()
+        s.run(w.max_iters)
+        b = s.fetch()
+        s.close()
+        for k in ("q", "res_norm", "lam"):
+            assert np.array_equal(a[k], b[k]), (name, k)   # value equality (+0 == -0)
+        for k in ("iters", "mask", "status"):
+            assert np.array_equal(a[k], b[k]), (name, k)
+    # anything else runs the generic kernel: other robots, a rotated tool, a theta offset
+    other = wl.panda_chain()
+    other.theta = other.theta + np.array([0, 0, 0.1, 0, 0, 0, 0])
+    s = H.make_solver(wl.Workload("o", other, 1, 4, cases[0][1].target_pos[:4], cases[0][1].target_quat[:4],
+                                  cases[0][1].seeds[:4], 0.0, 2))
+    assert s.kernel_name == "generic"
+    s.close()
+    assert H.make_solver(wl.config3(H.oracle_fk(wl.random_chain_8dof(5)), B=1, n=4)).kernel_name == "generic"
