@@ -43,8 +43,15 @@ __device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z,
     Rt[0][2] = mul(2.f, sub(xz, wy));        Rt[1][2] = mul(2.f, add(yz, wx));        Rt[2][2] = fma_(-2.f, add(xx, yy), 1.f);
 }
 
+#ifndef LM_MAX_THREADS
+#define LM_MAX_THREADS 256
+#endif
+#ifndef LM_MIN_BLOCKS
+#define LM_MIN_BLOCKS 1
+#endif
+
 template <int D, bool FAST, bool WEIGHTED, typename SpecT>
-__global__ void __launch_bounds__(256) lm_iterate_kernel(const __grid_constant__ KArgs A) {
+__global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kernel(const __grid_constant__ KArgs A) {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = w < A.W;
     const int64_t wc = live ? w : A.W - 1; // tail lanes shadow the last waypoint, never store
