@@ -37,6 +37,9 @@ UNIT = "waypoint-iterations/s"
 ALG_FLOP = {7: 1459.0, 8: 1762.0}
 # FP32 FMA-pipe peak derived from the guide's unit counts and clocks: 148 SMs x 128 lanes x 2 x f_max
 SM_COUNT, FP32_LANES = 148, 128
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/r1_lm_iterate_full.md); keyed by (workload, kernel variant).
+NCU_DRAM_TRAFFIC = {("C4", "panda7"): 68.864e6 + 27.270e6}
 
 
 def load_peaks() -> dict:
@@ -295,9 +298,13 @@ def run_gpu(args) -> None:
     peak_tf = SM_COUNT * FP32_LANES * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     achieved_tf = flop / (ms_kernel * 1e-3) / 1e12
     hbm_bytes = alg_bytes_per_waypoint(d) * w.W
+    fma_tf = lm.lm_fp32_peak(int(stream.cuda_stream))
+    full_size = (args.B is None and args.n is None)
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": achieved_tf / peak_tf, "traffic": None,
-                "kernel": f"lm_iterate_kernel<{d}>", "kernel_ms": ms_kernel,
+                "frac": achieved_tf / peak_tf,
+                "traffic": NCU_DRAM_TRAFFIC.get((args.workload, solver.kernel_name)) if full_size else None,
+                "kernel": f"lm_iterate_kernel<{d}, {solver.kernel_name}>", "kernel_ms": ms_kernel,
+                "peak_measured_fma": fma_tf, "frac_of_measured_fma": achieved_tf / fma_tf if fma_tf > 0 else None,
                 "alg_flop_per_waypoint_iteration": ALG_FLOP.get(d),
                 "peak_how": f"derived: {SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz "
                             f"(sm_max_mhz {peaks['_source']})",
@@ -308,7 +315,11 @@ def run_gpu(args) -> None:
     cpu = time_oracle(make_workload(args.workload, fk, ref_traj, w.n), ref_traj)
     cfg = workload_desc(w)
     cfg.update({"parallelism": f"dp{world} (independent batches, no collective)", "l2": "flushed between steps (256 MiB write)",
-                "block_threads": args.block or 128})
+                "block_threads": args.block or 128, "kernel": solver.kernel_name})
+    extra = {}
+    if args.workload == "C4" and full_size:
+        # the "to convergence" statistic of the metric, on BASELINE.json configs[1] (512 x 300, tol 1e-5)
+        extra["to_convergence_C2"] = time_to_convergence(lm, torch, wl, fk, device, stream)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms_all / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
@@ -320,7 +331,34 @@ def run_gpu(args) -> None:
                     "ms_per_step": e2e_ms_all / e2e["steps"], "how": "lm_init(LM_MEM_HOST, pinned) + lm_run + lm_fetch(host q, |r|, iters, status)"},
             "roofline": roofline,
             "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}}
+    line.update(extra)
     print(json.dumps(line))
+
+
+def time_to_convergence(lm, torch, wl, fk, device, stream, reps: int = 20) -> dict:
+    """Trajectories/s to convergence on configs[1] (512 x 300, Panda, |r| < 1e-5 or 50 iterations):
+    median CUDA-event time of lm_reset + lm_run over `reps` launches after 3 warm-ups."""
+    w = wl.config2(fk)
+    prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol)
+    s = lm.Solver(w.chain, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, device=str(device), stream=stream)
+    ts = []
+    with torch.cuda.stream(stream):
+        for i in range(reps + 3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s.reset()
+            a.record(stream)
+            s.run(w.max_iters)
+            b.record(stream)
+            stream.synchronize()
+            if i >= 3:
+                ts.append(a.elapsed_time(b))
+        iters, conv = s.fetch_totals()
+    s.close()
+    ms = float(np.median(ts))
+    return {"workload": f"C2: {w.B} x {w.n}, tol={w.tol:g}, max_iters={w.max_iters}", "ms": ms,
+            "trajectories_per_sec": w.B / (ms * 1e-3), "converged_trajectories": conv,
+            "waypoint_iterations": iters, "waypoint_iterations_per_sec": iters / (ms * 1e-3),
+            "mean_iterations_per_waypoint": iters / w.W}
 
 
 def measure_e2e(lm, torch, chain, w, prm, device, steps: int) -> dict:

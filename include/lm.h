@@ -157,6 +157,11 @@ const char *lm_kernel_name(lm_ctx *ctx);
  * q [d][count] -> pos [3][count], rot [9][count] (row-major R, SoA).  Device pointers.  Async. */
 int lm_fk(lm_ctx *ctx, const float *q, int64_t count, float *pos, float *rot);
 
+/* Measure the FP32 FMA throughput of the current device with an FMA-only micro-kernel (16 independent
+ * chains per thread, best of 5 timed launches, CUDA events on `cuda_stream`); blocks the host.
+ * tflops_out: 2 * FFMA / s / 1e12.  The measured counterpart of the ALU roofline. */
+int lm_fp32_peak(void *cuda_stream, double *tflops_out);
+
 void lm_free(lm_ctx *ctx);
 
 /* Static string for a status code; for LM_ECUDA the last CUDA error string seen by this thread. */

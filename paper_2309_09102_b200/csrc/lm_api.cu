@@ -295,6 +295,22 @@ __global__ void lm_traj_stats_kernel(const uint32_t *__restrict__ its, int64_t B
     }
 }
 
+// FP32 FMA-pipe ceiling of this device, measured: 16 independent FFMA chains per thread, nothing
+// else in the loop.  Used by bench.py as the measured counterpart of the derived ALU peak.
+__global__ void __launch_bounds__(256) lm_fma_peak_kernel(float *out, int iters, float a, float b) {
+    float x[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = (float)(threadIdx.x + i) * 1e-3f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = __fmaf_rn(x[i], a, b);
+    }
+    float sum = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) sum += x[i];
+    if (sum == 12345.678f) out[0] = sum; // never true: keeps the chains alive
+}
+
 __global__ void lm_unpack_kernel(const uint32_t *__restrict__ its, int64_t W, int32_t *__restrict__ iters,
                                  uint32_t *__restrict__ status) {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -438,6 +454,38 @@ int lm_fetch(lm_ctx *c, float *q_out, lm_stats *s) {
         return LM_OK;
     }
     LM_CUDA(cudaStreamSynchronize(c->stream));
+    return LM_OK;
+}
+
+int lm_fp32_peak(void *cuda_stream, double *tflops_out) {
+    if (!tflops_out) return LM_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int dev = 0, sms = 0;
+    LM_CUDA(cudaGetDevice(&dev));
+    LM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float *scratch = nullptr;
+    LM_CUDA(cudaMalloc(&scratch, 256));
+    cudaEvent_t e0, e1;
+    LM_CUDA(cudaEventCreate(&e0));
+    LM_CUDA(cudaEventCreate(&e1));
+    const int iters = 32768, blocks = sms * 8, threads = 256;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0, st);
+        g_launches.fetch_add(1);
+        lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(scratch, iters, 0.999f, 1e-3f);
+        cudaEventRecord(e1, st);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaFree(scratch); return cuda_fail(e); }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * 16.0 * iters * (double)blocks * threads / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(scratch);
+    *tflops_out = best;
     return LM_OK;
 }
 

@@ -27,7 +27,7 @@ LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1
 
 # every symbol include/lm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_run", "lm_fetch",
-           "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_option", "lm_kernel_name", "lm_fk", "lm_free",
+           "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_option", "lm_kernel_name", "lm_fk", "lm_fp32_peak", "lm_free",
            "lm_strerror", "lm_launch_count")
 
 
@@ -88,6 +88,7 @@ def lib() -> C.CDLL:
         L.lm_kernel_name.argtypes = [C.c_void_p]
         L.lm_kernel_name.restype = C.c_char_p
         L.lm_fk.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+        L.lm_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.lm_free.argtypes = [C.c_void_p]
         L.lm_free.restype = None
         L.lm_strerror.argtypes = [C.c_int]
@@ -186,6 +187,12 @@ def lm_kernel_name(ctx: int) -> str:
 
 def lm_fk(ctx: int, q_ptr: int, count: int, pos_ptr: int, rot_ptr: int) -> None:
     _check(lib().lm_fk(ctx, q_ptr, int(count), pos_ptr, rot_ptr), "lm_fk")
+
+
+def lm_fp32_peak(cuda_stream: int = 0) -> float:
+    out = C.c_double(0.0)
+    _check(lib().lm_fp32_peak(C.c_void_p(cuda_stream), C.byref(out)), "lm_fp32_peak")
+    return float(out.value)
 
 
 def lm_free(ctx: int) -> None:
