@@ -19,18 +19,19 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "lm_oracle.c")
 _HDR = os.path.join(_HERE, "lm_oracle.h")
+_SRCS = [_SRC, os.path.join(_HERE, "lm_traj_oracle.c")]   # one shared object: pose LM + trajectory-level LM
+_DEPS = _SRCS + [_HDR, os.path.join(_HERE, "lm_traj_oracle.h")]
 _LIB = os.path.join(_HERE, "liblm_oracle.so")
 MAX_DOF = 8
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (plain C11 + OpenMP for the timing leg)."""
-    stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < max(
-        os.path.getmtime(_SRC), os.path.getmtime(_HDR))
+    stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < max(os.path.getmtime(p) for p in _DEPS)
     if force or stale:
         tmp = _LIB + f".tmp{os.getpid()}"
         subprocess.check_call(["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-fPIC", "-fopenmp",
-                               "-shared", _SRC, "-o", tmp, "-lm"])
+                               "-shared"] + _SRCS + ["-o", tmp, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
