@@ -157,10 +157,86 @@ const char *lm_kernel_name(lm_ctx *ctx);
  * q [d][count] -> pos [3][count], rot [9][count] (row-major R, SoA).  Device pointers.  Async. */
 int lm_fk(lm_ctx *ctx, const float *q, int64_t count, float *pos, float *rot);
 
+/* ------------------------------------------------------------------------------------------------
+ * Trajectory-level LM step: the paper's trajectory-length term.
+ *
+ * Residual of ONE trajectory (Fig. 6):
+ *     r = [ w_pose * r_pose ; w_diff * (q_2 - q_1, ..., q_n - q_{n-1}) ]
+ * with Jacobian blocks J_i (kinematic Jacobian) on the pose rows of waypoint i and
+ * -I (for q_k), +I (for q_{k+1}) on the differencing rows.  The LM update
+ * (J^T J + lambda I) delta = -J^T r then has, per trajectory, the block-tridiagonal matrix
+ *     diag blocks  w_pose^2 J_i^T J_i + (c_i w_diff^2 + lambda) I   (c_i = 1 at the ends, 2 inside),
+ *     off-diagonal blocks  -w_diff^2 I,
+ * which is solved keeping that block structure (block elimination along the waypoint index, one
+ * thread per trajectory, d x d blocks in registers) plus `refine_steps` steps of iterative
+ * refinement with the residual formed from J, never from J^T J (DESIGN R4 / T4).  lambda, the
+ * accept/reject decision (strict decrease of |r|^2 at the clamped trial point) and
+ * the iteration count are per TRAJECTORY (DESIGN T3).  w_pose = 0 gives the paper's
+ * trajectory-length step on its own; w_diff = 0 reduces to B*n independent pose blocks sharing
+ * one lambda per trajectory.
+ *
+ * The step works on the context's CURRENT joint values (after lm_run / lm_set_state) and writes
+ * the result back into them, so lm_run and lm_traj_run can be alternated.
+ */
+typedef struct {
+    float w_pose, w_diff; /* 1 and 1 (the paper gives no weights: DESIGN T1) */
+    float lambda0;        /* 1e-3 */
+    float nu_up, nu_down; /* 10, 10 */
+    float lambda_min;     /* 1e-4 */
+    float lambda_max;     /* 1e7 */
+    int32_t refine_steps; /* 0..2, default 1 */
+} lm_traj_params;
+
+/* lm_traj_fetch outputs; every pointer nullable, device or host. */
+typedef struct {
+    float *cost;           /* [B] |r|^2 = w_pose^2 cost_pose + w_diff^2 cost_diff at the current q */
+    float *cost_pose;      /* [B] sum_i |r_pose,i|^2 (pose weights w_pos / w_rot applied, w_pose not) */
+    float *cost_diff;      /* [B] sum_k |q_{k+1} - q_k|^2: the trajectory-length surrogate of PAPER.md:L123 */
+    float *lambda;         /* [B] */
+    int32_t *iters;        /* [B] trajectory-level iterations executed since lm_traj_attach / lm_traj_reset */
+    uint64_t *accept_mask; /* [B] bit k = iteration k accepted */
+    uint32_t *status;      /* [B] LM_ST_MAXITER | LM_ST_BREAKDOWN | LM_ST_NONFINITE | LM_ST_CLAMPED */
+    int64_t total_traj_iters; /* OUT: sum of iters */
+} lm_traj_stats;
+
+/* Device scratch for the trajectory-level step of a (dof, B, n) problem. */
+size_t lm_traj_workspace_bytes(int32_t dof, int64_t B, int64_t n);
+
+int lm_traj_default_params(lm_traj_params *out);
+
+/* Bind a caller-owned device workspace (256-byte aligned, >= lm_traj_workspace_bytes, borrowed until
+ * lm_free) and the parameters; lambda := lambda0, iters := 0 for every trajectory.  Async. */
+int lm_traj_attach(lm_ctx *ctx, const lm_traj_params *params, void *workspace, size_t workspace_bytes);
+
+/* `iters` (1..64 in total per trajectory since the last attach / reset) more trajectory-level LM
+ * iterations from the context's current joint values; the result replaces them.  The per-waypoint
+ * state of lm_run (lambda, iteration count, accept mask) is left as it is; |r|, the pose errors and
+ * the frozen flag reported by lm_fetch are re-evaluated at the new joint values.  Kernel launches only,
+ * no host round trip; async.  lm_traj_run(N) and N calls of lm_traj_run(1) give identical bits. */
+int lm_traj_run(lm_ctx *ctx, int32_t iters);
+
+/* lambda [B] := the given values (device or host; NULL = lambda0); iters, masks, status := 0.  Async. */
+int lm_traj_reset(lm_ctx *ctx, const float *lambda);
+
+/* Synchronise the stream and copy out the per-trajectory state of the trajectory-level step. */
+int lm_traj_fetch(lm_ctx *ctx, lm_traj_stats *stats_out);
+
+/* Debug trace (device pointers, nullable, borrowed): every executed iteration overwrites
+ * trial_q [d][W] (w-order) = the clamped trial point and trial_F [2][B] = (|r|^2 before, at the trial point). */
+int lm_traj_set_trace(lm_ctx *ctx, float *trial_q, float *trial_F);
+
 /* Measure the FP32 FMA throughput of the current device with an FMA-only micro-kernel (16 independent
  * chains per thread, best of 5 timed launches, CUDA events on `cuda_stream`); blocks the host.
  * tflops_out: 2 * FFMA / s / 1e12.  The measured counterpart of the ALU roofline. */
 int lm_fp32_peak(void *cuda_stream, double *tflops_out);
+
+/* The same measurement for one operand form of FFMA: LM_FMA_FORM_RCC = one register operand, the
+ * other two from the constant bank (what lm_fp32_peak reports: the pipe's ceiling), LM_FMA_FORM_RRR =
+ * three distinct register operands (what dense in-register linear algebra issues; register-file
+ * read bandwidth limits it well below the pipe's ceiling on sm_100a). */
+#define LM_FMA_FORM_RCC 0
+#define LM_FMA_FORM_RRR 1
+int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out);
 
 void lm_free(lm_ctx *ctx);
 

@@ -1,9 +1,8 @@
 // lm_api.cu -- C ABI of include/lm.h: validation, workspace carving, launches.  No torch types,
 // no CPU compute path: every step of the hot path runs in the kernels of lm_kernels.cuh.
-#include "../../include/lm.h"
+#include "lm_ctx.h"
 #include "lm_launch.h"
 
-#include <atomic>
 #include <climits>
 #include <cmath>
 #include <cstdio>
@@ -16,23 +15,6 @@ namespace {
 
 thread_local char g_cuda_err[256] = "no CUDA error recorded";
 std::atomic<long long> g_launches{0};
-
-int cuda_fail(cudaError_t e) {
-    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
-    return LM_ECUDA;
-}
-#define LM_CUDA(x)                                 \
-    do {                                           \
-        cudaError_t e_ = (x);                      \
-        if (e_ != cudaSuccess) return cuda_fail(e_); \
-    } while (0)
-
-inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
-inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
-
-struct Layout { // byte offsets into the workspace
-    size_t q, lam, res, perr, rerr, its, mask, ui, us, conv, titers, totals, s_seeds, s_tp, s_tq, total;
-};
 
 Layout make_layout(int dof, int64_t B, int64_t n, int shared, int memory) {
     const size_t W = (size_t)B * (size_t)n, Wt = shared ? (size_t)n : W;
@@ -99,20 +81,13 @@ int match_spec(const ChainSpec &s) {
 
 } // namespace
 
-struct lm_ctx {
-    int dof;
-    int64_t B, n, W;
-    int shared;
-    KArgs args; // template for every launch
-    Layout lay;
-    char *ws;
-    cudaStream_t stream;
-    bool fresh;
-    int block;
-    bool fast;
-    int spec_id;     // structure-matched specialised kernel (lm_specs.cuh) or SPEC_GENERIC
-    bool use_generic; // LM_OPT_GENERIC_KERNEL
-};
+namespace lmk {
+int cuda_fail(cudaError_t e) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    return LM_ECUDA;
+}
+std::atomic<long long> &launch_counter() { return g_launches; }
+} // namespace lmk
 
 extern "C" {
 
@@ -259,6 +234,15 @@ int iterate(lm_ctx *c, int max_total, int at_most) {
     return LM_OK;
 }
 
+} // namespace
+
+namespace lmk {
+int materialize_state(lm_ctx *c) { return c->fresh ? iterate(c, 0, 0) : LM_OK; }
+int refresh_waypoint_outputs(lm_ctx *c) { return iterate(c, LM_MAX_ITERS, 0); }
+} // namespace lmk
+
+namespace {
+
 // copy `bytes` from a device workspace array to a device-or-host destination (UVA decides)
 cudaError_t copy_out(void *dst, const void *src, size_t bytes, cudaStream_t s) {
     if (!dst) return cudaSuccess;
@@ -309,6 +293,26 @@ __global__ void __launch_bounds__(256) lm_fma_peak_kernel(float *out, int iters,
 #pragma unroll
     for (int i = 0; i < 16; ++i) sum += x[i];
     if (sum == 12345.678f) out[0] = sum; // never true: keeps the chains alive
+}
+
+// The same with three distinct REGISTER operands per FFMA (x = x * y + z), the form dense
+// in-register linear algebra issues: limited by register-file read bandwidth, not by the FMA pipe.
+__global__ void __launch_bounds__(256) lm_fma_rrr_kernel(float *out, int iters, const float *in) {
+    float x[16], y[16], z[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        x[i] = (float)(threadIdx.x + i) * 1e-3f;
+        y[i] = in[i];
+        z[i] = in[16 + i];
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = __fmaf_rn(x[i], y[i], z[i]);
+    }
+    float sum = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) sum += x[i];
+    if (sum == 12345.678f) out[0] = sum;
 }
 
 __global__ void lm_unpack_kernel(const uint32_t *__restrict__ its, int64_t W, int32_t *__restrict__ iters,
@@ -457,14 +461,22 @@ int lm_fetch(lm_ctx *c, float *q_out, lm_stats *s) {
     return LM_OK;
 }
 
-int lm_fp32_peak(void *cuda_stream, double *tflops_out) {
-    if (!tflops_out) return LM_EINVAL;
+int lm_fp32_peak(void *cuda_stream, double *tflops_out) { return lm_fp32_peak_form(cuda_stream, LM_FMA_FORM_RCC, tflops_out); }
+
+int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out) {
+    if (!tflops_out || (form != LM_FMA_FORM_RCC && form != LM_FMA_FORM_RRR)) return LM_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int dev = 0, sms = 0;
     LM_CUDA(cudaGetDevice(&dev));
     LM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     float *scratch = nullptr;
     LM_CUDA(cudaMalloc(&scratch, 256));
+    {
+        float h[64];
+        for (int i = 0; i < 64; ++i) h[i] = (i < 16 || i >= 32) ? 0.999f : 1e-3f; // y = 0.999, z = 1e-3
+        for (int i = 16; i < 32; ++i) h[i] = 1e-3f;
+        LM_CUDA(cudaMemcpy(scratch, h, sizeof(h), cudaMemcpyHostToDevice));
+    }
     cudaEvent_t e0, e1;
     LM_CUDA(cudaEventCreate(&e0));
     LM_CUDA(cudaEventCreate(&e1));
@@ -473,7 +485,8 @@ int lm_fp32_peak(void *cuda_stream, double *tflops_out) {
     for (int rep = 0; rep < 6; ++rep) {
         cudaEventRecord(e0, st);
         g_launches.fetch_add(1);
-        lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(scratch, iters, 0.999f, 1e-3f);
+        if (form == LM_FMA_FORM_RCC) lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(scratch + 32, iters, 0.999f, 1e-3f);
+        else lm_fma_rrr_kernel<<<blocks, threads, 0, st>>>(scratch + 32, iters, scratch);
         cudaEventRecord(e1, st);
         cudaError_t e = cudaEventSynchronize(e1);
         if (e != cudaSuccess) { cudaFree(scratch); return cuda_fail(e); }

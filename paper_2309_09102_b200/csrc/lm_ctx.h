@@ -1,0 +1,59 @@
+// lm_ctx.h -- private: the context behind the opaque lm_ctx of include/lm.h, shared by the
+// translation units that implement the C ABI (lm_api.cu, lm_traj_api.cu).
+#pragma once
+#include "../../include/lm.h"
+#include "lm_kernels.cuh"
+#include "lm_traj.cuh"
+
+#include <atomic>
+
+namespace lmk {
+
+struct Layout { // byte offsets into the workspace
+    size_t q, lam, res, perr, rerr, its, mask, ui, us, conv, titers, totals, s_seeds, s_tp, s_tq, total;
+};
+
+struct TrajState { // trajectory-level LM (lm_traj_*), bound by lm_traj_attach
+    bool attached = false;
+    bool targets_packed = false;
+    TArgs args{};
+    float lambda0 = 1e-3f;
+    int refine = 1;
+    size_t bytes = 0;
+    char *ws = nullptr;
+    size_t off_totals = 0, off_ui = 0, off_us = 0;
+};
+
+int cuda_fail(cudaError_t e);              // records the error string for lm_strerror, returns LM_ECUDA
+std::atomic<long long> &launch_counter();  // lm_launch_count
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+} // namespace lmk
+
+struct lm_ctx {
+    int dof;
+    int64_t B, n, W;
+    int shared;
+    lmk::KArgs args; // template for every launch
+    lmk::Layout lay;
+    char *ws;
+    cudaStream_t stream;
+    bool fresh;
+    int block;
+    bool fast;
+    int spec_id;      // structure-matched specialised kernel (lm_specs.cuh) or SPEC_GENERIC
+    bool use_generic; // LM_OPT_GENERIC_KERNEL
+    lmk::TrajState traj;
+};
+
+namespace lmk {
+int materialize_state(lm_ctx *c);        // if nothing has run yet: state := seeds (a zero-iteration launch)
+int refresh_waypoint_outputs(lm_ctx *c); // zero-iteration launch: re-evaluates |r|, errors, frozen flag at the current q
+}
+
+#define LM_CUDA(x)                                        \
+    do {                                                  \
+        cudaError_t e_ = (x);                             \
+        if (e_ != cudaSuccess) return lmk::cuda_fail(e_); \
+    } while (0)

@@ -1,0 +1,236 @@
+// lm_traj_api.cu -- C ABI of the trajectory-level LM step (include/lm.h, lm_traj_*): workspace
+// carving and the launch sequence of one iteration.  Every arithmetic step runs in the kernels
+// of lm_traj.cuh; the host only enqueues launches (no synchronisation before lm_traj_fetch).
+#define LM_TRAJ_PLAIN_KERNELS
+#include "lm_ctx.h"
+#include "lm_traj_launch.h"
+
+#include <cstring>
+
+using namespace lmk;
+
+namespace {
+
+struct TLayout {
+    size_t tp, tq, q, A, gp, cst, V, z, delta, rho, lam, F, Fp, Fd, its, mask, sel, ok, totals, ui, us, total;
+};
+
+TLayout make_tlayout(int d, int64_t B, int64_t n) {
+    const size_t nB = (size_t)B * (size_t)n, NA = (size_t)d * (d + 1) / 2;
+    TLayout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
+    L.tp = take(4 * 3 * nB);
+    L.tq = take(4 * 4 * nB);
+    L.q = take(4 * 2 * d * nB);
+    L.A = take(4 * 2 * NA * nB);
+    L.gp = take(4 * 2 * d * nB);
+    L.cst = take(4 * 2 * 2 * nB);
+    L.V = take(4 * NA * nB);
+    L.z = take(4 * d * nB);
+    L.delta = take(4 * d * nB);
+    L.rho = take(4 * d * nB);
+    L.lam = take(4 * (size_t)B);
+    L.F = take(4 * (size_t)B);
+    L.Fp = take(4 * (size_t)B);
+    L.Fd = take(4 * (size_t)B);
+    L.its = take(4 * (size_t)B);
+    L.mask = take(8 * (size_t)B);
+    L.sel = take(4 * (size_t)B);
+    L.ok = take(4 * (size_t)B);
+    L.totals = take(16);
+    L.ui = take(4 * (size_t)B);
+    L.us = take(4 * (size_t)B);
+    L.total = off;
+    return L;
+}
+
+cudaError_t launch_pose(lm_ctx *c, int which, const TArgs &a) {
+    launch_counter().fetch_add(1);
+    const unsigned block = 128, grid = (unsigned)((a.nB + block - 1) / block);
+    const bool weighted = c->args.weighted != 0;
+    if (c->spec_id != SPEC_GENERIC && !c->use_generic)
+        return launch_traj_pose_spec(which, c->spec_id, weighted, grid, block, c->stream, a);
+    return c->dof <= 4 ? launch_traj_pose_generic_lo(which, c->dof, weighted, grid, block, c->stream, a)
+                       : launch_traj_pose_generic_hi(which, c->dof, weighted, grid, block, c->stream, a);
+}
+
+cudaError_t launch_plain(lm_ctx *c, int which, const TArgs &a) {
+    launch_counter().fetch_add(1);
+    if (which == TK_SOLVE) {
+        const unsigned block = 32, grid = (unsigned)((a.B + block - 1) / block);
+        return launch_traj_plain(which, c->dof, grid, block, c->stream, a);
+    }
+    const unsigned block = 256, grid = (unsigned)((a.nB + block - 1) / block);
+    return launch_traj_plain(which, c->dof, grid, block, c->stream, a);
+}
+
+__global__ void tl_stats_kernel(const uint32_t *__restrict__ its, int64_t B, int32_t *__restrict__ iters,
+                                uint32_t *__restrict__ status, unsigned long long *__restrict__ totals) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const uint32_t pk = its[b];
+    if (iters) iters[b] = (int32_t)(pk & 0xffu);
+    if (status) status[b] = (pk >> 8) & ~32u;
+    atomicAdd(totals, (unsigned long long)(pk & 0xffu)); // integer: order-free
+}
+
+bool is_host_ptr(const void *p) {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, p) != cudaSuccess) { cudaGetLastError(); return true; }
+    return pa.type != cudaMemoryTypeDevice && pa.type != cudaMemoryTypeManaged;
+}
+
+} // namespace
+
+extern "C" {
+
+size_t lm_traj_workspace_bytes(int32_t dof, int64_t B, int64_t n) {
+    if (dof < 1 || dof > LM_MAX_DOF || B <= 0 || n <= 0) return 0;
+    return make_tlayout(dof, B, n).total;
+}
+
+int lm_traj_default_params(lm_traj_params *out) {
+    if (!out) return LM_EINVAL;
+    out->w_pose = 1.f;
+    out->w_diff = 1.f;
+    out->lambda0 = 1e-3f;
+    out->nu_up = 10.f;
+    out->nu_down = 10.f;
+    out->lambda_min = 1e-4f;
+    out->lambda_max = 1e7f;
+    out->refine_steps = 1;
+    return LM_OK;
+}
+
+int lm_traj_attach(lm_ctx *c, const lm_traj_params *p, void *workspace, size_t bytes) {
+    if (!c || !p || !workspace) return LM_EINVAL;
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LM_EINVAL;
+    if (!(p->w_pose >= 0.f) || !(p->w_diff >= 0.f) || !(p->lambda0 > 0.f) || !(p->nu_up > 1.f) || !(p->nu_down > 1.f) ||
+        !(p->lambda_min > 0.f) || !(p->lambda_max >= p->lambda_min) || p->refine_steps < 0 || p->refine_steps > 2)
+        return LM_EINVAL;
+    const TLayout L = make_tlayout(c->dof, c->B, c->n);
+    if (bytes < L.total) return LM_ENOMEM;
+    TrajState &t = c->traj;
+    t = TrajState{};
+    t.ws = static_cast<char *>(workspace);
+    t.bytes = bytes;
+    t.lambda0 = p->lambda0;
+    t.refine = p->refine_steps;
+    t.off_totals = L.totals; t.off_ui = L.ui; t.off_us = L.us;
+    TArgs &a = t.args;
+    std::memset(&a, 0, sizeof(a));
+    a.ch = c->args.ch;
+    a.w_pos = c->args.w_pos; a.w_rot = c->args.w_rot;
+    a.wp2 = p->w_pose * p->w_pose;
+    a.wd2 = p->w_diff * p->w_diff;
+    a.wd4 = a.wd2 * a.wd2;
+    a.nu_up = p->nu_up; a.inv_nu_down = (float)(1.0 / (double)p->nu_down);
+    a.lambda_min = p->lambda_min; a.lambda_max = p->lambda_max;
+    a.B = c->B; a.n = (int32_t)c->n; a.nB = c->W;
+    a.shared_targets = c->shared;
+    a.max_total = LM_MAX_ITERS;
+    auto f = [&](size_t off) { return reinterpret_cast<float *>(t.ws + off); };
+    if (c->shared) { // one path for all trajectories: the w-order arrays [.][n] are already what e-order needs
+        a.tp = c->args.tp; a.tq = c->args.tq;
+    } else {
+        a.tp = f(L.tp); a.tq = f(L.tq);
+    }
+    a.q = f(L.q); a.A = f(L.A); a.gp = f(L.gp); a.cst = f(L.cst); a.V = f(L.V); a.z = f(L.z);
+    a.delta = f(L.delta); a.rho = f(L.rho); a.lam = f(L.lam); a.F = f(L.F); a.Fp = f(L.Fp); a.Fd = f(L.Fd);
+    a.its = reinterpret_cast<uint32_t *>(t.ws + L.its);
+    a.mask = reinterpret_cast<unsigned long long *>(t.ws + L.mask);
+    a.sel = reinterpret_cast<int32_t *>(t.ws + L.sel);
+    a.ok = reinterpret_cast<int32_t *>(t.ws + L.ok);
+    a.src_tp = c->args.tp; a.src_tq = c->args.tq;
+    t.attached = true;
+    return lm_traj_reset(c, nullptr);
+}
+
+int lm_traj_reset(lm_ctx *c, const float *lambda) {
+    if (!c || !c->traj.attached) return LM_EINVAL;
+    TrajState &t = c->traj;
+    const float *lam_dev = lambda;
+    if (lambda && is_host_ptr(lambda)) { // stage through the (not yet used) rho array
+        LM_CUDA(cudaMemcpyAsync(t.args.rho, lambda, 4 * (size_t)c->B, cudaMemcpyHostToDevice, c->stream));
+        lam_dev = t.args.rho;
+    }
+    launch_counter().fetch_add(1);
+    tl_reset_kernel<<<(unsigned)((c->B + 255) / 256), 256, 0, c->stream>>>(t.args, lam_dev, t.lambda0);
+    LM_CUDA(cudaGetLastError());
+    return LM_OK;
+}
+
+int lm_traj_set_trace(lm_ctx *c, float *trial_q, float *trial_F) {
+    if (!c || !c->traj.attached || ((trial_q == nullptr) != (trial_F == nullptr))) return LM_EINVAL;
+    c->traj.args.trace_q = trial_q;
+    c->traj.args.trace_F = trial_F;
+    return LM_OK;
+}
+
+int lm_traj_run(lm_ctx *c, int32_t iters) {
+    if (!c || !c->traj.attached || iters < 0 || iters > LM_MAX_ITERS) return LM_EINVAL;
+    TrajState &t = c->traj;
+    int rc = materialize_state(c);
+    if (rc != LM_OK) return rc;
+    TArgs a = t.args;
+    a.src_q = c->args.q;
+    a.dst_q = c->args.q;
+    if (!t.targets_packed && !c->shared) {
+        LM_CUDA(launch_plain(c, TK_PACK_TARGETS, a));
+        t.targets_packed = true;
+    }
+    // current point -> e-order, its normal equations and cost
+    LM_CUDA(launch_plain(c, TK_PACK_Q, a));
+    LM_CUDA(launch_pose(c, TK_ASSEMBLE, a));
+    launch_counter().fetch_add(1);
+    tl_init_cost_kernel<<<(unsigned)((c->B + 127) / 128), 128, 0, c->stream>>>(a);
+    LM_CUDA(cudaGetLastError());
+    for (int it = 0; it < iters; ++it) {
+        a.mode = 0;
+        LM_CUDA(launch_plain(c, TK_SOLVE, a));
+        for (int r = 0; r < t.refine; ++r) {
+            LM_CUDA(launch_pose(c, TK_RHO, a));
+            a.mode = 1;
+            LM_CUDA(launch_plain(c, TK_SOLVE, a));
+        }
+        LM_CUDA(launch_pose(c, TK_TRIAL, a));
+        launch_counter().fetch_add(1);
+        tl_decide_kernel<<<(unsigned)((c->B + 127) / 128), 128, 0, c->stream>>>(a);
+        LM_CUDA(cudaGetLastError());
+    }
+    LM_CUDA(launch_plain(c, TK_UNPACK, a));
+    // refresh the per-waypoint outputs of lm_fetch (|r|, pos / rot error, frozen flag) at the new joint values
+    return refresh_waypoint_outputs(c);
+}
+
+int lm_traj_fetch(lm_ctx *c, lm_traj_stats *s) {
+    if (!c || !c->traj.attached || !s) return LM_EINVAL;
+    TrajState &t = c->traj;
+    const TArgs &a = t.args;
+    const size_t B = (size_t)c->B;
+    auto out = [&](void *dst, const void *src, size_t bytes) -> cudaError_t {
+        return dst ? cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, c->stream) : cudaSuccess;
+    };
+    LM_CUDA(out(s->cost, a.F, 4 * B));
+    LM_CUDA(out(s->cost_pose, a.Fp, 4 * B));
+    LM_CUDA(out(s->cost_diff, a.Fd, 4 * B));
+    LM_CUDA(out(s->lambda, a.lam, 4 * B));
+    LM_CUDA(out(s->accept_mask, a.mask, 8 * B));
+    unsigned long long *tot = reinterpret_cast<unsigned long long *>(t.ws + t.off_totals);
+    int32_t *ui = reinterpret_cast<int32_t *>(t.ws + t.off_ui);
+    uint32_t *us = reinterpret_cast<uint32_t *>(t.ws + t.off_us);
+    LM_CUDA(cudaMemsetAsync(tot, 0, 16, c->stream));
+    launch_counter().fetch_add(1);
+    tl_stats_kernel<<<(unsigned)((B + 255) / 256), 256, 0, c->stream>>>(a.its, c->B, ui, us, tot);
+    LM_CUDA(cudaGetLastError());
+    LM_CUDA(out(s->iters, ui, 4 * B));
+    LM_CUDA(out(s->status, us, 4 * B));
+    unsigned long long h[2] = {0, 0};
+    LM_CUDA(cudaMemcpyAsync(h, tot, 16, cudaMemcpyDeviceToHost, c->stream));
+    LM_CUDA(cudaStreamSynchronize(c->stream));
+    s->total_traj_iters = (int64_t)h[0];
+    return LM_OK;
+}
+
+} // extern "C"

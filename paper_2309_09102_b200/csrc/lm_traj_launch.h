@@ -1,0 +1,51 @@
+// lm_traj_launch.h -- launch entry points of the trajectory-level kernels (lm_traj.cuh); one
+// translation unit per group of instantiations so that the build compiles them in parallel.
+#pragma once
+#include "lm_specs.cuh"
+#include "lm_traj.cuh"
+
+namespace lmk {
+
+enum TrajPoseKernel : int { TK_ASSEMBLE = 0, TK_RHO = 1, TK_TRIAL = 2 };
+enum TrajPlainKernel : int { TK_PACK_Q = 0, TK_PACK_TARGETS = 1, TK_UNPACK = 2, TK_SOLVE = 3 };
+
+// kernels that evaluate FK (chain-structure specialised or generic), thread per waypoint
+cudaError_t launch_traj_pose_spec(int which, int spec_id, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
+cudaError_t launch_traj_pose_generic_lo(int which, int dof, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
+cudaError_t launch_traj_pose_generic_hi(int which, int dof, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
+// kernels that depend on the dof only
+cudaError_t launch_traj_plain(int which, int dof, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
+
+template <int D, typename SpecT>
+cudaError_t launch_traj_pose_t(int which, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a) {
+    switch (which) {
+    case TK_ASSEMBLE:
+        if (weighted) tl_assemble_kernel<D, false, true, SpecT><<<grid, block, 0, s>>>(a);
+        else tl_assemble_kernel<D, false, false, SpecT><<<grid, block, 0, s>>>(a);
+        break;
+    case TK_RHO:
+        if (weighted) tl_rho_kernel<D, false, true, SpecT><<<grid, block, 0, s>>>(a);
+        else tl_rho_kernel<D, false, false, SpecT><<<grid, block, 0, s>>>(a);
+        break;
+    case TK_TRIAL:
+        if (weighted) tl_trial_kernel<D, false, true, SpecT><<<grid, block, 0, s>>>(a);
+        else tl_trial_kernel<D, false, false, SpecT><<<grid, block, 0, s>>>(a);
+        break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+template <int D>
+cudaError_t launch_traj_plain_t(int which, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a) {
+    switch (which) {
+    case TK_PACK_Q: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 0); break;
+    case TK_PACK_TARGETS: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 1); break;
+    case TK_UNPACK: tl_unpack_kernel<D><<<grid, block, 0, s>>>(a); break;
+    case TK_SOLVE: tl_solve_kernel<D><<<grid, block, 0, s>>>(a); break;
+    default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+} // namespace lmk

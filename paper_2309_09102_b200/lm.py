@@ -28,7 +28,10 @@ LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1
 # every symbol include/lm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_run", "lm_fetch",
            "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_option", "lm_kernel_name", "lm_fk", "lm_fp32_peak", "lm_free",
-           "lm_strerror", "lm_launch_count")
+           "lm_strerror", "lm_launch_count", "lm_fp32_peak_form",
+           "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
+           "lm_traj_fetch", "lm_traj_set_trace")
+LM_FMA_FORM_RCC, LM_FMA_FORM_RRR = 0, 1
 
 
 class LmChain(C.Structure):
@@ -54,6 +57,18 @@ class LmStats(C.Structure):
                 ("lambda_", C.c_void_p), ("iters", C.c_void_p), ("accept_mask", C.c_void_p),
                 ("status", C.c_void_p), ("traj_converged", C.c_void_p), ("traj_iters", C.c_void_p),
                 ("total_waypoint_iters", C.c_int64), ("converged_trajectories", C.c_int64)]
+
+
+class LmTrajParams(C.Structure):
+    _fields_ = [("w_pose", C.c_float), ("w_diff", C.c_float), ("lambda0", C.c_float), ("nu_up", C.c_float),
+                ("nu_down", C.c_float), ("lambda_min", C.c_float), ("lambda_max", C.c_float),
+                ("refine_steps", C.c_int32)]
+
+
+class LmTrajStats(C.Structure):
+    _fields_ = [("cost", C.c_void_p), ("cost_pose", C.c_void_p), ("cost_diff", C.c_void_p),
+                ("lambda_", C.c_void_p), ("iters", C.c_void_p), ("accept_mask", C.c_void_p),
+                ("status", C.c_void_p), ("total_traj_iters", C.c_int64)]
 
 
 class LmError(RuntimeError):
@@ -94,6 +109,15 @@ def lib() -> C.CDLL:
         L.lm_strerror.argtypes = [C.c_int]
         L.lm_strerror.restype = C.c_char_p
         L.lm_launch_count.restype = C.c_int64
+        L.lm_fp32_peak_form.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
+        L.lm_traj_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64]
+        L.lm_traj_workspace_bytes.restype = C.c_size_t
+        L.lm_traj_default_params.argtypes = [C.POINTER(LmTrajParams)]
+        L.lm_traj_attach.argtypes = [C.c_void_p, C.POINTER(LmTrajParams), C.c_void_p, C.c_size_t]
+        L.lm_traj_run.argtypes = [C.c_void_p, C.c_int32]
+        L.lm_traj_reset.argtypes = [C.c_void_p, C.c_void_p]
+        L.lm_traj_fetch.argtypes = [C.c_void_p, C.POINTER(LmTrajStats)]
+        L.lm_traj_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -193,6 +217,46 @@ def lm_fp32_peak(cuda_stream: int = 0) -> float:
     out = C.c_double(0.0)
     _check(lib().lm_fp32_peak(C.c_void_p(cuda_stream), C.byref(out)), "lm_fp32_peak")
     return float(out.value)
+
+
+def lm_fp32_peak_form(form: int, cuda_stream: int = 0) -> float:
+    out = C.c_double(0.0)
+    _check(lib().lm_fp32_peak_form(C.c_void_p(cuda_stream), int(form), C.byref(out)), "lm_fp32_peak_form")
+    return float(out.value)
+
+
+def lm_traj_workspace_bytes(dof: int, B: int, n: int) -> int:
+    return int(lib().lm_traj_workspace_bytes(dof, B, n))
+
+
+def lm_traj_default_params(**overrides) -> LmTrajParams:
+    p = LmTrajParams()
+    _check(lib().lm_traj_default_params(C.byref(p)), "lm_traj_default_params")
+    for k, v in overrides.items():
+        if not hasattr(p, k):
+            raise AttributeError(k)
+        setattr(p, k, v)
+    return p
+
+
+def lm_traj_attach(ctx: int, params: LmTrajParams, workspace_ptr: int, workspace_bytes: int) -> None:
+    _check(lib().lm_traj_attach(ctx, C.byref(params), workspace_ptr, workspace_bytes), "lm_traj_attach")
+
+
+def lm_traj_run(ctx: int, iters: int) -> None:
+    _check(lib().lm_traj_run(ctx, int(iters)), "lm_traj_run")
+
+
+def lm_traj_reset(ctx: int, lambda_ptr: Optional[int]) -> None:
+    _check(lib().lm_traj_reset(ctx, lambda_ptr), "lm_traj_reset")
+
+
+def lm_traj_fetch(ctx: int, stats: LmTrajStats) -> None:
+    _check(lib().lm_traj_fetch(ctx, C.byref(stats)), "lm_traj_fetch")
+
+
+def lm_traj_set_trace(ctx: int, trial_q_ptr: Optional[int], trial_F_ptr: Optional[int]) -> None:
+    _check(lib().lm_traj_set_trace(ctx, trial_q_ptr, trial_F_ptr), "lm_traj_set_trace")
 
 
 def lm_free(ctx: int) -> None:
@@ -305,6 +369,57 @@ class Solver:
         if getattr(self, "trace_q", None) is not None:
             res["trial_q"] = np.ascontiguousarray(self.trace_q.cpu().numpy().T)
             tf = self.trace_F.cpu().numpy()
+            res["F_before"], res["F_trial"] = tf[0], tf[1]
+        return res
+
+    # -- trajectory-level step (include/lm.h, lm_traj_*)
+    def traj_attach(self, tparams: Optional[LmTrajParams] = None) -> None:
+        torch = self.torch
+        self.tparams = tparams if tparams is not None else lm_traj_default_params()
+        nbytes = lm_traj_workspace_bytes(self.d, self.B, self.n)
+        self.traj_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self.traj_workspace.data_ptr() + 255) // 256 * 256
+        lm_traj_attach(self._ctx, self.tparams, ptr, nbytes)
+
+    def traj_run(self, iters: int) -> None:
+        lm_traj_run(self._ctx, iters)
+
+    def traj_reset(self, lam=None) -> None:
+        """lam [B] numpy or None (= lambda0)."""
+        if lam is None:
+            lm_traj_reset(self._ctx, None)
+        else:
+            self._tlam_in = self.torch.from_numpy(np.ascontiguousarray(lam, dtype=np.float32)).to(self.device)
+            lm_traj_reset(self._ctx, self._tlam_in.data_ptr())
+
+    def traj_enable_trace(self) -> None:
+        torch = self.torch
+        self.ttrace_q = torch.full((self.d, self.W), float("nan"), dtype=torch.float32, device=self.device)
+        self.ttrace_F = torch.full((2, self.B), float("nan"), dtype=torch.float32, device=self.device)
+        lm_traj_set_trace(self._ctx, self.ttrace_q.data_ptr(), self.ttrace_F.data_ptr())
+
+    def traj_fetch(self) -> dict:
+        """lm_traj_fetch into pinned host buffers -> numpy; q comes from fetch()."""
+        torch = self.torch
+        B = self.B
+
+        def buf(dtype):
+            return torch.empty((B,), dtype=dtype).pin_memory()
+
+        out = {"cost": buf(torch.float32), "cost_pose": buf(torch.float32), "cost_diff": buf(torch.float32),
+               "lam": buf(torch.float32), "iters": buf(torch.int32), "mask": buf(torch.int64),
+               "status": buf(torch.int32)}
+        st = LmTrajStats(out["cost"].data_ptr(), out["cost_pose"].data_ptr(), out["cost_diff"].data_ptr(),
+                         out["lam"].data_ptr(), out["iters"].data_ptr(), out["mask"].data_ptr(),
+                         out["status"].data_ptr(), 0)
+        lm_traj_fetch(self._ctx, st)
+        res = {k: v.numpy().copy() for k, v in out.items()}
+        res["mask"] = res["mask"].view(np.uint64)
+        res["status"] = res["status"].view(np.uint32)
+        res["total_traj_iters"] = int(st.total_traj_iters)
+        if getattr(self, "ttrace_q", None) is not None:
+            res["trial_q"] = np.ascontiguousarray(self.ttrace_q.cpu().numpy().T)
+            tf = self.ttrace_F.cpu().numpy()
             res["F_before"], res["F_trial"] = tf[0], tf[1]
         return res
 
