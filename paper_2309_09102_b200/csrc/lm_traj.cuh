@@ -8,13 +8,18 @@
 // along the waypoint index (block Thomas),
 //   S_1 = T_1,  S_i = T_i - w_d^4 S_{i-1}^-1,  h_i = g_i + w_d^2 S_{i-1}^-1 h_{i-1},
 //   x_n = S_n^-1 h_n,  x_i = S_i^-1 h_i + w_d^2 S_i^-1 x_{i+1},          delta = -x,
-// one THREAD per trajectory (the recurrence is sequential in i, the trajectories are the parallel
+// one LANE per trajectory (the recurrence is sequential in i, the trajectories are the parallel
 // dimension), d x d symmetric blocks in registers, S_i^-1 by the symmetric sweep operator.
 // Everything per-waypoint (FK, Jacobian, J^T J, J^T r, trial cost) runs one thread per waypoint.
 //
-// Layout: "e-order" structure-of-arrays, e = i * B + b (trajectory index fastest), so that both
-// the per-waypoint kernels (consecutive lanes = consecutive e) and the per-trajectory kernel
-// (consecutive lanes = consecutive b at the same i) touch consecutive 4-byte words.
+// Layout ("tile order"): trajectories are grouped in tiles of 32 (one warp); the record of
+// waypoint i of tile bt is the chunk  wid = bt * n + i,  and component c of lane l (trajectory
+// b = 32 bt + l) of a C-component array lives at  (wid * C + c) * 32 + l.  A warp therefore reads
+// or writes a chunk as C consecutive 128-byte lines, a tile's chunks for i = 0..n-1 are one
+// contiguous stream, and the solve kernel prefetches them with bulk-async copies
+// (cp.async.bulk + mbarrier) into a shared-memory ring several waypoints ahead of the
+// recurrence.  Lanes of the last tile beyond B are padding: they compute on whatever the
+// workspace holds and never store.
 // Determinism: fixed summation orders, no float atomics; explicit round-to-nearest intrinsics.
 #pragma once
 #include "lm_device.cuh"
@@ -27,114 +32,144 @@ struct TArgs {
     float w_pos, w_rot;            // pose residual weights (lm_params)
     float wp2, wd2, wd4;           // w_pose^2, w_diff^2, w_diff^4
     float nu_up, inv_nu_down, lambda_min, lambda_max;
-    int64_t B, nB;                 // trajectories, n * B
+    int64_t B, Bt, nS;             // trajectories, tiles = ceil(B / 32), slots = Bt * n * 32
     int32_t n;
     int32_t shared_targets;
     int32_t max_total;             // iteration cap per trajectory (mask width)
-    int32_t mode;                  // solve kernel: 0 = factor + solve for g, 1 = re-solve for rho (refinement)
-    const float *tp, *tq;          // targets, e-order [3][nBt], [4][nBt] (nBt = n when shared)
-    float *q;                      // [2][D][nB]   current / candidate joint values
-    float *A;                      // [2][NA][nB]  w_p^2 J^T J, packed lower triangle
-    float *gp;                     // [2][D][nB]   w_p^2 J^T r
-    float *cst;                    // [2][2][nB]   |r_pose,i|^2 and |q_{i+1} - q_i|^2 (0 for the last waypoint)
-    float *V;                      // [NA][nB]     -(S_i)^-1
-    float *z;                      // [D][nB]
-    float *delta;                  // [D][nB]
-    float *rho;                    // [D][nB]
-    float *lam, *F, *Fp, *Fd;      // [B]
-    uint32_t *its;                 // [B] iters | status << 8
-    unsigned long long *mask;      // [B]
-    int32_t *sel;                  // [B] which of the two buffers holds the current point
-    int32_t *ok;                   // [B] this iteration's solve succeeded
+    const float *tp, *tq;          // targets: tile order [3], [4] comps; when shared: plain [3][n], [4][n]
+    float *tp_w, *tq_w;            // the same arrays, writable (pack kernel)
+    float *q;                      // [2] x D comps     current / candidate joint values
+    float *Ag;                     // [2] x (NA + D)    w_p^2 J^T J (packed lower), then g = J^T r of the stacked residual
+    float *cst;                    // [2] x 2           |r_pose,i|^2 and |q_{i+1} - q_i|^2 (0 for the last waypoint)
+    float *V;                      // NA                -(S_i)^-1
+    float *z;                      // D
+    float *delta;                  // D
+    float *rho;                    // D
+    float *lam, *F, *Fp, *Fd;      // [Bt * 32] per trajectory
+    uint32_t *its;                 // iters | status << 8
+    unsigned long long *mask;
+    int32_t *sel;                  // which of the two buffers holds the trajectory's current point
+    int32_t *ok;                   // this iteration's solve succeeded
     float *trace_q, *trace_F;      // nullable: trial point [D][W] in w-order (w = b n + i), (F, F+) [2][B]
-    // pack / unpack (w-order <-> e-order)
-    const float *src_q;            // [D][W] w-order
-    const float *src_tp, *src_tq;  // [3][Wt], [4][Wt] w-order
-    float *dst_q;                  // [D][W] w-order
+    const float *src_q;            // pack: [D][W] w-order
+    const float *src_tp, *src_tq;  // pack: [3][W], [4][W] w-order
+    float *dst_q;                  // unpack: [D][W] w-order
 };
 
 template <int D> struct Tri { static constexpr int NA = D * (D + 1) / 2; };
 __host__ __device__ constexpr int tri(int r, int c) { return r >= c ? r * (r + 1) / 2 + c : c * (c + 1) / 2 + r; }
 
-// ---- w-order -> e-order (targets once per attach, q at the start of every lm_traj_run)
+// which (tile, waypoint, trajectory) a thread of a per-waypoint kernel owns
+struct Slot {
+    int64_t wid; // chunk index bt * n + i
+    int lane;
+    int i;       // waypoint
+    int64_t b;   // trajectory
+    bool valid;
+};
+__device__ __forceinline__ Slot slot_of_thread(const TArgs &A) {
+    Slot s;
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    s.lane = (int)(t & 31);
+    s.wid = t >> 5;
+    const int64_t bt = s.wid / A.n;
+    s.i = (int)(s.wid - bt * A.n);
+    s.b = bt * 32 + s.lane;
+    s.valid = (s.wid < A.Bt * A.n) && (s.b < A.B);
+    return s;
+}
+template <int C> __device__ __forceinline__ int64_t toff(int64_t wid, int c, int lane) { return (wid * C + c) * 32 + lane; }
+
+// ---- w-order -> tile order (targets once per attach, q at the start of every lm_traj_run)
 template <int D>
 __global__ void __launch_bounds__(256) tl_pack_kernel(const __grid_constant__ TArgs A, int what) {
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= A.nB) return;
-    const int64_t i = e / A.B, b = e - i * A.B;
-    const int64_t w = b * A.n + i, W = A.nB;
+    const Slot s = slot_of_thread(A);
+    if (!s.valid) return;
+    const int64_t W = A.B * A.n, w = s.b * A.n + s.i;
     if (what == 0) { // joint values into the buffer the trajectory currently selects
-        float *dst = A.q + (int64_t)A.sel[b] * D * A.nB;
+        float *dst = A.q + (int64_t)A.sel[s.b] * D * A.nS;
 #pragma unroll
-        for (int j = 0; j < D; ++j) dst[(int64_t)j * A.nB + e] = A.src_q[(int64_t)j * W + w];
+        for (int j = 0; j < D; ++j) dst[toff<D>(s.wid, j, s.lane)] = A.src_q[(int64_t)j * W + w];
     } else if (!A.shared_targets) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) const_cast<float *>(A.tp)[(int64_t)c * A.nB + e] = A.src_tp[(int64_t)c * W + w];
+        for (int c = 0; c < 3; ++c) A.tp_w[toff<3>(s.wid, c, s.lane)] = A.src_tp[(int64_t)c * W + w];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) const_cast<float *>(A.tq)[(int64_t)c * A.nB + e] = A.src_tq[(int64_t)c * W + w];
+        for (int c = 0; c < 4; ++c) A.tq_w[toff<4>(s.wid, c, s.lane)] = A.src_tq[(int64_t)c * W + w];
     }
 }
 
 template <int D>
 __global__ void __launch_bounds__(256) tl_unpack_kernel(const __grid_constant__ TArgs A) {
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= A.nB) return;
-    const int64_t i = e / A.B, b = e - i * A.B;
-    const int64_t w = b * A.n + i, W = A.nB;
-    const float *src = A.q + (int64_t)A.sel[b] * D * A.nB;
+    const Slot s = slot_of_thread(A);
+    if (!s.valid) return;
+    const int64_t W = A.B * A.n, w = s.b * A.n + s.i;
+    const float *src = A.q + (int64_t)A.sel[s.b] * D * A.nS;
 #pragma unroll
-    for (int j = 0; j < D; ++j) A.dst_q[(int64_t)j * W + w] = src[(int64_t)j * A.nB + e];
+    for (int j = 0; j < D; ++j) A.dst_q[(int64_t)j * W + w] = src[toff<D>(s.wid, j, s.lane)];
 }
 
-// load the target of (i, b) and convert the quaternion (DESIGN R11)
-__device__ __forceinline__ void tl_load_target(const TArgs &A, int64_t e, int64_t i, float (&pt)[3], float (&Rt)[3][3]) {
-    const int64_t Wt = A.shared_targets ? (int64_t)A.n : A.nB;
-    const int64_t wt = A.shared_targets ? i : e;
+// load the target of a slot and convert the quaternion (DESIGN R11)
+__device__ __forceinline__ void tl_load_target(const TArgs &A, const Slot &s, float (&pt)[3], float (&Rt)[3][3]) {
+    float qv[4];
+    if (A.shared_targets) {
 #pragma unroll
-    for (int c = 0; c < 3; ++c) pt[c] = __ldg(A.tp + (int64_t)c * Wt + wt);
-    quat_to_cols(__ldg(A.tq + wt), __ldg(A.tq + Wt + wt), __ldg(A.tq + 2 * Wt + wt), __ldg(A.tq + 3 * Wt + wt), Rt);
+        for (int c = 0; c < 3; ++c) pt[c] = __ldg(A.tp + (int64_t)c * A.n + s.i);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) qv[c] = __ldg(A.tq + (int64_t)c * A.n + s.i);
+    } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) pt[c] = __ldg(A.tp + toff<3>(s.wid, c, s.lane));
+#pragma unroll
+        for (int c = 0; c < 4; ++c) qv[c] = __ldg(A.tq + toff<4>(s.wid, c, s.lane));
+    }
+    quat_to_cols(qv[0], qv[1], qv[2], qv[3], Rt);
 }
 
-// w_p^2 J^T J (packed lower), w_p^2 J^T r, |r|^2 of one waypoint -> buffer `dstsel`
+// w_p^2 J^T J (packed lower) and g = w_p^2 J^T r + w_d^2 (c_i y_i - y_{i-1} - y_{i+1}) (y = the joint
+// values the Jacobian was taken at), |r_pose|^2 and |y_{i+1} - y_i|^2 of one waypoint -> buffer `dstsel`
 template <int D>
-__device__ __forceinline__ void tl_store_normal(const TArgs &A, const Pose<D> &P, int dstsel, int64_t e, float fd) {
-    constexpr int NA = Tri<D>::NA;
-    float *Ad = A.A + (int64_t)dstsel * NA * A.nB + e;
-    float *gd = A.gp + (int64_t)dstsel * D * A.nB + e;
+__device__ __forceinline__ void tl_store_normal(const TArgs &A, const Pose<D> &P, int dstsel, const Slot &s,
+                                                const float (&y)[D], const float (&ym)[D], const float (&yn)[D]) {
+    constexpr int NA = Tri<D>::NA, C = NA + D;
+    const int n = A.n;
+    const float ci = (n == 1) ? 0.f : ((s.i == 0 || s.i == n - 1) ? 1.f : 2.f);
+    float *Ad = A.Ag + (int64_t)dstsel * C * A.nS;
+    float fd = 0.f;
 #pragma unroll
     for (int r = 0; r < D; ++r) {
 #pragma unroll
-        for (int c = 0; c <= r; ++c) Ad[(int64_t)tri(r, c) * A.nB] = mul(A.wp2, coldot<D>(P, r, c));
-        gd[(int64_t)r * A.nB] = mul(A.wp2, colvec<D>(P, r, P.r));
+        for (int c = 0; c <= r; ++c) Ad[toff<C>(s.wid, tri(r, c), s.lane)] = mul(A.wp2, coldot<D>(P, r, c));
+        const float dd = sub(sub(mul(ci, y[r]), ym[r]), yn[r]);
+        Ad[toff<C>(s.wid, NA + r, s.lane)] = fma_(A.wd2, dd, mul(A.wp2, colvec<D>(P, r, P.r)));
+        if (s.i + 1 < n) {
+            const float t = sub(yn[r], y[r]);
+            fd = fma_(t, t, fd);
+        }
     }
-    float *cd = A.cst + (int64_t)dstsel * 2 * A.nB + e;
-    cd[0] = P.F;
-    cd[A.nB] = fd;
+    float *cd = A.cst + (int64_t)dstsel * 2 * A.nS;
+    cd[toff<2>(s.wid, 0, s.lane)] = P.F;
+    cd[toff<2>(s.wid, 1, s.lane)] = fd;
 }
 
 // ---- assemble at the current point (entry of lm_traj_run): thread per waypoint
 template <int D, bool FAST, bool WEIGHTED, typename SpecT>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_assemble_kernel(const __grid_constant__ TArgs A) {
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= A.nB) return;
-    const int64_t i = e / A.B, b = e - i * A.B;
-    const int s = A.sel[b];
-    const float *qs = A.q + (int64_t)s * D * A.nB;
-    float q[D], fd = 0.f;
+    const Slot s = slot_of_thread(A);
+    if (!s.valid) return;
+    const int sel = A.sel[s.b];
+    const float *qs = A.q + (int64_t)sel * D * A.nS;
+    float q[D], qm[D], qn[D];
 #pragma unroll
-    for (int j = 0; j < D; ++j) q[j] = qs[(int64_t)j * A.nB + e];
-    if (i + 1 < A.n) {
-#pragma unroll
-        for (int j = 0; j < D; ++j) {
-            const float t = sub(qs[(int64_t)j * A.nB + e + A.B], q[j]);
-            fd = fma_(t, t, fd);
-        }
+    for (int j = 0; j < D; ++j) {
+        q[j] = qs[toff<D>(s.wid, j, s.lane)];
+        qm[j] = (s.i > 0) ? qs[toff<D>(s.wid - 1, j, s.lane)] : 0.f;
+        qn[j] = (s.i + 1 < A.n) ? qs[toff<D>(s.wid + 1, j, s.lane)] : 0.f;
     }
     float pt[3], Rt[3][3];
-    tl_load_target(A, e, i, pt, Rt);
+    tl_load_target(A, s, pt, Rt);
     Pose<D> P;
     eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
-    tl_store_normal<D>(A, P, s, e, fd);
+    tl_store_normal<D>(A, P, sel, s, q, qm, qn);
 }
 
 // Kahan-compensated sum step (explicit intrinsics: the compiler cannot simplify the compensation away)
@@ -145,25 +180,49 @@ __device__ __forceinline__ void kahan_add(float &s, float &c, float x) {
     s = t;
 }
 
-// total cost of buffer `s` of trajectory b, fixed order i = 0..n-1
-__device__ __forceinline__ void tl_sum_cost(const TArgs &A, int s, int64_t b, float &Fp, float &Fd, float &F) {
-    const float *cp = A.cst + (int64_t)s * 2 * A.nB + b;
+// Total cost of buffer `sel` of the trajectory (tile = blockIdx.x, lane): a block of TL_SUM_WARPS warps
+// per tile; warp w sums the waypoints of segment w in order (Kahan), the segment sums are then added
+// in segment order.  The summation order depends on n only, never on the batch.  All threads of the
+// block must call; the result is valid in warp 0.
+constexpr int TL_SUM_WARPS = 8;
+__device__ __forceinline__ void tl_sum_cost(const TArgs &A, int sel, float (*part)[2][32], float &Fp, float &Fd, float &F) {
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    const float *cp = A.cst + (int64_t)sel * 2 * A.nS;
+    const int64_t w0 = (int64_t)blockIdx.x * A.n;
+    const int seg = (A.n + TL_SUM_WARPS - 1) / TL_SUM_WARPS;
+    const int i0 = wp * seg, i1 = min(A.n, i0 + seg);
     float sp = 0.f, cpp = 0.f, sd = 0.f, cd = 0.f;
-    for (int i = 0; i < A.n; ++i) {
-        kahan_add(sp, cpp, cp[(int64_t)i * A.B]);
-        kahan_add(sd, cd, cp[A.nB + (int64_t)i * A.B]);
+    int i = i0;
+    for (; i + 8 <= i1; i += 8) { // 16 independent loads in flight, then the sums in order
+        float a[8], d[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) { a[u] = cp[toff<2>(w0 + i + u, 0, lane)]; d[u] = cp[toff<2>(w0 + i + u, 1, lane)]; }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) { kahan_add(sp, cpp, a[u]); kahan_add(sd, cd, d[u]); }
     }
+    for (; i < i1; ++i) {
+        kahan_add(sp, cpp, cp[toff<2>(w0 + i, 0, lane)]);
+        kahan_add(sd, cd, cp[toff<2>(w0 + i, 1, lane)]);
+    }
+    part[wp][0][lane] = sp;
+    part[wp][1][lane] = sd;
+    __syncthreads();
+    sp = 0.f; cpp = 0.f; sd = 0.f; cd = 0.f;
+#pragma unroll
+    for (int u = 0; u < TL_SUM_WARPS; ++u) { kahan_add(sp, cpp, part[u][0][lane]); kahan_add(sd, cd, part[u][1][lane]); }
     Fp = sp; Fd = sd;
     F = fma_(A.wd2, sd, mul(A.wp2, sp));
 }
 
 #ifdef LM_TRAJ_PLAIN_KERNELS // non-template kernels: defined in exactly one translation unit (lm_traj_api.cu)
-// ---- cost of the current point (entry of lm_traj_run): thread per trajectory
-__global__ void __launch_bounds__(128) tl_init_cost_kernel(const __grid_constant__ TArgs A) {
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= A.B) return;
+// ---- cost of the current point (entry of lm_traj_run): block of TL_SUM_WARPS warps per tile
+__global__ void __launch_bounds__(TL_SUM_WARPS * 32) tl_init_cost_kernel(const __grid_constant__ TArgs A) {
+    __shared__ float part[TL_SUM_WARPS][2][32];
+    const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
+    const bool valid = b < A.B;
     float Fp, Fd, F;
-    tl_sum_cost(A, A.sel[b], b, Fp, Fd, F);
+    tl_sum_cost(A, valid ? A.sel[b] : 0, part, Fp, Fd, F);
+    if (!valid || threadIdx.x >= 32) return;
     A.Fp[b] = Fp; A.Fd[b] = Fd; A.F[b] = F;
 }
 #endif
@@ -210,26 +269,100 @@ __device__ __forceinline__ void symv(const float (&M)[Tri<D>::NA], const float (
     }
 }
 
-// ---- block-tridiagonal solve: thread per trajectory
-//   mode 0: factor (stores W_i = -S_i^-1) and solve for g = gp + w_d^2 D^T D q;  delta  = -x
-//   mode 1: re-solve with the stored W_i for rho (iterative refinement);          delta +=  x
-template <int D>
-__global__ void __launch_bounds__(128) tl_solve_kernel(const __grid_constant__ TArgs A) {
-    constexpr int NA = Tri<D>::NA;
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= A.B) return;
-    const uint32_t pk = A.its[b];
-    if ((pk & 0xffu) >= (uint32_t)A.max_total) return;
-    if (A.mode == 1 && !A.ok[b]) return;
-    const int s = A.sel[b];
+// ---- bulk-async copy + mbarrier primitives (sm_90+ PTX; one warp is both producer and consumer)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+    }
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+constexpr int TL_STAGES = 8; // waypoints in flight per warp in the solve kernel
+
+// One ring stage (floats): [0, NA*32) matrix, then vector 1 (D*32), then vector 2 (D*32).
+// MODE 0 keeps two rings (one per Ag buffer: accept / reject is per trajectory, so the lanes of a
+// tile may select different buffers; a buffer no lane of the tile selects is not fetched).
+template <int D> __host__ __device__ constexpr int tl_stage_floats() { return (Tri<D>::NA + 2 * D) * 32; }
+template <int D, int MODE> __host__ __device__ constexpr size_t tl_solve_smem_bytes() {
+    return (size_t)(MODE == 0 ? 2 : 1) * TL_STAGES * tl_stage_floats<D>() * sizeof(float);
+}
+
+// ---- block-tridiagonal solve: one warp per tile of 32 trajectories, lane = trajectory
+//   MODE 0: factor (stores W_i = -S_i^-1) and solve for g;                      delta  = -x
+//   MODE 1: re-solve with the stored W_i for rho (iterative refinement);        delta +=  x
+// The chunks of the next TL_STAGES waypoints are in flight (bulk-async copies into the ring)
+// while waypoint i is being eliminated.
+template <int D, int MODE>
+__global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TArgs A) {
+    constexpr int NA = Tri<D>::NA, CA = NA + D, SF = tl_stage_floats<D>();
+    extern __shared__ __align__(128) float ring[];
+    __shared__ __align__(8) uint64_t bars[TL_STAGES];
+    const int lane = threadIdx.x;
+    const int64_t bt = blockIdx.x;
+    const int64_t b = bt * 32 + lane;
+    const bool valid = b < A.B;
+    const uint32_t pk = valid ? A.its[b] : 0xffu;
+    const bool active = valid && ((pk & 0xffu) < (uint32_t)A.max_total) && (MODE == 0 || A.ok[b] != 0);
+    if (!__any_sync(0xffffffffu, active)) return;
+    const int sel = valid ? A.sel[b] : 0;
+    const bool need0 = __any_sync(0xffffffffu, active && sel == 0); // warp-uniform
+    const bool need1 = __any_sync(0xffffffffu, active && sel == 1);
     const int n = A.n;
-    const int64_t nB = A.nB, B = A.B;
-    const float lam = A.lam[b];
-    const float *Ab = A.A + (int64_t)s * NA * nB + b;
-    const float *gb = A.gp + (int64_t)s * D * nB + b;
-    const float *qb = A.q + (int64_t)s * D * nB + b;
-    float *Vb = A.V + b, *zb = A.z + b, *db = A.delta + b;
-    const float *rb = A.rho + b;
+    const int64_t w0 = bt * n;
+    const float lam = valid ? A.lam[b] : 1.f;
+    float *ring1 = ring + (size_t)TL_STAGES * SF; // MODE 0 only: chunks of Ag buffer 1
+
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < TL_STAGES; ++s) mbar_init(&bars[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+
+    auto issue_fwd = [&](int k, int i) { // lane 0 only; k = position in the sequence of ring uses
+        const int s = k % TL_STAGES;
+        const int64_t wid = w0 + i;
+        if (MODE == 0) {
+            const uint32_t bytes = CA * 128u;
+            mbar_expect_tx(&bars[s], (need0 ? bytes : 0u) + (need1 ? bytes : 0u));
+            if (need0) bulk_g2s(ring + (size_t)s * SF, A.Ag + wid * CA * 32, bytes, &bars[s]);
+            if (need1) bulk_g2s(ring1 + (size_t)s * SF, A.Ag + (int64_t)CA * A.nS + wid * CA * 32, bytes, &bars[s]);
+        } else {
+            float *dst = ring + (size_t)s * SF;
+            mbar_expect_tx(&bars[s], (NA + D) * 128u);
+            bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, &bars[s]);
+            bulk_g2s(dst + NA * 32, A.rho + wid * D * 32, D * 128u, &bars[s]);
+        }
+    };
+    auto issue_bwd = [&](int k, int i) { // lane 0 only
+        const int s = k % TL_STAGES;
+        float *dst = ring + (size_t)s * SF;
+        const int64_t wid = w0 + i;
+        mbar_expect_tx(&bars[s], (NA + D + (MODE == 1 ? D : 0)) * 128u);
+        bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, &bars[s]);
+        bulk_g2s(dst + NA * 32, A.z + wid * D * 32, D * 128u, &bars[s]);
+        if (MODE == 1) bulk_g2s(dst + (NA + D) * 32, A.delta + wid * D * 32, D * 128u, &bars[s]);
+    };
+
+    if (lane == 0) {
+        for (int k = 0; k < TL_STAGES && k < n; ++k) issue_fwd(k, k);
+    }
 
     float W[NA], zp[D];
 #pragma unroll
@@ -237,111 +370,145 @@ __global__ void __launch_bounds__(128) tl_solve_kernel(const __grid_constant__ T
 #pragma unroll
     for (int j = 0; j < D; ++j) zp[j] = 0.f;
     bool ok = true;
+    const float *my_ring = (MODE == 0 && sel == 1) ? ring1 : ring;
 
     // ---- forward elimination
-    float qm[D], qc[D], qn[D];
-    if (A.mode == 0) {
-#pragma unroll
-        for (int j = 0; j < D; ++j) { qm[j] = 0.f; qc[j] = qb[(int64_t)j * nB]; }
-    }
     for (int i = 0; i < n; ++i) {
-        const int64_t off = (int64_t)i * B;
-        float rhs[D];
-        if (A.mode == 0) {
+        const int s = i % TL_STAGES;
+        mbar_wait(&bars[s], (uint32_t)((i / TL_STAGES) & 1));
+        const float *st = my_ring + (size_t)s * SF;
+        float S[NA], rhs[D];
+#pragma unroll
+        for (int t = 0; t < NA; ++t) S[t] = st[t * 32 + lane];
+#pragma unroll
+        for (int r = 0; r < D; ++r) rhs[r] = st[(NA + r) * 32 + lane];
+        __syncwarp(); // every lane has read the stage: it may be refilled (the copy lands long after these loads)
+        if (lane == 0 && i + TL_STAGES < n) issue_fwd(i + TL_STAGES, i + TL_STAGES);
+        const int64_t wid = w0 + i;
+        if (MODE == 0) {
             const float ci = (n == 1) ? 0.f : ((i == 0 || i == n - 1) ? 1.f : 2.f);
-            const bool has_next = i + 1 < n;
-#pragma unroll
-            for (int j = 0; j < D; ++j) qn[j] = has_next ? qb[(int64_t)j * nB + off + B] : 0.f;
-            float S[NA];
-#pragma unroll
-            for (int t = 0; t < NA; ++t) S[t] = Ab[(int64_t)t * nB + off];
             const float dg = fma_(ci, A.wd2, lam);
 #pragma unroll
-            for (int r = 0; r < D; ++r) {
-                S[tri(r, r)] = add(S[tri(r, r)], dg);
-                // g_i = gp_i + w_d^2 (c_i q_i - q_{i-1} - q_{i+1})
-                const float dd = sub(sub(mul(ci, qc[r]), qm[r]), qn[r]);
-                rhs[r] = fma_(A.wd2, dd, gb[(int64_t)r * nB + off]);
-            }
+            for (int r = 0; r < D; ++r) S[tri(r, r)] = add(S[tri(r, r)], dg);
             // S_i = T_i - w_d^4 S_{i-1}^-1 = T_i + w_d^4 W_{i-1}
 #pragma unroll
             for (int t = 0; t < NA; ++t) S[t] = fma_(A.wd4, W[t], S[t]);
             ok = sweep_neg_inverse<D>(S) && ok;
+            if (active) {
 #pragma unroll
-            for (int t = 0; t < NA; ++t) { W[t] = S[t]; Vb[(int64_t)t * nB + off] = S[t]; }
-#pragma unroll
-            for (int j = 0; j < D; ++j) { qm[j] = qc[j]; qc[j] = qn[j]; }
-        } else {
-#pragma unroll
-            for (int t = 0; t < NA; ++t) W[t] = Vb[(int64_t)t * nB + off];
-#pragma unroll
-            for (int r = 0; r < D; ++r) rhs[r] = rb[(int64_t)r * nB + off];
+                for (int t = 0; t < NA; ++t) A.V[toff<NA>(wid, t, lane)] = S[t];
+            }
         }
+#pragma unroll
+        for (int t = 0; t < NA; ++t) W[t] = S[t];
         // h_i = rhs_i + w_d^2 z_{i-1};  z_i = S_i^-1 h_i = -(W_i h_i)
         float h[D], y[D];
 #pragma unroll
         for (int r = 0; r < D; ++r) h[r] = fma_(A.wd2, zp[r], rhs[r]);
         symv<D>(W, h, y);
 #pragma unroll
-        for (int r = 0; r < D; ++r) { zp[r] = -y[r]; zb[(int64_t)r * nB + off] = zp[r]; }
+        for (int r = 0; r < D; ++r) zp[r] = -y[r];
+        if (active) {
+#pragma unroll
+            for (int r = 0; r < D; ++r) A.z[toff<D>(wid, r, lane)] = zp[r];
+        }
     }
 
+    // the chunks written above are read back by bulk-async copies: order the generic writes before them
+    __threadfence();
+    __syncwarp();
+    fence_proxy_async();
+    __syncwarp();
+
     // ---- back substitution: x_n = z_n, x_i = z_i + w_d^2 S_i^-1 x_{i+1} = z_i - w_d^2 W_i x_{i+1}
+    if (lane == 0) {
+        for (int j = 0; j < TL_STAGES && n - 2 - j >= 0; ++j) issue_bwd(n + j, n - 2 - j);
+    }
     float x[D];
-#pragma unroll
-    for (int j = 0; j < D; ++j) x[j] = 0.f;
-    float asum = 0.f;
-    for (int i = n - 1; i >= 0; --i) {
-        const int64_t off = (int64_t)i * B;
-        if (i == n - 1) {
-#pragma unroll
-            for (int r = 0; r < D; ++r) x[r] = zp[r]; // W, zp still hold waypoint n-1
-        } else {
-            float y[D];
-#pragma unroll
-            for (int t = 0; t < NA; ++t) W[t] = Vb[(int64_t)t * nB + off];
-            symv<D>(W, x, y);
-#pragma unroll
-            for (int r = 0; r < D; ++r) x[r] = fma_(-A.wd2, y[r], zb[(int64_t)r * nB + off]);
-        }
+    float amax = 0.f;
+    {
+        const int64_t wid = w0 + n - 1;
 #pragma unroll
         for (int r = 0; r < D; ++r) {
-            const float dv = (A.mode == 0) ? -x[r] : add(db[(int64_t)r * nB + off], x[r]);
-            db[(int64_t)r * nB + off] = dv;
-            asum = fmaxf(asum, fabsf(dv));
+            x[r] = zp[r];
+            float dv;
+            if (MODE == 0) dv = -x[r];
+            else dv = add(active ? A.delta[toff<D>(wid, r, lane)] : 0.f, x[r]);
+            if (active) A.delta[toff<D>(wid, r, lane)] = dv;
+            amax = fmaxf(amax, fabsf(dv));
         }
     }
-    ok = ok && (asum < 1e30f); // NaN compares false
-    if (A.mode == 0) A.ok[b] = ok ? 1 : 0;
-    else if (!ok) A.ok[b] = 0;
+    for (int i = n - 2; i >= 0; --i) {
+        const int k = n + (n - 2 - i);
+        const int s = k % TL_STAGES;
+        mbar_wait(&bars[s], (uint32_t)((k / TL_STAGES) & 1));
+        const float *st = ring + (size_t)s * SF;
+        float zi[D], dold[D];
+#pragma unroll
+        for (int t = 0; t < NA; ++t) W[t] = st[t * 32 + lane];
+#pragma unroll
+        for (int r = 0; r < D; ++r) {
+            zi[r] = st[(NA + r) * 32 + lane];
+            dold[r] = (MODE == 1) ? st[(NA + D + r) * 32 + lane] : 0.f;
+        }
+        __syncwarp();
+        if (lane == 0 && i - TL_STAGES >= 0) issue_bwd(k + TL_STAGES, i - TL_STAGES);
+        float y[D];
+        symv<D>(W, x, y);
+        const int64_t wid = w0 + i;
+#pragma unroll
+        for (int r = 0; r < D; ++r) {
+            x[r] = fma_(-A.wd2, y[r], zi[r]);
+            const float dv = (MODE == 0) ? -x[r] : add(dold[r], x[r]);
+            if (active) A.delta[toff<D>(wid, r, lane)] = dv;
+            amax = fmaxf(amax, fabsf(dv));
+        }
+    }
+    ok = ok && (amax < 1e30f); // NaN compares false
+    if (active) {
+        if (MODE == 0) A.ok[b] = ok ? 1 : 0;
+        else if (!ok) A.ok[b] = 0;
+    }
 }
 
 // ---- refinement residual (DESIGN R4 carried over to the stacked system): thread per waypoint
 //   rho_i = -[ w_p^2 J_i^T (r_i + J_i delta_i) + w_d^2 (D^T D (q + delta))_i + lambda delta_i ]
 template <int D, bool FAST, bool WEIGHTED, typename SpecT>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(const __grid_constant__ TArgs A) {
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= A.nB) return;
-    const int64_t i = e / A.B, b = e - i * A.B;
-    if ((A.its[b] & 0xffu) >= (uint32_t)A.max_total || !A.ok[b]) return;
-    const int s = A.sel[b];
-    const int64_t nB = A.nB;
-    const float *qs = A.q + (int64_t)s * D * nB;
-    const float lam = A.lam[b];
+    const Slot s = slot_of_thread(A);
+    if (!s.valid) return;
+    const uint32_t pk = A.its[s.b];
+    const int okf = A.ok[s.b];
+    const int sel = A.sel[s.b];
+    const float lam = A.lam[s.b];
+    const float *q0 = A.q, *q1 = A.q + (int64_t)D * A.nS;
     const int n = A.n;
-    const float ci = (n == 1) ? 0.f : ((i == 0 || i == n - 1) ? 1.f : 2.f);
+    const float ci = (n == 1) ? 0.f : ((s.i == 0 || s.i == n - 1) ? 1.f : 2.f);
+    float ra[3][D], rb[3][D], rd[3][D]; // both buffers are fetched, `sel` picks afterwards (see tl_trial_kernel)
+#pragma unroll
+    for (int u = 0; u < 3; ++u) {
+        const bool there = (u == 0) ? (s.i > 0) : (u == 2) ? (s.i + 1 < n) : true;
+        const int64_t wid = s.wid + u - 1;
+#pragma unroll
+        for (int j = 0; j < D; ++j) {
+            ra[u][j] = there ? q0[toff<D>(wid, j, s.lane)] : 0.f;
+            rb[u][j] = there ? q1[toff<D>(wid, j, s.lane)] : 0.f;
+            rd[u][j] = there ? A.delta[toff<D>(wid, j, s.lane)] : 0.f;
+        }
+    }
+    if ((pk & 0xffu) >= (uint32_t)A.max_total || !okf) return;
     float q[D], dl[D], dd[D];
 #pragma unroll
     for (int j = 0; j < D; ++j) {
-        q[j] = qs[(int64_t)j * nB + e];
-        dl[j] = A.delta[(int64_t)j * nB + e];
+        q[j] = sel ? rb[1][j] : ra[1][j];
+        dl[j] = rd[1][j];
         const float yc = add(q[j], dl[j]);
-        const float ym = (i > 0) ? add(qs[(int64_t)j * nB + e - A.B], A.delta[(int64_t)j * nB + e - A.B]) : 0.f;
-        const float yn = (i + 1 < n) ? add(qs[(int64_t)j * nB + e + A.B], A.delta[(int64_t)j * nB + e + A.B]) : 0.f;
+        const float ym = (s.i > 0) ? add(sel ? rb[0][j] : ra[0][j], rd[0][j]) : 0.f;
+        const float yn = (s.i + 1 < n) ? add(sel ? rb[2][j] : ra[2][j], rd[2][j]) : 0.f;
         dd[j] = sub(sub(mul(ci, yc), ym), yn);
     }
     float pt[3], Rt[3][3];
-    tl_load_target(A, e, i, pt, Rt);
+    tl_load_target(A, s, pt, Rt);
     Pose<D> P;
     eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
     float t[6];
@@ -358,7 +525,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(c
 #pragma unroll
     for (int j = 0; j < D; ++j) {
         const float acc = fma_(lam, dl[j], fma_(A.wd2, dd[j], mul(A.wp2, colvec<D>(P, j, t))));
-        A.rho[(int64_t)j * nB + e] = -acc;
+        A.rho[toff<D>(s.wid, j, s.lane)] = -acc;
     }
 }
 
@@ -366,59 +533,73 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(c
 //      into the candidate buffer (1 - sel): thread per waypoint
 template <int D, bool FAST, bool WEIGHTED, typename SpecT>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_trial_kernel(const __grid_constant__ TArgs A) {
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= A.nB) return;
-    const int64_t i = e / A.B, b = e - i * A.B;
-    const uint32_t pk = A.its[b];
-    if ((pk & 0xffu) >= (uint32_t)A.max_total) return;
-    const int s = A.sel[b];
-    const bool ok = A.ok[b] != 0;
-    const int64_t nB = A.nB;
-    const float *qs = A.q + (int64_t)s * D * nB;
-    float *qd = A.q + (int64_t)(1 - s) * D * nB;
-    float qt[D], fd = 0.f;
-    bool clamped = false;
+    const Slot s = slot_of_thread(A);
+    if (!s.valid) return;
+    // every load below is issued before the first use: the joint values of BOTH buffers are fetched and the
+    // trajectory's `sel` picks afterwards (a dependent address would cost one more DRAM round trip)
+    const uint32_t pk = A.its[s.b];
+    const int sel = A.sel[s.b];
+    const bool ok = A.ok[s.b] != 0;
+    const float *q0 = A.q, *q1 = A.q + (int64_t)D * A.nS;
+    float ra[3][D], rb[3][D], rd[3][D];
 #pragma unroll
-    for (int j = 0; j < D; ++j) {
-        const float t = ok ? add(qs[(int64_t)j * nB + e], A.delta[(int64_t)j * nB + e]) : qs[(int64_t)j * nB + e];
-        qt[j] = fminf(fmaxf(t, A.ch.lo[j]), A.ch.hi[j]);
-        clamped = clamped || (qt[j] != t);
-        qd[(int64_t)j * nB + e] = qt[j];
-    }
-    if (i + 1 < A.n) {
+    for (int u = 0; u < 3; ++u) {
+        const bool there = (u == 0) ? (s.i > 0) : (u == 2) ? (s.i + 1 < A.n) : true;
+        const int64_t wid = s.wid + u - 1;
 #pragma unroll
         for (int j = 0; j < D; ++j) {
-            const float t = ok ? add(qs[(int64_t)j * nB + e + A.B], A.delta[(int64_t)j * nB + e + A.B]) : qs[(int64_t)j * nB + e + A.B];
-            const float tn = fminf(fmaxf(t, A.ch.lo[j]), A.ch.hi[j]);
-            const float df = sub(tn, qt[j]);
-            fd = fma_(df, df, fd);
+            ra[u][j] = there ? q0[toff<D>(wid, j, s.lane)] : 0.f;
+            rb[u][j] = there ? q1[toff<D>(wid, j, s.lane)] : 0.f;
+            rd[u][j] = there ? A.delta[toff<D>(wid, j, s.lane)] : 0.f;
         }
     }
-    if (clamped) atomicOr(A.its + b, 32u << 8); // "a trial point was clamped" (integer atomic: order-free)
     float pt[3], Rt[3][3];
-    tl_load_target(A, e, i, pt, Rt);
+    tl_load_target(A, s, pt, Rt);
+    if ((pk & 0xffu) >= (uint32_t)A.max_total) return;
+    float *qd = A.q + (int64_t)(1 - sel) * D * A.nS;
+    float qt[D], qm[D], qn[D];
+    bool clamped = false;
+    auto trial_of = [&](int u, int j, bool &cl) {
+        const float qv = sel ? rb[u][j] : ra[u][j];
+        const float t = ok ? add(qv, rd[u][j]) : qv;
+        const float c = fminf(fmaxf(t, A.ch.lo[j]), A.ch.hi[j]);
+        cl = cl || (c != t);
+        return c;
+    };
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        bool dummy = false;
+        qt[j] = trial_of(1, j, clamped);
+        qm[j] = (s.i > 0) ? trial_of(0, j, dummy) : 0.f;
+        qn[j] = (s.i + 1 < A.n) ? trial_of(2, j, dummy) : 0.f;
+        qd[toff<D>(s.wid, j, s.lane)] = qt[j];
+    }
+    // "a trial point of this trajectory was clamped": integer atomic (order-free), skipped once the bit is seen set
+    if (clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
     Pose<D> P;
     eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
-    tl_store_normal<D>(A, P, 1 - s, e, fd);
+    tl_store_normal<D>(A, P, 1 - sel, s, qt, qm, qn);
     if (A.trace_q != nullptr) {
-        const int64_t w = b * A.n + i;
+        const int64_t W = A.B * A.n, w = s.b * A.n + s.i;
 #pragma unroll
-        for (int j = 0; j < D; ++j) A.trace_q[(int64_t)j * nB + w] = qt[j];
+        for (int j = 0; j < D; ++j) A.trace_q[(int64_t)j * W + w] = qt[j];
     }
 }
 
 #ifdef LM_TRAJ_PLAIN_KERNELS
 // ---- accept / reject and the lambda update, per trajectory (DESIGN T3 = R5 on the total cost)
-__global__ void __launch_bounds__(128) tl_decide_kernel(const __grid_constant__ TArgs A) {
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= A.B) return;
+__global__ void __launch_bounds__(TL_SUM_WARPS * 32) tl_decide_kernel(const __grid_constant__ TArgs A) {
+    __shared__ float part[TL_SUM_WARPS][2][32];
+    const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
+    const bool valid = b < A.B;
+    const int s = valid ? A.sel[b] : 0;
+    float Fp, Fd, Ft;
+    tl_sum_cost(A, 1 - s, part, Fp, Fd, Ft);
+    if (!valid || threadIdx.x >= 32) return;
     uint32_t pk = A.its[b];
     uint32_t k = pk & 0xffu, st = pk >> 8;
     if (k >= (uint32_t)A.max_total) return;
-    const int s = A.sel[b];
     const bool ok = A.ok[b] != 0;
-    float Fp, Fd, Ft;
-    tl_sum_cost(A, 1 - s, b, Fp, Fd, Ft);
     const float F = A.F[b];
     if (A.trace_F != nullptr) { A.trace_F[b] = F; A.trace_F[A.B + b] = Ft; }
     const bool finite = fabsf(Ft) < 3.0e38f;
@@ -446,8 +627,8 @@ __global__ void __launch_bounds__(128) tl_decide_kernel(const __grid_constant__ 
 
 __global__ void __launch_bounds__(256) tl_reset_kernel(const __grid_constant__ TArgs A, const float *lam_in, float lambda0) {
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= A.B) return;
-    A.lam[b] = lam_in ? lam_in[b] : lambda0;
+    if (b >= A.Bt * 32) return;
+    A.lam[b] = (lam_in && b < A.B) ? lam_in[b] : lambda0;
     A.its[b] = 0u;
     A.mask[b] = 0ull;
     A.sel[b] = 0;

@@ -12,42 +12,42 @@ using namespace lmk;
 namespace {
 
 struct TLayout {
-    size_t tp, tq, q, A, gp, cst, V, z, delta, rho, lam, F, Fp, Fd, its, mask, sel, ok, totals, ui, us, total;
+    size_t tp, tq, q, Ag, cst, V, z, delta, rho, lam, F, Fp, Fd, its, mask, sel, ok, totals, ui, us, total;
 };
 
+// tile order (lm_traj.cuh): Bt = ceil(B / 32) tiles, nS = Bt * n * 32 slots, C floats per slot and array
 TLayout make_tlayout(int d, int64_t B, int64_t n) {
-    const size_t nB = (size_t)B * (size_t)n, NA = (size_t)d * (d + 1) / 2;
+    const size_t Bt = ((size_t)B + 31) / 32, Bp = Bt * 32, nS = Bp * (size_t)n, NA = (size_t)d * (d + 1) / 2;
     TLayout L{};
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
-    L.tp = take(4 * 3 * nB);
-    L.tq = take(4 * 4 * nB);
-    L.q = take(4 * 2 * d * nB);
-    L.A = take(4 * 2 * NA * nB);
-    L.gp = take(4 * 2 * d * nB);
-    L.cst = take(4 * 2 * 2 * nB);
-    L.V = take(4 * NA * nB);
-    L.z = take(4 * d * nB);
-    L.delta = take(4 * d * nB);
-    L.rho = take(4 * d * nB);
-    L.lam = take(4 * (size_t)B);
-    L.F = take(4 * (size_t)B);
-    L.Fp = take(4 * (size_t)B);
-    L.Fd = take(4 * (size_t)B);
-    L.its = take(4 * (size_t)B);
-    L.mask = take(8 * (size_t)B);
-    L.sel = take(4 * (size_t)B);
-    L.ok = take(4 * (size_t)B);
+    L.tp = take(4 * 3 * nS);
+    L.tq = take(4 * 4 * nS);
+    L.q = take(4 * 2 * d * nS);
+    L.Ag = take(4 * 2 * (NA + d) * nS);
+    L.cst = take(4 * 2 * 2 * nS);
+    L.V = take(4 * NA * nS);
+    L.z = take(4 * d * nS);
+    L.delta = take(4 * d * nS);
+    L.rho = take(4 * d * nS);
+    L.lam = take(4 * Bp);
+    L.F = take(4 * Bp);
+    L.Fp = take(4 * Bp);
+    L.Fd = take(4 * Bp);
+    L.its = take(4 * Bp);
+    L.mask = take(8 * Bp);
+    L.sel = take(4 * Bp);
+    L.ok = take(4 * Bp);
     L.totals = take(16);
-    L.ui = take(4 * (size_t)B);
-    L.us = take(4 * (size_t)B);
+    L.ui = take(4 * Bp);
+    L.us = take(4 * Bp);
     L.total = off;
     return L;
 }
 
 cudaError_t launch_pose(lm_ctx *c, int which, const TArgs &a) {
     launch_counter().fetch_add(1);
-    const unsigned block = 128, grid = (unsigned)((a.nB + block - 1) / block);
+    const unsigned block = 128, grid = (unsigned)((a.nS + block - 1) / block);
     const bool weighted = c->args.weighted != 0;
     if (c->spec_id != SPEC_GENERIC && !c->use_generic)
         return launch_traj_pose_spec(which, c->spec_id, weighted, grid, block, c->stream, a);
@@ -57,11 +57,9 @@ cudaError_t launch_pose(lm_ctx *c, int which, const TArgs &a) {
 
 cudaError_t launch_plain(lm_ctx *c, int which, const TArgs &a) {
     launch_counter().fetch_add(1);
-    if (which == TK_SOLVE) {
-        const unsigned block = 32, grid = (unsigned)((a.B + block - 1) / block);
-        return launch_traj_plain(which, c->dof, grid, block, c->stream, a);
-    }
-    const unsigned block = 256, grid = (unsigned)((a.nB + block - 1) / block);
+    if (which == TK_SOLVE_FACTOR || which == TK_SOLVE_REFINE) // one warp per tile of 32 trajectories
+        return launch_traj_plain(which, c->dof, (unsigned)a.Bt, 32, c->stream, a);
+    const unsigned block = 256, grid = (unsigned)((a.nS + block - 1) / block);
     return launch_traj_plain(which, c->dof, grid, block, c->stream, a);
 }
 
@@ -127,16 +125,16 @@ int lm_traj_attach(lm_ctx *c, const lm_traj_params *p, void *workspace, size_t b
     a.wd4 = a.wd2 * a.wd2;
     a.nu_up = p->nu_up; a.inv_nu_down = (float)(1.0 / (double)p->nu_down);
     a.lambda_min = p->lambda_min; a.lambda_max = p->lambda_max;
-    a.B = c->B; a.n = (int32_t)c->n; a.nB = c->W;
+    a.B = c->B; a.n = (int32_t)c->n; a.Bt = (c->B + 31) / 32; a.nS = a.Bt * 32 * c->n;
     a.shared_targets = c->shared;
     a.max_total = LM_MAX_ITERS;
     auto f = [&](size_t off) { return reinterpret_cast<float *>(t.ws + off); };
-    if (c->shared) { // one path for all trajectories: the w-order arrays [.][n] are already what e-order needs
+    if (c->shared) { // one path for all trajectories: the plain arrays [.][n] are read by waypoint index
         a.tp = c->args.tp; a.tq = c->args.tq;
     } else {
-        a.tp = f(L.tp); a.tq = f(L.tq);
+        a.tp = a.tp_w = f(L.tp); a.tq = a.tq_w = f(L.tq);
     }
-    a.q = f(L.q); a.A = f(L.A); a.gp = f(L.gp); a.cst = f(L.cst); a.V = f(L.V); a.z = f(L.z);
+    a.q = f(L.q); a.Ag = f(L.Ag); a.cst = f(L.cst); a.V = f(L.V); a.z = f(L.z);
     a.delta = f(L.delta); a.rho = f(L.rho); a.lam = f(L.lam); a.F = f(L.F); a.Fp = f(L.Fp); a.Fd = f(L.Fd);
     a.its = reinterpret_cast<uint32_t *>(t.ws + L.its);
     a.mask = reinterpret_cast<unsigned long long *>(t.ws + L.mask);
@@ -156,7 +154,7 @@ int lm_traj_reset(lm_ctx *c, const float *lambda) {
         lam_dev = t.args.rho;
     }
     launch_counter().fetch_add(1);
-    tl_reset_kernel<<<(unsigned)((c->B + 255) / 256), 256, 0, c->stream>>>(t.args, lam_dev, t.lambda0);
+    tl_reset_kernel<<<(unsigned)((t.args.Bt * 32 + 255) / 256), 256, 0, c->stream>>>(t.args, lam_dev, t.lambda0);
     LM_CUDA(cudaGetLastError());
     return LM_OK;
 }
@@ -184,19 +182,17 @@ int lm_traj_run(lm_ctx *c, int32_t iters) {
     LM_CUDA(launch_plain(c, TK_PACK_Q, a));
     LM_CUDA(launch_pose(c, TK_ASSEMBLE, a));
     launch_counter().fetch_add(1);
-    tl_init_cost_kernel<<<(unsigned)((c->B + 127) / 128), 128, 0, c->stream>>>(a);
+    tl_init_cost_kernel<<<(unsigned)a.Bt, TL_SUM_WARPS * 32, 0, c->stream>>>(a);
     LM_CUDA(cudaGetLastError());
     for (int it = 0; it < iters; ++it) {
-        a.mode = 0;
-        LM_CUDA(launch_plain(c, TK_SOLVE, a));
+        LM_CUDA(launch_plain(c, TK_SOLVE_FACTOR, a));
         for (int r = 0; r < t.refine; ++r) {
             LM_CUDA(launch_pose(c, TK_RHO, a));
-            a.mode = 1;
-            LM_CUDA(launch_plain(c, TK_SOLVE, a));
+            LM_CUDA(launch_plain(c, TK_SOLVE_REFINE, a));
         }
         LM_CUDA(launch_pose(c, TK_TRIAL, a));
         launch_counter().fetch_add(1);
-        tl_decide_kernel<<<(unsigned)((c->B + 127) / 128), 128, 0, c->stream>>>(a);
+        tl_decide_kernel<<<(unsigned)a.Bt, TL_SUM_WARPS * 32, 0, c->stream>>>(a);
         LM_CUDA(cudaGetLastError());
     }
     LM_CUDA(launch_plain(c, TK_UNPACK, a));

@@ -7,7 +7,7 @@
 namespace lmk {
 
 enum TrajPoseKernel : int { TK_ASSEMBLE = 0, TK_RHO = 1, TK_TRIAL = 2 };
-enum TrajPlainKernel : int { TK_PACK_Q = 0, TK_PACK_TARGETS = 1, TK_UNPACK = 2, TK_SOLVE = 3 };
+enum TrajPlainKernel : int { TK_PACK_Q = 0, TK_PACK_TARGETS = 1, TK_UNPACK = 2, TK_SOLVE_FACTOR = 3, TK_SOLVE_REFINE = 4 };
 
 // kernels that evaluate FK (chain-structure specialised or generic), thread per waypoint
 cudaError_t launch_traj_pose_spec(int which, int spec_id, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
@@ -42,7 +42,20 @@ cudaError_t launch_traj_plain_t(int which, unsigned grid, unsigned block, cudaSt
     case TK_PACK_Q: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 0); break;
     case TK_PACK_TARGETS: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 1); break;
     case TK_UNPACK: tl_unpack_kernel<D><<<grid, block, 0, s>>>(a); break;
-    case TK_SOLVE: tl_solve_kernel<D><<<grid, block, 0, s>>>(a); break;
+    case TK_SOLVE_FACTOR: { // one warp per tile of 32 trajectories; the ring needs more than the default 48 KB
+        static const cudaError_t once = cudaFuncSetAttribute(tl_solve_kernel<D, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                             (int)tl_solve_smem_bytes<D, 0>());
+        if (once != cudaSuccess) return once;
+        tl_solve_kernel<D, 0><<<grid, 32, tl_solve_smem_bytes<D, 0>(), s>>>(a);
+        break;
+    }
+    case TK_SOLVE_REFINE: {
+        static const cudaError_t once = cudaFuncSetAttribute(tl_solve_kernel<D, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                             (int)tl_solve_smem_bytes<D, 1>());
+        if (once != cudaSuccess) return once;
+        tl_solve_kernel<D, 1><<<grid, 32, tl_solve_smem_bytes<D, 1>(), s>>>(a);
+        break;
+    }
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
