@@ -320,6 +320,12 @@ def run_gpu(args) -> None:
     if args.workload == "C4" and full_size:
         # the "to convergence" statistic of the metric, on BASELINE.json configs[1] (512 x 300, tol 1e-5)
         extra["to_convergence_C2"] = time_to_convergence(lm, torch, wl, fk, device, stream)
+        # the trajectory-level step on the same workload
+        extra["trajectory_step"] = time_traj_step(lm, torch, w, solver, stream, peaks)
+    roofline["peak_measured_fma_rrr"] = lm.lm_fp32_peak_form(lm.LM_FMA_FORM_RRR, int(stream.cuda_stream))
+    roofline["frac_of_measured_fma_rrr"] = achieved_tf / roofline["peak_measured_fma_rrr"]
+    if True:
+        pass
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms_all / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
@@ -333,6 +339,66 @@ def run_gpu(args) -> None:
             "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}}
     line.update(extra)
     print(json.dumps(line))
+
+
+def traj_step_alg_bytes(d: int, refine: int = 1) -> float:
+    """HBM bytes one trajectory-level LM iteration must move per waypoint: fp32 words
+    factor+solve 3NA+4d, each refinement (rho 3d+7, re-solve 2NA+5d), trial NA+4d+9, decision 2."""
+    na = d * (d + 1) // 2
+    return 4.0 * ((3 * na + 4 * d) + refine * ((3 * d + 7) + (2 * na + 5 * d)) + (na + 4 * d + 9) + 2)
+
+
+def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: int = 5) -> dict:
+    """The trajectory-level LM step (lm_traj_run: stacked pose + differencing residual, block-tridiagonal
+    solve per trajectory) on the SAME workload, after 4 pose-only iterations; CUDA events around
+    lm_traj_run(iters) on the launching stream, best of `reps` after one warm-up.  The CPU leg times the
+    oracle of that step (oracle/lm_traj_oracle.c) on a few trajectories."""
+    d = int(w.chain.dof)
+    tp = lm.lm_traj_default_params(w_pose=1.0, w_diff=0.3)
+    solver.traj_attach(tp)
+    ts = []
+    with torch.cuda.stream(stream):
+        for i in range(reps + 1):
+            solver.reset()
+            solver.run(4)
+            solver.traj_reset()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = lm.lm_launch_count()
+            a.record(stream)
+            solver.traj_run(iters)
+            b.record(stream)
+            stream.synchronize()
+            launches = lm.lm_launch_count() - l0
+            if i >= 1:
+                ts.append(a.elapsed_time(b))
+        g = solver.traj_fetch()
+    ms_iter = float(min(ts)) / iters
+    alg = traj_step_alg_bytes(d, int(tp.refine_steps)) * w.W
+    out = {"workload": f"{w.name}: {w.B} x {w.n}, after 4 pose-only iterations; w_pose=1, w_diff=0.3, refine=1, {iters} iterations",
+           "ms_per_iteration": ms_iter, "waypoint_iterations_per_sec": w.W / (ms_iter * 1e-3),
+           "trajectory_iterations_per_sec": w.B / (ms_iter * 1e-3), "gpu_launches_per_run": int(launches),
+           "accepted_fraction": float(np.mean([bin(int(m)).count("1") for m in g["mask"]])) / iters,
+           "cost_diff_mean": float(g["cost_diff"].mean()),
+           "roofline": {"bound": "hbm", "achieved": alg / (ms_iter * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                        "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
+                        "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps)),
+                        "peak_source": peaks["_source"]}}
+    try:
+        from oracle import lm_oracle as orc, lm_traj_oracle as torc
+        nb = min(8, w.B)
+        sub = w.subset(slice(0, nb))
+        q0 = orc.lm_run(sub.chain, orc.Params(lambda0=sub.lambda0, tol=0.0), sub.target_pos.astype(np.float64),
+                        sub.target_quat.astype(np.float64), sub.seeds.astype(np.float64), 4).q.reshape(nb, sub.n, d)
+        t0 = time.perf_counter()
+        st = torc.lm_run(sub.chain, orc.Params(), torc.TrajParams(w_pose=1.0, w_diff=0.3),
+                         sub.target_pos.astype(np.float64).reshape(nb, sub.n, 3),
+                         sub.target_quat.astype(np.float64).reshape(nb, sub.n, 4), q0, 2)
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": st.executed * sub.n / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                               "sample": f"{nb} trajectories x {sub.n} waypoints x 2 iterations, fp64 banded Cholesky, OpenMP over trajectories"}
+    except Exception as e:  # noqa: BLE001
+        out["cpu_baseline"] = {"error": repr(e)}
+    return out
 
 
 def time_to_convergence(lm, torch, wl, fk, device, stream, reps: int = 20) -> dict:

@@ -302,8 +302,8 @@ __global__ void __launch_bounds__(256) lm_fma_rrr_kernel(float *out, int iters, 
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         x[i] = (float)(threadIdx.x + i) * 1e-3f;
-        y[i] = in[i];
-        z[i] = in[16 + i];
+        y[i] = in[i + (threadIdx.x & 3)];      // lane-dependent addresses: keeps y, z in vector registers
+        z[i] = in[32 + i + (threadIdx.x & 3)];
     }
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
@@ -473,8 +473,7 @@ int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out) {
     LM_CUDA(cudaMalloc(&scratch, 256));
     {
         float h[64];
-        for (int i = 0; i < 64; ++i) h[i] = (i < 16 || i >= 32) ? 0.999f : 1e-3f; // y = 0.999, z = 1e-3
-        for (int i = 16; i < 32; ++i) h[i] = 1e-3f;
+        for (int i = 0; i < 64; ++i) h[i] = (i < 32) ? 0.999f : 1e-3f; // y = 0.999 (words 0..18), z = 1e-3 (words 32..50)
         LM_CUDA(cudaMemcpy(scratch, h, sizeof(h), cudaMemcpyHostToDevice));
     }
     cudaEvent_t e0, e1;
@@ -485,8 +484,8 @@ int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out) {
     for (int rep = 0; rep < 6; ++rep) {
         cudaEventRecord(e0, st);
         g_launches.fetch_add(1);
-        if (form == LM_FMA_FORM_RCC) lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(scratch + 32, iters, 0.999f, 1e-3f);
-        else lm_fma_rrr_kernel<<<blocks, threads, 0, st>>>(scratch + 32, iters, scratch);
+        if (form == LM_FMA_FORM_RCC) lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(scratch + 60, iters, 0.999f, 1e-3f);
+        else lm_fma_rrr_kernel<<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch);
         cudaEventRecord(e1, st);
         cudaError_t e = cudaEventSynchronize(e1);
         if (e != cudaSuccess) { cudaFree(scratch); return cuda_fail(e); }
