@@ -293,40 +293,57 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
-constexpr int TL_STAGES = 8; // waypoints in flight per warp in the solve kernel
+constexpr int TL_STAGES = 6; // waypoints in flight per warp in the solve kernel
 
-// One ring stage (floats): [0, NA*32) matrix, then vector 1 (D*32), then vector 2 (D*32).
-// MODE 0 keeps two rings (one per Ag buffer: accept / reject is per trajectory, so the lanes of a
-// tile may select different buffers; a buffer no lane of the tile selects is not fetched).
-template <int D> __host__ __device__ constexpr int tl_stage_floats() { return (Tri<D>::NA + 2 * D) * 32; }
+// One ring stage (floats): [0, NA*32) matrix, then vector 1 (D*32) and, in MODE 1, vector 2 (D*32).
+// Each of the two warps of a block has its own rings; MODE 0 keeps two per warp (one per Ag buffer:
+// accept / reject is per trajectory, so the lanes of a tile may select different buffers; a
+// buffer no lane of the tile selects is not fetched).
+template <int D, int MODE> __host__ __device__ constexpr int tl_stage_floats() { return (Tri<D>::NA + (MODE == 0 ? D : 2 * D)) * 32; }
 template <int D, int MODE> __host__ __device__ constexpr size_t tl_solve_smem_bytes() {
-    return (size_t)(MODE == 0 ? 2 : 1) * TL_STAGES * tl_stage_floats<D>() * sizeof(float);
+    return (size_t)2 * (MODE == 0 ? 2 : 1) * TL_STAGES * tl_stage_floats<D, MODE>() * sizeof(float);
 }
 
-// ---- block-tridiagonal solve: one warp per tile of 32 trajectories, lane = trajectory
+// ---- block-tridiagonal solve: one block of TWO warps per tile of 32 trajectories, lane = trajectory.
+// Two-sided ("twisted") block elimination halves the sequential chain: with m = n / 2,
+//   warp 0 eliminates i = 0, 1, .., m-1      (S_i = T_i - w_d^4 S_{i-1}^-1,  h_i = g_i + w_d^2 z_{i-1}),
+//   warp 1 eliminates i = n-1, n-2, .., m+1  (S_i = T_i - w_d^4 S_{i+1}^-1,  h_i = g_i + w_d^2 z_{i+1}),
+//   z_i = S_i^-1 h_i; they meet at the middle block
+//   S_m = T_m - w_d^4 (S_{m-1}^-1 + S_{m+1}^-1),  x_m = S_m^-1 (g_m + w_d^2 (z_{m-1} + z_{m+1})),
+// and both substitute outwards from x_m:  x_i = z_i + w_d^2 S_i^-1 x_{i+-1}.
 //   MODE 0: factor (stores W_i = -S_i^-1) and solve for g;                      delta  = -x
 //   MODE 1: re-solve with the stored W_i for rho (iterative refinement);        delta +=  x
-// The chunks of the next TL_STAGES waypoints are in flight (bulk-async copies into the ring)
-// while waypoint i is being eliminated.
+// The chunks of the next TL_STAGES waypoints of a warp's sequence are in flight (bulk-async copies
+// into its ring) while it eliminates the current one.
 template <int D, int MODE>
-__global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TArgs A) {
-    constexpr int NA = Tri<D>::NA, CA = NA + D, SF = tl_stage_floats<D>();
-    extern __shared__ __align__(128) float ring[];
-    __shared__ __align__(8) uint64_t bars[TL_STAGES];
-    const int lane = threadIdx.x;
+__global__ void __launch_bounds__(64) tl_solve_kernel(const __grid_constant__ TArgs A) {
+    constexpr int NA = Tri<D>::NA, CA = NA + D, SF = tl_stage_floats<D, MODE>(), NR = (MODE == 0) ? 2 : 1;
+    extern __shared__ __align__(128) float smem[];
+    __shared__ __align__(8) uint64_t bars_all[2][TL_STAGES];
+    __shared__ float xch[NA + D][32]; // warp 1 -> warp 0: W_{m+1}, z_{m+1}
+    __shared__ float xmid[D][32];     // warp 0 -> both: x_m
+    __shared__ int okx[2][32];
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
     const int64_t bt = blockIdx.x;
     const int64_t b = bt * 32 + lane;
     const bool valid = b < A.B;
     const uint32_t pk = valid ? A.its[b] : 0xffu;
     const bool active = valid && ((pk & 0xffu) < (uint32_t)A.max_total) && (MODE == 0 || A.ok[b] != 0);
-    if (!__any_sync(0xffffffffu, active)) return;
+    if (!__any_sync(0xffffffffu, active)) return; // the same lanes in both warps: block-uniform
     const int sel = valid ? A.sel[b] : 0;
     const bool need0 = __any_sync(0xffffffffu, active && sel == 0); // warp-uniform
     const bool need1 = __any_sync(0xffffffffu, active && sel == 1);
     const int n = A.n;
     const int64_t w0 = bt * n;
     const float lam = valid ? A.lam[b] : 1.f;
+    float *ring = smem + (size_t)wp * NR * TL_STAGES * SF;
     float *ring1 = ring + (size_t)TL_STAGES * SF; // MODE 0 only: chunks of Ag buffer 1
+    uint64_t *bars = bars_all[wp];
+
+    const int m = n / 2;
+    const int len = (wp == 0) ? m : n - 1 - m;  // waypoints this warp eliminates
+    const int uses1 = len + (wp == 0 ? 1 : 0);  // ring uses of the elimination phase (warp 0 also fetches chunk m)
+    auto idx = [&](int k) { return wp == 0 ? k : n - 1 - k; }; // k-th waypoint of this warp's sequence (idx(m) = m for warp 0)
 
     if (lane == 0) {
 #pragma unroll
@@ -335,9 +352,9 @@ __global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TA
     }
     __syncwarp();
 
-    auto issue_fwd = [&](int k, int i) { // lane 0 only; k = position in the sequence of ring uses
+    auto issue_fwd = [&](int k) { // lane 0 only; k = position in this warp's sequence of ring uses
         const int s = k % TL_STAGES;
-        const int64_t wid = w0 + i;
+        const int64_t wid = w0 + idx(k);
         if (MODE == 0) {
             const uint32_t bytes = CA * 128u;
             mbar_expect_tx(&bars[s], (need0 ? bytes : 0u) + (need1 ? bytes : 0u));
@@ -350,8 +367,8 @@ __global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TA
             bulk_g2s(dst + NA * 32, A.rho + wid * D * 32, D * 128u, &bars[s]);
         }
     };
-    auto issue_bwd = [&](int k, int i) { // lane 0 only
-        const int s = k % TL_STAGES;
+    auto issue_bwd = [&](int kk, int i) { // lane 0 only
+        const int s = kk % TL_STAGES;
         float *dst = ring + (size_t)s * SF;
         const int64_t wid = w0 + i;
         mbar_expect_tx(&bars[s], (NA + D + (MODE == 1 ? D : 0)) * 128u);
@@ -361,7 +378,7 @@ __global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TA
     };
 
     if (lane == 0) {
-        for (int k = 0; k < TL_STAGES && k < n; ++k) issue_fwd(k, k);
+        for (int k = 0; k < TL_STAGES && k < uses1; ++k) issue_fwd(k);
     }
 
     float W[NA], zp[D];
@@ -372,10 +389,11 @@ __global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TA
     bool ok = true;
     const float *my_ring = (MODE == 0 && sel == 1) ? ring1 : ring;
 
-    // ---- forward elimination
-    for (int i = 0; i < n; ++i) {
-        const int s = i % TL_STAGES;
-        mbar_wait(&bars[s], (uint32_t)((i / TL_STAGES) & 1));
+    // one elimination step on the chunk in stage k of this warp's ring; `Wo`, `zo`: the contribution of the
+    // other side (only at the middle block), zero otherwise
+    auto eliminate = [&](int k, int i, const float (&Wo)[NA], const float (&zo)[D], bool middle) {
+        const int s = k % TL_STAGES;
+        mbar_wait(&bars[s], (uint32_t)((k / TL_STAGES) & 1));
         const float *st = my_ring + (size_t)s * SF;
         float S[NA], rhs[D];
 #pragma unroll
@@ -383,16 +401,20 @@ __global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TA
 #pragma unroll
         for (int r = 0; r < D; ++r) rhs[r] = st[(NA + r) * 32 + lane];
         __syncwarp(); // every lane has read the stage: it may be refilled (the copy lands long after these loads)
-        if (lane == 0 && i + TL_STAGES < n) issue_fwd(i + TL_STAGES, i + TL_STAGES);
+        if (lane == 0 && k + TL_STAGES < uses1) issue_fwd(k + TL_STAGES);
         const int64_t wid = w0 + i;
         if (MODE == 0) {
             const float ci = (n == 1) ? 0.f : ((i == 0 || i == n - 1) ? 1.f : 2.f);
             const float dg = fma_(ci, A.wd2, lam);
 #pragma unroll
             for (int r = 0; r < D; ++r) S[tri(r, r)] = add(S[tri(r, r)], dg);
-            // S_i = T_i - w_d^4 S_{i-1}^-1 = T_i + w_d^4 W_{i-1}
+            // S_i = T_i - w_d^4 S_prev^-1 = T_i + w_d^4 W_prev (+ the other side's at the middle)
 #pragma unroll
             for (int t = 0; t < NA; ++t) S[t] = fma_(A.wd4, W[t], S[t]);
+            if (middle) {
+#pragma unroll
+                for (int t = 0; t < NA; ++t) S[t] = fma_(A.wd4, Wo[t], S[t]);
+            }
             ok = sweep_neg_inverse<D>(S) && ok;
             if (active) {
 #pragma unroll
@@ -401,47 +423,72 @@ __global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TA
         }
 #pragma unroll
         for (int t = 0; t < NA; ++t) W[t] = S[t];
-        // h_i = rhs_i + w_d^2 z_{i-1};  z_i = S_i^-1 h_i = -(W_i h_i)
+        // h_i = rhs_i + w_d^2 z_prev;  z_i = S_i^-1 h_i = -(W_i h_i)
         float h[D], y[D];
 #pragma unroll
-        for (int r = 0; r < D; ++r) h[r] = fma_(A.wd2, zp[r], rhs[r]);
+        for (int r = 0; r < D; ++r) {
+            h[r] = fma_(A.wd2, zp[r], rhs[r]);
+            if (middle) h[r] = fma_(A.wd2, zo[r], h[r]);
+        }
         symv<D>(W, h, y);
 #pragma unroll
         for (int r = 0; r < D; ++r) zp[r] = -y[r];
-        if (active) {
+        if (active && !middle) {
 #pragma unroll
             for (int r = 0; r < D; ++r) A.z[toff<D>(wid, r, lane)] = zp[r];
         }
-    }
+    };
 
-    // the chunks written above are read back by bulk-async copies: order the generic writes before them
-    __threadfence();
-    __syncwarp();
-    fence_proxy_async();
-    __syncwarp();
-
-    // ---- back substitution: x_n = z_n, x_i = z_i + w_d^2 S_i^-1 x_{i+1} = z_i - w_d^2 W_i x_{i+1}
-    if (lane == 0) {
-        for (int j = 0; j < TL_STAGES && n - 2 - j >= 0; ++j) issue_bwd(n + j, n - 2 - j);
-    }
-    float x[D];
-    float amax = 0.f;
+    // ---- elimination from both ends
     {
-        const int64_t wid = w0 + n - 1;
+        float Wz[NA], zz[D];
+#pragma unroll
+        for (int t = 0; t < NA; ++t) Wz[t] = 0.f;
+#pragma unroll
+        for (int r = 0; r < D; ++r) zz[r] = 0.f;
+        for (int k = 0; k < len; ++k) eliminate(k, idx(k), Wz, zz, false);
+    }
+    if (wp == 1) { // hand W_{m+1}, z_{m+1} (zeros when this warp had nothing to eliminate) to warp 0
+#pragma unroll
+        for (int t = 0; t < NA; ++t) xch[t][lane] = W[t];
+#pragma unroll
+        for (int r = 0; r < D; ++r) xch[NA + r][lane] = zp[r];
+    }
+    __syncthreads();
+    float amax = 0.f;
+    if (wp == 0) { // the middle block: x_m
+        float Wo[NA], zo[D];
+#pragma unroll
+        for (int t = 0; t < NA; ++t) Wo[t] = xch[t][lane];
+#pragma unroll
+        for (int r = 0; r < D; ++r) zo[r] = xch[NA + r][lane];
+        eliminate(len, m, Wo, zo, true);
+        const int64_t wid = w0 + m;
 #pragma unroll
         for (int r = 0; r < D; ++r) {
-            x[r] = zp[r];
-            float dv;
-            if (MODE == 0) dv = -x[r];
-            else dv = add(active ? A.delta[toff<D>(wid, r, lane)] : 0.f, x[r]);
+            xmid[r][lane] = zp[r];
+            const float dv = (MODE == 0) ? -zp[r] : add(active ? A.delta[toff<D>(wid, r, lane)] : 0.f, zp[r]);
             if (active) A.delta[toff<D>(wid, r, lane)] = dv;
             amax = fmaxf(amax, fabsf(dv));
         }
     }
-    for (int i = n - 2; i >= 0; --i) {
-        const int k = n + (n - 2 - i);
-        const int s = k % TL_STAGES;
-        mbar_wait(&bars[s], (uint32_t)((k / TL_STAGES) & 1));
+    // the chunks written above are read back by bulk-async copies: order the generic writes before them
+    __threadfence();
+    fence_proxy_async();
+    __syncthreads();
+
+    // ---- substitution outwards from the middle: x_i = z_i + w_d^2 S_i^-1 x_next = z_i - w_d^2 W_i x_next
+    if (lane == 0) {
+        for (int j = 0; j < TL_STAGES && j < len; ++j) issue_bwd(uses1 + j, idx(len - 1 - j));
+    }
+    float x[D];
+#pragma unroll
+    for (int r = 0; r < D; ++r) x[r] = xmid[r][lane];
+    for (int j = 0; j < len; ++j) {
+        const int kk = uses1 + j;
+        const int s = kk % TL_STAGES;
+        const int i = idx(len - 1 - j);
+        mbar_wait(&bars[s], (uint32_t)((kk / TL_STAGES) & 1));
         const float *st = ring + (size_t)s * SF;
         float zi[D], dold[D];
 #pragma unroll
@@ -452,7 +499,7 @@ __global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TA
             dold[r] = (MODE == 1) ? st[(NA + D + r) * 32 + lane] : 0.f;
         }
         __syncwarp();
-        if (lane == 0 && i - TL_STAGES >= 0) issue_bwd(k + TL_STAGES, i - TL_STAGES);
+        if (lane == 0 && j + TL_STAGES < len) issue_bwd(kk + TL_STAGES, idx(len - 1 - j - TL_STAGES));
         float y[D];
         symv<D>(W, x, y);
         const int64_t wid = w0 + i;
@@ -465,9 +512,12 @@ __global__ void __launch_bounds__(32) tl_solve_kernel(const __grid_constant__ TA
         }
     }
     ok = ok && (amax < 1e30f); // NaN compares false
-    if (active) {
-        if (MODE == 0) A.ok[b] = ok ? 1 : 0;
-        else if (!ok) A.ok[b] = 0;
+    okx[wp][lane] = ok ? 1 : 0;
+    __syncthreads();
+    if (wp == 0 && active) {
+        const bool both = okx[0][lane] && okx[1][lane];
+        if (MODE == 0) A.ok[b] = both ? 1 : 0;
+        else if (!both) A.ok[b] = 0;
     }
 }
 
