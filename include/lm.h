@@ -225,6 +225,53 @@ int lm_traj_fetch(lm_ctx *ctx, lm_traj_stats *stats_out);
  * trial_q [d][W] (w-order) = the clamped trial point and trial_F [2][B] = (|r|^2 before, at the trial point). */
 int lm_traj_set_trace(lm_ctx *ctx, float *trial_q, float *trial_F);
 
+/* ------------------------------------------------------------------------------------------------
+ * Non-stationary schedule with anytime bookkeeping:
+ * "the optimizer optimizes for pose error exclusively until the positional and rotational error ...
+ * is below the respective specified threshold at every timestep.  A trajectory length ... optimization
+ * step is then taken, after which the optimizer switches back to pose only, and the cycle continues";
+ * "The optimizer keeps track of the latest valid solution".
+ *
+ * One cycle = [pose-only phase: per-waypoint LM state reset (lambda0, 0 iterations), lm_run(pose_iters)]
+ *           -> [record: a trajectory is VALID when every waypoint has pos err < pos_tol and rot err < rot_tol
+ *                and no joint moves more than mjac_rev / mjac_pris across a timestep
+ *               (PAPER.md:L53); valid trajectories are copied to the "latest valid" slot with their length
+ *               sum_i sum_j |q_{i+1}[j] - q_i[j]|]
+ *           -> [ONE trajectory-level LM iteration (lm_traj_*) for the trajectories that are pose-valid now].
+ * lm_plan_run(cycles) runs `cycles` such cycles and then one more pose-only phase + record; everything is
+ * enqueued on the stream, no host round trip (readings P1-P4).
+ * Requires lm_traj_attach.  The freeze tolerance of the pose phase is lm_params.tol.
+ */
+typedef struct {
+    float pos_tol;      /* 1e-4 m (0.1 mm) */
+    float rot_tol;      /* 0.1 deg in rad */
+    float mjac_rev;     /* 7 deg in rad */
+    float mjac_pris;    /* 0.02 m */
+    int32_t pose_iters; /* cap of each pose-only phase, 1..64 (default 10) */
+} lm_plan_params;
+
+/* lm_plan_fetch outputs; every pointer nullable, device or host. */
+typedef struct {
+    uint8_t *valid;             /* [B] a valid trajectory has been recorded */
+    int32_t *first_valid_cycle; /* [B] cycle of the first record (0 = after the first pose phase), -1 = never */
+    int32_t *records;           /* [B] number of records */
+    float *length;              /* [B] trajectory length of the recorded trajectory (NaN if none) */
+    float *max_pos_err, *max_rot_err; /* [B] of the CURRENT trajectory at the last record point */
+    float *mjac_rev, *mjac_pris;      /* [B] likewise */
+    float *cur_length;                /* [B] likewise */
+    int64_t valid_trajectories;       /* OUT */
+} lm_plan_stats;
+
+size_t lm_plan_workspace_bytes(int32_t dof, int64_t B, int64_t n);
+int lm_plan_default_params(lm_plan_params *out);
+/* Bind a caller-owned device workspace (256-byte aligned, borrowed until lm_free); clears the bookkeeping. */
+int lm_plan_attach(lm_ctx *ctx, const lm_plan_params *params, void *workspace, size_t workspace_bytes);
+/* Clears the bookkeeping and the trajectory-level LM state, then runs the schedule from the context's
+ * current joint values.  cycles 0..64.  Async. */
+int lm_plan_run(lm_ctx *ctx, int32_t cycles);
+/* Synchronise; q_valid_out [d][W] (device or host, nullable) = latest valid trajectories (NaN where none). */
+int lm_plan_fetch(lm_ctx *ctx, float *q_valid_out, lm_plan_stats *stats_out);
+
 /* Measure the FP32 FMA throughput of the current device with an FMA-only micro-kernel (16 independent
  * chains per thread, best of 5 timed launches, CUDA events on `cuda_stream`); blocks the host.
  * tflops_out: 2 * FFMA / s / 1e12.  The measured counterpart of the ALU roofline. */

@@ -239,6 +239,7 @@ int iterate(lm_ctx *c, int max_total, int at_most) {
 namespace lmk {
 int materialize_state(lm_ctx *c) { return c->fresh ? iterate(c, 0, 0) : LM_OK; }
 int refresh_waypoint_outputs(lm_ctx *c) { return iterate(c, LM_MAX_ITERS, 0); }
+int run_pose_phase(lm_ctx *c, int max_iters) { return iterate(c, max_iters, INT_MAX); }
 } // namespace lmk
 
 namespace {
@@ -394,6 +395,20 @@ int lm_set_state(lm_ctx *c, const float *q, const float *lambda) {
     c->fresh = false;
     return LM_OK;
 }
+
+} // extern "C"
+
+namespace lmk {
+int reset_waypoint_lm_state(lm_ctx *c) {
+    const unsigned grid = (unsigned)((c->W + 255) / 256);
+    g_launches.fetch_add(1);
+    lm_fill_state_kernel<<<grid, 256, 0, c->stream>>>(c->args.lam, c->args.its, c->args.mask, c->W, c->args.lambda0, 1);
+    LM_CUDA(cudaGetLastError());
+    return LM_OK;
+}
+} // namespace lmk
+
+extern "C" {
 
 int lm_fk(lm_ctx *c, const float *q, int64_t count, float *pos, float *rot) {
     if (!c || !q || !pos || !rot || count <= 0) return LM_EINVAL;

@@ -24,6 +24,18 @@ struct TrajState { // trajectory-level LM (lm_traj_*), bound by lm_traj_attach
     size_t off_totals = 0, off_ui = 0, off_us = 0;
 };
 
+struct PlanState { // non-stationary schedule + anytime bookkeeping (lm_plan_*), bound by lm_plan_attach
+    bool attached = false;
+    lm_plan_params prm{};
+    char *ws = nullptr;
+    float *q_valid = nullptr;                 // [d][W] w-order
+    float *cur = nullptr;                     // [5][B] max pos err, max rot err, mjac rev, mjac pris, length of the current trajectory
+    float *len_valid = nullptr;               // [B]
+    int32_t *gate = nullptr, *first = nullptr, *records = nullptr; // [B]
+    uint8_t *valid = nullptr;                 // [B]
+    unsigned long long *total = nullptr;
+};
+
 int cuda_fail(cudaError_t e);              // records the error string for lm_strerror, returns LM_ECUDA
 std::atomic<long long> &launch_counter();  // lm_launch_count
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
@@ -45,11 +57,14 @@ struct lm_ctx {
     int spec_id;      // structure-matched specialised kernel (lm_specs.cuh) or SPEC_GENERIC
     bool use_generic; // LM_OPT_GENERIC_KERNEL
     lmk::TrajState traj;
+    lmk::PlanState plan;
 };
 
 namespace lmk {
 int materialize_state(lm_ctx *c);        // if nothing has run yet: state := seeds (a zero-iteration launch)
-int refresh_waypoint_outputs(lm_ctx *c); // zero-iteration launch: re-evaluates |r|, errors, frozen flag at the current q
+int refresh_waypoint_outputs(lm_ctx *c);
+int reset_waypoint_lm_state(lm_ctx *c);  // lambda := lambda0, iters := 0, mask := 0 for every waypoint; q is kept
+int run_pose_phase(lm_ctx *c, int max_iters); // = lm_run // zero-iteration launch: re-evaluates |r|, errors, frozen flag at the current q
 }
 
 #define LM_CUDA(x)                                        \

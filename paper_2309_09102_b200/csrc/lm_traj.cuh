@@ -50,6 +50,7 @@ struct TArgs {
     unsigned long long *mask;
     int32_t *sel;                  // which of the two buffers holds the trajectory's current point
     int32_t *ok;                   // this iteration's solve succeeded
+    const int32_t *gate;           // nullable: only trajectories with gate[b] != 0 take the step (lm_plan_run)
     float *trace_q, *trace_F;      // nullable: trial point [D][W] in w-order (w = b n + i), (F, F+) [2][B]
     const float *src_q;            // pack: [D][W] w-order
     const float *src_tp, *src_tq;  // pack: [3][W], [4][W] w-order
@@ -328,7 +329,8 @@ __global__ void __launch_bounds__(64) tl_solve_kernel(const __grid_constant__ TA
     const int64_t b = bt * 32 + lane;
     const bool valid = b < A.B;
     const uint32_t pk = valid ? A.its[b] : 0xffu;
-    const bool active = valid && ((pk & 0xffu) < (uint32_t)A.max_total) && (MODE == 0 || A.ok[b] != 0);
+    const bool active = valid && ((pk & 0xffu) < (uint32_t)A.max_total) && (MODE == 0 || A.ok[b] != 0) &&
+                        (A.gate == nullptr || A.gate[b] != 0);
     if (!__any_sync(0xffffffffu, active)) return; // the same lanes in both warps: block-uniform
     const int sel = valid ? A.sel[b] : 0;
     const bool need0 = __any_sync(0xffffffffu, active && sel == 0); // warp-uniform
@@ -546,7 +548,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(c
             rd[u][j] = there ? A.delta[toff<D>(wid, j, s.lane)] : 0.f;
         }
     }
-    if ((pk & 0xffu) >= (uint32_t)A.max_total || !okf) return;
+    if ((pk & 0xffu) >= (uint32_t)A.max_total || !okf || (A.gate != nullptr && A.gate[s.b] == 0)) return;
     float q[D], dl[D], dd[D];
 #pragma unroll
     for (int j = 0; j < D; ++j) {
@@ -605,7 +607,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_trial_kernel
     }
     float pt[3], Rt[3][3];
     tl_load_target(A, s, pt, Rt);
-    if ((pk & 0xffu) >= (uint32_t)A.max_total) return;
+    if ((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0)) return;
     float *qd = A.q + (int64_t)(1 - sel) * D * A.nS;
     float qt[D], qm[D], qn[D];
     bool clamped = false;
@@ -648,7 +650,7 @@ __global__ void __launch_bounds__(TL_SUM_WARPS * 32) tl_decide_kernel(const __gr
     if (!valid || threadIdx.x >= 32) return;
     uint32_t pk = A.its[b];
     uint32_t k = pk & 0xffu, st = pk >> 8;
-    if (k >= (uint32_t)A.max_total) return;
+    if (k >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[b] == 0)) return;
     const bool ok = A.ok[b] != 0;
     const float F = A.F[b];
     if (A.trace_F != nullptr) { A.trace_F[b] = F; A.trace_F[A.B + b] = Ft; }

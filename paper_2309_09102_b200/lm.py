@@ -30,7 +30,8 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_option", "lm_kernel_name", "lm_fk", "lm_fp32_peak", "lm_free",
            "lm_strerror", "lm_launch_count", "lm_fp32_peak_form",
            "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
-           "lm_traj_fetch", "lm_traj_set_trace")
+           "lm_traj_fetch", "lm_traj_set_trace",
+           "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR = 0, 1
 
 
@@ -69,6 +70,18 @@ class LmTrajStats(C.Structure):
     _fields_ = [("cost", C.c_void_p), ("cost_pose", C.c_void_p), ("cost_diff", C.c_void_p),
                 ("lambda_", C.c_void_p), ("iters", C.c_void_p), ("accept_mask", C.c_void_p),
                 ("status", C.c_void_p), ("total_traj_iters", C.c_int64)]
+
+
+class LmPlanParams(C.Structure):
+    _fields_ = [("pos_tol", C.c_float), ("rot_tol", C.c_float), ("mjac_rev", C.c_float), ("mjac_pris", C.c_float),
+                ("pose_iters", C.c_int32)]
+
+
+class LmPlanStats(C.Structure):
+    _fields_ = [("valid", C.c_void_p), ("first_valid_cycle", C.c_void_p), ("records", C.c_void_p),
+                ("length", C.c_void_p), ("max_pos_err", C.c_void_p), ("max_rot_err", C.c_void_p),
+                ("mjac_rev", C.c_void_p), ("mjac_pris", C.c_void_p), ("cur_length", C.c_void_p),
+                ("valid_trajectories", C.c_int64)]
 
 
 class LmError(RuntimeError):
@@ -118,6 +131,12 @@ def lib() -> C.CDLL:
         L.lm_traj_reset.argtypes = [C.c_void_p, C.c_void_p]
         L.lm_traj_fetch.argtypes = [C.c_void_p, C.POINTER(LmTrajStats)]
         L.lm_traj_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lm_plan_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64]
+        L.lm_plan_workspace_bytes.restype = C.c_size_t
+        L.lm_plan_default_params.argtypes = [C.POINTER(LmPlanParams)]
+        L.lm_plan_attach.argtypes = [C.c_void_p, C.POINTER(LmPlanParams), C.c_void_p, C.c_size_t]
+        L.lm_plan_run.argtypes = [C.c_void_p, C.c_int32]
+        L.lm_plan_fetch.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(LmPlanStats)]
         _lib = L
     return _lib
 
@@ -257,6 +276,32 @@ def lm_traj_fetch(ctx: int, stats: LmTrajStats) -> None:
 
 def lm_traj_set_trace(ctx: int, trial_q_ptr: Optional[int], trial_F_ptr: Optional[int]) -> None:
     _check(lib().lm_traj_set_trace(ctx, trial_q_ptr, trial_F_ptr), "lm_traj_set_trace")
+
+
+def lm_plan_workspace_bytes(dof: int, B: int, n: int) -> int:
+    return int(lib().lm_plan_workspace_bytes(dof, B, n))
+
+
+def lm_plan_default_params(**overrides) -> LmPlanParams:
+    p = LmPlanParams()
+    _check(lib().lm_plan_default_params(C.byref(p)), "lm_plan_default_params")
+    for k, v in overrides.items():
+        if not hasattr(p, k):
+            raise AttributeError(k)
+        setattr(p, k, v)
+    return p
+
+
+def lm_plan_attach(ctx: int, params: LmPlanParams, workspace_ptr: int, workspace_bytes: int) -> None:
+    _check(lib().lm_plan_attach(ctx, C.byref(params), workspace_ptr, workspace_bytes), "lm_plan_attach")
+
+
+def lm_plan_run(ctx: int, cycles: int) -> None:
+    _check(lib().lm_plan_run(ctx, int(cycles)), "lm_plan_run")
+
+
+def lm_plan_fetch(ctx: int, q_valid_ptr: Optional[int], stats: Optional[LmPlanStats]) -> None:
+    _check(lib().lm_plan_fetch(ctx, q_valid_ptr, C.byref(stats) if stats is not None else None), "lm_plan_fetch")
 
 
 def lm_free(ctx: int) -> None:
@@ -421,6 +466,38 @@ class Solver:
             res["trial_q"] = np.ascontiguousarray(self.ttrace_q.cpu().numpy().T)
             tf = self.ttrace_F.cpu().numpy()
             res["F_before"], res["F_trial"] = tf[0], tf[1]
+        return res
+
+    # -- non-stationary schedule with anytime bookkeeping (include/lm.h, lm_plan_*)
+    def plan_attach(self, pparams: Optional[LmPlanParams] = None) -> None:
+        torch = self.torch
+        self.pparams = pparams if pparams is not None else lm_plan_default_params()
+        nbytes = lm_plan_workspace_bytes(self.d, self.B, self.n)
+        self.plan_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self.plan_workspace.data_ptr() + 255) // 256 * 256
+        lm_plan_attach(self._ctx, self.pparams, ptr, nbytes)
+
+    def plan_run(self, cycles: int) -> None:
+        lm_plan_run(self._ctx, cycles)
+
+    def plan_fetch(self) -> dict:
+        torch = self.torch
+        B = self.B
+
+        def buf(dtype):
+            return torch.empty((B,), dtype=dtype).pin_memory()
+
+        qv = torch.empty((self.d, self.W), dtype=torch.float32).pin_memory()
+        out = {"valid": buf(torch.uint8), "first_valid_cycle": buf(torch.int32), "records": buf(torch.int32),
+               "length": buf(torch.float32), "max_pos_err": buf(torch.float32), "max_rot_err": buf(torch.float32),
+               "mjac_rev": buf(torch.float32), "mjac_pris": buf(torch.float32), "cur_length": buf(torch.float32)}
+        st = LmPlanStats(*[out[k].data_ptr() for k in ("valid", "first_valid_cycle", "records", "length", "max_pos_err",
+                                                       "max_rot_err", "mjac_rev", "mjac_pris", "cur_length")], 0)
+        lm_plan_fetch(self._ctx, qv.data_ptr(), st)
+        res = {k: v.numpy().copy() for k, v in out.items()}
+        res["valid"] = res["valid"].astype(bool)
+        res["q_valid"] = np.ascontiguousarray(qv.numpy().T)
+        res["valid_trajectories"] = int(st.valid_trajectories)
         return res
 
     def fetch_totals(self) -> tuple:
