@@ -322,6 +322,8 @@ def run_gpu(args) -> None:
         extra["to_convergence_C2"] = time_to_convergence(lm, torch, wl, fk, device, stream)
         # the trajectory-level step on the same workload
         extra["trajectory_step"] = time_traj_step(lm, torch, w, solver, stream, peaks)
+        # the paper's alternating schedule with anytime bookkeeping (NEXT-2), valid trajectories per second
+        extra["schedule_C2"] = time_plan(lm, torch, wl, fk, device, stream)
     roofline["peak_measured_fma_rrr"] = lm.lm_fp32_peak_form(lm.LM_FMA_FORM_RRR, int(stream.cuda_stream))
     roofline["frac_of_measured_fma_rrr"] = achieved_tf / roofline["peak_measured_fma_rrr"]
     if True:
@@ -398,6 +400,40 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
                                "sample": f"{nb} trajectories x {sub.n} waypoints x 2 iterations, fp64 banded Cholesky, OpenMP over trajectories"}
     except Exception as e:  # noqa: BLE001
         out["cpu_baseline"] = {"error": repr(e)}
+    return out
+
+
+def time_plan(lm, torch, wl, fk, device, stream, cycles: int = 3, reps: int = 5) -> dict:
+    """The paper's schedule (lm_plan_run) on configs[1] (512 x 300, Panda): `cycles` x
+    [pose-only phase, record, one trajectory-level step] + a final pose phase and record.  Reports valid
+    trajectories (0.1 mm / 0.1 deg at every waypoint, no joint step above 7 deg) per second."""
+    w = wl.config2(fk)
+    prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol)
+    s = lm.Solver(w.chain, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, device=str(device), stream=stream)
+    s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=1.0))
+    s.plan_attach(lm.lm_plan_default_params(pose_iters=10))
+    out = {}
+    with torch.cuda.stream(stream):
+        for cyc in (0, cycles):
+            ts = []
+            for i in range(reps + 1):
+                s.set_state(w.seeds)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                l0 = lm.lm_launch_count()
+                a.record(stream)
+                s.plan_run(cyc)
+                b.record(stream)
+                stream.synchronize()
+                launches = lm.lm_launch_count() - l0
+                if i >= 1:
+                    ts.append(a.elapsed_time(b))
+            g = s.plan_fetch()
+            ms = float(min(ts))
+            out[f"cycles_{cyc}"] = {"ms": ms, "gpu_launches": int(launches), "valid_trajectories": g["valid_trajectories"],
+                                    "valid_trajectories_per_sec": g["valid_trajectories"] / (ms * 1e-3),
+                                    "mean_length_of_valid_rad": float(np.nanmean(g["length"])) if g["valid_trajectories"] else None}
+    s.close()
+    out["workload"] = f"C2: {w.B} x {w.n}, tol={w.tol:g}, pose_iters=10, w_pose=1, w_diff=1"
     return out
 
 
