@@ -58,8 +58,8 @@ __device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b);
 __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
 __device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 
-// sin and cos of x for |x| < ~1e4 (joint angles are bounded by the joint limits).
-// Cody-Waite reduction by pi/2 in three parts, then the classic single-precision minimax
+// sin and cos of x for |x| < ~100 (joint angles are bounded by the joint limits).
+// Cody-Waite reduction by pi/2 in two parts (FMA: the products are exact), then the classic single-precision minimax
 // polynomials on [-pi/4, pi/4]; max error ~1 ulp.  FAST: the MUFU approximations (abs err ~5e-7).
 template <bool FAST>
 __device__ __forceinline__ void sincos_(float x, float &s, float &c) {
@@ -71,9 +71,8 @@ __device__ __forceinline__ void sincos_(float x, float &s, float &c) {
     float t = fma_(x, 0.636619772f, magic);              // x * 2/pi
     int qd = __float_as_int(t);                          // quadrant in the low mantissa bits
     float j = sub(t, magic);
-    float r = fma_(j, -1.57079601e+00f, x);
-    r = fma_(j, -3.13916473e-07f, r);
-    r = fma_(j, -5.39030253e-15f, r);
+    float r = fma_(j, -1.57079601e+00f, x);   // pi/2 = 1.57079601 + 3.13916473e-07 + 5.4e-15: the third part moves r by
+    r = fma_(j, -3.13916473e-07f, r);         // < 2e-14 for the |j| <= 3 the joint limits allow and is dropped
     float r2 = mul(r, r);
     float ps = fma_(r2, -1.9515295891e-4f, 8.3321608736e-3f);
     ps = fma_(ps, r2, -1.6666654611e-1f);
@@ -146,13 +145,92 @@ __device__ __forceinline__ void log_near_pi(const float (&X)[3], const float (&Y
     for (int i = 0; i < 3; ++i) w[i] = mul(th, ax[i]);
 }
 
+// Entries of the Jacobian that the chain STRUCTURE fixes to exactly 0 or exactly 1 (unweighted):
+// bit 3 j + k of `zv` / `zw` = linear / angular component k of column j is 0, `ov` / `ow` likewise 1.
+//   joint 0 with alpha = 0: z_0 = e_z and o_0 on the z axis  => revolute: Jw_0 = (0,0,1), Jv_0[2] = 0;
+//                                                               prismatic: Jv_0 = (0,0,1), Jw_0 = 0
+//   joint 1 after such a joint 0: alpha = +-pi/2 => z_1 = -+Y_0 with Y_0[2] = 0; alpha = 0 => z_1 = e_z
+//   any prismatic joint: Jw_j = 0.
+// Terms with a known 0 are skipped and multiplications by a known 1 become additions in the dot
+// products below: the results equal the generic kernel's up to the sign of zero.
+struct JKnown { uint32_t zv, zw, ov, ow; };
+__host__ __device__ constexpr JKnown jknown(const ChainSpec S, bool weighted) {
+    JKnown K{0, 0, 0, 0};
+    if (S.generic) return K;
+    for (int j = 0; j < S.dof; ++j)
+        if ((S.pris >> j) & 1u) K.zw |= 7u << (3 * j);
+    const bool z0_ez = (S.al0 & 1u) != 0;
+    if (z0_ez) {
+        if (S.pris & 1u) { K.zv |= 3u; K.ov |= 4u; }
+        else { K.zw |= 3u; K.ow |= 4u; K.zv |= 4u; }
+        if (S.dof > 1) {
+            const bool p1 = (S.pris & 2u) != 0;
+            if ((S.al0 >> 1) & 1u) { // z_1 = e_z as well
+                if (p1) { K.zv |= 3u << 3; K.ov |= 4u << 3; }
+                else { K.zw |= 3u << 3; K.ow |= 4u << 3; }
+                // Jv_1[2] = 0 needs o_1 on the z axis too (a_1 = 0): not assumed
+            } else if (((S.alp | S.aln) >> 1) & 1u) { // z_1 = -+Y_0, Y_0[2] = 0
+                if (p1) K.zv |= 4u << 3;
+                else K.zw |= 4u << 3;
+            }
+        }
+    }
+    if (weighted) { K.ov = 0; K.ow = 0; } // a known 1 becomes the weight
+    return K;
+}
+
+template <bool WEIGHTED, typename SpecT>
+struct JK {
+    static constexpr JKnown K = jknown(SpecT::spec, WEIGHTED);
+    __device__ __forceinline__ static constexpr bool zero(int j, int k) { return (((k < 3 ? K.zv : K.zw) >> (3 * j + (k < 3 ? k : k - 3))) & 1u) != 0; }
+    __device__ __forceinline__ static constexpr bool one(int j, int k) { return (((k < 3 ? K.ov : K.ow) >> (3 * j + (k < 3 ? k : k - 3))) & 1u) != 0; }
+};
+struct NoSpec { static constexpr ChainSpec spec = generic_spec(MAX_DOF); };
+
+// S3: geometric Jacobian (DESIGN R3): revolute [z x (p - o); z], prismatic [z; 0], from the joint axes z_j
+// (src.Jw) and frame origins o_j (src.Jv) that FK retained; dst may be src.
+template <int D, bool WEIGHTED, typename SpecT>
+__device__ __forceinline__ void finish_jacobian(const KChain &ch, const Pose<D> &src, const float (&p)[3], float w_pos,
+                                                float w_rot, Pose<D> &dst) {
+    constexpr ChainSpec S = SpecT::spec;
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
+        const float z[3] = {src.Jw[j][0], src.Jw[j][1], src.Jw[j][2]};
+        if (!pris) {
+            // z x e with the components of z the chain structure fixes to 0 / 1 folded away (jknown)
+            using K = JK<false, SpecT>;
+            const float e[3] = {sub(p[0], src.Jv[j][0]), sub(p[1], src.Jv[j][1]), sub(p[2], src.Jv[j][2])};
+            float c[3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { // c_i = z_a e_b - z_b e_a, (a, b) = (i+1, i+2) mod 3, as fma(z_a, e_b, -z_b * e_a)
+                const int a = (i + 1) % 3, b = (i + 2) % 3;
+                const bool za0 = K::zero(j, 3 + a), za1 = K::one(j, 3 + a), zb0 = K::zero(j, 3 + b), zb1 = K::one(j, 3 + b);
+                const float inner = zb0 ? 0.f : zb1 ? -e[a] : mul(-z[b], e[a]);
+                c[i] = za0 ? inner : za1 ? (zb0 ? e[b] : add(e[b], inner)) : (zb0 ? mul(z[a], e[b]) : fma_(z[a], e[b], inner));
+            }
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { dst.Jv[j][i] = c[i]; dst.Jw[j][i] = z[i]; }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { dst.Jv[j][i] = z[i]; dst.Jw[j][i] = 0.f; }
+        }
+        if (WEIGHTED) {
+#pragma unroll
+            for (int i = 0; i < 3; ++i) { dst.Jv[j][i] = mul(w_pos, dst.Jv[j][i]); dst.Jw[j][i] = mul(w_rot, dst.Jw[j][i]); }
+        }
+    }
+}
+
 // S1 + S2 + S3: serial-chain FK (modified DH, DESIGN R1), pose residual against the target
 // (p_t, R_t given as COLUMNS Rt[k] = k-th column), geometric Jacobian from the retained joint axes.
 //   A_j = Rot_x(alpha) Trans_x(a) Rot_z(theta) Trans_z(d);  frame columns X, Y, Z and origin o.
-template <int D, bool FAST, bool WEIGHTED, typename SpecT>
+//   WITH_JAC = false: S3 is left to the caller (finish_jacobian); P.Jw / P.Jv then hold z_j / o_j and
+//   frame_p (nullable) receives the flange position.
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool WITH_JAC = true>
 __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D], const float (&pt)[3],
                                           const float (&Rt)[3][3], float w_pos, float w_rot,
-                                          Pose<D> &P, float *p_out, float (*R_out)[3]) {
+                                          Pose<D> &P, float *p_out, float (*R_out)[3], float *frame_p = nullptr) {
     constexpr ChainSpec S = SpecT::spec;
     float X[3], Y[3], Z[3], o[3];
 #pragma unroll
@@ -271,38 +349,56 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
     P.F = fma_(P.r[5], P.r[5], fma_(P.r[4], P.r[4], fma_(P.r[3], P.r[3],
           fma_(P.r[2], P.r[2], fma_(P.r[1], P.r[1], mul(P.r[0], P.r[0]))))));
 
-    // S3: geometric Jacobian (DESIGN R3): revolute [z x (p - o); z], prismatic [z; 0]
+    if (frame_p) {
 #pragma unroll
-    for (int j = 0; j < D; ++j) {
-        const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
-        if (!pris) {
-            const float e0 = sub(p[0], P.Jv[j][0]), e1 = sub(p[1], P.Jv[j][1]), e2 = sub(p[2], P.Jv[j][2]);
-            const float z0 = P.Jw[j][0], z1 = P.Jw[j][1], z2 = P.Jw[j][2];
-            P.Jv[j][0] = fma_(z1, e2, mul(-z2, e1));
-            P.Jv[j][1] = fma_(z2, e0, mul(-z0, e2));
-            P.Jv[j][2] = fma_(z0, e1, mul(-z1, e0));
-        } else {
-#pragma unroll
-            for (int i = 0; i < 3; ++i) { P.Jv[j][i] = P.Jw[j][i]; P.Jw[j][i] = 0.f; }
-        }
-        if (WEIGHTED) {
-#pragma unroll
-            for (int i = 0; i < 3; ++i) { P.Jv[j][i] = mul(w_pos, P.Jv[j][i]); P.Jw[j][i] = mul(w_rot, P.Jw[j][i]); }
-        }
+        for (int i = 0; i < 3; ++i) frame_p[i] = p[i];
     }
+    if (WITH_JAC) finish_jacobian<D, WEIGHTED, SpecT>(ch, P, p, w_pos, w_rot, P);
 }
 
-// 6-term dot products of Jacobian columns (rows 0..2 linear, 3..5 angular)
 template <int D>
-__device__ __forceinline__ float coldot(const Pose<D> &P, int i, int j) {
-    return fma_(P.Jw[i][2], P.Jw[j][2], fma_(P.Jw[i][1], P.Jw[j][1], fma_(P.Jw[i][0], P.Jw[j][0],
-           fma_(P.Jv[i][2], P.Jv[j][2], fma_(P.Jv[i][1], P.Jv[j][1], mul(P.Jv[i][0], P.Jv[j][0]))))));
+__device__ __forceinline__ float jentry(const Pose<D> &P, int j, int k) { return k < 3 ? P.Jv[j][k] : P.Jw[j][k - 3]; }
+
+// init + sum_k J[k][i] J[k][j] in the order k = 0..5 (rows 0..2 linear, 3..5 angular); HAVE = false: no init term
+template <int D, bool WEIGHTED, typename SpecT, bool HAVE>
+__device__ __forceinline__ float coldot_k(const Pose<D> &P, int i, int j, float init) {
+    using K = JK<WEIGHTED, SpecT>;
+    float acc = init;
+    bool have = HAVE;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        if (K::zero(i, k) || K::zero(j, k)) continue;
+        const float a = jentry<D>(P, i, k), b = jentry<D>(P, j, k);
+        const bool oi = K::one(i, k), oj = K::one(j, k);
+        if (oi && oj) acc = have ? add(acc, 1.f) : 1.f;
+        else if (oi) acc = have ? add(acc, b) : b;
+        else if (oj) acc = have ? add(acc, a) : a;
+        else acc = have ? fma_(a, b, acc) : mul(a, b);
+        have = true;
+    }
+    return have ? acc : 0.f;
 }
+// sum_k J[k][i] t[k]
+template <int D, bool WEIGHTED, typename SpecT>
+__device__ __forceinline__ float colvec_k(const Pose<D> &P, int i, const float (&t)[6]) {
+    using K = JK<WEIGHTED, SpecT>;
+    float acc = 0.f;
+    bool have = false;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        if (K::zero(i, k)) continue;
+        const float a = jentry<D>(P, i, k);
+        if (K::one(i, k)) acc = have ? add(acc, t[k]) : t[k];
+        else acc = have ? fma_(a, t[k], acc) : mul(a, t[k]);
+        have = true;
+    }
+    return have ? acc : 0.f;
+}
+// structure-agnostic forms (trajectory-level kernels)
 template <int D>
-__device__ __forceinline__ float colvec(const Pose<D> &P, int i, const float (&t)[6]) {
-    return fma_(P.Jw[i][2], t[5], fma_(P.Jw[i][1], t[4], fma_(P.Jw[i][0], t[3],
-           fma_(P.Jv[i][2], t[2], fma_(P.Jv[i][1], t[1], mul(P.Jv[i][0], t[0]))))));
-}
+__device__ __forceinline__ float coldot(const Pose<D> &P, int i, int j) { return coldot_k<D, false, NoSpec, false>(P, i, j, 0.f); }
+template <int D>
+__device__ __forceinline__ float colvec(const Pose<D> &P, int i, const float (&t)[6]) { return colvec_k<D, false, NoSpec>(P, i, t); }
 
 // x = (L L^T)^-1 b with L's strictly-lower part in L and 1/diag in invd
 template <int D>
@@ -330,16 +426,16 @@ __device__ __forceinline__ void chol_solve(const float (&L)[D][D], const float (
 //   rho = -J^T (r + J delta) - lambda delta,  delta += A^-1 rho                     (DESIGN R4)
 // which removes the 1/lambda amplification of fp32 rounding along the self-motion direction.
 // Returns false on a non-positive pivot or a non-finite step (=> the iteration is a reject).
-template <int D>
+template <int D, bool WEIGHTED, typename SpecT>
 __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine, float (&delta)[D]) {
+    using K = JK<WEIGHTED, SpecT>;
     float L[D][D], invd[D], g[D];
 #pragma unroll
     for (int i = 0; i < D; ++i) {
 #pragma unroll
-        for (int j = 0; j < i; ++j) L[i][j] = coldot<D>(P, i, j);
-        L[i][i] = fma_(P.Jw[i][2], P.Jw[i][2], fma_(P.Jw[i][1], P.Jw[i][1], fma_(P.Jw[i][0], P.Jw[i][0],
-                  fma_(P.Jv[i][2], P.Jv[i][2], fma_(P.Jv[i][1], P.Jv[i][1], fma_(P.Jv[i][0], P.Jv[i][0], lam))))));
-        g[i] = -colvec<D>(P, i, P.r);
+        for (int j = 0; j < i; ++j) L[i][j] = coldot_k<D, WEIGHTED, SpecT, false>(P, i, j, 0.f);
+        L[i][i] = coldot_k<D, WEIGHTED, SpecT, true>(P, i, i, lam); // lambda folded into the first FMA of the diagonal
+        g[i] = -colvec_k<D, WEIGHTED, SpecT>(P, i, P.r);
     }
     bool ok = true;
 #pragma unroll
@@ -363,14 +459,14 @@ __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine
             float sv = P.r[k], sw = P.r[3 + k];
 #pragma unroll
             for (int j = 0; j < D; ++j) {
-                sv = fma_(P.Jv[j][k], delta[j], sv);
-                sw = fma_(P.Jw[j][k], delta[j], sw);
+                if (!K::zero(j, k)) sv = K::one(j, k) ? add(sv, delta[j]) : fma_(P.Jv[j][k], delta[j], sv);
+                if (!K::zero(j, 3 + k)) sw = K::one(j, 3 + k) ? add(sw, delta[j]) : fma_(P.Jw[j][k], delta[j], sw);
             }
             t[k] = sv;
             t[3 + k] = sw;
         }
 #pragma unroll
-        for (int i = 0; i < D; ++i) rho[i] = -fma_(lam, delta[i], colvec<D>(P, i, t));
+        for (int i = 0; i < D; ++i) rho[i] = -fma_(lam, delta[i], colvec_k<D, WEIGHTED, SpecT>(P, i, t));
         chol_solve<D>(L, invd, rho, e);
 #pragma unroll
         for (int i = 0; i < D; ++i) delta[i] = add(delta[i], e[i]);

@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         if (!__any_sync(0xffffffffu, active)) break;
 
         float delta[D];
-        const bool ok = lm_delta<D>(cur, lam, A.refine, delta);     // S4, S5
+        const bool ok = lm_delta<D, WEIGHTED, SpecT>(cur, lam, A.refine, delta);     // S4, S5
         float qt[D];
         bool clamped = false;
 #pragma unroll
@@ -103,8 +103,9 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
             qt[j] = fminf(fmaxf(t, A.ch.lo[j]), A.ch.hi[j]);
             clamped = clamped || (qt[j] != t);
         }
-        Pose<D> tri;
-        eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, tri, nullptr, nullptr); // S7
+        Pose<D> tri; // S7: FK + residual at the trial point; its Jacobian (S3) is formed only if the step is accepted
+        float ptri[3];
+        eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, tri, nullptr, nullptr, ptri);
 
         if (A.trace_q != nullptr && active && live) {
 #pragma unroll
@@ -128,11 +129,8 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         }
         if (accept) {
 #pragma unroll
-            for (int j = 0; j < D; ++j) {
-                q[j] = qt[j];
-#pragma unroll
-                for (int i = 0; i < 3; ++i) { cur.Jv[j][i] = tri.Jv[j][i]; cur.Jw[j][i] = tri.Jw[j][i]; }
-            }
+            for (int j = 0; j < D; ++j) q[j] = qt[j];
+            finish_jacobian<D, WEIGHTED, SpecT>(A.ch, tri, ptri, A.w_pos, A.w_rot, cur); // S3 straight into the current state
 #pragma unroll
             for (int i = 0; i < 6; ++i) cur.r[i] = tri.r[i];
             cur.F = tri.F;
