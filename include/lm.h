@@ -131,6 +131,17 @@ int lm_run(lm_ctx *ctx, int32_t max_iters);
 /* Synchronise the stream and copy out the current state.  q_out: [d][W] device or host, nullable. */
 int lm_fetch(lm_ctx *ctx, float *q_out, lm_stats *stats_out);
 
+/* One call for HOST data (the end-to-end path): refine all B*n waypoints from host arrays (pinned memory makes
+ * the copies asynchronous) and write the results to host arrays.  The batch is split into `chunks` groups of
+ * whole trajectories that are pipelined over three internal streams, so that the host->device copy of chunk k+1,
+ * the LM kernel of chunk k and the device->host copy of chunk k-1 overlap (waypoints are independent:
+ * PAPER.md:L121, so the result does not depend on `chunks`).  problem->memory must be LM_MEM_HOST,
+ * shared_targets 0, problem->workspace DEVICE scratch of >= lm_solve_host_workspace_bytes().  q_out [d][B*n]
+ * and every non-null array of `stats` are HOST pointers.  Blocks until everything has arrived. */
+size_t lm_solve_host_workspace_bytes(int32_t dof, int64_t B, int64_t n, int32_t chunks);
+int lm_solve_host(const lm_chain *chain, const lm_problem *problem, const lm_params *params, int32_t max_iters,
+                  int32_t chunks, float *q_out, lm_stats *stats);
+
 /* Restart from the seeds given to lm_init (state := seeds, lambda := lambda0, iters := 0).  Host-only, no launch. */
 int lm_reset(lm_ctx *ctx);
 

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 using namespace lmk;
@@ -474,6 +475,141 @@ int lm_fetch(lm_ctx *c, float *q_out, lm_stats *s) {
     }
     LM_CUDA(cudaStreamSynchronize(c->stream));
     return LM_OK;
+}
+
+namespace {
+// trajectories [b0, b1) of chunk k when B trajectories are split into `chunks` nearly equal parts
+inline void chunk_range(int64_t B, int chunks, int k, int64_t &b0, int64_t &b1) {
+    b0 = B * k / chunks;
+    b1 = B * (k + 1) / chunks;
+}
+} // namespace
+
+size_t lm_solve_host_workspace_bytes(int32_t dof, int64_t B, int64_t n, int32_t chunks) {
+    if (dof < 1 || dof > LM_MAX_DOF || B <= 0 || n <= 0 || chunks < 1 || chunks > B) return 0;
+    size_t total = 0;
+    for (int k = 0; k < chunks; ++k) {
+        int64_t b0, b1;
+        chunk_range(B, chunks, k, b0, b1);
+        total += make_layout(dof, b1 - b0, n, 0, LM_MEM_HOST).total;
+    }
+    return total;
+}
+
+int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *prm, int32_t max_iters, int32_t chunks,
+                  float *q_out, lm_stats *st) {
+    if (!chain || !pb || !prm || max_iters < 0 || max_iters > LM_MAX_ITERS) return LM_EINVAL;
+    if (pb->memory != LM_MEM_HOST || pb->shared_targets || pb->B <= 0 || pb->n <= 0 || chunks < 1 || chunks > pb->B) return LM_EINVAL;
+    if (!pb->target_pos || !pb->target_quat || !pb->seeds || !pb->workspace) return LM_EINVAL;
+    const int d = chain->dof;
+    if (d < 1 || d > LM_MAX_DOF) return LM_EINVAL;
+    if (pb->workspace_bytes < lm_solve_host_workspace_bytes(d, pb->B, pb->n, chunks)) return LM_ENOMEM;
+    const size_t W = (size_t)pb->B * (size_t)pb->n;
+    constexpr int NS = 3, MAX_CHUNKS = 256;
+    if (chunks > MAX_CHUNKS) return LM_EINVAL;
+    // streams and the pinned totals buffer are created once per process and device and kept (creating
+    // them costs more than a whole step); calls are serialised by the mutex
+    struct Pipe { int dev = -1; cudaStream_t st[NS] = {nullptr, nullptr, nullptr}; unsigned long long *totals = nullptr; };
+    static Pipe pipe;
+    static std::mutex pipe_mutex;
+    std::lock_guard<std::mutex> lock(pipe_mutex);
+    int rc = LM_OK;
+    auto fail = [&](cudaError_t e) { rc = cuda_fail(e); };
+    int dev = 0;
+    LM_CUDA(cudaGetDevice(&dev));
+    if (pipe.dev != dev) {
+        for (int i = 0; i < NS; ++i) {
+            if (pipe.st[i]) cudaStreamDestroy(pipe.st[i]);
+            LM_CUDA(cudaStreamCreateWithFlags(&pipe.st[i], cudaStreamNonBlocking));
+        }
+        if (!pipe.totals) LM_CUDA(cudaMallocHost(reinterpret_cast<void **>(&pipe.totals), 16 * (size_t)MAX_CHUNKS));
+        pipe.dev = dev;
+    }
+    cudaStream_t *streams = pipe.st;
+    unsigned long long *totals = pipe.totals;
+    lm_ctx **ctxs = new (std::nothrow) lm_ctx *[chunks]();
+    if (!ctxs) return LM_ENOMEM;
+    char *ws = static_cast<char *>(pb->workspace);
+    for (int k = 0; k < chunks && rc == LM_OK; ++k) {
+        int64_t b0, b1;
+        chunk_range(pb->B, chunks, k, b0, b1);
+        const int64_t Bc = b1 - b0;
+        const size_t Wc = (size_t)Bc * (size_t)pb->n, w0 = (size_t)b0 * (size_t)pb->n;
+        const Layout lay = make_layout(d, Bc, pb->n, 0, LM_MEM_HOST);
+        cudaStream_t s = streams[k % NS];
+        float *sd = reinterpret_cast<float *>(ws + lay.s_seeds), *tpd = reinterpret_cast<float *>(ws + lay.s_tp),
+              *tqd = reinterpret_cast<float *>(ws + lay.s_tq);
+        // rows of the SoA arrays are W apart on the host, Wc apart in the chunk's staging area
+        cudaError_t e = cudaMemcpy2DAsync(sd, 4 * Wc, pb->seeds + w0, 4 * W, 4 * Wc, d, cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpy2DAsync(tpd, 4 * Wc, pb->target_pos + w0, 4 * W, 4 * Wc, 3, cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpy2DAsync(tqd, 4 * Wc, pb->target_quat + w0, 4 * W, 4 * Wc, 4, cudaMemcpyHostToDevice, s);
+        if (e != cudaSuccess) { fail(e); break; }
+        lm_problem pk = *pb;
+        pk.B = Bc; pk.target_pos = tpd; pk.target_quat = tqd; pk.seeds = sd; pk.memory = LM_MEM_DEVICE;
+        pk.workspace = ws; pk.workspace_bytes = lay.total;
+        rc = lm_init(&ctxs[k], chain, &pk, prm, s);
+        if (rc != LM_OK) break;
+        lm_ctx *c = ctxs[k];
+        rc = iterate(c, max_iters, INT_MAX);
+        if (rc != LM_OK) break;
+        const KArgs &a = c->args;
+        auto out1 = [&](void *dst, const void *src, size_t elem, size_t off, size_t count) {
+            if (dst && rc == LM_OK) {
+                cudaError_t e2 = cudaMemcpyAsync(static_cast<char *>(dst) + elem * off, src, elem * count, cudaMemcpyDeviceToHost, s);
+                if (e2 != cudaSuccess) fail(e2);
+            }
+        };
+        if (q_out) {
+            e = cudaMemcpy2DAsync(q_out + w0, 4 * W, a.q, 4 * Wc, 4 * Wc, d, cudaMemcpyDeviceToHost, s);
+            if (e != cudaSuccess) { fail(e); break; }
+        }
+        unsigned long long *tot = reinterpret_cast<unsigned long long *>(ws + lay.totals);
+        e = cudaMemsetAsync(tot, 0, 16, s);
+        if (e != cudaSuccess) { fail(e); break; }
+        uint8_t *conv = reinterpret_cast<uint8_t *>(ws + lay.conv);
+        int32_t *tit = reinterpret_cast<int32_t *>(ws + lay.titers);
+        g_launches.fetch_add(1);
+        lm_traj_stats_kernel<<<(unsigned)((Bc * 32 + 255) / 256), 256, 0, s>>>(a.its, Bc, (int32_t)pb->n, conv, tit, tot);
+        if (st) {
+            out1(st->res_norm, a.res, 4, w0, Wc);
+            out1(st->pos_err, a.perr, 4, w0, Wc);
+            out1(st->rot_err, a.rerr, 4, w0, Wc);
+            out1(st->lambda, a.lam, 4, w0, Wc);
+            out1(st->accept_mask, a.mask, 8, w0, Wc);
+            out1(st->traj_converged, conv, 1, (size_t)b0, (size_t)Bc);
+            out1(st->traj_iters, tit, 4, (size_t)b0, (size_t)Bc);
+            if (st->iters || st->status) {
+                int32_t *ui = reinterpret_cast<int32_t *>(ws + lay.ui);
+                uint32_t *us = reinterpret_cast<uint32_t *>(ws + lay.us);
+                g_launches.fetch_add(1);
+                lm_unpack_kernel<<<(unsigned)((Wc + 255) / 256), 256, 0, s>>>(a.its, (int64_t)Wc, st->iters ? ui : nullptr, st->status ? us : nullptr);
+                out1(st->iters, ui, 4, w0, Wc);
+                out1(st->status, us, 4, w0, Wc);
+            }
+        }
+        if (rc == LM_OK) {
+            e = cudaMemcpyAsync(totals + 2 * k, tot, 16, cudaMemcpyDeviceToHost, s);
+            if (e == cudaSuccess) e = cudaGetLastError();
+            if (e != cudaSuccess) fail(e);
+        }
+        ws += lay.total;
+    }
+    for (int i = 0; i < NS; ++i)
+        if (streams[i]) {
+            cudaError_t e = cudaStreamSynchronize(streams[i]);
+            if (e != cudaSuccess && rc == LM_OK) fail(e);
+        }
+    if (st && rc == LM_OK) {
+        st->total_waypoint_iters = 0;
+        st->converged_trajectories = 0;
+        for (int k = 0; k < chunks; ++k) {
+            st->total_waypoint_iters += (int64_t)totals[2 * k];
+            st->converged_trajectories += (int64_t)totals[2 * k + 1];
+        }
+    }
+    for (int k = 0; k < chunks; ++k) delete ctxs[k];
+    delete[] ctxs;
+    return rc;
 }
 
 int lm_fp32_peak(void *cuda_stream, double *tflops_out) { return lm_fp32_peak_form(cuda_stream, LM_FMA_FORM_RCC, tflops_out); }

@@ -31,6 +31,7 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_strerror", "lm_launch_count", "lm_fp32_peak_form",
            "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
            "lm_traj_fetch", "lm_traj_set_trace",
+           "lm_solve_host_workspace_bytes", "lm_solve_host",
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR = 0, 1
 
@@ -131,6 +132,10 @@ def lib() -> C.CDLL:
         L.lm_traj_reset.argtypes = [C.c_void_p, C.c_void_p]
         L.lm_traj_fetch.argtypes = [C.c_void_p, C.POINTER(LmTrajStats)]
         L.lm_traj_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lm_solve_host_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.c_int32]
+        L.lm_solve_host_workspace_bytes.restype = C.c_size_t
+        L.lm_solve_host.argtypes = [C.POINTER(LmChain), C.POINTER(LmProblem), C.POINTER(LmParams), C.c_int32, C.c_int32,
+                                    C.c_void_p, C.POINTER(LmStats)]
         L.lm_plan_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64]
         L.lm_plan_workspace_bytes.restype = C.c_size_t
         L.lm_plan_default_params.argtypes = [C.POINTER(LmPlanParams)]
@@ -276,6 +281,16 @@ def lm_traj_fetch(ctx: int, stats: LmTrajStats) -> None:
 
 def lm_traj_set_trace(ctx: int, trial_q_ptr: Optional[int], trial_F_ptr: Optional[int]) -> None:
     _check(lib().lm_traj_set_trace(ctx, trial_q_ptr, trial_F_ptr), "lm_traj_set_trace")
+
+
+def lm_solve_host_workspace_bytes(dof: int, B: int, n: int, chunks: int) -> int:
+    return int(lib().lm_solve_host_workspace_bytes(dof, B, n, chunks))
+
+
+def lm_solve_host(chain: LmChain, problem: LmProblem, params: LmParams, max_iters: int, chunks: int,
+                  q_out_ptr: Optional[int], stats: Optional[LmStats]) -> None:
+    _check(lib().lm_solve_host(C.byref(chain), C.byref(problem), C.byref(params), int(max_iters), int(chunks),
+                               q_out_ptr, C.byref(stats) if stats is not None else None), "lm_solve_host")
 
 
 def lm_plan_workspace_bytes(dof: int, B: int, n: int) -> int:

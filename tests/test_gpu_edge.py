@@ -262,3 +262,46 @@ def test_specialised_kernels_equal_generic(lm):
                                   cases[1][1].seeds[:4], 0.0, 2))
     assert s.kernel_name == "generic"
     s.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("chunks", [1, 3, 8])
+def test_solve_host_pipelined_equals_the_stepwise_path(chunks):
+    """lm_solve_host (host arrays, chunked + pipelined over streams) returns exactly what
+    lm_init + lm_run + lm_fetch return: waypoints are independent."""
+    import torch
+    from paper_2309_09102_b200 import lm, workloads as wl
+    from oracle import lm_oracle as orc
+    ch = wl.panda_chain()
+    w = wl.config2(lambda q: orc.fk(ch, q), B=13, n=37)
+    prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol)
+    ref_s = lm.Solver(ch, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm)
+    ref_s.run(w.max_iters)
+    ref = ref_s.fetch()
+    ref_s.close()
+    d, W = 7, w.W
+    soa = lambda x: torch.from_numpy(np.ascontiguousarray(np.asarray(x, np.float32).T)).pin_memory()
+    tp, tq, seeds = soa(w.target_pos), soa(w.target_quat), soa(w.seeds)
+    nbytes = lm.lm_solve_host_workspace_bytes(d, w.B, w.n, chunks)
+    ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+    ptr = (ws.data_ptr() + 255) // 256 * 256
+    cchain, keep = lm.make_chain(ch)
+    q = torch.empty((d, W), dtype=torch.float32).pin_memory()
+    res = torch.empty(W, dtype=torch.float32).pin_memory()
+    its = torch.empty(W, dtype=torch.int32).pin_memory()
+    sts = torch.empty(W, dtype=torch.int32).pin_memory()
+    msk = torch.empty(W, dtype=torch.int64).pin_memory()
+    conv = torch.empty(w.B, dtype=torch.uint8).pin_memory()
+    pb = lm.LmProblem(w.B, w.n, tp.data_ptr(), tq.data_ptr(), 0, seeds.data_ptr(), lm.LM_MEM_HOST, ptr, nbytes)
+    st = lm.LmStats(res.data_ptr(), None, None, None, its.data_ptr(), msk.data_ptr(), sts.data_ptr(), conv.data_ptr(), None, 0, 0)
+    lm.lm_solve_host(cchain, pb, prm, w.max_iters, chunks, q.data_ptr(), st)
+    assert np.array_equal(q.numpy().T, ref["q"])
+    assert np.array_equal(res.numpy(), ref["res_norm"])
+    assert np.array_equal(its.numpy(), ref["iters"])
+    assert np.array_equal(msk.numpy().view(np.uint64), ref["mask"])
+    assert np.array_equal(sts.numpy().view(np.uint32), ref["status"])
+    assert np.array_equal(conv.numpy(), ref["traj_converged"])
+    assert st.total_waypoint_iters == ref["total_waypoint_iters"]
+    assert st.converged_trajectories == ref["converged_trajectories"]
+    with pytest.raises(lm.LmError):
+        lm.lm_solve_host(cchain, pb, prm, w.max_iters, w.B + 1, q.data_ptr(), st)
