@@ -38,8 +38,8 @@ ALG_FLOP = {7: 1459.0, 8: 1762.0}
 # FP32 FMA-pipe peak derived from the guide's unit counts and clocks: 148 SMs x 128 lanes x 2 x f_max
 SM_COUNT, FP32_LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r1_lm_iterate_full.md); keyed by (workload, kernel variant).
-NCU_DRAM_TRAFFIC = {("C4", "panda7"): 68.864e6 + 27.270e6}
+# `ncu --set full` capture (profiles/r1c_lm_iterate_full.md); keyed by (workload, kernel variant).
+NCU_DRAM_TRAFFIC = {("C4", "panda7"): 68.849e6 + 27.575e6}
 
 
 def load_peaks() -> dict:
