@@ -35,6 +35,9 @@ UNIT = "waypoint-iterations/s"
 
 # Algorithmic FLOPs per waypoint-iteration (DESIGN.md section 6 / SURVEY.md section 8d; FMA = 2).
 ALG_FLOP = {7: 1459.0, 8: 1762.0}
+# the dual 6 x 6 variant (LM_SOLVER_DUAL): Jacobian 84, J J^T + lambda 42 d + 6, Cholesky 70,
+# solves 72, J^T y 12 d, update 3 d, FK 48 d + 6, residual 77, accept 5
+ALG_FLOP_DUAL = {7: 1055.0, 8: 1160.0}
 # FP32 FMA-pipe peak derived from the guide's unit counts and clocks: 148 SMs x 128 lanes x 2 x f_max
 SM_COUNT, FP32_LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
@@ -322,6 +325,7 @@ def run_gpu(args) -> None:
     if args.workload == "C4" and full_size:
         # the "to convergence" statistic of the metric, on BASELINE.json configs[1] (512 x 300, tol 1e-5)
         extra["to_convergence_C2"] = time_to_convergence(lm, torch, wl, fk, device, stream)
+        extra["variant_dual"] = time_dual_variant(lm, torch, w, device, stream, peak_tf)
         # the trajectory-level step on the same workload
         extra["trajectory_step"] = time_traj_step(lm, torch, w, solver, stream, peaks)
         # the paper's alternating schedule with anytime bookkeeping (NEXT-2), valid trajectories per second
@@ -440,6 +444,32 @@ def time_plan(lm, torch, wl, fk, device, stream, cycles: int = 3, reps: int = 5)
     s.close()
     out["workload"] = f"C2: {w.B} x {w.n}, tol={w.tol:g}, pose_iters=10, w_pose=1, w_diff=1"
     return out
+
+
+def time_dual_variant(lm, torch, w, device, stream, peak_tf: float, reps: int = 10) -> dict:
+    """The disclosed variant LM_SOLVER_DUAL (same LM step through the 6 x 6 system) on the same workload:
+    median CUDA-event time of lm_reset + lm_run after 3 warm-ups."""
+    d = int(w.chain.dof)
+    prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol, solver=lm.LM_SOLVER_DUAL)
+    s = lm.Solver(w.chain, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, device=str(device), stream=stream)
+    ts = []
+    with torch.cuda.stream(stream):
+        for i in range(reps + 3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s.reset()
+            a.record(stream)
+            s.run(w.max_iters)
+            b.record(stream)
+            stream.synchronize()
+            if i >= 3:
+                ts.append(a.elapsed_time(b))
+        iters, _ = s.fetch_totals()
+    s.close()
+    ms = float(np.median(ts))
+    tf = ALG_FLOP_DUAL.get(d, 1055.0) * iters / (ms * 1e-3) / 1e12
+    return {"solver": "LM_SOLVER_DUAL: delta = -J^T (J J^T + lambda I_6)^-1 r, no refinement", "ms_per_step": ms,
+            "waypoint_iterations_per_sec": iters / (ms * 1e-3), "alg_flop_per_waypoint_iteration": ALG_FLOP_DUAL.get(d),
+            "achieved_tflops": tf, "frac_of_derived_peak": tf / peak_tf}
 
 
 def time_to_convergence(lm, torch, wl, fk, device, stream, reps: int = 20) -> dict:

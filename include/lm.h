@@ -88,7 +88,12 @@ typedef struct {
     float w_pos, w_rot;   /* residual weights, 1 and 1 (DESIGN R2b) */
     int32_t refine_steps; /* iterative-refinement steps on the fp32 Cholesky solve, 0..2 (default 1, DESIGN R4) */
     int32_t fast_sincos;  /* 0 = accurate sincosf (default); 1 = MUFU __sincosf */
+    int32_t solver;       /* LM_SOLVER_PRIMAL (default): the d x d system (J^T J + lambda I) delta = -J^T r of PAPER.md:L121;
+                             LM_SOLVER_DUAL: the same step as delta = -J^T (J J^T + lambda I_6)^-1 r (6 x 6, no refinement;
+                             a disclosed variant) */
 } lm_params;
+#define LM_SOLVER_PRIMAL 0
+#define LM_SOLVER_DUAL 1
 
 /* lm_fetch outputs.  Every pointer is nullable; each may be DEVICE or HOST memory (detected). */
 typedef struct {

@@ -477,4 +477,57 @@ __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine
     return ok && (asum < 1e30f);
 }
 
+// The same step in its DUAL form (SURVEY section 8f NEXT-4 i, a disclosed variant):
+//   delta = -J^T (J J^T + lambda I_6)^-1 r,
+// identical to -(J^T J + lambda I_d)^-1 J^T r in exact arithmetic (push-through identity; the oracle pins
+// it, tests/test_oracle_pins.py P5).  6 x 6 instead of d x d, and delta lies in range(J^T) by construction,
+// so fp32 rounding has no self-motion component to amplify by 1/lambda: no refinement step is needed.
+template <int D, bool WEIGHTED, typename SpecT>
+__device__ __forceinline__ bool lm_delta_dual(const Pose<D> &P, float lam, float (&delta)[D]) {
+    using K = JK<WEIGHTED, SpecT>;
+    float L[6][6], invd[6], y[6];
+#pragma unroll
+    for (int a = 0; a < 6; ++a) {
+#pragma unroll
+        for (int b = 0; b <= a; ++b) { // (J J^T)_ab = sum_j J[a][j] J[b][j], lambda on the diagonal
+            float acc = lam;
+            bool have = (a == b);
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                if (K::zero(j, a) || K::zero(j, b)) continue;
+                const float u = jentry<D>(P, j, a), v = jentry<D>(P, j, b);
+                const bool ou = K::one(j, a), ov = K::one(j, b);
+                if (ou && ov) acc = have ? add(acc, 1.f) : 1.f;
+                else if (ou) acc = have ? add(acc, v) : v;
+                else if (ov) acc = have ? add(acc, u) : u;
+                else acc = have ? fma_(u, v, acc) : mul(u, v);
+                have = true;
+            }
+            L[a][b] = have ? acc : 0.f;
+        }
+    }
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const float piv = L[k][k];
+        ok = ok && (piv > 0.f);
+        const float id = rsqrtf(piv);
+        invd[k] = id;
+#pragma unroll
+        for (int i = k + 1; i < 6; ++i) L[i][k] = mul(L[i][k], id);
+#pragma unroll
+        for (int j = k + 1; j < 6; ++j)
+#pragma unroll
+            for (int i = j; i < 6; ++i) L[i][j] = fma_(-L[i][k], L[j][k], L[i][j]);
+    }
+    chol_solve<6>(L, invd, P.r, y);
+    float asum = 0.f;
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        delta[j] = -colvec_k<D, WEIGHTED, SpecT>(P, j, y);
+        asum = add(asum, fabsf(delta[j]));
+    }
+    return ok && (asum < 1e30f);
+}
+
 } // namespace lmk

@@ -16,7 +16,7 @@ struct KArgs {
     KChain ch;
     float lambda0, nu_up, inv_nu_down, lambda_min, lambda_max, tol2;
     float w_pos, w_rot, inv_w_pos, inv_w_rot;
-    int32_t weighted, refine;
+    int32_t weighted, refine, dual;
     int64_t W;              // waypoint blocks
     int32_t n;              // waypoints per trajectory
     int32_t shared_targets; // target index = w % n
@@ -50,7 +50,7 @@ __device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z,
 #define LM_MIN_BLOCKS 1
 #endif
 
-template <int D, bool FAST, bool WEIGHTED, typename SpecT>
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool DUAL = false>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kernel(const __grid_constant__ KArgs A) {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = w < A.W;
@@ -94,7 +94,8 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         if (!__any_sync(0xffffffffu, active)) break;
 
         float delta[D];
-        const bool ok = lm_delta<D, WEIGHTED, SpecT>(cur, lam, A.refine, delta);     // S4, S5
+        const bool ok = DUAL ? lm_delta_dual<D, WEIGHTED, SpecT>(cur, lam, delta)            // S4, S5 (variant)
+                             : lm_delta<D, WEIGHTED, SpecT>(cur, lam, A.refine, delta);     // S4, S5
         float qt[D];
         bool clamped = false;
 #pragma unroll

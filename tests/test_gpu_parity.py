@@ -191,3 +191,28 @@ def test_teacher_forced_steps(lm, cfg):
     s.close()
     assert worst <= H.TOL_Q, worst
     assert decided > 0 and mism == 0, (decided, mism)
+
+
+# ------------------------------------------------------------------ NEXT-4 (i): dual 6 x 6 form
+
+def test_dual_form_variant_matches_the_oracle(lm):
+    """LM_SOLVER_DUAL: delta = -J^T (J J^T + lambda I_6)^-1 r is the SAME step (push-through identity,
+    pinned on the oracle by P5), so the oracle's primal fp64 sequence is the reference: configs[0]
+    and configs[1] at full size, same bars as the primal path; no refinement step is involved."""
+    w = wl.config1(H.oracle_fk(wl.panda_chain()))
+    g, o = H.run_gpu(w, solver=lm.LM_SOLVER_DUAL, refine_steps=0), H.run_oracle(w)
+    _check_free_running(w, g, o)
+    assert np.abs(g["q"] - o.q).max() < 5e-6
+    compared, bad = H.decisive_mismatches(w, g, 20)
+    assert compared >= 100 and bad == 0
+    w = wl.config2(H.oracle_fk(wl.panda_chain()))
+    g, o = H.run_gpu(w, solver=lm.LM_SOLVER_DUAL, refine_steps=0), H.run_oracle(w)
+    _check_free_running(w, g, o)
+    assert g["converged_trajectories"] == w.B
+    compared, bad = H.decisive_mismatches(w, g, int(o.iters.max()))
+    assert compared > w.W and bad == 0
+    # 8-DoF chain with a prismatic joint
+    ch = wl.random_chain_8dof(3)
+    w = wl.config3(H.oracle_fk(ch), B=128)
+    g, o = H.run_gpu(w, solver=lm.LM_SOLVER_DUAL), H.run_oracle(w)
+    _check_free_running(w, g, o)
