@@ -121,6 +121,27 @@ void orc_fk(const orc_chain *c, const double *q, double *p, double *R, double *z
     }
 }
 
+
+/* Frames of every link: Rj[j] (row-major 3x3) and oj[j] = rotation and origin of the frame attached to the
+ * link that joint j moves (T_1 .. T_d of DESIGN R1, before the tool transform).  Used by the collision
+ * oracle (capsules are attached to link frames). */
+void orc_fk_frames(const orc_chain *c, const double *q, double *Rj, double *oj) {
+    double T[4][4], M[4][4];
+    mat4_identity(T);
+    for (int j = 0; j < c->dof; ++j) {
+        double theta = c->theta[j], dd = c->d[j];
+        if (c->joint_type[j] == 0) theta += q[j]; else dd += q[j];
+        rot_x(c->alpha[j], M);   mat4_mul(T, M, T);
+        trans(c->a[j], 0, 0, M); mat4_mul(T, M, T);
+        rot_z(theta, M);         mat4_mul(T, M, T);
+        trans(0, 0, dd, M);      mat4_mul(T, M, T);
+        for (int i = 0; i < 3; ++i) {
+            for (int k = 0; k < 3; ++k) Rj[9 * j + 3 * i + k] = T[i][k];
+            oj[3 * j + i] = T[i][3];
+        }
+    }
+}
+
 /* ------------------------------------------------------------------ residual */
 
 void orc_residual(const double *p, const double *R, const double *tp, const double *tquat,

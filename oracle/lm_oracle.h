@@ -57,6 +57,9 @@ typedef struct {
  * joint j in the world frame (nullable). */
 void orc_fk(const orc_chain *c, const double *q, double *p, double *R, double *z, double *o);
 
+/* link frames T_1..T_d: Rj[d][9] row-major rotations, oj[d][3] origins (world frame) */
+void orc_fk_frames(const orc_chain *c, const double *q, double *Rj, double *oj);
+
 /* unit-normalise then convert quaternion (w,x,y,z) to a rotation matrix, DESIGN R11 */
 void orc_quat_to_R(const double *quat, double *R);
 

@@ -19,8 +19,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "lm_oracle.c")
 _HDR = os.path.join(_HERE, "lm_oracle.h")
-_SRCS = [_SRC, os.path.join(_HERE, "lm_traj_oracle.c")]   # one shared object: pose LM + trajectory-level LM
-_DEPS = _SRCS + [_HDR, os.path.join(_HERE, "lm_traj_oracle.h")]
+_SRCS = [_SRC, os.path.join(_HERE, "lm_traj_oracle.c"), os.path.join(_HERE, "lm_coll_oracle.c")]  # one shared object
+_DEPS = _SRCS + [_HDR, os.path.join(_HERE, "lm_traj_oracle.h"), os.path.join(_HERE, "lm_coll_oracle.h")]
 _LIB = os.path.join(_HERE, "liblm_oracle.so")
 MAX_DOF = 8
 

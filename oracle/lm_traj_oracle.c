@@ -14,6 +14,12 @@
 
 int64_t orc_traj_rows(int32_t dof, int64_t n) { return 6 * n + (int64_t)dof * (n - 1); }
 
+static int coll_rows(const orc_traj_params *t) { return (t->caps && t->caps->w_coll != 0.0) ? t->caps->npairs : 0; }
+
+int64_t orc_traj_rows_all(const orc_traj_params *t, int32_t dof, int64_t n) {
+    return orc_traj_rows(dof, n) + (int64_t)coll_rows(t) * n;
+}
+
 /* ------------------------------------------------------------------ residual, PAPER.md:L117 (Fig. 6) */
 
 void orc_traj_residual(const orc_chain *c, const orc_params *prm, const orc_traj_params *t,
@@ -28,6 +34,9 @@ void orc_traj_residual(const orc_chain *c, const orc_params *prm, const orc_traj
     for (int64_t k = 0; k + 1 < n; ++k) /* r_diff: q_{k+1} - q_k */
         for (int a = 0; a < d; ++a)
             r[6 * n + d * k + a] = t->w_diff * (q[(k + 1) * d + a] - q[k * d + a]);
+    const int np = coll_rows(t);
+    for (int64_t i = 0; i < n && np > 0; ++i) /* self-collision hinge rows, PAPER.md:L117 (Fig. 6) */
+        orc_coll_residual(c, t->caps, q + i * d, NULL, r + orc_traj_rows(d, n) + np * i);
 }
 
 /* ------------------------------------------------------------------ Jacobian */
@@ -35,7 +44,7 @@ void orc_traj_residual(const orc_chain *c, const orc_params *prm, const orc_traj
 void orc_traj_jacobian(const orc_chain *c, const orc_params *prm, const orc_traj_params *t,
                        int64_t n, const double *q, double *J) {
     const int d = c->dof;
-    const int64_t rows = orc_traj_rows(d, n), cols = n * d;
+    const int64_t rows = orc_traj_rows_all(t, d, n), cols = n * d;
     memset(J, 0, sizeof(double) * (size_t)(rows * cols));
     for (int64_t i = 0; i < n; ++i) {
         double Ji[6 * ORC_MAX_DOF];
@@ -50,6 +59,13 @@ void orc_traj_jacobian(const orc_chain *c, const orc_params *prm, const orc_traj
             J[(6 * n + d * k + a) * cols + d * k + a] = -t->w_diff;
             J[(6 * n + d * k + a) * cols + d * (k + 1) + a] = t->w_diff;
         }
+    const int np = coll_rows(t);
+    for (int64_t i = 0; i < n && np > 0; ++i) { /* collision rows of waypoint i depend on q_i only */
+        double Jc[ORC_MAX_PAIRS * ORC_MAX_DOF];
+        orc_coll_jacobian(c, t->caps, q + i * d, Jc);
+        for (int p = 0; p < np; ++p)
+            for (int a = 0; a < d; ++a) J[(orc_traj_rows(d, n) + np * i + p) * cols + d * i + a] = Jc[p * d + a];
+    }
 }
 
 /* ------------------------------------------------------------------ dense solve (the definition) */
@@ -92,7 +108,7 @@ int orc_traj_delta_dense(const orc_chain *c, const orc_params *prm, const orc_tr
                          int64_t n, const double *tp, const double *tquat, const double *q,
                          double lambda, double *delta) {
     const int d = c->dof;
-    const int64_t rows = orc_traj_rows(d, n), N = n * d;
+    const int64_t rows = orc_traj_rows_all(t, d, n), N = n * d;
     double *J = (double *)malloc(sizeof(double) * (size_t)(rows * N));
     double *r = (double *)malloc(sizeof(double) * (size_t)rows);
     double *A = (double *)malloc(sizeof(double) * (size_t)(N * N));
@@ -175,6 +191,17 @@ int orc_traj_delta_banded(const orc_chain *c, const orc_params *prm, const orc_t
             delta[d * i + a] = -s;
             ab[(d * i + a) * ld] += lambda;
         }
+        const int np = coll_rows(t);
+        if (np > 0) { /* collision rows of waypoint i: J_c^T J_c on the diagonal block, J_c^T r_c in the gradient */
+            double Jc[ORC_MAX_PAIRS * ORC_MAX_DOF], rc[ORC_MAX_PAIRS];
+            orc_coll_jacobian(c, t->caps, q + i * d, Jc);
+            orc_coll_residual(c, t->caps, q + i * d, NULL, rc);
+            for (int p = 0; p < np; ++p)
+                for (int a = 0; a < d; ++a) {
+                    for (int b = 0; b <= a; ++b) ab[(d * i + b) * ld + (a - b)] += Jc[p * d + a] * Jc[p * d + b];
+                    delta[d * i + a] -= Jc[p * d + a] * rc[p];
+                }
+        }
     }
     for (int64_t k = 0; k + 1 < n; ++k) /* differencing row (k, a): -w at column (k, a), +w at (k+1, a) */
         for (int a = 0; a < d; ++a) {
@@ -207,8 +234,15 @@ static void traj_cost(const orc_chain *c, const orc_params *prm, const orc_traj_
             const double e = q[(k + 1) * d + a] - q[k * d + a];
             fd += e * e;
         }
+    double fc = 0.0;
+    const int np = coll_rows(t);
+    for (int64_t i = 0; i < n && np > 0; ++i) {
+        double rc[ORC_MAX_PAIRS];
+        orc_coll_residual(c, t->caps, q + i * d, NULL, rc);
+        for (int p = 0; p < np; ++p) fc += rc[p] * rc[p];
+    }
     *Fp = fp; *Fd = fd;
-    *F = t->w_pose * t->w_pose * fp + t->w_diff * t->w_diff * fd;
+    *F = t->w_pose * t->w_pose * fp + t->w_diff * t->w_diff * fd + fc;
 }
 
 int64_t orc_traj_lm_advance(const orc_chain *c, const orc_params *prm, const orc_traj_params *t,

@@ -30,15 +30,20 @@
 #ifndef LM_TRAJ_ORACLE_H
 #define LM_TRAJ_ORACLE_H
 
+#include "lm_coll_oracle.h"
 #include "lm_oracle.h"
 
 typedef struct {
     double w_pose, w_diff;                                  /* DESIGN T1 */
     double lambda0, nu_up, nu_down, lambda_min, lambda_max; /* DESIGN T3 (= R5, per trajectory) */
+    const orc_capsules *caps; /* nullable: self-collision rows (lm_coll_oracle.h, Fig. 6 "self-coll-dist(q_i)"),
+                                 caps->npairs hinge rows per waypoint appended after the differencing rows:
+                                 row 6n + d(n-1) + npairs * i + p  =  residual of pair p at waypoint i */
 } orc_traj_params;
 
-/* rows of the stacked residual / Jacobian of one n-waypoint trajectory */
+/* rows of the stacked residual / Jacobian of one n-waypoint trajectory (without / with the collision rows) */
 int64_t orc_traj_rows(int32_t dof, int64_t n);
+int64_t orc_traj_rows_all(const orc_traj_params *tp_, int32_t dof, int64_t n);
 
 /* r[6n + d(n-1)]: rows 6i..6i+5 = w_pose * pose residual of waypoint i (orc_residual, weights
  * prm->w_pos / w_rot); rows 6n + d k + a = w_diff * (q[k+1][a] - q[k][a]).   q: [n][d], tp: [n][3],
@@ -64,7 +69,7 @@ int orc_traj_delta_banded(const orc_chain *c, const orc_params *prm, const orc_t
  * tp[B][n][3], tquat[B][n][4]).  Per trajectory: state q, lambda, iters, mask, status; advances
  * until iters == max_total_iters or `at_most` iterations were done in this call (< 0: no cap).
  * Outputs (nullable): F_total = w_pose^2 F_pose + w_diff^2 F_diff, F_pose = sum_i |r_pose,i|^2,
- * F_diff = sum_k |q_{k+1} - q_k|^2 at the current q.  Trace of the LAST iteration executed in
+ * F_diff = sum_k |q_{k+1} - q_k|^2 at the current q (the collision rows add their squares to F_total only).  Trace of the LAST iteration executed in
  * this call (nullable): trial_q[B][n][d], F_before[B], F_trial[B], accepted[B] (-1 = none).
  * use_dense != 0 selects orc_traj_delta_dense.  Returns the number of trajectory-iterations executed. */
 int64_t orc_traj_lm_advance(const orc_chain *c, const orc_params *prm, const orc_traj_params *tp_,

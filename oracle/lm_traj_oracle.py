@@ -14,6 +14,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
+from . import lm_coll_oracle as _co
 from . import lm_oracle as _o
 
 _dp = C.POINTER(C.c_double)
@@ -21,7 +22,7 @@ _dp = C.POINTER(C.c_double)
 
 class _TParams(C.Structure):
     _fields_ = [(k, C.c_double) for k in
-                ("w_pose", "w_diff", "lambda0", "nu_up", "nu_down", "lambda_min", "lambda_max")]
+                ("w_pose", "w_diff", "lambda0", "nu_up", "nu_down", "lambda_min", "lambda_max")] + [("caps", C.c_void_p)]
 
 
 @dataclass
@@ -34,10 +35,15 @@ class TrajParams:
     nu_down: float = 10.0
     lambda_min: float = 1e-4
     lambda_max: float = 1e7
+    caps: object = None   # lm_coll_oracle.Capsules or None: self-collision hinge rows
 
     def _c(self) -> _TParams:
-        return _TParams(self.w_pose, self.w_diff, self.lambda0, self.nu_up, self.nu_down,
-                        self.lambda_min, self.lambda_max)
+        t = _TParams(self.w_pose, self.w_diff, self.lambda0, self.nu_up, self.nu_down,
+                     self.lambda_min, self.lambda_max, None)
+        if self.caps is not None:
+            t._caps_keep = self.caps._c()          # keep the struct alive as long as the params struct
+            t.caps = C.addressof(t._caps_keep)
+        return t
 
 
 _ready = False
@@ -50,6 +56,8 @@ def _lib():
         ch, pp, tp = C.POINTER(_o._Chain), C.POINTER(_o._Params), C.POINTER(_TParams)
         L.orc_traj_rows.argtypes = [C.c_int32, C.c_int64]
         L.orc_traj_rows.restype = C.c_int64
+        L.orc_traj_rows_all.argtypes = [tp, C.c_int32, C.c_int64]
+        L.orc_traj_rows_all.restype = C.c_int64
         L.orc_traj_residual.argtypes = [ch, pp, tp, C.c_int64, _dp, _dp, _dp, _dp]
         L.orc_traj_residual.restype = None
         L.orc_traj_jacobian.argtypes = [ch, pp, tp, C.c_int64, _dp, _dp]
@@ -70,8 +78,11 @@ def _p(a):
     return a.ctypes.data_as(_dp)
 
 
-def rows(dof: int, n: int) -> int:
-    return int(_lib().orc_traj_rows(dof, n))
+def rows(dof: int, n: int, tparams: "TrajParams" = None) -> int:
+    if tparams is None:
+        return int(_lib().orc_traj_rows(dof, n))
+    tp = tparams._c()
+    return int(_lib().orc_traj_rows_all(C.byref(tp), dof, n))
 
 
 def residual(chain, pose_params: _o.Params, tparams: TrajParams, target_pos, target_quat, q):
@@ -79,7 +90,7 @@ def residual(chain, pose_params: _o.Params, tparams: TrajParams, target_pos, tar
     q = _o._f64(q)
     n, d = q.shape
     c, pp, tp = _o._chain_c(chain), pose_params._c(), tparams._c()
-    r = np.empty(rows(d, n))
+    r = np.empty(rows(d, n, tparams))
     _lib().orc_traj_residual(C.byref(c), C.byref(pp), C.byref(tp), n, _p(_o._f64(target_pos, (n, 3))),
                              _p(_o._f64(target_quat, (n, 4))), _p(q), _p(r))
     return r
@@ -90,7 +101,7 @@ def jacobian(chain, pose_params: _o.Params, tparams: TrajParams, q):
     q = _o._f64(q)
     n, d = q.shape
     c, pp, tp = _o._chain_c(chain), pose_params._c(), tparams._c()
-    J = np.empty((rows(d, n), n * d))
+    J = np.empty((rows(d, n, tparams), n * d))
     _lib().orc_traj_jacobian(C.byref(c), C.byref(pp), C.byref(tp), n, _p(q), _p(J))
     return J
 

@@ -87,6 +87,42 @@ def random_chain_8dof(seed: int = 3) -> Chain:
 
 
 @dataclass
+class CapsuleModel:
+    """Capsules rigidly attached to link frames and the pairs to check -- config data.
+    link[k] = -1 for the base (world) frame, j for the frame that joint j (0-based) moves."""
+    name: str
+    link: np.ndarray     # [K] int
+    a: np.ndarray        # [K, 3] endpoint in the link frame (m)
+    b: np.ndarray        # [K, 3]
+    radius: np.ndarray   # [K] (m)
+    pairs: np.ndarray    # [P, 2] capsule indices
+
+
+def panda_capsules() -> CapsuleModel:
+    """SYNTHETIC capsule model for the Panda DH chain (the paper fits capsules to the link meshes, which are
+    not available): one capsule per major link placed along the link's extent in its modified-DH frame --
+    base column, shoulder, upper arm, elbow, forearm, wrist, hand -- and the 9 pairs of non-adjacent links
+    that can actually meet."""
+    link = np.array([-1, 0, 2, 3, 4, 5, 6])
+    a = np.array([[0, 0, 0.0], [0, 0, -0.10], [0, 0, -0.25], [0, 0, -0.03], [0, 0, -0.30], [0, 0, -0.02], [0, 0, 0.02]], float)
+    b = np.array([[0, 0, 0.25], [0, 0, 0.0], [0, 0, -0.05], [0, 0, 0.03], [0, 0, -0.05], [0, 0, 0.05], [0, 0, 0.17]], float)
+    radius = np.array([0.09, 0.08, 0.07, 0.07, 0.06, 0.06, 0.05])
+    pairs = np.array([[0, 4], [0, 5], [0, 6], [1, 4], [1, 5], [1, 6], [2, 5], [2, 6], [3, 6]])
+    return CapsuleModel("panda_synthetic", link, a, b, radius, pairs)
+
+
+def chain_capsules(chain: "Chain", radius: float = 0.05) -> CapsuleModel:
+    """SYNTHETIC capsule model for any chain: one capsule per joint frame along its z axis (+-6 cm), one on the
+    base, all pairs at least three links apart."""
+    d = chain.dof
+    link = np.arange(-1, d)
+    a = np.tile(np.array([0, 0, -0.06]), (d + 1, 1)).astype(float)
+    b = np.tile(np.array([0, 0, 0.06]), (d + 1, 1)).astype(float)
+    pairs = np.array([[i, j] for i in range(d + 1) for j in range(i + 3, d + 1)])
+    return CapsuleModel(f"{chain.name}_synthetic", link, a, b, np.full(d + 1, radius), pairs)
+
+
+@dataclass
 class Workload:
     name: str
     chain: Chain
