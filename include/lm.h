@@ -208,6 +208,7 @@ typedef struct {
     float *cost;           /* [B] |r|^2 = w_pose^2 cost_pose + w_diff^2 cost_diff at the current q */
     float *cost_pose;      /* [B] sum_i |r_pose,i|^2 (pose weights w_pos / w_rot applied, w_pose not) */
     float *cost_diff;      /* [B] sum_k |q_{k+1} - q_k|^2: the trajectory-length surrogate of PAPER.md:L123 */
+    float *cost_coll;      /* [B] sum of the squared collision hinge residuals (0 without capsules); cost includes it */
     float *lambda;         /* [B] */
     int32_t *iters;        /* [B] trajectory-level iterations executed since lm_traj_attach / lm_traj_reset */
     uint64_t *accept_mask; /* [B] bit k = iteration k accepted */
@@ -236,6 +237,27 @@ int lm_traj_reset(lm_ctx *ctx, const float *lambda);
 
 /* Synchronise the stream and copy out the per-trajectory state of the trajectory-level step. */
 int lm_traj_fetch(lm_ctx *ctx, lm_traj_stats *stats_out);
+
+/* Robot-robot collision rows of the trajectory-level step:
+ * the robot is a set of capsules (endpoints a, b in the frame of a link, radius c); for every listed pair and
+ * every waypoint one hinge row  r = w_coll * max(0, d_safe - dist),  dist = min over t1, t2 in [0,1] of
+ * |(a1 + (b1-a1) t1) - (a2 + (b2-a2) t2)| - c1 - c2  (the paper's QP), with  d r / d q = -w_coll n^T (J_p1 - J_p2)
+ * at the closest points.  The rows add d x d terms to the diagonal blocks of the
+ * block-tridiagonal system and their squares to the cost.  HOST pointers, copied by the call; NULL, npairs = 0
+ * or w_coll = 0 removes the rows.  Requires lm_traj_attach (which also clears any capsules). */
+#define LM_MAX_CAPSULES 16
+#define LM_MAX_CAPSULE_PAIRS 32
+typedef struct {
+    int32_t ncaps;
+    const int32_t *link;   /* [ncaps] -1 = base (world) frame, j = the frame joint j (0-based) moves */
+    const float *a, *b;    /* [ncaps][3] endpoints in the link frame (m) */
+    const float *radius;   /* [ncaps] (m) */
+    int32_t npairs;
+    const int32_t *pairs;  /* [npairs][2] capsule indices */
+    float w_coll;          /* weight of a collision row */
+    float d_safe;          /* clearance below which a pair is penalised (m) */
+} lm_capsules;
+int lm_traj_set_capsules(lm_ctx *ctx, const lm_capsules *model);
 
 /* Debug trace (device pointers, nullable, borrowed): every executed iteration overwrites
  * trial_q [d][W] (w-order) = the clamped trial point and trial_F [2][B] = (|r|^2 before, at the trial point). */

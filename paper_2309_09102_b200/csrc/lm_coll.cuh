@@ -1,0 +1,155 @@
+// lm_coll.cuh -- robot-robot collision rows of the trajectory-level step (sm_100a).
+//
+// "each robot is represented as a set of capsules with endpoints (a, b) and radius c ... the minimum distance
+//  between a capsule pair [is] the minimum cost, less c1 + c2, of [the] convex quadratic program
+//  min |(a1 + (b1 - a1) t1) - (a2 + (b2 - a2) t2)|^2, 0 <= t1, t2 <= 1"
+// Per waypoint and listed pair one hinge row  r = w_coll * max(0, d_safe - dist)  (C4)
+// with  d r / d q = -w_coll n^T (J_p1 - J_p2),  n = (p1 - p2) / |p1 - p2|  (C5): the closest points are held
+// fixed on their links, which is what forward-mode differentiation through the QP solution gives
+// (PAPER.md:L168).  Joints that move BOTH links of a pair move the two points rigidly together and drop
+// out, so only the joints between the two links contribute.
+//
+// The box-constrained 2-variable QP is solved in closed form (the active set is found by clamping:
+// interior stationary point, else the edge minimisers), thread per waypoint; capsule endpoints are
+// carried into the world frame by a frame sink of the FK loop (lm_device.cuh).
+#pragma once
+#include "lm_device.cuh"
+
+namespace lmk {
+
+constexpr int MAX_CAPS = 16, MAX_PAIRS = 32;
+
+struct KCaps {
+    int32_t ncaps, npairs;
+    float w_coll, d_safe;
+    int8_t link[MAX_CAPS];          // -1 = base frame, j = frame moved by joint j
+    float a[MAX_CAPS][3], b[MAX_CAPS][3], c[MAX_CAPS];
+    uint8_t pair[MAX_PAIRS][2];
+};
+
+// world endpoints of the capsules: filled link by link while FK runs
+struct CapsWorld {
+    float wa[MAX_CAPS][3], wb[MAX_CAPS][3];
+};
+
+struct CapsSink {
+    const KCaps &C;
+    CapsWorld &W;
+    __device__ __forceinline__ CapsSink(const KCaps &c, CapsWorld &w) : C(c), W(w) {}
+    __device__ __forceinline__ void base() const { // capsules on the base link: the world frame
+        for (int k = 0; k < C.ncaps; ++k)
+            if (C.link[k] < 0) {
+#pragma unroll
+                for (int i = 0; i < 3; ++i) { W.wa[k][i] = C.a[k][i]; W.wb[k][i] = C.b[k][i]; }
+            }
+    }
+    __device__ __forceinline__ void operator()(int j, const float (&X)[3], const float (&Y)[3], const float (&Z)[3],
+                                               const float (&o)[3]) const {
+        for (int k = 0; k < C.ncaps; ++k)
+            if (C.link[k] == j) {
+#pragma unroll
+                for (int i = 0; i < 3; ++i) {
+                    W.wa[k][i] = fma_(Z[i], C.a[k][2], fma_(Y[i], C.a[k][1], fma_(X[i], C.a[k][0], o[i])));
+                    W.wb[k][i] = fma_(Z[i], C.b[k][2], fma_(Y[i], C.b[k][1], fma_(X[i], C.b[k][0], o[i])));
+                }
+            }
+    }
+};
+
+__device__ __forceinline__ float dot3(const float (&x)[3], const float (&y)[3]) {
+    return fma_(x[2], y[2], fma_(x[1], y[1], mul(x[0], y[0])));
+}
+__device__ __forceinline__ float clamp01(float x) { return fminf(fmaxf(x, 0.f), 1.f); }
+
+// minimiser (t1, t2) of |r + d1 t1 - d2 t2|^2 on the unit box, r = a1 - a2: the interior stationary point when
+// it is feasible, otherwise the better of the clamped edge minimisers (a convex quadratic on a box)
+__device__ __forceinline__ void segment_closest(const float (&a1)[3], const float (&b1)[3], const float (&a2)[3],
+                                                const float (&b2)[3], float &t1, float &t2) {
+    float d1[3], d2[3], r[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { d1[i] = sub(b1[i], a1[i]); d2[i] = sub(b2[i], a2[i]); r[i] = sub(a1[i], a2[i]); }
+    const float A = dot3(d1, d1), B = dot3(d1, d2), E = dot3(d2, d2), C = dot3(d1, r), F = dot3(d2, r);
+    const float det = fma_(A, E, -mul(B, B));
+    float s1 = 0.f, s2 = 0.f;
+    bool interior = false;
+    if (det > 1e-6f * mul(A, E)) {
+        const float inv = __fdividef(1.0f, det);
+        s1 = mul(fma_(B, F, -mul(C, E)), inv);
+        s2 = mul(fma_(A, F, -mul(B, C)), inv);
+        interior = (s1 >= 0.f) && (s1 <= 1.f) && (s2 >= 0.f) && (s2 <= 1.f);
+    }
+    if (!interior) {
+        const float iA = A > 0.f ? __fdividef(1.0f, A) : 0.f, iE = E > 0.f ? __fdividef(1.0f, E) : 0.f;
+        float best = 3.0e38f;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            float u1, u2;
+            if (e < 2) { u1 = (float)e; u2 = clamp01(mul(fma_(B, u1, F), iE)); }
+            else { u2 = (float)(e - 2); u1 = clamp01(mul(fma_(B, u2, -C), iA)); }
+            float cst = 0.f;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                const float v = fma_(-d2[i], u2, fma_(d1[i], u1, r[i]));
+                cst = fma_(v, v, cst);
+            }
+            if (cst < best) { best = cst; s1 = u1; s2 = u2; }
+        }
+    }
+    t1 = s1; t2 = s2;
+}
+
+// Calls f(g, r) for every pair whose hinge is active at this waypoint: g[D] = d r / d q, r = the residual.
+// Fr = frames retained by FK (Fr.Jw[j] = z_j, Fr.Jv[j] = o_j: eval_pose with WITH_JAC = false).
+template <int D, typename SpecT, typename F>
+__device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, const CapsWorld &W, const Pose<D> &Fr, F &&f) {
+    constexpr ChainSpec S = SpecT::spec;
+    for (int p = 0; p < C.npairs; ++p) {
+        const int k1 = C.pair[p][0], k2 = C.pair[p][1];
+        float a1[3], b1[3], a2[3], b2[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { a1[i] = W.wa[k1][i]; b1[i] = W.wb[k1][i]; a2[i] = W.wa[k2][i]; b2[i] = W.wb[k2][i]; }
+        float t1, t2;
+        segment_closest(a1, b1, a2, b2, t1, t2);
+        float p1[3], p2[3], e[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            p1[i] = fma_(sub(b1[i], a1[i]), t1, a1[i]);
+            p2[i] = fma_(sub(b2[i], a2[i]), t2, a2[i]);
+            e[i] = sub(p1[i], p2[i]);
+        }
+        const float len = sqrtf(dot3(e, e));
+        const float dist = sub(sub(len, C.c[k1]), C.c[k2]);
+        if (!(dist < C.d_safe) || !(len > 0.f)) continue;
+        const float r = mul(C.w_coll, sub(C.d_safe, dist));
+        const float il = __fdividef(1.0f, len);
+        const float n[3] = {mul(e[0], il), mul(e[1], il), mul(e[2], il)};
+        const int L1 = C.link[k1], L2 = C.link[k2];
+        const int lo = min(L1, L2), hi = max(L1, L2);
+        // the point on the link farther down the chain; its motion relative to the other point
+        const float sgn = (L1 > L2) ? -C.w_coll : C.w_coll; // d r / d q_j = -w n.c1 (L1 farther) or +w n.c2 (L2 farther)
+        float g[D];
+#pragma unroll
+        for (int j = 0; j < D; ++j) {
+            float gj = 0.f;
+            if (j > lo && j <= hi) {
+                const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
+                const float z[3] = {Fr.Jw[j][0], Fr.Jw[j][1], Fr.Jw[j][2]};
+                float col[3];
+                if (pris) { col[0] = z[0]; col[1] = z[1]; col[2] = z[2]; }
+                else {
+                    float d[3];
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) d[i] = sub((L1 > L2) ? p1[i] : p2[i], Fr.Jv[j][i]);
+                    col[0] = fma_(z[1], d[2], -mul(z[2], d[1]));
+                    col[1] = fma_(z[2], d[0], -mul(z[0], d[2]));
+                    col[2] = fma_(z[0], d[1], -mul(z[1], d[0]));
+                }
+                gj = mul(sgn, dot3(n, col));
+            }
+            g[j] = gj;
+        }
+        f(g, r);
+    }
+}
+
+} // namespace lmk

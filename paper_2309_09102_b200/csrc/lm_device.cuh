@@ -227,10 +227,16 @@ __device__ __forceinline__ void finish_jacobian(const KChain &ch, const Pose<D> 
 //   A_j = Rot_x(alpha) Trans_x(a) Rot_z(theta) Trans_z(d);  frame columns X, Y, Z and origin o.
 //   WITH_JAC = false: S3 is left to the caller (finish_jacobian); P.Jw / P.Jv then hold z_j / o_j and
 //   frame_p (nullable) receives the flange position.
-template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool WITH_JAC = true>
+//   sink(j, X, Y, Z, o) is called with the frame of every link right after joint j (collision capsules ride on
+//   link frames, lm_traj.cuh); the default does nothing.
+struct NoFrameSink {
+    __device__ __forceinline__ void operator()(int, const float (&)[3], const float (&)[3], const float (&)[3], const float (&)[3]) const {}
+};
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool WITH_JAC = true, typename Sink = NoFrameSink>
 __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D], const float (&pt)[3],
                                           const float (&Rt)[3][3], float w_pos, float w_rot,
-                                          Pose<D> &P, float *p_out, float (*R_out)[3], float *frame_p = nullptr) {
+                                          Pose<D> &P, float *p_out, float (*R_out)[3], float *frame_p = nullptr,
+                                          const Sink &sink = Sink()) {
     constexpr ChainSpec S = SpecT::spec;
     float X[3], Y[3], Z[3], o[3];
 #pragma unroll
@@ -265,6 +271,7 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
             o[2] = d_zero ? 0.f : (al0 ? dj : (alp || aln) ? 0.f : mul(dj, z1[2]));
 #pragma unroll
             for (int i = 0; i < 3; ++i) { Z[i] = z1[i]; P.Jw[j][i] = z1[i]; P.Jv[j][i] = o[i]; }
+            sink(j, X, Y, Z, o);
             continue;
         }
 #pragma unroll
@@ -285,6 +292,7 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
             P.Jw[j][i] = z1;                                                // joint axis z_j
             P.Jv[j][i] = o[i];                                              // frame origin o_j (-> J_v below)
         }
+        sink(j, X, Y, Z, o);
     }
     // flange: p = o + R tool_p ;  R_ee = R R_tool
     float p[3];

@@ -22,6 +22,7 @@
 // workspace holds and never store.
 // Determinism: fixed summation orders, no float atomics; explicit round-to-nearest intrinsics.
 #pragma once
+#include "lm_coll.cuh"
 #include "lm_device.cuh"
 #include "lm_kernels.cuh"
 
@@ -40,16 +41,17 @@ struct TArgs {
     float *tp_w, *tq_w;            // the same arrays, writable (pack kernel)
     float *q;                      // [2] x D comps     current / candidate joint values
     float *Ag;                     // [2] x (NA + D)    w_p^2 J^T J (packed lower), then g = J^T r of the stacked residual
-    float *cst;                    // [2] x 2           |r_pose,i|^2 and |q_{i+1} - q_i|^2 (0 for the last waypoint)
+    float *cst;                    // [2] x 3           |r_pose,i|^2, |q_{i+1} - q_i|^2 (0 for the last waypoint), collision cost
     float *V;                      // NA                -(S_i)^-1
     float *z;                      // D
     float *delta;                  // D
     float *rho;                    // D
-    float *lam, *F, *Fp, *Fd;      // [Bt * 32] per trajectory
+    float *lam, *F, *Fp, *Fd, *Fc; // [Bt * 32] per trajectory
     uint32_t *its;                 // iters | status << 8
     unsigned long long *mask;
     int32_t *sel;                  // which of the two buffers holds the trajectory's current point
     int32_t *ok;                   // this iteration's solve succeeded
+    KCaps caps;                    // self-collision capsules (npairs = 0: none), lm_coll.cuh
     const int32_t *gate;           // nullable: only trajectories with gate[b] != 0 take the step (lm_plan_run)
     float *trace_q, *trace_F;      // nullable: trial point [D][W] in w-order (w = b n + i), (F, F+) [2][B]
     const float *src_q;            // pack: [D][W] w-order
@@ -128,9 +130,11 @@ __device__ __forceinline__ void tl_load_target(const TArgs &A, const Slot &s, fl
 
 // w_p^2 J^T J (packed lower) and g = w_p^2 J^T r + w_d^2 (c_i y_i - y_{i-1} - y_{i+1}) (y = the joint
 // values the Jacobian was taken at), |r_pose|^2 and |y_{i+1} - y_i|^2 of one waypoint -> buffer `dstsel`
+// Ac, gc, fc: the collision rows' J_c^T J_c (packed lower), J_c^T r_c and |r_c|^2 (zeros without capsules)
 template <int D>
 __device__ __forceinline__ void tl_store_normal(const TArgs &A, const Pose<D> &P, int dstsel, const Slot &s,
-                                                const float (&y)[D], const float (&ym)[D], const float (&yn)[D]) {
+                                                const float (&y)[D], const float (&ym)[D], const float (&yn)[D],
+                                                const float (&Ac)[Tri<D>::NA], const float (&gc)[D], float fc) {
     constexpr int NA = Tri<D>::NA, C = NA + D;
     const int n = A.n;
     const float ci = (n == 1) ? 0.f : ((s.i == 0 || s.i == n - 1) ? 1.f : 2.f);
@@ -139,21 +143,57 @@ __device__ __forceinline__ void tl_store_normal(const TArgs &A, const Pose<D> &P
 #pragma unroll
     for (int r = 0; r < D; ++r) {
 #pragma unroll
-        for (int c = 0; c <= r; ++c) Ad[toff<C>(s.wid, tri(r, c), s.lane)] = mul(A.wp2, coldot<D>(P, r, c));
+        for (int c = 0; c <= r; ++c) Ad[toff<C>(s.wid, tri(r, c), s.lane)] = fma_(A.wp2, coldot<D>(P, r, c), Ac[tri(r, c)]);
         const float dd = sub(sub(mul(ci, y[r]), ym[r]), yn[r]);
-        Ad[toff<C>(s.wid, NA + r, s.lane)] = fma_(A.wd2, dd, mul(A.wp2, colvec<D>(P, r, P.r)));
+        Ad[toff<C>(s.wid, NA + r, s.lane)] = fma_(A.wd2, dd, fma_(A.wp2, colvec<D>(P, r, P.r), gc[r]));
         if (s.i + 1 < n) {
             const float t = sub(yn[r], y[r]);
             fd = fma_(t, t, fd);
         }
     }
-    float *cd = A.cst + (int64_t)dstsel * 2 * A.nS;
-    cd[toff<2>(s.wid, 0, s.lane)] = P.F;
-    cd[toff<2>(s.wid, 1, s.lane)] = fd;
+    float *cd = A.cst + (int64_t)dstsel * 3 * A.nS;
+    cd[toff<3>(s.wid, 0, s.lane)] = P.F;
+    cd[toff<3>(s.wid, 1, s.lane)] = fd;
+    cd[toff<3>(s.wid, 2, s.lane)] = fc;
+}
+
+// FK + residual + Jacobian of one waypoint and, when capsules are set, its collision rows
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
+__device__ __forceinline__ void tl_eval_waypoint(const TArgs &A, const float (&q)[D], const float (&pt)[3], const float (&Rt)[3][3],
+                                                 Pose<D> &P, float (&Ac)[Tri<D>::NA], float (&gc)[D], float &fc) {
+    constexpr int NA = Tri<D>::NA;
+#pragma unroll
+    for (int t = 0; t < NA; ++t) Ac[t] = 0.f;
+#pragma unroll
+    for (int j = 0; j < D; ++j) gc[j] = 0.f;
+    fc = 0.f;
+    if (COLL) {
+        Pose<D> Fr; // frames: Fr.Jw = z_j, Fr.Jv = o_j
+        CapsWorld W;
+        CapsSink sink(A.caps, W);
+        sink.base();
+        float pf[3];
+        eval_pose<D, FAST, WEIGHTED, SpecT, false, CapsSink>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, Fr, nullptr, nullptr, pf, sink);
+        coll_rows<D, SpecT>(A.ch, A.caps, W, Fr, [&](const float (&g)[D], float r) {
+#pragma unroll
+            for (int a = 0; a < D; ++a) {
+#pragma unroll
+                for (int b = 0; b <= a; ++b) Ac[tri(a, b)] = fma_(g[a], g[b], Ac[tri(a, b)]);
+                gc[a] = fma_(g[a], r, gc[a]);
+            }
+            fc = fma_(r, r, fc);
+        });
+        finish_jacobian<D, WEIGHTED, SpecT>(A.ch, Fr, pf, A.w_pos, A.w_rot, P);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) P.r[k] = Fr.r[k];
+        P.F = Fr.F;
+    } else {
+        eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+    }
 }
 
 // ---- assemble at the current point (entry of lm_traj_run): thread per waypoint
-template <int D, bool FAST, bool WEIGHTED, typename SpecT>
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_assemble_kernel(const __grid_constant__ TArgs A) {
     const Slot s = slot_of_thread(A);
     if (!s.valid) return;
@@ -169,8 +209,9 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_assemble_ker
     float pt[3], Rt[3][3];
     tl_load_target(A, s, pt, Rt);
     Pose<D> P;
-    eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
-    tl_store_normal<D>(A, P, sel, s, q, qm, qn);
+    float Ac[Tri<D>::NA], gc[D], fc;
+    tl_eval_waypoint<D, FAST, WEIGHTED, SpecT, COLL>(A, q, pt, Rt, P, Ac, gc, fc);
+    tl_store_normal<D>(A, P, sel, s, q, qm, qn, Ac, gc, fc);
 }
 
 // Kahan-compensated sum step (explicit intrinsics: the compiler cannot simplify the compensation away)
@@ -186,45 +227,51 @@ __device__ __forceinline__ void kahan_add(float &s, float &c, float x) {
 // in segment order.  The summation order depends on n only, never on the batch.  All threads of the
 // block must call; the result is valid in warp 0.
 constexpr int TL_SUM_WARPS = 8;
-__device__ __forceinline__ void tl_sum_cost(const TArgs &A, int sel, float (*part)[2][32], float &Fp, float &Fd, float &F) {
+__device__ __forceinline__ void tl_sum_cost(const TArgs &A, int sel, float (*part)[3][32], float &Fp, float &Fd, float &Fc, float &F) {
     const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
-    const float *cp = A.cst + (int64_t)sel * 2 * A.nS;
+    const float *cp = A.cst + (int64_t)sel * 3 * A.nS;
     const int64_t w0 = (int64_t)blockIdx.x * A.n;
     const int seg = (A.n + TL_SUM_WARPS - 1) / TL_SUM_WARPS;
     const int i0 = wp * seg, i1 = min(A.n, i0 + seg);
-    float sp = 0.f, cpp = 0.f, sd = 0.f, cd = 0.f;
+    float sm[3] = {0.f, 0.f, 0.f}, cm[3] = {0.f, 0.f, 0.f};
     int i = i0;
-    for (; i + 8 <= i1; i += 8) { // 16 independent loads in flight, then the sums in order
-        float a[8], d[8];
+    for (; i + 8 <= i1; i += 8) { // 24 independent loads in flight, then the sums in order
+        float a[8][3];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) { a[u] = cp[toff<2>(w0 + i + u, 0, lane)]; d[u] = cp[toff<2>(w0 + i + u, 1, lane)]; }
+        for (int u = 0; u < 8; ++u)
 #pragma unroll
-        for (int u = 0; u < 8; ++u) { kahan_add(sp, cpp, a[u]); kahan_add(sd, cd, d[u]); }
+            for (int c = 0; c < 3; ++c) a[u][c] = cp[toff<3>(w0 + i + u, c, lane)];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) kahan_add(sm[c], cm[c], a[u][c]);
     }
-    for (; i < i1; ++i) {
-        kahan_add(sp, cpp, cp[toff<2>(w0 + i, 0, lane)]);
-        kahan_add(sd, cd, cp[toff<2>(w0 + i, 1, lane)]);
-    }
-    part[wp][0][lane] = sp;
-    part[wp][1][lane] = sd;
+    for (; i < i1; ++i)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) kahan_add(sm[c], cm[c], cp[toff<3>(w0 + i, c, lane)]);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) part[wp][c][lane] = sm[c];
     __syncthreads();
-    sp = 0.f; cpp = 0.f; sd = 0.f; cd = 0.f;
 #pragma unroll
-    for (int u = 0; u < TL_SUM_WARPS; ++u) { kahan_add(sp, cpp, part[u][0][lane]); kahan_add(sd, cd, part[u][1][lane]); }
-    Fp = sp; Fd = sd;
-    F = fma_(A.wd2, sd, mul(A.wp2, sp));
+    for (int c = 0; c < 3; ++c) {
+        sm[c] = 0.f; cm[c] = 0.f;
+#pragma unroll
+        for (int u = 0; u < TL_SUM_WARPS; ++u) kahan_add(sm[c], cm[c], part[u][c][lane]);
+    }
+    Fp = sm[0]; Fd = sm[1]; Fc = sm[2];
+    F = add(fma_(A.wd2, sm[1], mul(A.wp2, sm[0])), sm[2]);
 }
 
 #ifdef LM_TRAJ_PLAIN_KERNELS // non-template kernels: defined in exactly one translation unit (lm_traj_api.cu)
 // ---- cost of the current point (entry of lm_traj_run): block of TL_SUM_WARPS warps per tile
 __global__ void __launch_bounds__(TL_SUM_WARPS * 32) tl_init_cost_kernel(const __grid_constant__ TArgs A) {
-    __shared__ float part[TL_SUM_WARPS][2][32];
+    __shared__ float part[TL_SUM_WARPS][3][32];
     const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
     const bool valid = b < A.B;
-    float Fp, Fd, F;
-    tl_sum_cost(A, valid ? A.sel[b] : 0, part, Fp, Fd, F);
+    float Fp, Fd, Fc, F;
+    tl_sum_cost(A, valid ? A.sel[b] : 0, part, Fp, Fd, Fc, F);
     if (!valid || threadIdx.x >= 32) return;
-    A.Fp[b] = Fp; A.Fd[b] = Fd; A.F[b] = F;
+    A.Fp[b] = Fp; A.Fd[b] = Fd; A.Fc[b] = Fc; A.F[b] = F;
 }
 #endif
 
@@ -524,8 +571,9 @@ __global__ void __launch_bounds__(64) tl_solve_kernel(const __grid_constant__ TA
 }
 
 // ---- refinement residual (DESIGN R4 carried over to the stacked system): thread per waypoint
-//   rho_i = -[ w_p^2 J_i^T (r_i + J_i delta_i) + w_d^2 (D^T D (q + delta))_i + lambda delta_i ]
-template <int D, bool FAST, bool WEIGHTED, typename SpecT>
+//   rho_i = -[ w_p^2 J_i^T (r_i + J_i delta_i) + w_d^2 (D^T D (q + delta))_i + lambda delta_i
+//             + sum over active collision pairs of g (r_c + g . delta_i) ]
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(const __grid_constant__ TArgs A) {
     const Slot s = slot_of_thread(A);
     if (!s.valid) return;
@@ -562,7 +610,29 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(c
     float pt[3], Rt[3][3];
     tl_load_target(A, s, pt, Rt);
     Pose<D> P;
-    eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+    float ec[D]; // collision rows: sum over the active pairs of g (r + g . delta)
+#pragma unroll
+    for (int j = 0; j < D; ++j) ec[j] = 0.f;
+    if (COLL) {
+        Pose<D> Fr;
+        CapsWorld W;
+        CapsSink sink(A.caps, W);
+        sink.base();
+        float pf[3];
+        eval_pose<D, FAST, WEIGHTED, SpecT, false, CapsSink>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, Fr, nullptr, nullptr, pf, sink);
+        coll_rows<D, SpecT>(A.ch, A.caps, W, Fr, [&](const float (&g)[D], float r) {
+            float u = r;
+#pragma unroll
+            for (int j = 0; j < D; ++j) u = fma_(g[j], dl[j], u);
+#pragma unroll
+            for (int j = 0; j < D; ++j) ec[j] = fma_(g[j], u, ec[j]);
+        });
+        finish_jacobian<D, WEIGHTED, SpecT>(A.ch, Fr, pf, A.w_pos, A.w_rot, P);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) P.r[k] = Fr.r[k];
+    } else {
+        eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+    }
     float t[6];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
@@ -576,14 +646,14 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(c
     }
 #pragma unroll
     for (int j = 0; j < D; ++j) {
-        const float acc = fma_(lam, dl[j], fma_(A.wd2, dd[j], mul(A.wp2, colvec<D>(P, j, t))));
+        const float acc = add(fma_(lam, dl[j], fma_(A.wd2, dd[j], mul(A.wp2, colvec<D>(P, j, t)))), ec[j]);
         A.rho[toff<D>(s.wid, j, s.lane)] = -acc;
     }
 }
 
 // ---- trial point: q+ = clamp(q + delta), its cost terms and its normal equations
 //      into the candidate buffer (1 - sel): thread per waypoint
-template <int D, bool FAST, bool WEIGHTED, typename SpecT>
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_trial_kernel(const __grid_constant__ TArgs A) {
     const Slot s = slot_of_thread(A);
     if (!s.valid) return;
@@ -629,8 +699,9 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_trial_kernel
     // "a trial point of this trajectory was clamped": integer atomic (order-free), skipped once the bit is seen set
     if (clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
     Pose<D> P;
-    eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
-    tl_store_normal<D>(A, P, 1 - sel, s, qt, qm, qn);
+    float Ac[Tri<D>::NA], gc[D], fc;
+    tl_eval_waypoint<D, FAST, WEIGHTED, SpecT, COLL>(A, qt, pt, Rt, P, Ac, gc, fc);
+    tl_store_normal<D>(A, P, 1 - sel, s, qt, qm, qn, Ac, gc, fc);
     if (A.trace_q != nullptr) {
         const int64_t W = A.B * A.n, w = s.b * A.n + s.i;
 #pragma unroll
@@ -641,12 +712,12 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_trial_kernel
 #ifdef LM_TRAJ_PLAIN_KERNELS
 // ---- accept / reject and the lambda update, per trajectory (DESIGN T3 = R5 on the total cost)
 __global__ void __launch_bounds__(TL_SUM_WARPS * 32) tl_decide_kernel(const __grid_constant__ TArgs A) {
-    __shared__ float part[TL_SUM_WARPS][2][32];
+    __shared__ float part[TL_SUM_WARPS][3][32];
     const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
     const bool valid = b < A.B;
     const int s = valid ? A.sel[b] : 0;
-    float Fp, Fd, Ft;
-    tl_sum_cost(A, 1 - s, part, Fp, Fd, Ft);
+    float Fp, Fd, Fc, Ft;
+    tl_sum_cost(A, 1 - s, part, Fp, Fd, Fc, Ft);
     if (!valid || threadIdx.x >= 32) return;
     uint32_t pk = A.its[b];
     uint32_t k = pk & 0xffu, st = pk >> 8;
@@ -666,7 +737,7 @@ __global__ void __launch_bounds__(TL_SUM_WARPS * 32) tl_decide_kernel(const __gr
         lam = fmaxf(mul(lam, A.inv_nu_down), A.lambda_min);
         A.mask[b] |= 1ull << k;
         A.sel[b] = 1 - s;
-        A.F[b] = Ft; A.Fp[b] = Fp; A.Fd[b] = Fd;
+        A.F[b] = Ft; A.Fp[b] = Fp; A.Fd[b] = Fd; A.Fc[b] = Fc;
     } else {
         lam = fminf(mul(lam, A.nu_up), A.lambda_max);
     }

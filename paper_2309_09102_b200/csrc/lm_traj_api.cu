@@ -12,7 +12,7 @@ using namespace lmk;
 namespace {
 
 struct TLayout {
-    size_t tp, tq, q, Ag, cst, V, z, delta, rho, lam, F, Fp, Fd, its, mask, sel, ok, totals, ui, us, total;
+    size_t tp, tq, q, Ag, cst, V, z, delta, rho, lam, F, Fp, Fd, Fc, its, mask, sel, ok, totals, ui, us, total;
 };
 
 // tile order (lm_traj.cuh): Bt = ceil(B / 32) tiles, nS = Bt * n * 32 slots, C floats per slot and array
@@ -25,7 +25,7 @@ TLayout make_tlayout(int d, int64_t B, int64_t n) {
     L.tq = take(4 * 4 * nS);
     L.q = take(4 * 2 * d * nS);
     L.Ag = take(4 * 2 * (NA + d) * nS);
-    L.cst = take(4 * 2 * 2 * nS);
+    L.cst = take(4 * 2 * 3 * nS);
     L.V = take(4 * NA * nS);
     L.z = take(4 * d * nS);
     L.delta = take(4 * d * nS);
@@ -34,6 +34,7 @@ TLayout make_tlayout(int d, int64_t B, int64_t n) {
     L.F = take(4 * Bp);
     L.Fp = take(4 * Bp);
     L.Fd = take(4 * Bp);
+    L.Fc = take(4 * Bp);
     L.its = take(4 * Bp);
     L.mask = take(8 * Bp);
     L.sel = take(4 * Bp);
@@ -135,7 +136,7 @@ int lm_traj_attach(lm_ctx *c, const lm_traj_params *p, void *workspace, size_t b
         a.tp = a.tp_w = f(L.tp); a.tq = a.tq_w = f(L.tq);
     }
     a.q = f(L.q); a.Ag = f(L.Ag); a.cst = f(L.cst); a.V = f(L.V); a.z = f(L.z);
-    a.delta = f(L.delta); a.rho = f(L.rho); a.lam = f(L.lam); a.F = f(L.F); a.Fp = f(L.Fp); a.Fd = f(L.Fd);
+    a.delta = f(L.delta); a.rho = f(L.rho); a.lam = f(L.lam); a.F = f(L.F); a.Fp = f(L.Fp); a.Fd = f(L.Fd); a.Fc = f(L.Fc);
     a.its = reinterpret_cast<uint32_t *>(t.ws + L.its);
     a.mask = reinterpret_cast<unsigned long long *>(t.ws + L.mask);
     a.sel = reinterpret_cast<int32_t *>(t.ws + L.sel);
@@ -156,6 +157,28 @@ int lm_traj_reset(lm_ctx *c, const float *lambda) {
     launch_counter().fetch_add(1);
     tl_reset_kernel<<<(unsigned)((t.args.Bt * 32 + 255) / 256), 256, 0, c->stream>>>(t.args, lam_dev, t.lambda0);
     LM_CUDA(cudaGetLastError());
+    return LM_OK;
+}
+
+int lm_traj_set_capsules(lm_ctx *c, const lm_capsules *m) {
+    if (!c || !c->traj.attached) return LM_EINVAL;
+    KCaps &k = c->traj.args.caps;
+    std::memset(&k, 0, sizeof(k));
+    if (!m || m->npairs == 0 || m->w_coll == 0.f) return LM_OK; // no collision rows
+    if (m->ncaps < 1 || m->ncaps > LM_MAX_CAPSULES || m->npairs < 0 || m->npairs > LM_MAX_CAPSULE_PAIRS) return LM_EINVAL;
+    if (!m->link || !m->a || !m->b || !m->radius || !m->pairs || !(m->w_coll > 0.f) || !(m->d_safe >= 0.f)) return LM_EINVAL;
+    for (int i = 0; i < m->ncaps; ++i) {
+        if (m->link[i] < -1 || m->link[i] >= c->dof || !(m->radius[i] >= 0.f)) return LM_EINVAL;
+        k.link[i] = (int8_t)m->link[i];
+        k.c[i] = m->radius[i];
+        for (int x = 0; x < 3; ++x) { k.a[i][x] = m->a[3 * i + x]; k.b[i][x] = m->b[3 * i + x]; }
+    }
+    for (int p = 0; p < m->npairs; ++p) {
+        const int32_t k1 = m->pairs[2 * p], k2 = m->pairs[2 * p + 1];
+        if (k1 < 0 || k1 >= m->ncaps || k2 < 0 || k2 >= m->ncaps || k1 == k2) return LM_EINVAL;
+        k.pair[p][0] = (uint8_t)k1; k.pair[p][1] = (uint8_t)k2;
+    }
+    k.ncaps = m->ncaps; k.npairs = m->npairs; k.w_coll = m->w_coll; k.d_safe = m->d_safe;
     return LM_OK;
 }
 
@@ -211,6 +234,7 @@ int lm_traj_fetch(lm_ctx *c, lm_traj_stats *s) {
     LM_CUDA(out(s->cost, a.F, 4 * B));
     LM_CUDA(out(s->cost_pose, a.Fp, 4 * B));
     LM_CUDA(out(s->cost_diff, a.Fd, 4 * B));
+    LM_CUDA(out(s->cost_coll, a.Fc, 4 * B));
     LM_CUDA(out(s->lambda, a.lam, 4 * B));
     LM_CUDA(out(s->accept_mask, a.mask, 8 * B));
     unsigned long long *tot = reinterpret_cast<unsigned long long *>(t.ws + t.off_totals);

@@ -18,21 +18,21 @@ cudaError_t launch_traj_plain(int which, int dof, unsigned grid, unsigned block,
 
 template <int D, typename SpecT>
 cudaError_t launch_traj_pose_t(int which, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a) {
+    const bool coll = a.caps.npairs > 0; // collision rows: their own instantiations (lm_coll.cuh)
+#define LM_TL_LAUNCH(K)                                                                   \
+    do {                                                                                  \
+        if (weighted) { if (coll) K<D, false, true, SpecT, true><<<grid, block, 0, s>>>(a);   \
+                        else K<D, false, true, SpecT, false><<<grid, block, 0, s>>>(a); }     \
+        else { if (coll) K<D, false, false, SpecT, true><<<grid, block, 0, s>>>(a);           \
+               else K<D, false, false, SpecT, false><<<grid, block, 0, s>>>(a); }             \
+    } while (0)
     switch (which) {
-    case TK_ASSEMBLE:
-        if (weighted) tl_assemble_kernel<D, false, true, SpecT><<<grid, block, 0, s>>>(a);
-        else tl_assemble_kernel<D, false, false, SpecT><<<grid, block, 0, s>>>(a);
-        break;
-    case TK_RHO:
-        if (weighted) tl_rho_kernel<D, false, true, SpecT><<<grid, block, 0, s>>>(a);
-        else tl_rho_kernel<D, false, false, SpecT><<<grid, block, 0, s>>>(a);
-        break;
-    case TK_TRIAL:
-        if (weighted) tl_trial_kernel<D, false, true, SpecT><<<grid, block, 0, s>>>(a);
-        else tl_trial_kernel<D, false, false, SpecT><<<grid, block, 0, s>>>(a);
-        break;
+    case TK_ASSEMBLE: LM_TL_LAUNCH(tl_assemble_kernel); break;
+    case TK_RHO: LM_TL_LAUNCH(tl_rho_kernel); break;
+    case TK_TRIAL: LM_TL_LAUNCH(tl_trial_kernel); break;
     default: return cudaErrorInvalidValue;
     }
+#undef LM_TL_LAUNCH
     return cudaGetLastError();
 }
 

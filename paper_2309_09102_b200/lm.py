@@ -30,7 +30,7 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_option", "lm_kernel_name", "lm_fk", "lm_fp32_peak", "lm_free",
            "lm_strerror", "lm_launch_count", "lm_fp32_peak_form",
            "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
-           "lm_traj_fetch", "lm_traj_set_trace",
+           "lm_traj_fetch", "lm_traj_set_trace", "lm_traj_set_capsules",
            "lm_solve_host_workspace_bytes", "lm_solve_host",
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR = 0, 1
@@ -69,9 +69,15 @@ class LmTrajParams(C.Structure):
 
 
 class LmTrajStats(C.Structure):
-    _fields_ = [("cost", C.c_void_p), ("cost_pose", C.c_void_p), ("cost_diff", C.c_void_p),
+    _fields_ = [("cost", C.c_void_p), ("cost_pose", C.c_void_p), ("cost_diff", C.c_void_p), ("cost_coll", C.c_void_p),
                 ("lambda_", C.c_void_p), ("iters", C.c_void_p), ("accept_mask", C.c_void_p),
                 ("status", C.c_void_p), ("total_traj_iters", C.c_int64)]
+
+
+class LmCapsules(C.Structure):
+    _fields_ = [("ncaps", C.c_int32), ("link", C.POINTER(C.c_int32)), ("a", C.POINTER(C.c_float)), ("b", C.POINTER(C.c_float)),
+                ("radius", C.POINTER(C.c_float)), ("npairs", C.c_int32), ("pairs", C.POINTER(C.c_int32)),
+                ("w_coll", C.c_float), ("d_safe", C.c_float)]
 
 
 class LmPlanParams(C.Structure):
@@ -133,6 +139,7 @@ def lib() -> C.CDLL:
         L.lm_traj_reset.argtypes = [C.c_void_p, C.c_void_p]
         L.lm_traj_fetch.argtypes = [C.c_void_p, C.POINTER(LmTrajStats)]
         L.lm_traj_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lm_traj_set_capsules.argtypes = [C.c_void_p, C.POINTER(LmCapsules)]
         L.lm_solve_host_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.c_int32]
         L.lm_solve_host_workspace_bytes.restype = C.c_size_t
         L.lm_solve_host.argtypes = [C.POINTER(LmChain), C.POINTER(LmProblem), C.POINTER(LmParams), C.c_int32, C.c_int32,
@@ -278,6 +285,22 @@ def lm_traj_reset(ctx: int, lambda_ptr: Optional[int]) -> None:
 
 def lm_traj_fetch(ctx: int, stats: LmTrajStats) -> None:
     _check(lib().lm_traj_fetch(ctx, C.byref(stats)), "lm_traj_fetch")
+
+
+def lm_traj_set_capsules(ctx: int, model, w_coll: float = 1.0, d_safe: float = 0.05) -> None:
+    """model: a workloads.CapsuleModel-like object (link, a, b, radius, pairs) or None to remove the rows."""
+    if model is None:
+        _check(lib().lm_traj_set_capsules(ctx, None), "lm_traj_set_capsules")
+        return
+    link = np.ascontiguousarray(model.link, dtype=np.int32)
+    a = np.ascontiguousarray(model.a, dtype=np.float32)
+    b = np.ascontiguousarray(model.b, dtype=np.float32)
+    rad = np.ascontiguousarray(model.radius, dtype=np.float32)
+    pairs = np.ascontiguousarray(model.pairs, dtype=np.int32)
+    m = LmCapsules(len(link), link.ctypes.data_as(C.POINTER(C.c_int32)), a.ctypes.data_as(C.POINTER(C.c_float)),
+                   b.ctypes.data_as(C.POINTER(C.c_float)), rad.ctypes.data_as(C.POINTER(C.c_float)), len(pairs),
+                   pairs.ctypes.data_as(C.POINTER(C.c_int32)), float(w_coll), float(d_safe))
+    _check(lib().lm_traj_set_capsules(ctx, C.byref(m)), "lm_traj_set_capsules")
 
 
 def lm_traj_set_trace(ctx: int, trial_q_ptr: Optional[int], trial_F_ptr: Optional[int]) -> None:
@@ -442,6 +465,9 @@ class Solver:
         ptr = (self.traj_workspace.data_ptr() + 255) // 256 * 256
         lm_traj_attach(self._ctx, self.tparams, ptr, nbytes)
 
+    def traj_set_capsules(self, model, w_coll: float = 1.0, d_safe: float = 0.05) -> None:
+        lm_traj_set_capsules(self._ctx, model, w_coll, d_safe)
+
     def traj_run(self, iters: int) -> None:
         lm_traj_run(self._ctx, iters)
 
@@ -468,10 +494,10 @@ class Solver:
             return torch.empty((B,), dtype=dtype).pin_memory()
 
         out = {"cost": buf(torch.float32), "cost_pose": buf(torch.float32), "cost_diff": buf(torch.float32),
-               "lam": buf(torch.float32), "iters": buf(torch.int32), "mask": buf(torch.int64),
+               "cost_coll": buf(torch.float32), "lam": buf(torch.float32), "iters": buf(torch.int32), "mask": buf(torch.int64),
                "status": buf(torch.int32)}
         st = LmTrajStats(out["cost"].data_ptr(), out["cost_pose"].data_ptr(), out["cost_diff"].data_ptr(),
-                         out["lam"].data_ptr(), out["iters"].data_ptr(), out["mask"].data_ptr(),
+                         out["cost_coll"].data_ptr(), out["lam"].data_ptr(), out["iters"].data_ptr(), out["mask"].data_ptr(),
                          out["status"].data_ptr(), 0)
         lm_traj_fetch(self._ctx, st)
         res = {k: v.numpy().copy() for k, v in out.items()}

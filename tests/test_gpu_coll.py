@@ -1,0 +1,141 @@
+"""GPU parity of the self-collision rows of the trajectory-level step (lm_traj_set_capsules, NEXT-3) against
+oracle/lm_coll_oracle.c + lm_traj_oracle.c: trial points within 1e-4 rad (measured ~1e-6), costs within 1e-4
+relative, same decisions where the oracle's margin is clear."""
+import numpy as np
+import pytest
+
+from oracle import lm_coll_oracle as corc
+from oracle import lm_oracle as orc
+from oracle import lm_traj_oracle as torc
+from paper_2309_09102_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+def folded_problem(ch, model, B, n, seed, base):
+    """Trajectories around a folded configuration (several capsule pairs closer than d_safe): a smooth random
+    walk in joint space, targets = FK(truth), seeds = truth + small noise; fp32-rounded."""
+    rng = np.random.default_rng(seed)
+    steps = 0.01 * rng.normal(size=(B, n, ch.dof))
+    truth = np.clip(base[None, None, :] + 0.1 * rng.normal(size=(B, 1, ch.dof)) + np.cumsum(steps, axis=1), ch.q_lo, ch.q_hi)
+    w = wl._from_truth("F", ch, truth, 0.01, rng, lambda q: orc.fk(ch, q), 0.0, 20)
+    return w
+
+
+def run_pair(ch, model, w, iters, w_coll, d_safe, w_pose=0.5, w_diff=0.3, lam=None, trace=True):
+    from paper_2309_09102_b200 import lm
+    B, n, d = w.B, w.n, ch.dof
+    s = lm.Solver(ch, B, n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0))
+    s.traj_attach(lm.lm_traj_default_params(w_pose=w_pose, w_diff=w_diff))
+    s.traj_set_capsules(model, w_coll, d_safe)
+    if lam is not None:
+        s.traj_reset(lam)
+    if trace:
+        s.traj_enable_trace()
+    s.traj_run(iters)
+    g = s.traj_fetch()
+    g["q"] = s.fetch()["q"].reshape(B, n, d)
+    s.close()
+    tprm = torc.TrajParams(w_pose=w_pose, w_diff=w_diff, caps=corc.Capsules(model, w_coll=w_coll, d_safe=d_safe))
+    st = torc.init_state(w.seeds.astype(np.float64).reshape(B, n, d), tprm)
+    if lam is not None:
+        st.lam[:] = lam.astype(np.float64)
+    tp = w.target_pos.astype(np.float64).reshape(B, n, 3)
+    tq = w.target_quat.astype(np.float64).reshape(B, n, 4)
+    tr = []
+    for _ in range(iters):
+        torc.advance(ch, orc.Params(), tprm, tp, tq, st, iters, at_most=1)
+        tr.append(st.copy())
+    return g, st, tr
+
+
+PANDA_FOLDED = np.array([0.0, 1.2, 0.0, -2.9, 0.0, 2.2, 0.8])
+
+
+def test_single_step_with_capsules_panda():
+    ch, model = wl.panda_chain(), wl.panda_capsules()
+    B, n = 21, 40
+    w = folded_problem(ch, model, B, n, 51, PANDA_FOLDED)
+    lam = (10.0 ** np.random.default_rng(1).uniform(-3, -1, size=B)).astype(np.float32)
+    g, st, _ = run_pair(ch, model, w, 1, w_coll=2.0, d_safe=0.25, lam=lam)
+    # the hinges are active on this workload (otherwise the test proves nothing)
+    caps = corc.Capsules(model, w_coll=2.0, d_safe=0.25)
+    q0 = w.seeds.astype(np.float64).reshape(B, n, 7)
+    active = sum(int((corc.residual(ch, caps, q0[b, i])[1] > 0).sum()) for b in range(0, B, 5) for i in range(0, n, 7))
+    assert active > 30
+    assert np.abs(g["trial_q"].reshape(B, n, 7) - st.trial_q).max() <= 2e-5
+    assert np.allclose(g["F_before"], st.F_before, rtol=1e-4) and np.allclose(g["F_trial"], st.F_trial, rtol=1e-4)
+    margin = np.abs(st.F_before - st.F_trial) > 1e-3 * st.F_before
+    acc = (g["mask"] & np.uint64(1)).astype(bool)
+    assert np.array_equal(acc[margin], (st.accepted == 1)[margin])
+    same = acc == (st.accepted == 1)
+    coll_o = st.F_total - 0.25 * st.F_pose - 0.09 * st.F_diff
+    assert np.allclose(g["cost_coll"][same], coll_o[same], rtol=1e-3, atol=1e-7)
+    assert (g["cost_coll"] > 0).mean() > 0.5
+
+
+def test_free_running_with_capsules():
+    """The Gauss-Newton matrix of a hinge row is discontinuous where the hinge switches (dist = d_safe): a pair
+    that fp32 sees on one side and fp64 on the other contributes a whole rank-1 term or nothing, and along a
+    trajectory some pair always sits near the switch.  Strict free-running parity is therefore asserted with
+    d_safe = 1 m (every listed pair stays active: a smooth problem); with a realistic d_safe the run must make
+    the same kind of progress as the oracle's."""
+    ch, model = wl.panda_chain(), wl.panda_capsules()
+    B, n, iters = 16, 40, 4
+    w = folded_problem(ch, model, B, n, 52, PANDA_FOLDED)
+    g, st, tr = run_pair(ch, model, w, iters, w_coll=0.3, d_safe=1.0, trace=False)
+    alive = np.ones(B, bool)
+    for k in range(iters):
+        gb = ((g["mask"] >> np.uint64(k)) & np.uint64(1)).astype(bool)
+        dec = alive & (np.abs(tr[k].F_before - tr[k].F_trial) > 1e-3 * tr[k].F_before)
+        assert np.array_equal(gb[dec], (tr[k].accepted == 1)[dec])
+        alive &= gb == (tr[k].accepted == 1)
+    assert alive.mean() > 0.8
+    assert np.abs(g["q"][alive] - st.q[alive]).max() <= 1e-4
+    assert np.allclose(g["cost"][alive], st.F_total[alive], rtol=1e-4)
+    assert np.allclose(g["cost_coll"][alive], (st.F_total - 0.25 * st.F_pose - 0.09 * st.F_diff)[alive], rtol=1e-4)
+    # realistic clearance threshold: cost down, worst clearance up, final cost close to the oracle's
+    g, st, tr = run_pair(ch, model, w, iters, w_coll=2.0, d_safe=0.25, trace=False)
+    caps = corc.Capsules(model, w_coll=2.0, d_safe=0.25)
+    q0 = w.seeds.astype(np.float64).reshape(B, n, 7)
+    assert np.all(g["cost"] < tr[0].F_before)
+    assert np.allclose(g["cost"], st.F_total, rtol=0.05)
+    before = min(corc.residual(ch, caps, q0[b, i])[0].min() for b in range(B) for i in range(0, n, 5))
+    after = min(corc.residual(ch, caps, g["q"][b, i].astype(np.float64))[0].min() for b in range(B) for i in range(0, n, 5))
+    assert after > before
+
+
+def test_single_step_with_capsules_8dof_prismatic():
+    ch = wl.random_chain_8dof(3)
+    model = wl.chain_capsules(ch)
+    B, n = 9, 30
+    base = 0.5 * (ch.q_lo + ch.q_hi)
+    w = folded_problem(ch, model, B, n, 53, base)
+    g, st, _ = run_pair(ch, model, w, 1, w_coll=1.0, d_safe=0.4)
+    assert (g["cost_coll"] > 0).any()
+    assert np.abs(g["trial_q"].reshape(B, n, 8) - st.trial_q).max() <= 2e-5
+    assert np.allclose(g["F_trial"], st.F_trial, rtol=1e-4)
+
+
+def test_no_capsules_is_bitwise_the_plain_step_and_errors():
+    from paper_2309_09102_b200 import lm
+    ch, model = wl.panda_chain(), wl.panda_capsules()
+    w = folded_problem(ch, model, 6, 25, 54, PANDA_FOLDED)
+    outs = []
+    for mode in ("never", "cleared"):
+        s = lm.Solver(ch, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0))
+        s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=0.3))
+        if mode == "cleared":
+            s.traj_set_capsules(model, 2.0, 0.25)
+            s.traj_set_capsules(None)
+        s.traj_run(3)
+        outs.append((s.fetch()["q"], s.traj_fetch()))
+        if mode == "never":
+            bad = wl.panda_capsules()
+            bad.link = bad.link.copy()
+            bad.link[1] = 9
+            with pytest.raises(lm.LmError):
+                s.traj_set_capsules(bad)
+        s.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1]["cost"], outs[1][1]["cost"])
+    assert np.all(outs[1][1]["cost_coll"] == 0)
