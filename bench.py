@@ -354,9 +354,9 @@ def run_gpu(args) -> None:
 
 def traj_step_alg_bytes(d: int, refine: int = 1) -> float:
     """HBM bytes one trajectory-level LM iteration must move per waypoint: fp32 words
-    factor+solve 3NA+4d, each refinement (rho 3d+7, re-solve 2NA+5d), trial NA+4d+9, decision 2."""
+    factor+solve 3NA+4d, each refinement (rho 3d+7, re-solve 2NA+5d), trial NA+4d+10, decision 3."""
     na = d * (d + 1) // 2
-    return 4.0 * ((3 * na + 4 * d) + refine * ((3 * d + 7) + (2 * na + 5 * d)) + (na + 4 * d + 9) + 2)
+    return 4.0 * ((3 * na + 4 * d) + refine * ((3 * d + 7) + (2 * na + 5 * d)) + (na + 4 * d + 10) + 3)
 
 
 def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: int = 5) -> dict:
@@ -383,13 +383,34 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
             if i >= 1:
                 ts.append(a.elapsed_time(b))
         g = solver.traj_fetch()
+        # the same iterations with the robot-robot collision rows (NEXT-3; synthetic Panda capsules, 9 pairs)
+        coll = None
+        if w.chain.name == "panda":
+            from paper_2309_09102_b200 import workloads as wl_
+            solver.traj_set_capsules(wl_.panda_capsules(), 1.0, 0.05)
+            tc = []
+            for i in range(reps + 1):
+                solver.reset()
+                solver.run(4)
+                solver.traj_reset()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                solver.traj_run(iters)
+                b.record(stream)
+                stream.synchronize()
+                if i >= 1:
+                    tc.append(a.elapsed_time(b))
+            gc_ = solver.traj_fetch()
+            solver.traj_set_capsules(None)
+            coll = {"ms_per_iteration": float(min(tc)) / iters, "capsules": 7, "pairs": 9, "w_coll": 1.0, "d_safe_m": 0.05,
+                    "trajectories_with_active_pairs": int((gc_["cost_coll"] > 0).sum())}
     ms_iter = float(min(ts)) / iters
     alg = traj_step_alg_bytes(d, int(tp.refine_steps)) * w.W
     out = {"workload": f"{w.name}: {w.B} x {w.n}, after 4 pose-only iterations; w_pose=1, w_diff=0.3, refine=1, {iters} iterations",
            "ms_per_iteration": ms_iter, "waypoint_iterations_per_sec": w.W / (ms_iter * 1e-3),
            "trajectory_iterations_per_sec": w.B / (ms_iter * 1e-3), "gpu_launches_per_run": int(launches),
            "accepted_fraction": float(np.mean([bin(int(m)).count("1") for m in g["mask"]])) / iters,
-           "cost_diff_mean": float(g["cost_diff"].mean()),
+           "cost_diff_mean": float(g["cost_diff"].mean()), "with_self_collision_rows": coll,
            "roofline": {"bound": "hbm", "achieved": alg / (ms_iter * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
                         "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps)),
