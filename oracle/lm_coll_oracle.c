@@ -55,6 +55,61 @@ double orc_segment_distance(const double *a1, const double *b1, const double *a2
     return sqrt(best);
 }
 
+static double box_cost(const double *a, const double *d, const double *pmin, const double *pmax, double t, double *p) {
+    double s = 0.0;
+    for (int i = 0; i < 3; ++i) {
+        const double x = a[i] + d[i] * t;
+        const double c = x < pmin[i] ? pmin[i] : (x > pmax[i] ? pmax[i] : x);
+        if (p) p[i] = c;
+        s += (x - c) * (x - c);
+    }
+    return s;
+}
+
+double orc_segment_box_distance(const double *a, const double *b, const double *pmin, const double *pmax,
+                                double *t_out, double *p_out) {
+    double d[3], bp[8];
+    int nb = 0;
+    bp[nb++] = 0.0;
+    for (int i = 0; i < 3; ++i) {
+        d[i] = b[i] - a[i];
+        if (d[i] != 0.0) {
+            const double t1 = (pmin[i] - a[i]) / d[i], t2 = (pmax[i] - a[i]) / d[i];
+            if (t1 > 0.0 && t1 < 1.0) bp[nb++] = t1;
+            if (t2 > 0.0 && t2 < 1.0) bp[nb++] = t2;
+        }
+    }
+    bp[nb++] = 1.0;
+    for (int i = 1; i < nb; ++i) /* insertion sort of the breakpoints */
+        for (int j = i; j > 0 && bp[j] < bp[j - 1]; --j) { const double tmp = bp[j]; bp[j] = bp[j - 1]; bp[j - 1] = tmp; }
+    double best = INFINITY, bt = 0.0;
+    for (int k = 0; k + 1 < nb; ++k) {
+        const double lo = bp[k], hi = bp[k + 1], mid = 0.5 * (lo + hi);
+        /* on [lo, hi] every coordinate stays on one side of each face: cost = sum over the outside axes of
+         * (a_i + d_i t - bound_i)^2, a quadratic in t */
+        double num = 0.0, den = 0.0;
+        for (int i = 0; i < 3; ++i) {
+            const double x = a[i] + d[i] * mid;
+            double bound;
+            if (x < pmin[i]) bound = pmin[i]; else if (x > pmax[i]) bound = pmax[i]; else continue;
+            num += d[i] * (a[i] - bound);
+            den += d[i] * d[i];
+        }
+        double ts = den > 0.0 ? -num / den : lo;
+        if (ts < lo) ts = lo;
+        if (ts > hi) ts = hi;
+        const double cand[3] = {ts, lo, hi};
+        for (int c = 0; c < 3; ++c) {
+            const double v = box_cost(a, d, pmin, pmax, cand[c], NULL);
+            if (v < best) { best = v; bt = cand[c]; }
+        }
+    }
+    if (nb == 2 && best == INFINITY) { best = box_cost(a, d, pmin, pmax, 0.0, NULL); bt = 0.0; }
+    box_cost(a, d, pmin, pmax, bt, p_out);
+    if (t_out) *t_out = bt;
+    return sqrt(best);
+}
+
 /* frame of link L: identity for L = -1 */
 static void link_frame(int d, const double *Rj, const double *oj, int L, double *R, double *o) {
     (void)d;
@@ -80,9 +135,32 @@ void orc_capsule_world(const orc_chain *c, const orc_capsules *m, const double *
     }
 }
 
+int orc_coll_rows(const orc_capsules *m) {
+    return (m->w_coll != 0.0 ? m->npairs : 0) + (m->w_env != 0.0 ? m->nenv : 0);
+}
+
+/* world point -> frame of obstacle o:  x_box = Ro^T (x - to) */
+static void to_box(const orc_capsules *m, int o, const double *x, double *y) {
+    for (int i = 0; i < 3; ++i) {
+        y[i] = 0.0;
+        for (int k = 0; k < 3; ++k) y[i] += m->Ro[o][3 * k + i] * (x[k] - m->to[o][k]);
+    }
+}
+
 void orc_coll_residual(const orc_chain *c, const orc_capsules *m, const double *q, double *dist, double *r) {
     double wa[3 * ORC_MAX_CAPS], wb[3 * ORC_MAX_CAPS];
     orc_capsule_world(c, m, q, wa, wb);
+    const int ns = m->w_coll != 0.0 ? m->npairs : 0;
+    for (int p = 0; p < (m->w_env != 0.0 ? m->nenv : 0); ++p) { /* robot-environment rows */
+        const int k = m->env_pair[p][0], o = m->env_pair[p][1];
+        double ab[3], bb[3];
+        to_box(m, o, wa + 3 * k, ab);
+        to_box(m, o, wb + 3 * k, bb);
+        const double dd = orc_segment_box_distance(ab, bb, m->pmin[o], m->pmax[o], NULL, NULL) - m->c[k];
+        if (dist) dist[ns + p] = dd;
+        if (r) r[ns + p] = m->w_env * (dd < m->d_safe_env ? m->d_safe_env - dd : 0.0);
+    }
+    if (ns == 0) return;
     for (int p = 0; p < m->npairs; ++p) {
         const int k1 = m->pair[p][0], k2 = m->pair[p][1];
         const double dd = orc_segment_distance(wa + 3 * k1, wb + 3 * k1, wa + 3 * k2, wb + 3 * k2, NULL, NULL)
@@ -113,8 +191,29 @@ void orc_coll_jacobian(const orc_chain *c, const orc_capsules *m, const double *
     double wa[3 * ORC_MAX_CAPS], wb[3 * ORC_MAX_CAPS], pe[3], Re[9], z[3 * ORC_MAX_DOF], o[3 * ORC_MAX_DOF];
     orc_capsule_world(c, m, q, wa, wb);
     orc_fk(c, q, pe, Re, z, o);
-    memset(J, 0, sizeof(double) * (size_t)(m->npairs * d));
-    for (int p = 0; p < m->npairs; ++p) {
+    memset(J, 0, sizeof(double) * (size_t)(orc_coll_rows(m) * d));
+    const int ns = m->w_coll != 0.0 ? m->npairs : 0;
+    for (int p = 0; p < (m->w_env != 0.0 ? m->nenv : 0); ++p) { /* environment rows: the obstacle does not move */
+        const int k = m->env_pair[p][0], ob = m->env_pair[p][1];
+        double ab[3], bb[3], t, pb[3];
+        to_box(m, ob, wa + 3 * k, ab);
+        to_box(m, ob, wb + 3 * k, bb);
+        const double len = orc_segment_box_distance(ab, bb, m->pmin[ob], m->pmax[ob], &t, pb);
+        const double dd = len - m->c[k];
+        if (!(dd < m->d_safe_env) || !(len > 0.0)) continue;
+        double ps[3], nb[3], n[3];
+        for (int i = 0; i < 3; ++i) {
+            ps[i] = wa[3 * k + i] + (wb[3 * k + i] - wa[3 * k + i]) * t;      /* closest point on the capsule axis, world */
+            nb[i] = ((ab[i] + (bb[i] - ab[i]) * t) - pb[i]) / len;             /* direction box point -> axis point, box frame */
+        }
+        for (int i = 0; i < 3; ++i) n[i] = m->Ro[ob][3 * i] * nb[0] + m->Ro[ob][3 * i + 1] * nb[1] + m->Ro[ob][3 * i + 2] * nb[2];
+        for (int j = 0; j < d; ++j) {
+            double c1[3];
+            point_jacobian_col(c, z, o, m->link[k], j, ps, c1);
+            J[(ns + p) * d + j] = -m->w_env * (n[0] * c1[0] + n[1] * c1[1] + n[2] * c1[2]);
+        }
+    }
+    for (int p = 0; p < ns; ++p) {
         const int k1 = m->pair[p][0], k2 = m->pair[p][1];
         double t1, t2;
         const double len = orc_segment_distance(wa + 3 * k1, wb + 3 * k1, wa + 3 * k2, wb + 3 * k2, &t1, &t2);

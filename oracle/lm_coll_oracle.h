@@ -31,6 +31,7 @@
 
 #define ORC_MAX_CAPS 16
 #define ORC_MAX_PAIRS 32
+#define ORC_MAX_OBS 8
 
 typedef struct {
     int32_t ncaps;
@@ -40,19 +41,39 @@ typedef struct {
     int32_t npairs;
     int32_t pair[ORC_MAX_PAIRS][2];
     double w_coll, d_safe;       /* C4 */
+    /* robot-environment rows: cuboid obstacles "with arbitrary spatial positioning", each given
+     * by its frame in the world (rotation Ro row-major = box axes as columns, origin to) and extents pmin, pmax
+     * in that frame; env_pair lists (capsule, obstacle) pairs; one hinge row per pair and waypoint:
+     * r = w_env * max(0, d_safe_env - dist), dist = min over t in [0,1], pmin <= p <= pmax of |p - (a + (b-a) t)| - c
+     * (the paper's QP "in a frame axis-aligned to the cuboid"); d dist / d q = n^T J_p(capsule point) (C5). */
+    int32_t nobs;
+    double Ro[ORC_MAX_OBS][9], to[ORC_MAX_OBS][3], pmin[ORC_MAX_OBS][3], pmax[ORC_MAX_OBS][3];
+    int32_t nenv;
+    int32_t env_pair[ORC_MAX_PAIRS][2];
+    double w_env, d_safe_env;
 } orc_capsules;
 
 /* minimum of |(a1 + (b1-a1) t1) - (a2 + (b2-a2) t2)| over the unit box; t1, t2: a minimiser */
 double orc_segment_distance(const double *a1, const double *b1, const double *a2, const double *b2,
                             double *t1, double *t2);
 
+/* minimum of |p - (a + (b-a) t)| over t in [0,1] and p in the box [pmin, pmax] (all in the box frame): the QP of
+ * PAPER.md:L176-178.  For fixed t the best p is the clamp of the segment point, so the cost is a convex
+ * piecewise quadratic in t: its pieces are delimited by the t at which a coordinate of the segment point crosses
+ * a face plane; every piece is minimised exactly and the smallest value wins.  t, p: a minimiser. */
+double orc_segment_box_distance(const double *a, const double *b, const double *pmin, const double *pmax,
+                                double *t, double *p);
+
 /* world-frame endpoints of every capsule at configuration q: wa[ncaps][3], wb[ncaps][3] */
 void orc_capsule_world(const orc_chain *c, const orc_capsules *m, const double *q, double *wa, double *wb);
 
-/* dist[npairs] (C3) and hinge residuals r[npairs] (C4) at q (either nullable) */
+/* rows per waypoint: npairs self-collision rows followed by nenv environment rows (those with zero weight excluded) */
+int orc_coll_rows(const orc_capsules *m);
+
+/* dist[rows] (C3) and hinge residuals r[rows] (C4) at q (either nullable) */
 void orc_coll_residual(const orc_chain *c, const orc_capsules *m, const double *q, double *dist, double *r);
 
-/* J[npairs][dof] = d r / d q (C5); rows of inactive pairs are zero */
+/* J[rows][dof] = d r / d q (C5); rows of inactive pairs are zero */
 void orc_coll_jacobian(const orc_chain *c, const orc_capsules *m, const double *q, double *J);
 
 #endif

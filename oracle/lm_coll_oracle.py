@@ -9,14 +9,17 @@ import numpy as np
 
 from . import lm_oracle as _o
 
-MAX_CAPS, MAX_PAIRS = 16, 32
+MAX_CAPS, MAX_PAIRS, MAX_OBS = 16, 32, 8
 _dp = C.POINTER(C.c_double)
 
 
 class _Caps(C.Structure):
     _fields_ = [("ncaps", C.c_int32), ("link", C.c_int32 * MAX_CAPS), ("a", (C.c_double * 3) * MAX_CAPS),
                 ("b", (C.c_double * 3) * MAX_CAPS), ("c", C.c_double * MAX_CAPS), ("npairs", C.c_int32),
-                ("pair", (C.c_int32 * 2) * MAX_PAIRS), ("w_coll", C.c_double), ("d_safe", C.c_double)]
+                ("pair", (C.c_int32 * 2) * MAX_PAIRS), ("w_coll", C.c_double), ("d_safe", C.c_double),
+                ("nobs", C.c_int32), ("Ro", (C.c_double * 9) * MAX_OBS), ("to", (C.c_double * 3) * MAX_OBS),
+                ("pmin", (C.c_double * 3) * MAX_OBS), ("pmax", (C.c_double * 3) * MAX_OBS), ("nenv", C.c_int32),
+                ("env_pair", (C.c_int32 * 2) * MAX_PAIRS), ("w_env", C.c_double), ("d_safe_env", C.c_double)]
 
 
 @dataclass
@@ -26,6 +29,9 @@ class Capsules:
     model: object
     w_coll: float = 1.0
     d_safe: float = 0.05
+    scene: object = None     # obstacles: R [M,3,3] (box axes as columns), t [M,3], pmin [M,3], pmax [M,3], pairs [Q,2] (capsule, obstacle)
+    w_env: float = 0.0
+    d_safe_env: float = 0.05
 
     def _c(self) -> _Caps:
         m = self.model
@@ -42,6 +48,19 @@ class Capsules:
         for p in range(P):
             s.pair[p][0], s.pair[p][1] = int(m.pairs[p][0]), int(m.pairs[p][1])
         s.w_coll, s.d_safe = float(self.w_coll), float(self.d_safe)
+        if self.scene is not None:
+            sc = self.scene
+            M, Q = len(sc.t), len(sc.pairs)
+            assert M <= MAX_OBS and Q <= MAX_PAIRS
+            s.nobs, s.nenv = M, Q
+            for o in range(M):
+                for i in range(9):
+                    s.Ro[o][i] = float(np.asarray(sc.R[o]).reshape(9)[i])
+                for i in range(3):
+                    s.to[o][i], s.pmin[o][i], s.pmax[o][i] = float(sc.t[o][i]), float(sc.pmin[o][i]), float(sc.pmax[o][i])
+            for p in range(Q):
+                s.env_pair[p][0], s.env_pair[p][1] = int(sc.pairs[p][0]), int(sc.pairs[p][1])
+            s.w_env, s.d_safe_env = float(self.w_env), float(self.d_safe_env)
         return s
 
 
@@ -55,6 +74,10 @@ def _lib():
         ch, cp = C.POINTER(_o._Chain), C.POINTER(_Caps)
         L.orc_segment_distance.argtypes = [_dp, _dp, _dp, _dp, _dp, _dp]
         L.orc_segment_distance.restype = C.c_double
+        L.orc_segment_box_distance.argtypes = [_dp, _dp, _dp, _dp, _dp, _dp]
+        L.orc_segment_box_distance.restype = C.c_double
+        L.orc_coll_rows.argtypes = [cp]
+        L.orc_coll_rows.restype = C.c_int
         L.orc_capsule_world.argtypes = [ch, cp, _dp, _dp, _dp]
         L.orc_capsule_world.restype = None
         L.orc_coll_residual.argtypes = [ch, cp, _dp, _dp, _dp]
@@ -79,6 +102,15 @@ def segment_distance(a1, b1, a2, b2):
     return float(d), float(t1.value), float(t2.value)
 
 
+def segment_box_distance(a, b, pmin, pmax):
+    """(min distance, t, p[3]) of the QP of PAPER.md:L176-178 (box frame)."""
+    t = C.c_double()
+    p = np.empty(3)
+    a, b, pmin, pmax = (_o._f64(x, (3,)) for x in (a, b, pmin, pmax))
+    d = _lib().orc_segment_box_distance(_p(a), _p(b), _p(pmin), _p(pmax), C.byref(t), _p(p))
+    return float(d), float(t.value), p
+
+
 def fk_frames(chain, q):
     c = _o._chain_c(chain)
     q = _o._f64(q, (chain.dof,))
@@ -99,7 +131,8 @@ def residual(chain, caps: Capsules, q):
     """(dist [P], r [P]) at one configuration."""
     c, m = _o._chain_c(chain), caps._c()
     q = _o._f64(q, (chain.dof,))
-    dist, r = np.empty(m.npairs), np.empty(m.npairs)
+    rows = int(_lib().orc_coll_rows(C.byref(m)))
+    dist, r = np.empty(rows), np.empty(rows)
     _lib().orc_coll_residual(C.byref(c), C.byref(m), _p(q), _p(dist), _p(r))
     return dist, r
 
@@ -107,6 +140,6 @@ def residual(chain, caps: Capsules, q):
 def jacobian(chain, caps: Capsules, q):
     c, m = _o._chain_c(chain), caps._c()
     q = _o._f64(q, (chain.dof,))
-    J = np.empty((m.npairs, chain.dof))
+    J = np.empty((int(_lib().orc_coll_rows(C.byref(m))), chain.dof))
     _lib().orc_coll_jacobian(C.byref(c), C.byref(m), _p(q), _p(J))
     return J

@@ -14,7 +14,7 @@
 
 int64_t orc_traj_rows(int32_t dof, int64_t n) { return 6 * n + (int64_t)dof * (n - 1); }
 
-static int coll_rows(const orc_traj_params *t) { return (t->caps && t->caps->w_coll != 0.0) ? t->caps->npairs : 0; }
+static int coll_rows(const orc_traj_params *t) { return t->caps ? orc_coll_rows(t->caps) : 0; }
 
 int64_t orc_traj_rows_all(const orc_traj_params *t, int32_t dof, int64_t n) {
     return orc_traj_rows(dof, n) + (int64_t)coll_rows(t) * n;
@@ -61,7 +61,7 @@ void orc_traj_jacobian(const orc_chain *c, const orc_params *prm, const orc_traj
         }
     const int np = coll_rows(t);
     for (int64_t i = 0; i < n && np > 0; ++i) { /* collision rows of waypoint i depend on q_i only */
-        double Jc[ORC_MAX_PAIRS * ORC_MAX_DOF];
+        double Jc[2 * ORC_MAX_PAIRS * ORC_MAX_DOF];
         orc_coll_jacobian(c, t->caps, q + i * d, Jc);
         for (int p = 0; p < np; ++p)
             for (int a = 0; a < d; ++a) J[(orc_traj_rows(d, n) + np * i + p) * cols + d * i + a] = Jc[p * d + a];
@@ -193,7 +193,7 @@ int orc_traj_delta_banded(const orc_chain *c, const orc_params *prm, const orc_t
         }
         const int np = coll_rows(t);
         if (np > 0) { /* collision rows of waypoint i: J_c^T J_c on the diagonal block, J_c^T r_c in the gradient */
-            double Jc[ORC_MAX_PAIRS * ORC_MAX_DOF], rc[ORC_MAX_PAIRS];
+            double Jc[2 * ORC_MAX_PAIRS * ORC_MAX_DOF], rc[2 * ORC_MAX_PAIRS];
             orc_coll_jacobian(c, t->caps, q + i * d, Jc);
             orc_coll_residual(c, t->caps, q + i * d, NULL, rc);
             for (int p = 0; p < np; ++p)
@@ -237,7 +237,7 @@ static void traj_cost(const orc_chain *c, const orc_params *prm, const orc_traj_
     double fc = 0.0;
     const int np = coll_rows(t);
     for (int64_t i = 0; i < n && np > 0; ++i) {
-        double rc[ORC_MAX_PAIRS];
+        double rc[2 * ORC_MAX_PAIRS];
         orc_coll_residual(c, t->caps, q + i * d, NULL, rc);
         for (int p = 0; p < np; ++p) fc += rc[p] * rc[p];
     }

@@ -37,8 +37,8 @@ typedef struct {
     double w_pose, w_diff;                                  /* DESIGN T1 */
     double lambda0, nu_up, nu_down, lambda_min, lambda_max; /* DESIGN T3 (= R5, per trajectory) */
     const orc_capsules *caps; /* nullable: self-collision rows (lm_coll_oracle.h, Fig. 6 "self-coll-dist(q_i)"),
-                                 caps->npairs hinge rows per waypoint appended after the differencing rows:
-                                 row 6n + d(n-1) + npairs * i + p  =  residual of pair p at waypoint i */
+                                 np = orc_coll_rows(caps) hinge rows per waypoint (self-collision pairs, then capsule-obstacle
+                                 pairs) appended after the differencing rows: row 6n + d(n-1) + np * i + p */
 } orc_traj_params;
 
 /* rows of the stacked residual / Jacobian of one n-waypoint trajectory (without / with the collision rows) */

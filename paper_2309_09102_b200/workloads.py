@@ -123,6 +123,32 @@ def chain_capsules(chain: "Chain", radius: float = 0.05) -> CapsuleModel:
 
 
 @dataclass
+class ObstacleScene:
+    """Cuboid obstacles "with arbitrary spatial positioning": frame of each box in the world
+    (R = box axes as columns, t = origin), extents pmin / pmax in that frame, and the (capsule, obstacle)
+    pairs to check -- config data."""
+    name: str
+    R: np.ndarray      # [M, 3, 3]
+    t: np.ndarray      # [M, 3]
+    pmin: np.ndarray   # [M, 3]
+    pmax: np.ndarray   # [M, 3]
+    pairs: np.ndarray  # [Q, 2] (capsule index, obstacle index)
+
+
+def panda_scene(seed: int = 7) -> ObstacleScene:
+    """SYNTHETIC scene for the Panda capsule model (the paper's obstacle scenes are not available): a table slab in
+    front of the robot, a tilted post beside it and a small box above the table; forearm, wrist and hand capsules
+    are checked against all three, the elbow against the post."""
+    rng = np.random.default_rng(seed)
+    R = np.stack([np.eye(3), Rotation.from_rotvec([0.2, -0.1, 0.5]).as_matrix(),
+                  Rotation.from_rotvec(rng.normal(size=3) * 0.4).as_matrix()])
+    t = np.array([[0.55, 0.0, 0.15], [0.25, 0.45, 0.35], [0.45, -0.25, 0.45]])
+    half = np.array([[0.30, 0.40, 0.02], [0.05, 0.05, 0.35], [0.08, 0.06, 0.10]])
+    pairs = np.array([[4, 0], [5, 0], [6, 0], [4, 1], [5, 1], [6, 1], [3, 1], [4, 2], [5, 2], [6, 2]])
+    return ObstacleScene("panda_synthetic_scene", R, t, -half, half, pairs)
+
+
+@dataclass
 class Workload:
     name: str
     chain: Chain

@@ -148,3 +148,96 @@ def test_trajectory_step_with_collision_rows():
     assert d_after > d_before + 0.01
     assert st.F_total[0] < (r @ r) * 0.8
     assert np.isclose(st.F_total[0], np.sum(torc.residual(ch, pp, tprm, tp, tq, st.q[0]) ** 2), rtol=1e-12)
+
+
+# ------------------------------------------------------------------ robot-environment rows
+
+def brute_box(a, b, pmin, pmax, m=4001):
+    t = np.linspace(0, 1, m)
+    x = a[None] + (b - a)[None] * t[:, None]
+    return np.sqrt(((x - np.clip(x, pmin, pmax)) ** 2).sum(-1)).min()
+
+
+def test_segment_box_distance_is_the_qp_minimum():
+    rng = np.random.default_rng(5)
+    for k in range(400):
+        half = rng.uniform(0.05, 0.5, size=3)
+        a, b = rng.normal(size=(2, 3)) * rng.uniform(0.2, 1.5)
+        if k % 4 == 1:
+            b[rng.integers(3)] = a[rng.integers(3)]            # (partly) axis-parallel
+        if k % 9 == 2:
+            b = a.copy()
+        d, t, p = corc.segment_box_distance(a, b, -half, half)
+        assert 0 <= t <= 1 and np.all(p >= -half - 1e-15) and np.all(p <= half + 1e-15)
+        x = a + (b - a) * t
+        assert np.isclose(np.linalg.norm(x - p), d, atol=1e-12)                 # the minimiser attains it
+        g = brute_box(a, b, -half, half)
+        assert d <= g + 1e-12 and g - d <= np.linalg.norm(b - a) / 4000 + 1e-12
+    # closed forms: above a face, beside an edge, beyond a corner, passing through
+    assert np.isclose(corc.segment_box_distance([-1, 0, 0.7], [1, 0, 0.7], [-0.5] * 3, [0.5] * 3)[0], 0.2)
+    assert np.isclose(corc.segment_box_distance([1, 1, -2], [1, 1, 2], [-0.5] * 3, [0.5] * 3)[0], np.sqrt(0.5))
+    assert np.isclose(corc.segment_box_distance([1, 1, 1], [2, 2, 2], [-0.5] * 3, [0.5] * 3)[0], np.sqrt(0.75))
+    assert corc.segment_box_distance([-1, 0.1, 0], [1, 0.2, 0.1], [-0.5] * 3, [0.5] * 3)[0] < 1e-15
+
+
+def test_environment_rows_value_and_jacobian():
+    ch, model, scene = wl.panda_chain(), wl.panda_capsules(), wl.panda_scene()
+    rng = np.random.default_rng(6)
+    caps = corc.Capsules(model, w_coll=0.0, scene=scene, w_env=1.3, d_safe_env=0.6)
+    checked = 0
+    for trial in range(30):
+        q = np.clip(0.5 * (ch.q_lo + ch.q_hi) + 0.5 * rng.normal(size=7), ch.q_lo, ch.q_hi)
+        dist, r = corc.residual(ch, caps, q)
+        assert dist.shape == (len(scene.pairs),)
+        wa, wb = corc.capsule_world(ch, caps, q)
+        for p, (k, o) in enumerate(scene.pairs):
+            ab = scene.R[o].T @ (wa[k] - scene.t[o])
+            bb = scene.R[o].T @ (wb[k] - scene.t[o])
+            d = corc.segment_box_distance(ab, bb, scene.pmin[o], scene.pmax[o])[0] - model.radius[k]
+            assert np.isclose(dist[p], d, atol=1e-13)
+            assert np.isclose(r[p], 1.3 * max(0.0, 0.6 - d), atol=1e-13)
+        J = corc.jacobian(ch, caps, q)
+        h = 1e-6
+        Jfd = np.zeros_like(J)
+        kink = np.zeros(len(r), bool)
+        for j in range(7):
+            e = np.zeros(7)
+            e[j] = h
+            dp, rp = corc.residual(ch, caps, q + e)
+            dm, rm = corc.residual(ch, caps, q - e)
+            Jfd[:, j] = (rp - rm) / (2 * h)
+            kink |= (rp == 0) != (rm == 0)
+        act = (r > 1e-3) & ~kink & (dist + model.radius[scene.pairs[:, 0]] > 1e-3)     # not penetrating the box itself
+        if act.any():
+            assert np.abs(J[act] - Jfd[act]).max() < 5e-6, np.abs(J[act] - Jfd[act]).max()
+            checked += int(act.sum())
+    assert checked > 100
+    # both kinds of rows together: self rows first, then environment rows
+    both = corc.Capsules(model, w_coll=1.0, d_safe=0.3, scene=scene, w_env=1.3, d_safe_env=0.6)
+    q = np.array([0.0, 1.2, 0.0, -2.9, 0.0, 2.2, 0.8])
+    d_all, r_all = corc.residual(ch, both, q)
+    d_s, r_s = corc.residual(ch, corc.Capsules(model, w_coll=1.0, d_safe=0.3), q)
+    d_e, r_e = corc.residual(ch, caps, q)
+    assert np.array_equal(r_all, np.r_[r_s, r_e]) and np.array_equal(d_all, np.r_[d_s, d_e])
+    assert np.array_equal(corc.jacobian(ch, both, q), np.vstack([corc.jacobian(ch, corc.Capsules(model, w_coll=1.0, d_safe=0.3), q),
+                                                                 corc.jacobian(ch, caps, q)]))
+
+
+def test_trajectory_step_with_environment_rows():
+    ch, model, scene = wl.panda_chain(), wl.panda_capsules(), wl.panda_scene()
+    rng = np.random.default_rng(7)
+    n = 6
+    q0 = np.clip(0.5 * (ch.q_lo + ch.q_hi) + np.cumsum(0.02 * rng.normal(size=(n, 7)), axis=0), ch.q_lo, ch.q_hi)
+    p, R = orc.fk(ch, q0)
+    tp, tq = p, wl._R_to_quat_wxyz(R)
+    caps = corc.Capsules(model, w_coll=1.0, d_safe=0.2, scene=scene, w_env=1.5, d_safe_env=0.5)
+    tprm = torc.TrajParams(w_pose=0.5, w_diff=0.3, caps=caps)
+    rows = 6 * n + 7 * (n - 1) + (len(model.pairs) + len(scene.pairs)) * n
+    r = torc.residual(ch, orc.Params(), tprm, tp, tq, q0)
+    J = torc.jacobian(ch, orc.Params(), tprm, q0)
+    assert r.shape == (rows,) and J.shape == (rows, 7 * n) and (r[-len(scene.pairs):] > 0).any()
+    lam = 1e-2
+    x = np.linalg.lstsq(np.vstack([J, np.sqrt(lam) * np.eye(7 * n)]), -np.r_[r, np.zeros(7 * n)], rcond=None)[0]
+    dd = torc.delta(ch, orc.Params(), tprm, tp, tq, q0, lam, dense=True)
+    db = torc.delta(ch, orc.Params(), tprm, tp, tq, q0, lam, dense=False)
+    assert np.abs(dd.ravel() - x).max() < 1e-8 and np.abs(db - dd).max() < 1e-10
