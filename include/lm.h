@@ -259,6 +259,24 @@ typedef struct {
 } lm_capsules;
 int lm_traj_set_capsules(lm_ctx *ctx, const lm_capsules *model);
 
+/* Robot-environment collision rows: obstacles are cuboids "with arbitrary spatial positioning";
+ * the distance of a capsule to a cuboid is, in the cuboid's axis-aligned frame, the minimum over 0 <= t <= 1 and
+ * pmin <= p <= pmax of |p - (a + (b-a) t)|, less the radius (the paper's QP); per listed (capsule, obstacle) pair
+ * and waypoint one hinge row  r = w_env * max(0, d_safe - dist)  with  d r / d q = -w_env n^T J_p  at the closest
+ * point of the capsule axis.  Uses the capsules of lm_traj_set_capsules (call that first; it clears the obstacles;
+ * a capsule model with npairs = 0 gives environment rows only).  HOST pointers, copied by the call. */
+#define LM_MAX_OBSTACLES 8
+typedef struct {
+    int32_t nobs;
+    const float *pose;     /* [nobs][7] frame of the cuboid in the world: xyz (m) + unit quaternion w,x,y,z */
+    const float *pmin, *pmax; /* [nobs][3] extents in that frame (m) */
+    int32_t npairs;
+    const int32_t *pairs;  /* [npairs][2] (capsule index, obstacle index) */
+    float w_env;
+    float d_safe;
+} lm_obstacles;
+int lm_traj_set_obstacles(lm_ctx *ctx, const lm_obstacles *scene);
+
 /* Debug trace (device pointers, nullable, borrowed): every executed iteration overwrites
  * trial_q [d][W] (w-order) = the clamped trial point and trial_F [2][B] = (|r|^2 before, at the trial point). */
 int lm_traj_set_trace(lm_ctx *ctx, float *trial_q, float *trial_F);

@@ -17,7 +17,7 @@
 
 namespace lmk {
 
-constexpr int MAX_CAPS = 16, MAX_PAIRS = 32;
+constexpr int MAX_CAPS = 16, MAX_PAIRS = 32, MAX_OBS = 8;
 
 struct KCaps {
     int32_t ncaps, npairs;
@@ -25,6 +25,12 @@ struct KCaps {
     int8_t link[MAX_CAPS];          // -1 = base frame, j = frame moved by joint j
     float a[MAX_CAPS][3], b[MAX_CAPS][3], c[MAX_CAPS];
     uint8_t pair[MAX_PAIRS][2];
+    // robot-environment rows: cuboids given by their frame in the world (Ro row-major, box axes
+    // as columns; origin to) and extents pmin / pmax in that frame; env_pair = (capsule, obstacle)
+    int32_t nobs, nenv;
+    float w_env, d_safe_env;
+    float Ro[MAX_OBS][9], to[MAX_OBS][3], pmin[MAX_OBS][3], pmax[MAX_OBS][3];
+    uint8_t env_pair[MAX_PAIRS][2];
 };
 
 // world endpoints of the capsules: filled link by link while FK runs
@@ -98,11 +104,107 @@ __device__ __forceinline__ void segment_closest(const float (&a1)[3], const floa
     t1 = s1; t2 = s2;
 }
 
+// min over t in [0,1], p in [pmin, pmax] of |p - (a + (b-a) t)|^2 (box frame): for fixed t the best p is the clamp of
+// the segment point, so the cost is a convex piecewise quadratic in t with breakpoints where a coordinate crosses a
+// face plane.  Half its derivative, gder(t) = sum_i d_i * (excess of coordinate i over the box), is non-decreasing:
+// the breakpoints on either side of its sign change bracket ONE quadratic piece, whose stationary point is exact.
+__device__ __forceinline__ float segment_box_closest(const float (&a)[3], const float (&b)[3], const float (&pmin)[3],
+                                                     const float (&pmax)[3]) {
+    float d[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) d[i] = sub(b[i], a[i]);
+    auto gder = [&](float t) {
+        float s = 0.f;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            const float x = fma_(d[i], t, a[i]);
+            const float ex = (x > pmax[i]) ? sub(x, pmax[i]) : (x < pmin[i]) ? sub(x, pmin[i]) : 0.f;
+            s = fma_(d[i], ex, s);
+        }
+        return s;
+    };
+    if (gder(0.f) >= 0.f) return 0.f;
+    if (gder(1.f) <= 0.f) return 1.f;
+    float tl = 0.f, th = 1.f;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const float id = (d[i] != 0.f) ? __fdividef(1.0f, d[i]) : 0.f;
+#pragma unroll
+        for (int side = 0; side < 2; ++side) {
+            const float c = clamp01(mul(sub(side ? pmax[i] : pmin[i], a[i]), id));
+            if (gder(c) <= 0.f) tl = fmaxf(tl, c); else th = fminf(th, c);
+        }
+    }
+    const float mid = mul(0.5f, add(tl, th));
+    float num = 0.f, den = 0.f;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const float x = fma_(d[i], mid, a[i]);
+        if (x > pmax[i]) { num = fma_(d[i], sub(a[i], pmax[i]), num); den = fma_(d[i], d[i], den); }
+        else if (x < pmin[i]) { num = fma_(d[i], sub(a[i], pmin[i]), num); den = fma_(d[i], d[i], den); }
+    }
+    const float ts = den > 0.f ? -__fdividef(num, den) : tl;
+    return fminf(fmaxf(ts, tl), th);
+}
+
 // Calls f(g, r) for every pair whose hinge is active at this waypoint: g[D] = d r / d q, r = the residual.
 // Fr = frames retained by FK (Fr.Jw[j] = z_j, Fr.Jv[j] = o_j: eval_pose with WITH_JAC = false).
 template <int D, typename SpecT, typename F>
 __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, const CapsWorld &W, const Pose<D> &Fr, F &&f) {
     constexpr ChainSpec S = SpecT::spec;
+    for (int p = 0; p < C.nenv; ++p) { // robot-environment rows: the obstacle does not move
+        const int k = C.env_pair[p][0], ob = C.env_pair[p][1];
+        float ab[3], bb[3], wa[3], wb[3], pmin[3], pmax[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { wa[i] = W.wa[k][i]; wb[i] = W.wb[k][i]; pmin[i] = C.pmin[ob][i]; pmax[i] = C.pmax[ob][i]; }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { // x_box = Ro^T (x - to)
+            float sa = 0.f, sb = 0.f;
+#pragma unroll
+            for (int kk = 0; kk < 3; ++kk) {
+                sa = fma_(C.Ro[ob][3 * kk + i], sub(wa[kk], C.to[ob][kk]), sa);
+                sb = fma_(C.Ro[ob][3 * kk + i], sub(wb[kk], C.to[ob][kk]), sb);
+            }
+            ab[i] = sa; bb[i] = sb;
+        }
+        const float t = segment_box_closest(ab, bb, pmin, pmax);
+        float eb[3], ps[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            const float x = fma_(sub(bb[i], ab[i]), t, ab[i]);
+            eb[i] = sub(x, fminf(fmaxf(x, pmin[i]), pmax[i]));
+            ps[i] = fma_(sub(wb[i], wa[i]), t, wa[i]);
+        }
+        const float len = sqrtf(dot3(eb, eb));
+        const float dist = sub(len, C.c[k]);
+        if (!(dist < C.d_safe_env)) continue;
+        const float r = mul(C.w_env, sub(C.d_safe_env, dist));
+        const float il = (len > 0.f) ? __fdividef(1.0f, len) : 0.f; // axis inside the box: no direction, the row keeps its value
+        float n[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) n[i] = mul(il, fma_(C.Ro[ob][3 * i + 2], eb[2], fma_(C.Ro[ob][3 * i + 1], eb[1], mul(C.Ro[ob][3 * i], eb[0]))));
+        const int L = C.link[k];
+        float g[D];
+#pragma unroll
+        for (int j = 0; j < D; ++j) {
+            float gj = 0.f;
+            if (j <= L) {
+                const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
+                const float z[3] = {Fr.Jw[j][0], Fr.Jw[j][1], Fr.Jw[j][2]};
+                float col[3];
+                if (pris) { col[0] = z[0]; col[1] = z[1]; col[2] = z[2]; }
+                else {
+                    const float dd[3] = {sub(ps[0], Fr.Jv[j][0]), sub(ps[1], Fr.Jv[j][1]), sub(ps[2], Fr.Jv[j][2])};
+                    col[0] = fma_(z[1], dd[2], -mul(z[2], dd[1]));
+                    col[1] = fma_(z[2], dd[0], -mul(z[0], dd[2]));
+                    col[2] = fma_(z[0], dd[1], -mul(z[1], dd[0]));
+                }
+                gj = mul(-C.w_env, dot3(n, col));
+            }
+            g[j] = gj;
+        }
+        f(g, r);
+    }
     for (int p = 0; p < C.npairs; ++p) {
         const int k1 = C.pair[p][0], k2 = C.pair[p][1];
         float a1[3], b1[3], a2[3], b2[3];
@@ -119,9 +221,9 @@ __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, cons
         }
         const float len = sqrtf(dot3(e, e));
         const float dist = sub(sub(len, C.c[k1]), C.c[k2]);
-        if (!(dist < C.d_safe) || !(len > 0.f)) continue;
+        if (!(dist < C.d_safe)) continue;
         const float r = mul(C.w_coll, sub(C.d_safe, dist));
-        const float il = __fdividef(1.0f, len);
+        const float il = (len > 0.f) ? __fdividef(1.0f, len) : 0.f; // the axes touch: no direction, the row keeps its value
         const float n[3] = {mul(e[0], il), mul(e[1], il), mul(e[2], il)};
         const int L1 = C.link[k1], L2 = C.link[k2];
         const int lo = min(L1, L2), hi = max(L1, L2);

@@ -5,6 +5,7 @@
 #include "lm_ctx.h"
 #include "lm_traj_launch.h"
 
+#include <cmath>
 #include <cstring>
 
 using namespace lmk;
@@ -164,9 +165,10 @@ int lm_traj_set_capsules(lm_ctx *c, const lm_capsules *m) {
     if (!c || !c->traj.attached) return LM_EINVAL;
     KCaps &k = c->traj.args.caps;
     std::memset(&k, 0, sizeof(k));
-    if (!m || m->npairs == 0 || m->w_coll == 0.f) return LM_OK; // no collision rows
+    if (!m || m->ncaps == 0) return LM_OK; // no capsules: no collision rows of either kind
     if (m->ncaps < 1 || m->ncaps > LM_MAX_CAPSULES || m->npairs < 0 || m->npairs > LM_MAX_CAPSULE_PAIRS) return LM_EINVAL;
-    if (!m->link || !m->a || !m->b || !m->radius || !m->pairs || !(m->w_coll > 0.f) || !(m->d_safe >= 0.f)) return LM_EINVAL;
+    if (!m->link || !m->a || !m->b || !m->radius || (m->npairs > 0 && !m->pairs) || !(m->w_coll >= 0.f) || !(m->d_safe >= 0.f))
+        return LM_EINVAL;
     for (int i = 0; i < m->ncaps; ++i) {
         if (m->link[i] < -1 || m->link[i] >= c->dof || !(m->radius[i] >= 0.f)) return LM_EINVAL;
         k.link[i] = (int8_t)m->link[i];
@@ -178,7 +180,40 @@ int lm_traj_set_capsules(lm_ctx *c, const lm_capsules *m) {
         if (k1 < 0 || k1 >= m->ncaps || k2 < 0 || k2 >= m->ncaps || k1 == k2) return LM_EINVAL;
         k.pair[p][0] = (uint8_t)k1; k.pair[p][1] = (uint8_t)k2;
     }
-    k.ncaps = m->ncaps; k.npairs = m->npairs; k.w_coll = m->w_coll; k.d_safe = m->d_safe;
+    k.ncaps = m->ncaps; k.npairs = (m->w_coll > 0.f) ? m->npairs : 0; k.w_coll = m->w_coll; k.d_safe = m->d_safe;
+    return LM_OK;
+}
+
+int lm_traj_set_obstacles(lm_ctx *c, const lm_obstacles *o) {
+    if (!c || !c->traj.attached) return LM_EINVAL;
+    KCaps &k = c->traj.args.caps;
+    k.nobs = 0; k.nenv = 0; k.w_env = 0.f; k.d_safe_env = 0.f;
+    if (!o || o->npairs == 0 || o->w_env == 0.f) return LM_OK;
+    if (k.ncaps == 0) return LM_EINVAL; // lm_traj_set_capsules first
+    if (o->nobs < 1 || o->nobs > LM_MAX_OBSTACLES || o->npairs < 0 || o->npairs > LM_MAX_CAPSULE_PAIRS) return LM_EINVAL;
+    if (!o->pose || !o->pmin || !o->pmax || !o->pairs || !(o->w_env > 0.f) || !(o->d_safe >= 0.f)) return LM_EINVAL;
+    for (int i = 0; i < o->nobs; ++i) {
+        const float *ps = o->pose + 7 * i;
+        const double n = std::sqrt((double)ps[3] * ps[3] + (double)ps[4] * ps[4] + (double)ps[5] * ps[5] + (double)ps[6] * ps[6]);
+        if (!(n > 0.0)) return LM_EINVAL;
+        const double w = ps[3] / n, x = ps[4] / n, y = ps[5] / n, z = ps[6] / n;
+        const double R[9] = {1 - 2 * (y * y + z * z), 2 * (x * y - w * z), 2 * (x * z + w * y),
+                             2 * (x * y + w * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w * x),
+                             2 * (x * z - w * y), 2 * (y * z + w * x), 1 - 2 * (x * x + y * y)};
+        for (int e = 0; e < 9; ++e) k.Ro[i][e] = (float)R[e];
+        for (int e = 0; e < 3; ++e) {
+            k.to[i][e] = ps[e];
+            k.pmin[i][e] = o->pmin[3 * i + e];
+            k.pmax[i][e] = o->pmax[3 * i + e];
+            if (!(k.pmin[i][e] <= k.pmax[i][e])) return LM_EINVAL;
+        }
+    }
+    for (int p = 0; p < o->npairs; ++p) {
+        const int32_t kc = o->pairs[2 * p], ob = o->pairs[2 * p + 1];
+        if (kc < 0 || kc >= k.ncaps || ob < 0 || ob >= o->nobs) return LM_EINVAL;
+        k.env_pair[p][0] = (uint8_t)kc; k.env_pair[p][1] = (uint8_t)ob;
+    }
+    k.nobs = o->nobs; k.nenv = o->npairs; k.w_env = o->w_env; k.d_safe_env = o->d_safe;
     return LM_OK;
 }
 

@@ -18,7 +18,7 @@ cudaError_t launch_traj_plain(int which, int dof, unsigned grid, unsigned block,
 
 template <int D, typename SpecT>
 cudaError_t launch_traj_pose_t(int which, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a) {
-    const bool coll = a.caps.npairs > 0; // collision rows: their own instantiations (lm_coll.cuh)
+    const bool coll = a.caps.npairs + a.caps.nenv > 0; // collision rows: their own instantiations (lm_coll.cuh)
 #define LM_TL_LAUNCH(K)                                                                   \
     do {                                                                                  \
         if (weighted) { if (coll) K<D, false, true, SpecT, true><<<grid, block, 0, s>>>(a);   \

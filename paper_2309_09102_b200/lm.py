@@ -30,7 +30,7 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_option", "lm_kernel_name", "lm_fk", "lm_fp32_peak", "lm_free",
            "lm_strerror", "lm_launch_count", "lm_fp32_peak_form",
            "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
-           "lm_traj_fetch", "lm_traj_set_trace", "lm_traj_set_capsules",
+           "lm_traj_fetch", "lm_traj_set_trace", "lm_traj_set_capsules", "lm_traj_set_obstacles",
            "lm_solve_host_workspace_bytes", "lm_solve_host",
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR = 0, 1
@@ -78,6 +78,12 @@ class LmCapsules(C.Structure):
     _fields_ = [("ncaps", C.c_int32), ("link", C.POINTER(C.c_int32)), ("a", C.POINTER(C.c_float)), ("b", C.POINTER(C.c_float)),
                 ("radius", C.POINTER(C.c_float)), ("npairs", C.c_int32), ("pairs", C.POINTER(C.c_int32)),
                 ("w_coll", C.c_float), ("d_safe", C.c_float)]
+
+
+class LmObstacles(C.Structure):
+    _fields_ = [("nobs", C.c_int32), ("pose", C.POINTER(C.c_float)), ("pmin", C.POINTER(C.c_float)),
+                ("pmax", C.POINTER(C.c_float)), ("npairs", C.c_int32), ("pairs", C.POINTER(C.c_int32)),
+                ("w_env", C.c_float), ("d_safe", C.c_float)]
 
 
 class LmPlanParams(C.Structure):
@@ -140,6 +146,7 @@ def lib() -> C.CDLL:
         L.lm_traj_fetch.argtypes = [C.c_void_p, C.POINTER(LmTrajStats)]
         L.lm_traj_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.lm_traj_set_capsules.argtypes = [C.c_void_p, C.POINTER(LmCapsules)]
+        L.lm_traj_set_obstacles.argtypes = [C.c_void_p, C.POINTER(LmObstacles)]
         L.lm_solve_host_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64, C.c_int32]
         L.lm_solve_host_workspace_bytes.restype = C.c_size_t
         L.lm_solve_host.argtypes = [C.POINTER(LmChain), C.POINTER(LmProblem), C.POINTER(LmParams), C.c_int32, C.c_int32,
@@ -301,6 +308,23 @@ def lm_traj_set_capsules(ctx: int, model, w_coll: float = 1.0, d_safe: float = 0
                    b.ctypes.data_as(C.POINTER(C.c_float)), rad.ctypes.data_as(C.POINTER(C.c_float)), len(pairs),
                    pairs.ctypes.data_as(C.POINTER(C.c_int32)), float(w_coll), float(d_safe))
     _check(lib().lm_traj_set_capsules(ctx, C.byref(m)), "lm_traj_set_capsules")
+
+
+def lm_traj_set_obstacles(ctx: int, scene, w_env: float = 1.0, d_safe: float = 0.05) -> None:
+    """scene: a workloads.ObstacleScene-like object (R [M,3,3], t, pmin, pmax, pairs) or None to remove the rows."""
+    if scene is None:
+        _check(lib().lm_traj_set_obstacles(ctx, None), "lm_traj_set_obstacles")
+        return
+    from scipy.spatial.transform import Rotation
+    xyzw = Rotation.from_matrix(np.asarray(scene.R, dtype=np.float64)).as_quat()
+    pose = np.ascontiguousarray(np.concatenate([scene.t, xyzw[:, 3:4], xyzw[:, 0:3]], axis=1), dtype=np.float32)
+    pmin = np.ascontiguousarray(scene.pmin, dtype=np.float32)
+    pmax = np.ascontiguousarray(scene.pmax, dtype=np.float32)
+    pairs = np.ascontiguousarray(scene.pairs, dtype=np.int32)
+    fp = C.POINTER(C.c_float)
+    o = LmObstacles(len(pose), pose.ctypes.data_as(fp), pmin.ctypes.data_as(fp), pmax.ctypes.data_as(fp), len(pairs),
+                    pairs.ctypes.data_as(C.POINTER(C.c_int32)), float(w_env), float(d_safe))
+    _check(lib().lm_traj_set_obstacles(ctx, C.byref(o)), "lm_traj_set_obstacles")
 
 
 def lm_traj_set_trace(ctx: int, trial_q_ptr: Optional[int], trial_F_ptr: Optional[int]) -> None:
@@ -467,6 +491,9 @@ class Solver:
 
     def traj_set_capsules(self, model, w_coll: float = 1.0, d_safe: float = 0.05) -> None:
         lm_traj_set_capsules(self._ctx, model, w_coll, d_safe)
+
+    def traj_set_obstacles(self, scene, w_env: float = 1.0, d_safe: float = 0.05) -> None:
+        lm_traj_set_obstacles(self._ctx, scene, w_env, d_safe)
 
     def traj_run(self, iters: int) -> None:
         lm_traj_run(self._ctx, iters)

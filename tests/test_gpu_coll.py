@@ -139,3 +139,97 @@ def test_no_capsules_is_bitwise_the_plain_step_and_errors():
         s.close()
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1]["cost"], outs[1][1]["cost"])
     assert np.all(outs[1][1]["cost_coll"] == 0)
+
+
+# ------------------------------------------------------------------ robot-environment rows
+
+def run_pair_env(ch, model, scene, w, iters, w_coll, d_safe, w_env, d_safe_env, lam=None):
+    from paper_2309_09102_b200 import lm
+    B, n, d = w.B, w.n, ch.dof
+    s = lm.Solver(ch, B, n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0))
+    s.traj_attach(lm.lm_traj_default_params(w_pose=0.5, w_diff=0.3))
+    s.traj_set_capsules(model, w_coll, d_safe)
+    s.traj_set_obstacles(scene, w_env, d_safe_env)
+    if lam is not None:
+        s.traj_reset(lam)
+    s.traj_enable_trace()
+    s.traj_run(iters)
+    g = s.traj_fetch()
+    g["q"] = s.fetch()["q"].reshape(B, n, d)
+    s.close()
+    caps = corc.Capsules(model, w_coll=w_coll, d_safe=d_safe, scene=scene, w_env=w_env, d_safe_env=d_safe_env)
+    tprm = torc.TrajParams(w_pose=0.5, w_diff=0.3, caps=caps)
+    st = torc.init_state(w.seeds.astype(np.float64).reshape(B, n, d), tprm)
+    if lam is not None:
+        st.lam[:] = lam.astype(np.float64)
+    torc.advance(ch, orc.Params(), tprm, w.target_pos.astype(np.float64).reshape(B, n, 3),
+                 w.target_quat.astype(np.float64).reshape(B, n, 4), st, iters)
+    return g, st
+
+
+@pytest.mark.parametrize("w_coll", [0.0, 1.0])
+def test_single_step_with_obstacles(w_coll):
+    """Environment rows alone (capsule model without self pairs active) and together with the self-collision rows."""
+    ch, model, scene = wl.panda_chain(), wl.panda_capsules(), wl.panda_scene()
+    B, n = 17, 30
+    base = 0.5 * (ch.q_lo + ch.q_hi)
+    w = folded_problem(ch, model, B, n, 55, base if w_coll == 0.0 else PANDA_FOLDED)
+    lam = (10.0 ** np.random.default_rng(2).uniform(-3, -1, size=B)).astype(np.float32)
+    g, st = run_pair_env(ch, model, scene, w, 1, w_coll, 0.25, 1.5, 0.5, lam=lam)
+    assert (g["cost_coll"] > 0).mean() > 0.5                       # rows are active
+    # a pair within 1e-4 m of its hinge switch contributes a whole rank-1 term or nothing depending on rounding
+    # (DESIGN section 13): trajectories with such a pair at the linearisation point are compared loosely
+    caps = corc.Capsules(model, w_coll=w_coll, d_safe=0.25, scene=scene, w_env=1.5, d_safe_env=0.5)
+    thr = np.r_[np.full(len(model.pairs) if w_coll else 0, 0.25), np.full(len(scene.pairs), 0.5)]
+    q0 = w.seeds.astype(np.float64).reshape(B, n, 7)
+    clear = np.array([all(np.all(np.abs(corc.residual(ch, caps, q0[b, i])[0] - thr) > 1e-4) for i in range(n)) for b in range(B)])
+    # ... and so does a pair whose closest point is not unique (axis parallel to the other axis / to a face: the
+    # minimiser jumps along the segment under an fp32-ulp change of q).  Such trajectories are found with the oracle
+    # The same happens where two capsule AXES cross (deep penetration): the direction n = e / |e| is undefined at
+    # |e| = 0 and amplifies rounding by 1 / |e|.  Such trajectories are found with the oracle alone: its own step
+    # moves by more than the bar when its input is perturbed by 1e-6 (the size of fp32 FK rounding).
+    tprm = torc.TrajParams(w_pose=0.5, w_diff=0.3, caps=caps)
+    st2 = torc.init_state(q0 + 1e-6 * np.random.default_rng(9).normal(size=q0.shape), tprm)
+    st2.lam[:] = lam.astype(np.float64)
+    torc.advance(ch, orc.Params(), tprm, w.target_pos.astype(np.float64).reshape(B, n, 3),
+                 w.target_quat.astype(np.float64).reshape(B, n, 4), st2, 1)
+    clear &= np.abs(st2.trial_q - st.trial_q).max(axis=(1, 2)) < 2e-5
+    # crossing axes, explicitly: |e| below 1 mm makes n = e / |e| lose three digits in fp32
+    rad = np.r_[model.radius[model.pairs[:, 0]] + model.radius[model.pairs[:, 1]] if w_coll else [], model.radius[scene.pairs[:, 0]]]
+    clear &= np.array([all(np.all(corc.residual(ch, caps, q0[b, i])[0] + rad > 1e-3) for i in range(n)) for b in range(B)])
+    assert clear.mean() > 0.5
+    err = np.abs(g["trial_q"].reshape(B, n, 7) - st.trial_q).max(axis=(1, 2))
+    assert err[clear].max() <= 2e-5 and err.max() <= 5e-3
+    assert np.allclose(g["F_before"], st.F_before, rtol=1e-4) and np.allclose(g["F_trial"][clear], st.F_trial[clear], rtol=1e-4)
+    margin = clear & (np.abs(st.F_before - st.F_trial) > 1e-3 * st.F_before)
+    acc = (g["mask"] & np.uint64(1)).astype(bool)
+    assert np.array_equal(acc[margin], (st.accepted == 1)[margin])
+
+
+def test_obstacle_argument_errors_and_removal():
+    from paper_2309_09102_b200 import lm
+    ch, model, scene = wl.panda_chain(), wl.panda_capsules(), wl.panda_scene()
+    w = folded_problem(ch, model, 4, 20, 56, 0.5 * (ch.q_lo + ch.q_hi))
+    s = lm.Solver(ch, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0))
+    s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=0.3))
+    with pytest.raises(lm.LmError):
+        s.traj_set_obstacles(scene)                       # capsules first
+    s.traj_run(2)
+    plain = s.fetch()["q"]
+    s.set_state(w.seeds)
+    s.traj_reset()
+    s.traj_set_capsules(model, 0.0, 0.0)
+    s.traj_set_obstacles(scene, 1.0, 0.5)
+    s.traj_run(2)
+    with_env = s.fetch()["q"]
+    assert np.abs(with_env - plain).max() > 1e-4           # the rows act
+    s.set_state(w.seeds)
+    s.traj_reset()
+    s.traj_set_obstacles(None)
+    s.traj_run(2)
+    assert np.array_equal(s.fetch()["q"], plain)           # and removing them gives the plain step back
+    bad = wl.panda_scene()
+    bad.pairs = np.array([[99, 0]])
+    with pytest.raises(lm.LmError):
+        s.traj_set_obstacles(bad)
+    s.close()
