@@ -401,9 +401,26 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
                 if i >= 1:
                     tc.append(a.elapsed_time(b))
             gc_ = solver.traj_fetch()
+            # ... and with the robot-environment rows as well (synthetic scene: 3 cuboids, 10 capsule-cuboid pairs)
+            solver.traj_set_obstacles(wl_.panda_scene(), 1.0, 0.05)
+            te = []
+            for i in range(reps + 1):
+                solver.reset()
+                solver.run(4)
+                solver.traj_reset()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                solver.traj_run(iters)
+                b.record(stream)
+                stream.synchronize()
+                if i >= 1:
+                    te.append(a.elapsed_time(b))
+            ge_ = solver.traj_fetch()
             solver.traj_set_capsules(None)
             coll = {"ms_per_iteration": float(min(tc)) / iters, "capsules": 7, "pairs": 9, "w_coll": 1.0, "d_safe_m": 0.05,
-                    "trajectories_with_active_pairs": int((gc_["cost_coll"] > 0).sum())}
+                    "trajectories_with_active_pairs": int((gc_["cost_coll"] > 0).sum()),
+                    "with_environment_rows": {"ms_per_iteration": float(min(te)) / iters, "cuboids": 3, "pairs": 10,
+                                              "trajectories_with_active_pairs": int((ge_["cost_coll"] > 0).sum())}}
     ms_iter = float(min(ts)) / iters
     alg = traj_step_alg_bytes(d, int(tp.refine_steps)) * w.W
     out = {"workload": f"{w.name}: {w.B} x {w.n}, after 4 pose-only iterations; w_pose=1, w_diff=0.3, refine=1, {iters} iterations",
