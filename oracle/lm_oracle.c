@@ -162,6 +162,46 @@ void orc_residual(const double *p, const double *R, const double *tp, const doub
     }
 }
 
+/* ------------------------------------------------------------------ variant: roll-pitch-yaw residual */
+
+void orc_rpy(const double *R, double *rpy) {
+    /* R = Rz(yaw) Ry(pitch) Rx(roll):  R31 = -sin(pitch), R32 = cos(pitch) sin(roll), R33 = cos(pitch) cos(roll),
+     * R11 = cos(yaw) cos(pitch), R21 = sin(yaw) cos(pitch) */
+    rpy[0] = atan2(R[7], R[8]);
+    rpy[1] = atan2(-R[6], sqrt(R[0] * R[0] + R[3] * R[3]));
+    rpy[2] = atan2(R[3], R[0]);
+}
+
+static double wrap_pi(double x) {
+    const double two_pi = 6.283185307179586476925287;
+    x -= two_pi * floor((x + 0.5 * two_pi) / two_pi);
+    return x;
+}
+
+void orc_residual_rpy(const double *p, const double *R, const double *tp, const double *tquat,
+                      double w_pos, double w_rot, double *r) {
+    double Rt[9], a[3], b[3];
+    orc_quat_to_R(tquat, Rt);
+    orc_rpy(R, a);
+    orc_rpy(Rt, b);
+    for (int i = 0; i < 3; ++i) {
+        r[i] = w_pos * (p[i] - tp[i]);
+        r[3 + i] = w_rot * wrap_pi(a[i] - b[i]);
+    }
+}
+
+void orc_jacobian_to_rpy(int n, const double *R, double *J) {
+    double rpy[3];
+    orc_rpy(R, rpy);
+    const double cp = cos(rpy[1]), sp = sin(rpy[1]), cy = cos(rpy[2]), sy = sin(rpy[2]);
+    /* E = [[cy cp, -sy, 0], [sy cp, cy, 0], [-sp, 0, 1]];  E^-1 = 1/cp [[cy, sy, 0], [-sy cp, cy cp, 0], [cy sp, sy sp, cp]] */
+    const double Ei[9] = {cy / cp, sy / cp, 0.0, -sy, cy, 0.0, cy * sp / cp, sy * sp / cp, 1.0};
+    for (int j = 0; j < n; ++j) {
+        const double w[3] = {J[3 * n + j], J[4 * n + j], J[5 * n + j]};
+        for (int i = 0; i < 3; ++i) J[(3 + i) * n + j] = Ei[3 * i] * w[0] + Ei[3 * i + 1] * w[1] + Ei[3 * i + 2] * w[2];
+    }
+}
+
 /* ------------------------------------------------------------------ Jacobian */
 
 static void jacobian_from_axes(const orc_chain *c, const double *p, const double *z, const double *o,
@@ -244,7 +284,8 @@ typedef struct {
 static void wp_evaluate(const orc_chain *c, const orc_params *prm, const double *tp,
                         const double *tquat, wp_eval *e) {
     orc_fk(c, e->q, e->p, e->R, e->z, e->o);
-    orc_residual(e->p, e->R, tp, tquat, prm->w_pos, prm->w_rot, e->r);
+    if (prm->rot_mode == 1) orc_residual_rpy(e->p, e->R, tp, tquat, prm->w_pos, prm->w_rot, e->r);
+    else orc_residual(e->p, e->R, tp, tquat, prm->w_pos, prm->w_rot, e->r);
     e->F = 0.0;
     for (int k = 0; k < 6; ++k) e->F += e->r[k] * e->r[k];
 }
@@ -279,6 +320,7 @@ int64_t orc_lm_advance(const orc_chain *c, const orc_params *prm, int64_t W, con
         while (k < max_total_iters && (at_most < 0 || done < at_most) && !(sqrt(cur.F) < prm->tol)) {
             double J[6 * ORC_MAX_DOF], Jw[6 * ORC_MAX_DOF], delta[ORC_MAX_DOF];
             jacobian_from_axes(c, cur.p, cur.z, cur.o, J);          /* DESIGN R3 */
+            if (prm->rot_mode == 1) orc_jacobian_to_rpy(n, cur.R, J); /* variant: d(rpy)/dq = E^-1 J_w */
             for (int row = 0; row < 6; ++row)                         /* DESIGN R2b */
                 for (int j = 0; j < n; ++j) Jw[row * n + j] = (row < 3 ? prm->w_pos : prm->w_rot) * J[row * n + j];
             int ok = (orc_lm_delta(n, Jw, cur.r, lam, delta) == 0) && all_finite(delta, n);

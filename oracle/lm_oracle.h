@@ -42,6 +42,8 @@ typedef struct {
     double lambda0, nu_up, nu_down, lambda_min, lambda_max; /* DESIGN R5 */
     double tol;                                             /* DESIGN R7/R8: freeze when sqrt(F) < tol */
     double w_pos, w_rot;                                    /* DESIGN R2b */
+    int32_t rot_mode; /* 0 (default): r_rot = Log(R R_t^T)^vee, DESIGN R2.  1: the paper's literal wording (PAPER.md:L47,
+                         L115-117): element-wise difference of roll, pitch, yaw (variant) */
 } orc_params;
 
 /* status bits (same meaning as include/lm.h, restated, not shared) */
@@ -69,6 +71,18 @@ void orc_log_so3(const double *E, double *w);
 /* r = [w_pos (p - p_t) ; w_rot Log(R R_t^T)^vee], PAPER.md:L47, L115-117 as read by DESIGN R2 */
 void orc_residual(const double *p, const double *R, const double *tp, const double *tquat,
                   double w_pos, double w_rot, double *r);
+
+/* roll, pitch, yaw of R = Rot_z(yaw) Rot_y(pitch) Rot_x(roll) (fixed-axis x-y-z; pitch in [-pi/2, pi/2]) */
+void orc_rpy(const double *R, double *rpy);
+
+/* the paper's literal pose residual: r = [w_pos (p - p_t) ; w_rot wrap(rpy(R) - rpy(R_t))],
+ * every angle difference wrapped to (-pi, pi] */
+void orc_residual_rpy(const double *p, const double *R, const double *tp, const double *tquat,
+                      double w_pos, double w_rot, double *r);
+
+/* rows 3..5 of J (6 x dof row-major, geometric Jacobian) <- E(rpy(R))^-1 J_w, the exact derivative of (roll, pitch,
+ * yaw) wrt q:  w = E d(rpy)/dt,  E = [Rz Ry e_x | Rz e_y | e_z] */
+void orc_jacobian_to_rpy(int dof, const double *R, double *J);
 
 /* geometric Jacobian 6 x dof (row-major, leading dimension dof), DESIGN R3 */
 void orc_jacobian(const orc_chain *c, const double *q, double *J);

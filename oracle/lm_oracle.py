@@ -46,7 +46,7 @@ class _Chain(C.Structure):
 
 class _Params(C.Structure):
     _fields_ = [(k, C.c_double) for k in
-                ("lambda0", "nu_up", "nu_down", "lambda_min", "lambda_max", "tol", "w_pos", "w_rot")]
+                ("lambda0", "nu_up", "nu_down", "lambda_min", "lambda_max", "tol", "w_pos", "w_rot")] + [("rot_mode", C.c_int32)]
 
 
 @dataclass
@@ -60,10 +60,11 @@ class Params:
     tol: float = 0.0
     w_pos: float = 1.0
     w_rot: float = 1.0
+    rot_mode: int = 0   # 0: rotation-vector residual (DESIGN R2); 1: the paper's literal roll-pitch-yaw differences (variant)
 
     def _c(self) -> _Params:
         return _Params(self.lambda0, self.nu_up, self.nu_down, self.lambda_min, self.lambda_max,
-                       self.tol, self.w_pos, self.w_rot)
+                       self.tol, self.w_pos, self.w_rot, int(self.rot_mode))
 
 
 def _chain_c(chain) -> _Chain:
@@ -101,6 +102,12 @@ def lib():
         L.orc_quat_to_R.argtypes = [_dp, _dp]
         L.orc_log_so3.argtypes = [_dp, _dp]
         L.orc_residual.argtypes = [_dp, _dp, _dp, _dp, C.c_double, C.c_double, _dp]
+        L.orc_rpy.argtypes = [_dp, _dp]
+        L.orc_rpy.restype = None
+        L.orc_residual_rpy.argtypes = [_dp, _dp, _dp, _dp, C.c_double, C.c_double, _dp]
+        L.orc_residual_rpy.restype = None
+        L.orc_jacobian_to_rpy.argtypes = [C.c_int, _dp, _dp]
+        L.orc_jacobian_to_rpy.restype = None
         L.orc_jacobian.argtypes = [C.POINTER(_Chain), _dp, _dp]
         L.orc_lu_solve.argtypes = [C.c_int, _dp, _dp, _dp]
         L.orc_lu_solve.restype = C.c_int
@@ -171,6 +178,28 @@ def residual(p, R, target_pos, target_quat, w_pos=1.0, w_rot=1.0):
     lib().orc_residual(_p(_f64(p, (3,))), _p(_f64(R, (3, 3))), _p(_f64(target_pos, (3,))),
                        _p(_f64(target_quat, (4,))), w_pos, w_rot, _p(r))
     return r
+
+
+def rpy(R):
+    """(roll, pitch, yaw) of R = Rz(yaw) Ry(pitch) Rx(roll)."""
+    out = np.empty(3)
+    lib().orc_rpy(_p(_f64(R, (3, 3))), _p(out))
+    return out
+
+
+def residual_rpy(p, R, target_pos, target_quat, w_pos=1.0, w_rot=1.0):
+    r = np.empty(6)
+    lib().orc_residual_rpy(_p(_f64(p, (3,))), _p(_f64(R, (3, 3))), _p(_f64(target_pos, (3,))),
+                           _p(_f64(target_quat, (4,))), w_pos, w_rot, _p(r))
+    return r
+
+
+def jacobian_rpy(chain, q):
+    """6 x d Jacobian of (x, y, z, roll, pitch, yaw) of the flange wrt q: rows 3..5 = E(rpy)^-1 J_w."""
+    J = jacobian(chain, q)
+    _, R = fk(chain, _f64(q, (chain.dof,)))
+    lib().orc_jacobian_to_rpy(chain.dof, _p(_f64(R, (3, 3))), _p(J))
+    return J
 
 
 def jacobian(chain, q):
