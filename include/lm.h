@@ -91,9 +91,15 @@ typedef struct {
     int32_t solver;       /* LM_SOLVER_PRIMAL (default): the d x d system (J^T J + lambda I) delta = -J^T r of PAPER.md:L121;
                              LM_SOLVER_DUAL: the same step as delta = -J^T (J J^T + lambda I_6)^-1 r (6 x 6, no refinement;
                              a disclosed variant) */
+    int32_t rot_residual; /* LM_ROT_LOG (default): r_rot = Log(R R_t^T)^vee (DESIGN R2);  LM_ROT_RPY: the paper's literal wording
+                             (PAPER.md:L47, L115-117), the wrapped element-wise difference of roll, pitch, yaw with
+                             d(rpy)/dq = E(rpy)^-1 J_w (a disclosed variant; singular at pitch = +-90 deg;
+                             not combined with LM_SOLVER_DUAL or lm_traj_*) */
 } lm_params;
 #define LM_SOLVER_PRIMAL 0
 #define LM_SOLVER_DUAL 1
+#define LM_ROT_LOG 0
+#define LM_ROT_RPY 1
 
 /* lm_fetch outputs.  Every pointer is nullable; each may be DEVICE or HOST memory (detected). */
 typedef struct {

@@ -110,6 +110,7 @@ int lm_default_params(lm_params *out) {
     out->refine_steps = 1;
     out->fast_sincos = 0;
     out->solver = LM_SOLVER_PRIMAL;
+    out->rot_residual = LM_ROT_LOG;
     return LM_OK;
 }
 
@@ -128,7 +129,9 @@ int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_
         return LM_EINVAL;
     if (!(prm->lambda0 > 0.f) || !(prm->nu_up > 1.f) || !(prm->nu_down > 1.f) || !(prm->lambda_min > 0.f) ||
         !(prm->lambda_max >= prm->lambda_min) || !(prm->tol >= 0.f) || !(prm->w_pos > 0.f) || !(prm->w_rot > 0.f) ||
-        prm->refine_steps < 0 || prm->refine_steps > 2 || (prm->solver != LM_SOLVER_PRIMAL && prm->solver != LM_SOLVER_DUAL))
+        prm->refine_steps < 0 || prm->refine_steps > 2 || (prm->solver != LM_SOLVER_PRIMAL && prm->solver != LM_SOLVER_DUAL) ||
+        (prm->rot_residual != LM_ROT_LOG && prm->rot_residual != LM_ROT_RPY) ||
+        (prm->solver == LM_SOLVER_DUAL && prm->rot_residual == LM_ROT_RPY))
         return LM_EINVAL;
     for (int j = 0; j < d; ++j) {
         if (!(chain->q_lo[j] <= chain->q_hi[j])) return LM_EINVAL;
@@ -185,7 +188,7 @@ int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_
     a.inv_w_pos = (float)(1.0 / (double)prm->w_pos); a.inv_w_rot = (float)(1.0 / (double)prm->w_rot);
     a.weighted = (prm->w_pos != 1.f || prm->w_rot != 1.f) ? 1 : 0;
     a.refine = prm->refine_steps;
-    a.dual = prm->solver == LM_SOLVER_DUAL ? 1 : 0;
+    a.variant = prm->solver == LM_SOLVER_DUAL ? LM_VAR_DUAL : (prm->rot_residual == LM_ROT_RPY ? LM_VAR_RPY : 0);
     a.W = c->W; a.n = (int32_t)c->n; a.shared_targets = c->shared;
     a.q = reinterpret_cast<float *>(c->ws + lay.q);
     a.lam = reinterpret_cast<float *>(c->ws + lay.lam);

@@ -106,6 +106,9 @@ __device__ __forceinline__ float atan2_pos(float s, float c) {
     return (c < 0.0f) ? sub(3.14159265359f, th) : th;
 }
 
+// atan2(y, x) in (-pi, pi]
+__device__ __forceinline__ float atan2_full(float y, float x) { return copysignf(atan2_pos(fabsf(y), x), y); }
+
 // Pose of one waypoint: everything the LM iteration needs from FK.
 template <int D>
 struct Pose {
@@ -113,6 +116,7 @@ struct Pose {
     float Jw[D][3]; // angular part = joint axis z_j (0 for prismatic)
     float r[6];     // residual (S2)
     float F;        // r . r
+    float Ei[9];    // roll-pitch-yaw variant only: E(rpy)^-1 at this pose (row-major), d(rpy)/dq = E^-1 J_w
 };
 
 // w = Log(E)^vee for theta within 1e-4 of pi (rare: never reached by the documented workloads).
@@ -154,7 +158,7 @@ __device__ __forceinline__ void log_near_pi(const float (&X)[3], const float (&Y
 // Terms with a known 0 are skipped and multiplications by a known 1 become additions in the dot
 // products below: the results equal the generic kernel's up to the sign of zero.
 struct JKnown { uint32_t zv, zw, ov, ow; };
-__host__ __device__ constexpr JKnown jknown(const ChainSpec S, bool weighted) {
+__host__ __device__ constexpr JKnown jknown(const ChainSpec S, bool weighted, bool rpy = false) {
     JKnown K{0, 0, 0, 0};
     if (S.generic) return K;
     for (int j = 0; j < S.dof; ++j)
@@ -176,12 +180,13 @@ __host__ __device__ constexpr JKnown jknown(const ChainSpec S, bool weighted) {
         }
     }
     if (weighted) { K.ov = 0; K.ow = 0; } // a known 1 becomes the weight
+    if (rpy) { K.zw = 0; K.ow = 0; }      // the angular rows are E^-1 J_w: nothing is known about them
     return K;
 }
 
-template <bool WEIGHTED, typename SpecT>
+template <bool WEIGHTED, typename SpecT, bool RPY = false>
 struct JK {
-    static constexpr JKnown K = jknown(SpecT::spec, WEIGHTED);
+    static constexpr JKnown K = jknown(SpecT::spec, WEIGHTED, RPY);
     __device__ __forceinline__ static constexpr bool zero(int j, int k) { return (((k < 3 ? K.zv : K.zw) >> (3 * j + (k < 3 ? k : k - 3))) & 1u) != 0; }
     __device__ __forceinline__ static constexpr bool one(int j, int k) { return (((k < 3 ? K.ov : K.ow) >> (3 * j + (k < 3 ? k : k - 3))) & 1u) != 0; }
 };
@@ -189,7 +194,7 @@ struct NoSpec { static constexpr ChainSpec spec = generic_spec(MAX_DOF); };
 
 // S3: geometric Jacobian (DESIGN R3): revolute [z x (p - o); z], prismatic [z; 0], from the joint axes z_j
 // (src.Jw) and frame origins o_j (src.Jv) that FK retained; dst may be src.
-template <int D, bool WEIGHTED, typename SpecT>
+template <int D, bool WEIGHTED, typename SpecT, bool RPY = false>
 __device__ __forceinline__ void finish_jacobian(const KChain &ch, const Pose<D> &src, const float (&p)[3], float w_pos,
                                                 float w_rot, Pose<D> &dst) {
     constexpr ChainSpec S = SpecT::spec;
@@ -210,7 +215,11 @@ __device__ __forceinline__ void finish_jacobian(const KChain &ch, const Pose<D> 
                 c[i] = za0 ? inner : za1 ? (zb0 ? e[b] : add(e[b], inner)) : (zb0 ? mul(z[a], e[b]) : fma_(z[a], e[b], inner));
             }
 #pragma unroll
-            for (int i = 0; i < 3; ++i) { dst.Jv[j][i] = c[i]; dst.Jw[j][i] = z[i]; }
+            for (int i = 0; i < 3; ++i) {
+                dst.Jv[j][i] = c[i];
+                // roll-pitch-yaw variant: the angular rows become d(rpy)/dq = E^-1 z_j
+                dst.Jw[j][i] = RPY ? fma_(src.Ei[3 * i + 2], z[2], fma_(src.Ei[3 * i + 1], z[1], mul(src.Ei[3 * i], z[0]))) : z[i];
+            }
         } else {
 #pragma unroll
             for (int i = 0; i < 3; ++i) { dst.Jv[j][i] = z[i]; dst.Jw[j][i] = 0.f; }
@@ -232,11 +241,13 @@ __device__ __forceinline__ void finish_jacobian(const KChain &ch, const Pose<D> 
 struct NoFrameSink {
     __device__ __forceinline__ void operator()(int, const float (&)[3], const float (&)[3], const float (&)[3], const float (&)[3]) const {}
 };
-template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool WITH_JAC = true, typename Sink = NoFrameSink>
+//   RPY = true (variant): the rotational residual is the wrapped element-wise difference of
+//   roll, pitch, yaw (PAPER.md:L47, L115-117 read literally) against `trpy` = rpy of the target.
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool WITH_JAC = true, typename Sink = NoFrameSink, bool RPY = false>
 __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D], const float (&pt)[3],
                                           const float (&Rt)[3][3], float w_pos, float w_rot,
                                           Pose<D> &P, float *p_out, float (*R_out)[3], float *frame_p = nullptr,
-                                          const Sink &sink = Sink()) {
+                                          const Sink &sink = Sink(), const float *trpy = nullptr) {
     constexpr ChainSpec S = SpecT::spec;
     float X[3], Y[3], Z[3], o[3];
 #pragma unroll
@@ -321,6 +332,24 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
         }
     }
 
+    float w[3];
+    if (RPY) {
+        // R = Rz(yaw) Ry(pitch) Rx(roll): R31 = X[2] = -sin(pitch), R32 = Y[2], R33 = Z[2], R11 = X[0], R21 = X[1]
+        const float cp = sqrtf(fma_(X[1], X[1], mul(X[0], X[0])));
+        const float a[3] = {atan2_full(Y[2], Z[2]), atan2_full(-X[2], cp), atan2_full(X[1], X[0])};
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { // wrap to (-pi, pi]
+            const float dlt = sub(a[i], trpy[i]);
+            const float k = rintf(mul(dlt, 0.159154943f));
+            w[i] = fma_(k, -1.74845553e-07f, fma_(k, -6.28318548f, dlt)); // 2 pi = 6.28318548 - 1.74845553e-07
+        }
+        // E^-1 = 1/cp [[cy, sy, 0], [-sy cp, cy cp, 0], [cy sp, sy sp, cp]]
+        const float icp = __fdividef(1.0f, cp);
+        const float cy = mul(X[0], icp), sy = mul(X[1], icp), tp_ = mul(-X[2], icp);
+        P.Ei[0] = mul(cy, icp); P.Ei[1] = mul(sy, icp); P.Ei[2] = 0.f;
+        P.Ei[3] = -sy;          P.Ei[4] = cy;           P.Ei[5] = 0.f;
+        P.Ei[6] = mul(cy, tp_); P.Ei[7] = mul(sy, tp_); P.Ei[8] = 1.f;
+    } else {
     // S2: E = R_ee R_t^T = sum_k a_k b_k^T (a_k, b_k = k-th columns);
     //     vee(antisym E) = 1/2 sum_k b_k x a_k,  tr E = sum_k a_k . b_k          (DESIGN R2)
     float v[3], tr;
@@ -346,8 +375,9 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
     const float theta = atan2_pos(sn, cth);
     // theta / s; the small-angle series 1 + s^2/6 takes over below s = 1e-4
     const float scale = (sn < 1e-4f) ? fma_(s2, 0.166666667f, 1.0f) : __fdividef(theta, sn);
-    float w[3] = {mul(scale, v[0]), mul(scale, v[1]), mul(scale, v[2])};
+    w[0] = mul(scale, v[0]); w[1] = mul(scale, v[1]); w[2] = mul(scale, v[2]);
     if (sn < 1e-4f && cth <= 0.f) log_near_pi(X, Y, Z, Rt, v, cth, theta, w);
+    }
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         const float rp = sub(p[i], pt[i]);
@@ -361,16 +391,16 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
 #pragma unroll
         for (int i = 0; i < 3; ++i) frame_p[i] = p[i];
     }
-    if (WITH_JAC) finish_jacobian<D, WEIGHTED, SpecT>(ch, P, p, w_pos, w_rot, P);
+    if (WITH_JAC) finish_jacobian<D, WEIGHTED, SpecT, RPY>(ch, P, p, w_pos, w_rot, P);
 }
 
 template <int D>
 __device__ __forceinline__ float jentry(const Pose<D> &P, int j, int k) { return k < 3 ? P.Jv[j][k] : P.Jw[j][k - 3]; }
 
 // init + sum_k J[k][i] J[k][j] in the order k = 0..5 (rows 0..2 linear, 3..5 angular); HAVE = false: no init term
-template <int D, bool WEIGHTED, typename SpecT, bool HAVE>
+template <int D, bool WEIGHTED, typename SpecT, bool HAVE, bool RPY = false>
 __device__ __forceinline__ float coldot_k(const Pose<D> &P, int i, int j, float init) {
-    using K = JK<WEIGHTED, SpecT>;
+    using K = JK<WEIGHTED, SpecT, RPY>;
     float acc = init;
     bool have = HAVE;
 #pragma unroll
@@ -387,9 +417,9 @@ __device__ __forceinline__ float coldot_k(const Pose<D> &P, int i, int j, float 
     return have ? acc : 0.f;
 }
 // sum_k J[k][i] t[k]
-template <int D, bool WEIGHTED, typename SpecT>
+template <int D, bool WEIGHTED, typename SpecT, bool RPY = false>
 __device__ __forceinline__ float colvec_k(const Pose<D> &P, int i, const float (&t)[6]) {
-    using K = JK<WEIGHTED, SpecT>;
+    using K = JK<WEIGHTED, SpecT, RPY>;
     float acc = 0.f;
     bool have = false;
 #pragma unroll
@@ -434,16 +464,16 @@ __device__ __forceinline__ void chol_solve(const float (&L)[D][D], const float (
 //   rho = -J^T (r + J delta) - lambda delta,  delta += A^-1 rho                     (DESIGN R4)
 // which removes the 1/lambda amplification of fp32 rounding along the self-motion direction.
 // Returns false on a non-positive pivot or a non-finite step (=> the iteration is a reject).
-template <int D, bool WEIGHTED, typename SpecT>
+template <int D, bool WEIGHTED, typename SpecT, bool RPY = false>
 __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine, float (&delta)[D]) {
-    using K = JK<WEIGHTED, SpecT>;
+    using K = JK<WEIGHTED, SpecT, RPY>;
     float L[D][D], invd[D], g[D];
 #pragma unroll
     for (int i = 0; i < D; ++i) {
 #pragma unroll
-        for (int j = 0; j < i; ++j) L[i][j] = coldot_k<D, WEIGHTED, SpecT, false>(P, i, j, 0.f);
-        L[i][i] = coldot_k<D, WEIGHTED, SpecT, true>(P, i, i, lam); // lambda folded into the first FMA of the diagonal
-        g[i] = -colvec_k<D, WEIGHTED, SpecT>(P, i, P.r);
+        for (int j = 0; j < i; ++j) L[i][j] = coldot_k<D, WEIGHTED, SpecT, false, RPY>(P, i, j, 0.f);
+        L[i][i] = coldot_k<D, WEIGHTED, SpecT, true, RPY>(P, i, i, lam); // lambda folded into the first FMA of the diagonal
+        g[i] = -colvec_k<D, WEIGHTED, SpecT, RPY>(P, i, P.r);
     }
     bool ok = true;
 #pragma unroll
@@ -474,7 +504,7 @@ __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine
             t[3 + k] = sw;
         }
 #pragma unroll
-        for (int i = 0; i < D; ++i) rho[i] = -fma_(lam, delta[i], colvec_k<D, WEIGHTED, SpecT>(P, i, t));
+        for (int i = 0; i < D; ++i) rho[i] = -fma_(lam, delta[i], colvec_k<D, WEIGHTED, SpecT, RPY>(P, i, t));
         chol_solve<D>(L, invd, rho, e);
 #pragma unroll
         for (int i = 0; i < D; ++i) delta[i] = add(delta[i], e[i]);

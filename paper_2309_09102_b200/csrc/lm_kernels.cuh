@@ -16,7 +16,7 @@ struct KArgs {
     KChain ch;
     float lambda0, nu_up, inv_nu_down, lambda_min, lambda_max, tol2;
     float w_pos, w_rot, inv_w_pos, inv_w_rot;
-    int32_t weighted, refine, dual;
+    int32_t weighted, refine, variant; // variant: 0, LM_VAR_DUAL or LM_VAR_RPY
     int64_t W;              // waypoint blocks
     int32_t n;              // waypoints per trajectory
     int32_t shared_targets; // target index = w % n
@@ -50,7 +50,10 @@ __device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z,
 #define LM_MIN_BLOCKS 1
 #endif
 
-template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool DUAL = false>
+// VAR: 0 = the d x d system with the rotation-vector residual (the hot path), LM_VAR_DUAL = the 6 x 6 dual form,
+// LM_VAR_RPY = the roll-pitch-yaw residual (disclosed variants, DESIGN.md sections 12 and 14)
+constexpr int LM_VAR_DUAL = 1, LM_VAR_RPY = 2;
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, int VAR = 0>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kernel(const __grid_constant__ KArgs A) {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = w < A.W;
@@ -83,8 +86,16 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         for (int i = 0; i < 3; ++i) pt[i] = __ldg(A.tp + (int64_t)i * Wt + wt);
         quat_to_cols(__ldg(A.tq + wt), __ldg(A.tq + Wt + wt), __ldg(A.tq + 2 * Wt + wt), __ldg(A.tq + 3 * Wt + wt), Rt);
     }
+    constexpr bool DUAL = VAR == LM_VAR_DUAL, RPY = VAR == LM_VAR_RPY;
+    float trpy[3] = {0.f, 0.f, 0.f}; // roll, pitch, yaw of the target (Rt[k] = k-th column of R_t)
+    if (RPY) {
+        trpy[0] = atan2_full(Rt[1][2], Rt[2][2]);
+        trpy[1] = atan2_full(-Rt[0][2], sqrtf(fma_(Rt[0][1], Rt[0][1], mul(Rt[0][0], Rt[0][0]))));
+        trpy[2] = atan2_full(Rt[0][1], Rt[0][0]);
+    }
     Pose<D> cur;
-    eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, cur, nullptr, nullptr);
+    eval_pose<D, FAST, WEIGHTED, SpecT, true, NoFrameSink, RPY>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, cur, nullptr, nullptr, nullptr,
+                                                                NoFrameSink(), trpy);
 
     // ---- S3..S9: the LM loop, entirely on the device.  A lane is `active` while it is not
     // frozen and has iterations left; the warp leaves the loop when no lane is active.
@@ -95,7 +106,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
 
         float delta[D];
         const bool ok = DUAL ? lm_delta_dual<D, WEIGHTED, SpecT>(cur, lam, delta)            // S4, S5 (variant)
-                             : lm_delta<D, WEIGHTED, SpecT>(cur, lam, A.refine, delta);     // S4, S5
+                             : lm_delta<D, WEIGHTED, SpecT, RPY>(cur, lam, A.refine, delta); // S4, S5
         float qt[D];
         bool clamped = false;
 #pragma unroll
@@ -106,7 +117,8 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         }
         Pose<D> tri; // S7: FK + residual at the trial point; its Jacobian (S3) is formed only if the step is accepted
         float ptri[3];
-        eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, tri, nullptr, nullptr, ptri);
+        eval_pose<D, FAST, WEIGHTED, SpecT, false, NoFrameSink, RPY>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, tri, nullptr, nullptr, ptri,
+                                                                     NoFrameSink(), trpy);
 
         if (A.trace_q != nullptr && active && live) {
 #pragma unroll
@@ -131,7 +143,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         if (accept) {
 #pragma unroll
             for (int j = 0; j < D; ++j) q[j] = qt[j];
-            finish_jacobian<D, WEIGHTED, SpecT>(A.ch, tri, ptri, A.w_pos, A.w_rot, cur); // S3 straight into the current state
+            finish_jacobian<D, WEIGHTED, SpecT, RPY>(A.ch, tri, ptri, A.w_pos, A.w_rot, cur); // S3 straight into the current state
 #pragma unroll
             for (int i = 0; i < 6; ++i) cur.r[i] = tri.r[i];
             cur.F = tri.F;

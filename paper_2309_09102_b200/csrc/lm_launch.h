@@ -16,14 +16,16 @@ cudaError_t launch_fk_spec(int spec_id, bool fast, unsigned grid, unsigned block
 // ---- launch helpers used by the instantiation units
 template <int D, typename SpecT>
 cudaError_t launch_iterate_t(bool fast, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const KArgs &a) {
-    if (a.dual) { // LM_SOLVER_DUAL (a disclosed variant): its own instantiations, the primal kernels are untouched
-        if (fast) {
-            if (weighted) lm_iterate_kernel<D, true, true, SpecT, true><<<grid, block, 0, s>>>(a);
-            else lm_iterate_kernel<D, true, false, SpecT, true><<<grid, block, 0, s>>>(a);
-        } else {
-            if (weighted) lm_iterate_kernel<D, false, true, SpecT, true><<<grid, block, 0, s>>>(a);
-            else lm_iterate_kernel<D, false, false, SpecT, true><<<grid, block, 0, s>>>(a);
-        }
+    if (a.variant == LM_VAR_DUAL || a.variant == LM_VAR_RPY) { // disclosed variants: their own instantiations, the hot path's kernels are untouched
+#define LM_IT_LAUNCH(V)                                                                                \
+    do {                                                                                               \
+        if (fast) { if (weighted) lm_iterate_kernel<D, true, true, SpecT, V><<<grid, block, 0, s>>>(a);   \
+                    else lm_iterate_kernel<D, true, false, SpecT, V><<<grid, block, 0, s>>>(a); }         \
+        else { if (weighted) lm_iterate_kernel<D, false, true, SpecT, V><<<grid, block, 0, s>>>(a);       \
+               else lm_iterate_kernel<D, false, false, SpecT, V><<<grid, block, 0, s>>>(a); }             \
+    } while (0)
+        if (a.variant == LM_VAR_DUAL) LM_IT_LAUNCH(LM_VAR_DUAL); else LM_IT_LAUNCH(LM_VAR_RPY);
+#undef LM_IT_LAUNCH
     } else if (fast) {
         if (weighted) lm_iterate_kernel<D, true, true, SpecT><<<grid, block, 0, s>>>(a);
         else lm_iterate_kernel<D, true, false, SpecT><<<grid, block, 0, s>>>(a);

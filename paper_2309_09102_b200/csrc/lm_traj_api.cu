@@ -105,6 +105,7 @@ int lm_traj_default_params(lm_traj_params *out) {
 
 int lm_traj_attach(lm_ctx *c, const lm_traj_params *p, void *workspace, size_t bytes) {
     if (!c || !p || !workspace) return LM_EINVAL;
+    if (c->args.variant == LM_VAR_RPY) return LM_EINVAL; // the trajectory-level step uses the rotation-vector residual
     if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return LM_EINVAL;
     if (!(p->w_pose >= 0.f) || !(p->w_diff >= 0.f) || !(p->lambda0 > 0.f) || !(p->nu_up > 1.f) || !(p->nu_down > 1.f) ||
         !(p->lambda_min > 0.f) || !(p->lambda_max >= p->lambda_min) || p->refine_steps < 0 || p->refine_steps > 2)

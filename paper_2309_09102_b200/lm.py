@@ -35,6 +35,7 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR = 0, 1
 LM_SOLVER_PRIMAL, LM_SOLVER_DUAL = 0, 1
+LM_ROT_LOG, LM_ROT_RPY = 0, 1
 
 
 class LmChain(C.Structure):
@@ -52,7 +53,7 @@ class LmParams(C.Structure):
     _fields_ = [("lambda0", C.c_float), ("nu_up", C.c_float), ("nu_down", C.c_float),
                 ("lambda_min", C.c_float), ("lambda_max", C.c_float), ("tol", C.c_float),
                 ("w_pos", C.c_float), ("w_rot", C.c_float), ("refine_steps", C.c_int32),
-                ("fast_sincos", C.c_int32), ("solver", C.c_int32)]
+                ("fast_sincos", C.c_int32), ("solver", C.c_int32), ("rot_residual", C.c_int32)]
 
 
 class LmStats(C.Structure):

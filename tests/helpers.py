@@ -28,7 +28,7 @@ def run_oracle(w: wl.Workload, max_iters=None, **kw) -> orc.State:
 def make_solver(w: wl.Workload, **kw):
     from paper_2309_09102_b200 import lm
     pkw = {k: kw.pop(k) for k in list(kw) if k in ("lambda_min", "lambda_max", "nu_up", "nu_down", "w_pos",
-                                                    "w_rot", "refine_steps", "fast_sincos", "solver")}
+                                                    "w_rot", "refine_steps", "fast_sincos", "solver", "rot_residual")}
     prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol, **pkw)
     return lm.Solver(w.chain, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, **kw)
 

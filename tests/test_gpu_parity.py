@@ -216,3 +216,30 @@ def test_dual_form_variant_matches_the_oracle(lm):
     w = wl.config3(H.oracle_fk(ch), B=128)
     g, o = H.run_gpu(w, solver=lm.LM_SOLVER_DUAL), H.run_oracle(w)
     _check_free_running(w, g, o)
+
+
+# ------------------------------------------------------------------ NEXT-4 (ii): roll-pitch-yaw residual
+
+def test_rpy_residual_variant_matches_the_oracle(lm):
+    """LM_ROT_RPY: the paper's literal residual, wrapped element-wise rpy differences with
+    d(rpy)/dq = E^-1 J_w, against the oracle run with rot_mode = 1: configs[0] and a 64-trajectory configs[1]."""
+    w = wl.config1(H.oracle_fk(wl.panda_chain()))
+    g = H.run_gpu(w, rot_residual=lm.LM_ROT_RPY)
+    o = H.run_oracle(w, rot_mode=1)
+    _check_free_running(w, g, o, check_pose=False)
+    assert np.abs(g["q"] - o.q).max() < 2e-5
+    w = wl.config2(H.oracle_fk(wl.panda_chain()), B=64)
+    g = H.run_gpu(w, rot_residual=lm.LM_ROT_RPY)
+    o = H.run_oracle(w, rot_mode=1)
+    _check_free_running(w, g, o, frac_edge=0.01, check_pose=False)
+    assert (g["status"] & 1).mean() > 0.99
+    # the pose it converges to is the target pose: the rotation-vector error of the result is small too
+    pe, re = H.pose_errors_by_oracle(w, g["q"])
+    assert pe.max() < 2e-5 and re.max() < 2e-5
+    # not combinable with the dual solver or the trajectory-level step
+    with pytest.raises(lm.LmError):
+        H.make_solver(w, rot_residual=lm.LM_ROT_RPY, solver=lm.LM_SOLVER_DUAL)
+    s = H.make_solver(w, rot_residual=lm.LM_ROT_RPY)
+    with pytest.raises(lm.LmError):
+        s.traj_attach()
+    s.close()
