@@ -1,4 +1,5 @@
-// lm_coll.cuh -- robot-robot collision rows of the trajectory-level step (sm_100a).
+// lm_coll.cuh -- collision rows of the trajectory-level step (sm_100a): robot-robot
+// (capsule-capsule, below) and robot-environment (capsule-cuboid: segment_box_closest).
 //
 // "each robot is represented as a set of capsules with endpoints (a, b) and radius c ... the minimum distance
 //  between a capsule pair [is] the minimum cost, less c1 + c2, of [the] convex quadratic program

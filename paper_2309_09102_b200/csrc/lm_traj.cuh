@@ -5,12 +5,12 @@
 //   J^T J + lambda I = block-tridiag( T_i , -w_d^2 I ),   T_i = w_p^2 J_i^T J_i + (c_i w_d^2 + lambda) I,
 //   c_i = 1 at the two ends, 2 inside (0 for n = 1).
 // The block structure is kept (include/lm.h): block Gaussian elimination
-// along the waypoint index (block Thomas),
-//   S_1 = T_1,  S_i = T_i - w_d^4 S_{i-1}^-1,  h_i = g_i + w_d^2 S_{i-1}^-1 h_{i-1},
-//   x_n = S_n^-1 h_n,  x_i = S_i^-1 h_i + w_d^2 S_i^-1 x_{i+1},          delta = -x,
-// one LANE per trajectory (the recurrence is sequential in i, the trajectories are the parallel
-// dimension), d x d symmetric blocks in registers, S_i^-1 by the symmetric sweep operator.
-// Everything per-waypoint (FK, Jacobian, J^T J, J^T r, trial cost) runs one thread per waypoint.
+// along the waypoint index,
+//   S_i = T_i - w_d^4 S_prev^-1,  z_i = S_i^-1 (g_i + w_d^2 z_prev),  x_i = z_i + w_d^2 S_i^-1 x_next,  delta = -x,
+// run from BOTH ends of the trajectory towards the middle waypoint (tl_solve_kernel), one LANE per
+// trajectory (the recurrence is sequential in i, the trajectories are the parallel dimension), d x d
+// symmetric blocks in registers, S_i^-1 by the symmetric sweep operator.  Everything per-waypoint
+// (FK, Jacobian, J^T J, J^T r, collision rows, trial cost) runs one thread per waypoint.
 //
 // Layout ("tile order"): trajectories are grouped in tiles of 32 (one warp); the record of
 // waypoint i of tile bt is the chunk  wid = bt * n + i,  and component c of lane l (trajectory
