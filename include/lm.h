@@ -310,6 +310,8 @@ typedef struct {
     float mjac_rev;     /* 7 deg in rad */
     float mjac_pris;    /* 0.02 m */
     int32_t pose_iters; /* cap of each pose-only phase, 1..64 (default 10) */
+    float min_clearance; /* with capsules / obstacles set (lm_traj_set_capsules): a valid trajectory keeps every listed pair at
+                            least this far apart at every waypoint ("at no timestep ... collide"); default 0 */
 } lm_plan_params;
 
 /* lm_plan_fetch outputs; every pointer nullable, device or host. */
@@ -321,6 +323,7 @@ typedef struct {
     float *max_pos_err, *max_rot_err; /* [B] of the CURRENT trajectory at the last record point */
     float *mjac_rev, *mjac_pris;      /* [B] likewise */
     float *cur_length;                /* [B] likewise */
+    float *min_clearance;             /* [B] likewise: smallest capsule clearance (NaN without capsules) */
     int64_t valid_trajectories;       /* OUT */
 } lm_plan_stats;
 

@@ -16,7 +16,8 @@ L170), and no joint changes by more than 7 deg (revolute) / 2 cm (prismatic) acr
 Trajectory length: "the cumulative change in configuration-space across a
 trajectory (measured in radians and meters)" = sum_i sum_j |q_{i+1}[j] - q_i[j]|.
 mjac: max_i max_j |q_{i+1}[j] - q_i[j]|, here kept per joint type because the two
-limits have different units.  Collision terms are out of scope.
+limits have different units.  With a capsule model (lm_coll_oracle.py, synthetic) a valid trajectory is also
+collision free: "At no timestep in the trajectory can the robot collide with itself or the environment" (L49).
 
 Readings: P1 a pose-only phase is lm_run from fresh LM state (lambda0,
 0 iterations) with the per-waypoint freeze |r|_2 < tol, capped at `pose_iters`; P2 the
@@ -31,6 +32,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
+from . import lm_coll_oracle as corc
 from . import lm_oracle as orc
 from . import lm_traj_oracle as torc
 
@@ -44,6 +46,7 @@ class PlanParams:
     mjac_rev: float = 7.0 * DEG    # rad
     mjac_pris: float = 0.02        # m,
     pose_iters: int = 10           # cap of each pose-only phase (reading P1)
+    min_clearance: float = 0.0     # m: with a capsule model, every listed pair keeps at least this clearance
 
 
 def trajectory_length(q: np.ndarray) -> np.ndarray:
@@ -80,9 +83,16 @@ class PlanResult:
     history: list = field(default_factory=list)  # per record point: dict(valid_now, margins)
 
 
+def min_clearance(chain, caps, q: np.ndarray) -> np.ndarray:
+    """q [B, n, d] -> [B]: smallest clearance over all listed capsule pairs and all waypoints."""
+    B, n, _ = q.shape
+    return np.array([min(corc.residual(chain, caps, q[b, i])[0].min() for i in range(n)) for b in range(B)])
+
+
 def plan(chain, pose_params: orc.Params, tparams: torc.TrajParams, pparams: PlanParams, target_pos, target_quat,
          seeds, cycles: int, nthreads: int = 0) -> PlanResult:
-    """target_pos [B, n, 3], target_quat [B, n, 4], seeds [B, n, d] (fp64)."""
+    """target_pos [B, n, 3], target_quat [B, n, 4], seeds [B, n, d] (fp64).  With tparams.caps set, the collision
+    rows are part of the trajectory-level step and a valid trajectory must also be collision free."""
     q = np.array(seeds, dtype=np.float64)
     B, n, d = q.shape
     tp = np.asarray(target_pos, np.float64).reshape(B * n, 3)
@@ -104,13 +114,18 @@ def plan(chain, pose_params: orc.Params, tparams: torc.TrajParams, pparams: Plan
         re_ = st.rot_err.reshape(B, n).max(axis=1)
         mr, mp = mjac(q, jt)
         ok = (pe < pparams.pos_tol) & (re_ < pparams.rot_tol) & (mr <= pparams.mjac_rev) & (mp <= pparams.mjac_pris)
+        clr = None
+        if tparams.caps is not None:
+            clr = min_clearance(chain, tparams.caps, q)
+            ok &= clr >= pparams.min_clearance
         # ---- anytime bookkeeping (P3)
         q_valid[ok] = q[ok]
         length[ok] = trajectory_length(q[ok])
         first[ok & ~valid] = c
         valid |= ok
         records += ok
-        hist.append({"valid_now": ok.copy(), "pos": pe.copy(), "rot": re_.copy(), "mjac_rev": mr.copy(), "mjac_pris": mp.copy()})
+        hist.append({"valid_now": ok.copy(), "pos": pe.copy(), "rot": re_.copy(), "mjac_rev": mr.copy(), "mjac_pris": mp.copy(),
+                     "clearance": None if clr is None else clr.copy()})
         if c == cycles:
             break
         # ---- one trajectory-level step for the trajectories that are pose-valid now (P2)

@@ -150,8 +150,11 @@ __device__ __forceinline__ float segment_box_closest(const float (&a)[3], const 
 
 // Calls f(g, r) for every pair whose hinge is active at this waypoint: g[D] = d r / d q, r = the residual.
 // Fr = frames retained by FK (Fr.Jw[j] = z_j, Fr.Jv[j] = o_j: eval_pose with WITH_JAC = false).
-template <int D, typename SpecT, typename F>
-__device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, const CapsWorld &W, const Pose<D> &Fr, F &&f) {
+// CLEAR_ONLY: no rows; *min_clear receives the smallest clearance `dist` over all listed pairs (lm_plan_*: a valid
+// trajectory must be collision free).
+template <int D, typename SpecT, bool CLEAR_ONLY = false, typename F>
+__device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, const CapsWorld &W, const Pose<D> &Fr, F &&f,
+                                          float *min_clear = nullptr) {
     constexpr ChainSpec S = SpecT::spec;
     for (int p = 0; p < C.nenv; ++p) { // robot-environment rows: the obstacle does not move
         const int k = C.env_pair[p][0], ob = C.env_pair[p][1];
@@ -178,6 +181,7 @@ __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, cons
         }
         const float len = sqrtf(dot3(eb, eb));
         const float dist = sub(len, C.c[k]);
+        if (CLEAR_ONLY) { *min_clear = fminf(*min_clear, dist); continue; }
         if (!(dist < C.d_safe_env)) continue;
         const float r = mul(C.w_env, sub(C.d_safe_env, dist));
         const float il = (len > 0.f) ? __fdividef(1.0f, len) : 0.f; // axis inside the box: no direction, the row keeps its value
@@ -222,6 +226,7 @@ __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, cons
         }
         const float len = sqrtf(dot3(e, e));
         const float dist = sub(sub(len, C.c[k1]), C.c[k2]);
+        if (CLEAR_ONLY) { *min_clear = fminf(*min_clear, dist); continue; }
         if (!(dist < C.d_safe)) continue;
         const float r = mul(C.w_coll, sub(C.d_safe, dist));
         const float il = (len > 0.f) ? __fdividef(1.0f, len) : 0.f; // the axes touch: no direction, the row keeps its value

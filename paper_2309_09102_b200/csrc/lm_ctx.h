@@ -29,7 +29,8 @@ struct PlanState { // non-stationary schedule + anytime bookkeeping (lm_plan_*),
     lm_plan_params prm{};
     char *ws = nullptr;
     float *q_valid = nullptr;                 // [d][W] w-order
-    float *cur = nullptr;                     // [5][B] max pos err, max rot err, mjac rev, mjac pris, length of the current trajectory
+    float *cur = nullptr;                     // [6][B] max pos err, max rot err, mjac rev, mjac pris, length, min capsule clearance
+    float *clear = nullptr;                   // [W] per-waypoint clearance (only with capsules)
     float *len_valid = nullptr;               // [B]
     int32_t *gate = nullptr, *first = nullptr, *records = nullptr; // [B]
     uint8_t *valid = nullptr;                 // [B]
@@ -64,6 +65,7 @@ namespace lmk {
 int materialize_state(lm_ctx *c);        // if nothing has run yet: state := seeds (a zero-iteration launch)
 int refresh_waypoint_outputs(lm_ctx *c);
 int reset_waypoint_lm_state(lm_ctx *c);  // lambda := lambda0, iters := 0, mask := 0 for every waypoint; q is kept
+int launch_clearance(lm_ctx *c, float *clear_out); // lm_traj_api.cu
 int run_pose_phase(lm_ctx *c, int max_iters); // = lm_run // zero-iteration launch: re-evaluates |r|, errors, frozen flag at the current q
 }
 

@@ -15,7 +15,7 @@ namespace {
 constexpr int PLAN_THREADS = 128;
 
 struct PLayout {
-    size_t q_valid, cur, len_valid, gate, first, records, valid, total, all;
+    size_t q_valid, clear, cur, len_valid, gate, first, records, valid, total, all;
 };
 
 PLayout make_playout(int d, int64_t B, int64_t n) {
@@ -24,7 +24,8 @@ PLayout make_playout(int d, int64_t B, int64_t n) {
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes); return o; };
     L.q_valid = take(4 * W * d);
-    L.cur = take(4 * 5 * (size_t)B);
+    L.clear = take(4 * W);
+    L.cur = take(4 * 6 * (size_t)B);
     L.len_valid = take(4 * (size_t)B);
     L.gate = take(4 * (size_t)B);
     L.first = take(4 * (size_t)B);
@@ -39,8 +40,9 @@ struct PArgs {
     int32_t dof, n;
     int64_t B, W;
     uint32_t prismatic_mask;
-    float pos_tol, rot_tol, mjac_rev, mjac_pris;
-    int32_t cycle;
+    float pos_tol, rot_tol, mjac_rev, mjac_pris, min_clearance;
+    int32_t cycle, use_clear;
+    const float *clear;        // [W] smallest capsule clearance per waypoint (use_clear)
     const float *q;            // [d][W] w-order, current joint values
     const float *perr, *rerr;  // [W] of the pose kernel's last launch
     float *q_valid, *cur, *len_valid;
@@ -51,13 +53,14 @@ struct PArgs {
 // One block per trajectory.  max is order-free; the length is summed in a fixed order (each thread
 // its strided waypoints in order, then a fixed tree): it depends on n only.
 __global__ void __launch_bounds__(PLAN_THREADS) plan_check_kernel(const PArgs A) {
-    __shared__ float red[5][PLAN_THREADS];
+    __shared__ float red[6][PLAN_THREADS];
     __shared__ int s_valid;
     const int64_t b = blockIdx.x;
     const int t = threadIdx.x;
     const int64_t w0 = b * A.n;
-    float mpos = 0.f, mrot = 0.f, mrev = 0.f, mpris = 0.f, len = 0.f;
+    float mpos = 0.f, mrot = 0.f, mrev = 0.f, mpris = 0.f, len = 0.f, mclr = 3.0e38f;
     for (int i = t; i < A.n; i += PLAN_THREADS) {
+        if (A.use_clear) mclr = fminf(mclr, A.clear[w0 + i]);
         mpos = fmaxf(mpos, A.perr[w0 + i]);
         mrot = fmaxf(mrot, A.rerr[w0 + i]);
         if (i + 1 < A.n) {
@@ -70,7 +73,7 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_check_kernel(const PArgs A)
             }
         }
     }
-    red[0][t] = mpos; red[1][t] = mrot; red[2][t] = mrev; red[3][t] = mpris; red[4][t] = len;
+    red[0][t] = mpos; red[1][t] = mrot; red[2][t] = mrev; red[3][t] = mpris; red[4][t] = len; red[5][t] = mclr;
     __syncthreads();
     for (int s = PLAN_THREADS / 2; s > 0; s >>= 1) {
         if (t < s) {
@@ -79,14 +82,15 @@ __global__ void __launch_bounds__(PLAN_THREADS) plan_check_kernel(const PArgs A)
             red[2][t] = fmaxf(red[2][t], red[2][t + s]);
             red[3][t] = fmaxf(red[3][t], red[3][t + s]);
             red[4][t] = __fadd_rn(red[4][t], red[4][t + s]);
+            red[5][t] = fminf(red[5][t], red[5][t + s]);
         }
         __syncthreads();
     }
     if (t == 0) {
-        mpos = red[0][0]; mrot = red[1][0]; mrev = red[2][0]; mpris = red[3][0]; len = red[4][0];
-        A.cur[b] = mpos; A.cur[A.B + b] = mrot; A.cur[2 * A.B + b] = mrev; A.cur[3 * A.B + b] = mpris; A.cur[4 * A.B + b] = len;
+        mpos = red[0][0]; mrot = red[1][0]; mrev = red[2][0]; mpris = red[3][0]; len = red[4][0]; mclr = red[5][0];
+        A.cur[b] = mpos; A.cur[A.B + b] = mrot; A.cur[2 * A.B + b] = mrev; A.cur[3 * A.B + b] = mpris; A.cur[4 * A.B + b] = len; A.cur[5 * A.B + b] = A.use_clear ? mclr : nanf("");
         const bool pose_ok = (mpos < A.pos_tol) && (mrot < A.rot_tol) && (len == len);
-        const bool ok = pose_ok && (mrev <= A.mjac_rev) && (mpris <= A.mjac_pris);
+        const bool ok = pose_ok && (mrev <= A.mjac_rev) && (mpris <= A.mjac_pris) && (!A.use_clear || mclr >= A.min_clearance);
         A.gate[b] = pose_ok ? 1 : 0;
         if (ok) {
             if (!A.valid[b]) A.first[b] = A.cycle;
@@ -107,7 +111,7 @@ __global__ void plan_clear_kernel(PArgs A, float nanv) {
     if (x < A.W * A.dof) A.q_valid[x] = nanv;
     if (x < A.B) {
         A.gate[x] = 0; A.first[x] = -1; A.records[x] = 0; A.valid[x] = 0; A.len_valid[x] = nanv;
-        for (int k = 0; k < 5; ++k) A.cur[k * A.B + x] = nanv;
+        for (int k = 0; k < 6; ++k) A.cur[k * A.B + x] = nanv;
     }
 }
 
@@ -123,6 +127,9 @@ PArgs plan_args(lm_ctx *c, int cycle) {
     a.prismatic_mask = c->args.ch.prismatic_mask;
     a.pos_tol = p.prm.pos_tol; a.rot_tol = p.prm.rot_tol; a.mjac_rev = p.prm.mjac_rev; a.mjac_pris = p.prm.mjac_pris;
     a.cycle = cycle;
+    a.min_clearance = p.prm.min_clearance;
+    a.use_clear = (c->traj.args.caps.npairs + c->traj.args.caps.nenv) > 0 ? 1 : 0;
+    a.clear = p.clear;
     a.q = c->args.q; a.perr = c->args.perr; a.rerr = c->args.rerr;
     a.q_valid = p.q_valid; a.cur = p.cur; a.len_valid = p.len_valid;
     a.gate = p.gate; a.first = p.first; a.records = p.records; a.valid = p.valid;
@@ -146,6 +153,7 @@ int lm_plan_default_params(lm_plan_params *out) {
     out->mjac_rev = (float)(7.0 * deg);
     out->mjac_pris = 0.02f;
     out->pose_iters = 10;
+    out->min_clearance = 0.f;
     return LM_OK;
 }
 
@@ -163,6 +171,7 @@ int lm_plan_attach(lm_ctx *c, const lm_plan_params *p, void *workspace, size_t b
     s.ws = static_cast<char *>(workspace);
     s.q_valid = reinterpret_cast<float *>(s.ws + L.q_valid);
     s.cur = reinterpret_cast<float *>(s.ws + L.cur);
+    s.clear = reinterpret_cast<float *>(s.ws + L.clear);
     s.len_valid = reinterpret_cast<float *>(s.ws + L.len_valid);
     s.gate = reinterpret_cast<int32_t *>(s.ws + L.gate);
     s.first = reinterpret_cast<int32_t *>(s.ws + L.first);
@@ -192,7 +201,11 @@ int lm_plan_run(lm_ctx *c, int32_t cycles) {
         if (rc != LM_OK) return rc;
         rc = run_pose_phase(c, c->plan.prm.pose_iters);
         if (rc != LM_OK) return rc;
-        // validity, measurements, latest valid solution (P3)
+        // validity, measurements, latest valid solution (P3); with capsules set, the smallest clearance per waypoint first
+        if ((c->traj.args.caps.npairs + c->traj.args.caps.nenv) > 0) {
+            rc = launch_clearance(c, c->plan.clear);
+            if (rc != LM_OK) return rc;
+        }
         launch_counter().fetch_add(1);
         plan_check_kernel<<<(unsigned)c->B, PLAN_THREADS, 0, c->stream>>>(plan_args(c, cyc));
         LM_CUDA(cudaGetLastError());
@@ -225,6 +238,7 @@ int lm_plan_fetch(lm_ctx *c, float *q_valid_out, lm_plan_stats *s) {
         LM_CUDA(out(s->mjac_rev, p.cur + 2 * B, 4 * B));
         LM_CUDA(out(s->mjac_pris, p.cur + 3 * B, 4 * B));
         LM_CUDA(out(s->cur_length, p.cur + 4 * B, 4 * B));
+        LM_CUDA(out(s->min_clearance, p.cur + 5 * B, 4 * B));
         LM_CUDA(cudaMemsetAsync(p.total, 0, 16, c->stream));
         launch_counter().fetch_add(1);
         plan_count_kernel<<<(unsigned)((B + 255) / 256), 256, 0, c->stream>>>(p.valid, c->B, p.total);

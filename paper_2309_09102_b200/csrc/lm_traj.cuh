@@ -57,6 +57,7 @@ struct TArgs {
     const float *src_q;            // pack: [D][W] w-order
     const float *src_tp, *src_tq;  // pack: [3][W], [4][W] w-order
     float *dst_q;                  // unpack: [D][W] w-order
+    float *clear_out;              // tl_clearance_kernel: [W] w-order, smallest capsule clearance of the waypoint
 };
 
 template <int D> struct Tri { static constexpr int NA = D * (D + 1) / 2; };
@@ -190,6 +191,28 @@ __device__ __forceinline__ void tl_eval_waypoint(const TArgs &A, const float (&q
     } else {
         eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
     }
+}
+
+// ---- smallest clearance over all listed capsule pairs at the joint values src_q (w-order): thread per waypoint.
+//      Used by lm_plan_run: a valid trajectory is collision free.
+template <int D, typename SpecT>
+__global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_clearance_kernel(const __grid_constant__ TArgs A) {
+    const int64_t W = A.B * A.n;
+    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (w >= W) return;
+    float q[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) q[j] = A.src_q[(int64_t)j * W + w];
+    const float pt[3] = {0.f, 0.f, 0.f};
+    const float Rt[3][3] = {{1.f, 0.f, 0.f}, {0.f, 1.f, 0.f}, {0.f, 0.f, 1.f}};
+    Pose<D> Fr;
+    CapsWorld Wc;
+    CapsSink sink(A.caps, Wc);
+    sink.base();
+    eval_pose<D, false, false, SpecT, false, CapsSink>(A.ch, q, pt, Rt, 1.f, 1.f, Fr, nullptr, nullptr, nullptr, sink);
+    float mc = 3.0e38f;
+    coll_rows<D, SpecT, true>(A.ch, A.caps, Wc, Fr, [](const float (&)[D], float) {}, &mc);
+    A.clear_out[w] = mc;
 }
 
 // ---- assemble at the current point (entry of lm_traj_run): thread per waypoint

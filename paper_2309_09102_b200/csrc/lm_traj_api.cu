@@ -49,7 +49,8 @@ TLayout make_tlayout(int d, int64_t B, int64_t n) {
 
 cudaError_t launch_pose(lm_ctx *c, int which, const TArgs &a) {
     launch_counter().fetch_add(1);
-    const unsigned block = 128, grid = (unsigned)((a.nS + block - 1) / block);
+    const unsigned block = 128;
+    const unsigned grid = (unsigned)(((which == TK_CLEARANCE ? a.B * a.n : a.nS) + block - 1) / block);
     const bool weighted = c->args.weighted != 0;
     if (c->spec_id != SPEC_GENERIC && !c->use_generic)
         return launch_traj_pose_spec(which, c->spec_id, weighted, grid, block, c->stream, a);
@@ -82,6 +83,16 @@ bool is_host_ptr(const void *p) {
 }
 
 } // namespace
+
+namespace lmk {
+int launch_clearance(lm_ctx *c, float *clear_out) { // smallest capsule clearance per waypoint at the context's current q
+    TArgs a = c->traj.args;
+    a.src_q = c->args.q;
+    a.clear_out = clear_out;
+    LM_CUDA(launch_pose(c, TK_CLEARANCE, a));
+    return LM_OK;
+}
+} // namespace lmk
 
 extern "C" {
 

@@ -6,7 +6,7 @@
 
 namespace lmk {
 
-enum TrajPoseKernel : int { TK_ASSEMBLE = 0, TK_RHO = 1, TK_TRIAL = 2 };
+enum TrajPoseKernel : int { TK_ASSEMBLE = 0, TK_RHO = 1, TK_TRIAL = 2, TK_CLEARANCE = 3 };
 enum TrajPlainKernel : int { TK_PACK_Q = 0, TK_PACK_TARGETS = 1, TK_UNPACK = 2, TK_SOLVE_FACTOR = 3, TK_SOLVE_REFINE = 4 };
 
 // kernels that evaluate FK (chain-structure specialised or generic), thread per waypoint
@@ -30,6 +30,7 @@ cudaError_t launch_traj_pose_t(int which, bool weighted, unsigned grid, unsigned
     case TK_ASSEMBLE: LM_TL_LAUNCH(tl_assemble_kernel); break;
     case TK_RHO: LM_TL_LAUNCH(tl_rho_kernel); break;
     case TK_TRIAL: LM_TL_LAUNCH(tl_trial_kernel); break;
+    case TK_CLEARANCE: tl_clearance_kernel<D, SpecT><<<grid, block, 0, s>>>(a); break;
     default: return cudaErrorInvalidValue;
     }
 #undef LM_TL_LAUNCH

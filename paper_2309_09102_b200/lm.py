@@ -89,14 +89,14 @@ class LmObstacles(C.Structure):
 
 class LmPlanParams(C.Structure):
     _fields_ = [("pos_tol", C.c_float), ("rot_tol", C.c_float), ("mjac_rev", C.c_float), ("mjac_pris", C.c_float),
-                ("pose_iters", C.c_int32)]
+                ("pose_iters", C.c_int32), ("min_clearance", C.c_float)]
 
 
 class LmPlanStats(C.Structure):
     _fields_ = [("valid", C.c_void_p), ("first_valid_cycle", C.c_void_p), ("records", C.c_void_p),
                 ("length", C.c_void_p), ("max_pos_err", C.c_void_p), ("max_rot_err", C.c_void_p),
                 ("mjac_rev", C.c_void_p), ("mjac_pris", C.c_void_p), ("cur_length", C.c_void_p),
-                ("valid_trajectories", C.c_int64)]
+                ("min_clearance", C.c_void_p), ("valid_trajectories", C.c_int64)]
 
 
 class LmError(RuntimeError):
@@ -560,9 +560,10 @@ class Solver:
         qv = torch.empty((self.d, self.W), dtype=torch.float32).pin_memory()
         out = {"valid": buf(torch.uint8), "first_valid_cycle": buf(torch.int32), "records": buf(torch.int32),
                "length": buf(torch.float32), "max_pos_err": buf(torch.float32), "max_rot_err": buf(torch.float32),
-               "mjac_rev": buf(torch.float32), "mjac_pris": buf(torch.float32), "cur_length": buf(torch.float32)}
+               "mjac_rev": buf(torch.float32), "mjac_pris": buf(torch.float32), "cur_length": buf(torch.float32),
+               "min_clearance": buf(torch.float32)}
         st = LmPlanStats(*[out[k].data_ptr() for k in ("valid", "first_valid_cycle", "records", "length", "max_pos_err",
-                                                       "max_rot_err", "mjac_rev", "mjac_pris", "cur_length")], 0)
+                                                       "max_rot_err", "mjac_rev", "mjac_pris", "cur_length", "min_clearance")], 0)
         lm_plan_fetch(self._ctx, qv.data_ptr(), st)
         res = {k: v.numpy().copy() for k, v in out.items()}
         res["valid"] = res["valid"].astype(bool)

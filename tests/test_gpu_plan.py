@@ -119,3 +119,35 @@ def test_plan_is_repeatable_and_argument_errors():
     s.close()
     for k in ("q_valid", "length", "valid", "records", "mjac_rev"):
         assert np.array_equal(outs[0][k], outs[1][k], equal_nan=True), k
+
+
+def test_schedule_with_capsules_requires_collision_free_trajectories():
+    """validity includes "no collision"; with lm_traj_set_capsules the schedule checks the smallest
+    capsule clearance of every waypoint and the trajectory-level step carries the collision rows."""
+    from paper_2309_09102_b200 import lm
+    from oracle import lm_coll_oracle as corc
+    ch, model, scene = wl.panda_chain(), wl.panda_capsules(), wl.panda_scene()
+    B, n = 6, 60
+    rng = np.random.default_rng(44)
+    base = np.array([[0.0, 0.2, 0.0, -1.8, 0.0, 2.0, 0.8]] * 3 + [[0.0, 1.2, 0.0, -2.9, 0.0, 2.2, 0.8]] * 3)
+    truth = np.clip(base[:, None, :] + np.cumsum(0.004 * rng.normal(size=(B, n, 7)), axis=1), ch.q_lo, ch.q_hi)
+    w = wl._from_truth("PC", ch, truth, 0.002, rng, lambda q: orc.fk(ch, q), 1e-5, 10)
+    s = lm.Solver(ch, B, n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=1e-5))
+    s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=0.1))
+    s.traj_set_capsules(model, 1.0, 0.02)
+    s.traj_set_obstacles(scene, 1.0, 0.02)
+    s.plan_attach(lm.lm_plan_default_params(pose_iters=8))
+    s.plan_run(1)
+    g = s.plan_fetch()
+    s.close()
+    caps = corc.Capsules(model, w_coll=1.0, d_safe=0.02, scene=scene, w_env=1.0, d_safe_env=0.02)
+    o = porc.plan(ch, orc.Params(tol=1e-5), torc.TrajParams(w_pose=1.0, w_diff=0.1, caps=caps), porc.PlanParams(pose_iters=8),
+                  w.target_pos.astype(np.float64).reshape(B, n, 3), w.target_quat.astype(np.float64).reshape(B, n, 4),
+                  w.seeds.astype(np.float64).reshape(B, n, 7), 1)
+    clr_o = o.history[-1]["clearance"]
+    assert np.allclose(g["min_clearance"], clr_o, atol=2e-4)
+    decisive = np.abs(clr_o) > 1e-3
+    assert np.array_equal(g["valid"][decisive], o.valid[decisive])
+    assert o.valid[:3].any() and not o.valid[3:].any()            # the folded trajectories go through the base column
+    v = o.valid & decisive
+    assert np.abs(g["q_valid"].reshape(B, n, 7)[v] - o.q_valid[v]).max() <= 1e-4

@@ -93,3 +93,27 @@ def test_discontinuity_and_unreachable_targets_are_not_valid_and_gate_the_trajec
     assert res.max_pos_err[2] > 1.0
     assert np.isnan(res.q_valid[1]).all() and np.isnan(res.length[2])
     assert res.traj_iters[0] == 2 and res.traj_iters[1] == 2 and res.traj_iters[2] == 0   # only pose-valid ones step (P2)
+
+
+def test_collision_free_is_part_of_validity():
+    """PAPER.md:L49: "At no timestep in the trajectory can the robot collide with itself or the environment"."""
+    from oracle import lm_coll_oracle as corc
+    ch, model = wl.panda_chain(), wl.panda_capsules()
+    B, n = 2, 60
+    rng = np.random.default_rng(35)
+    base = np.array([[0.0, 0.2, 0.0, -1.8, 0.0, 2.0, 0.8], [0.0, 1.2, 0.0, -2.9, 0.0, 2.2, 0.8]])   # open arm / folded through the base
+    truth = np.clip(base[:, None, :] + np.cumsum(0.004 * rng.normal(size=(B, n, 7)), axis=1), ch.q_lo, ch.q_hi)
+    p, R = orc.fk(ch, truth.reshape(-1, 7))
+    tp, tq = p.reshape(B, n, 3), wl._R_to_quat_wxyz(R).reshape(B, n, 4)
+    caps = corc.Capsules(model, w_coll=1.0, d_safe=0.02)
+    clr = porc.min_clearance(ch, caps, truth)
+    assert clr[0] > 0.02 and clr[1] < 0                                   # the second one penetrates
+    # brute check of min_clearance against the per-waypoint distances
+    assert np.isclose(clr[1], min(corc.residual(ch, caps, truth[1, i])[0].min() for i in range(n)))
+    res = porc.plan(ch, orc.Params(tol=1e-6), torc.TrajParams(w_pose=1.0, w_diff=0.1, caps=caps),
+                    porc.PlanParams(pose_iters=8), tp, tq, truth, 0)
+    assert res.valid[0] and not res.valid[1]
+    assert res.max_pos_err[1] < 1e-4 and res.mjac_rev[1] < 7 * DEG       # pose-valid and smooth: only the collision fails it
+    # without a capsule model both are valid
+    res0 = porc.plan(ch, orc.Params(tol=1e-6), torc.TrajParams(w_pose=1.0, w_diff=0.1), porc.PlanParams(pose_iters=8), tp, tq, truth, 0)
+    assert res0.valid.all()
