@@ -243,3 +243,60 @@ def test_rpy_residual_variant_matches_the_oracle(lm):
     with pytest.raises(lm.LmError):
         s.traj_attach()
     s.close()
+
+
+# ------------------------------------------------------------------ full sizes of the bench, sampled outputs
+
+def test_config4_full_size_sampled(lm):
+    """configs[3] at FULL size (4096 x 300) in the launch configuration bench.py times (one lm_run(50) launch,
+    128-thread blocks); every 128th trajectory (32 trajectories, 9600 waypoints) is checked against the oracle --
+    waypoints are independent and a waypoint's bits do not depend on the batch (test_gpu_edge), so
+    the oracle only has to run the sample."""
+    w = wl.config4(H.oracle_fk(wl.panda_chain()))
+    assert (w.B, w.n) == (4096, 300)
+    g = H.run_gpu(w)
+    assert g["total_waypoint_iters"] == w.W * 50 and np.all(g["iters"] == 50)
+    assert np.all(np.isfinite(g["q"])) and np.all(g["q"] >= w.chain.q_lo.astype(np.float32)) and np.all(g["q"] <= w.chain.q_hi.astype(np.float32))
+    pick = np.arange(0, w.B, 128)
+    idx = (pick[:, None] * w.n + np.arange(w.n)[None, :]).ravel()
+    sub = wl.Workload(w.name, w.chain, len(pick), w.n, w.target_pos[idx], w.target_quat[idx], w.seeds[idx], w.tol, w.max_iters)
+    o = H.run_oracle(sub)
+    tr = H.oracle_trace(sub, 50)
+    Fb = np.stack([a.F_before for _, a in tr], 1)
+    Ft = np.stack([a.F_trial for _, a in tr], 1)
+    clear = np.all((np.abs(Fb - Ft) > 1e-3 * Fb) | (np.sqrt(Fb) < 1e-5), axis=1)
+    floor = np.sqrt(Fb) >= 1e-5
+    same = np.all((H.mask_bits(o.mask, 50) == H.mask_bits(g["mask"][idx], 50)) | ~floor, axis=1)
+    assert clear.mean() > 0.3 and same[clear].mean() > 0.995
+    dq = np.abs(g["q"][idx] - o.q).max(axis=1)
+    assert np.percentile(dq[clear & same], 99.5) <= H.TOL_Q
+    assert abs((g["res_norm"][idx] < 1e-5).mean() - (o.res_norm < 1e-5).mean()) <= 0.01
+    # the errors the library reports are the ones its q really has (oracle FK of the GPU's q), sampled over the whole batch
+    rnd = np.random.default_rng(0).choice(w.W, 4000, replace=False)
+    s2 = wl.Workload(w.name, w.chain, 1, len(rnd), w.target_pos[rnd], w.target_quat[rnd], w.seeds[rnd], w.tol, w.max_iters)
+    pe, re = H.pose_errors_by_oracle(s2, g["q"][rnd])
+    assert np.abs(g["pos_err"][rnd] - pe).max() <= 5e-6 and np.abs(g["rot_err"][rnd] - re).max() <= 5e-6
+
+
+@pytest.mark.parametrize("B,n", [(1, 100), (7, 1000), (16384, 100)])
+def test_config5_sweep_points(lm, B, n):
+    """configs[4] (throughput sweep, fixed 20 iterations): the smallest, a long ragged and the largest-batch point;
+    the large one on a sample of trajectories."""
+    w = wl.config5(H.oracle_fk(wl.panda_chain()), B=min(B, 64), n=n) if B <= 64 else None
+    if w is not None:
+        g, o = H.run_gpu(w), H.run_oracle(w)
+        _check_free_running(w, g, o)
+        assert np.all(g["iters"] == 20)
+        return
+    # large batch: targets need one oracle FK per waypoint, so the batch is built by tiling 64 distinct trajectories
+    base = wl.config5(H.oracle_fk(wl.panda_chain()), B=64, n=n)
+    reps = B // 64
+    big = wl.Workload(base.name, base.chain, B, n, np.tile(base.target_pos, (reps, 1)), np.tile(base.target_quat, (reps, 1)),
+                      np.tile(base.seeds, (reps, 1)), base.tol, base.max_iters)
+    g, o = H.run_gpu(big), H.run_oracle(base)
+    assert g["total_waypoint_iters"] == big.W * 20
+    for r in (0, reps // 2, reps - 1):          # copies of the same trajectories anywhere in the batch: same bits, oracle parity
+        sl = slice(r * base.W, (r + 1) * base.W)
+        assert np.array_equal(g["q"][sl], g["q"][:base.W])
+        assert np.abs(g["q"][sl] - o.q).max() <= H.TOL_Q
+        assert np.array_equal(g["iters"][sl], o.iters)
