@@ -514,7 +514,12 @@ int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *
     if (chunks > MAX_CHUNKS) return LM_EINVAL;
     // streams and the pinned totals buffer are created once per process and device and kept (creating
     // them costs more than a whole step); calls are serialised by the mutex
-    struct Pipe { int dev = -1; cudaStream_t st[NS] = {nullptr, nullptr, nullptr}; unsigned long long *totals = nullptr; };
+    struct Pipe {
+        int dev = -1;
+        cudaStream_t st[NS] = {nullptr, nullptr, nullptr}; // host->device copies, kernels, device->host copies
+        cudaEvent_t ev_in[MAX_CHUNKS] = {}, ev_done[MAX_CHUNKS] = {};
+        unsigned long long *totals = nullptr;
+    };
     static Pipe pipe;
     static std::mutex pipe_mutex;
     std::lock_guard<std::mutex> lock(pipe_mutex);
@@ -527,83 +532,115 @@ int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *
             if (pipe.st[i]) cudaStreamDestroy(pipe.st[i]);
             LM_CUDA(cudaStreamCreateWithFlags(&pipe.st[i], cudaStreamNonBlocking));
         }
+        for (int i = 0; i < MAX_CHUNKS; ++i) {
+            if (pipe.ev_in[i]) cudaEventDestroy(pipe.ev_in[i]);
+            if (pipe.ev_done[i]) cudaEventDestroy(pipe.ev_done[i]);
+            LM_CUDA(cudaEventCreateWithFlags(&pipe.ev_in[i], cudaEventDisableTiming));
+            LM_CUDA(cudaEventCreateWithFlags(&pipe.ev_done[i], cudaEventDisableTiming));
+        }
         if (!pipe.totals) LM_CUDA(cudaMallocHost(reinterpret_cast<void **>(&pipe.totals), 16 * (size_t)MAX_CHUNKS));
         pipe.dev = dev;
     }
-    cudaStream_t *streams = pipe.st;
+    cudaStream_t s_in = pipe.st[0], s_k = pipe.st[1], s_out = pipe.st[2];
     unsigned long long *totals = pipe.totals;
     lm_ctx **ctxs = new (std::nothrow) lm_ctx *[chunks]();
     if (!ctxs) return LM_ENOMEM;
-    char *ws = static_cast<char *>(pb->workspace);
+    struct Chunk { int64_t b0, Bc; size_t w0, Wc; Layout lay; char *ws; };
+    Chunk *ck = new (std::nothrow) Chunk[chunks];
+    if (!ck) { delete[] ctxs; return LM_ENOMEM; }
+    {
+        char *ws = static_cast<char *>(pb->workspace);
+        for (int k = 0; k < chunks; ++k) {
+            int64_t b0, b1;
+            chunk_range(pb->B, chunks, k, b0, b1);
+            ck[k].b0 = b0; ck[k].Bc = b1 - b0;
+            ck[k].w0 = (size_t)b0 * (size_t)pb->n; ck[k].Wc = (size_t)(b1 - b0) * (size_t)pb->n;
+            ck[k].lay = make_layout(d, b1 - b0, pb->n, 0, LM_MEM_HOST);
+            ck[k].ws = ws;
+            ws += ck[k].lay.total;
+        }
+    }
+    // stage 1 (copy stream): every chunk's inputs, in order; rows of the SoA arrays are W apart on the host,
+    // Wc apart in the chunk's staging area
     for (int k = 0; k < chunks && rc == LM_OK; ++k) {
-        int64_t b0, b1;
-        chunk_range(pb->B, chunks, k, b0, b1);
-        const int64_t Bc = b1 - b0;
-        const size_t Wc = (size_t)Bc * (size_t)pb->n, w0 = (size_t)b0 * (size_t)pb->n;
-        const Layout lay = make_layout(d, Bc, pb->n, 0, LM_MEM_HOST);
-        cudaStream_t s = streams[k % NS];
-        float *sd = reinterpret_cast<float *>(ws + lay.s_seeds), *tpd = reinterpret_cast<float *>(ws + lay.s_tp),
-              *tqd = reinterpret_cast<float *>(ws + lay.s_tq);
-        // rows of the SoA arrays are W apart on the host, Wc apart in the chunk's staging area
-        cudaError_t e = cudaMemcpy2DAsync(sd, 4 * Wc, pb->seeds + w0, 4 * W, 4 * Wc, d, cudaMemcpyHostToDevice, s);
-        if (e == cudaSuccess) e = cudaMemcpy2DAsync(tpd, 4 * Wc, pb->target_pos + w0, 4 * W, 4 * Wc, 3, cudaMemcpyHostToDevice, s);
-        if (e == cudaSuccess) e = cudaMemcpy2DAsync(tqd, 4 * Wc, pb->target_quat + w0, 4 * W, 4 * Wc, 4, cudaMemcpyHostToDevice, s);
+        const Chunk &c = ck[k];
+        float *sd = reinterpret_cast<float *>(c.ws + c.lay.s_seeds), *tpd = reinterpret_cast<float *>(c.ws + c.lay.s_tp),
+              *tqd = reinterpret_cast<float *>(c.ws + c.lay.s_tq);
+        cudaError_t e = cudaMemcpy2DAsync(sd, 4 * c.Wc, pb->seeds + c.w0, 4 * W, 4 * c.Wc, d, cudaMemcpyHostToDevice, s_in);
+        if (e == cudaSuccess) e = cudaMemcpy2DAsync(tpd, 4 * c.Wc, pb->target_pos + c.w0, 4 * W, 4 * c.Wc, 3, cudaMemcpyHostToDevice, s_in);
+        if (e == cudaSuccess) e = cudaMemcpy2DAsync(tqd, 4 * c.Wc, pb->target_quat + c.w0, 4 * W, 4 * c.Wc, 4, cudaMemcpyHostToDevice, s_in);
+        if (e == cudaSuccess) e = cudaEventRecord(pipe.ev_in[k], s_in);
+        if (e != cudaSuccess) fail(e);
+    }
+    // stage 2 (kernel stream): the LM kernel of chunk k as soon as its inputs have arrived, then its statistics
+    for (int k = 0; k < chunks && rc == LM_OK; ++k) {
+        const Chunk &c = ck[k];
+        cudaError_t e = cudaStreamWaitEvent(s_k, pipe.ev_in[k], 0);
         if (e != cudaSuccess) { fail(e); break; }
         lm_problem pk = *pb;
-        pk.B = Bc; pk.target_pos = tpd; pk.target_quat = tqd; pk.seeds = sd; pk.memory = LM_MEM_DEVICE;
-        pk.workspace = ws; pk.workspace_bytes = lay.total;
-        rc = lm_init(&ctxs[k], chain, &pk, prm, s);
+        pk.B = c.Bc;
+        pk.seeds = reinterpret_cast<float *>(c.ws + c.lay.s_seeds);
+        pk.target_pos = reinterpret_cast<float *>(c.ws + c.lay.s_tp);
+        pk.target_quat = reinterpret_cast<float *>(c.ws + c.lay.s_tq);
+        pk.memory = LM_MEM_DEVICE;
+        pk.workspace = c.ws; pk.workspace_bytes = c.lay.total;
+        rc = lm_init(&ctxs[k], chain, &pk, prm, s_k);
         if (rc != LM_OK) break;
-        lm_ctx *c = ctxs[k];
-        rc = iterate(c, max_iters, INT_MAX);
+        rc = iterate(ctxs[k], max_iters, INT_MAX);
         if (rc != LM_OK) break;
-        const KArgs &a = c->args;
+        const KArgs &a = ctxs[k]->args;
+        unsigned long long *tot = reinterpret_cast<unsigned long long *>(c.ws + c.lay.totals);
+        e = cudaMemsetAsync(tot, 0, 16, s_k);
+        if (e != cudaSuccess) { fail(e); break; }
+        g_launches.fetch_add(1);
+        lm_traj_stats_kernel<<<(unsigned)((c.Bc * 32 + 255) / 256), 256, 0, s_k>>>(
+            a.its, c.Bc, (int32_t)pb->n, reinterpret_cast<uint8_t *>(c.ws + c.lay.conv), reinterpret_cast<int32_t *>(c.ws + c.lay.titers), tot);
+        if (st && (st->iters || st->status)) {
+            g_launches.fetch_add(1);
+            lm_unpack_kernel<<<(unsigned)((c.Wc + 255) / 256), 256, 0, s_k>>>(
+                a.its, (int64_t)c.Wc, st->iters ? reinterpret_cast<int32_t *>(c.ws + c.lay.ui) : nullptr,
+                st->status ? reinterpret_cast<uint32_t *>(c.ws + c.lay.us) : nullptr);
+        }
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaEventRecord(pipe.ev_done[k], s_k);
+        if (e != cudaSuccess) fail(e);
+    }
+    // stage 3 (copy-back stream): the outputs of chunk k as soon as its kernels are done
+    for (int k = 0; k < chunks && rc == LM_OK; ++k) {
+        const Chunk &c = ck[k];
+        const KArgs &a = ctxs[k]->args;
+        cudaError_t e = cudaStreamWaitEvent(s_out, pipe.ev_done[k], 0);
+        if (e != cudaSuccess) { fail(e); break; }
         auto out1 = [&](void *dst, const void *src, size_t elem, size_t off, size_t count) {
             if (dst && rc == LM_OK) {
-                cudaError_t e2 = cudaMemcpyAsync(static_cast<char *>(dst) + elem * off, src, elem * count, cudaMemcpyDeviceToHost, s);
+                cudaError_t e2 = cudaMemcpyAsync(static_cast<char *>(dst) + elem * off, src, elem * count, cudaMemcpyDeviceToHost, s_out);
                 if (e2 != cudaSuccess) fail(e2);
             }
         };
         if (q_out) {
-            e = cudaMemcpy2DAsync(q_out + w0, 4 * W, a.q, 4 * Wc, 4 * Wc, d, cudaMemcpyDeviceToHost, s);
+            e = cudaMemcpy2DAsync(q_out + c.w0, 4 * W, a.q, 4 * c.Wc, 4 * c.Wc, d, cudaMemcpyDeviceToHost, s_out);
             if (e != cudaSuccess) { fail(e); break; }
         }
-        unsigned long long *tot = reinterpret_cast<unsigned long long *>(ws + lay.totals);
-        e = cudaMemsetAsync(tot, 0, 16, s);
-        if (e != cudaSuccess) { fail(e); break; }
-        uint8_t *conv = reinterpret_cast<uint8_t *>(ws + lay.conv);
-        int32_t *tit = reinterpret_cast<int32_t *>(ws + lay.titers);
-        g_launches.fetch_add(1);
-        lm_traj_stats_kernel<<<(unsigned)((Bc * 32 + 255) / 256), 256, 0, s>>>(a.its, Bc, (int32_t)pb->n, conv, tit, tot);
         if (st) {
-            out1(st->res_norm, a.res, 4, w0, Wc);
-            out1(st->pos_err, a.perr, 4, w0, Wc);
-            out1(st->rot_err, a.rerr, 4, w0, Wc);
-            out1(st->lambda, a.lam, 4, w0, Wc);
-            out1(st->accept_mask, a.mask, 8, w0, Wc);
-            out1(st->traj_converged, conv, 1, (size_t)b0, (size_t)Bc);
-            out1(st->traj_iters, tit, 4, (size_t)b0, (size_t)Bc);
-            if (st->iters || st->status) {
-                int32_t *ui = reinterpret_cast<int32_t *>(ws + lay.ui);
-                uint32_t *us = reinterpret_cast<uint32_t *>(ws + lay.us);
-                g_launches.fetch_add(1);
-                lm_unpack_kernel<<<(unsigned)((Wc + 255) / 256), 256, 0, s>>>(a.its, (int64_t)Wc, st->iters ? ui : nullptr, st->status ? us : nullptr);
-                out1(st->iters, ui, 4, w0, Wc);
-                out1(st->status, us, 4, w0, Wc);
-            }
+            out1(st->res_norm, a.res, 4, c.w0, c.Wc);
+            out1(st->pos_err, a.perr, 4, c.w0, c.Wc);
+            out1(st->rot_err, a.rerr, 4, c.w0, c.Wc);
+            out1(st->lambda, a.lam, 4, c.w0, c.Wc);
+            out1(st->accept_mask, a.mask, 8, c.w0, c.Wc);
+            out1(st->traj_converged, c.ws + c.lay.conv, 1, (size_t)c.b0, (size_t)c.Bc);
+            out1(st->traj_iters, c.ws + c.lay.titers, 4, (size_t)c.b0, (size_t)c.Bc);
+            out1(st->iters, c.ws + c.lay.ui, 4, c.w0, c.Wc);
+            out1(st->status, c.ws + c.lay.us, 4, c.w0, c.Wc);
         }
         if (rc == LM_OK) {
-            e = cudaMemcpyAsync(totals + 2 * k, tot, 16, cudaMemcpyDeviceToHost, s);
-            if (e == cudaSuccess) e = cudaGetLastError();
+            e = cudaMemcpyAsync(totals + 2 * k, c.ws + c.lay.totals, 16, cudaMemcpyDeviceToHost, s_out);
             if (e != cudaSuccess) fail(e);
         }
-        ws += lay.total;
     }
-    for (int i = 0; i < NS; ++i)
-        if (streams[i]) {
-            cudaError_t e = cudaStreamSynchronize(streams[i]);
-            if (e != cudaSuccess && rc == LM_OK) fail(e);
-        }
+    for (int i = 0; i < NS; ++i) {
+        cudaError_t e = cudaStreamSynchronize(pipe.st[i]);
+        if (e != cudaSuccess && rc == LM_OK) fail(e);
+    }
     if (st && rc == LM_OK) {
         st->total_waypoint_iters = 0;
         st->converged_trajectories = 0;
@@ -612,6 +649,7 @@ int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *
             st->converged_trajectories += (int64_t)totals[2 * k + 1];
         }
     }
+    delete[] ck;
     for (int k = 0; k < chunks; ++k) delete ctxs[k];
     delete[] ctxs;
     return rc;
