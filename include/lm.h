@@ -144,7 +144,7 @@ int lm_fetch(lm_ctx *ctx, float *q_out, lm_stats *stats_out);
 
 /* One call for HOST data (the end-to-end path): refine all B*n waypoints from host arrays (pinned memory makes
  * the copies asynchronous) and write the results to host arrays.  The batch is split into `chunks` groups of
- * whole trajectories that are pipelined over three internal streams (copies in, kernels, copies out), so that the host->device copy of chunk k+1,
+ * whole trajectories that are pipelined over internal streams (copies in, kernels, copies out), so that the host->device copy of chunk k+1,
  * the LM kernel of chunk k and the device->host copy of chunk k-1 overlap (waypoints are independent:
  * PAPER.md:L121, so the result does not depend on `chunks`).  problem->memory must be LM_MEM_HOST,
  * shared_targets 0, problem->workspace DEVICE scratch of >= lm_solve_host_workspace_bytes().  q_out [d][B*n]

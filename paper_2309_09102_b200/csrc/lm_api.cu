@@ -510,13 +510,13 @@ int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *
     if (d < 1 || d > LM_MAX_DOF) return LM_EINVAL;
     if (pb->workspace_bytes < lm_solve_host_workspace_bytes(d, pb->B, pb->n, chunks)) return LM_ENOMEM;
     const size_t W = (size_t)pb->B * (size_t)pb->n;
-    constexpr int NS = 3, MAX_CHUNKS = 256;
+    constexpr int NS = 4, MAX_CHUNKS = 256;
     if (chunks > MAX_CHUNKS) return LM_EINVAL;
     // streams and the pinned totals buffer are created once per process and device and kept (creating
     // them costs more than a whole step); calls are serialised by the mutex
     struct Pipe {
         int dev = -1;
-        cudaStream_t st[NS] = {nullptr, nullptr, nullptr}; // host->device copies, kernels, device->host copies
+        cudaStream_t st[NS] = {nullptr, nullptr, nullptr, nullptr}; // host->device copies, device->host copies, 2 x kernels
         cudaEvent_t ev_in[MAX_CHUNKS] = {}, ev_done[MAX_CHUNKS] = {};
         unsigned long long *totals = nullptr;
     };
@@ -541,7 +541,9 @@ int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *
         if (!pipe.totals) LM_CUDA(cudaMallocHost(reinterpret_cast<void **>(&pipe.totals), 16 * (size_t)MAX_CHUNKS));
         pipe.dev = dev;
     }
-    cudaStream_t s_in = pipe.st[0], s_k = pipe.st[1], s_out = pipe.st[2];
+    cudaStream_t s_in = pipe.st[0], s_out = pipe.st[1];
+    cudaStream_t s_kk[2] = {pipe.st[2], pipe.st[3]}; // chunks alternate between two kernel streams: the tail of one
+                                                     // chunk's last wave overlaps the head of the next chunk's kernel
     unsigned long long *totals = pipe.totals;
     lm_ctx **ctxs = new (std::nothrow) lm_ctx *[chunks]();
     if (!ctxs) return LM_ENOMEM;
@@ -575,6 +577,7 @@ int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *
     // stage 2 (kernel stream): the LM kernel of chunk k as soon as its inputs have arrived, then its statistics
     for (int k = 0; k < chunks && rc == LM_OK; ++k) {
         const Chunk &c = ck[k];
+        cudaStream_t s_k = s_kk[k & 1];
         cudaError_t e = cudaStreamWaitEvent(s_k, pipe.ev_in[k], 0);
         if (e != cudaSuccess) { fail(e); break; }
         lm_problem pk = *pb;
