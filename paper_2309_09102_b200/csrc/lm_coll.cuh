@@ -25,6 +25,7 @@ struct KCaps {
     float w_coll, d_safe;
     int8_t link[MAX_CAPS];          // -1 = base frame, j = frame moved by joint j
     float a[MAX_CAPS][3], b[MAX_CAPS][3], c[MAX_CAPS];
+    float hl[MAX_CAPS];             // half length |b - a| / 2 (bounding sphere of the axis, for culling)
     uint8_t pair[MAX_PAIRS][2];
     // robot-environment rows: cuboids given by their frame in the world (Ro row-major, box axes
     // as columns; origin to) and extents pmin / pmax in that frame; env_pair = (capsule, obstacle)
@@ -32,6 +33,7 @@ struct KCaps {
     float w_env, d_safe_env;
     float Ro[MAX_OBS][9], to[MAX_OBS][3], pmin[MAX_OBS][3], pmax[MAX_OBS][3];
     uint8_t env_pair[MAX_PAIRS][2];
+    float oc[MAX_OBS][3], orad[MAX_OBS]; // bounding sphere of every cuboid in the world frame (for culling)
 };
 
 // world endpoints of the capsules: filled link by link while FK runs
@@ -161,6 +163,20 @@ __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, cons
         float ab[3], bb[3], wa[3], wb[3], pmin[3], pmax[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) { wa[i] = W.wa[k][i]; wb[i] = W.wb[k][i]; pmin[i] = C.pmin[ob][i]; pmax[i] = C.pmax[ob][i]; }
+        if (!CLEAR_ONLY) { // distance of the axis MIDPOINT to the box minus the half length bounds the clearance from below:
+                           // far pairs have no row
+            float mw[3], e2 = 0.f;
+#pragma unroll
+            for (int i = 0; i < 3; ++i) mw[i] = sub(mul(0.5f, add(wa[i], wb[i])), C.to[ob][i]);
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                const float x = fma_(C.Ro[ob][6 + i], mw[2], fma_(C.Ro[ob][3 + i], mw[1], mul(C.Ro[ob][i], mw[0])));
+                const float ex = sub(x, fminf(fmaxf(x, pmin[i]), pmax[i]));
+                e2 = fma_(ex, ex, e2);
+            }
+            const float reach = add(add(C.hl[k], C.c[k]), add(C.d_safe_env, 1e-4f));
+            if (e2 > mul(reach, reach)) continue;
+        }
 #pragma unroll
         for (int i = 0; i < 3; ++i) { // x_box = Ro^T (x - to)
             float sa = 0.f, sb = 0.f;
@@ -215,6 +231,13 @@ __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, cons
         float a1[3], b1[3], a2[3], b2[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) { a1[i] = W.wa[k1][i]; b1[i] = W.wb[k1][i]; a2[i] = W.wa[k2][i]; b2[i] = W.wb[k2][i]; }
+        if (!CLEAR_ONLY) { // bounding spheres of the two axes: far pairs have no row
+            float cc[3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) cc[i] = mul(0.5f, sub(add(a1[i], b1[i]), add(a2[i], b2[i])));
+            const float reach = add(add(add(C.hl[k1], C.c[k1]), add(C.hl[k2], C.c[k2])), add(C.d_safe, 1e-4f));
+            if (dot3(cc, cc) > mul(reach, reach)) continue;
+        }
         float t1, t2;
         segment_closest(a1, b1, a2, b2, t1, t2);
         float p1[3], p2[3], e[3];

@@ -185,7 +185,12 @@ int lm_traj_set_capsules(lm_ctx *c, const lm_capsules *m) {
         if (m->link[i] < -1 || m->link[i] >= c->dof || !(m->radius[i] >= 0.f)) return LM_EINVAL;
         k.link[i] = (int8_t)m->link[i];
         k.c[i] = m->radius[i];
-        for (int x = 0; x < 3; ++x) { k.a[i][x] = m->a[3 * i + x]; k.b[i][x] = m->b[3 * i + x]; }
+        double l2 = 0.0;
+        for (int x = 0; x < 3; ++x) {
+            k.a[i][x] = m->a[3 * i + x]; k.b[i][x] = m->b[3 * i + x];
+            l2 += ((double)k.b[i][x] - k.a[i][x]) * ((double)k.b[i][x] - k.a[i][x]);
+        }
+        k.hl[i] = (float)(0.5 * std::sqrt(l2) * (1.0 + 1e-6)); // rounded up: the bounding sphere must contain the axis
     }
     for (int p = 0; p < m->npairs; ++p) {
         const int32_t k1 = m->pairs[2 * p], k2 = m->pairs[2 * p + 1];
@@ -219,6 +224,15 @@ int lm_traj_set_obstacles(lm_ctx *c, const lm_obstacles *o) {
             k.pmax[i][e] = o->pmax[3 * i + e];
             if (!(k.pmin[i][e] <= k.pmax[i][e])) return LM_EINVAL;
         }
+        double r2 = 0.0;
+        for (int e = 0; e < 3; ++e) { // bounding sphere: centre = to + R (pmin + pmax) / 2, radius = |pmax - pmin| / 2
+            const double mid[3] = {0.5 * ((double)k.pmin[i][0] + k.pmax[i][0]), 0.5 * ((double)k.pmin[i][1] + k.pmax[i][1]),
+                                   0.5 * ((double)k.pmin[i][2] + k.pmax[i][2])};
+            k.oc[i][e] = (float)(ps[e] + R[3 * e] * mid[0] + R[3 * e + 1] * mid[1] + R[3 * e + 2] * mid[2]);
+            const double h = 0.5 * ((double)k.pmax[i][e] - k.pmin[i][e]);
+            r2 += h * h;
+        }
+        k.orad[i] = (float)(std::sqrt(r2) * (1.0 + 1e-6));
     }
     for (int p = 0; p < o->npairs; ++p) {
         const int32_t kc = o->pairs[2 * p], ob = o->pairs[2 * p + 1];
