@@ -330,6 +330,8 @@ def run_gpu(args) -> None:
         extra["trajectory_step"] = time_traj_step(lm, torch, w, solver, stream, peaks)
         # the paper's alternating schedule with anytime bookkeeping (NEXT-2), valid trajectories per second
         extra["schedule_C2"] = time_plan(lm, torch, wl, fk, device, stream)
+        # the global discrete search over K candidates of one path (NEXT-4 iii)
+        extra["search_K175_n300"] = time_search(lm, torch, wl, fk, device, stream)
     roofline["peak_measured_fma_rrr"] = lm.lm_fp32_peak_form(lm.LM_FMA_FORM_RRR, int(stream.cuda_stream))
     roofline["frac_of_measured_fma_rrr"] = achieved_tf / roofline["peak_measured_fma_rrr"]
     if True:
@@ -482,6 +484,43 @@ def time_plan(lm, torch, wl, fk, device, stream, cycles: int = 3, reps: int = 5)
     s.close()
     out["workload"] = f"C2: {w.B} x {w.n}, tol={w.tol:g}, pose_iters=10, w_pose=1, w_diff=1"
     return out
+
+
+def time_search(lm, torch, wl, fk, device, stream, K: int = 175, n: int = 300, reps: int = 10) -> dict:
+    """lm_search on K synthetic candidate trajectories of one n-waypoint path (Panda): median
+    CUDA-event time of one call (edge costs + penalties, the layered dynamic program, backtracking, xi gather) after
+    3 warm-ups.  The CPU leg runs the oracle (oracle/lm_search_oracle.py, fp32 decisions) once on the same input."""
+    import time as _time
+    from oracle import lm_search_oracle as sorc
+    ch = wl.panda_chain()
+    q = wl.search_candidates(ch, K, n, 2, limit_frac=0.02)
+    tp = np.zeros((K * n, 3), np.float32)                      # the search reads joint values only
+    tq = np.tile(np.array([[1, 0, 0, 0]], np.float32), (K * n, 1))
+    s = lm.Solver(ch, K, n, tp, tq, q.reshape(K * n, ch.dof), device=str(device), stream=stream)
+    ts = []
+    with torch.cuda.stream(stream):
+        for i in range(reps + 3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = lm.lm_launch_count()
+            a.record(stream)
+            s.search(to_host=False)
+            b.record(stream)
+            stream.synchronize()
+            launches = lm.lm_launch_count() - l0
+            if i >= 3:
+                ts.append(a.elapsed_time(b))
+        g = s.search()
+    s.close()
+    pen = sorc.penalties(q, ch.q_lo.astype(np.float32), ch.q_hi.astype(np.float32), ch.joint_type,
+                         margin_rev=np.float32(np.deg2rad(1.5)), margin_pris=np.float32(0.03))
+    t0 = _time.perf_counter()
+    choice, xi, cost, mj = sorc.search(q, pen, dtype=np.float32)
+    cpu_s = _time.perf_counter() - t0
+    ms = float(np.median(ts))
+    return {"workload": f"{K} candidates x {n} waypoints, Panda, synthetic (workloads.search_candidates)", "ms": ms,
+            "gpu_launches": int(launches), "edges_per_sec": (n - 1) * K * K / (ms * 1e-3), "mjac_rad": g["mjac"],
+            "candidates_used": int(len(set(g["choice"].tolist()))), "same_choice_as_oracle": bool(np.array_equal(g["choice"], choice)),
+            "cpu_baseline": {"ms": cpu_s * 1e3, "kind": "oracle", "cores": 1, "sample": "the same input, once"}}
 
 
 def time_dual_variant(lm, torch, w, device, stream, peak_tf: float, reps: int = 10) -> dict:

@@ -337,6 +337,35 @@ int lm_plan_run(lm_ctx *ctx, int32_t cycles);
 /* Synchronise; q_valid_out [d][W] (device or host, nullable) = latest valid trajectories (NaN where none). */
 int lm_plan_fetch(lm_ctx *ctx, float *q_valid_out, lm_plan_stats *stats_out);
 
+/* ---- Global discrete search over the context's B = K candidate trajectories of ONE path ------------------
+ * (sec. III-B; SURVEY.md section 8f NEXT-4 iii.)  The K x n joint
+ * configurations are the nodes of a layered graph, every node of timestep i-1 is joined to every node of
+ * timestep i, and a dynamic program finds the path whose largest joint change across a timestep (mjac,
+ * PAPER.md:L95) is smallest:
+ *     c[0][k] = pen[0][k],   c[i][k] = pen[i][k] + min_k' max(c[i-1][k'], max_j |q[k][i][j] - q[k'][i-1][j]|)
+ * pen = pen_limit (paper: 10) where a joint is within margin_rev (1.5 deg) / margin_pris (3 cm) of a limit,
+ * plus pen_collision (paper: 100) where the smallest capsule clearance of the node is < 0 (use_clearance;
+ * needs lm_traj_attach + a capsule model).  Ties go to the lowest candidate; the path ends at
+ * argmin_k c[n-1][k] and is read back through the stored predecessors ("backtracking", L97).  All arithmetic
+ * is fp32, rounded to nearest, in the order written above. */
+#define LM_SEARCH_MAX_K 1024
+typedef struct {
+    float margin_rev, margin_pris; /* rad, m (1.5 deg / 3 cm) */
+    float pen_limit, pen_collision; /* 10, 100 */
+    int32_t use_clearance;          /* 1: add pen_collision from the capsule model set by lm_traj_set_capsules/obstacles */
+} lm_search_params;
+
+size_t lm_search_workspace_bytes(int32_t dof, int64_t K, int64_t n);
+int lm_search_default_params(lm_search_params *out);
+/* Runs the search on the context's CURRENT joint values (seeds if nothing has run), B = K <= LM_SEARCH_MAX_K.
+ * workspace: caller-owned device memory, 256-byte aligned, >= lm_search_workspace_bytes, used during the call only.
+ * Outputs (device or host, each nullable): choice_out [n] candidate index per timestep; xi_out [d][n] the
+ * selected configurations (xi_search); result_out [2] = { c[n-1][choice[n-1]], mjac of xi }.
+ * Synchronises the context's stream before returning.  LM_EINVAL: null / misaligned arguments, B > LM_SEARCH_MAX_K,
+ * use_clearance without a capsule model; LM_ENOMEM: workspace too small. */
+int lm_search(lm_ctx *ctx, const lm_search_params *params, void *workspace, size_t workspace_bytes,
+              int32_t *choice_out, float *xi_out, float *result_out);
+
 /* Measure the FP32 FMA throughput of the current device with an FMA-only micro-kernel (16 independent
  * chains per thread, best of 5 timed launches, CUDA events on `cuda_stream`); blocks the host.
  * tflops_out: 2 * FFMA / s / 1e12.  The measured counterpart of the ALU roofline. */

@@ -32,7 +32,8 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
            "lm_traj_fetch", "lm_traj_set_trace", "lm_traj_set_capsules", "lm_traj_set_obstacles",
            "lm_solve_host_workspace_bytes", "lm_solve_host",
-           "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch")
+           "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch",
+           "lm_search_workspace_bytes", "lm_search_default_params", "lm_search")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR = 0, 1
 LM_SOLVER_PRIMAL, LM_SOLVER_DUAL = 0, 1
 LM_ROT_LOG, LM_ROT_RPY = 0, 1
@@ -99,6 +100,11 @@ class LmPlanStats(C.Structure):
                 ("min_clearance", C.c_void_p), ("valid_trajectories", C.c_int64)]
 
 
+class LmSearchParams(C.Structure):
+    _fields_ = [("margin_rev", C.c_float), ("margin_pris", C.c_float), ("pen_limit", C.c_float),
+                ("pen_collision", C.c_float), ("use_clearance", C.c_int32)]
+
+
 class LmError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
@@ -158,6 +164,10 @@ def lib() -> C.CDLL:
         L.lm_plan_attach.argtypes = [C.c_void_p, C.POINTER(LmPlanParams), C.c_void_p, C.c_size_t]
         L.lm_plan_run.argtypes = [C.c_void_p, C.c_int32]
         L.lm_plan_fetch.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(LmPlanStats)]
+        L.lm_search_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64]
+        L.lm_search_workspace_bytes.restype = C.c_size_t
+        L.lm_search_default_params.argtypes = [C.POINTER(LmSearchParams)]
+        L.lm_search.argtypes = [C.c_void_p, C.POINTER(LmSearchParams), C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -368,6 +378,25 @@ def lm_plan_fetch(ctx: int, q_valid_ptr: Optional[int], stats: Optional[LmPlanSt
     _check(lib().lm_plan_fetch(ctx, q_valid_ptr, C.byref(stats) if stats is not None else None), "lm_plan_fetch")
 
 
+def lm_search_workspace_bytes(dof: int, K: int, n: int) -> int:
+    return int(lib().lm_search_workspace_bytes(dof, K, n))
+
+
+def lm_search_default_params(**overrides) -> LmSearchParams:
+    p = LmSearchParams()
+    _check(lib().lm_search_default_params(C.byref(p)), "lm_search_default_params")
+    for k, v in overrides.items():
+        if not hasattr(p, k):
+            raise AttributeError(k)
+        setattr(p, k, v)
+    return p
+
+
+def lm_search(ctx: int, params: LmSearchParams, workspace_ptr: int, workspace_bytes: int, choice_ptr: Optional[int],
+              xi_ptr: Optional[int], result_ptr: Optional[int]) -> None:
+    _check(lib().lm_search(ctx, C.byref(params), workspace_ptr, workspace_bytes, choice_ptr, xi_ptr, result_ptr), "lm_search")
+
+
 def lm_free(ctx: int) -> None:
     lib().lm_free(ctx)
 
@@ -570,6 +599,23 @@ class Solver:
         res["q_valid"] = np.ascontiguousarray(qv.numpy().T)
         res["valid_trajectories"] = int(st.valid_trajectories)
         return res
+
+    # -- global discrete search over the B = K candidates of one path (include/lm.h, lm_search)
+    def search(self, sparams: Optional[LmSearchParams] = None, to_host: bool = True) -> dict:
+        torch = self.torch
+        sparams = sparams if sparams is not None else lm_search_default_params()
+        nbytes = lm_search_workspace_bytes(self.d, self.B, self.n)
+        if getattr(self, "search_workspace", None) is None or self.search_workspace.numel() < nbytes + 256:
+            self.search_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self.search_workspace.data_ptr() + 255) // 256 * 256
+        if not to_host:
+            lm_search(self._ctx, sparams, ptr, nbytes, None, None, None)
+            return {}
+        choice = torch.empty((self.n,), dtype=torch.int32).pin_memory()
+        xi = torch.empty((self.d, self.n), dtype=torch.float32).pin_memory()
+        res = torch.empty((2,), dtype=torch.float32).pin_memory()
+        lm_search(self._ctx, sparams, ptr, nbytes, choice.data_ptr(), xi.data_ptr(), res.data_ptr())
+        return {"choice": choice.numpy().copy(), "xi": np.ascontiguousarray(xi.numpy().T), "cost": float(res[0]), "mjac": float(res[1])}
 
     def fetch_totals(self) -> tuple:
         """lm_fetch of the two scalar totals only (synchronises the stream)."""

@@ -291,3 +291,32 @@ def config4(fk: FkFn, B: int = 4096, n: int = 300, seed_offset: int = 0) -> Work
 def to_soa(x: np.ndarray) -> np.ndarray:
     """[W, k] waypoint-major -> [k, W] structure-of-arrays (the device layout, include/lm.h)."""
     return np.ascontiguousarray(x.T)
+
+
+def search_candidates(ch: Chain, K: int, n: int, seed: int, jump: float = 0.8, quant=None, limit_frac: float = 0.0) -> np.ndarray:
+    """Input of the global discrete search (synthetic stand-in for K IK-generated motion plans of one
+    path): q [K, n, d] fp32.  K candidate trajectories of one path as the search stage sees them: smooth pieces on different self-motion
+    branches, each with a few pieces on another branch (a jump in, a jump out); optionally quantised (many exact ties) and with some values pushed to a limit."""
+    rng = np.random.default_rng(seed)
+    base = smooth_joint_paths(ch, 1, n, 3, 0.3, rng)[0]
+    t = np.linspace(0.0, 1.0, n)[None, :, None]
+    q = base[None] + 0.03 * np.sin(2 * np.pi * (t * rng.uniform(0.5, 2.0, (K, 1, ch.dof)) + rng.random((K, 1, ch.dof))))
+    for k in range(K):
+        for _ in range(int(rng.integers(1, 4)) if K > 1 else 0):    # every candidate jumps somewhere: no single one is smooth
+            i0 = int(rng.integers(1, max(n, 2)))
+            i1 = i0 + 1 + int(rng.integers(0, max(n // 3, 1)))
+            q[k, i0:i1, :] += rng.normal(size=ch.dof) * jump * (rng.random(ch.dof) < 0.4)
+    span = ch.q_hi - ch.q_lo
+    q = np.clip(q, ch.q_lo + 0.05 * span, ch.q_hi - 0.05 * span)
+    if limit_frac > 0:
+        hit = rng.random(q.shape[:2]) < limit_frac
+        j = rng.integers(0, ch.dof, size=q.shape[:2])
+        side = rng.random(q.shape[:2]) < 0.5
+        for k, i in zip(*np.nonzero(hit)):
+            jj = j[k, i]
+            marg = 0.01 if ch.joint_type[jj] == 1 else np.deg2rad(0.5)
+            q[k, i, jj] = ch.q_lo[jj] + marg if side[k, i] else ch.q_hi[jj] - marg
+    if quant:
+        q = np.round(q / quant) * quant
+        q = np.clip(q, np.ceil((ch.q_lo + 0.05 * span) / quant) * quant, np.floor((ch.q_hi - 0.05 * span) / quant) * quant)
+    return q.astype(np.float32)

@@ -1,0 +1,62 @@
+"""Pins of the search oracle (oracle/lm_search_oracle.py; NEXT-4 iii) -- CPU only."""
+import numpy as np
+
+from oracle import lm_search_oracle as sorc
+from paper_2309_09102_b200 import workloads as wl
+
+
+def test_dp_equals_brute_force_over_all_paths():
+    rng = np.random.default_rng(0)
+    for K, n in ((2, 6), (3, 5), (4, 4)):
+        for trial in range(20):
+            q = rng.normal(size=(K, n, 3)) * 0.3
+            pen = 10.0 * (rng.random((n, K)) < 0.2) + 100.0 * (rng.random((n, K)) < 0.05)
+            choice, xi, cost, mj = sorc.search(q, pen)
+            assert np.isclose(cost, sorc.brute_force(q, pen), atol=1e-12)
+            # the returned path really has that cost and xi is the selected configurations
+            c = pen[0, choice[0]]
+            for i in range(1, n):
+                c = max(c, np.abs(q[choice[i], i] - q[choice[i - 1], i - 1]).max()) + pen[i, choice[i]]
+            assert np.isclose(c, cost, atol=1e-12)
+            assert np.array_equal(xi, q[choice, np.arange(n)])
+            assert np.isclose(mj, np.abs(np.diff(xi, axis=0)).max())
+
+
+def test_search_stitches_the_smooth_pieces_together():
+    """Two candidates that are each smooth on one half and jump on the other: the search switches between them once and
+    returns a path whose mjac is the small step, not the jump (the purpose of the module)."""
+    n, d = 40, 7
+    t = np.linspace(0, 1, n)[:, None]
+    smooth = 0.5 * np.sin(2 * np.pi * t + np.arange(d)[None, :])
+    a, b = smooth.copy(), smooth.copy() + 0.004          # b is a slightly shifted copy
+    a[n // 2:] += 1.0                                      # a jumps in the middle
+    b[:n // 2] -= 1.0                                      # b has its jump on the other side
+    q = np.stack([a, b])
+    choice, xi, cost, mj = sorc.search(q, np.zeros((n, 2)))
+    assert np.all(choice[:n // 2] == 0) and np.all(choice[n // 2:] == 1)
+    step = np.abs(np.diff(smooth, axis=0)).max()
+    assert mj <= step + 0.0041 and cost == mj
+    assert np.abs(np.diff(a, axis=0)).max() > 0.9 and np.abs(np.diff(b, axis=0)).max() > 0.9
+
+
+def test_penalties_match_the_paper():
+    ch = wl.random_chain_8dof(3)
+    q = np.tile(0.5 * (ch.q_lo + ch.q_hi), (2, 3, 1))
+    q[0, 1, 2] = ch.q_hi[2] - np.deg2rad(1.0)             # revolute joint within 1.5 deg of its limit
+    q[1, 2, 0] = ch.q_lo[0] + 0.02                        # prismatic joint within 3 cm
+    q[1, 0, 3] = ch.q_lo[3] + np.deg2rad(2.0)             # 2 deg away: fine
+    pen = sorc.penalties(q, ch.q_lo, ch.q_hi, ch.joint_type)
+    expect = np.zeros((3, 2))
+    expect[1, 0] = 10.0
+    expect[2, 1] = 10.0
+    assert np.array_equal(pen, expect)
+    clr = np.full((2, 3), 0.1)
+    clr[0, 0] = -0.01
+    assert np.array_equal(sorc.penalties(q, ch.q_lo, ch.q_hi, ch.joint_type, clr), expect + 100.0 * (clr.T < 0))
+    # a penalised node is avoided whenever an unpenalised path exists (10 > the largest possible mjac of pi)
+    rng = np.random.default_rng(1)
+    qq = rng.uniform(-1, 1, size=(3, 8, 4))
+    pen = np.zeros((8, 3))
+    pen[3, 0] = pen[3, 1] = 10.0
+    choice, _, cost, _ = sorc.search(qq, pen)
+    assert choice[3] == 2 and cost < 10.0
