@@ -326,6 +326,8 @@ def run_gpu(args) -> None:
         # the "to convergence" statistic of the metric, on BASELINE.json configs[1] (512 x 300, tol 1e-5)
         extra["to_convergence_C2"] = time_to_convergence(lm, torch, wl, fk, device, stream)
         extra["variant_dual"] = time_dual_variant(lm, torch, w, device, stream, peak_tf)
+        # lm_step: one iteration per launch, the state round-trips through HBM (report both bounds)
+        extra["single_step_C4"] = time_single_step(lm, torch, w, solver, stream, peak_tf, peaks)
         # the trajectory-level step on the same workload
         extra["trajectory_step"] = time_traj_step(lm, torch, w, solver, stream, peaks)
         # the paper's alternating schedule with anytime bookkeeping (NEXT-2), valid trajectories per second
@@ -484,6 +486,37 @@ def time_plan(lm, torch, wl, fk, device, stream, cycles: int = 3, reps: int = 5)
     s.close()
     out["workload"] = f"C2: {w.B} x {w.n}, tol={w.tol:g}, pose_iters=10, w_pose=1, w_diff=1"
     return out
+
+
+def time_single_step(lm, torch, w, solver, stream, peak_tf: float, peaks: dict, nsteps: int = 20, reps: int = 5) -> dict:
+    """lm_step on the headline workload: `nsteps` launches of one LM iteration each (state in / out of HBM every
+    launch, FK recomputed at entry), CUDA events around the launches on the launching stream, best of `reps`.
+    Per waypoint-iteration: 1459 + one more FK (342) + residual (77) = 1878 FLOP (d = 7; SURVEY 8d counts 1.87 k) and
+    4 (2d + 18) bytes (q, lambda, iters|status, 64-bit mask both ways, targets in, |r| / pos / rot error out)."""
+    d = int(w.chain.dof)
+    flop = ALG_FLOP.get(d, 1459.0 * d / 7.0) + 48.0 * d + 6.0 + 77.0
+    nbytes = 4.0 * (2 * d + 18)
+    ts = []
+    with torch.cuda.stream(stream):
+        for i in range(reps + 1):
+            solver.reset()
+            solver.step()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(nsteps):
+                solver.step()
+            b.record(stream)
+            stream.synchronize()
+            if i >= 1:
+                ts.append(a.elapsed_time(b) / nsteps)
+    ms = float(min(ts))
+    W = w.B * w.n
+    tf = flop * W / (ms * 1e-3) / 1e12
+    gbs = nbytes * W / (ms * 1e-3) / 1e9
+    return {"ms_per_lm_step": ms, "waypoint_iterations_per_sec": W / (ms * 1e-3), "alg_flop_per_waypoint_iteration": flop,
+            "alg_bytes_per_waypoint_iteration": nbytes, "alu": {"achieved_tflops": tf, "frac_of_derived_peak": tf / peak_tf},
+            "hbm": {"achieved_gbs": gbs, "peak_gbs": peaks["hbm_gbs"], "frac": gbs / peaks["hbm_gbs"]},
+            "note": "tol = 0 workload: every waypoint executes every step"}
 
 
 def time_search(lm, torch, wl, fk, device, stream, K: int = 175, n: int = 300, reps: int = 10) -> dict:
