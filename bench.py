@@ -425,6 +425,27 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
                     "trajectories_with_active_pairs": int((gc_["cost_coll"] > 0).sum()),
                     "with_environment_rows": {"ms_per_iteration": float(min(te)) / iters, "cuboids": 3, "pairs": 10,
                                               "trajectories_with_active_pairs": int((ge_["cost_coll"] > 0).sum())}}
+    # the same step without the refinement re-solve (refine_steps = 0: 3 launches per iteration instead of 5).  At this
+    # workload's weights the fp32 block elimination alone is within 1e-5 rad of the fp64 oracle (bar 1e-4; the refinement
+    # matters when w_diff^2 + lambda is small), so it is an option, not the default.
+    solver.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=0.3, refine_steps=0))
+    t0_ = []
+    with torch.cuda.stream(stream):
+        for i in range(reps + 1):
+            solver.reset()
+            solver.run(4)
+            solver.traj_reset()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            solver.traj_run(iters)
+            b.record(stream)
+            stream.synchronize()
+            if i >= 1:
+                t0_.append(a.elapsed_time(b))
+    ms0 = float(min(t0_)) / iters
+    alg0 = traj_step_alg_bytes(d, 0) * w.W
+    norefine = {"ms_per_iteration": ms0, "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, 0),
+                "hbm_frac": alg0 / (ms0 * 1e-3) / 1e9 / peaks["hbm_gbs"]}
     ms_iter = float(min(ts)) / iters
     alg = traj_step_alg_bytes(d, int(tp.refine_steps)) * w.W
     out = {"workload": f"{w.name}: {w.B} x {w.n}, after 4 pose-only iterations; w_pose=1, w_diff=0.3, refine=1, {iters} iterations",
@@ -432,6 +453,7 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
            "trajectory_iterations_per_sec": w.B / (ms_iter * 1e-3), "gpu_launches_per_run": int(launches),
            "accepted_fraction": float(np.mean([bin(int(m)).count("1") for m in g["mask"]])) / iters,
            "cost_diff_mean": float(g["cost_diff"].mean()), "with_self_collision_rows": coll,
+           "without_refinement": norefine,
            "roofline": {"bound": "hbm", "achieved": alg / (ms_iter * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
                         "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps)),

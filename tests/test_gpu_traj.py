@@ -83,6 +83,41 @@ def test_teacher_forced_single_step(chain_name, weights):
     assert np.all(g["iters"] == 1) and g["total_traj_iters"] == B
 
 
+@pytest.mark.parametrize("w_diff", [1.0, 0.3, 0.1])
+def test_single_step_without_refinement_is_inside_the_bar(w_diff):
+    """refine_steps = 0 (no rho / re-solve launches): the fp32 two-sided block elimination alone stays inside the 1e-4 rad
+    bar when the differencing weight keeps the blocks well conditioned (measured 4e-6 / 1e-5 / 2e-5 for w_diff = 1 / 0.3 /
+    0.1; 3e-4 at w_diff = 0, which is why the default is one refinement)."""
+    ch = wl.panda_chain()
+    B, n = 37, 64
+    w = make_problem(ch, B, n, 0.1, 11)
+    tp, tq, q0 = oracle_inputs(w)
+    lam = (10.0 ** np.random.default_rng(5).uniform(-4, -1, size=B)).astype(np.float32)
+    tprm = torc.TrajParams(w_pose=1.0, w_diff=w_diff)
+    s = solver_for(w, w_pose=1.0, w_diff=w_diff, refine_steps=0)
+    s.traj_reset(lam)
+    s.traj_enable_trace()
+    l0 = lm().lm_launch_count()
+    s.traj_run(1)
+    launches = lm().lm_launch_count() - l0
+    g = s.traj_fetch()
+    s.close()
+    st = torc.init_state(q0, tprm)
+    st.lam[:] = lam.astype(np.float64)
+    torc.advance(ch, orc.Params(), tprm, tp, tq, st, 1)
+    err = np.abs(g["trial_q"].reshape(B, n, ch.dof) - st.trial_q).max()
+    assert err <= 5e-5 and err <= TOL_Q
+    margin = np.abs(st.F_before - st.F_trial) > 1e-3 * st.F_before
+    acc_g = (g["mask"] & np.uint64(1)).astype(bool)
+    assert np.array_equal(acc_g[margin], (st.accepted == 1)[margin])
+    s1 = solver_for(w, w_pose=1.0, w_diff=w_diff)                  # default: one refinement = two more launches
+    s1.traj_reset(lam)
+    l0 = lm().lm_launch_count()
+    s1.traj_run(1)
+    assert lm().lm_launch_count() - l0 == launches + 2
+    s1.close()
+
+
 def decisive_compare(tr, gmask, iters):
     """Accept bits on the decisive prefix of every trajectory (oracle margin > 1e-3); returns
     (#compared, #mismatching trajectories, alive mask after the last iteration)."""
