@@ -233,3 +233,56 @@ def test_obstacle_argument_errors_and_removal():
     with pytest.raises(lm.LmError):
         s.traj_set_obstacles(bad)
     s.close()
+
+
+def test_full_size_sampled_with_all_rows():
+    """The trajectory-level step with the 9 self-collision and 10 capsule-cuboid pairs at the size and in the
+    configuration bench.py's trajectory_step.with_environment_rows section times (configs[3]: 4096 x 300, after 4
+    pose-only iterations, w_pose 1, w_diff 0.3, w_coll = w_env = 1, d_safe 0.05): every 256th trajectory against the
+    oracle.  Both sides start the step from the ORACLE's joint values after its own pose phase (fp32, lm_set_state)."""
+    from paper_2309_09102_b200 import lm
+    ch, model, scene = wl.panda_chain(), wl.panda_capsules(), wl.panda_scene()
+    w = wl.config4(lambda q: orc.fk(ch, q))
+    B, n = w.B, w.n
+    pick = np.arange(0, B, 256)
+    P = len(pick)
+    tp_s = w.target_pos.astype(np.float64).reshape(B, n, 3)[pick]
+    tq_s = w.target_quat.astype(np.float64).reshape(B, n, 4)[pick]
+    q_o = orc.lm_run(ch, orc.Params(lambda0=w.lambda0, tol=0.0), tp_s.reshape(-1, 3), tq_s.reshape(-1, 4),
+                     w.seeds.astype(np.float64).reshape(B, n, 7)[pick].reshape(-1, 7), 4).q.astype(np.float32).reshape(P, n, 7)
+    s = lm.Solver(ch, B, n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0))
+    s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=0.3))
+    s.traj_set_capsules(model, 1.0, 0.05)
+    s.traj_set_obstacles(scene, 1.0, 0.05)
+    s.run(4)
+    q_all = s.fetch()["q"].reshape(B, n, 7).copy()
+    q_all[pick] = q_o
+    s.set_state(q_all.reshape(B * n, 7))
+    s.traj_enable_trace()
+    s.traj_run(1)
+    g = s.traj_fetch()
+    s.close()
+    caps = corc.Capsules(model, w_coll=1.0, d_safe=0.05, scene=scene, w_env=1.0, d_safe_env=0.05)
+    tprm = torc.TrajParams(w_pose=1.0, w_diff=0.3, caps=caps)
+    q0 = q_o.astype(np.float64)
+    st = torc.init_state(q0, tprm)
+    torc.advance(ch, orc.Params(), tprm, tp_s, tq_s, st, 1)
+    assert g["total_traj_iters"] == B
+    assert np.allclose(g["F_before"][pick], st.F_before, rtol=1e-4)
+    assert (g["cost_coll"] > 0).sum() > B // 4                     # the rows are active in the bench's configuration
+    # trajectories excluded from the strict comparison, by oracle-only criteria (see test_single_step_with_obstacles):
+    # a pair within 1e-4 m of its hinge switch, the oracle's own step sensitive to a 1e-6 perturbation, crossing axes
+    thr = np.r_[np.full(len(model.pairs), 0.05), np.full(len(scene.pairs), 0.05)]
+    rad = np.r_[model.radius[model.pairs[:, 0]] + model.radius[model.pairs[:, 1]], model.radius[scene.pairs[:, 0]]]
+    dist = np.array([[corc.residual(ch, caps, q0[b, i])[0] for i in range(n)] for b in range(P)])      # [P, n, pairs]
+    clear = np.all(np.abs(dist - thr) > 1e-4, axis=(1, 2)) & np.all(dist + rad > 1e-3, axis=(1, 2))
+    st2 = torc.init_state(q0 + 1e-6 * np.random.default_rng(9).normal(size=q0.shape), tprm)
+    torc.advance(ch, orc.Params(), tprm, tp_s, tq_s, st2, 1)
+    clear &= np.abs(st2.trial_q - st.trial_q).max(axis=(1, 2)) < 2e-5
+    assert clear.sum() >= P // 2
+    err = np.abs(g["trial_q"].reshape(B, n, 7)[pick] - st.trial_q).max(axis=(1, 2))
+    assert err[clear].max() <= 2e-5
+    assert np.allclose(g["F_trial"][pick][clear], st.F_trial[clear], rtol=1e-4)
+    margin = clear & (np.abs(st.F_before - st.F_trial) > 1e-3 * st.F_before)
+    acc = (g["mask"][pick] & np.uint64(1)).astype(bool)
+    assert np.array_equal(acc[margin], (st.accepted == 1)[margin])

@@ -151,3 +151,36 @@ def test_schedule_with_capsules_requires_collision_free_trajectories():
     assert o.valid[:3].any() and not o.valid[3:].any()            # the folded trajectories go through the base column
     v = o.valid & decisive
     assert np.abs(g["q_valid"].reshape(B, n, 7)[v] - o.q_valid[v]).max() <= 1e-4
+
+
+def test_schedule_full_size_sampled():
+    """The schedule at the size and in the configuration bench.py's schedule_C2 section times (configs[1]: 512 x 300,
+    tol 1e-5, pose_iters 10, w_pose = w_diff = 1, 3 cycles): every 64th trajectory against the oracle run on those
+    trajectories alone, from the same seeds (trajectories are independent)."""
+    from paper_2309_09102_b200 import lm
+    ch = wl.panda_chain()
+    w = wl.config2(lambda q: orc.fk(ch, q))
+    B, n, d = w.B, w.n, 7
+    s = lm.Solver(ch, B, n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(lambda0=w.lambda0, tol=w.tol))
+    s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=1.0))
+    s.plan_attach(lm.lm_plan_default_params(pose_iters=10))
+    s.plan_run(3)
+    g = s.plan_fetch()
+    g["q"] = s.fetch()["q"].reshape(B, n, d)
+    g["traj"] = s.traj_fetch()
+    s.close()
+    pick = np.arange(0, B, 64)
+    o = porc.plan(ch, orc.Params(lambda0=w.lambda0, tol=w.tol), torc.TrajParams(w_pose=1.0, w_diff=1.0), porc.PlanParams(pose_iters=10),
+                  w.target_pos.astype(np.float64).reshape(B, n, 3)[pick], w.target_quat.astype(np.float64).reshape(B, n, 4)[pick],
+                  w.seeds.astype(np.float64).reshape(B, n, d)[pick], 3)
+    assert np.array_equal(g["valid"][pick], o.valid) and np.array_equal(g["first_valid_cycle"][pick], o.first_valid_cycle)
+    assert np.array_equal(g["traj"]["iters"][pick], o.traj_iters)
+    same = g["traj"]["mask"][pick] == o.traj_mask
+    assert same.mean() >= 0.75
+    v = o.valid & same
+    assert v.any()
+    assert np.abs(g["q_valid"].reshape(B, n, d)[pick][v] - o.q_valid[v]).max() <= 1e-4
+    assert np.allclose(g["length"][pick][v], o.length[v], rtol=1e-4)
+    assert np.array_equal(g["records"][pick][v], o.records[v])
+    assert np.abs(g["q"][pick][same] - o.q[same]).max() <= 1e-4
+    assert g["valid_trajectories"] == int(g["valid"].sum())

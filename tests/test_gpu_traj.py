@@ -331,26 +331,34 @@ def test_argument_errors():
 
 def test_full_size_sampled():
     """The trajectory-level step at the bench's size (4096 x 300, configs[3] inputs, after 4 pose-only iterations, as
-    bench.py's trajectory_step section runs it): every 256th trajectory against the oracle, started from the joint
-    values the GPU had after the pose phase (trajectories are independent; bits do not depend on the batch)."""
+    bench.py's trajectory_step section runs it): every 256th trajectory against the oracle.  Both sides start the step
+    from the ORACLE's joint values after its own 4 pose-only iterations (rounded to fp32 and injected with lm_set_state
+    -- oracle -> GPU, never the other way round); the other 4080 trajectories keep the GPU's own pose-phase state
+    (trajectories are independent; bits do not depend on the batch)."""
     from paper_2309_09102_b200 import lm
     ch = wl.panda_chain()
     w = wl.config4(lambda q: orc.fk(ch, q))
     B, n = w.B, w.n
+    pick = np.arange(0, B, 256)
+    tp_s = w.target_pos.astype(np.float64).reshape(B, n, 3)[pick]
+    tq_s = w.target_quat.astype(np.float64).reshape(B, n, 4)[pick]
+    q_o = orc.lm_run(ch, orc.Params(lambda0=w.lambda0, tol=0.0), tp_s.reshape(-1, 3), tq_s.reshape(-1, 4),
+                     w.seeds.astype(np.float64).reshape(B, n, 7)[pick].reshape(-1, 7), 4).q.astype(np.float32)
     s = lm.Solver(ch, B, n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0))
     s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=0.3))
     s.run(4)
-    q_start = s.fetch()["q"].reshape(B, n, 7)
+    q_all = s.fetch()["q"].reshape(B, n, 7).copy()
+    q_all[pick] = q_o.reshape(len(pick), n, 7)
+    s.set_state(q_all.reshape(B * n, 7))
+    q_start = q_o.reshape(len(pick), n, 7)
     s.traj_enable_trace()
     s.traj_run(1)
     g = s.traj_fetch()
     s.close()
     assert g["total_traj_iters"] == B
-    pick = np.arange(0, B, 256)
     tprm = torc.TrajParams(w_pose=1.0, w_diff=0.3)
-    st = torc.init_state(q_start[pick].astype(np.float64), tprm)
-    torc.advance(ch, orc.Params(), tprm, w.target_pos.astype(np.float64).reshape(B, n, 3)[pick],
-                 w.target_quat.astype(np.float64).reshape(B, n, 4)[pick], st, 1)
+    st = torc.init_state(q_start.astype(np.float64), tprm)
+    torc.advance(ch, orc.Params(), tprm, tp_s, tq_s, st, 1)
     assert np.abs(g["trial_q"].reshape(B, n, 7)[pick] - st.trial_q).max() <= 2e-5
     assert np.allclose(g["F_before"][pick], st.F_before, rtol=1e-4) and np.allclose(g["F_trial"][pick], st.F_trial, rtol=1e-4)
     margin = np.abs(st.F_before - st.F_trial) > 1e-3 * st.F_before
