@@ -336,8 +336,6 @@ def run_gpu(args) -> None:
         extra["search_K175_n300"] = time_search(lm, torch, wl, fk, device, stream)
     roofline["peak_measured_fma_rrr"] = lm.lm_fp32_peak_form(lm.LM_FMA_FORM_RRR, int(stream.cuda_stream))
     roofline["frac_of_measured_fma_rrr"] = achieved_tf / roofline["peak_measured_fma_rrr"]
-    if True:
-        pass
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms_all / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
