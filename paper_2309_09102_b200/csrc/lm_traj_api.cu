@@ -184,6 +184,7 @@ int lm_traj_set_capsules(lm_ctx *c, const lm_capsules *m) {
     for (int i = 0; i < m->ncaps; ++i) {
         if (m->link[i] < -1 || m->link[i] >= c->dof || !(m->radius[i] >= 0.f)) return LM_EINVAL;
         k.link[i] = (int8_t)m->link[i];
+        k.on_link[m->link[i] + 1] |= (uint16_t)(1u << i);
         k.c[i] = m->radius[i];
         double l2 = 0.0;
         for (int x = 0; x < 3; ++x) {
