@@ -217,7 +217,7 @@ def run_reference(args) -> None:
     r = time_oracle(w, n_traj, steps=args.steps, warmup=min(args.warmup, 1))
     full = workload_desc(w)
     full["workload"] += f" [oracle timed on a {n_traj}-trajectory sample of the {args.B or 4096}-trajectory workload]"
-    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": 0,
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": int(args.gpus), "gpus_used": 0,
             "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": r["ms_per_step"],
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": full,
