@@ -364,3 +364,43 @@ def test_full_size_sampled():
     margin = np.abs(st.F_before - st.F_trial) > 1e-3 * st.F_before
     acc = (g["mask"][pick] & np.uint64(1)).astype(bool)
     assert np.array_equal(acc[margin], (st.accepted == 1)[margin])
+
+
+@pytest.mark.parametrize("d", [1, 3, 6])
+def test_low_dof_trajectory_step_and_search(d):
+    """The generic instantiations of the trajectory-level kernels (D = 1..6) and the search on a short chain."""
+    from oracle import lm_search_oracle as sorc
+    rng = np.random.default_rng(70 + d)
+    ch = wl.Chain(f"gen{d}", d, (rng.random(d) < 0.25).astype(np.int32), rng.uniform(-0.3, 0.3, d),
+                  rng.choice([0.0, np.pi / 2, -np.pi / 2, 0.7], d), rng.uniform(0.0, 0.3, d), rng.uniform(-1, 1, d),
+                  np.full(d, -2.0), np.full(d, 2.0), np.array([0.05, 0.0, 0.1, 1, 0, 0, 0.0]))
+    B, n = 35, 40
+    truth = np.cumsum(rng.normal(size=(B, n, d)) * 0.02, axis=1) + rng.uniform(-1.0, 1.0, size=(B, 1, d))
+    w = wl._from_truth("lowT", ch, np.clip(truth, -1.9, 1.9), 0.05, rng, lambda q: orc.fk(ch, q), 0.0, 10)
+    tp, tq, q0 = oracle_inputs(w)
+    lam = (10.0 ** rng.uniform(-3, -1, size=B)).astype(np.float32)
+    tprm = torc.TrajParams(w_pose=1.0, w_diff=0.5)
+    s = solver_for(w, w_pose=1.0, w_diff=0.5)
+    s.traj_reset(lam)
+    s.traj_enable_trace()
+    s.traj_run(1)
+    g = s.traj_fetch()
+    gs = s.search()                                   # on the joint values after the step
+    q_after = s.fetch()["q"].reshape(B, n, d)
+    s.close()
+    st = torc.init_state(q0, tprm)
+    st.lam[:] = lam.astype(np.float64)
+    torc.advance(ch, orc.Params(), tprm, tp, tq, st, 1)
+    assert np.abs(g["trial_q"].reshape(B, n, d) - st.trial_q).max() <= 2e-5
+    assert np.allclose(g["F_before"], st.F_before, rtol=1e-4, atol=1e-9) and np.allclose(g["F_trial"], st.F_trial, rtol=1e-4, atol=1e-9)
+    # the search is an exact (fp32) function of the joint values it ran on: feed the oracle the same candidates through
+    # the seeds of a second context (host -> GPU), not the fetched values
+    q32 = wl.search_candidates(ch, 9, 25, 80 + d)
+    s2 = lm().Solver(ch, 9, 25, np.zeros((225, 3), np.float32), np.tile(np.array([[1, 0, 0, 0]], np.float32), (225, 1)), q32.reshape(225, d))
+    g2 = s2.search()
+    s2.close()
+    pen = sorc.penalties(q32, ch.q_lo.astype(np.float32), ch.q_hi.astype(np.float32), ch.joint_type,
+                         margin_rev=np.float32(np.deg2rad(1.5)), margin_pris=np.float32(0.03))
+    choice, xi, cost, mj = sorc.search(q32, pen, dtype=np.float32)
+    assert np.array_equal(g2["choice"], choice) and np.array_equal(g2["xi"], xi) and np.float32(g2["cost"]) == np.float32(cost)
+    assert gs["choice"].shape == (n,) and q_after.shape == (B, n, d)
