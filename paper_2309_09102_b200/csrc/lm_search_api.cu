@@ -1,9 +1,9 @@
 // lm_search_api.cu -- C ABI of the global discrete search over K candidate trajectories of one path
 // (include/lm.h, lm_search*; sec. III-B).
 //
-// Two kernels.  search_edges_kernel is the parallel part: block i holds the K configurations of
-// timesteps i-1 and i in shared memory and writes the K x K edge costs max_j |dq_j| (coalesced) and
-// the K node penalties of timestep i.  search_dp_kernel is the sequential part: one thread-block cluster
+// Two kernels.  search_edges_kernel is the parallel part: block (i, y) holds the K configurations of
+// timesteps i-1 and i in shared memory and writes a slice of the K x K edge costs max_j |dq_j| (coalesced);
+// the y = 0 blocks also write the K node penalties of timestep i.  search_dp_kernel is the sequential part: one thread-block cluster
 // walks the n layers, G lanes per node scan its K incoming edges (L2-resident), then CTA 0 picks the cheapest
 // end node, reads the path back through the stored predecessors and gathers xi_search.  Every
 // subtraction and addition is a single fp32 operation rounded to nearest, max and < are exact, ties go
@@ -75,14 +75,16 @@ struct SArgs {
     float *result;      // [2]
 };
 
-// Block (i, y): for i >= 1 the edge costs between layers i-1 and i into the nodes k = y, y + gridDim.y, ...;
-// blocks with y = 0 also write the penalties of layer i.
+// Block (i, y): for i >= 1 the edge costs between layers i-1 and i into a slice of the nodes k; blocks with y = 0
+// also write the penalties of layer i.  A thread owns one predecessor k' (its D joint values stay in registers) and
+// walks the rows k of the slice: per edge D broadcast shared-memory reads, D subtractions, D max.
+template <int D>
 __global__ void __launch_bounds__(EDGE_THREADS) search_edges_kernel(const SArgs A) {
     extern __shared__ float sm[];
-    const int K = A.K, KP = A.KP, d = A.dof, i = blockIdx.x, t = threadIdx.x;
-    float *qa = sm;          // [d][K] layer i-1
-    float *qb = sm + d * K;  // [d][K] layer i
-    for (int e = t; e < d * K; e += EDGE_THREADS) {
+    const int K = A.K, KP = A.KP, i = blockIdx.x, t = threadIdx.x;
+    float *qa = sm;          // [D][K] layer i-1
+    float *qb = sm + D * K;  // [D][K] layer i
+    for (int e = t; e < D * K; e += EDGE_THREADS) {
         const int j = e / K, k = e - j * K;
         const int64_t w = (int64_t)j * A.W + (int64_t)k * A.n + i;
         qb[e] = A.q[w];
@@ -92,7 +94,8 @@ __global__ void __launch_bounds__(EDGE_THREADS) search_edges_kernel(const SArgs 
     if (blockIdx.y == 0) {
         for (int k = t; k < K; k += EDGE_THREADS) {
             bool near = false;
-            for (int j = 0; j < d; ++j) {
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
                 const float m = ((A.prismatic_mask >> j) & 1u) ? A.margin_pris : A.margin_rev;
                 const float v = qb[j * K + k];
                 near = near || (__fsub_rn(v, A.lo[j]) < m) || (__fsub_rn(A.hi[j], v) < m);
@@ -104,18 +107,19 @@ __global__ void __launch_bounds__(EDGE_THREADS) search_edges_kernel(const SArgs 
     }
     if (i == 0) return;
     float *out = A.edges + (size_t)(i - 1) * K * KP;
-    for (int k = blockIdx.y; k < K; k += gridDim.y) {
-        float qk[MAX_DOF];
+    const int rows = (K + gridDim.y - 1) / gridDim.y, k0 = blockIdx.y * rows, k1 = min(K, k0 + rows);
+    for (int kp = t; kp < KP; kp += EDGE_THREADS) {
+        if (kp >= K) { // the padding of every row: never chosen
+            for (int k = k0; k < k1; ++k) out[(size_t)k * KP + kp] = __int_as_float(0x7f800000);
+            continue;
+        }
+        float qp[D];
 #pragma unroll
-        for (int j = 0; j < MAX_DOF; ++j) qk[j] = j < d ? qb[j * K + k] : 0.f;
-        for (int kp = t; kp < KP; kp += EDGE_THREADS) {
-            float s = __int_as_float(0x7f800000);
-            if (kp < K) {
-                s = 0.f;
+        for (int j = 0; j < D; ++j) qp[j] = qa[j * K + kp];
+        for (int k = k0; k < k1; ++k) {
+            float s = 0.f;
 #pragma unroll
-                for (int j = 0; j < MAX_DOF; ++j)
-                    if (j < d) s = fmaxf(s, fabsf(__fsub_rn(qk[j], qa[j * K + kp])));
-            }
+            for (int j = 0; j < D; ++j) s = fmaxf(s, fabsf(__fsub_rn(qb[j * K + k], qp[j])));
             out[(size_t)k * KP + kp] = s;
         }
     }
@@ -345,13 +349,23 @@ int lm_search(lm_ctx *c, const lm_search_params *p, void *workspace, size_t byte
     const size_t pred_bytes = 2 * (size_t)c->n * ((size_t)a.KC + (size_t)K); // the owner's slice + CTA 0's gathered copy
     a.pred_in_smem = (dp_smem + pred_bytes + 2048 <= SMEM_OPT_IN) ? 1 : 0;
     if (a.pred_in_smem) dp_smem += pred_bytes;
-    LM_CUDA(cudaFuncSetAttribute(search_edges_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536));
     launch_counter().fetch_add(2);
     {
         int split = (int)((4 * 148 + c->n - 1) / c->n); // about four blocks per SM, more when the trajectory is short
         if (split > K) split = K;
         if (split < 1) split = 1;
-        search_edges_kernel<<<dim3((unsigned)c->n, (unsigned)split), EDGE_THREADS, edge_smem, c->stream>>>(a);
+        const dim3 grid((unsigned)c->n, (unsigned)split);
+#define LM_EDGE_LAUNCH(DD)                                                                                                  \
+    case DD:                                                                                                                \
+        LM_CUDA(cudaFuncSetAttribute(search_edges_kernel<DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536));         \
+        search_edges_kernel<DD><<<grid, EDGE_THREADS, edge_smem, c->stream>>>(a);                                           \
+        break;
+        switch (d) {
+            LM_EDGE_LAUNCH(1) LM_EDGE_LAUNCH(2) LM_EDGE_LAUNCH(3) LM_EDGE_LAUNCH(4)
+            LM_EDGE_LAUNCH(5) LM_EDGE_LAUNCH(6) LM_EDGE_LAUNCH(7) LM_EDGE_LAUNCH(8)
+            default: return LM_EINVAL;
+        }
+#undef LM_EDGE_LAUNCH
         LM_CUDA(cudaGetLastError());
     }
     {
