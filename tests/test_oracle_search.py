@@ -60,3 +60,40 @@ def test_penalties_match_the_paper():
     pen[3, 0] = pen[3, 1] = 10.0
     choice, _, cost, _ = sorc.search(qq, pen)
     assert choice[3] == 2 and cost < 10.0
+
+
+def test_invariants_of_the_optimal_cost():
+    """Properties any correct minimax path search has: relabelling the candidates leaves the cost unchanged, more
+    candidates never make it worse, reversing time (no penalties) gives the same cost, and the cost is never below the
+    largest layer-to-layer gap min_{k,k'} step (every path crosses every layer)."""
+    rng = np.random.default_rng(3)
+    for trial in range(10):
+        K, n, d = 6, 30, 4
+        q = np.cumsum(rng.normal(size=(K, n, d)) * 0.05, axis=1) + rng.normal(size=(K, 1, d)) * 0.2
+        for k in range(K):
+            i0 = int(rng.integers(1, n))
+            q[k, i0:] += rng.normal(size=d) * 0.5
+        pen = 10.0 * (rng.random((n, K)) < 0.1)
+        c0 = sorc.search(q, pen)[2]
+        perm = rng.permutation(K)
+        assert np.isclose(sorc.search(q[perm], pen[:, perm])[2], c0, atol=1e-12)
+        extra = np.concatenate([q, q[:2] + 0.01 * rng.normal(size=(2, n, d))])
+        assert sorc.search(extra, np.concatenate([pen, pen[:, :2]], axis=1))[2] <= c0 + 1e-12
+        zero = np.zeros((n, K))
+        cz = sorc.search(q, zero)[2]
+        assert np.isclose(sorc.search(q[:, ::-1], zero)[2], cz, atol=1e-12)
+        gap = max(np.abs(q[:, None, i] - q[None, :, i - 1]).max(axis=2).min() for i in range(1, n))
+        assert cz >= gap - 1e-12
+        assert cz <= min(np.abs(np.diff(q[k], axis=0)).max() for k in range(K)) + 1e-12     # a single candidate is a path
+
+
+def test_fp32_mode_rounds_like_the_kernel():
+    """dtype=np.float32: every difference and sum is an fp32 operation (what the CUDA path does with __fsub_rn /
+    __fadd_rn); on inputs that are exactly representable and whose differences are too, both modes agree exactly."""
+    rng = np.random.default_rng(4)
+    q = (rng.integers(-64, 64, size=(5, 12, 3)) / 32.0).astype(np.float32)      # multiples of 1/32: exact arithmetic
+    pen = 10.0 * (rng.random((12, 5)) < 0.2)
+    a = sorc.search(q, pen, dtype=np.float32)
+    b = sorc.search(q.astype(np.float64), pen, dtype=np.float64)
+    assert np.array_equal(a[0], b[0]) and a[2] == b[2] and a[3] == b[3]
+    assert a[1].dtype == np.float32
