@@ -43,6 +43,10 @@ SM_COUNT, FP32_LANES = 148, 128
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/r1c_lm_iterate_full.md); keyed by (workload, kernel variant).
 NCU_DRAM_TRAFFIC = {("C4", "panda7"): 68.849e6 + 27.575e6}
+# FP32 flop the kernel EXECUTES per waypoint-iteration (2 x FFMA + FMUL + FADD per warp-iteration from the source page of
+# the same capture: 2 x 532.9 + 165.6 + 68.2): fewer than the algorithmic count because multiplications by the
+# structural zeros / ones of the Panda chain are folded out.
+NCU_EXECUTED_FLOP = {("C4", "panda7"): 1300.0}
 
 
 def load_peaks() -> dict:
@@ -311,11 +315,14 @@ def run_gpu(args) -> None:
                 "kernel": f"lm_iterate_kernel<{d}, {solver.kernel_name}>", "kernel_ms": ms_kernel,
                 "peak_measured_fma": fma_tf, "frac_of_measured_fma": achieved_tf / fma_tf if fma_tf > 0 else None,
                 "alg_flop_per_waypoint_iteration": ALG_FLOP.get(d),
+                "ncu_executed_flop_per_waypoint_iteration": NCU_EXECUTED_FLOP.get((args.workload, solver.kernel_name)) if full_size else None,
                 "peak_how": f"derived: {SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz "
                             f"(sm_max_mhz {peaks['_source']})",
                 "hbm": {"alg_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / (ms_kernel * 1e-3) / 1e9,
                         "peak_gbs": peaks["hbm_gbs"], "frac": hbm_bytes / (ms_kernel * 1e-3) / 1e9 / peaks["hbm_gbs"],
                         "peak_source": peaks["_source"]}}
+    if roofline["ncu_executed_flop_per_waypoint_iteration"]:
+        roofline["executed_tflops"] = roofline["ncu_executed_flop_per_waypoint_iteration"] * iters_per_step / (ms_kernel * 1e-3) / 1e12
     ref_traj = min(args.ref_traj or 256, w.B)
     cpu = time_oracle(make_workload(args.workload, fk, ref_traj, w.n), ref_traj)
     cfg = workload_desc(w)
