@@ -22,7 +22,7 @@ namespace {
 constexpr int EDGE_THREADS = 256;
 constexpr int DP_THREADS = 512;
 constexpr int DP_CLUSTER = 8;   // portable maximum
-constexpr int DP_BATCH = 12;    // edge costs per lane held in registers across the cluster barrier
+constexpr int DP_BATCH = 12;    // edge costs per lane prefetched into registers before the wait that closes a layer
 constexpr size_t SMEM_OPT_IN = 232448; // 227 KB
 
 struct SLayout {
