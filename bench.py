@@ -426,10 +426,14 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
                     te.append(a.elapsed_time(b))
             ge_ = solver.traj_fetch()
             solver.traj_set_capsules(None)
+            # the same rows when the 32 trajectories of every tile are candidates for ONE path (the paper's use: K plans
+            # of one problem): the lanes of a warp are then near the same obstacles and walk similar pair lists
+            corr_ms, corr_active = time_correlated_tiles(lm, torch, w, wl_, stream, iters, reps)
             coll = {"ms_per_iteration": float(min(tc)) / iters, "capsules": 7, "pairs": 9, "w_coll": 1.0, "d_safe_m": 0.05,
                     "trajectories_with_active_pairs": int((gc_["cost_coll"] > 0).sum()),
                     "with_environment_rows": {"ms_per_iteration": float(min(te)) / iters, "cuboids": 3, "pairs": 10,
-                                              "trajectories_with_active_pairs": int((ge_["cost_coll"] > 0).sum())}}
+                                              "trajectories_with_active_pairs": int((ge_["cost_coll"] > 0).sum()),
+                                              "tiles_of_32_candidates_per_path": {"ms_per_iteration": corr_ms, "trajectories_with_active_pairs": corr_active}}}
     # the same step without the refinement re-solve (refine_steps = 0: 3 launches per iteration instead of 5).  At this
     # workload's weights the fp32 block elimination alone is within 1e-5 rad of the fp64 oracle (bar 1e-4; the refinement
     # matters when w_diff^2 + lambda is small), so it is an option, not the default.
@@ -479,6 +483,42 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
     except Exception as e:  # noqa: BLE001
         out["cpu_baseline"] = {"error": repr(e)}
     return out
+
+
+def time_correlated_tiles(lm, torch, w, wl_, stream, iters: int, reps: int):
+    """The headline workload with every tile of 32 trajectories replaced by 32 noisy copies (seed noise N(0, 0.02)) of
+    its first trajectory, all collision rows on: (ms per trajectory-level iteration, trajectories with active rows)."""
+    B, n, d = w.B, w.n, int(w.chain.dof)
+    tp = w.target_pos.reshape(B, n, 3).copy()
+    tq = w.target_quat.reshape(B, n, 4).copy()
+    sd = w.seeds.reshape(B, n, d).copy()
+    rng = np.random.default_rng(0)
+    for t0 in range(0, B, 32):
+        t1 = min(B, t0 + 32)
+        tp[t0:t1], tq[t0:t1] = tp[t0], tq[t0]
+        sd[t0:t1] = sd[t0] + rng.normal(size=(t1 - t0, n, d)).astype(np.float32) * np.float32(0.02)
+    sd = np.clip(sd, w.chain.q_lo.astype(np.float32) + np.float32(1e-4), w.chain.q_hi.astype(np.float32) - np.float32(1e-4))
+    s = lm.Solver(w.chain, B, n, tp.reshape(-1, 3), tq.reshape(-1, 4), sd.reshape(-1, d), params=lm.lm_default_params(tol=0.0),
+                  device=str(stream.device), stream=stream)
+    s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=0.3))
+    s.traj_set_capsules(wl_.panda_capsules(), 1.0, 0.05)
+    s.traj_set_obstacles(wl_.panda_scene(), 1.0, 0.05)
+    ts = []
+    with torch.cuda.stream(stream):
+        for i in range(reps + 1):
+            s.reset()
+            s.run(4)
+            s.traj_reset()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            s.traj_run(iters)
+            b.record(stream)
+            stream.synchronize()
+            if i >= 1:
+                ts.append(a.elapsed_time(b))
+        g = s.traj_fetch()
+    s.close()
+    return float(min(ts)) / iters, int((g["cost_coll"] > 0).sum())
 
 
 def time_plan(lm, torch, wl, fk, device, stream, cycles: int = 3, reps: int = 5) -> dict:
