@@ -362,6 +362,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
                      : "memory");
     }
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 #ifndef LM_TL_STAGE_BUDGET
@@ -399,74 +402,111 @@ template <int D, int MODE> __host__ __device__ constexpr size_t tl_solve_smem_by
 //   MODE 0: factor (stores W_i = -S_i^-1) and solve for g;                      delta  = -x
 //   MODE 1: re-solve with the stored W_i for rho (iterative refinement);        delta +=  x
 // The chunks of the next tl_stages<D, MODE>() waypoints of a warp's sequence are in flight (bulk-async copies
-// into its ring) while it eliminates the current one.
+// into its ring) while it eliminates the current one.  A THIRD warp is the producer of both rings: one of its lanes
+// waits for a stage to be released ("empty" mbarrier, armed by the consumer once all its lanes have read the stage),
+// posts the byte count on the stage's "full" mbarrier and issues the copies -- the address arithmetic, the
+// uniform-register traffic of UBLKCP and the divergent lane-0 branch (38 % of the refinement re-solve's issue slots
+// when every warp fed its own ring) are off the two sequential chains.
+constexpr int TL_SOLVE_THREADS = 96;
 template <int D, int MODE>
-__global__ void __launch_bounds__(64) tl_solve_kernel(const __grid_constant__ TArgs A) {
+__global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid_constant__ TArgs A) {
     constexpr int NA = Tri<D>::NA, CA = NA + D, SF = tl_stage_floats<D, MODE>(), NR = (MODE == 0) ? 2 : 1;
     constexpr int TL_STAGES = tl_stages<D, MODE>();
     extern __shared__ __align__(128) float smem[];
-    __shared__ __align__(8) uint64_t bars_all[2][TL_STAGES];
+    __shared__ __align__(8) uint64_t full_all[2][TL_STAGES], empty_all[2][TL_STAGES];
     __shared__ float xch[NA + D][32]; // warp 1 -> warp 0: W_{m+1}, z_{m+1}
     __shared__ float xmid[D][32];     // warp 0 -> both: x_m
     __shared__ int okx[2][32];
-    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5; // warps 0, 1: the two chains; warp 2: the producer
     const int64_t bt = blockIdx.x;
     const int64_t b = bt * 32 + lane;
     const bool valid = b < A.B;
     const uint32_t pk = valid ? A.its[b] : 0xffu;
     const bool active = valid && ((pk & 0xffu) < (uint32_t)A.max_total) && (MODE == 0 || A.ok[b] != 0) &&
                         (A.gate == nullptr || A.gate[b] != 0);
-    if (!__any_sync(0xffffffffu, active)) return; // the same lanes in both warps: block-uniform
+    if (!__any_sync(0xffffffffu, active)) return; // the same lanes in all three warps: block-uniform
     const int sel = valid ? A.sel[b] : 0;
-    const bool need0 = __any_sync(0xffffffffu, active && sel == 0); // warp-uniform
+    const bool need0 = __any_sync(0xffffffffu, active && sel == 0); // warp-uniform, the same in all three warps
     const bool need1 = __any_sync(0xffffffffu, active && sel == 1);
     const int n = A.n;
     const int64_t w0 = bt * n;
+    const int m = n / 2;
+    // sequence of warp q: q = 0 eliminates 0 .. m-1 and then the middle block m; q = 1 eliminates n-1 .. m+1
+    auto len_of = [&](int q) { return q == 0 ? m : n - 1 - m; };          // waypoints warp q eliminates
+    auto uses1_of = [&](int q) { return len_of(q) + (q == 0 ? 1 : 0); };  // ring uses of its elimination phase
+    auto idx_of = [&](int q, int k) { return q == 0 ? k : n - 1 - k; };   // k-th waypoint of its sequence (idx(0, m) = m)
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < TL_STAGES; ++s) {
+            mbar_init(&full_all[0][s], 1); mbar_init(&full_all[1][s], 1);
+            mbar_init(&empty_all[0][s], 1); mbar_init(&empty_all[1][s], 1);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (wp == 2) { // ---- the producer
+        auto ring_of = [&](int q) { return smem + (size_t)q * NR * TL_STAGES * SF; };
+        auto issue_fwd = [&](int q, int k) { // k = position in warp q's sequence of ring uses
+            const int s = k % TL_STAGES;
+            uint64_t *bar = &full_all[q][s];
+            const int64_t wid = w0 + idx_of(q, k);
+            float *dst = ring_of(q) + (size_t)s * SF;
+            if (MODE == 0) {
+                const uint32_t bytes = CA * 128u;
+                mbar_expect_tx(bar, (need0 ? bytes : 0u) + (need1 ? bytes : 0u));
+                if (need0) bulk_g2s(dst, A.Ag + wid * CA * 32, bytes, bar);
+                if (need1) bulk_g2s(dst + (size_t)TL_STAGES * SF, A.Ag + (int64_t)CA * A.nS + wid * CA * 32, bytes, bar);
+            } else {
+                mbar_expect_tx(bar, (NA + D) * 128u);
+                bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, bar);
+                bulk_g2s(dst + NA * 32, A.rho + wid * D * 32, D * 128u, bar);
+            }
+        };
+        auto issue_bwd = [&](int q, int kk, int i) {
+            const int s = kk % TL_STAGES;
+            uint64_t *bar = &full_all[q][s];
+            float *dst = ring_of(q) + (size_t)s * SF;
+            const int64_t wid = w0 + i;
+            mbar_expect_tx(bar, (NA + D + (MODE == 1 ? D : 0)) * 128u);
+            bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, bar);
+            bulk_g2s(dst + NA * 32, A.z + wid * D * 32, D * 128u, bar);
+            if (MODE == 1) bulk_g2s(dst + (NA + D) * 32, A.delta + wid * D * 32, D * 128u, bar);
+        };
+        // use u of a stage may be filled once use u - 1 has been released (uses are numbered per warp, both phases)
+        auto wait_free = [&](int q, int k) {
+            if (k >= TL_STAGES) mbar_wait(&empty_all[q][k % TL_STAGES], (uint32_t)(((k / TL_STAGES) - 1) & 1));
+        };
+        if (lane == 0) {
+            const int u0 = uses1_of(0), u1 = uses1_of(1);
+            for (int k = 0; k < u0 || k < u1; ++k) {
+                if (k < u0) { wait_free(0, k); issue_fwd(0, k); }
+                if (k < u1) { wait_free(1, k); issue_fwd(1, k); }
+            }
+        }
+        __syncthreads(); // (1) warp 1 has handed its last block to warp 0
+        __syncthreads(); // (2) the chunks written by the elimination are ordered before the copies below
+        fence_proxy_async();
+        if (lane == 0) {
+            const int l0 = len_of(0), l1 = len_of(1), u0 = uses1_of(0), u1 = uses1_of(1);
+            for (int j = 0; j < l0 || j < l1; ++j) {
+                if (j < l0) { wait_free(0, u0 + j); issue_bwd(0, u0 + j, idx_of(0, l0 - 1 - j)); }
+                if (j < l1) { wait_free(1, u1 + j); issue_bwd(1, u1 + j, idx_of(1, l1 - 1 - j)); }
+            }
+        }
+        __syncthreads(); // (3) the verdicts of the two chains
+        return;
+    }
+
+    // ---- the two chains
     const float lam = valid ? A.lam[b] : 1.f;
     float *ring = smem + (size_t)wp * NR * TL_STAGES * SF;
     float *ring1 = ring + (size_t)TL_STAGES * SF; // MODE 0 only: chunks of Ag buffer 1
-    uint64_t *bars = bars_all[wp];
-
-    const int m = n / 2;
-    const int len = (wp == 0) ? m : n - 1 - m;  // waypoints this warp eliminates
-    const int uses1 = len + (wp == 0 ? 1 : 0);  // ring uses of the elimination phase (warp 0 also fetches chunk m)
-    auto idx = [&](int k) { return wp == 0 ? k : n - 1 - k; }; // k-th waypoint of this warp's sequence (idx(m) = m for warp 0)
-
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < TL_STAGES; ++s) mbar_init(&bars[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncwarp();
-
-    auto issue_fwd = [&](int k) { // lane 0 only; k = position in this warp's sequence of ring uses
-        const int s = k % TL_STAGES;
-        const int64_t wid = w0 + idx(k);
-        if (MODE == 0) {
-            const uint32_t bytes = CA * 128u;
-            mbar_expect_tx(&bars[s], (need0 ? bytes : 0u) + (need1 ? bytes : 0u));
-            if (need0) bulk_g2s(ring + (size_t)s * SF, A.Ag + wid * CA * 32, bytes, &bars[s]);
-            if (need1) bulk_g2s(ring1 + (size_t)s * SF, A.Ag + (int64_t)CA * A.nS + wid * CA * 32, bytes, &bars[s]);
-        } else {
-            float *dst = ring + (size_t)s * SF;
-            mbar_expect_tx(&bars[s], (NA + D) * 128u);
-            bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, &bars[s]);
-            bulk_g2s(dst + NA * 32, A.rho + wid * D * 32, D * 128u, &bars[s]);
-        }
-    };
-    auto issue_bwd = [&](int kk, int i) { // lane 0 only
-        const int s = kk % TL_STAGES;
-        float *dst = ring + (size_t)s * SF;
-        const int64_t wid = w0 + i;
-        mbar_expect_tx(&bars[s], (NA + D + (MODE == 1 ? D : 0)) * 128u);
-        bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, &bars[s]);
-        bulk_g2s(dst + NA * 32, A.z + wid * D * 32, D * 128u, &bars[s]);
-        if (MODE == 1) bulk_g2s(dst + (NA + D) * 32, A.delta + wid * D * 32, D * 128u, &bars[s]);
-    };
-
-    if (lane == 0) {
-        for (int k = 0; k < TL_STAGES && k < uses1; ++k) issue_fwd(k);
-    }
+    uint64_t *bars = full_all[wp], *empt = empty_all[wp];
+    const int len = len_of(wp);
+    const int uses1 = uses1_of(wp);
+    auto idx = [&](int k) { return idx_of(wp, k); };
 
     float W[NA], zp[D];
 #pragma unroll
@@ -488,7 +528,7 @@ __global__ void __launch_bounds__(64) tl_solve_kernel(const __grid_constant__ TA
 #pragma unroll
         for (int r = 0; r < D; ++r) rhs[r] = st[(NA + r) * 32 + lane];
         __syncwarp(); // every lane has read the stage: it may be refilled (the copy lands long after these loads)
-        if (lane == 0 && k + TL_STAGES < uses1) issue_fwd(k + TL_STAGES);
+        if (lane == 0) mbar_arrive(&empt[s]);
         const int64_t wid = w0 + i;
         if (MODE == 0) {
             const float ci = (n == 1) ? 0.f : ((i == 0 || i == n - 1) ? 1.f : 2.f);
@@ -565,9 +605,6 @@ __global__ void __launch_bounds__(64) tl_solve_kernel(const __grid_constant__ TA
     __syncthreads();
 
     // ---- substitution outwards from the middle: x_i = z_i + w_d^2 S_i^-1 x_next = z_i - w_d^2 W_i x_next
-    if (lane == 0) {
-        for (int j = 0; j < TL_STAGES && j < len; ++j) issue_bwd(uses1 + j, idx(len - 1 - j));
-    }
     float x[D];
 #pragma unroll
     for (int r = 0; r < D; ++r) x[r] = xmid[r][lane];
@@ -586,7 +623,7 @@ __global__ void __launch_bounds__(64) tl_solve_kernel(const __grid_constant__ TA
             dold[r] = (MODE == 1) ? st[(NA + D + r) * 32 + lane] : 0.f;
         }
         __syncwarp();
-        if (lane == 0 && j + TL_STAGES < len) issue_bwd(kk + TL_STAGES, idx(len - 1 - j - TL_STAGES));
+        if (lane == 0) mbar_arrive(&empt[s]);
         float y[D];
         symv<D>(W, x, y);
         const int64_t wid = w0 + i;

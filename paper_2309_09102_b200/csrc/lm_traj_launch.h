@@ -43,18 +43,18 @@ cudaError_t launch_traj_plain_t(int which, unsigned grid, unsigned block, cudaSt
     case TK_PACK_Q: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 0); break;
     case TK_PACK_TARGETS: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 1); break;
     case TK_UNPACK: tl_unpack_kernel<D><<<grid, block, 0, s>>>(a); break;
-    case TK_SOLVE_FACTOR: { // two warps per tile of 32 trajectories; the rings need more than the default 48 KB
+    case TK_SOLVE_FACTOR: { // two chain warps + one producer warp per tile of 32 trajectories; the rings need more than the default 48 KB
         static const cudaError_t once = cudaFuncSetAttribute(tl_solve_kernel<D, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                              (int)tl_solve_smem_bytes<D, 0>());
         if (once != cudaSuccess) return once;
-        tl_solve_kernel<D, 0><<<grid, 64, tl_solve_smem_bytes<D, 0>(), s>>>(a);
+        tl_solve_kernel<D, 0><<<grid, TL_SOLVE_THREADS, tl_solve_smem_bytes<D, 0>(), s>>>(a);
         break;
     }
     case TK_SOLVE_REFINE: {
         static const cudaError_t once = cudaFuncSetAttribute(tl_solve_kernel<D, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                              (int)tl_solve_smem_bytes<D, 1>());
         if (once != cudaSuccess) return once;
-        tl_solve_kernel<D, 1><<<grid, 64, tl_solve_smem_bytes<D, 1>(), s>>>(a);
+        tl_solve_kernel<D, 1><<<grid, TL_SOLVE_THREADS, tl_solve_smem_bytes<D, 1>(), s>>>(a);
         break;
     }
     default: return cudaErrorInvalidValue;
