@@ -379,9 +379,9 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // accept / reject is per trajectory, so the lanes of a tile may select different buffers; a
 // buffer no lane of the tile selects is not fetched).
 template <int D, int MODE> __host__ __device__ constexpr int tl_stage_floats() { return (Tri<D>::NA + (MODE == 0 ? D : 2 * D)) * 32; }
-// Waypoints in flight per warp in the solve kernel.  Measured on B200 (n = 300, us per iteration at B = 4096 / 16384):
-// 2 stages 477 / 1269, 3: 441 / 1372, 4: 432 / 1266, 6: 432 / 1319, 8: 431 / 1461, 11-16: 432 / 1635.  At C4 the kernel
-// is bound by the latency of its sequential chain, not by bytes in flight, and a deeper ring only costs occupancy once
+// Waypoints in flight per chain warp in the solve kernel.  Measured on B200 (n = 300, us per iteration at B = 4096 /
+// 16384, with the producer warp): 2 stages 486 / 1276, 3: 425 / 1363, 4: 403 / 1279, 6: 393 / 1329.  At C4 the kernel
+// is bound by the latency of its sequential chain, not by bytes in flight, and a deeper ring costs occupancy once
 // there are more tiles than SMs: 4 (a power of two: the stage index is a mask).
 template <int D, int MODE> __host__ __device__ constexpr int tl_stages() {
     const size_t per_stage = (size_t)2 * (MODE == 0 ? 2 : 1) * tl_stage_floats<D, MODE>() * sizeof(float);
@@ -392,7 +392,8 @@ template <int D, int MODE> __host__ __device__ constexpr size_t tl_solve_smem_by
     return (size_t)2 * (MODE == 0 ? 2 : 1) * tl_stages<D, MODE>() * tl_stage_floats<D, MODE>() * sizeof(float);
 }
 
-// ---- block-tridiagonal solve: one block of TWO warps per tile of 32 trajectories, lane = trajectory.
+// ---- block-tridiagonal solve: one block of two chain warps (+ one producer warp) per tile of 32 trajectories,
+// lane = trajectory.
 // Two-sided ("twisted") block elimination halves the sequential chain: with m = n / 2,
 //   warp 0 eliminates i = 0, 1, .., m-1      (S_i = T_i - w_d^4 S_{i-1}^-1,  h_i = g_i + w_d^2 z_{i-1}),
 //   warp 1 eliminates i = n-1, n-2, .., m+1  (S_i = T_i - w_d^4 S_{i+1}^-1,  h_i = g_i + w_d^2 z_{i+1}),
