@@ -370,26 +370,26 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 #ifndef LM_TL_STAGE_BUDGET
 #define LM_TL_STAGE_BUDGET (200 * 1024) // shared memory one solve block may spend on its rings
 #endif
-#ifndef LM_TL_MAX_STAGES
-#define LM_TL_MAX_STAGES 4
-#endif
 
 // One ring stage (floats): [0, NA*32) matrix, then vector 1 (D*32) and, in MODE 1, vector 2 (D*32).
 // Each of the two warps of a block has its own rings; MODE 0 keeps two per warp (one per Ag buffer:
 // accept / reject is per trajectory, so the lanes of a tile may select different buffers; a
 // buffer no lane of the tile selects is not fetched).
 template <int D, int MODE> __host__ __device__ constexpr int tl_stage_floats() { return (Tri<D>::NA + (MODE == 0 ? D : 2 * D)) * 32; }
-// Waypoints in flight per chain warp in the solve kernel.  Measured on B200 (n = 300, us per iteration at B = 4096 /
-// 16384, with the producer warp): 2 stages 486 / 1276, 3: 425 / 1363, 4: 403 / 1279, 6: 393 / 1329.  At C4 the kernel
-// is bound by the latency of its sequential chain, not by bytes in flight, and a deeper ring costs occupancy once
-// there are more tiles than SMs: 4 (a power of two: the stage index is a mask).
-template <int D, int MODE> __host__ __device__ constexpr int tl_stages() {
+// Waypoints in flight per chain warp in the solve kernel: WANT, cut to what the shared-memory budget holds.  Measured
+// on B200 (n = 300, us per iteration at B = 4096 / 16384, with the producer warp): 2 stages 486 / 1276, 3: 425 / 1363,
+// 4: 403 / 1279, 6: 393 / 1329, 8: 387 / -- (8192: 707 vs 640 with 4).  A deeper ring helps while every SM holds one
+// block (the chain is latency-bound and more chunks are in flight) and costs occupancy once there are more tiles than
+// SMs: the launch takes TL_STAGES_DEEP when the tiles fit one per SM, TL_STAGES_SHALLOW otherwise (powers of two:
+// the stage index is a mask).
+constexpr int TL_STAGES_SHALLOW = 4, TL_STAGES_DEEP = 8;
+template <int D, int MODE, int WANT> __host__ __device__ constexpr int tl_stages() {
     const size_t per_stage = (size_t)2 * (MODE == 0 ? 2 : 1) * tl_stage_floats<D, MODE>() * sizeof(float);
     const int fit = (int)((size_t)LM_TL_STAGE_BUDGET / per_stage);
-    return fit > LM_TL_MAX_STAGES ? LM_TL_MAX_STAGES : fit;
+    return fit > WANT ? WANT : fit;
 }
-template <int D, int MODE> __host__ __device__ constexpr size_t tl_solve_smem_bytes() {
-    return (size_t)2 * (MODE == 0 ? 2 : 1) * tl_stages<D, MODE>() * tl_stage_floats<D, MODE>() * sizeof(float);
+template <int D, int MODE, int WANT> __host__ __device__ constexpr size_t tl_solve_smem_bytes() {
+    return (size_t)2 * (MODE == 0 ? 2 : 1) * tl_stages<D, MODE, WANT>() * tl_stage_floats<D, MODE>() * sizeof(float);
 }
 
 // ---- block-tridiagonal solve: one block of two chain warps (+ one producer warp) per tile of 32 trajectories,
@@ -402,17 +402,17 @@ template <int D, int MODE> __host__ __device__ constexpr size_t tl_solve_smem_by
 // and both substitute outwards from x_m:  x_i = z_i + w_d^2 S_i^-1 x_{i+-1}.
 //   MODE 0: factor (stores W_i = -S_i^-1) and solve for g;                      delta  = -x
 //   MODE 1: re-solve with the stored W_i for rho (iterative refinement);        delta +=  x
-// The chunks of the next tl_stages<D, MODE>() waypoints of a warp's sequence are in flight (bulk-async copies
+// The chunks of the next tl_stages<D, MODE, WANT>() waypoints of a warp's sequence are in flight (bulk-async copies
 // into its ring) while it eliminates the current one.  A THIRD warp is the producer of both rings: one of its lanes
 // waits for a stage to be released ("empty" mbarrier, armed by the consumer once all its lanes have read the stage),
 // posts the byte count on the stage's "full" mbarrier and issues the copies -- the address arithmetic, the
 // uniform-register traffic of UBLKCP and the divergent lane-0 branch (38 % of the refinement re-solve's issue slots
 // when every warp fed its own ring) are off the two sequential chains.
 constexpr int TL_SOLVE_THREADS = 96;
-template <int D, int MODE>
+template <int D, int MODE, int WANT>
 __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid_constant__ TArgs A) {
     constexpr int NA = Tri<D>::NA, CA = NA + D, SF = tl_stage_floats<D, MODE>(), NR = (MODE == 0) ? 2 : 1;
-    constexpr int TL_STAGES = tl_stages<D, MODE>();
+    constexpr int TL_STAGES = tl_stages<D, MODE, WANT>();
     extern __shared__ __align__(128) float smem[];
     __shared__ __align__(8) uint64_t full_all[2][TL_STAGES], empty_all[2][TL_STAGES];
     __shared__ float xch[NA + D][32]; // warp 1 -> warp 0: W_{m+1}, z_{m+1}

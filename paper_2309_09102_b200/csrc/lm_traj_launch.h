@@ -43,18 +43,27 @@ cudaError_t launch_traj_plain_t(int which, unsigned grid, unsigned block, cudaSt
     case TK_PACK_Q: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 0); break;
     case TK_PACK_TARGETS: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 1); break;
     case TK_UNPACK: tl_unpack_kernel<D><<<grid, block, 0, s>>>(a); break;
-    case TK_SOLVE_FACTOR: { // two chain warps + one producer warp per tile of 32 trajectories; the rings need more than the default 48 KB
-        static const cudaError_t once = cudaFuncSetAttribute(tl_solve_kernel<D, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                             (int)tl_solve_smem_bytes<D, 0>());
-        if (once != cudaSuccess) return once;
-        tl_solve_kernel<D, 0><<<grid, TL_SOLVE_THREADS, tl_solve_smem_bytes<D, 0>(), s>>>(a);
-        break;
+    case TK_SOLVE_FACTOR:  // two chain warps + one producer warp per tile of 32 trajectories; the rings need more than
+    case TK_SOLVE_REFINE: { // the default 48 KB.  Ring depth: deep while every SM holds at most one block (lm_traj.cuh)
+        int dev = 0, sms = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        const bool deep = grid <= (unsigned)sms;
+#define LM_SOLVE_LAUNCH(MODE, WANT)                                                                                          \
+    {                                                                                                                        \
+        static const cudaError_t once = cudaFuncSetAttribute(tl_solve_kernel<D, MODE, WANT>,                                 \
+                                                             cudaFuncAttributeMaxDynamicSharedMemorySize,                    \
+                                                             (int)tl_solve_smem_bytes<D, MODE, WANT>());                     \
+        if (once != cudaSuccess) return once;                                                                                \
+        tl_solve_kernel<D, MODE, WANT><<<grid, TL_SOLVE_THREADS, tl_solve_smem_bytes<D, MODE, WANT>(), s>>>(a);              \
     }
-    case TK_SOLVE_REFINE: {
-        static const cudaError_t once = cudaFuncSetAttribute(tl_solve_kernel<D, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                             (int)tl_solve_smem_bytes<D, 1>());
-        if (once != cudaSuccess) return once;
-        tl_solve_kernel<D, 1><<<grid, TL_SOLVE_THREADS, tl_solve_smem_bytes<D, 1>(), s>>>(a);
+        if (which == TK_SOLVE_FACTOR) {
+            if (deep) LM_SOLVE_LAUNCH(0, TL_STAGES_DEEP) else LM_SOLVE_LAUNCH(0, TL_STAGES_SHALLOW)
+        } else {
+            if (deep) LM_SOLVE_LAUNCH(1, TL_STAGES_DEEP) else LM_SOLVE_LAUNCH(1, TL_STAGES_SHALLOW)
+        }
+#undef LM_SOLVE_LAUNCH
         break;
     }
     default: return cudaErrorInvalidValue;
