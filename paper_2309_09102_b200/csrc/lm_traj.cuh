@@ -403,12 +403,12 @@ template <int D, int MODE, int WANT> __host__ __device__ constexpr size_t tl_sol
 //   MODE 0: factor (stores W_i = -S_i^-1) and solve for g;                      delta  = -x
 //   MODE 1: re-solve with the stored W_i for rho (iterative refinement);        delta +=  x
 // The chunks of the next tl_stages<D, MODE, WANT>() waypoints of a warp's sequence are in flight (bulk-async copies
-// into its ring) while it eliminates the current one.  A THIRD warp is the producer of both rings: one of its lanes
+// into its ring) while it eliminates the current one.  Two more warps are the producers of the two chains' rings: one lane of each
 // waits for a stage to be released ("empty" mbarrier, armed by the consumer once all its lanes have read the stage),
 // posts the byte count on the stage's "full" mbarrier and issues the copies -- the address arithmetic, the
 // uniform-register traffic of UBLKCP and the divergent lane-0 branch (38 % of the refinement re-solve's issue slots
 // when every warp fed its own ring) are off the two sequential chains.
-constexpr int TL_SOLVE_THREADS = 96;
+constexpr int TL_SOLVE_THREADS = 128;
 template <int D, int MODE, int WANT>
 __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid_constant__ TArgs A) {
     constexpr int NA = Tri<D>::NA, CA = NA + D, SF = tl_stage_floats<D, MODE>(), NR = (MODE == 0) ? 2 : 1;
@@ -418,16 +418,16 @@ __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid
     __shared__ float xch[NA + D][32]; // warp 1 -> warp 0: W_{m+1}, z_{m+1}
     __shared__ float xmid[D][32];     // warp 0 -> both: x_m
     __shared__ int okx[2][32];
-    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5; // warps 0, 1: the two chains; warp 2: the producer
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5; // warps 0, 1: the two chains; warps 2, 3: their producers
     const int64_t bt = blockIdx.x;
     const int64_t b = bt * 32 + lane;
     const bool valid = b < A.B;
     const uint32_t pk = valid ? A.its[b] : 0xffu;
     const bool active = valid && ((pk & 0xffu) < (uint32_t)A.max_total) && (MODE == 0 || A.ok[b] != 0) &&
                         (A.gate == nullptr || A.gate[b] != 0);
-    if (!__any_sync(0xffffffffu, active)) return; // the same lanes in all three warps: block-uniform
+    if (!__any_sync(0xffffffffu, active)) return; // the same lanes in all four warps: block-uniform
     const int sel = valid ? A.sel[b] : 0;
-    const bool need0 = __any_sync(0xffffffffu, active && sel == 0); // warp-uniform, the same in all three warps
+    const bool need0 = __any_sync(0xffffffffu, active && sel == 0); // warp-uniform, the same in all four warps
     const bool need1 = __any_sync(0xffffffffu, active && sel == 1);
     const int n = A.n;
     const int64_t w0 = bt * n;
@@ -447,7 +447,8 @@ __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid
     }
     __syncthreads();
 
-    if (wp == 2) { // ---- the producer
+    if (wp >= 2) { // ---- the producers: warp 2 feeds the rings of warp 0, warp 3 those of warp 1
+        const int q = wp - 2;
         auto ring_of = [&](int q) { return smem + (size_t)q * NR * TL_STAGES * SF; };
         auto issue_fwd = [&](int q, int k) { // k = position in warp q's sequence of ring uses
             const int s = k % TL_STAGES;
@@ -480,21 +481,15 @@ __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid
             if (k >= TL_STAGES) mbar_wait(&empty_all[q][k % TL_STAGES], (uint32_t)(((k / TL_STAGES) - 1) & 1));
         };
         if (lane == 0) {
-            const int u0 = uses1_of(0), u1 = uses1_of(1);
-            for (int k = 0; k < u0 || k < u1; ++k) {
-                if (k < u0) { wait_free(0, k); issue_fwd(0, k); }
-                if (k < u1) { wait_free(1, k); issue_fwd(1, k); }
-            }
+            const int u = uses1_of(q);
+            for (int k = 0; k < u; ++k) { wait_free(q, k); issue_fwd(q, k); }
         }
         __syncthreads(); // (1) warp 1 has handed its last block to warp 0
         __syncthreads(); // (2) the chunks written by the elimination are ordered before the copies below
         fence_proxy_async();
         if (lane == 0) {
-            const int l0 = len_of(0), l1 = len_of(1), u0 = uses1_of(0), u1 = uses1_of(1);
-            for (int j = 0; j < l0 || j < l1; ++j) {
-                if (j < l0) { wait_free(0, u0 + j); issue_bwd(0, u0 + j, idx_of(0, l0 - 1 - j)); }
-                if (j < l1) { wait_free(1, u1 + j); issue_bwd(1, u1 + j, idx_of(1, l1 - 1 - j)); }
-            }
+            const int l = len_of(q), u = uses1_of(q);
+            for (int j = 0; j < l; ++j) { wait_free(q, u + j); issue_bwd(q, u + j, idx_of(q, l - 1 - j)); }
         }
         __syncthreads(); // (3) the verdicts of the two chains
         return;
