@@ -392,7 +392,7 @@ template <int D, int MODE, int WANT> __host__ __device__ constexpr size_t tl_sol
     return (size_t)2 * (MODE == 0 ? 2 : 1) * tl_stages<D, MODE, WANT>() * tl_stage_floats<D, MODE>() * sizeof(float);
 }
 
-// ---- block-tridiagonal solve: one block of two chain warps (+ one producer warp) per tile of 32 trajectories,
+// ---- block-tridiagonal solve: one block of two chain warps (+ their two producer warps) per tile of 32 trajectories,
 // lane = trajectory.
 // Two-sided ("twisted") block elimination halves the sequential chain: with m = n / 2,
 //   warp 0 eliminates i = 0, 1, .., m-1      (S_i = T_i - w_d^4 S_{i-1}^-1,  h_i = g_i + w_d^2 z_{i-1}),

@@ -43,7 +43,7 @@ cudaError_t launch_traj_plain_t(int which, unsigned grid, unsigned block, cudaSt
     case TK_PACK_Q: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 0); break;
     case TK_PACK_TARGETS: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 1); break;
     case TK_UNPACK: tl_unpack_kernel<D><<<grid, block, 0, s>>>(a); break;
-    case TK_SOLVE_FACTOR:  // two chain warps + one producer warp per tile of 32 trajectories; the rings need more than
+    case TK_SOLVE_FACTOR:  // two chain warps + two producer warps per tile of 32 trajectories; the rings need more than
     case TK_SOLVE_REFINE: { // the default 48 KB.  Ring depth: deep while every SM holds at most one block (lm_traj.cuh)
         int dev = 0, sms = 0;
         cudaError_t e = cudaGetDevice(&dev);
