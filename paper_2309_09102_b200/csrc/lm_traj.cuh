@@ -372,7 +372,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 #endif
 
 // One ring stage (floats): [0, NA*32) matrix, then vector 1 (D*32) and, in MODE 1, vector 2 (D*32).
-// Each of the two warps of a block has its own rings; MODE 0 keeps two per warp (one per Ag buffer:
+// Each of the two chain warps of a block has its own rings; MODE 0 keeps two per warp (one per Ag buffer:
 // accept / reject is per trajectory, so the lanes of a tile may select different buffers; a
 // buffer no lane of the tile selects is not fetched).
 template <int D, int MODE> __host__ __device__ constexpr int tl_stage_floats() { return (Tri<D>::NA + (MODE == 0 ? D : 2 * D)) * 32; }

@@ -60,7 +60,7 @@ cudaError_t launch_pose(lm_ctx *c, int which, const TArgs &a) {
 
 cudaError_t launch_plain(lm_ctx *c, int which, const TArgs &a) {
     launch_counter().fetch_add(1);
-    if (which == TK_SOLVE_FACTOR || which == TK_SOLVE_REFINE) // one block (two warps) per tile of 32 trajectories
+    if (which == TK_SOLVE_FACTOR || which == TK_SOLVE_REFINE) // one block (two chain warps + their producer warps) per tile of 32 trajectories
         return launch_traj_plain(which, c->dof, (unsigned)a.Bt, 64, c->stream, a);
     const unsigned block = 256, grid = (unsigned)((a.nS + block - 1) / block);
     return launch_traj_plain(which, c->dof, grid, block, c->stream, a);
