@@ -111,3 +111,14 @@ def test_search_rejects_bad_arguments():
         lm.lm_search(s._ctx, lm.lm_search_default_params(), ptr + 4, nbytes, None, None, None)
     s.close()
     assert lm.lm_search_workspace_bytes(7, 1025, 10) == 0 and lm.lm_search_workspace_bytes(9, 10, 10) == 0
+
+
+def test_search_random_shapes():
+    """Twelve seeded (K, n) pairs on both chains, with near-limit nodes and (every fourth) quantised inputs: the GPU's
+    choice / xi / cost / mjac stay bit-identical to the fp32 oracle whatever the cluster slicing (KC, G, padding)."""
+    chains = (wl.panda_chain(), wl.random_chain_8dof(3))
+    for seed in range(100, 112):
+        rng = np.random.default_rng(seed)
+        K, n = int(rng.integers(1, 200)), int(rng.integers(1, 120))
+        ch = chains[seed % 2]
+        check(ch, candidates(ch, K, n, seed, limit_frac=0.05 * (seed % 3), quant=(0.125 if seed % 4 == 0 else None)))
