@@ -47,6 +47,9 @@ NCU_DRAM_TRAFFIC = {("C4", "panda7"): 68.849e6 + 27.575e6}
 # the same capture: 2 x 532.9 + 165.6 + 68.2): fewer than the algorithmic count because multiplications by the
 # structural zeros / ones of the Panda chain are folded out.
 NCU_EXECUTED_FLOP = {("C4", "panda7"): 1300.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of the four big kernels of ONE trajectory-level iteration on C4 (solve<0>,
+# rho, solve<1>, trial; an iteration in which ~30 % of the trajectories rejected), profiles/r1h_traj_full.md
+NCU_TRAJ_DRAM_TRAFFIC = {"C4": (477.025 + 190.604 + 137.713 + 21.786 + 314.961 + 55.676 + 448.207 + 379.615) * 1e6}
 
 
 def load_peaks() -> dict:
@@ -464,7 +467,8 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
            "cost_diff_mean": float(g["cost_diff"].mean()), "with_self_collision_rows": coll,
            "without_refinement": norefine,
            "roofline": {"bound": "hbm", "achieved": alg / (ms_iter * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                        "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"], "traffic": None,
+                        "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                        "traffic": NCU_TRAJ_DRAM_TRAFFIC.get(w.name.split(":")[0]) if (w.B, w.n) == (4096, 300) else None,
                         "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps)),
                         "peak_source": peaks["_source"]}}
     try:
