@@ -32,11 +32,14 @@ def penalties(q, q_lo, q_hi, joint_type, clearance=None, margin_rev=np.deg2rad(1
     return pen
 
 
-def search(q, pen, dtype=np.float64):
+def search(q, pen, dtype=np.float64, return_table=False):
     """q [K, n, d], pen [n, K] -> (choice [n] int, xi [n, d], cost, mjac of xi).  Plain DP, S1-S3.
     dtype: the precision every subtraction and addition is rounded to (max and < are exact).  The choice is an
-    argmin decided by floating point, so the parity test takes the decision in the kernel's precision
-    (dtype=np.float32 on fp32 inputs); the pins run in fp64."""
+    argmin decided by floating point, so the bit-for-bit parity test takes the decision in the kernel's precision
+    (dtype=np.float32 on fp32 inputs).  The fp64 mode is pinned to brute force over all K^n paths; the fp32 mode is
+    pinned to the fp64 mode (tests/test_oracle_search.py: cost within the rounding bound, identical choices on
+    instances without near-ties), and the GPU's choice is ALSO judged by its fp64 path cost (path_cost below).
+    return_table: also return the node costs c [n, K] and predecessors pred [n, K]."""
     q = np.asarray(q, dtype)
     pen = np.asarray(pen, dtype)
     K, n, d = q.shape
@@ -56,7 +59,21 @@ def search(q, pen, dtype=np.float64):
         choice[i - 1] = pred[i, choice[i]]
     xi = q[choice, np.arange(n)]
     mj = float(np.abs(np.diff(xi, axis=0)).max()) if n > 1 else 0.0
+    if return_table:
+        return choice, xi, float(c[n - 1, choice[n - 1]]), mj, c, pred
     return choice, xi, float(c[n - 1, choice[n - 1]]), mj
+
+
+def path_cost(q, pen, choice):
+    """S1 cost of ONE given path (choice [n]) in fp64, straight from the definition: the running maximum of the
+    steps plus the penalties of the nodes it visits.  Judges a path without trusting whoever found it."""
+    q = np.asarray(q, np.float64)
+    pen = np.asarray(pen, np.float64)
+    n = q.shape[1]
+    c = pen[0, choice[0]]
+    for i in range(1, n):
+        c = max(c, np.abs(q[choice[i], i] - q[choice[i - 1], i - 1]).max()) + pen[i, choice[i]]
+    return float(c)
 
 
 def brute_force(q, pen):

@@ -149,7 +149,7 @@ int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_
     c->dof = d; c->B = pb->B; c->n = pb->n; c->W = pb->B * pb->n; c->shared = pb->shared_targets ? 1 : 0;
     c->lay = lay; c->ws = static_cast<char *>(pb->workspace);
     c->stream = static_cast<cudaStream_t>(cuda_stream);
-    c->fresh = true; c->block = 128; c->fast = prm->fast_sincos != 0;
+    c->fresh = true; c->stale = false; c->block = 128; c->fast = prm->fast_sincos != 0;
 
     KArgs &a = c->args;
     std::memset(&a, 0, sizeof(a));
@@ -237,6 +237,7 @@ int iterate(lm_ctx *c, int max_total, int at_most) {
     cudaError_t e = launch_iterate(c, a);
     if (e != cudaSuccess) return cuda_fail(e);
     c->fresh = false;
+    c->stale = false; // every launch re-evaluates |r|, the errors and the frozen flag at the state it loads
     return LM_OK;
 }
 
@@ -399,6 +400,7 @@ int lm_set_state(lm_ctx *c, const float *q, const float *lambda) {
                                                       c->args.lambda0, lambda ? 0 : 1);
     LM_CUDA(cudaGetLastError());
     c->fresh = false;
+    c->stale = true; // res_norm / pos_err / rot_err / status still describe the previous q: lm_fetch re-evaluates them
     return LM_OK;
 }
 
@@ -436,6 +438,9 @@ int lm_fetch(lm_ctx *c, float *q_out, lm_stats *s) {
     const KArgs &a = c->args;
     if (c->fresh) { // nothing has run yet: materialise the initial state so that fetch is well defined
         int rc = iterate(c, 0, 0);
+        if (rc != LM_OK) return rc;
+    } else if (c->stale) { // lm_set_state and nothing since: a zero-iteration launch evaluates the outputs at the injected q
+        int rc = iterate(c, LM_MAX_ITERS, 0);
         if (rc != LM_OK) return rc;
     }
     LM_CUDA(copy_out(q_out, a.q, 4 * W * c->dof, c->stream));

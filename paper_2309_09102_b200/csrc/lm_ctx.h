@@ -53,6 +53,7 @@ struct lm_ctx {
     char *ws;
     cudaStream_t stream;
     bool fresh;
+    bool stale;       // lm_set_state injected q: res / pos_err / rot_err / frozen flag belong to the previous q until a launch
     int block;
     bool fast;
     int spec_id;      // structure-matched specialised kernel (lm_specs.cuh) or SPEC_GENERIC

@@ -146,7 +146,11 @@ __device__ __forceinline__ void st_async_f32(uint32_t raddr, float v, uint32_t r
 // mbarrier of that layer's parity, and a CTA starts layer i+1 when all 4 K bytes of layer i have arrived: no
 // cluster-wide barrier (and no memory fence that would wait for the prefetch) inside the loop.  Two buffers and two
 // mbarriers are enough: nobody can send layer i+1 before it has received every node of layer i, i.e. before every
-// owner has finished reading layer i-1.  The edge costs do not depend on the DP, so the first NB per lane of the
+// owner has finished reading layer i-1.  That argument paces OWNERS only, so only CTAs and warps that own a node
+// take part in the layer loop: a CTA without nodes (K <= 7; K = 9 gives KC = 2 and ranks 5-7 empty) is sent nothing
+// and a warp without nodes (the tail of the last active rank) never waits -- nobody would wait for either, and one
+// that fell two layers behind would see layer i+2 counted on the mbarrier phase of layer i.  Both go straight to
+// the cluster barrier after the loop.  The edge costs do not depend on the DP, so the first NB per lane of the
 // NEXT layer are loaded before the wait and their L2 latency hides behind it.  Predecessors stay in the owner's
 // shared memory and are gathered into CTA 0 after the last layer (or go to global memory when n * K of them do not
 // fit); CTA 0 picks the end node, walks back and gathers xi_search.
@@ -165,6 +169,9 @@ __global__ void __launch_bounds__(DP_THREADS) search_dp_kernel(const SArgs A) {
     const int k = rank * KC + kl;
     const bool node = kl < KC && k < K;
     const bool owner = node && g == 0;
+    const int nact = (K + KC - 1) / KC;                         // ranks 0 .. nact-1 own nodes (rank 0 always does)
+    const int kw = rank * KC + (t & ~31) / G;                   // first node of this warp: the warp takes part in the
+    const bool in_loop = rank < nact && (t & ~31) / G < KC && kw < K; // layer loop iff it owns at least one node
     const float INF = __int_as_float(0x7f800000);
     if (t == 0) {
         mbar_init(&bars[0], 1);
@@ -195,7 +202,7 @@ __global__ void __launch_bounds__(DP_THREADS) search_dp_kernel(const SArgs A) {
         if (owner) pn = __ldg(A.pen + (size_t)K + k);
     }
     cl.sync(); // mbarriers initialised everywhere, c[0] in place
-    for (int i = 1; i < n; ++i) {
+    for (int i = 1; in_loop && i < n; ++i) { // in_loop is warp-uniform; thread 0 (node 0 of its rank) is always in
         const int par = i & 1;
         if (t == 0) mbar_expect_tx(&bars[par], 4u * (uint32_t)K); // layer i: one 4-byte store per node, from its owner
         const float *cprev = (par ? c0 : c1) + g;
@@ -221,7 +228,8 @@ __global__ void __launch_bounds__(DP_THREADS) search_dp_kernel(const SArgs A) {
             const float cnew = __fadd_rn(best, pn);
             const uint32_t shift = par ? 4u * (uint32_t)KP : 0u, bshift = par ? 8u : 0u;
 #pragma unroll
-            for (int r = 0; r < DP_CLUSTER; ++r) st_async_f32(rdst[r] + shift, cnew, rbar[r] + bshift);
+            for (int r = 0; r < DP_CLUSTER; ++r)
+                if (r < nact) st_async_f32(rdst[r] + shift, cnew, rbar[r] + bshift);
             if (A.pred_in_smem) pred_mine[(size_t)i * KC + kl] = (uint16_t)arg;
             else A.pred[(size_t)i * K + k] = (uint16_t)arg;
         }

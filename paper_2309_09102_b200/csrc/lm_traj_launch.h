@@ -52,10 +52,10 @@ cudaError_t launch_traj_plain_t(int which, unsigned grid, unsigned block, cudaSt
         const bool deep = grid <= (unsigned)sms;
 #define LM_SOLVE_LAUNCH(MODE, WANT)                                                                                          \
     {                                                                                                                        \
-        static const cudaError_t once = cudaFuncSetAttribute(tl_solve_kernel<D, MODE, WANT>,                                 \
-                                                             cudaFuncAttributeMaxDynamicSharedMemorySize,                    \
-                                                             (int)tl_solve_smem_bytes<D, MODE, WANT>());                     \
-        if (once != cudaSuccess) return once;                                                                                \
+        /* the attribute is per DEVICE: set it on every launch (cheap), never once per process */                           \
+        e = cudaFuncSetAttribute(tl_solve_kernel<D, MODE, WANT>, cudaFuncAttributeMaxDynamicSharedMemorySize,                \
+                                 (int)tl_solve_smem_bytes<D, MODE, WANT>());                                                 \
+        if (e != cudaSuccess) return e;                                                                                      \
         tl_solve_kernel<D, MODE, WANT><<<grid, TL_SOLVE_THREADS, tl_solve_smem_bytes<D, MODE, WANT>(), s>>>(a);              \
     }
         if (which == TK_SOLVE_FACTOR) {

@@ -432,7 +432,7 @@ class Solver:
             t = torch.from_numpy(np.ascontiguousarray(np.asarray(x, dtype=np.float32).T))
             return t.pin_memory() if self.host_inputs else t.to(self.device)
 
-        with torch.cuda.device(self.device):
+        with torch.cuda.device(self.device), self._on_stream():
             self.tp, self.tq, self.seeds = soa(target_pos), soa(target_quat), soa(seeds)
             mem = LM_MEM_HOST if self.host_inputs else LM_MEM_DEVICE
             nbytes = lm_workspace_bytes(self.d, self.B, self.n, int(self.shared), mem)
@@ -444,6 +444,15 @@ class Solver:
             s = stream if stream is not None else torch.cuda.current_stream(self.device)
             self._stream_handle = int(s.cuda_stream)
             self._ctx = lm_init(self._cchain, pb, self.params, self._stream_handle)
+
+    def _on_stream(self):
+        """Uploads and allocations happen on the stream the library launches on: with a caller-supplied
+        (possibly non-blocking) stream nothing else orders an H2D upload before the library's use of it, or the
+        caching allocator's reuse of a freed block after it."""
+        import contextlib
+        if self.stream is None:
+            return contextlib.nullcontext()
+        return self.torch.cuda.stream(self.stream)
 
     # -- the hot path
     def step(self) -> None:
@@ -468,14 +477,16 @@ class Solver:
     def set_state(self, q, lam=None) -> None:
         """q [W,d], lam [W] numpy (waypoint-major)."""
         torch = self.torch
-        self._q_in = torch.from_numpy(np.ascontiguousarray(np.asarray(q, dtype=np.float32).T)).to(self.device)
-        self._lam_in = None if lam is None else torch.from_numpy(np.ascontiguousarray(lam, dtype=np.float32)).to(self.device)
+        with self._on_stream():
+            self._q_in = torch.from_numpy(np.ascontiguousarray(np.asarray(q, dtype=np.float32).T)).to(self.device)
+            self._lam_in = None if lam is None else torch.from_numpy(np.ascontiguousarray(lam, dtype=np.float32)).to(self.device)
         lm_set_state(self._ctx, self._q_in.data_ptr(), None if lam is None else self._lam_in.data_ptr())
 
     def enable_trace(self) -> None:
         torch = self.torch
-        self.trace_q = torch.full((self.d, self.W), float("nan"), dtype=torch.float32, device=self.device)
-        self.trace_F = torch.full((2, self.W), float("nan"), dtype=torch.float32, device=self.device)
+        with self._on_stream():
+            self.trace_q = torch.full((self.d, self.W), float("nan"), dtype=torch.float32, device=self.device)
+            self.trace_F = torch.full((2, self.W), float("nan"), dtype=torch.float32, device=self.device)
         lm_set_trace(self._ctx, self.trace_q.data_ptr(), self.trace_F.data_ptr())
 
     def fetch(self, host: bool = True) -> dict:
@@ -487,7 +498,8 @@ class Solver:
         def buf(shape, dtype):
             if host:
                 return torch.empty(shape, dtype=dtype).pin_memory()
-            return torch.empty(shape, dtype=dtype, device=self.device)
+            with self._on_stream():
+                return torch.empty(shape, dtype=dtype, device=self.device)
 
         out = {"q": buf((d, W), torch.float32), "res_norm": buf((W,), torch.float32),
                "pos_err": buf((W,), torch.float32), "rot_err": buf((W,), torch.float32),
@@ -497,7 +509,7 @@ class Solver:
         st = LmStats(out["res_norm"].data_ptr(), out["pos_err"].data_ptr(), out["rot_err"].data_ptr(),
                      out["lam"].data_ptr(), out["iters"].data_ptr(), out["mask"].data_ptr(),
                      out["status"].data_ptr(), out["traj_converged"].data_ptr(), out["traj_iters"].data_ptr(), 0, 0)
-        lm_fetch(self._ctx, out["q"].data_ptr(), st)
+        lm_fetch(self._ctx, out["q"].data_ptr(), st)      # synchronises the library's stream
         res = {k: v.cpu().numpy() for k, v in out.items()}
         res["q"] = np.ascontiguousarray(res["q"].T)
         res["mask"] = res["mask"].view(np.uint64)
@@ -515,7 +527,8 @@ class Solver:
         torch = self.torch
         self.tparams = tparams if tparams is not None else lm_traj_default_params()
         nbytes = lm_traj_workspace_bytes(self.d, self.B, self.n)
-        self.traj_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        with self._on_stream():
+            self.traj_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (self.traj_workspace.data_ptr() + 255) // 256 * 256
         lm_traj_attach(self._ctx, self.tparams, ptr, nbytes)
 
@@ -533,13 +546,15 @@ class Solver:
         if lam is None:
             lm_traj_reset(self._ctx, None)
         else:
-            self._tlam_in = self.torch.from_numpy(np.ascontiguousarray(lam, dtype=np.float32)).to(self.device)
+            with self._on_stream():
+                self._tlam_in = self.torch.from_numpy(np.ascontiguousarray(lam, dtype=np.float32)).to(self.device)
             lm_traj_reset(self._ctx, self._tlam_in.data_ptr())
 
     def traj_enable_trace(self) -> None:
         torch = self.torch
-        self.ttrace_q = torch.full((self.d, self.W), float("nan"), dtype=torch.float32, device=self.device)
-        self.ttrace_F = torch.full((2, self.B), float("nan"), dtype=torch.float32, device=self.device)
+        with self._on_stream():
+            self.ttrace_q = torch.full((self.d, self.W), float("nan"), dtype=torch.float32, device=self.device)
+            self.ttrace_F = torch.full((2, self.B), float("nan"), dtype=torch.float32, device=self.device)
         lm_traj_set_trace(self._ctx, self.ttrace_q.data_ptr(), self.ttrace_F.data_ptr())
 
     def traj_fetch(self) -> dict:
@@ -572,7 +587,8 @@ class Solver:
         torch = self.torch
         self.pparams = pparams if pparams is not None else lm_plan_default_params()
         nbytes = lm_plan_workspace_bytes(self.d, self.B, self.n)
-        self.plan_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        with self._on_stream():
+            self.plan_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (self.plan_workspace.data_ptr() + 255) // 256 * 256
         lm_plan_attach(self._ctx, self.pparams, ptr, nbytes)
 
@@ -606,7 +622,8 @@ class Solver:
         sparams = sparams if sparams is not None else lm_search_default_params()
         nbytes = lm_search_workspace_bytes(self.d, self.B, self.n)
         if getattr(self, "search_workspace", None) is None or self.search_workspace.numel() < nbytes + 256:
-            self.search_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            with self._on_stream():
+                self.search_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (self.search_workspace.data_ptr() + 255) // 256 * 256
         if not to_host:
             lm_search(self._ctx, sparams, ptr, nbytes, None, None, None)
@@ -628,9 +645,10 @@ class Solver:
         torch = self.torch
         q = np.asarray(q, dtype=np.float32)
         count = q.shape[0]
-        qd = torch.from_numpy(np.ascontiguousarray(q.T)).to(self.device)
-        pos = torch.empty((3, count), dtype=torch.float32, device=self.device)
-        rot = torch.empty((9, count), dtype=torch.float32, device=self.device)
+        with self._on_stream():
+            qd = torch.from_numpy(np.ascontiguousarray(q.T)).to(self.device)
+            pos = torch.empty((3, count), dtype=torch.float32, device=self.device)
+            rot = torch.empty((9, count), dtype=torch.float32, device=self.device)
         lm_fk(self._ctx, qd.data_ptr(), count, pos.data_ptr(), rot.data_ptr())
         torch.cuda.synchronize(self.device)
         return (pos.cpu().numpy().T.astype(np.float64),

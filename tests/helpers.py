@@ -9,6 +9,19 @@ from paper_2309_09102_b200 import workloads as wl
 TOL_Q = 1e-4      # rad (m for prismatic) per joint        -- BASELINE.json north_star
 TOL_POS = 1e-5    # m, pose error after a fixed iteration count
 TOL_ROT = 1e-4    # rad
+FLOOR = 1e-5      # |r| below which accept/reject is no longer compared (the fp32 floor region)
+EPS_POSE = 5e-7   # abs error of an fp32 pose residual norm: 7-8 joints x ulp(1) ~ 2e-7 in position and in rotation
+
+
+def decisive(F_before, F_trial, floor: float = FLOOR, margin: float = 1e-3):
+    """The ORACLE's decision between F and F+ is one fp32 arithmetic must reproduce (P9/P10):
+    |r| is above the floor, the relative margin exceeds 1e-3 AND the absolute margin exceeds the fp32
+    noise of the comparison itself: F = |r|^2 carries an error of 2 |r| EPS_POSE on either side, so F - F+ is only
+    known to 4 |r| EPS_POSE.  (At |r| = 2e-4 a 0.4 % decrease of F is 2e-10, the noise is 4e-10: such a step is
+    accepted by one side and rejected by the other at random -- measured on configs[3], waypoint 7086 of the sample.)"""
+    r = np.sqrt(F_before)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        return (r >= floor) & (np.abs(F_before - F_trial) > np.maximum(margin * F_before, 4.0 * EPS_POSE * r))
 
 
 def oracle_fk(chain):
@@ -73,8 +86,7 @@ def oracle_trace(w: wl.Workload, n_iters: int, **kw):
 
 def decisive_mismatches(w: wl.Workload, gpu: dict, n_iters: int, floor: float = 1e-5, margin: float = 1e-3, **kw):
     """Compare accept/reject bits on the decisive iterations (P10): both sides
-    executed iteration k, the oracle's sqrt(F) before it was >= floor, and the oracle's own
-    decision had relative margin |F - F+| / F > margin.  Stops at the first mismatch of a
+    executed iteration k and the oracle's own decision was decisive (see `decisive`).  Stops at the first mismatch of a
     waypoint (after it the two sequences are different problems).
     Returns (number of decisive decisions compared, number of waypoints with a mismatch)."""
     tr = oracle_trace(w, n_iters, **kw)
@@ -85,8 +97,7 @@ def decisive_mismatches(w: wl.Workload, gpu: dict, n_iters: int, floor: float = 
         ran_o = a.accepted >= 0                      # oracle executed iteration k
         ran_g = gpu["iters"] > k
         Fb, Ft = a.F_before, a.F_trial
-        with np.errstate(invalid="ignore", divide="ignore"):
-            dec = ran_o & ran_g & alive & (np.sqrt(Fb) >= floor) & (np.abs(Fb - Ft) > margin * Fb)
+        dec = ran_o & ran_g & alive & decisive(Fb, Ft, floor, margin)
         mism = dec & ((a.accepted == 1) != gbits[:, k])
         compared += int(dec.sum())
         bad |= mism
@@ -94,3 +105,73 @@ def decisive_mismatches(w: wl.Workload, gpu: dict, n_iters: int, floor: float = 
         alive &= ~(ran_o & ran_g & ((a.accepted == 1) != gbits[:, k]))
         alive &= ran_o & ran_g
     return compared, int(bad.sum())
+
+
+def oracle_spread(w: wl.Workload, o: orc.State, n_iters: int, eps: float = 1e-6, draws: int = 3, seed: int = 0, **kw) -> np.ndarray:
+    """How far the ORACLE's own result moves when its seeds move by eps (N(0, eps) per joint, `draws` independent
+    draws; fp64 throughout): [W] max-abs change of the final joints.  eps = 1e-6 is the size of ONE fp32 LM step's
+    error (P9) and a few ulps of the fp32 inputs, so a waypoint whose spread exceeds the 1e-4 bar is one whose result
+    the ALGORITHM does not determine to 1e-4 from fp32 data -- an unreachable / clamped target whose limit point slides
+    along the self-motion manifold ("C4").  Computed from the oracle alone."""
+    rng = np.random.default_rng(seed)
+    prm = oracle_params(w, **kw)
+    tp, tq = w.target_pos.astype(np.float64), w.target_quat.astype(np.float64)
+    spread = np.zeros(w.W)
+    for _ in range(draws):
+        seeds = w.seeds.astype(np.float64) + eps * rng.normal(size=w.seeds.shape)
+        o2 = orc.lm_run(w.chain, prm, tp, tq, seeds, n_iters)
+        spread = np.maximum(spread, np.abs(o2.q - o.q).max(axis=1))
+    return spread
+
+
+WELL_CONDITIONED = 2e-5   # the oracle's result moves by no more than this under the two tests below
+
+
+def oracle_travel_below_fp32(tr, o: orc.State, resolve: float = 1e-6) -> np.ndarray:
+    """[W] how far the ORACLE's own iterates still move after its residual has fallen below what an fp32 pose can
+    resolve (|r| < 1e-6 ~ 2 EPS_POSE): max_k |q_k - q_final| from that iteration on.  Quadratic convergence leaves
+    ~0; a target on the edge of the workspace converges linearly along a near-singular direction and keeps moving
+    q by 1e-5 per iteration while |r| is already 1e-7 -- fp32 stalls there (measured: sample waypoint 4057)."""
+    W = o.q.shape[0]
+    res_after = np.stack([np.sqrt(a.F_before) for _, a in tr][1:] + [o.res_norm], 1)      # |r| after iteration k
+    oq = np.stack([a.q for _, a in tr])
+    travel = np.zeros(W)
+    first = np.argmax(res_after < resolve, axis=1)
+    has = (res_after < resolve).any(axis=1)
+    for wi in np.where(has)[0]:
+        travel[wi] = np.abs(oq[first[wi]:, wi] - o.q[wi]).max()
+    return travel
+
+
+def check_chaotic_config(w: wl.Workload, g: dict, o: orc.State, n_iters: int, min_clear: float = 0.3) -> dict:
+    """Free-running protocol for configs[3] (far seeds): `g` = GPU outputs for exactly the
+    waypoints of `w`.  Every set below is chosen from the ORACLE alone.
+      clear  = every oracle decision above the 1e-5 floor is decisive (see `decisive`);
+      well   = clear, the oracle's result moves by <= 2e-5 under a 1e-6 perturbation of its seeds (oracle_spread)
+               and by <= 2e-5 after its residual is below fp32 resolution (oracle_travel_below_fp32).
+    Asserted: on ALL clear waypoints the accept/reject sequence is identical (no allowance) and |r| agrees to 5e-6;
+    on ALL well-conditioned ones every joint is within 1e-4; on the ill-conditioned rest of the clear set (a few %)
+    the joints stay within the oracle's own spread / travel.  Returns the counts (printed by the tests)."""
+    tr = oracle_trace(w, n_iters)
+    Fb = np.stack([a.F_before for _, a in tr], 1)
+    Ft = np.stack([a.F_trial for _, a in tr], 1)
+    floor = np.sqrt(Fb) >= FLOOR
+    clear = np.all(decisive(Fb, Ft) | ~floor, axis=1)
+    same = np.all((mask_bits(o.mask, n_iters) == mask_bits(g["mask"], n_iters)) | ~floor, axis=1)
+    dq = np.abs(g["q"] - o.q).max(axis=1)
+    wobble = np.maximum(oracle_spread(w, o, n_iters), oracle_travel_below_fp32(tr, o))
+    well = clear & (wobble <= WELL_CONDITIONED)
+    ill = clear & ~well
+    rep = {"waypoints": int(w.W), "clear": int(clear.sum()), "sequence_mismatches_among_clear": int((clear & ~same).sum()),
+           "well_conditioned": int(well.sum()), "ill_conditioned": int(ill.sum()),
+           "max_dq_well": float(dq[well].max()) if well.any() else 0.0,
+           "max_dq_ill": float(dq[ill].max()) if ill.any() else 0.0,
+           "over_bar_among_clear": int((dq[clear] > TOL_Q).sum())}
+    print("chaotic-config parity:", rep)
+    assert clear.mean() > min_clear, rep
+    assert rep["sequence_mismatches_among_clear"] == 0, rep
+    assert np.abs(g["res_norm"] - o.res_norm)[clear].max() <= 5e-6, rep
+    assert rep["max_dq_well"] <= TOL_Q, rep
+    assert well.sum() >= 0.95 * clear.sum(), rep          # ill-conditioning is the exception, not an escape hatch
+    assert np.all(dq[ill] <= np.maximum(TOL_Q, wobble[ill])), rep
+    return rep

@@ -121,26 +121,15 @@ def test_config3_eight_dof_prismatic(lm):
 
 
 def test_config4_chaotic_far_seeds(lm):
-    """configs[3] (far seeds, unreachable path ends): fp32 and fp64 sequences part on a few % of
-    the waypoints whatever the solver.  Graded as: strict parity on the
-    waypoints whose oracle decisions are all decisive, plus agreement of the aggregate statistics."""
+    """configs[3] (far seeds, unreachable path ends): 44 % of the decisions are rejects and fp32 / fp64 sequences
+    part on a few % of the waypoints whatever the solver.  Graded by H.check_chaotic_config:
+    STRICT sequence parity on every waypoint whose oracle decisions are all clear-cut, strict 1e-4 joint parity on
+    every such waypoint the oracle itself determines to 2e-5 (the others are shown ill-conditioned from the oracle
+    alone and must stay inside its spread), plus agreement of the aggregate statistics of the whole batch."""
     w = wl.config4(H.oracle_fk(wl.panda_chain()), B=64, n=300)
     g, o = H.run_gpu(w), H.run_oracle(w)
     assert np.all(g["iters"] == 50)
-    tr = H.oracle_trace(w, 50)
-    Fb = np.stack([a.F_before for _, a in tr], 1)
-    Ft = np.stack([a.F_trial for _, a in tr], 1)
-    clear = np.all((np.abs(Fb - Ft) > 1e-3 * Fb) | (np.sqrt(Fb) < 1e-5), axis=1)
-    obits = H.mask_bits(o.mask, 50)
-    gbits = H.mask_bits(g["mask"], 50)
-    floor = np.sqrt(Fb) >= 1e-5
-    same = np.all((obits == gbits) | ~floor, axis=1)
-    assert clear.mean() > 0.3
-    # every waypoint with clear-cut oracle decisions follows the same accept/reject sequence ...
-    assert same[clear].mean() > 0.995, same[clear].mean()
-    # ... and lands on the same joints
-    dq = np.abs(g["q"] - o.q).max(axis=1)
-    assert np.percentile(dq[clear & same], 99.5) <= H.TOL_Q
+    H.check_chaotic_config(w, g, o, 50)
     # aggregate statistics of the whole batch
     conv_g, conv_o = (g["res_norm"] < 1e-5).mean(), (o.res_norm < 1e-5).mean()
     assert abs(conv_g - conv_o) <= 0.005
@@ -183,7 +172,7 @@ def test_teacher_forced_steps(lm, cfg):
         worst = max(worst, d[sig].max())
         # |r| agrees to the fp32 floor of the pose (~1e-7 m / rad per component)
         assert np.abs(np.sqrt(g["F_before"][sig]) - np.sqrt(st.F_before[sig])).max() <= 1e-6
-        dec = sig & (np.abs(st.F_before - st.F_trial) > 1e-3 * st.F_before)
+        dec = sig & H.decisive(st.F_before, st.F_trial)
         acc_g = (g["mask"] & np.uint64(1)) == 1
         decided += int(dec.sum())
         mism += int((dec & (acc_g != (st.accepted == 1))).sum())
@@ -261,15 +250,8 @@ def test_config4_full_size_sampled(lm):
     idx = (pick[:, None] * w.n + np.arange(w.n)[None, :]).ravel()
     sub = wl.Workload(w.name, w.chain, len(pick), w.n, w.target_pos[idx], w.target_quat[idx], w.seeds[idx], w.tol, w.max_iters)
     o = H.run_oracle(sub)
-    tr = H.oracle_trace(sub, 50)
-    Fb = np.stack([a.F_before for _, a in tr], 1)
-    Ft = np.stack([a.F_trial for _, a in tr], 1)
-    clear = np.all((np.abs(Fb - Ft) > 1e-3 * Fb) | (np.sqrt(Fb) < 1e-5), axis=1)
-    floor = np.sqrt(Fb) >= 1e-5
-    same = np.all((H.mask_bits(o.mask, 50) == H.mask_bits(g["mask"][idx], 50)) | ~floor, axis=1)
-    assert clear.mean() > 0.3 and same[clear].mean() > 0.995
-    dq = np.abs(g["q"][idx] - o.q).max(axis=1)
-    assert np.percentile(dq[clear & same], 99.5) <= H.TOL_Q
+    gs = {k: v[idx] for k, v in g.items() if isinstance(v, np.ndarray) and v.shape[:1] == (w.W,)}
+    H.check_chaotic_config(sub, gs, o, 50)
     assert abs((g["res_norm"][idx] < 1e-5).mean() - (o.res_norm < 1e-5).mean()) <= 0.01
     # the errors the library reports are the ones its q really has (oracle FK of the GPU's q), sampled over the whole batch
     rnd = np.random.default_rng(0).choice(w.W, 4000, replace=False)

@@ -1,7 +1,15 @@
 """GPU parity of the global discrete search (lm_search, NEXT-4 iii) against oracle/lm_search_oracle.py
-(PAPER.md:L93-99).  The choice is an argmin decided by floating point, so both sides take it in fp32 (the kernel's
-precision, every operation rounded to nearest in the order the header states): choice, xi, cost and mjac are
-compared BIT FOR BIT.  Inputs are the seeds (fp32), never anything read back from the GPU."""
+(PAPER.md:L93-99).  Two checks on every case:
+
+(1) VALIDITY, independent of the kernel's precision: the S1 cost of the GPU's path, re-evaluated in fp64 by the
+    definition (sorc.path_cost), is the fp64 oracle's optimum (sorc.search in fp64: pinned to brute force over all
+    K^n paths) within twice the rounding bound of DESIGN.md section 15 -- (1 + L) * 2^-24 relative, L = number of
+    layers holding a penalised node; the reported cost and mjac are those of that path to one rounding.
+(2) The choice is an argmin decided by floating point, so it is ALSO compared bit for bit (choice, xi, cost, mjac)
+    with the oracle's fp32 mode (every subtraction / addition rounded to fp32; pinned against the fp64 mode on
+    inputs where rounding matters, tests/test_oracle_search.py).
+
+Inputs are the seeds (fp32), never anything read back from the GPU."""
 import numpy as np
 import pytest
 
@@ -39,7 +47,29 @@ def check(ch, q32, clearance=None, solver=None, sparams=None):
     assert np.array_equal(g["xi"], xi)
     assert np.float32(g["cost"]) == np.float32(cost)
     assert np.float32(g["mjac"]) == np.float32(mj)
+    validity(q32, pen, g)
     return g, pen
+
+
+U32 = 2.0 ** -24
+
+
+def validity(q32, pen, g):
+    """The fp64 path cost of the GPU's choice against the fp64 optimum (no fp32 oracle mode involved).  The penalty
+    table is an integer-valued INPUT of the DP (decided once, in fp32, by both sides)."""
+    K, n, d = q32.shape
+    q64, pen64 = q32.astype(np.float64), pen.astype(np.float64)
+    best = sorc.search(q64, pen64, dtype=np.float64)[2]
+    bound = 1.01 * (1 + int((pen64 != 0).any(axis=1).sum())) * U32
+    choice = np.asarray(g["choice"])
+    assert choice.shape == (n,) and choice.min() >= 0 and choice.max() < K
+    pc = sorc.path_cost(q64, pen64, choice)
+    assert best <= pc <= best * (1 + 2 * bound), (best, pc)
+    assert abs(float(g["cost"]) - pc) <= bound * pc
+    xi64 = q64[choice, np.arange(n)]
+    assert np.array_equal(g["xi"].astype(np.float64), xi64)
+    mj = np.abs(np.diff(xi64, axis=0)).max() if n > 1 else 0.0
+    assert abs(float(g["mjac"]) - mj) <= U32 * mj
 
 
 def test_search_matches_the_oracle_panda():

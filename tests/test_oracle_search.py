@@ -97,3 +97,90 @@ def test_fp32_mode_rounds_like_the_kernel():
     b = sorc.search(q.astype(np.float64), pen, dtype=np.float64)
     assert np.array_equal(a[0], b[0]) and a[2] == b[2] and a[3] == b[3]
     assert a[1].dtype == np.float32
+
+
+# ---------------------------------------------------------------- pins of the fp32 mode where rounding matters
+U32 = 2.0 ** -24  # unit roundoff of fp32
+
+
+def rounding_bound(pen):
+    """Relative error bound of any fp32 node cost against its fp64 value ("Precision"): the
+    inputs are fp32, a step |q_a - q_b| is ONE rounded subtraction (relative error <= u), max and min keep a relative
+    bound, adding a non-zero penalty rounds once more (adding 0 is exact) => (1 + u)^(1 + L) - 1 with L = number of
+    layers that hold a penalised node.  1 % slack for the second-order terms."""
+    L = int((np.asarray(pen) != 0).any(axis=1).sum())
+    return 1.01 * (1 + L) * U32
+
+
+def clear_cut(q, pen, c):
+    """True if no comparison the DP makes is between two DIFFERENT fp64 values closer than twice the rounding bound:
+    per layer the compared values are the previous node costs and the K x K steps, at the end the last node costs."""
+    K, n, _ = q.shape
+    tol = 2.0 * rounding_bound(pen)
+    for i in range(1, n + 1):
+        vals = [c[i - 1]]
+        if i < n:
+            vals.append(np.abs(q[:, None, i, :] - q[None, :, i - 1, :]).max(axis=2).ravel())
+        v = np.unique(np.concatenate(vals))
+        if v.size > 1 and np.min(np.diff(v) / v[1:]) <= tol:
+            return False
+    return True
+
+
+def test_fp32_mode_against_the_fp64_mode_on_inputs_where_rounding_matters():
+    """Random fp32 inputs whose differences are NOT representable: the fp32 mode's cost stays within the rounding bound
+    of the (brute-force-pinned, here exact) fp64 optimum, the path it returns is optimal within twice that bound when
+    its cost is re-evaluated in fp64 by the definition, and on instances without near-ties it is the SAME path."""
+    rng = np.random.default_rng(5)
+    same, total, inexact = 0, 0, 0
+    for trial in range(60):
+        K, n, d = int(rng.integers(2, 14)), int(rng.integers(2, 18)), int(rng.integers(1, 8))
+        if trial % 2:   # smooth candidates: neighbouring values are within a factor 2, their difference is exact (Sterbenz)
+            q = (np.cumsum(rng.normal(size=(K, n, d)) * 0.07, axis=1) + rng.normal(size=(K, 1, d)) * 0.2).astype(np.float32)
+        else:           # unrelated values of either sign: the subtraction rounds
+            q = (rng.normal(size=(K, n, d)) * 0.3).astype(np.float32)
+        pen = 10.0 * (rng.random((n, K)) < 0.15) + 100.0 * (rng.random((n, K)) < 0.03)
+        if trial % 3 == 0:
+            pen[int(rng.integers(0, n))] += 10.0            # a layer nobody can avoid: the addition rounds
+        q64 = q.astype(np.float64)
+        ch64, _, c64, _, table, _ = sorc.search(q64, pen, dtype=np.float64, return_table=True)
+        ch32, xi32, c32, mj32 = sorc.search(q, pen, dtype=np.float32)
+        b = rounding_bound(pen)
+        assert abs(c32 - c64) <= b * c64
+        pc = sorc.path_cost(q64, pen, ch32)
+        assert c64 <= pc <= c64 * (1 + 2 * b)
+        assert abs(pc - c32) <= b * pc                      # the reported cost is the (rounded) cost of the reported path
+        assert np.array_equal(xi32, q[ch32, np.arange(n)])
+        inexact += int(float(c32) != float(c64))
+        if clear_cut(q64, pen, table):
+            total += 1
+            same += int(np.array_equal(ch32, ch64))
+    assert total >= 40 and same == total
+    assert inexact >= 20                                    # rounding really was exercised
+
+
+def test_fp32_mode_against_brute_force():
+    """Tiny K^n cases with fp32 inputs: the fp64 cost of the fp32 mode's path is the brute-force optimum over all
+    paths, within twice the rounding bound."""
+    rng = np.random.default_rng(6)
+    for K, n in ((2, 6), (3, 5), (4, 4)):
+        for trial in range(15):
+            q = (rng.normal(size=(K, n, 3)) * 0.3).astype(np.float32)
+            pen = 10.0 * (rng.random((n, K)) < 0.2) + 100.0 * (rng.random((n, K)) < 0.05)
+            ch32 = sorc.search(q, pen, dtype=np.float32)[0]
+            best = sorc.brute_force(q.astype(np.float64), pen)
+            pc = sorc.path_cost(q, pen, ch32)
+            assert best <= pc <= best * (1 + 2 * rounding_bound(pen))
+
+
+def test_path_cost_is_the_definition():
+    """path_cost on a hand-made instance: steps 0.5, 0.25 and a penalised node."""
+    q = np.zeros((2, 3, 1))
+    q[0, :, 0] = [0.0, 0.5, 0.75]
+    q[1, :, 0] = [1.0, 1.0, 1.0]
+    pen = np.zeros((3, 2))
+    pen[1, 0] = 10.0
+    assert sorc.path_cost(q, pen, [0, 0, 0]) == 10.5      # max(0, .5) + 10, then max(10.5, .25)
+    assert sorc.path_cost(q, pen, [1, 1, 1]) == 0.0
+    assert sorc.path_cost(q, pen, [0, 1, 1]) == 1.0
+    assert sorc.path_cost(q, pen, [1, 1, 0]) == 0.25
