@@ -21,7 +21,13 @@ _SRC = os.path.join(_HERE, "lm_oracle.c")
 _HDR = os.path.join(_HERE, "lm_oracle.h")
 _SRCS = [_SRC, os.path.join(_HERE, "lm_traj_oracle.c"), os.path.join(_HERE, "lm_coll_oracle.c")]  # one shared object
 _DEPS = _SRCS + [_HDR, os.path.join(_HERE, "lm_traj_oracle.h"), os.path.join(_HERE, "lm_coll_oracle.h")]
-_LIB = os.path.join(_HERE, "liblm_oracle.so")
+# LM_ORACLE_SANITIZE=1: the same sources built with AddressSanitizer + UndefinedBehaviorSanitizer into a library of
+# their own.  Run the CPU pins under it with
+#   LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 LM_ORACLE_SANITIZE=1 \
+#       python -m pytest tests -m "not gpu" -q
+# (libasan must be loaded before python; leak detection is off because the interpreter itself "leaks").
+_SANITIZE = os.environ.get("LM_ORACLE_SANITIZE", "") not in ("", "0")
+_LIB = os.path.join(_HERE, "liblm_oracle_asan.so" if _SANITIZE else "liblm_oracle.so")
 MAX_DOF = 8
 
 
@@ -30,7 +36,9 @@ def build(force: bool = False) -> str:
     stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < max(os.path.getmtime(p) for p in _DEPS)
     if force or stale:
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-fPIC", "-fopenmp",
+        opt = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] \
+            if _SANITIZE else ["-O2"]
+        subprocess.check_call(["gcc"] + opt + ["-std=c11", "-Wall", "-Wextra", "-fPIC", "-fopenmp",
                                "-shared"] + _SRCS + ["-o", tmp, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB

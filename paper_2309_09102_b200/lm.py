@@ -413,7 +413,8 @@ class Solver:
     """
 
     def __init__(self, chain, B: int, n: int, target_pos, target_quat, seeds, params: Optional[LmParams] = None,
-                 shared_targets: bool = False, host_inputs: bool = False, device: str = "cuda:0", stream=None):
+                 shared_targets: bool = False, host_inputs: bool = False, device: str = "cuda:0", stream=None,
+                 guarded: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the batched-LM path has no CPU fallback")
@@ -425,6 +426,8 @@ class Solver:
         self.host_inputs = bool(host_inputs)
         self.stream = stream
         self._ctx = None
+        self.guarded = bool(guarded)      # test knob: guard bands around every workspace + poisoned interior
+        self._guards = []
         Wt = self.n if self.shared else self.W
         assert np.shape(target_pos) == (Wt, 3) and np.shape(target_quat) == (Wt, 4) and np.shape(seeds) == (self.W, self.d)
 
@@ -436,14 +439,40 @@ class Solver:
             self.tp, self.tq, self.seeds = soa(target_pos), soa(target_quat), soa(seeds)
             mem = LM_MEM_HOST if self.host_inputs else LM_MEM_DEVICE
             nbytes = lm_workspace_bytes(self.d, self.B, self.n, int(self.shared), mem)
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-            ws_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+            self.workspace, ws_ptr = self._alloc_ws(nbytes)
             self._cchain, self._keep = make_chain(chain)
             pb = LmProblem(self.B, self.n, self.tp.data_ptr(), self.tq.data_ptr(), int(self.shared),
                            self.seeds.data_ptr(), mem, ws_ptr, nbytes)
             s = stream if stream is not None else torch.cuda.current_stream(self.device)
             self._stream_handle = int(s.cuda_stream)
             self._ctx = lm_init(self._cchain, pb, self.params, self._stream_handle)
+
+    GUARD_BYTES = 4096
+
+    def _alloc_ws(self, nbytes: int):
+        """Device scratch of `nbytes` (256-byte aligned pointer).  guarded=True (tests/test_gpu_guards.py; the stand-in
+        for compute-sanitizer's memcheck / initcheck, which is closed on this pool): 4 KiB guard bands filled with 0xA5
+        on either side -- an out-of-bounds WRITE of any kernel shows up in guards_intact() -- and the interior
+        poisoned with 0xFF bytes (fp32 NaN, int -1) so that a read of memory no kernel has written ends up in the
+        outputs."""
+        torch = self.torch
+        if not self.guarded:
+            t = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            return t, (t.data_ptr() + 255) // 256 * 256
+        G = self.GUARD_BYTES
+        t = torch.full((nbytes + 2 * G + 256,), 0xA5, dtype=torch.uint8, device=self.device)
+        ptr = (t.data_ptr() + G + 255) // 256 * 256
+        off = ptr - t.data_ptr()
+        t[off:off + nbytes] = 0xFF
+        self._guards.append((t, off, nbytes))
+        return t, ptr
+
+    def guards_intact(self) -> bool:
+        self.torch.cuda.synchronize(self.device)
+        ok = True
+        for t, off, nbytes in self._guards:
+            ok = ok and bool((t[:off] == 0xA5).all().item()) and bool((t[off + nbytes:] == 0xA5).all().item())
+        return ok
 
     def _on_stream(self):
         """Uploads and allocations happen on the stream the library launches on: with a caller-supplied
@@ -528,8 +557,7 @@ class Solver:
         self.tparams = tparams if tparams is not None else lm_traj_default_params()
         nbytes = lm_traj_workspace_bytes(self.d, self.B, self.n)
         with self._on_stream():
-            self.traj_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-        ptr = (self.traj_workspace.data_ptr() + 255) // 256 * 256
+            self.traj_workspace, ptr = self._alloc_ws(nbytes)
         lm_traj_attach(self._ctx, self.tparams, ptr, nbytes)
 
     def traj_set_capsules(self, model, w_coll: float = 1.0, d_safe: float = 0.05) -> None:
@@ -588,8 +616,7 @@ class Solver:
         self.pparams = pparams if pparams is not None else lm_plan_default_params()
         nbytes = lm_plan_workspace_bytes(self.d, self.B, self.n)
         with self._on_stream():
-            self.plan_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-        ptr = (self.plan_workspace.data_ptr() + 255) // 256 * 256
+            self.plan_workspace, ptr = self._alloc_ws(nbytes)
         lm_plan_attach(self._ctx, self.pparams, ptr, nbytes)
 
     def plan_run(self, cycles: int) -> None:
@@ -621,10 +648,11 @@ class Solver:
         torch = self.torch
         sparams = sparams if sparams is not None else lm_search_default_params()
         nbytes = lm_search_workspace_bytes(self.d, self.B, self.n)
-        if getattr(self, "search_workspace", None) is None or self.search_workspace.numel() < nbytes + 256:
+        if getattr(self, "search_workspace", None) is None or self._search_ws_bytes < nbytes:
             with self._on_stream():
-                self.search_workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-        ptr = (self.search_workspace.data_ptr() + 255) // 256 * 256
+                self.search_workspace, self._search_ws_ptr = self._alloc_ws(nbytes)
+            self._search_ws_bytes = nbytes
+        ptr = self._search_ws_ptr
         if not to_host:
             lm_search(self._ctx, sparams, ptr, nbytes, None, None, None)
             return {}
