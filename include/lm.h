@@ -169,6 +169,13 @@ int lm_set_trace(lm_ctx *ctx, float *trial_q, float *trial_F);
  * specialised one (the two return the same values).  Results never depend on either. */
 #define LM_OPT_BLOCK_THREADS 1
 #define LM_OPT_GENERIC_KERNEL 2
+/* LM_OPT_LANES_PER_WAYPOINT: 1 (default: one thread owns a waypoint block), 2 or 4 = the lane-group form BASELINE.json's
+ * north_star names ("thread group per waypoint block ... warp-shuffle reductions for J^T J / J^T r"): the sums over the
+ * rows of J are split over 2 / 4 adjacent lanes and closed with shuffles, everything else is replicated.  Kept as a
+ * MEASURED alternative (it is slower); only for chains with a specialised kernel, the default
+ * residual / solver, unit weights and exact sincos (else LM_EINVAL).  Results agree with the default to rounding (the
+ * summation order of the row sums differs), not bitwise. */
+#define LM_OPT_LANES_PER_WAYPOINT 3
 int lm_set_option(lm_ctx *ctx, int32_t option, int32_t value);
 
 /* Name of the LM kernel variant this context launches: "panda7", "rand8" (compile-time chain

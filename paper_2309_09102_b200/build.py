@@ -15,7 +15,7 @@ _ROOT = os.path.dirname(_HERE)
 LIB_PATH = os.path.join(_HERE, "liblm_b200.so")
 SOURCES = [os.path.join(_CSRC, f) for f in ("lm_api.cu", "lm_inst_specs.cu", "lm_inst_generic_lo.cu",
                                             "lm_inst_generic_hi.cu", "lm_traj_api.cu", "lm_plan_api.cu", "lm_search_api.cu", "lm_inst_traj_spec.cu",
-                                            "lm_inst_traj_generic_lo.cu", "lm_inst_traj_generic_hi.cu")]
+                                            "lm_inst_traj_generic_lo.cu", "lm_inst_traj_generic_hi.cu", "lm_inst_lanegroup.cu")]
 DEPS = SOURCES + [os.path.join(_CSRC, f) for f in ("lm_kernels.cuh", "lm_device.cuh", "lm_specs.cuh", "lm_launch.h",
                                                    "lm_ctx.h", "lm_traj.cuh", "lm_traj_launch.h", "lm_coll.cuh")] \
     + [os.path.join(_ROOT, "include", "lm.h")]

@@ -182,6 +182,7 @@ int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_
     }
     c->spec_id = match_spec(chain_signature(d, k));
     c->use_generic = false;
+    c->lanes = 1;
     a.lambda0 = prm->lambda0; a.nu_up = prm->nu_up; a.inv_nu_down = (float)(1.0 / (double)prm->nu_down);
     a.lambda_min = prm->lambda_min; a.lambda_max = prm->lambda_max; a.tol2 = prm->tol * prm->tol;
     a.w_pos = prm->w_pos; a.w_rot = prm->w_rot;
@@ -221,8 +222,13 @@ namespace {
 
 cudaError_t launch_iterate(lm_ctx *c, const KArgs &a) {
     g_launches.fetch_add(1);
-    const unsigned grid = (unsigned)((c->W + c->block - 1) / c->block);
     const bool weighted = a.weighted != 0;
+    if (c->lanes > 1) { // lane-group form: validated by lm_set_option, re-checked here because the parameters can change after it
+        if (c->spec_id == SPEC_GENERIC || c->use_generic || c->fast || weighted || a.variant != 0) return cudaErrorInvalidValue;
+        const unsigned grid_lg = (unsigned)((c->W * c->lanes + c->block - 1) / c->block);
+        return launch_iterate_lanegroup(c->spec_id, c->lanes, grid_lg, c->block, c->stream, a);
+    }
+    const unsigned grid = (unsigned)((c->W + c->block - 1) / c->block);
     if (c->spec_id != SPEC_GENERIC && !c->use_generic)
         return launch_iterate_spec(c->spec_id, c->fast, weighted, grid, c->block, c->stream, a);
     return c->dof <= 4 ? launch_iterate_generic_lo(c->dof, c->fast, weighted, grid, c->block, c->stream, a)
@@ -377,7 +383,14 @@ int lm_set_option(lm_ctx *c, int32_t option, int32_t value) {
         c->block = value;
         return LM_OK;
     case LM_OPT_GENERIC_KERNEL:
+        if (value != 0 && c->lanes > 1) return LM_EINVAL;
         c->use_generic = value != 0;
+        return LM_OK;
+    case LM_OPT_LANES_PER_WAYPOINT:
+        if (value != 1 && value != 2 && value != 4) return LM_EINVAL;
+        if (value > 1 && (c->spec_id == SPEC_GENERIC || c->use_generic || c->fast || c->args.weighted || c->args.variant != 0))
+            return LM_EINVAL;
+        c->lanes = value;
         return LM_OK;
     default:
         return LM_EINVAL;

@@ -58,6 +58,7 @@ struct lm_ctx {
     bool fast;
     int spec_id;      // structure-matched specialised kernel (lm_specs.cuh) or SPEC_GENERIC
     bool use_generic; // LM_OPT_GENERIC_KERNEL
+    int lanes;        // LM_OPT_LANES_PER_WAYPOINT: 1 (default), 2 or 4
     lmk::TrajState traj;
     lmk::PlanState plan;
 };

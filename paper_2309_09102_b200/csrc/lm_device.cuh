@@ -515,6 +515,210 @@ __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine
     return ok && (asum < 1e30f);
 }
 
+// ---- packed form of S4 + S5 (sm_100a FFMA2 / FMUL2: two fp32 operations per instruction, each IEEE round-to-nearest).
+// Layout: the Jacobian in PAIRS OF COLUMNS, Jp[k][c] = (J[k][2c], J[k][2c+1]) (row k of 6, pad column = 0 when D is
+// odd), and the lower triangle of A = J^T J + lambda I as column vectors paired along the row index,
+// Ap[c][j] = (A[2c][j], A[2c+1][j]) for 2c+1 >= j.  Every entry goes through the same sequence of fused operations as
+// in lm_delta (sum over k = 0..5, right-looking Cholesky, forward substitution by columns), so the step has the same
+// bits up to the sign of zero; the extra lane of a boundary pair (a row above the diagonal, the pad row) is never read.
+using f2 = float2;
+__device__ __forceinline__ f2 bc2(float s) { return make_float2(s, s); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ f2 neg2(f2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float lane2(f2 a, int l) { return l ? a.y : a.x; }
+
+// x = (L L^T)^-1 b: forward substitution by columns on pairs (bp is consumed), backward substitution on scalars
+template <int D>
+__device__ __forceinline__ void chol_solve_p(const f2 (&Lp)[(D + 1) / 2][D], const float (&invd)[D], f2 (&bp)[(D + 1) / 2],
+                                             float (&x)[D]) {
+    constexpr int NP = (D + 1) / 2;
+    float y[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        y[j] = mul(lane2(bp[j / 2], j & 1), invd[j]);
+#pragma unroll
+        for (int c = (j + 1) / 2; c < NP; ++c) bp[c] = fma2(neg2(Lp[c][j]), bc2(y[j]), bp[c]);
+    }
+#pragma unroll
+    for (int i = D - 1; i >= 0; --i) {
+        float s = y[i];
+#pragma unroll
+        for (int j = i + 1; j < D; ++j) s = fma_(-lane2(Lp[j / 2][i], j & 1), x[j], s);
+        x[i] = mul(s, invd[i]);
+    }
+}
+
+template <int D, bool WEIGHTED, typename SpecT, bool RPY = false>
+__device__ __forceinline__ bool lm_delta_p(const Pose<D> &P, float lam, int refine, float (&delta)[D]) {
+    using K = JK<WEIGHTED, SpecT, RPY>;
+    constexpr int NP = (D + 1) / 2;
+    f2 Jp[6][NP];
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+#pragma unroll
+        for (int c = 0; c < NP; ++c) Jp[k][c] = make_float2(jentry<D>(P, 2 * c, k), 2 * c + 1 < D ? jentry<D>(P, 2 * c + 1, k) : 0.f);
+    f2 Ap[NP][D], gp[NP];
+#pragma unroll
+    for (int j = 0; j < D; ++j)
+#pragma unroll
+        for (int c = j / 2; c < NP; ++c) {
+            f2 a = make_float2(2 * c == j ? lam : 0.f, 2 * c + 1 == j ? lam : 0.f);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) {
+                if (K::zero(j, k)) continue;
+                a = fma2(Jp[k][c], bc2(jentry<D>(P, j, k)), a);
+            }
+            Ap[c][j] = a;
+        }
+#pragma unroll
+    for (int c = 0; c < NP; ++c) {
+        f2 a = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) a = fma2(Jp[k][c], bc2(P.r[k]), a);
+        gp[c] = neg2(a);
+    }
+    float invd[D];
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < D; ++k) {
+        const float piv = lane2(Ap[k / 2][k], k & 1);
+        ok = ok && (piv > 0.f);
+        const float id = rsqrtf(piv);
+        invd[k] = id;
+#pragma unroll
+        for (int c = (k + 1) / 2; c < NP; ++c) Ap[c][k] = mul2(Ap[c][k], bc2(id));
+#pragma unroll
+        for (int j = k + 1; j < D; ++j) {
+            const float b = lane2(Ap[j / 2][k], j & 1);
+#pragma unroll
+            for (int c = j / 2; c < NP; ++c) Ap[c][j] = fma2(neg2(Ap[c][k]), bc2(b), Ap[c][j]);
+        }
+    }
+    chol_solve_p<D>(Ap, invd, gp, delta);
+    for (int it = 0; it < refine; ++it) {
+        float t[6], e[D];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            float sv = P.r[k], sw = P.r[3 + k];
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                if (!K::zero(j, k)) sv = K::one(j, k) ? add(sv, delta[j]) : fma_(P.Jv[j][k], delta[j], sv);
+                if (!K::zero(j, 3 + k)) sw = K::one(j, 3 + k) ? add(sw, delta[j]) : fma_(P.Jw[j][k], delta[j], sw);
+            }
+            t[k] = sv;
+            t[3 + k] = sw;
+        }
+        f2 rp[NP];
+#pragma unroll
+        for (int c = 0; c < NP; ++c) {
+            f2 a = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) a = fma2(Jp[k][c], bc2(t[k]), a);
+            rp[c] = neg2(fma2(bc2(lam), make_float2(delta[2 * c], 2 * c + 1 < D ? delta[2 * c + 1] : 0.f), a));
+        }
+        chol_solve_p<D>(Ap, invd, rp, e);
+#pragma unroll
+        for (int i = 0; i < D; ++i) delta[i] = add(delta[i], e[i]);
+    }
+    float asum = 0.f;
+#pragma unroll
+    for (int i = 0; i < D; ++i) asum = add(asum, fabsf(delta[i]));
+    return ok && (asum < 1e30f);
+}
+
+// ---- lane-group form of S4 + S5 (BASELINE.json north_star: "one warp or thread group per waypoint block ... warp-shuffle
+// reductions for J^T J / J^T r"; measured against the one-thread form in DESIGN.md section 7): G = 2 or 4 adjacent
+// lanes share one waypoint.  FK, the Jacobian, the Cholesky factorisation and the triangular solves are replicated on
+// the G lanes (a serial chain and a 7 x 7 triangle do not split without per-step exchanges); the sums over the six rows
+// of J -- J^T J, J^T r and J^T t of the refinement -- are split by rows (lane g takes rows g, g + G, ...) and closed with
+// an xor butterfly, which leaves bit-identical totals on every lane of the group, so the G lanes take the same decisions.
+// The summation order differs from lm_delta, so results agree with the one-thread kernel to rounding, not bitwise.
+template <int G>
+__device__ __forceinline__ float group_sum(float v) {
+#pragma unroll
+    for (int o = 1; o < G; o <<= 1) v = add(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+template <int D, int G>
+__device__ __forceinline__ bool lm_delta_lg(const Pose<D> &P, float lam, int refine, int g, float (&delta)[D]) {
+    static_assert(G == 2 || G == 4, "lane groups of 2 or 4");
+    constexpr int R = (6 + G - 1) / G; // rows per lane
+    float Jh[D][R], rh[R];
+#pragma unroll
+    for (int m = 0; m < R; ++m) {
+        float rv = 0.f;
+#pragma unroll
+        for (int gg = 0; gg < G; ++gg)
+            if (gg + G * m < 6) rv = (g == gg) ? P.r[gg + G * m] : rv;
+        rh[m] = rv;
+#pragma unroll
+        for (int j = 0; j < D; ++j) {
+            float v = 0.f;
+#pragma unroll
+            for (int gg = 0; gg < G; ++gg)
+                if (gg + G * m < 6) v = (g == gg) ? jentry<D>(P, j, gg + G * m) : v;
+            Jh[j][m] = v;
+        }
+    }
+    float L[D][D], invd[D], gv[D];
+#pragma unroll
+    for (int i = 0; i < D; ++i) {
+#pragma unroll
+        for (int j = 0; j <= i; ++j) {
+            float a = mul(Jh[i][0], Jh[j][0]);
+#pragma unroll
+            for (int m = 1; m < R; ++m) a = fma_(Jh[i][m], Jh[j][m], a);
+            a = group_sum<G>(a);
+            L[i][j] = (i == j) ? add(a, lam) : a;
+        }
+        float a = mul(Jh[i][0], rh[0]);
+#pragma unroll
+        for (int m = 1; m < R; ++m) a = fma_(Jh[i][m], rh[m], a);
+        gv[i] = -group_sum<G>(a);
+    }
+    bool ok = true;
+#pragma unroll
+    for (int k = 0; k < D; ++k) {
+        const float piv = L[k][k];
+        ok = ok && (piv > 0.f);
+        const float id = rsqrtf(piv);
+        invd[k] = id;
+#pragma unroll
+        for (int i = k + 1; i < D; ++i) L[i][k] = mul(L[i][k], id);
+#pragma unroll
+        for (int j = k + 1; j < D; ++j)
+#pragma unroll
+            for (int i = j; i < D; ++i) L[i][j] = fma_(-L[i][k], L[j][k], L[i][j]);
+    }
+    chol_solve<D>(L, invd, gv, delta);
+    for (int it = 0; it < refine; ++it) {
+        float th[R], rho[D], e[D];
+#pragma unroll
+        for (int m = 0; m < R; ++m) {
+            float sv = rh[m];
+#pragma unroll
+            for (int j = 0; j < D; ++j) sv = fma_(Jh[j][m], delta[j], sv);
+            th[m] = sv;
+        }
+#pragma unroll
+        for (int i = 0; i < D; ++i) {
+            float a = mul(Jh[i][0], th[0]);
+#pragma unroll
+            for (int m = 1; m < R; ++m) a = fma_(Jh[i][m], th[m], a);
+            rho[i] = -fma_(lam, delta[i], group_sum<G>(a));
+        }
+        chol_solve<D>(L, invd, rho, e);
+#pragma unroll
+        for (int i = 0; i < D; ++i) delta[i] = add(delta[i], e[i]);
+    }
+    float asum = 0.f;
+#pragma unroll
+    for (int i = 0; i < D; ++i) asum = add(asum, fabsf(delta[i]));
+    return ok && (asum < 1e30f);
+}
+
 // The same step in its DUAL form (SURVEY section 8f NEXT-4 i, a disclosed variant):
 //   delta = -J^T (J J^T + lambda I_6)^-1 r,
 // identical to -(J^T J + lambda I_d)^-1 J^T r in exact arithmetic (push-through identity; the oracle pins

@@ -43,6 +43,13 @@ __device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z,
     Rt[0][2] = mul(2.f, sub(xz, wy));        Rt[1][2] = mul(2.f, add(yz, wx));        Rt[2][2] = fma_(-2.f, add(xx, yy), 1.f);
 }
 
+// LM_PACKED_DELTA: which kernels take S4 + S5 through the packed FFMA2 form (lm_delta_p, same bits): 0 none, 1 the
+// generic (run-time chain structure) kernels, 2 all.  Measured on C4 (profiles/r2_rf_model.md): generic 2.875 -> 2.807
+// ms, Panda-specialised 2.064 -> 2.316 ms (the specialised scalar form skips the structural zeros of J; the packed
+// form cannot, and register-file reads, not issue slots, are the limit), hence 1.
+#ifndef LM_PACKED_DELTA
+#define LM_PACKED_DELTA 1
+#endif
 #ifndef LM_MAX_THREADS
 #define LM_MAX_THREADS 256
 #endif
@@ -53,9 +60,12 @@ __device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z,
 // VAR: 0 = the d x d system with the rotation-vector residual (the hot path), LM_VAR_DUAL = the 6 x 6 dual form,
 // LM_VAR_RPY = the roll-pitch-yaw residual (disclosed variants, DESIGN.md sections 12 and 14)
 constexpr int LM_VAR_DUAL = 1, LM_VAR_RPY = 2;
-template <int D, bool FAST, bool WEIGHTED, typename SpecT, int VAR = 0>
+// G: lanes per waypoint (1 = the product path; 2 / 4 = the lane-group form lm_delta_lg, LM_OPT_LANES_PER_WAYPOINT)
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, int VAR = 0, int G = 1>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kernel(const __grid_constant__ KArgs A) {
-    const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t w = G == 1 ? tid : tid / G;
+    const int gl = G == 1 ? 0 : (int)(threadIdx.x % G); // lane within the waypoint's group
     const bool live = w < A.W;
     const int64_t wc = live ? w : A.W - 1; // tail lanes shadow the last waypoint, never store
     const int64_t W = A.W;
@@ -105,8 +115,12 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         if (!__any_sync(0xffffffffu, active)) break;
 
         float delta[D];
-        const bool ok = DUAL ? lm_delta_dual<D, WEIGHTED, SpecT>(cur, lam, delta)            // S4, S5 (variant)
-                             : lm_delta<D, WEIGHTED, SpecT, RPY>(cur, lam, A.refine, delta); // S4, S5
+        constexpr bool PACKED = LM_PACKED_DELTA == 2 || (LM_PACKED_DELTA == 1 && SpecT::spec.generic);
+        bool ok;
+        if constexpr (DUAL) ok = lm_delta_dual<D, WEIGHTED, SpecT>(cur, lam, delta);                // S4, S5 (variant)
+        else if constexpr (G > 1) ok = lm_delta_lg<D, G>(cur, lam, A.refine, gl, delta);
+        else if constexpr (PACKED) ok = lm_delta_p<D, WEIGHTED, SpecT, RPY>(cur, lam, A.refine, delta);
+        else ok = lm_delta<D, WEIGHTED, SpecT, RPY>(cur, lam, A.refine, delta);                      // S4, S5
         float qt[D];
         bool clamped = false;
 #pragma unroll
@@ -120,7 +134,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         eval_pose<D, FAST, WEIGHTED, SpecT, false, NoFrameSink, RPY>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, tri, nullptr, nullptr, ptri,
                                                                      NoFrameSink(), trpy);
 
-        if (A.trace_q != nullptr && active && live) {
+        if (A.trace_q != nullptr && active && live && gl == 0) {
 #pragma unroll
             for (int j = 0; j < D; ++j) A.trace_q[(int64_t)j * W + w] = qt[j];
             A.trace_F[w] = cur.F;
@@ -151,7 +165,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
     }
 
     // ---- S10 store
-    if (!live) return;
+    if (!live || gl != 0) return;
     const bool frozen = cur.F < A.tol2;
     if (frozen) st |= 1u;
     else if (k >= (uint32_t)A.max_total) st |= 2u;

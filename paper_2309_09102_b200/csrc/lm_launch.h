@@ -13,6 +13,9 @@ cudaError_t launch_fk_generic(int dof, bool fast, unsigned grid, unsigned block,
 cudaError_t launch_iterate_spec(int spec_id, bool fast, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const KArgs &a);
 cudaError_t launch_fk_spec(int spec_id, bool fast, unsigned grid, unsigned block, cudaStream_t s, const KFkArgs &a);
 
+// lane-group form (G = 2, 4 lanes per waypoint) of the registered chains; plain residual, unweighted, exact sincos only
+cudaError_t launch_iterate_lanegroup(int spec_id, int lanes, unsigned grid, unsigned block, cudaStream_t s, const KArgs &a);
+
 // ---- launch helpers used by the instantiation units
 template <int D, typename SpecT>
 cudaError_t launch_iterate_t(bool fast, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const KArgs &a) {

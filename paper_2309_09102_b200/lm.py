@@ -22,7 +22,7 @@ LM_MAX_DOF = 8
 LM_MAX_ITERS = 64
 LM_OK, LM_EINVAL, LM_ENOMEM, LM_ECUDA = 0, -1, -2, -3
 LM_MEM_DEVICE, LM_MEM_HOST = 0, 1
-LM_OPT_BLOCK_THREADS, LM_OPT_GENERIC_KERNEL = 1, 2
+LM_OPT_BLOCK_THREADS, LM_OPT_GENERIC_KERNEL, LM_OPT_LANES_PER_WAYPOINT = 1, 2, 3
 LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1, 2, 4, 8, 16
 
 # every symbol include/lm.h declares (checked by tests/test_abi.py)
@@ -498,6 +498,10 @@ class Solver:
 
     def use_generic_kernel(self, on: bool = True) -> None:
         lm_set_option(self._ctx, LM_OPT_GENERIC_KERNEL, int(on))
+
+    def set_lanes_per_waypoint(self, lanes: int) -> None:
+        """1 (default), 2 or 4 lanes per waypoint block (the measured lane-group alternative, include/lm.h)."""
+        lm_set_option(self._ctx, LM_OPT_LANES_PER_WAYPOINT, int(lanes))
 
     @property
     def kernel_name(self) -> str:

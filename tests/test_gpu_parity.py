@@ -282,3 +282,47 @@ def test_config5_sweep_points(lm, B, n):
         assert np.array_equal(g["q"][sl], g["q"][:base.W])
         assert np.abs(g["q"][sl] - o.q).max() <= H.TOL_Q
         assert np.array_equal(g["iters"][sl], o.iters)
+
+
+# ------------------------------------------------------------------ lane-group form (LM_OPT_LANES_PER_WAYPOINT)
+
+@pytest.mark.parametrize("lanes", [2, 4])
+def test_lane_group_variant_matches_the_oracle(lm, lanes):
+    """The measured alternative BASELINE.json's north_star names (2 / 4 lanes per waypoint, warp-shuffle reductions for
+    J^T J and J^T r): same bars as the one-thread kernel against the same oracle sequence --
+    configs[0], 64 trajectories of configs[1] (ragged: 64 x 300 waypoints x lanes is not a multiple of the block) and
+    32 trajectories of the 8-DoF configs[2]."""
+    for w, check_pose in ((wl.config1(H.oracle_fk(wl.panda_chain())), True),
+                          (wl.config2(H.oracle_fk(wl.panda_chain()), B=64, n=299), True),
+                          (wl.config3(H.oracle_fk(wl.random_chain_8dof(3)), B=32), False)):
+        s = H.make_solver(w)
+        s.set_lanes_per_waypoint(lanes)
+        s.run(w.max_iters)
+        g = s.fetch()
+        # the one-thread kernel on the same context: same decisions, joints to rounding
+        s.set_lanes_per_waypoint(1)
+        s.reset()
+        s.run(w.max_iters)
+        g1 = s.fetch()
+        s.close()
+        o = H.run_oracle(w)
+        _check_free_running(w, g, o, check_pose=check_pose)
+        compared, bad = H.decisive_mismatches(w, g, int(o.iters.max()))
+        assert compared >= w.W and bad == 0
+        same = g["iters"] == g1["iters"]
+        assert same.mean() > 0.998 and np.abs(g["q"] - g1["q"])[same].max() <= 2e-5
+
+
+def test_lane_group_option_is_validated(lm):
+    w = wl.config1(H.oracle_fk(wl.panda_chain()))
+    s = H.make_solver(w)
+    with pytest.raises(lm.LmError):
+        s.set_lanes_per_waypoint(3)
+    s.use_generic_kernel(True)
+    with pytest.raises(lm.LmError):      # no lane-group form of the generic kernel
+        s.set_lanes_per_waypoint(2)
+    s.close()
+    s = H.make_solver(w, solver=lm.LM_SOLVER_DUAL)
+    with pytest.raises(lm.LmError):      # nor of the disclosed variants
+        s.set_lanes_per_waypoint(2)
+    s.close()
