@@ -40,16 +40,28 @@ ALG_FLOP = {7: 1459.0, 8: 1762.0}
 ALG_FLOP_DUAL = {7: 1055.0, 8: 1160.0}
 # FP32 FMA-pipe peak derived from the guide's unit counts and clocks: 148 SMs x 128 lanes x 2 x f_max
 SM_COUNT, FP32_LANES = 148, 128
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r1c_lm_iterate_full.md); keyed by (workload, kernel variant).
-NCU_DRAM_TRAFFIC = {("C4", "panda7"): 68.849e6 + 27.575e6}
-# FP32 flop the kernel EXECUTES per waypoint-iteration (2 x FFMA + FMUL + FADD per warp-iteration from the source page of
-# the same capture: 2 x 532.9 + 165.6 + 68.2): fewer than the algorithmic count because multiplications by the
-# structural zeros / ones of the Panda chain are folded out.
-NCU_EXECUTED_FLOP = {("C4", "panda7"): 1300.0}
-# dram__bytes_read.sum + dram__bytes_write.sum of the four big kernels of ONE trajectory-level iteration on C4 (solve<0>,
-# rho, solve<1>, trial; an iteration in which ~30 % of the trajectories rejected), profiles/r1h_traj_full.md
-NCU_TRAJ_DRAM_TRAFFIC = {"C4": (477.025 + 190.604 + 137.713 + 21.786 + 314.961 + 55.676 + 448.207 + 379.615) * 1e6}
+# Numbers that only an ncu capture can give (DRAM bytes per launch, executed FP32 flop per waypoint-iteration) live in
+# profiles/ncu_constants.json, each entry naming the capture it was read from and the SHA-256 of the kernel sources it
+# was taken with; an entry whose hash does not match the sources of this checkout is reported as null (stale).
+HOT_SOURCES = ("lm_device.cuh", "lm_kernels.cuh", "lm_specs.cuh")
+TRAJ_SOURCES = ("lm_traj.cuh", "lm_coll.cuh", "lm_device.cuh", "lm_traj_launch.h")
+
+
+def source_hash(files) -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for f in files:
+        h.update(open(os.path.join(ROOT, "paper_2309_09102_b200", "csrc", f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_constant(key: str, field: str, files):
+    """profiles/ncu_constants.json[key][field] if the entry was captured with the current kernel sources, else None."""
+    try:
+        e = json.load(open(os.path.join(ROOT, "profiles", "ncu_constants.json")))[key]
+    except (OSError, KeyError, ValueError):
+        return None
+    return e.get(field) if e.get("source_sha256_16") == source_hash(files) else None
 
 
 def load_peaks() -> dict:
@@ -189,7 +201,7 @@ def workload_desc(w) -> dict:
 
 # ------------------------------------------------------------------ CPU oracle legs
 
-def time_oracle(w, n_traj: int, steps: int = 1, warmup: int = 0) -> dict:
+def time_oracle(w, n_traj: int, steps: int = 1, warmup: int = 0, nthreads: int = 0) -> dict:
     """The oracle as it stands, on the host cores, on the first n_traj trajectories of w."""
     from oracle import lm_oracle as orc
     sub = w.subset(slice(0, min(n_traj, w.B)))
@@ -198,13 +210,13 @@ def time_oracle(w, n_traj: int, steps: int = 1, warmup: int = 0) -> dict:
     times, executed = [], 0
     for i in range(warmup + steps):
         t0 = time.perf_counter()
-        st = orc.lm_run(sub.chain, prm, tp, tq, s, sub.max_iters)
+        st = orc.lm_run(sub.chain, prm, tp, tq, s, sub.max_iters, nthreads=nthreads)
         dt = time.perf_counter() - t0
         if i >= warmup:
             times.append(dt)
             executed += st.executed
     total = float(sum(times))
-    return {"value": executed / total, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+    return {"value": executed / total, "unit": UNIT, "cores": nthreads if nthreads > 0 else orc.num_threads(), "kind": "oracle",
             "sample": f"first {sub.B} of {w.B} trajectories ({sub.W} waypoints, {executed // max(steps, 1)} "
                       f"waypoint-iterations per step), fp64, OpenMP over waypoints",
             "seconds": total, "ms_per_step": 1e3 * total / max(steps, 1), "traj_per_s": sub.B * steps / total}
@@ -314,11 +326,11 @@ def run_gpu(args) -> None:
     full_size = (args.B is None and args.n is None)
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / peak_tf,
-                "traffic": NCU_DRAM_TRAFFIC.get((args.workload, solver.kernel_name)) if full_size else None,
+                "traffic": ncu_constant(f"lm_iterate_{solver.kernel_name}_{args.workload}", "dram_bytes_per_launch", HOT_SOURCES) if full_size else None,
                 "kernel": f"lm_iterate_kernel<{d}, {solver.kernel_name}>", "kernel_ms": ms_kernel,
                 "peak_measured_fma": fma_tf, "frac_of_measured_fma": achieved_tf / fma_tf if fma_tf > 0 else None,
                 "alg_flop_per_waypoint_iteration": ALG_FLOP.get(d),
-                "ncu_executed_flop_per_waypoint_iteration": NCU_EXECUTED_FLOP.get((args.workload, solver.kernel_name)) if full_size else None,
+                "ncu_executed_flop_per_waypoint_iteration": ncu_constant(f"lm_iterate_{solver.kernel_name}_{args.workload}", "executed_flop_per_waypoint_iteration", HOT_SOURCES) if full_size else None,
                 "peak_how": f"derived: {SM_COUNT} SMs x {FP32_LANES} FP32 lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz "
                             f"(sm_max_mhz {peaks['_source']})",
                 "hbm": {"alg_bytes": hbm_bytes, "achieved_gbs": hbm_bytes / (ms_kernel * 1e-3) / 1e9,
@@ -328,11 +340,29 @@ def run_gpu(args) -> None:
         roofline["executed_tflops"] = roofline["ncu_executed_flop_per_waypoint_iteration"] * iters_per_step / (ms_kernel * 1e-3) / 1e12
     ref_traj = min(args.ref_traj or 256, w.B)
     cpu = time_oracle(make_workload(args.workload, fk, ref_traj, w.n), ref_traj)
+    cpu1 = time_oracle(make_workload(args.workload, fk, min(16, w.B), w.n), min(16, w.B), nthreads=1)
     cfg = workload_desc(w)
     cfg.update({"parallelism": f"dp{world} (independent batches, no collective)", "l2": "flushed between steps (256 MiB write)",
-                "block_threads": args.block or 128, "kernel": solver.kernel_name})
+                "block_threads": args.block or 128, "kernel": solver.kernel_name,
+                "targets": "poses of the seeded joint paths / anchors through the library's fp32 lm_fk (the parity tests "
+                           "build theirs with the oracle's fp64 FK; bench.py may run the oracle only in its cpu_baseline leg)"})
     extra = {}
     if args.workload == "C4" and full_size:
+        # what an unregistered robot gets: the generic (run-time chain structure) kernel on the same workload
+        extra["generic_kernel_C4"] = time_kernel_option(lm, torch, w, device, stream, peak_tf, lm.LM_OPT_GENERIC_KERNEL, 1)
+        # the lane-group alternative the north star names (2 / 4 lanes per waypoint), measured beside the product kernel
+        extra["lane_group_variants"] = {f"{g}_lanes": time_kernel_option(lm, torch, w, device, stream, peak_tf, lm.LM_OPT_LANES_PER_WAYPOINT, g)
+                                        for g in (2, 4)}
+        extra["lane_group_variants"]["1_lane"] = {"ms_per_step": ms_kernel, "frac_of_derived_peak": achieved_tf / peak_tf}
+        # BASELINE.json configs[2]: 2048 x 300, 8-DoF chain with a prismatic joint, to |r| < tol or 50 iterations
+        extra["c3_8dof"] = time_c3(lm, torch, wl, device, stream, peak_tf)
+        # BASELINE.json configs[4], compact: B x n grid, exactly 20 iterations
+        extra["sweep_C5"] = time_sweep_c5(lm, torch, wl, fk, device, stream)
+        # FFMA / FFMA2 operand forms (register-file read-bandwidth calibration, profiles/r2_rf_model.md)
+        extra["fma_operand_forms_tflops"] = {n: lm.lm_fp32_peak_form(f, int(stream.cuda_stream)) for n, f in
+                                             (("R,c,c", lm.LM_FMA_FORM_RCC), ("R,R,R", lm.LM_FMA_FORM_RRR), ("R,Rreuse,R", lm.LM_FMA_FORM_RRS),
+                                              ("R,Rreuse,Rreuse", lm.LM_FMA_FORM_RSS), ("FMUL R,R", lm.LM_FMA_FORM_MUL),
+                                              ("FFMA2 P,P,P", lm.LM_FMA_FORM_PPP), ("FFMA2 P,Rbcast,P", lm.LM_FMA_FORM_PSP))}
         # the "to convergence" statistic of the metric, on BASELINE.json configs[1] (512 x 300, tol 1e-5)
         extra["to_convergence_C2"] = time_to_convergence(lm, torch, wl, fk, device, stream)
         extra["variant_dual"] = time_dual_variant(lm, torch, w, device, stream, peak_tf)
@@ -359,7 +389,8 @@ def run_gpu(args) -> None:
                     "unpipelined_ms_per_step": e2e_plain["ms_total"] / e2e_plain["steps"],
                     "unpipelined_how": "lm_init(LM_MEM_HOST, pinned) + lm_run + lm_fetch"},
             "roofline": roofline,
-            "cpu_baseline": {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}}
+            "cpu_baseline": {**{k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")},
+                             "single_thread": {k: cpu1[k] for k in ("value", "unit", "cores", "sample")}}}
     line.update(extra)
     print(json.dumps(line))
 
@@ -468,7 +499,7 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
            "without_refinement": norefine,
            "roofline": {"bound": "hbm", "achieved": alg / (ms_iter * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                        "traffic": NCU_TRAJ_DRAM_TRAFFIC.get(w.name.split(":")[0]) if (w.B, w.n) == (4096, 300) else None,
+                        "traffic": ncu_constant("traj_iteration_C4", "dram_bytes_per_iteration", TRAJ_SOURCES) if (w.B, w.n) == (4096, 300) else None,
                         "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps)),
                         "peak_source": peaks["_source"]}}
     try:
@@ -625,6 +656,76 @@ def time_search(lm, torch, wl, fk, device, stream, K: int = 175, n: int = 300, r
             "gpu_launches": int(launches), "edges_per_sec": (n - 1) * K * K / (ms * 1e-3), "mjac_rad": g["mjac"],
             "candidates_used": int(len(set(g["choice"].tolist()))), "same_choice_as_oracle": bool(np.array_equal(g["choice"], choice)),
             "cpu_baseline": {"ms": cpu_s * 1e3, "kind": "oracle", "cores": 1, "sample": "the same input, once"}}
+
+
+def _time_runs(torch, s, stream, max_iters: int, reps: int, flush=None):
+    ts = []
+    with torch.cuda.stream(stream):
+        for i in range(reps + 3):
+            if flush is not None:
+                flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s.reset()
+            a.record(stream)
+            s.run(max_iters)
+            b.record(stream)
+            stream.synchronize()
+            if i >= 3:
+                ts.append(a.elapsed_time(b))
+        iters, conv = s.fetch_totals()
+    return float(np.median(ts)), iters, conv
+
+
+def time_kernel_option(lm, torch, w, device, stream, peak_tf: float, option: int, value: int, reps: int = 10) -> dict:
+    """lm_reset + lm_run on the headline workload with one lm_set_option knob changed (median CUDA-event time)."""
+    d = int(w.chain.dof)
+    prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol)
+    s = lm.Solver(w.chain, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, device=str(device), stream=stream)
+    lm.lm_set_option(s._ctx, option, value)
+    ms, iters, _ = _time_runs(torch, s, stream, w.max_iters, reps)
+    name = s.kernel_name
+    s.close()
+    tf = ALG_FLOP.get(d, 1459.0 * d / 7.0) * iters / (ms * 1e-3) / 1e12
+    return {"kernel": name, "ms_per_step": ms, "waypoint_iterations_per_sec": iters / (ms * 1e-3), "achieved_tflops": tf,
+            "frac_of_derived_peak": tf / peak_tf}
+
+
+def time_c3(lm, torch, wl, device, stream, peak_tf: float, reps: int = 10) -> dict:
+    """BASELINE.json configs[2] at full size: 2048 x 300, the seeded 8-DoF chain (one prismatic joint), seeds N(0, 0.15),
+    |r| < 1e-5 or 50 iterations -- and the same batch for exactly 50 iterations (tol = 0), which is the figure comparable
+    with the headline's fraction (1762 FLOP per waypoint-iteration)."""
+    ch = wl.random_chain_8dof(3)
+    w = wl.config3(lm.device_fk(ch, device=str(device)))
+    out = {"workload": f"C3: {w.B} x {w.n}, 8-DoF (1 prismatic), tol={w.tol:g}, max_iters={w.max_iters}"}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)
+    for key, tol in (("to_convergence", w.tol), ("fixed_50_iterations", 0.0)):
+        prm = lm.lm_default_params(lambda0=w.lambda0, tol=tol)
+        s = lm.Solver(ch, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, device=str(device), stream=stream)
+        ms, iters, conv = _time_runs(torch, s, stream, w.max_iters, reps, flush)
+        name = s.kernel_name
+        s.close()
+        tf = ALG_FLOP[8] * iters / (ms * 1e-3) / 1e12
+        out[key] = {"kernel": name, "ms_per_step": ms, "waypoint_iterations": iters, "waypoint_iterations_per_sec": iters / (ms * 1e-3),
+                    "trajectories_per_sec": w.B / (ms * 1e-3), "converged_trajectories": conv,
+                    "alg_flop_per_waypoint_iteration": ALG_FLOP[8], "achieved_tflops": tf, "frac_of_derived_peak": tf / peak_tf}
+    return out
+
+
+def time_sweep_c5(lm, torch, wl, fk, device, stream, reps: int = 5) -> dict:
+    """BASELINE.json configs[4], compact: B in {1, 256, 4096, 16384} x n in {100, 300, 1000}, Panda, seeds N(0, 0.1), exactly
+    20 iterations; median CUDA-event time of lm_reset + lm_run(20), L2 flushed before every launch."""
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)
+    out = {"workload": "C5: Panda, smooth paths as configs[1], exactly 20 iterations", "points": []}
+    for n in (100, 300, 1000):
+        big = wl.config5(fk, B=16384, n=n)
+        for B in (1, 256, 4096, 16384):
+            w = big.subset(slice(0, B))
+            prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol)
+            s = lm.Solver(w.chain, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, device=str(device), stream=stream)
+            ms, iters, _ = _time_runs(torch, s, stream, w.max_iters, reps, flush)
+            s.close()
+            out["points"].append({"B": B, "n": n, "ms": ms, "waypoint_iterations_per_sec": iters / (ms * 1e-3)})
+    return out
 
 
 def time_dual_variant(lm, torch, w, device, stream, peak_tf: float, reps: int = 10) -> dict:

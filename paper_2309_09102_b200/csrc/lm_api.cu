@@ -329,6 +329,44 @@ __global__ void __launch_bounds__(256) lm_fma_rrr_kernel(float *out, int iters, 
     if (sum == 12345.678f) out[0] = sum;
 }
 
+// Further operand forms of the same loop (register-file read-bandwidth calibration, profiles/r2_rf_model.md):
+//   RRS  x = x * y0 + z[i]   (y0 shared by consecutive FFMAs: operand-reuse cache)      2 new register reads
+//   RSS  x = x * y0 + z0                                                                  1 new register read
+//   MUL  x = x * y[i]        (FMUL, two register operands)                                2
+//   PPP  (x, x') = (x, x') * (y, y') + (z, z')   FFMA2, three register pairs              6
+//   PSP  (x, x') = (x, x') * (y0, y0) + (z, z')  FFMA2, pair, broadcast scalar, pair      5
+template <int FORM>
+__global__ void __launch_bounds__(256) lm_fma_form_kernel(float *out, int iters, const float *in) {
+    float x[16], y[16], z[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        x[i] = (float)(threadIdx.x + i) * 1e-3f;
+        y[i] = in[i + (threadIdx.x & 3)];
+        z[i] = in[32 + i + (threadIdx.x & 3)];
+    }
+    for (int it = 0; it < iters; ++it) {
+        if (FORM == LM_FMA_FORM_PPP || FORM == LM_FMA_FORM_PSP) {
+#pragma unroll
+            for (int i = 0; i < 16; i += 2) {
+                const float2 yy = FORM == LM_FMA_FORM_PPP ? make_float2(y[i], y[i + 1]) : make_float2(y[0], y[0]);
+                const float2 r = __ffma2_rn(make_float2(x[i], x[i + 1]), yy, make_float2(z[i], z[i + 1]));
+                x[i] = r.x;
+                x[i + 1] = r.y;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 16; ++i)
+                x[i] = FORM == LM_FMA_FORM_RRS ? __fmaf_rn(x[i], y[0], z[i])
+                     : FORM == LM_FMA_FORM_RSS ? __fmaf_rn(x[i], y[0], z[0])
+                                               : __fmul_rn(x[i], y[i]);
+        }
+    }
+    float sum = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) sum += x[i];
+    if (sum == 12345.678f) out[0] = sum;
+}
+
 __global__ void lm_unpack_kernel(const uint32_t *__restrict__ its, int64_t W, int32_t *__restrict__ iters,
                                  uint32_t *__restrict__ status) {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -679,7 +717,7 @@ int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *
 int lm_fp32_peak(void *cuda_stream, double *tflops_out) { return lm_fp32_peak_form(cuda_stream, LM_FMA_FORM_RCC, tflops_out); }
 
 int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out) {
-    if (!tflops_out || (form != LM_FMA_FORM_RCC && form != LM_FMA_FORM_RRR)) return LM_EINVAL;
+    if (!tflops_out || form < LM_FMA_FORM_RCC || form > LM_FMA_FORM_PSP) return LM_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int dev = 0, sms = 0;
     LM_CUDA(cudaGetDevice(&dev));
@@ -699,13 +737,21 @@ int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out) {
     for (int rep = 0; rep < 6; ++rep) {
         cudaEventRecord(e0, st);
         g_launches.fetch_add(1);
-        if (form == LM_FMA_FORM_RCC) lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(scratch + 60, iters, 0.999f, 1e-3f);
-        else lm_fma_rrr_kernel<<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch);
+        switch (form) {
+        case LM_FMA_FORM_RCC: lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(scratch + 60, iters, 0.999f, 1e-3f); break;
+        case LM_FMA_FORM_RRR: lm_fma_rrr_kernel<<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
+        case LM_FMA_FORM_RRS: lm_fma_form_kernel<LM_FMA_FORM_RRS><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
+        case LM_FMA_FORM_RSS: lm_fma_form_kernel<LM_FMA_FORM_RSS><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
+        case LM_FMA_FORM_MUL: lm_fma_form_kernel<LM_FMA_FORM_MUL><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
+        case LM_FMA_FORM_PPP: lm_fma_form_kernel<LM_FMA_FORM_PPP><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
+        default: lm_fma_form_kernel<LM_FMA_FORM_PSP><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
+        }
         cudaEventRecord(e1, st);
         cudaError_t e = cudaEventSynchronize(e1);
         if (e != cudaSuccess) { cudaFree(scratch); return cuda_fail(e); }
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
+        // 2 flop per lane-operation also for the FMUL form: the figure is "lane-operations / s x 2", comparable across forms
         const double tf = 2.0 * 16.0 * iters * (double)blocks * threads / (ms * 1e-3) / 1e12;
         if (rep > 0 && tf > best) best = tf;
     }

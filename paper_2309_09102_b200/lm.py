@@ -34,7 +34,7 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_solve_host_workspace_bytes", "lm_solve_host",
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch",
            "lm_search_workspace_bytes", "lm_search_default_params", "lm_search")
-LM_FMA_FORM_RCC, LM_FMA_FORM_RRR = 0, 1
+LM_FMA_FORM_RCC, LM_FMA_FORM_RRR, LM_FMA_FORM_RRS, LM_FMA_FORM_RSS, LM_FMA_FORM_MUL, LM_FMA_FORM_PPP, LM_FMA_FORM_PSP = range(7)
 LM_SOLVER_PRIMAL, LM_SOLVER_DUAL = 0, 1
 LM_ROT_LOG, LM_ROT_RPY = 0, 1
 
