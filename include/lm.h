@@ -176,6 +176,11 @@ int lm_set_trace(lm_ctx *ctx, float *trial_q, float *trial_F);
  * residual / solver, unit weights and exact sincos (else LM_EINVAL).  Results agree with the default to rounding (the
  * summation order of the row sums differs), not bitwise. */
 #define LM_OPT_LANES_PER_WAYPOINT 3
+/* LM_OPT_TRAJ_FUSED (after lm_traj_attach, which resets it): where the trajectory-level step forms its normal equations.
+ * 1 = in the solve kernels' producer warps, straight into shared memory (nothing of J^T J, g, rho touches HBM), 2 = in
+ * per-waypoint kernels through HBM, 0 (default) = 1 when the batch has enough tiles of 32 trajectories to pay for it,
+ * else 2.  With collision rows the step always takes path 2.  Both paths return the same bits. */
+#define LM_OPT_TRAJ_FUSED 4
 int lm_set_option(lm_ctx *ctx, int32_t option, int32_t value);
 
 /* Name of the LM kernel variant this context launches: "panda7", "rand8" (compile-time chain

@@ -424,6 +424,10 @@ int lm_set_option(lm_ctx *c, int32_t option, int32_t value) {
         if (value != 0 && c->lanes > 1) return LM_EINVAL;
         c->use_generic = value != 0;
         return LM_OK;
+    case LM_OPT_TRAJ_FUSED:
+        if (value < 0 || value > 2 || !c->traj.attached) return LM_EINVAL;
+        c->traj.fused_mode = value;
+        return LM_OK;
     case LM_OPT_LANES_PER_WAYPOINT:
         if (value != 1 && value != 2 && value != 4) return LM_EINVAL;
         if (value > 1 && (c->spec_id == SPEC_GENERIC || c->use_generic || c->fast || c->args.weighted || c->args.variant != 0))

@@ -16,10 +16,11 @@
 // waypoint i of tile bt is the chunk  wid = bt * n + i,  and component c of lane l (trajectory
 // b = 32 bt + l) of a C-component array lives at  (wid * C + c) * 32 + l.  A warp therefore reads
 // or writes a chunk as C consecutive 128-byte lines, a tile's chunks for i = 0..n-1 are one
-// contiguous stream, and the solve kernel prefetches them with bulk-async copies
-// (cp.async.bulk + mbarrier) into a shared-memory ring several waypoints ahead of the
-// recurrence.  Lanes of the last tile beyond B are padding: they compute on whatever the
-// workspace holds and never store.
+// contiguous stream.  The normal equations of a waypoint never go to HBM: producer warps of the solve
+// kernel evaluate FK, the Jacobian and w_p^2 J^T J, g (or the refinement residual) of the next
+// waypoints straight into a shared-memory ring several waypoints ahead of the recurrence; what the
+// substitution reads back (-S^-1, z) arrives by bulk-async copies (cp.async.bulk + mbarrier).  Lanes of
+// the last tile beyond B are padding: they compute on whatever the workspace holds and never store.
 // Determinism: fixed summation orders, no float atomics; explicit round-to-nearest intrinsics.
 #pragma once
 #include "lm_coll.cuh"
@@ -39,13 +40,14 @@ struct TArgs {
     int32_t max_total;             // iteration cap per trajectory (mask width)
     const float *tp, *tq;          // targets: tile order [3], [4] comps; when shared: plain [3][n], [4][n]
     float *tp_w, *tq_w;            // the same arrays, writable (pack kernel)
-    float *q;                      // [2] x D comps     current / candidate joint values
-    float *Ag;                     // [2] x (NA + D)    w_p^2 J^T J (packed lower), then g = J^T r of the stacked residual
-    float *cst;                    // [2] x 3           |r_pose,i|^2, |q_{i+1} - q_i|^2 (0 for the last waypoint), collision cost
+    float *q;                      // [2] x D comps     current / candidate joint values (`sel` says which is current)
+    float *cst;                    // 3                 cost terms of the point last evaluated by tl_cost_kernel:
+                                   //                   |r_pose,i|^2, |q_{i+1} - q_i|^2 (0 for the last waypoint), collision cost
+    float *Ag;                     // NA + D            unfused path only: w_p^2 J^T J (packed lower), then g of the stacked residual
+    float *rho;                    // D                 unfused path only: refinement residual
     float *V;                      // NA                -(S_i)^-1
     float *z;                      // D
     float *delta;                  // D
-    float *rho;                    // D
     float *lam, *F, *Fp, *Fd, *Fc; // [Bt * 32] per trajectory
     uint32_t *its;                 // iters | status << 8
     unsigned long long *mask;
@@ -129,35 +131,6 @@ __device__ __forceinline__ void tl_load_target(const TArgs &A, const Slot &s, fl
     quat_to_cols(qv[0], qv[1], qv[2], qv[3], Rt);
 }
 
-// w_p^2 J^T J (packed lower) and g = w_p^2 J^T r + w_d^2 (c_i y_i - y_{i-1} - y_{i+1}) (y = the joint
-// values the Jacobian was taken at), |r_pose|^2 and |y_{i+1} - y_i|^2 of one waypoint -> buffer `dstsel`
-// Ac, gc, fc: the collision rows' J_c^T J_c (packed lower), J_c^T r_c and |r_c|^2 (zeros without capsules)
-template <int D>
-__device__ __forceinline__ void tl_store_normal(const TArgs &A, const Pose<D> &P, int dstsel, const Slot &s,
-                                                const float (&y)[D], const float (&ym)[D], const float (&yn)[D],
-                                                const float (&Ac)[Tri<D>::NA], const float (&gc)[D], float fc) {
-    constexpr int NA = Tri<D>::NA, C = NA + D;
-    const int n = A.n;
-    const float ci = (n == 1) ? 0.f : ((s.i == 0 || s.i == n - 1) ? 1.f : 2.f);
-    float *Ad = A.Ag + (int64_t)dstsel * C * A.nS;
-    float fd = 0.f;
-#pragma unroll
-    for (int r = 0; r < D; ++r) {
-#pragma unroll
-        for (int c = 0; c <= r; ++c) Ad[toff<C>(s.wid, tri(r, c), s.lane)] = fma_(A.wp2, coldot<D>(P, r, c), Ac[tri(r, c)]);
-        const float dd = sub(sub(mul(ci, y[r]), ym[r]), yn[r]);
-        Ad[toff<C>(s.wid, NA + r, s.lane)] = fma_(A.wd2, dd, fma_(A.wp2, colvec<D>(P, r, P.r), gc[r]));
-        if (s.i + 1 < n) {
-            const float t = sub(yn[r], y[r]);
-            fd = fma_(t, t, fd);
-        }
-    }
-    float *cd = A.cst + (int64_t)dstsel * 3 * A.nS;
-    cd[toff<3>(s.wid, 0, s.lane)] = P.F;
-    cd[toff<3>(s.wid, 1, s.lane)] = fd;
-    cd[toff<3>(s.wid, 2, s.lane)] = fc;
-}
-
 // FK + residual + Jacobian of one waypoint and, when capsules are set, its collision rows
 template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
 __device__ __forceinline__ void tl_eval_waypoint(const TArgs &A, const float (&q)[D], const float (&pt)[3], const float (&Rt)[3][3],
@@ -215,26 +188,147 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_clearance_ke
     A.clear_out[w] = mc;
 }
 
-// ---- assemble at the current point (entry of lm_traj_run): thread per waypoint
+// ---- what a producer warp of the solve kernel computes for waypoint i of its tile (lane = trajectory) into a ring
+// stage `st` ([C][32] floats, component c of lane l at st[c * 32 + l]); `qs` = the lane's CURRENT joint buffer.
+//   tl_chunk_normal: w_p^2 J^T J (+ collision rows; packed lower, NA entries) and
+//                    g = w_p^2 J^T r + w_d^2 (c_i y_i - y_{i-1} - y_{i+1}) (+ J_c^T r_c),  y = the joint values
+// the inputs of a chunk, loaded ahead of its turn by the fused producers (joint values of waypoints i-1, i, i+1 and the target)
+template <int D>
+struct ChunkIn {
+    float q[D], qm[D], qn[D], tg[7];
+};
+template <int D>
+__device__ __forceinline__ void tl_chunk_load(const TArgs &A, const float *qs, int64_t w0, int i, int lane, ChunkIn<D> &in) {
+    const int n = A.n;
+    const int64_t wid = w0 + i;
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        in.q[j] = qs[toff<D>(wid, j, lane)];
+        in.qm[j] = (i > 0) ? qs[toff<D>(wid - 1, j, lane)] : 0.f;
+        in.qn[j] = (i + 1 < n) ? qs[toff<D>(wid + 1, j, lane)] : 0.f;
+    }
+    if (A.shared_targets) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) in.tg[c] = __ldg(A.tp + (int64_t)c * n + i);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) in.tg[3 + c] = __ldg(A.tq + (int64_t)c * n + i);
+    } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) in.tg[c] = __ldg(A.tp + toff<3>(wid, c, lane));
+#pragma unroll
+        for (int c = 0; c < 4; ++c) in.tg[3 + c] = __ldg(A.tq + toff<4>(wid, c, lane));
+    }
+}
+
+template <int D, bool WEIGHTED, typename SpecT, bool COLL>
+__device__ __forceinline__ void tl_chunk_normal(const TArgs &A, const ChunkIn<D> &in, int i, int lane, float *st) {
+    constexpr int NA = Tri<D>::NA;
+    const int n = A.n;
+    const float (&q)[D] = in.q, (&qm)[D] = in.qm, (&qn)[D] = in.qn;
+    const float pt[3] = {in.tg[0], in.tg[1], in.tg[2]};
+    float Rt[3][3];
+    quat_to_cols(in.tg[3], in.tg[4], in.tg[5], in.tg[6], Rt);
+    Pose<D> P;
+    float Ac[NA], gc[D], fc;
+    tl_eval_waypoint<D, false, WEIGHTED, SpecT, COLL>(A, q, pt, Rt, P, Ac, gc, fc);
+    const float ci = (n == 1) ? 0.f : ((i == 0 || i == n - 1) ? 1.f : 2.f);
+#pragma unroll
+    for (int r = 0; r < D; ++r) {
+#pragma unroll
+        for (int c = 0; c <= r; ++c) st[tri(r, c) * 32 + lane] = fma_(A.wp2, coldot<D>(P, r, c), Ac[tri(r, c)]);
+        const float dd = sub(sub(mul(ci, q[r]), qm[r]), qn[r]);
+        st[(NA + r) * 32 + lane] = fma_(A.wd2, dd, fma_(A.wp2, colvec<D>(P, r, P.r), gc[r]));
+    }
+}
+
+//   tl_chunk_rho: the refinement residual (DESIGN R4 carried over to the stacked system)
+//     rho_i = -[ w_p^2 J_i^T (r_i + J_i delta_i) + w_d^2 (D^T D (q + delta))_i + lambda delta_i
+//               + sum over active collision pairs of g (r_c + g . delta_i) ]                  into st[0 .. D)
+template <int D, bool WEIGHTED, typename SpecT, bool COLL>
+__device__ __forceinline__ void tl_chunk_rho(const TArgs &A, const ChunkIn<D> &in, float lam, int64_t w0, int i, int lane, float *st) {
+    const int n = A.n;
+    const int64_t wid = w0 + i;
+    const float ci = (n == 1) ? 0.f : ((i == 0 || i == n - 1) ? 1.f : 2.f);
+    const float (&q)[D] = in.q;
+    float dl[D], dd[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        dl[j] = A.delta[toff<D>(wid, j, lane)];
+        const float yc = add(q[j], dl[j]);
+        const float ym = (i > 0) ? add(in.qm[j], A.delta[toff<D>(wid - 1, j, lane)]) : 0.f;
+        const float yn = (i + 1 < n) ? add(in.qn[j], A.delta[toff<D>(wid + 1, j, lane)]) : 0.f;
+        dd[j] = sub(sub(mul(ci, yc), ym), yn);
+    }
+    const float pt[3] = {in.tg[0], in.tg[1], in.tg[2]};
+    float Rt[3][3];
+    quat_to_cols(in.tg[3], in.tg[4], in.tg[5], in.tg[6], Rt);
+    Pose<D> P;
+    float ec[D]; // collision rows: sum over the active pairs of g (r + g . delta)
+#pragma unroll
+    for (int j = 0; j < D; ++j) ec[j] = 0.f;
+    if (COLL) {
+        Pose<D> Fr;
+        CapsWorld W;
+        CapsSink sink(A.caps, W);
+        sink.base();
+        float pf[3];
+        eval_pose<D, false, WEIGHTED, SpecT, false, CapsSink>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, Fr, nullptr, nullptr, pf, sink);
+        coll_rows<D, SpecT>(A.ch, A.caps, W, Fr, [&](const float (&g)[D], float r) {
+            float u = r;
+#pragma unroll
+            for (int j = 0; j < D; ++j) u = fma_(g[j], dl[j], u);
+#pragma unroll
+            for (int j = 0; j < D; ++j) ec[j] = fma_(g[j], u, ec[j]);
+        });
+        finish_jacobian<D, WEIGHTED, SpecT>(A.ch, Fr, pf, A.w_pos, A.w_rot, P);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) P.r[k] = Fr.r[k];
+    } else {
+        eval_pose<D, false, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+    }
+    float t[6];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        float sv = P.r[k], sw = P.r[3 + k];
+#pragma unroll
+        for (int j = 0; j < D; ++j) {
+            sv = fma_(P.Jv[j][k], dl[j], sv);
+            sw = fma_(P.Jw[j][k], dl[j], sw);
+        }
+        t[k] = sv; t[3 + k] = sw;
+    }
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        const float acc = add(fma_(lam, dl[j], fma_(A.wd2, dd[j], mul(A.wp2, colvec<D>(P, j, t)))), ec[j]);
+        st[j * 32 + lane] = -acc;
+    }
+}
+
+// ---- the unfused path (collision rows, or fewer tiles than the producers of a block can serve: lm_traj_api.cu): the same
+// chunks, one thread per waypoint, written to HBM (A.Ag / A.rho, one chunk = one "stage" in tile order) for the solve
+// kernel's producers to fetch with bulk-async copies.  Same functions, same bits as the fused path.
 template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_assemble_kernel(const __grid_constant__ TArgs A) {
     const Slot s = slot_of_thread(A);
     if (!s.valid) return;
-    const int sel = A.sel[s.b];
-    const float *qs = A.q + (int64_t)sel * D * A.nS;
-    float q[D], qm[D], qn[D];
-#pragma unroll
-    for (int j = 0; j < D; ++j) {
-        q[j] = qs[toff<D>(s.wid, j, s.lane)];
-        qm[j] = (s.i > 0) ? qs[toff<D>(s.wid - 1, j, s.lane)] : 0.f;
-        qn[j] = (s.i + 1 < A.n) ? qs[toff<D>(s.wid + 1, j, s.lane)] : 0.f;
-    }
-    float pt[3], Rt[3][3];
-    tl_load_target(A, s, pt, Rt);
-    Pose<D> P;
-    float Ac[Tri<D>::NA], gc[D], fc;
-    tl_eval_waypoint<D, FAST, WEIGHTED, SpecT, COLL>(A, q, pt, Rt, P, Ac, gc, fc);
-    tl_store_normal<D>(A, P, sel, s, q, qm, qn, Ac, gc, fc);
+    const uint32_t pk = A.its[s.b];
+    if ((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0)) return;
+    constexpr int C = Tri<D>::NA + D;
+    const float *qs = A.q + (int64_t)A.sel[s.b] * D * A.nS;
+    ChunkIn<D> in;
+    tl_chunk_load<D>(A, qs, s.wid - s.i, s.i, s.lane, in);
+    tl_chunk_normal<D, WEIGHTED, SpecT, COLL>(A, in, s.i, s.lane, A.Ag + s.wid * C * 32);
+}
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
+__global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(const __grid_constant__ TArgs A) {
+    const Slot s = slot_of_thread(A);
+    if (!s.valid) return;
+    const uint32_t pk = A.its[s.b];
+    if ((pk & 0xffu) >= (uint32_t)A.max_total || !A.ok[s.b] || (A.gate != nullptr && A.gate[s.b] == 0)) return;
+    const float *qs = A.q + (int64_t)A.sel[s.b] * D * A.nS;
+    ChunkIn<D> in;
+    tl_chunk_load<D>(A, qs, s.wid - s.i, s.i, s.lane, in);
+    tl_chunk_rho<D, WEIGHTED, SpecT, COLL>(A, in, A.lam[s.b], s.wid - s.i, s.i, s.lane, A.rho + s.wid * D * 32);
 }
 
 // Kahan-compensated sum step (explicit intrinsics: the compiler cannot simplify the compensation away)
@@ -245,14 +339,14 @@ __device__ __forceinline__ void kahan_add(float &s, float &c, float x) {
     s = t;
 }
 
-// Total cost of buffer `sel` of the trajectory (tile = blockIdx.x, lane): a block of TL_SUM_WARPS warps
+// Total cost of the point tl_cost_kernel evaluated last (tile = blockIdx.x, lane): a block of TL_SUM_WARPS warps
 // per tile; warp w sums the waypoints of segment w in order (Kahan), the segment sums are then added
 // in segment order.  The summation order depends on n only, never on the batch.  All threads of the
 // block must call; the result is valid in warp 0.
 constexpr int TL_SUM_WARPS = 8;
-__device__ __forceinline__ void tl_sum_cost(const TArgs &A, int sel, float (*part)[3][32], float &Fp, float &Fd, float &Fc, float &F) {
+__device__ __forceinline__ void tl_sum_cost(const TArgs &A, float (*part)[3][32], float &Fp, float &Fd, float &Fc, float &F) {
     const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
-    const float *cp = A.cst + (int64_t)sel * 3 * A.nS;
+    const float *cp = A.cst;
     const int64_t w0 = (int64_t)blockIdx.x * A.n;
     const int seg = (A.n + TL_SUM_WARPS - 1) / TL_SUM_WARPS;
     const int i0 = wp * seg, i1 = min(A.n, i0 + seg);
@@ -292,7 +386,7 @@ __global__ void __launch_bounds__(TL_SUM_WARPS * 32) tl_init_cost_kernel(const _
     const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
     const bool valid = b < A.B;
     float Fp, Fd, Fc, F;
-    tl_sum_cost(A, valid ? A.sel[b] : 0, part, Fp, Fd, Fc, F);
+    tl_sum_cost(A, part, Fp, Fd, Fc, F);
     if (!valid || threadIdx.x >= 32) return;
     A.Fp[b] = Fp; A.Fd[b] = Fd; A.Fc[b] = Fc; A.F[b] = F;
 }
@@ -372,28 +466,39 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 #endif
 
 // One ring stage (floats): [0, NA*32) matrix, then vector 1 (D*32) and, in MODE 1, vector 2 (D*32).
-// Each of the two chain warps of a block has its own rings; MODE 0 keeps two per warp (one per Ag buffer:
-// accept / reject is per trajectory, so the lanes of a tile may select different buffers; a
-// buffer no lane of the tile selects is not fetched).
+// Each of the two chain warps of a block has its own ring.
 template <int D, int MODE> __host__ __device__ constexpr int tl_stage_floats() { return (Tri<D>::NA + (MODE == 0 ? D : 2 * D)) * 32; }
-// Waypoints in flight per chain warp in the solve kernel: WANT, cut to what the shared-memory budget holds.  Measured
-// on B200 (n = 300, us per iteration at B = 4096 / 16384, with the producer warp): 2 stages 486 / 1276, 3: 425 / 1363,
-// 4: 403 / 1279, 6: 393 / 1329, 8: 387 / -- (8192: 707 vs 640 with 4).  A deeper ring helps while every SM holds one
-// block (the chain is latency-bound and more chunks are in flight) and costs occupancy once there are more tiles than
-// SMs: the launch takes TL_STAGES_DEEP when the tiles fit one per SM, TL_STAGES_SHALLOW otherwise (powers of two:
-// the stage index is a mask).
-constexpr int TL_STAGES_SHALLOW = 4, TL_STAGES_DEEP = 8;
-template <int D, int MODE, int WANT> __host__ __device__ constexpr int tl_stages() {
-    const size_t per_stage = (size_t)2 * (MODE == 0 ? 2 : 1) * tl_stage_floats<D, MODE>() * sizeof(float);
+// Waypoints in flight per chain warp in the solve kernel: TL_STAGES_WANT, cut to what the shared-memory budget holds
+// (a power of two is not required).  Round 1, when the stages were filled from HBM (n = 300, us per iteration at
+// B = 4096 / 16384): 2 stages 486 / 1276, 4: 403 / 1279, 8: 387 / --.
+#ifndef LM_TL_STAGES
+#define LM_TL_STAGES 8
+#endif
+constexpr int TL_STAGES_WANT = LM_TL_STAGES;
+// Block shapes of the solve kernel (chosen per launch, lm_traj_launch.h): warps 0, 1 are the chains, every further warp is
+// a producer and serves chain (warp & 1).  Measured on B200, n = 300, ms per iteration with one refinement step (fused
+// path; threads per block = 32 (2 + 2 producers per chain)):      256      320      384      512
+//                                     4096 trajectories (128 tiles, one block per SM)     0.341    0.340    0.326    0.328
+//                                     16384 trajectories (512 tiles)                      1.102    1.350    1.300    1.299
+// Keeping the producers off the two scheduler partitions the chains run on (idle warps in between) made no difference
+// (0.336 with 4 producers per chain).  A producer warp is never two ring turns ahead of its own last wait as long as
+// producers per chain <= ring stages.
+constexpr int TL_SOLVE_MAX_THREADS = 512;
+constexpr int TL_SOLVE_THREADS_MANY_TILES = 256; // more tiles than SMs: 2 chains + 3 producers each, two blocks per SM
+constexpr int TL_SOLVE_THREADS_FEW_TILES = 384;  // at most one block per SM: 2 chains + 5 producers each
+constexpr int TL_SOLVE_THREADS_HBM = 128;        // unfused: 2 chains + 1 copy-issuing producer each
+static_assert((TL_SOLVE_THREADS_FEW_TILES / 32 - 2) / 2 <= TL_STAGES_WANT, "more producers per chain than ring stages");
+template <int D, int MODE> __host__ __device__ constexpr int tl_stages() {
+    const size_t per_stage = (size_t)2 * tl_stage_floats<D, MODE>() * sizeof(float);
     const int fit = (int)((size_t)LM_TL_STAGE_BUDGET / per_stage);
-    return fit > WANT ? WANT : fit;
+    return fit > TL_STAGES_WANT ? TL_STAGES_WANT : fit;
 }
-template <int D, int MODE, int WANT> __host__ __device__ constexpr size_t tl_solve_smem_bytes() {
-    return (size_t)2 * (MODE == 0 ? 2 : 1) * tl_stages<D, MODE, WANT>() * tl_stage_floats<D, MODE>() * sizeof(float);
+template <int D, int MODE> __host__ __device__ constexpr size_t tl_solve_smem_bytes() {
+    return (size_t)2 * tl_stages<D, MODE>() * tl_stage_floats<D, MODE>() * sizeof(float);
 }
 
-// ---- block-tridiagonal solve: one block of two chain warps (+ their two producer warps) per tile of 32 trajectories,
-// lane = trajectory.
+// ---- block-tridiagonal solve: one block per tile of 32 trajectories -- two chain warps and a few producer warps for
+// each of them -- lane = trajectory.
 // Two-sided ("twisted") block elimination halves the sequential chain: with m = n / 2,
 //   warp 0 eliminates i = 0, 1, .., m-1      (S_i = T_i - w_d^4 S_{i-1}^-1,  h_i = g_i + w_d^2 z_{i-1}),
 //   warp 1 eliminates i = n-1, n-2, .., m+1  (S_i = T_i - w_d^4 S_{i+1}^-1,  h_i = g_i + w_d^2 z_{i+1}),
@@ -402,33 +507,41 @@ template <int D, int MODE, int WANT> __host__ __device__ constexpr size_t tl_sol
 // and both substitute outwards from x_m:  x_i = z_i + w_d^2 S_i^-1 x_{i+-1}.
 //   MODE 0: factor (stores W_i = -S_i^-1) and solve for g;                      delta  = -x
 //   MODE 1: re-solve with the stored W_i for rho (iterative refinement);        delta +=  x
-// The chunks of the next tl_stages<D, MODE, WANT>() waypoints of a warp's sequence are in flight (bulk-async copies
-// into its ring) while it eliminates the current one.  Two more warps are the producers of the two chains' rings: one lane of each
-// waits for a stage to be released ("empty" mbarrier, armed by the consumer once all its lanes have read the stage),
-// posts the byte count on the stage's "full" mbarrier and issues the copies -- the address arithmetic, the
-// uniform-register traffic of UBLKCP and the divergent lane-0 branch (38 % of the refinement re-solve's issue slots
-// when every warp fed its own ring) are off the two sequential chains.
-constexpr int TL_SOLVE_THREADS = 128;
-template <int D, int MODE, int WANT>
-__global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid_constant__ TArgs A) {
-    constexpr int NA = Tri<D>::NA, CA = NA + D, SF = tl_stage_floats<D, MODE>(), NR = (MODE == 0) ? 2 : 1;
-    constexpr int TL_STAGES = tl_stages<D, MODE, WANT>();
+// What a chain consumes is PRODUCED IN THE BLOCK, not fetched: the producer warps of a chain take the waypoints of its
+// sequence round robin and write T_i (without the diagonal shift) and g_i (MODE 0: tl_chunk_normal) or rho_i (MODE 1:
+// tl_chunk_rho, next to the bulk-async copy of W_i) into the chain's shared-memory ring, up to TL_STAGES waypoints ahead of the
+// recurrence; w_p^2 J^T J, g and rho never exist in HBM.  Per stage an "empty" mbarrier (armed by the consumer's lane 0
+// once all its lanes have read the stage) and a "full" one (the producer's lane 0 arrives after its warp's stores; the
+// byte count of a bulk copy is posted on the same barrier).  For the substitution phase producer 0 of each chain issues
+// the bulk-async copies of W_i, z_i (and the old delta_i) as before.  The chains only wait, load and compute.
+// fewer tiles than this: the unfused path (every SM assembles) beats a few producer warps per chain (lm_traj_api.cu)
+#ifndef LM_TL_FUSED_MIN_TILES
+#define LM_TL_FUSED_MIN_TILES 96
+#endif
+constexpr int64_t TL_FUSED_MIN_TILES = LM_TL_FUSED_MIN_TILES;
+// FUSED = false: the chunks come from HBM instead (A.Ag / A.rho, written by tl_assemble_kernel / tl_rho_kernel): producer
+// 0 of each chain fetches them with bulk-async copies, the other producer warps idle.
+template <int D, int MODE, bool FUSED, bool WEIGHTED, typename SpecT>
+__global__ void __launch_bounds__(TL_SOLVE_MAX_THREADS) tl_solve_kernel(const __grid_constant__ TArgs A) {
+    constexpr int NA = Tri<D>::NA, SF = tl_stage_floats<D, MODE>();
+    constexpr int TL_STAGES = tl_stages<D, MODE>();
+    constexpr uint32_t FULL_COUNT = (FUSED && MODE == 1) ? 2u : 1u; // fused MODE 1: the poster of the copy's byte count + the writer of rho
     extern __shared__ __align__(128) float smem[];
     __shared__ __align__(8) uint64_t full_all[2][TL_STAGES], empty_all[2][TL_STAGES];
     __shared__ float xch[NA + D][32]; // warp 1 -> warp 0: W_{m+1}, z_{m+1}
     __shared__ float xmid[D][32];     // warp 0 -> both: x_m
     __shared__ int okx[2][32];
-    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5; // warps 0, 1: the two chains; warps 2, 3: their producers
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5; // warps 0, 1: the two chains; warps 2..: their producers
+    const int npw = ((int)(blockDim.x >> 5) - 2) / 2; // producer warps per chain
+    const int pq = wp & 1, pi = (wp - 2) >> 1;         // a producer's chain and its index among that chain's producers
     const int64_t bt = blockIdx.x;
     const int64_t b = bt * 32 + lane;
     const bool valid = b < A.B;
     const uint32_t pk = valid ? A.its[b] : 0xffu;
     const bool active = valid && ((pk & 0xffu) < (uint32_t)A.max_total) && (MODE == 0 || A.ok[b] != 0) &&
                         (A.gate == nullptr || A.gate[b] != 0);
-    if (!__any_sync(0xffffffffu, active)) return; // the same lanes in all four warps: block-uniform
+    if (!__any_sync(0xffffffffu, active)) return; // the same lanes in every warp: block-uniform
     const int sel = valid ? A.sel[b] : 0;
-    const bool need0 = __any_sync(0xffffffffu, active && sel == 0); // warp-uniform, the same in all four warps
-    const bool need1 = __any_sync(0xffffffffu, active && sel == 1);
     const int n = A.n;
     const int64_t w0 = bt * n;
     const int m = n / 2;
@@ -440,56 +553,83 @@ __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < TL_STAGES; ++s) {
-            mbar_init(&full_all[0][s], 1); mbar_init(&full_all[1][s], 1);
+            mbar_init(&full_all[0][s], FULL_COUNT); mbar_init(&full_all[1][s], FULL_COUNT);
             mbar_init(&empty_all[0][s], 1); mbar_init(&empty_all[1][s], 1);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (wp >= 2) { // ---- the producers: warp 2 feeds the rings of warp 0, warp 3 those of warp 1
-        const int q = wp - 2;
-        auto ring_of = [&](int q) { return smem + (size_t)q * NR * TL_STAGES * SF; };
-        auto issue_fwd = [&](int q, int k) { // k = position in warp q's sequence of ring uses
-            const int s = k % TL_STAGES;
-            uint64_t *bar = &full_all[q][s];
-            const int64_t wid = w0 + idx_of(q, k);
-            float *dst = ring_of(q) + (size_t)s * SF;
-            if (MODE == 0) {
-                const uint32_t bytes = CA * 128u;
-                mbar_expect_tx(bar, (need0 ? bytes : 0u) + (need1 ? bytes : 0u));
-                if (need0) bulk_g2s(dst, A.Ag + wid * CA * 32, bytes, bar);
-                if (need1) bulk_g2s(dst + (size_t)TL_STAGES * SF, A.Ag + (int64_t)CA * A.nS + wid * CA * 32, bytes, bar);
-            } else {
-                mbar_expect_tx(bar, (NA + D) * 128u);
-                bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, bar);
-                bulk_g2s(dst + NA * 32, A.rho + wid * D * 32, D * 128u, bar);
+    if (wp >= 2) { // ---- the producers: warps 2, 4, 6, .. feed the ring of warp 0, warps 3, 5, 7, .. that of warp 1
+        const int q = pq;
+        float *ring_q = smem + (size_t)q * TL_STAGES * SF;
+        const float *qs = A.q + (int64_t)sel * D * A.nS; // the lane's current joint buffer
+        const float lam = valid ? A.lam[b] : 1.f;
+        // use u of a stage may be filled once use u - TL_STAGES has been released (uses are numbered per chain, both
+        // phases).  A producer is never two ring turns ahead of the consumer (producers per chain <= TL_STAGES), so the parity is unambiguous.
+        auto wait_free = [&](int k) {
+            if (k >= TL_STAGES) {
+                if (lane == 0) mbar_wait(&empty_all[q][k % TL_STAGES], (uint32_t)(((k / TL_STAGES) - 1) & 1));
+                __syncwarp();
             }
         };
-        auto issue_bwd = [&](int q, int kk, int i) {
-            const int s = kk % TL_STAGES;
-            uint64_t *bar = &full_all[q][s];
-            float *dst = ring_of(q) + (size_t)s * SF;
-            const int64_t wid = w0 + i;
-            mbar_expect_tx(bar, (NA + D + (MODE == 1 ? D : 0)) * 128u);
-            bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, bar);
-            bulk_g2s(dst + NA * 32, A.z + wid * D * 32, D * 128u, bar);
-            if (MODE == 1) bulk_g2s(dst + (NA + D) * 32, A.delta + wid * D * 32, D * 128u, bar);
-        };
-        // use u of a stage may be filled once use u - 1 has been released (uses are numbered per warp, both phases)
-        auto wait_free = [&](int q, int k) {
-            if (k >= TL_STAGES) mbar_wait(&empty_all[q][k % TL_STAGES], (uint32_t)(((k / TL_STAGES) - 1) & 1));
-        };
-        if (lane == 0) {
-            const int u = uses1_of(q);
-            for (int k = 0; k < u; ++k) { wait_free(q, k); issue_fwd(q, k); }
+        const int u = uses1_of(q);
+        if (FUSED) {
+            // the inputs of a producer's NEXT chunk are requested before it waits for / computes the current one
+            ChunkIn<D> nxt;
+            if (pi < u) tl_chunk_load<D>(A, qs, w0, idx_of(q, pi), lane, nxt);
+            for (int k = pi; k < u; k += npw) {
+                const int s = k % TL_STAGES;
+                const ChunkIn<D> cur = nxt;
+                if (k + npw < u) tl_chunk_load<D>(A, qs, w0, idx_of(q, k + npw), lane, nxt);
+                wait_free(k);
+                float *st = ring_q + (size_t)s * SF;
+                const int i = idx_of(q, k);
+                if (MODE == 0) {
+                    tl_chunk_normal<D, WEIGHTED, SpecT, false>(A, cur, i, lane, st);
+                } else {
+                    if (lane == 0) {
+                        mbar_expect_tx(&full_all[q][s], NA * 128u);
+                        bulk_g2s(st, A.V + (w0 + i) * NA * 32, NA * 128u, &full_all[q][s]);
+                    }
+                    tl_chunk_rho<D, WEIGHTED, SpecT, false>(A, cur, lam, w0, i, lane, st + NA * 32);
+                }
+                __syncwarp(); // every lane's stores precede the arrival below
+                if (lane == 0) mbar_arrive(&full_all[q][s]);
+            }
+        } else if (pi == 0 && lane == 0) {
+            for (int k = 0; k < u; ++k) {
+                const int s = k % TL_STAGES;
+                if (k >= TL_STAGES) mbar_wait(&empty_all[q][s], (uint32_t)(((k / TL_STAGES) - 1) & 1));
+                uint64_t *bar = &full_all[q][s];
+                float *dst = ring_q + (size_t)s * SF;
+                const int64_t wid = w0 + idx_of(q, k);
+                mbar_expect_tx(bar, (NA + D) * 128u);
+                if (MODE == 0) {
+                    bulk_g2s(dst, A.Ag + wid * (NA + D) * 32, (NA + D) * 128u, bar);
+                } else {
+                    bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, bar);
+                    bulk_g2s(dst + NA * 32, A.rho + wid * D * 32, D * 128u, bar);
+                }
+            }
         }
         __syncthreads(); // (1) warp 1 has handed its last block to warp 0
         __syncthreads(); // (2) the chunks written by the elimination are ordered before the copies below
         fence_proxy_async();
-        if (lane == 0) {
-            const int l = len_of(q), u = uses1_of(q);
-            for (int j = 0; j < l; ++j) { wait_free(q, u + j); issue_bwd(q, u + j, idx_of(q, l - 1 - j)); }
+        if (pi == 0 && lane == 0) {
+            const int l = len_of(q);
+            for (int j = 0; j < l; ++j) {
+                const int kk = u + j, s = kk % TL_STAGES;
+                if (kk >= TL_STAGES) mbar_wait(&empty_all[q][s], (uint32_t)(((kk / TL_STAGES) - 1) & 1));
+                uint64_t *bar = &full_all[q][s];
+                float *dst = ring_q + (size_t)s * SF;
+                const int64_t wid = w0 + idx_of(q, l - 1 - j);
+                mbar_expect_tx(bar, (NA + D + (MODE == 1 ? D : 0)) * 128u);
+                bulk_g2s(dst, A.V + wid * NA * 32, NA * 128u, bar);
+                bulk_g2s(dst + NA * 32, A.z + wid * D * 32, D * 128u, bar);
+                if (MODE == 1) bulk_g2s(dst + (NA + D) * 32, A.delta + wid * D * 32, D * 128u, bar);
+                if (FULL_COUNT == 2u) mbar_arrive(bar); // the barrier counts two arrivals per use in the fused MODE 1
+            }
         }
         __syncthreads(); // (3) the verdicts of the two chains
         return;
@@ -497,8 +637,7 @@ __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid
 
     // ---- the two chains
     const float lam = valid ? A.lam[b] : 1.f;
-    float *ring = smem + (size_t)wp * NR * TL_STAGES * SF;
-    float *ring1 = ring + (size_t)TL_STAGES * SF; // MODE 0 only: chunks of Ag buffer 1
+    float *ring = smem + (size_t)wp * TL_STAGES * SF;
     uint64_t *bars = full_all[wp], *empt = empty_all[wp];
     const int len = len_of(wp);
     const int uses1 = uses1_of(wp);
@@ -510,14 +649,13 @@ __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid
 #pragma unroll
     for (int j = 0; j < D; ++j) zp[j] = 0.f;
     bool ok = true;
-    const float *my_ring = (MODE == 0 && sel == 1) ? ring1 : ring;
 
     // one elimination step on the chunk in stage k of this warp's ring; `Wo`, `zo`: the contribution of the
     // other side (only at the middle block), zero otherwise
     auto eliminate = [&](int k, int i, const float (&Wo)[NA], const float (&zo)[D], bool middle) {
         const int s = k % TL_STAGES;
         mbar_wait(&bars[s], (uint32_t)((k / TL_STAGES) & 1));
-        const float *st = my_ring + (size_t)s * SF;
+        const float *st = ring + (size_t)s * SF;
         float S[NA], rhs[D];
 #pragma unroll
         for (int t = 0; t < NA; ++t) S[t] = st[t * 32 + lane];
@@ -641,139 +779,75 @@ __global__ void __launch_bounds__(TL_SOLVE_THREADS) tl_solve_kernel(const __grid
     }
 }
 
-// ---- refinement residual (DESIGN R4 carried over to the stacked system): thread per waypoint
-//   rho_i = -[ w_p^2 J_i^T (r_i + J_i delta_i) + w_d^2 (D^T D (q + delta))_i + lambda delta_i
-//             + sum over active collision pairs of g (r_c + g . delta_i) ]
-template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
-__global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(const __grid_constant__ TArgs A) {
-    const Slot s = slot_of_thread(A);
-    if (!s.valid) return;
-    const uint32_t pk = A.its[s.b];
-    const int okf = A.ok[s.b];
-    const int sel = A.sel[s.b];
-    const float lam = A.lam[s.b];
-    const float *q0 = A.q, *q1 = A.q + (int64_t)D * A.nS;
-    const int n = A.n;
-    const float ci = (n == 1) ? 0.f : ((s.i == 0 || s.i == n - 1) ? 1.f : 2.f);
-    float ra[3][D], rb[3][D], rd[3][D]; // both buffers are fetched, `sel` picks afterwards (see tl_trial_kernel)
-#pragma unroll
-    for (int u = 0; u < 3; ++u) {
-        const bool there = (u == 0) ? (s.i > 0) : (u == 2) ? (s.i + 1 < n) : true;
-        const int64_t wid = s.wid + u - 1;
-#pragma unroll
-        for (int j = 0; j < D; ++j) {
-            ra[u][j] = there ? q0[toff<D>(wid, j, s.lane)] : 0.f;
-            rb[u][j] = there ? q1[toff<D>(wid, j, s.lane)] : 0.f;
-            rd[u][j] = there ? A.delta[toff<D>(wid, j, s.lane)] : 0.f;
-        }
-    }
-    if ((pk & 0xffu) >= (uint32_t)A.max_total || !okf || (A.gate != nullptr && A.gate[s.b] == 0)) return;
-    float q[D], dl[D], dd[D];
-#pragma unroll
-    for (int j = 0; j < D; ++j) {
-        q[j] = sel ? rb[1][j] : ra[1][j];
-        dl[j] = rd[1][j];
-        const float yc = add(q[j], dl[j]);
-        const float ym = (s.i > 0) ? add(sel ? rb[0][j] : ra[0][j], rd[0][j]) : 0.f;
-        const float yn = (s.i + 1 < n) ? add(sel ? rb[2][j] : ra[2][j], rd[2][j]) : 0.f;
-        dd[j] = sub(sub(mul(ci, yc), ym), yn);
-    }
-    float pt[3], Rt[3][3];
-    tl_load_target(A, s, pt, Rt);
-    Pose<D> P;
-    float ec[D]; // collision rows: sum over the active pairs of g (r + g . delta)
-#pragma unroll
-    for (int j = 0; j < D; ++j) ec[j] = 0.f;
-    if (COLL) {
-        Pose<D> Fr;
-        CapsWorld W;
-        CapsSink sink(A.caps, W);
-        sink.base();
-        float pf[3];
-        eval_pose<D, FAST, WEIGHTED, SpecT, false, CapsSink>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, Fr, nullptr, nullptr, pf, sink);
-        coll_rows<D, SpecT>(A.ch, A.caps, W, Fr, [&](const float (&g)[D], float r) {
-            float u = r;
-#pragma unroll
-            for (int j = 0; j < D; ++j) u = fma_(g[j], dl[j], u);
-#pragma unroll
-            for (int j = 0; j < D; ++j) ec[j] = fma_(g[j], u, ec[j]);
-        });
-        finish_jacobian<D, WEIGHTED, SpecT>(A.ch, Fr, pf, A.w_pos, A.w_rot, P);
-#pragma unroll
-        for (int k = 0; k < 6; ++k) P.r[k] = Fr.r[k];
-    } else {
-        eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
-    }
-    float t[6];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        float sv = P.r[k], sw = P.r[3 + k];
-#pragma unroll
-        for (int j = 0; j < D; ++j) {
-            sv = fma_(P.Jv[j][k], dl[j], sv);
-            sw = fma_(P.Jw[j][k], dl[j], sw);
-        }
-        t[k] = sv; t[3 + k] = sw;
-    }
-#pragma unroll
-    for (int j = 0; j < D; ++j) {
-        const float acc = add(fma_(lam, dl[j], fma_(A.wd2, dd[j], mul(A.wp2, colvec<D>(P, j, t)))), ec[j]);
-        A.rho[toff<D>(s.wid, j, s.lane)] = -acc;
-    }
-}
-
-// ---- trial point: q+ = clamp(q + delta), its cost terms and its normal equations
-//      into the candidate buffer (1 - sel): thread per waypoint
-template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
-__global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_trial_kernel(const __grid_constant__ TArgs A) {
+// ---- cost of a point: thread per waypoint.
+//   INIT = false: the trial point q+ = clamp(q + delta) -> the candidate joint buffer (1 - sel), its cost
+//                 terms -> cst.  Only FK and the residual are evaluated: the Jacobian of an accepted point is formed by the
+//                 next solve's producers.
+//   INIT = true:  the cost terms of the current point (entry of lm_traj_run).
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL, bool INIT>
+__global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(const __grid_constant__ TArgs A) {
     const Slot s = slot_of_thread(A);
     if (!s.valid) return;
     // every load below is issued before the first use: the joint values of BOTH buffers are fetched and the
     // trajectory's `sel` picks afterwards (a dependent address would cost one more DRAM round trip)
     const uint32_t pk = A.its[s.b];
     const int sel = A.sel[s.b];
-    const bool ok = A.ok[s.b] != 0;
+    const bool ok = INIT ? false : (A.ok[s.b] != 0);
     const float *q0 = A.q, *q1 = A.q + (int64_t)D * A.nS;
-    float ra[3][D], rb[3][D], rd[3][D];
+    float ra[2][D], rb[2][D], rd[2][D]; // this waypoint and the next one (the differencing cost of row i)
 #pragma unroll
-    for (int u = 0; u < 3; ++u) {
-        const bool there = (u == 0) ? (s.i > 0) : (u == 2) ? (s.i + 1 < A.n) : true;
-        const int64_t wid = s.wid + u - 1;
+    for (int u = 0; u < 2; ++u) {
+        const bool there = (u == 0) || (s.i + 1 < A.n);
+        const int64_t wid = s.wid + u;
 #pragma unroll
         for (int j = 0; j < D; ++j) {
             ra[u][j] = there ? q0[toff<D>(wid, j, s.lane)] : 0.f;
             rb[u][j] = there ? q1[toff<D>(wid, j, s.lane)] : 0.f;
-            rd[u][j] = there ? A.delta[toff<D>(wid, j, s.lane)] : 0.f;
+            rd[u][j] = (there && !INIT) ? A.delta[toff<D>(wid, j, s.lane)] : 0.f;
         }
     }
     float pt[3], Rt[3][3];
     tl_load_target(A, s, pt, Rt);
-    if ((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0)) return;
-    float *qd = A.q + (int64_t)(1 - sel) * D * A.nS;
-    float qt[D], qm[D], qn[D];
+    if (!INIT && ((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0))) return;
+    float qt[D], qn[D];
     bool clamped = false;
-    auto trial_of = [&](int u, int j, bool &cl) {
+    auto point_of = [&](int u, int j, bool &cl) {
         const float qv = sel ? rb[u][j] : ra[u][j];
+        if (INIT) return qv;
         const float t = ok ? add(qv, rd[u][j]) : qv;
         const float c = fminf(fmaxf(t, A.ch.lo[j]), A.ch.hi[j]);
         cl = cl || (c != t);
         return c;
     };
+    float fd = 0.f;
 #pragma unroll
     for (int j = 0; j < D; ++j) {
         bool dummy = false;
-        qt[j] = trial_of(1, j, clamped);
-        qm[j] = (s.i > 0) ? trial_of(0, j, dummy) : 0.f;
-        qn[j] = (s.i + 1 < A.n) ? trial_of(2, j, dummy) : 0.f;
-        qd[toff<D>(s.wid, j, s.lane)] = qt[j];
+        qt[j] = point_of(0, j, clamped);
+        qn[j] = (s.i + 1 < A.n) ? point_of(1, j, dummy) : 0.f;
+        if (!INIT) A.q[(int64_t)(1 - sel) * D * A.nS + toff<D>(s.wid, j, s.lane)] = qt[j];
+        if (s.i + 1 < A.n) {
+            const float t = sub(qn[j], qt[j]);
+            fd = fma_(t, t, fd);
+        }
     }
     // "a trial point of this trajectory was clamped": integer atomic (order-free), skipped once the bit is seen set
-    if (clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
+    if (!INIT && clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
+    float fc = 0.f;
     Pose<D> P;
-    float Ac[Tri<D>::NA], gc[D], fc;
-    tl_eval_waypoint<D, FAST, WEIGHTED, SpecT, COLL>(A, qt, pt, Rt, P, Ac, gc, fc);
-    tl_store_normal<D>(A, P, 1 - sel, s, qt, qm, qn, Ac, gc, fc);
-    if (A.trace_q != nullptr) {
+    if (COLL) {
+        CapsWorld W;
+        CapsSink sink(A.caps, W);
+        sink.base();
+        eval_pose<D, FAST, WEIGHTED, SpecT, false, CapsSink>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr, nullptr, sink);
+        coll_rows<D, SpecT>(A.ch, A.caps, W, P, [&](const float (&)[D], float r) { fc = fma_(r, r, fc); });
+    } else {
+        eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+    }
+    A.cst[toff<3>(s.wid, 0, s.lane)] = P.F;
+    A.cst[toff<3>(s.wid, 1, s.lane)] = fd;
+    A.cst[toff<3>(s.wid, 2, s.lane)] = fc;
+    if (!INIT && A.trace_q != nullptr) {
         const int64_t W = A.B * A.n, w = s.b * A.n + s.i;
 #pragma unroll
         for (int j = 0; j < D; ++j) A.trace_q[(int64_t)j * W + w] = qt[j];
@@ -788,7 +862,7 @@ __global__ void __launch_bounds__(TL_SUM_WARPS * 32) tl_decide_kernel(const __gr
     const bool valid = b < A.B;
     const int s = valid ? A.sel[b] : 0;
     float Fp, Fd, Fc, Ft;
-    tl_sum_cost(A, 1 - s, part, Fp, Fd, Fc, Ft);
+    tl_sum_cost(A, part, Fp, Fd, Fc, Ft);
     if (!valid || threadIdx.x >= 32) return;
     uint32_t pk = A.its[b];
     uint32_t k = pk & 0xffu, st = pk >> 8;

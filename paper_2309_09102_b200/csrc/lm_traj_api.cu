@@ -13,7 +13,7 @@ using namespace lmk;
 namespace {
 
 struct TLayout {
-    size_t tp, tq, q, Ag, cst, V, z, delta, rho, lam, F, Fp, Fd, Fc, its, mask, sel, ok, totals, ui, us, total;
+    size_t tp, tq, q, Ag, rho, cst, V, z, delta, lam, F, Fp, Fd, Fc, its, mask, sel, ok, totals, ui, us, total;
 };
 
 // tile order (lm_traj.cuh): Bt = ceil(B / 32) tiles, nS = Bt * n * 32 slots, C floats per slot and array
@@ -25,12 +25,12 @@ TLayout make_tlayout(int d, int64_t B, int64_t n) {
     L.tp = take(4 * 3 * nS);
     L.tq = take(4 * 4 * nS);
     L.q = take(4 * 2 * d * nS);
-    L.Ag = take(4 * 2 * (NA + d) * nS);
-    L.cst = take(4 * 2 * 3 * nS);
+    L.Ag = take(4 * (NA + d) * nS);
+    L.rho = take(4 * d * nS);
+    L.cst = take(4 * 3 * nS);
     L.V = take(4 * NA * nS);
     L.z = take(4 * d * nS);
     L.delta = take(4 * d * nS);
-    L.rho = take(4 * d * nS);
     L.lam = take(4 * Bp);
     L.F = take(4 * Bp);
     L.Fp = take(4 * Bp);
@@ -60,8 +60,7 @@ cudaError_t launch_pose(lm_ctx *c, int which, const TArgs &a) {
 
 cudaError_t launch_plain(lm_ctx *c, int which, const TArgs &a) {
     launch_counter().fetch_add(1);
-    if (which == TK_SOLVE_FACTOR || which == TK_SOLVE_REFINE) // one block (two chain warps + their producer warps) per tile of 32 trajectories
-        return launch_traj_plain(which, c->dof, (unsigned)a.Bt, 64, c->stream, a);
+    if (which == TK_SOLVE_FACTOR_HBM || which == TK_SOLVE_REFINE_HBM) return launch_traj_plain(which, c->dof, 0, 0, c->stream, a);
     const unsigned block = 256, grid = (unsigned)((a.nS + block - 1) / block);
     return launch_traj_plain(which, c->dof, grid, block, c->stream, a);
 }
@@ -148,8 +147,8 @@ int lm_traj_attach(lm_ctx *c, const lm_traj_params *p, void *workspace, size_t b
     } else {
         a.tp = a.tp_w = f(L.tp); a.tq = a.tq_w = f(L.tq);
     }
-    a.q = f(L.q); a.Ag = f(L.Ag); a.cst = f(L.cst); a.V = f(L.V); a.z = f(L.z);
-    a.delta = f(L.delta); a.rho = f(L.rho); a.lam = f(L.lam); a.F = f(L.F); a.Fp = f(L.Fp); a.Fd = f(L.Fd); a.Fc = f(L.Fc);
+    a.q = f(L.q); a.Ag = f(L.Ag); a.rho = f(L.rho); a.cst = f(L.cst); a.V = f(L.V); a.z = f(L.z);
+    a.delta = f(L.delta); a.lam = f(L.lam); a.F = f(L.F); a.Fp = f(L.Fp); a.Fd = f(L.Fd); a.Fc = f(L.Fc);
     a.its = reinterpret_cast<uint32_t *>(t.ws + L.its);
     a.mask = reinterpret_cast<unsigned long long *>(t.ws + L.mask);
     a.sel = reinterpret_cast<int32_t *>(t.ws + L.sel);
@@ -163,9 +162,9 @@ int lm_traj_reset(lm_ctx *c, const float *lambda) {
     if (!c || !c->traj.attached) return LM_EINVAL;
     TrajState &t = c->traj;
     const float *lam_dev = lambda;
-    if (lambda && is_host_ptr(lambda)) { // stage through the (not yet used) rho array
-        LM_CUDA(cudaMemcpyAsync(t.args.rho, lambda, 4 * (size_t)c->B, cudaMemcpyHostToDevice, c->stream));
-        lam_dev = t.args.rho;
+    if (lambda && is_host_ptr(lambda)) { // stage through the z array (rewritten by every solve before it is read)
+        LM_CUDA(cudaMemcpyAsync(t.args.z, lambda, 4 * (size_t)c->B, cudaMemcpyHostToDevice, c->stream));
+        lam_dev = t.args.z;
     }
     launch_counter().fetch_add(1);
     tl_reset_kernel<<<(unsigned)((t.args.Bt * 32 + 255) / 256), 256, 0, c->stream>>>(t.args, lam_dev, t.lambda0);
@@ -263,21 +262,34 @@ int lm_traj_run(lm_ctx *c, int32_t iters) {
         LM_CUDA(launch_plain(c, TK_PACK_TARGETS, a));
         t.targets_packed = true;
     }
-    // current point -> e-order, its normal equations and cost
+    // current point -> tile order, and its cost
     LM_CUDA(launch_plain(c, TK_PACK_Q, a));
-    LM_CUDA(launch_pose(c, TK_ASSEMBLE, a));
+    LM_CUDA(launch_pose(c, TK_COST_INIT, a));
     launch_counter().fetch_add(1);
     tl_init_cost_kernel<<<(unsigned)a.Bt, TL_SUM_WARPS * 32, 0, c->stream>>>(a);
     LM_CUDA(cudaGetLastError());
-    for (int it = 0; it < iters; ++it) {
-        LM_CUDA(launch_plain(c, TK_SOLVE_FACTOR, a));
-        for (int r = 0; r < t.refine; ++r) {
-            LM_CUDA(launch_pose(c, TK_RHO, a));
-            LM_CUDA(launch_plain(c, TK_SOLVE_REFINE, a));
+    // Fused path: the solve kernel's producer warps assemble the normal equations / the refinement residual in shared
+    // memory (3 + refine launches per iteration).  Unfused path: per-waypoint kernels write them to HBM and the solve kernel
+    // fetches them (4 + 2 refine launches) -- with collision rows (their divergent pair loops need every SM, not the few
+    // producer warps of one block per tile) and when there are too few tiles to keep the producers of a block ahead of
+    // its chains.  Same functions, same bits either way (tests/test_gpu_traj.py).
+    const bool coll = a.caps.npairs + a.caps.nenv > 0;
+    const bool fused = !coll && (t.fused_mode == 1 || (t.fused_mode == 0 && a.Bt >= TL_FUSED_MIN_TILES));
+    for (int it = 0; it < iters; ++it) { // nothing on the host in between
+        if (fused) {
+            LM_CUDA(launch_pose(c, TK_SOLVE_FACTOR, a));                                    // assemble + factor + solve: delta
+            for (int r = 0; r < t.refine; ++r) LM_CUDA(launch_pose(c, TK_SOLVE_REFINE, a)); // rho + re-solve: delta += e
+        } else {
+            LM_CUDA(launch_pose(c, TK_ASSEMBLE, a));
+            LM_CUDA(launch_plain(c, TK_SOLVE_FACTOR_HBM, a));
+            for (int r = 0; r < t.refine; ++r) {
+                LM_CUDA(launch_pose(c, TK_RHO, a));
+                LM_CUDA(launch_plain(c, TK_SOLVE_REFINE_HBM, a));
+            }
         }
-        LM_CUDA(launch_pose(c, TK_TRIAL, a));
+        LM_CUDA(launch_pose(c, TK_COST, a));                                      // trial point and its cost
         launch_counter().fetch_add(1);
-        tl_decide_kernel<<<(unsigned)a.Bt, TL_SUM_WARPS * 32, 0, c->stream>>>(a);
+        tl_decide_kernel<<<(unsigned)a.Bt, TL_SUM_WARPS * 32, 0, c->stream>>>(a); // accept / reject, lambda
         LM_CUDA(cudaGetLastError());
     }
     LM_CUDA(launch_plain(c, TK_UNPACK, a));

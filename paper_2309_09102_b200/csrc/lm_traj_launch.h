@@ -6,34 +6,65 @@
 
 namespace lmk {
 
-enum TrajPoseKernel : int { TK_ASSEMBLE = 0, TK_RHO = 1, TK_TRIAL = 2, TK_CLEARANCE = 3 };
-enum TrajPlainKernel : int { TK_PACK_Q = 0, TK_PACK_TARGETS = 1, TK_UNPACK = 2, TK_SOLVE_FACTOR = 3, TK_SOLVE_REFINE = 4 };
+enum TrajPoseKernel : int { TK_COST_INIT = 0, TK_COST = 1, TK_CLEARANCE = 2, TK_SOLVE_FACTOR = 3, TK_SOLVE_REFINE = 4, TK_ASSEMBLE = 5, TK_RHO = 6 };
+enum TrajPlainKernel : int { TK_PACK_Q = 0, TK_PACK_TARGETS = 1, TK_UNPACK = 2, TK_SOLVE_FACTOR_HBM = 3, TK_SOLVE_REFINE_HBM = 4 };
 
-// kernels that evaluate FK (chain-structure specialised or generic), thread per waypoint
+// kernels that evaluate FK (chain-structure specialised or generic): the per-waypoint cost kernels and the solve kernels,
+// whose producer warps assemble the normal equations (fused path), and the per-waypoint assemble / rho kernels of the
+// unfused path.  `grid` is ignored for the solve kernels (one block per tile).
 cudaError_t launch_traj_pose_spec(int which, int spec_id, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
 cudaError_t launch_traj_pose_generic_lo(int which, int dof, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
 cudaError_t launch_traj_pose_generic_hi(int which, int dof, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
 // kernels that depend on the dof only
 cudaError_t launch_traj_plain(int which, int dof, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a);
 
+template <int D, int MODE, bool FUSED, bool WEIGHTED, typename SpecT>
+cudaError_t launch_traj_solve_t(cudaStream_t s, const TArgs &a) {
+    // the rings need more than the default 48 KB; the attribute is per DEVICE: set it on every launch (cheap)
+    cudaError_t e = cudaFuncSetAttribute(tl_solve_kernel<D, MODE, FUSED, WEIGHTED, SpecT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)tl_solve_smem_bytes<D, MODE>());
+    if (e != cudaSuccess) return e;
+    int dev = 0, sms = 0;
+    e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    // block shape (lm_traj.cuh): more producer warps while every SM holds at most one block
+    const unsigned threads = !FUSED ? TL_SOLVE_THREADS_HBM : a.Bt <= (int64_t)sms ? TL_SOLVE_THREADS_FEW_TILES : TL_SOLVE_THREADS_MANY_TILES;
+    tl_solve_kernel<D, MODE, FUSED, WEIGHTED, SpecT><<<(unsigned)a.Bt, threads, tl_solve_smem_bytes<D, MODE>(), s>>>(a);
+    return cudaGetLastError();
+}
+
 template <int D, typename SpecT>
 cudaError_t launch_traj_pose_t(int which, bool weighted, unsigned grid, unsigned block, cudaStream_t s, const TArgs &a) {
     const bool coll = a.caps.npairs + a.caps.nenv > 0; // collision rows: their own instantiations (lm_coll.cuh)
-#define LM_TL_LAUNCH(K)                                                                   \
-    do {                                                                                  \
-        if (weighted) { if (coll) K<D, false, true, SpecT, true><<<grid, block, 0, s>>>(a);   \
-                        else K<D, false, true, SpecT, false><<<grid, block, 0, s>>>(a); }     \
-        else { if (coll) K<D, false, false, SpecT, true><<<grid, block, 0, s>>>(a);           \
-               else K<D, false, false, SpecT, false><<<grid, block, 0, s>>>(a); }             \
+#define LM_TL_DISPATCH(CALL)                                               \
+    do {                                                                   \
+        if (weighted) { if (coll) { CALL(true, true); } else { CALL(true, false); } }   \
+        else { if (coll) { CALL(false, true); } else { CALL(false, false); } }          \
     } while (0)
+#define LM_TL_COST_INIT(W, C) tl_cost_kernel<D, false, W, SpecT, C, true><<<grid, block, 0, s>>>(a)
+#define LM_TL_COST(W, C) tl_cost_kernel<D, false, W, SpecT, C, false><<<grid, block, 0, s>>>(a)
+#define LM_TL_ASSEMBLE(W, C) tl_assemble_kernel<D, false, W, SpecT, C><<<grid, block, 0, s>>>(a)
+#define LM_TL_RHO(W, C) tl_rho_kernel<D, false, W, SpecT, C><<<grid, block, 0, s>>>(a)
     switch (which) {
-    case TK_ASSEMBLE: LM_TL_LAUNCH(tl_assemble_kernel); break;
-    case TK_RHO: LM_TL_LAUNCH(tl_rho_kernel); break;
-    case TK_TRIAL: LM_TL_LAUNCH(tl_trial_kernel); break;
+    case TK_COST_INIT: LM_TL_DISPATCH(LM_TL_COST_INIT); break;
+    case TK_COST: LM_TL_DISPATCH(LM_TL_COST); break;
     case TK_CLEARANCE: tl_clearance_kernel<D, SpecT><<<grid, block, 0, s>>>(a); break;
+    case TK_ASSEMBLE: LM_TL_DISPATCH(LM_TL_ASSEMBLE); break;
+    case TK_RHO: LM_TL_DISPATCH(LM_TL_RHO); break;
+    case TK_SOLVE_FACTOR: // fused: the producers assemble; never with collision rows (lm_traj_api.cu)
+        if (coll) return cudaErrorInvalidValue;
+        return weighted ? launch_traj_solve_t<D, 0, true, true, SpecT>(s, a) : launch_traj_solve_t<D, 0, true, false, SpecT>(s, a);
+    case TK_SOLVE_REFINE:
+        if (coll) return cudaErrorInvalidValue;
+        return weighted ? launch_traj_solve_t<D, 1, true, true, SpecT>(s, a) : launch_traj_solve_t<D, 1, true, false, SpecT>(s, a);
     default: return cudaErrorInvalidValue;
     }
-#undef LM_TL_LAUNCH
+#undef LM_TL_DISPATCH
+#undef LM_TL_COST_INIT
+#undef LM_TL_COST
+#undef LM_TL_ASSEMBLE
+#undef LM_TL_RHO
     return cudaGetLastError();
 }
 
@@ -43,29 +74,8 @@ cudaError_t launch_traj_plain_t(int which, unsigned grid, unsigned block, cudaSt
     case TK_PACK_Q: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 0); break;
     case TK_PACK_TARGETS: tl_pack_kernel<D><<<grid, block, 0, s>>>(a, 1); break;
     case TK_UNPACK: tl_unpack_kernel<D><<<grid, block, 0, s>>>(a); break;
-    case TK_SOLVE_FACTOR:  // two chain warps + two producer warps per tile of 32 trajectories; the rings need more than
-    case TK_SOLVE_REFINE: { // the default 48 KB.  Ring depth: deep while every SM holds at most one block (lm_traj.cuh)
-        int dev = 0, sms = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return e;
-        const bool deep = grid <= (unsigned)sms;
-#define LM_SOLVE_LAUNCH(MODE, WANT)                                                                                          \
-    {                                                                                                                        \
-        /* the attribute is per DEVICE: set it on every launch (cheap), never once per process */                           \
-        e = cudaFuncSetAttribute(tl_solve_kernel<D, MODE, WANT>, cudaFuncAttributeMaxDynamicSharedMemorySize,                \
-                                 (int)tl_solve_smem_bytes<D, MODE, WANT>());                                                 \
-        if (e != cudaSuccess) return e;                                                                                      \
-        tl_solve_kernel<D, MODE, WANT><<<grid, TL_SOLVE_THREADS, tl_solve_smem_bytes<D, MODE, WANT>(), s>>>(a);              \
-    }
-        if (which == TK_SOLVE_FACTOR) {
-            if (deep) LM_SOLVE_LAUNCH(0, TL_STAGES_DEEP) else LM_SOLVE_LAUNCH(0, TL_STAGES_SHALLOW)
-        } else {
-            if (deep) LM_SOLVE_LAUNCH(1, TL_STAGES_DEEP) else LM_SOLVE_LAUNCH(1, TL_STAGES_SHALLOW)
-        }
-#undef LM_SOLVE_LAUNCH
-        break;
-    }
+    case TK_SOLVE_FACTOR_HBM: return launch_traj_solve_t<D, 0, false, false, NoSpec>(s, a);
+    case TK_SOLVE_REFINE_HBM: return launch_traj_solve_t<D, 1, false, false, NoSpec>(s, a);
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();

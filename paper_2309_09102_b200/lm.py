@@ -22,7 +22,7 @@ LM_MAX_DOF = 8
 LM_MAX_ITERS = 64
 LM_OK, LM_EINVAL, LM_ENOMEM, LM_ECUDA = 0, -1, -2, -3
 LM_MEM_DEVICE, LM_MEM_HOST = 0, 1
-LM_OPT_BLOCK_THREADS, LM_OPT_GENERIC_KERNEL, LM_OPT_LANES_PER_WAYPOINT = 1, 2, 3
+LM_OPT_BLOCK_THREADS, LM_OPT_GENERIC_KERNEL, LM_OPT_LANES_PER_WAYPOINT, LM_OPT_TRAJ_FUSED = 1, 2, 3, 4
 LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1, 2, 4, 8, 16
 
 # every symbol include/lm.h declares (checked by tests/test_abi.py)
@@ -563,6 +563,10 @@ class Solver:
         with self._on_stream():
             self.traj_workspace, ptr = self._alloc_ws(nbytes)
         lm_traj_attach(self._ctx, self.tparams, ptr, nbytes)
+
+    def traj_set_fused(self, mode: int) -> None:
+        """LM_OPT_TRAJ_FUSED: 0 = chosen by tile count, 1 = fused solve kernels, 2 = per-waypoint kernels through HBM."""
+        lm_set_option(self._ctx, LM_OPT_TRAJ_FUSED, int(mode))
 
     def traj_set_capsules(self, model, w_coll: float = 1.0, d_safe: float = 0.05) -> None:
         lm_traj_set_capsules(self._ctx, model, w_coll, d_safe)

@@ -404,3 +404,39 @@ def test_low_dof_trajectory_step_and_search(d):
     choice, xi, cost, mj = sorc.search(q32, pen, dtype=np.float32)
     assert np.array_equal(g2["choice"], choice) and np.array_equal(g2["xi"], xi) and np.float32(g2["cost"]) == np.float32(cost)
     assert gs["choice"].shape == (n,) and q_after.shape == (B, n, d)
+
+
+# ------------------------------------------------------------------ fused (shared-memory) vs unfused (HBM) normal equations
+
+@pytest.mark.parametrize("shape", [(70, 57), (33, 5), (1, 1), (1, 2), (3, 1), (2, 301), (129, 40)])
+@pytest.mark.parametrize("chain_name", ["panda", "rand8", "generic3"])
+def test_fused_and_unfused_paths_return_the_same_bits(chain_name, shape):
+    """LM_OPT_TRAJ_FUSED (include/lm.h): the producer warps of the solve kernels build w_p^2 J^T J, g and rho with the very
+    functions of the per-waypoint kernels, so every output of lm_traj_run is bit-identical on both paths -- on ragged
+    tiles, one- and two-waypoint trajectories (no elimination on one or both sides), more waypoints than ring stages,
+    with 0, 1 and 2 refinement steps; and the fused path takes 3 + refine launches per iteration."""
+    ch = {"panda": wl.panda_chain, "rand8": lambda: wl.random_chain_8dof(3)}.get(chain_name, lambda: None)()
+    if ch is None:
+        ch = wl.Chain("gen3", 3, np.array([0, 1, 0], np.int32), np.array([0.1, 0.2, -0.3]), np.array([0.3, -1.1, 2.0]),
+                      np.array([0.05, 0.1, 0.2]), np.array([0.4, -0.7, 1.3]), np.full(3, -2.0), np.full(3, 2.0),
+                      np.array([0.1, 0.0, 0.2, 1, 0, 0, 0.0]))
+    B, n = shape
+    w = make_problem(ch, B, n, 0.1, 21)
+    for refine in (0, 1, 2):
+        outs = []
+        for mode in (1, 2):
+            s = solver_for(w, w_pose=1.0, w_diff=0.3, refine_steps=refine)
+            s.traj_set_fused(mode)
+            s.traj_enable_trace()
+            s.traj_run(1)                      # warm the launch path, then count
+            l0 = lm().lm_launch_count()
+            s.traj_run(2)
+            launches = lm().lm_launch_count() - l0
+            g, f = s.traj_fetch(), s.fetch()
+            s.close()
+            outs.append((g, f, launches))
+        (g1, f1, l1), (g2, f2, l2) = outs
+        for k in ("cost", "cost_pose", "cost_diff", "lam", "mask", "iters", "status", "trial_q"):
+            assert np.array_equal(g1[k], g2[k], equal_nan=g1[k].dtype.kind == "f"), (k, refine)
+        assert np.array_equal(f1["q"], f2["q"]) and np.array_equal(f1["res_norm"], f2["res_norm"])
+        assert l2 - l1 == 2 * (1 + refine), (l1, l2)   # per iteration: fused 3 + refine, unfused 4 + 2 refine
