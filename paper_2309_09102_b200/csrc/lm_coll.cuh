@@ -151,131 +151,121 @@ __device__ __forceinline__ float segment_box_closest(const float (&a)[3], const 
     return fminf(fmaxf(ts, tl), th);
 }
 
-// Calls f(g, r) for every pair whose hinge is active at this waypoint: g[D] = d r / d q, r = the residual.
-// Fr = frames retained by FK (Fr.Jw[j] = z_j, Fr.Jv[j] = o_j: eval_pose with WITH_JAC = false).
-// CLEAR_ONLY: no rows; *min_clear receives the smallest clearance `dist` over all listed pairs (lm_plan_*: a valid
-// trajectory must be collision free, PAPER.md:L49).
-template <int D, typename SpecT, bool CLEAR_ONLY = false, typename F>
-__device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, const CapsWorld &W, const Pose<D> &Fr, F &&f,
-                                          float *min_clear = nullptr) {
-    constexpr ChainSpec S = SpecT::spec;
-    // ---- one robot-environment pair: the obstacle does not move
-    auto env_item = [&](int p) {
-        const int k = C.env_pair[p][0], ob = C.env_pair[p][1];
-        float ab[3], bb[3], wa[3], wb[3], pmin[3], pmax[3];
+// ---- the two halves of a pair's work.  *_qp: the closest-point problem (divergent, expensive; depends on the capsule
+// endpoints and the obstacle only, so ANY lane can run it for the owner: coll_rows_compact).  *_finish: distance, hinge
+// test and the row, with the frames of the owning lane.  coll_rows runs both halves back to back.
+struct EnvQp { float t, eb[3]; };  // parameter of the closest axis point, (axis point - box point) in the box frame
+__device__ __forceinline__ EnvQp env_qp(const KCaps &C, int ob, const float (&wa)[3], const float (&wb)[3]) {
+    float ab[3], bb[3], pmin[3], pmax[3];
 #pragma unroll
-        for (int i = 0; i < 3; ++i) { wa[i] = W.wa[k][i]; wb[i] = W.wb[k][i]; pmin[i] = C.pmin[ob][i]; pmax[i] = C.pmax[ob][i]; }
+    for (int i = 0; i < 3; ++i) { pmin[i] = C.pmin[ob][i]; pmax[i] = C.pmax[ob][i]; }
 #pragma unroll
-        for (int i = 0; i < 3; ++i) { // x_box = Ro^T (x - to)
-            float sa = 0.f, sb = 0.f;
+    for (int i = 0; i < 3; ++i) { // x_box = Ro^T (x - to)
+        float sa = 0.f, sb = 0.f;
 #pragma unroll
-            for (int kk = 0; kk < 3; ++kk) {
-                sa = fma_(C.Ro[ob][3 * kk + i], sub(wa[kk], C.to[ob][kk]), sa);
-                sb = fma_(C.Ro[ob][3 * kk + i], sub(wb[kk], C.to[ob][kk]), sb);
-            }
-            ab[i] = sa; bb[i] = sb;
+        for (int kk = 0; kk < 3; ++kk) {
+            sa = fma_(C.Ro[ob][3 * kk + i], sub(wa[kk], C.to[ob][kk]), sa);
+            sb = fma_(C.Ro[ob][3 * kk + i], sub(wb[kk], C.to[ob][kk]), sb);
         }
-        const float t = segment_box_closest(ab, bb, pmin, pmax);
-        float eb[3], ps[3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            const float x = fma_(sub(bb[i], ab[i]), t, ab[i]);
-            eb[i] = sub(x, fminf(fmaxf(x, pmin[i]), pmax[i]));
-            ps[i] = fma_(sub(wb[i], wa[i]), t, wa[i]);
-        }
-        const float len = sqrtf(dot3(eb, eb));
-        const float dist = sub(len, C.c[k]);
-        if (CLEAR_ONLY) { *min_clear = fminf(*min_clear, dist); return; }
-        if (!(dist < C.d_safe_env)) return;
-        const float r = mul(C.w_env, sub(C.d_safe_env, dist));
-        const float il = (len > 0.f) ? __fdividef(1.0f, len) : 0.f; // axis inside the box: no direction, the row keeps its value
-        float n[3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) n[i] = mul(il, fma_(C.Ro[ob][3 * i + 2], eb[2], fma_(C.Ro[ob][3 * i + 1], eb[1], mul(C.Ro[ob][3 * i], eb[0]))));
-        const int L = C.link[k];
-        float g[D];
-#pragma unroll
-        for (int j = 0; j < D; ++j) {
-            float gj = 0.f;
-            if (j <= L) {
-                const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
-                const float z[3] = {Fr.Jw[j][0], Fr.Jw[j][1], Fr.Jw[j][2]};
-                float col[3];
-                if (pris) { col[0] = z[0]; col[1] = z[1]; col[2] = z[2]; }
-                else {
-                    const float dd[3] = {sub(ps[0], Fr.Jv[j][0]), sub(ps[1], Fr.Jv[j][1]), sub(ps[2], Fr.Jv[j][2])};
-                    col[0] = fma_(z[1], dd[2], -mul(z[2], dd[1]));
-                    col[1] = fma_(z[2], dd[0], -mul(z[0], dd[2]));
-                    col[2] = fma_(z[0], dd[1], -mul(z[1], dd[0]));
-                }
-                gj = mul(-C.w_env, dot3(n, col));
-            }
-            g[j] = gj;
-        }
-        f(g, r);
-    };
-    // ---- one robot-robot pair
-    auto self_item = [&](int p) {
-        const int k1 = C.pair[p][0], k2 = C.pair[p][1];
-        float a1[3], b1[3], a2[3], b2[3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) { a1[i] = W.wa[k1][i]; b1[i] = W.wb[k1][i]; a2[i] = W.wa[k2][i]; b2[i] = W.wb[k2][i]; }
-        float t1, t2;
-        segment_closest(a1, b1, a2, b2, t1, t2);
-        float p1[3], p2[3], e[3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            p1[i] = fma_(sub(b1[i], a1[i]), t1, a1[i]);
-            p2[i] = fma_(sub(b2[i], a2[i]), t2, a2[i]);
-            e[i] = sub(p1[i], p2[i]);
-        }
-        const float len = sqrtf(dot3(e, e));
-        const float dist = sub(sub(len, C.c[k1]), C.c[k2]);
-        if (CLEAR_ONLY) { *min_clear = fminf(*min_clear, dist); return; }
-        if (!(dist < C.d_safe)) return;
-        const float r = mul(C.w_coll, sub(C.d_safe, dist));
-        const float il = (len > 0.f) ? __fdividef(1.0f, len) : 0.f; // the axes touch: no direction, the row keeps its value
-        const float n[3] = {mul(e[0], il), mul(e[1], il), mul(e[2], il)};
-        const int L1 = C.link[k1], L2 = C.link[k2];
-        const int lo = min(L1, L2), hi = max(L1, L2);
-        // the point on the link farther down the chain; its motion relative to the other point
-        const float sgn = (L1 > L2) ? -C.w_coll : C.w_coll; // d r / d q_j = -w n.c1 (L1 farther) or +w n.c2 (L2 farther)
-        float g[D];
-#pragma unroll
-        for (int j = 0; j < D; ++j) {
-            float gj = 0.f;
-            if (j > lo && j <= hi) {
-                const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
-                const float z[3] = {Fr.Jw[j][0], Fr.Jw[j][1], Fr.Jw[j][2]};
-                float col[3];
-                if (pris) { col[0] = z[0]; col[1] = z[1]; col[2] = z[2]; }
-                else {
-                    float d[3];
-#pragma unroll
-                    for (int i = 0; i < 3; ++i) d[i] = sub((L1 > L2) ? p1[i] : p2[i], Fr.Jv[j][i]);
-                    col[0] = fma_(z[1], d[2], -mul(z[2], d[1]));
-                    col[1] = fma_(z[2], d[0], -mul(z[0], d[2]));
-                    col[2] = fma_(z[0], d[1], -mul(z[1], d[0]));
-                }
-                gj = mul(sgn, dot3(n, col));
-            }
-            g[j] = gj;
-        }
-        f(g, r);
-    };
-    if (CLEAR_ONLY) { // every listed pair counts towards the clearance
-        for (int p = 0; p < C.nenv; ++p) env_item(p);
-        for (int p = 0; p < C.npairs; ++p) self_item(p);
-        return;
+        ab[i] = sa; bb[i] = sb;
     }
-    // ---- culling by bounding volumes, all lanes in step (uniform): one bit per pair that may have a row.  Then the
-    // QP and the row for the survivors, every lane through ITS OWN list in ascending order: the lanes of a warp are 32
-    // different trajectories (uncorrelated), so a loop over the listed pairs in step would run every pair for the two or
-    // three lanes that need it; with the lists the warp iterates max-over-lanes times instead, and a lane's rows still
-    // arrive in the order of a plain loop over the pairs (bitwise the same sums).  Measured (C4, all 19 pairs, us per
-    // iteration): in-step loop 1225 -> lists 1054; a second, tighter culling level inside the lists (2 or 4 sample
-    // points per axis, clearance >= min_j dist(sample_j, body) - hl / K) costs more than it saves (1108 / 1096).
-    uint32_t need_env = 0u, need_self = 0u; // MAX_PAIRS = 32 of each kind
+    EnvQp o;
+    o.t = segment_box_closest(ab, bb, pmin, pmax);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        const float x = fma_(sub(bb[i], ab[i]), o.t, ab[i]);
+        o.eb[i] = sub(x, fminf(fmaxf(x, pmin[i]), pmax[i]));
+    }
+    return o;
+}
+template <int D, typename SpecT, bool CLEAR_ONLY, typename F>
+__device__ __forceinline__ void env_finish(const KChain &ch, const KCaps &C, int k, int ob, const float (&wa)[3], const float (&wb)[3],
+                                           const EnvQp &qp, const Pose<D> &Fr, F &&f, float *min_clear) {
+    constexpr ChainSpec S = SpecT::spec;
+    float ps[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) ps[i] = fma_(sub(wb[i], wa[i]), qp.t, wa[i]);
+    const float len = sqrtf(dot3(qp.eb, qp.eb));
+    const float dist = sub(len, C.c[k]);
+    if (CLEAR_ONLY) { *min_clear = fminf(*min_clear, dist); return; }
+    if (!(dist < C.d_safe_env)) return;
+    const float r = mul(C.w_env, sub(C.d_safe_env, dist));
+    const float il = (len > 0.f) ? __fdividef(1.0f, len) : 0.f; // axis inside the box: no direction, the row keeps its value
+    float n[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) n[i] = mul(il, fma_(C.Ro[ob][3 * i + 2], qp.eb[2], fma_(C.Ro[ob][3 * i + 1], qp.eb[1], mul(C.Ro[ob][3 * i], qp.eb[0]))));
+    const int L = C.link[k];
+    float g[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        float gj = 0.f;
+        if (j <= L) {
+            const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
+            const float z[3] = {Fr.Jw[j][0], Fr.Jw[j][1], Fr.Jw[j][2]};
+            float col[3];
+            if (pris) { col[0] = z[0]; col[1] = z[1]; col[2] = z[2]; }
+            else {
+                const float dd[3] = {sub(ps[0], Fr.Jv[j][0]), sub(ps[1], Fr.Jv[j][1]), sub(ps[2], Fr.Jv[j][2])};
+                col[0] = fma_(z[1], dd[2], -mul(z[2], dd[1]));
+                col[1] = fma_(z[2], dd[0], -mul(z[0], dd[2]));
+                col[2] = fma_(z[0], dd[1], -mul(z[1], dd[0]));
+            }
+            gj = mul(-C.w_env, dot3(n, col));
+        }
+        g[j] = gj;
+    }
+    f(g, r);
+}
+template <int D, typename SpecT, bool CLEAR_ONLY, typename F>
+__device__ __forceinline__ void self_finish(const KChain &ch, const KCaps &C, int k1, int k2, const float (&a1)[3], const float (&b1)[3],
+                                            const float (&a2)[3], const float (&b2)[3], float t1, float t2, const Pose<D> &Fr, F &&f,
+                                            float *min_clear) {
+    constexpr ChainSpec S = SpecT::spec;
+    float p1[3], p2[3], e[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        p1[i] = fma_(sub(b1[i], a1[i]), t1, a1[i]);
+        p2[i] = fma_(sub(b2[i], a2[i]), t2, a2[i]);
+        e[i] = sub(p1[i], p2[i]);
+    }
+    const float len = sqrtf(dot3(e, e));
+    const float dist = sub(sub(len, C.c[k1]), C.c[k2]);
+    if (CLEAR_ONLY) { *min_clear = fminf(*min_clear, dist); return; }
+    if (!(dist < C.d_safe)) return;
+    const float r = mul(C.w_coll, sub(C.d_safe, dist));
+    const float il = (len > 0.f) ? __fdividef(1.0f, len) : 0.f; // the axes touch: no direction, the row keeps its value
+    const float n[3] = {mul(e[0], il), mul(e[1], il), mul(e[2], il)};
+    const int L1 = C.link[k1], L2 = C.link[k2];
+    const int lo = min(L1, L2), hi = max(L1, L2);
+    // the point on the link farther down the chain; its motion relative to the other point
+    const float sgn = (L1 > L2) ? -C.w_coll : C.w_coll; // d r / d q_j = -w n.c1 (L1 farther) or +w n.c2 (L2 farther)
+    float g[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) {
+        float gj = 0.f;
+        if (j > lo && j <= hi) {
+            const bool pris = S.generic ? (((ch.prismatic_mask >> j) & 1u) != 0) : (((S.pris >> j) & 1u) != 0);
+            const float z[3] = {Fr.Jw[j][0], Fr.Jw[j][1], Fr.Jw[j][2]};
+            float col[3];
+            if (pris) { col[0] = z[0]; col[1] = z[1]; col[2] = z[2]; }
+            else {
+                float d[3];
+#pragma unroll
+                for (int i = 0; i < 3; ++i) d[i] = sub((L1 > L2) ? p1[i] : p2[i], Fr.Jv[j][i]);
+                col[0] = fma_(z[1], d[2], -mul(z[2], d[1]));
+                col[1] = fma_(z[2], d[0], -mul(z[0], d[2]));
+                col[2] = fma_(z[0], d[1], -mul(z[1], d[0]));
+            }
+            gj = mul(sgn, dot3(n, col));
+        }
+        g[j] = gj;
+    }
+    f(g, r);
+}
+
+// culling by bounding volumes: one bit per pair that may have a row (all lanes in step: the model is uniform)
+__device__ __forceinline__ void coll_cull(const KCaps &C, const CapsWorld &W, uint32_t &need_env, uint32_t &need_self) {
+    need_env = 0u; need_self = 0u; // MAX_PAIRS = 32 of each kind
     for (int p = 0; p < C.nenv; ++p) { // axis midpoint against the box
         const int k = C.env_pair[p][0], ob = C.env_pair[p][1];
         float mw[3], e2 = 0.f;
@@ -298,6 +288,48 @@ __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, cons
         const float reach = add(add(add(C.hl[k1], C.c[k1]), add(C.hl[k2], C.c[k2])), add(C.d_safe, 1e-4f));
         if (!(dot3(cc, cc) > mul(reach, reach))) need_self |= 1u << p;
     }
+}
+
+// Calls f(g, r) for every pair whose hinge is active at this waypoint: g[D] = d r / d q, r = the residual.
+// Fr = frames retained by FK (Fr.Jw[j] = z_j, Fr.Jv[j] = o_j: eval_pose with WITH_JAC = false).
+// CLEAR_ONLY: no rows; *min_clear receives the smallest clearance `dist` over all listed pairs (lm_plan_*: a valid
+// trajectory must be collision free, PAPER.md:L49).
+template <int D, typename SpecT, bool CLEAR_ONLY = false, typename F>
+__device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, const CapsWorld &W, const Pose<D> &Fr, F &&f,
+                                          float *min_clear = nullptr) {
+    // ---- one robot-environment pair: the obstacle does not move
+    auto env_item = [&](int p) {
+        const int k = C.env_pair[p][0], ob = C.env_pair[p][1];
+        float wa[3], wb[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { wa[i] = W.wa[k][i]; wb[i] = W.wb[k][i]; }
+        const EnvQp qp = env_qp(C, ob, wa, wb);
+        env_finish<D, SpecT, CLEAR_ONLY>(ch, C, k, ob, wa, wb, qp, Fr, f, min_clear);
+    };
+    // ---- one robot-robot pair
+    auto self_item = [&](int p) {
+        const int k1 = C.pair[p][0], k2 = C.pair[p][1];
+        float a1[3], b1[3], a2[3], b2[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { a1[i] = W.wa[k1][i]; b1[i] = W.wb[k1][i]; a2[i] = W.wa[k2][i]; b2[i] = W.wb[k2][i]; }
+        float t1, t2;
+        segment_closest(a1, b1, a2, b2, t1, t2);
+        self_finish<D, SpecT, CLEAR_ONLY>(ch, C, k1, k2, a1, b1, a2, b2, t1, t2, Fr, f, min_clear);
+    };
+    if (CLEAR_ONLY) { // every listed pair counts towards the clearance
+        for (int p = 0; p < C.nenv; ++p) env_item(p);
+        for (int p = 0; p < C.npairs; ++p) self_item(p);
+        return;
+    }
+    // ---- culling by bounding volumes, all lanes in step (uniform): one bit per pair that may have a row.  Then the
+    // QP and the row for the survivors, every lane through ITS OWN list in ascending order: the lanes of a warp are 32
+    // different trajectories (uncorrelated), so a loop over the listed pairs in step would run every pair for the two or
+    // three lanes that need it; with the lists the warp iterates max-over-lanes times instead, and a lane's rows still
+    // arrive in the order of a plain loop over the pairs (bitwise the same sums).  Measured (C4, all 19 pairs, us per
+    // iteration): in-step loop 1225 -> lists 1054; a second, tighter culling level inside the lists (2 or 4 sample
+    // points per axis, clearance >= min_j dist(sample_j, body) - hl / K) costs more than it saves (1108 / 1096).
+    uint32_t need_env, need_self;
+    coll_cull(C, W, need_env, need_self);
     while (need_env) {
         const int p = __ffs(need_env) - 1;
         need_env &= need_env - 1u;
@@ -307,6 +339,101 @@ __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, cons
         const int p = __ffs(need_self) - 1;
         need_self &= need_self - 1u;
         self_item(p);
+    }
+}
+
+// ---- the same rows with the closest-point problems COMPACTED over the warp.  The 32 lanes of a warp are 32 different
+// trajectories: after the culling each lane keeps its own short list of pairs, and running the lists in step leaves a
+// handful of lanes active through the most expensive code of the step (ncu, round 2: 13.8 of 32 threads per instruction
+// over the whole cost kernel).  Here the surviving (lane, pair) items of the warp are written to shared memory with the
+// endpoints they need, every lane solves the QP of ONE item per round -- whoever owns it -- and each owner then finishes
+// its own items in its own order (ascending pair index, environment pairs first: the order of coll_rows, so the sums the
+// callback forms are bitwise the same; the QP is a pure function of the endpoints, so it does not matter which lane ran
+// it).  All 32 lanes must call (lanes without work pass live = false); `sc` is the calling warp's scratch.
+constexpr int COLL_CAP = 64; // items per round
+struct CollScratch {
+    float in[COLL_CAP][12];  // env: wa, wb; self: a1, b1, a2, b2
+    int32_t meta[COLL_CAP];  // pair index | kind << 8 (1 = robot-robot)
+    float out[COLL_CAP][4];  // env: t, eb; self: t1, t2
+};
+template <int D, typename SpecT, typename F>
+__device__ __forceinline__ void coll_rows_compact(const KChain &ch, const KCaps &C, const CapsWorld &W, const Pose<D> &Fr, bool live,
+                                                  CollScratch &sc, F &&f) {
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    uint32_t need_env, need_self;
+    coll_cull(C, W, need_env, need_self);
+    if (!live) { need_env = 0u; need_self = 0u; }
+    const int cnt = __popc(need_env) + __popc(need_self);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(full, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const int total = __shfl_sync(full, incl, 31), off = incl - cnt; // this lane's items are off .. off + cnt - 1
+    for (int base = 0; base < total; base += COLL_CAP) {
+        { // owners: the items of this round
+            int idx = off;
+            for (uint32_t m = need_env; m; m &= m - 1u, ++idx) {
+                if (idx < base || idx >= base + COLL_CAP) continue;
+                const int p = __ffs(m) - 1, k = C.env_pair[p][0], sl = idx - base;
+                sc.meta[sl] = p;
+#pragma unroll
+                for (int i = 0; i < 3; ++i) { sc.in[sl][i] = W.wa[k][i]; sc.in[sl][3 + i] = W.wb[k][i]; }
+            }
+            for (uint32_t m = need_self; m; m &= m - 1u, ++idx) {
+                if (idx < base || idx >= base + COLL_CAP) continue;
+                const int p = __ffs(m) - 1, k1 = C.pair[p][0], k2 = C.pair[p][1], sl = idx - base;
+                sc.meta[sl] = p | (1 << 8);
+#pragma unroll
+                for (int i = 0; i < 3; ++i) {
+                    sc.in[sl][i] = W.wa[k1][i]; sc.in[sl][3 + i] = W.wb[k1][i];
+                    sc.in[sl][6 + i] = W.wa[k2][i]; sc.in[sl][9 + i] = W.wb[k2][i];
+                }
+            }
+        }
+        __syncwarp();
+        const int nround = min(COLL_CAP, total - base);
+        for (int sl = lane; sl < nround; sl += 32) { // workers: one closest-point problem each
+            const int mt = sc.meta[sl], p = mt & 0xff;
+            if (mt >> 8) {
+                float a1[3], b1[3], a2[3], b2[3], t1, t2;
+#pragma unroll
+                for (int i = 0; i < 3; ++i) { a1[i] = sc.in[sl][i]; b1[i] = sc.in[sl][3 + i]; a2[i] = sc.in[sl][6 + i]; b2[i] = sc.in[sl][9 + i]; }
+                segment_closest(a1, b1, a2, b2, t1, t2);
+                sc.out[sl][0] = t1; sc.out[sl][1] = t2;
+            } else {
+                float wa[3], wb[3];
+#pragma unroll
+                for (int i = 0; i < 3; ++i) { wa[i] = sc.in[sl][i]; wb[i] = sc.in[sl][3 + i]; }
+                const EnvQp qp = env_qp(C, C.env_pair[p][1], wa, wb);
+                sc.out[sl][0] = qp.t; sc.out[sl][1] = qp.eb[0]; sc.out[sl][2] = qp.eb[1]; sc.out[sl][3] = qp.eb[2];
+            }
+        }
+        __syncwarp();
+        { // owners: distance, hinge test and row of their items, in their order
+            int idx = off;
+            for (uint32_t m = need_env; m; m &= m - 1u, ++idx) {
+                if (idx < base || idx >= base + COLL_CAP) continue;
+                const int p = __ffs(m) - 1, k = C.env_pair[p][0], ob = C.env_pair[p][1], sl = idx - base;
+                float wa[3], wb[3];
+#pragma unroll
+                for (int i = 0; i < 3; ++i) { wa[i] = W.wa[k][i]; wb[i] = W.wb[k][i]; }
+                EnvQp qp;
+                qp.t = sc.out[sl][0]; qp.eb[0] = sc.out[sl][1]; qp.eb[1] = sc.out[sl][2]; qp.eb[2] = sc.out[sl][3];
+                env_finish<D, SpecT, false>(ch, C, k, ob, wa, wb, qp, Fr, f, nullptr);
+            }
+            for (uint32_t m = need_self; m; m &= m - 1u, ++idx) {
+                if (idx < base || idx >= base + COLL_CAP) continue;
+                const int p = __ffs(m) - 1, k1 = C.pair[p][0], k2 = C.pair[p][1], sl = idx - base;
+                float a1[3], b1[3], a2[3], b2[3];
+#pragma unroll
+                for (int i = 0; i < 3; ++i) { a1[i] = W.wa[k1][i]; b1[i] = W.wb[k1][i]; a2[i] = W.wa[k2][i]; b2[i] = W.wb[k2][i]; }
+                self_finish<D, SpecT, false>(ch, C, k1, k2, a1, b1, a2, b2, sc.out[sl][0], sc.out[sl][1], Fr, f, nullptr);
+            }
+        }
+        __syncwarp(); // the scratch is rewritten by the next round
     }
 }
 

@@ -45,6 +45,8 @@ struct TArgs {
                                    //                   |r_pose,i|^2, |q_{i+1} - q_i|^2 (0 for the last waypoint), collision cost
     float *Ag;                     // NA + D            unfused path only: w_p^2 J^T J (packed lower), then g of the stacked residual
     float *rho;                    // D                 unfused path only: refinement residual
+    float *rows;                   // [2] x TL_RMAX x (D + 1)  collision rows (g, r) of the point in q buffer 0 / 1, as tl_cost_kernel found them
+    int32_t *rcnt;                 // [2] x 1           how many (TL_ROWS_OVERFLOW: more than TL_RMAX, recompute)
     float *V;                      // NA                -(S_i)^-1
     float *z;                      // D
     float *delta;                  // D
@@ -131,38 +133,58 @@ __device__ __forceinline__ void tl_load_target(const TArgs &A, const Slot &s, fl
     quat_to_cols(qv[0], qv[1], qv[2], qv[3], Rt);
 }
 
-// FK + residual + Jacobian of one waypoint and, when capsules are set, its collision rows
-template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
-__device__ __forceinline__ void tl_eval_waypoint(const TArgs &A, const float (&q)[D], const float (&pt)[3], const float (&Rt)[3][3],
-                                                 Pose<D> &P, float (&Ac)[Tri<D>::NA], float (&gc)[D], float &fc) {
-    constexpr int NA = Tri<D>::NA;
+// ---- collision rows of a waypoint.  The pair loops (culling, the box-constrained QPs) are divergent and
+// expensive, and one point is visited three times per iteration (its cost as a trial point, then -- if accepted -- the
+// assembly and the refinement residual): tl_cost_kernel, which sees every point first, keeps the rows it finds
+// (g = d r / d q, r), up to TL_RMAX per waypoint, next to the joint buffer it writes; the other two read them back in the
+// same order (bitwise the same sums).  A waypoint with more active rows is marked TL_ROWS_OVERFLOW and recomputed.
+#ifndef LM_TL_RMAX
+#define LM_TL_RMAX 6
+#endif
+constexpr int TL_RMAX = LM_TL_RMAX, TL_ROWS_OVERFLOW = 255;
+template <int D> __host__ __device__ constexpr int tl_row_comps() { return TL_RMAX * (D + 1); }
+
+// the stored rows of one waypoint, requested before the FK pass that precedes their use (two dependent round trips --
+// count, then rows -- overlap with it instead of following it)
+template <int D>
+struct StoredRows {
+    int cnt;
+    float v[TL_RMAX][D + 1];
+};
+template <int D>
+__device__ __forceinline__ void tl_rows_fetch(const TArgs &A, int buf, int64_t wid, int lane, StoredRows<D> &R) {
+    constexpr int RC = tl_row_comps<D>();
+    R.cnt = A.rcnt[(int64_t)buf * A.nS + wid * 32 + lane];
+    const float *rw = A.rows + (int64_t)buf * RC * A.nS;
 #pragma unroll
-    for (int t = 0; t < NA; ++t) Ac[t] = 0.f;
+    for (int r = 0; r < TL_RMAX; ++r) {
+        const bool have = r < R.cnt && R.cnt != TL_ROWS_OVERFLOW;
 #pragma unroll
-    for (int j = 0; j < D; ++j) gc[j] = 0.f;
-    fc = 0.f;
-    if (COLL) {
-        Pose<D> Fr; // frames: Fr.Jw = z_j, Fr.Jv = o_j
+        for (int c = 0; c <= D; ++c) R.v[r][c] = have ? rw[toff<RC>(wid, r * (D + 1) + c, lane)] : 0.f;
+    }
+}
+// f(g, r) for every active row of the waypoint, in the order tl_cost_kernel found them
+template <int D, bool WEIGHTED, typename SpecT, typename F>
+__device__ __forceinline__ void tl_rows_apply(const TArgs &A, const StoredRows<D> &R, const float (&q)[D], const float (&pt)[3],
+                                              const float (&Rt)[3][3], F &&f) {
+    if (R.cnt == TL_ROWS_OVERFLOW) { // rare: recompute (frames by an FK pass with the capsule sink, then the pair loops)
+        Pose<D> Fr;
         CapsWorld W;
         CapsSink sink(A.caps, W);
         sink.base();
-        float pf[3];
-        eval_pose<D, FAST, WEIGHTED, SpecT, false, CapsSink>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, Fr, nullptr, nullptr, pf, sink);
-        coll_rows<D, SpecT>(A.ch, A.caps, W, Fr, [&](const float (&g)[D], float r) {
+        eval_pose<D, false, WEIGHTED, SpecT, false, CapsSink>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, Fr, nullptr, nullptr, nullptr, sink);
+        coll_rows<D, SpecT>(A.ch, A.caps, W, Fr, f);
+        return;
+    }
 #pragma unroll
-            for (int a = 0; a < D; ++a) {
+    for (int r = 0; r < TL_RMAX; ++r) {
+        if (__ballot_sync(__activemask(), r < R.cnt) == 0u) break;
+        if (r < R.cnt) {
+            float g[D];
 #pragma unroll
-                for (int b = 0; b <= a; ++b) Ac[tri(a, b)] = fma_(g[a], g[b], Ac[tri(a, b)]);
-                gc[a] = fma_(g[a], r, gc[a]);
-            }
-            fc = fma_(r, r, fc);
-        });
-        finish_jacobian<D, WEIGHTED, SpecT>(A.ch, Fr, pf, A.w_pos, A.w_rot, P);
-#pragma unroll
-        for (int k = 0; k < 6; ++k) P.r[k] = Fr.r[k];
-        P.F = Fr.F;
-    } else {
-        eval_pose<D, FAST, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+            for (int j = 0; j < D; ++j) g[j] = R.v[r][j];
+            f(g, R.v[r][D]);
+        }
     }
 }
 
@@ -221,16 +243,32 @@ __device__ __forceinline__ void tl_chunk_load(const TArgs &A, const float *qs, i
 }
 
 template <int D, bool WEIGHTED, typename SpecT, bool COLL>
-__device__ __forceinline__ void tl_chunk_normal(const TArgs &A, const ChunkIn<D> &in, int i, int lane, float *st) {
+__device__ __forceinline__ void tl_chunk_normal(const TArgs &A, const ChunkIn<D> &in, int buf, int64_t w0, int i, int lane, float *st) {
     constexpr int NA = Tri<D>::NA;
     const int n = A.n;
     const float (&q)[D] = in.q, (&qm)[D] = in.qm, (&qn)[D] = in.qn;
     const float pt[3] = {in.tg[0], in.tg[1], in.tg[2]};
     float Rt[3][3];
     quat_to_cols(in.tg[3], in.tg[4], in.tg[5], in.tg[6], Rt);
+    StoredRows<D> SR;
+    if (COLL) tl_rows_fetch<D>(A, buf, w0 + i, lane, SR);
     Pose<D> P;
-    float Ac[NA], gc[D], fc;
-    tl_eval_waypoint<D, false, WEIGHTED, SpecT, COLL>(A, q, pt, Rt, P, Ac, gc, fc);
+    eval_pose<D, false, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+    float Ac[NA], gc[D];
+#pragma unroll
+    for (int t = 0; t < NA; ++t) Ac[t] = 0.f;
+#pragma unroll
+    for (int j = 0; j < D; ++j) gc[j] = 0.f;
+    if (COLL) {
+        tl_rows_apply<D, WEIGHTED, SpecT>(A, SR, q, pt, Rt, [&](const float (&g)[D], float r) {
+#pragma unroll
+            for (int a = 0; a < D; ++a) {
+#pragma unroll
+                for (int b = 0; b <= a; ++b) Ac[tri(a, b)] = fma_(g[a], g[b], Ac[tri(a, b)]);
+                gc[a] = fma_(g[a], r, gc[a]);
+            }
+        });
+    }
     const float ci = (n == 1) ? 0.f : ((i == 0 || i == n - 1) ? 1.f : 2.f);
 #pragma unroll
     for (int r = 0; r < D; ++r) {
@@ -245,7 +283,7 @@ __device__ __forceinline__ void tl_chunk_normal(const TArgs &A, const ChunkIn<D>
 //     rho_i = -[ w_p^2 J_i^T (r_i + J_i delta_i) + w_d^2 (D^T D (q + delta))_i + lambda delta_i
 //               + sum over active collision pairs of g (r_c + g . delta_i) ]                  into st[0 .. D)
 template <int D, bool WEIGHTED, typename SpecT, bool COLL>
-__device__ __forceinline__ void tl_chunk_rho(const TArgs &A, const ChunkIn<D> &in, float lam, int64_t w0, int i, int lane, float *st) {
+__device__ __forceinline__ void tl_chunk_rho(const TArgs &A, const ChunkIn<D> &in, int buf, float lam, int64_t w0, int i, int lane, float *st) {
     const int n = A.n;
     const int64_t wid = w0 + i;
     const float ci = (n == 1) ? 0.f : ((i == 0 || i == n - 1) ? 1.f : 2.f);
@@ -266,25 +304,17 @@ __device__ __forceinline__ void tl_chunk_rho(const TArgs &A, const ChunkIn<D> &i
     float ec[D]; // collision rows: sum over the active pairs of g (r + g . delta)
 #pragma unroll
     for (int j = 0; j < D; ++j) ec[j] = 0.f;
+    StoredRows<D> SR;
+    if (COLL) tl_rows_fetch<D>(A, buf, wid, lane, SR);
+    eval_pose<D, false, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
     if (COLL) {
-        Pose<D> Fr;
-        CapsWorld W;
-        CapsSink sink(A.caps, W);
-        sink.base();
-        float pf[3];
-        eval_pose<D, false, WEIGHTED, SpecT, false, CapsSink>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, Fr, nullptr, nullptr, pf, sink);
-        coll_rows<D, SpecT>(A.ch, A.caps, W, Fr, [&](const float (&g)[D], float r) {
+        tl_rows_apply<D, WEIGHTED, SpecT>(A, SR, q, pt, Rt, [&](const float (&g)[D], float r) {
             float u = r;
 #pragma unroll
             for (int j = 0; j < D; ++j) u = fma_(g[j], dl[j], u);
 #pragma unroll
             for (int j = 0; j < D; ++j) ec[j] = fma_(g[j], u, ec[j]);
         });
-        finish_jacobian<D, WEIGHTED, SpecT>(A.ch, Fr, pf, A.w_pos, A.w_rot, P);
-#pragma unroll
-        for (int k = 0; k < 6; ++k) P.r[k] = Fr.r[k];
-    } else {
-        eval_pose<D, false, WEIGHTED, SpecT>(A.ch, q, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
     }
     float t[6];
 #pragma unroll
@@ -314,10 +344,11 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_assemble_ker
     const uint32_t pk = A.its[s.b];
     if ((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0)) return;
     constexpr int C = Tri<D>::NA + D;
-    const float *qs = A.q + (int64_t)A.sel[s.b] * D * A.nS;
+    const int sel = A.sel[s.b];
+    const float *qs = A.q + (int64_t)sel * D * A.nS;
     ChunkIn<D> in;
     tl_chunk_load<D>(A, qs, s.wid - s.i, s.i, s.lane, in);
-    tl_chunk_normal<D, WEIGHTED, SpecT, COLL>(A, in, s.i, s.lane, A.Ag + s.wid * C * 32);
+    tl_chunk_normal<D, WEIGHTED, SpecT, COLL>(A, in, sel, s.wid - s.i, s.i, s.lane, A.Ag + s.wid * C * 32);
 }
 template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(const __grid_constant__ TArgs A) {
@@ -325,10 +356,11 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_rho_kernel(c
     if (!s.valid) return;
     const uint32_t pk = A.its[s.b];
     if ((pk & 0xffu) >= (uint32_t)A.max_total || !A.ok[s.b] || (A.gate != nullptr && A.gate[s.b] == 0)) return;
-    const float *qs = A.q + (int64_t)A.sel[s.b] * D * A.nS;
+    const int sel = A.sel[s.b];
+    const float *qs = A.q + (int64_t)sel * D * A.nS;
     ChunkIn<D> in;
     tl_chunk_load<D>(A, qs, s.wid - s.i, s.i, s.lane, in);
-    tl_chunk_rho<D, WEIGHTED, SpecT, COLL>(A, in, A.lam[s.b], s.wid - s.i, s.i, s.lane, A.rho + s.wid * D * 32);
+    tl_chunk_rho<D, WEIGHTED, SpecT, COLL>(A, in, sel, A.lam[s.b], s.wid - s.i, s.i, s.lane, A.rho + s.wid * D * 32);
 }
 
 // Kahan-compensated sum step (explicit intrinsics: the compiler cannot simplify the compensation away)
@@ -586,13 +618,13 @@ __global__ void __launch_bounds__(TL_SOLVE_MAX_THREADS) tl_solve_kernel(const __
                 float *st = ring_q + (size_t)s * SF;
                 const int i = idx_of(q, k);
                 if (MODE == 0) {
-                    tl_chunk_normal<D, WEIGHTED, SpecT, false>(A, cur, i, lane, st);
+                    tl_chunk_normal<D, WEIGHTED, SpecT, false>(A, cur, sel, w0, i, lane, st);
                 } else {
                     if (lane == 0) {
                         mbar_expect_tx(&full_all[q][s], NA * 128u);
                         bulk_g2s(st, A.V + (w0 + i) * NA * 32, NA * 128u, &full_all[q][s]);
                     }
-                    tl_chunk_rho<D, WEIGHTED, SpecT, false>(A, cur, lam, w0, i, lane, st + NA * 32);
+                    tl_chunk_rho<D, WEIGHTED, SpecT, false>(A, cur, sel, lam, w0, i, lane, st + NA * 32);
                 }
                 __syncwarp(); // every lane's stores precede the arrival below
                 if (lane == 0) mbar_arrive(&full_all[q][s]);
@@ -787,7 +819,9 @@ __global__ void __launch_bounds__(TL_SOLVE_MAX_THREADS) tl_solve_kernel(const __
 template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL, bool INIT>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(const __grid_constant__ TArgs A) {
     const Slot s = slot_of_thread(A);
-    if (!s.valid) return;
+    // With collision rows all 32 lanes of a warp stay (a lane without work still solves other lanes' closest-point
+    // problems, coll_rows_compact); `live` gates every store.  wid is the same for the whole warp.
+    if (COLL ? (s.wid >= A.Bt * A.n) : !s.valid) return;
     // every load below is issued before the first use: the joint values of BOTH buffers are fetched and the
     // trajectory's `sel` picks afterwards (a dependent address would cost one more DRAM round trip)
     const uint32_t pk = A.its[s.b];
@@ -808,7 +842,8 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
     }
     float pt[3], Rt[3][3];
     tl_load_target(A, s, pt, Rt);
-    if (!INIT && ((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0))) return;
+    const bool live = s.valid && (INIT || !((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0)));
+    if (!COLL && !live) return;
     float qt[D], qn[D];
     bool clamped = false;
     auto point_of = [&](int u, int j, bool &cl) {
@@ -825,22 +860,39 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
         bool dummy = false;
         qt[j] = point_of(0, j, clamped);
         qn[j] = (s.i + 1 < A.n) ? point_of(1, j, dummy) : 0.f;
-        if (!INIT) A.q[(int64_t)(1 - sel) * D * A.nS + toff<D>(s.wid, j, s.lane)] = qt[j];
+        if (!INIT && live) A.q[(int64_t)(1 - sel) * D * A.nS + toff<D>(s.wid, j, s.lane)] = qt[j];
         if (s.i + 1 < A.n) {
             const float t = sub(qn[j], qt[j]);
             fd = fma_(t, t, fd);
         }
     }
     // "a trial point of this trajectory was clamped": integer atomic (order-free), skipped once the bit is seen set
-    if (!INIT && clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
+    if (!INIT && live && clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
     float fc = 0.f;
     Pose<D> P;
     if (COLL) {
+        __shared__ CollScratch scratch[LM_MAX_THREADS / 32];
         CapsWorld W;
         CapsSink sink(A.caps, W);
         sink.base();
         eval_pose<D, FAST, WEIGHTED, SpecT, false, CapsSink>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr, nullptr, sink);
-        coll_rows<D, SpecT>(A.ch, A.caps, W, P, [&](const float (&)[D], float r) { fc = fma_(r, r, fc); });
+        // the rows of this point, kept for the assembly and the refinement residual (tl_rows_fetch)
+        constexpr int RC = tl_row_comps<D>();
+        const int dst = INIT ? sel : 1 - sel;
+        float *rw = A.rows + (int64_t)dst * RC * A.nS + toff<RC>(s.wid, 0, s.lane); // component c at rw[c * 32]
+        int cnt = 0;
+        coll_rows_compact<D, SpecT>(A.ch, A.caps, W, P, live, scratch[threadIdx.x >> 5], [&](const float (&g)[D], float r) {
+            fc = fma_(r, r, fc);
+            if (cnt < TL_RMAX) {
+#pragma unroll
+                for (int j = 0; j < D; ++j) rw[j * 32] = g[j];
+                rw[D * 32] = r;
+                rw += (D + 1) * 32;
+            }
+            ++cnt;
+        });
+        if (!live) return;
+        A.rcnt[(int64_t)dst * A.nS + s.wid * 32 + s.lane] = cnt > TL_RMAX ? TL_ROWS_OVERFLOW : cnt;
     } else {
         eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
     }
