@@ -385,7 +385,7 @@ def run_gpu(args) -> None:
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                     "ms_per_step": e2e_ms_all / e2e["steps"],
-                    "how": f"lm_solve_host(pinned host inputs -> host q, |r|, iters, status; {e2e_chunks} chunks pipelined over the library's copy-in / kernel / copy-out streams)",
+                    "how": f"lm_pipe_solve(pinned host inputs -> host q, |r|, iters, status; {e2e_chunks} chunks pipelined over the handle's copy-in / kernel / copy-out streams)",
                     "unpipelined_ms_per_step": e2e_plain["ms_total"] / e2e_plain["steps"],
                     "unpipelined_how": "lm_init(LM_MEM_HOST, pinned) + lm_run + lm_fetch"},
             "roofline": roofline,
@@ -395,9 +395,25 @@ def run_gpu(args) -> None:
     print(json.dumps(line))
 
 
-def traj_step_alg_bytes(d: int, refine: int = 1) -> float:
-    """HBM bytes one trajectory-level LM iteration must move per waypoint: fp32 words
-    factor+solve 3NA+4d, each refinement (rho 3d+7, re-solve 2NA+5d), trial NA+4d+10, decision 3."""
+def traj_step_alg_bytes(d: int, refine: int = 1, fused: bool = True) -> float:
+    """HBM bytes one trajectory-level LM iteration must move per waypoint, fp32 words.
+    Fused path (the solve kernels' producers assemble in shared memory; J^T J, g, rho never exist in HBM):
+      factor + solve   q d + target 7 in, -S^-1 NA + z d + delta d out, -S^-1 NA + z d back in     = 2 NA + 4 d + 7
+      each refinement  q d + delta d + target 7 + -S^-1 NA in, z d out, NA + 2 d back in, delta d out = 2 NA + 6 d + 7
+      trial cost       q d + delta d + target 7 in, candidate q d + 3 cost terms out               = 3 d + 10
+      decision         3 cost terms in.
+    Unfused path (small batches, collision rows): + the round trip of w_p^2 J^T J, g (2 (NA + d)) and rho (2 d) and their
+    inputs a second time (d + 7)."""
+    na = d * (d + 1) // 2
+    words = (2 * na + 4 * d + 7) + refine * (2 * na + 6 * d + 7) + (3 * d + 10) + 3
+    if not fused:
+        words += (2 * (na + d) + d + 7) + refine * (2 * d)
+    return 4.0 * words
+
+
+def traj_step_alg_bytes_round1(d: int, refine: int = 1) -> float:
+    """The round-1 data flow (every kernel through HBM, candidate normal equations written by the trial kernel): the
+    figure VERDICT r1 recomputed the 0.546 from; kept so that the two rounds can be compared on one scale."""
     na = d * (d + 1) // 2
     return 4.0 * ((3 * na + 4 * d) + refine * ((3 * d + 7) + (2 * na + 5 * d)) + (na + 4 * d + 10) + 3)
 
@@ -486,11 +502,13 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
             if i >= 1:
                 t0_.append(a.elapsed_time(b))
     ms0 = float(min(t0_)) / iters
-    alg0 = traj_step_alg_bytes(d, 0) * w.W
-    norefine = {"ms_per_iteration": ms0, "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, 0),
+    fused = (w.B + 31) // 32 >= 96  # LM_TL_FUSED_MIN_TILES (csrc/lm_traj.cuh); no collision rows in this leg
+    alg0 = traj_step_alg_bytes(d, 0, fused) * w.W
+    norefine = {"ms_per_iteration": ms0, "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, 0, fused),
                 "hbm_frac": alg0 / (ms0 * 1e-3) / 1e9 / peaks["hbm_gbs"]}
     ms_iter = float(min(ts)) / iters
-    alg = traj_step_alg_bytes(d, int(tp.refine_steps)) * w.W
+    alg = traj_step_alg_bytes(d, int(tp.refine_steps), fused) * w.W
+    alg_r1 = traj_step_alg_bytes_round1(d, int(tp.refine_steps)) * w.W
     out = {"workload": f"{w.name}: {w.B} x {w.n}, after 4 pose-only iterations; w_pose=1, w_diff=0.3, refine=1, {iters} iterations",
            "ms_per_iteration": ms_iter, "waypoint_iterations_per_sec": w.W / (ms_iter * 1e-3),
            "trajectory_iterations_per_sec": w.B / (ms_iter * 1e-3), "gpu_launches_per_run": int(launches),
@@ -500,7 +518,12 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
            "roofline": {"bound": "hbm", "achieved": alg / (ms_iter * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                         "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"],
                         "traffic": ncu_constant("traj_iteration_C4", "dram_bytes_per_iteration", TRAJ_SOURCES) if (w.B, w.n) == (4096, 300) else None,
-                        "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps)),
+                        "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps), fused),
+                        "path": "fused (producer warps assemble in shared memory)" if fused else "unfused (per-waypoint kernels through HBM)",
+                        "frac_on_round1_bytes": alg_r1 / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                        "round1_alg_bytes_per_waypoint_iteration": traj_step_alg_bytes_round1(d, int(tp.refine_steps)),
+                        "note": "the fused step needs 23 % fewer bytes than round 1's data flow, so the same time is a lower fraction; "
+                                "its solve kernels are bound by the issue slots of one SM per tile, not by HBM (DESIGN.md section 10)",
                         "peak_source": peaks["_source"]}}
     try:
         from oracle import lm_oracle as orc, lm_traj_oracle as torc
@@ -800,7 +823,9 @@ def measure_e2e(lm, torch, chain, w, prm, device, steps: int, chunks: int = 0) -
     times, units = [], 0
 
     msk = None
+    pipe = None
     if chunks > 0:
+        pipe = lm.lm_pipe_create(chunks)  # the handle (streams, events, pinned totals) outlives the calls, as in a serving loop
         nbytes = lm.lm_solve_host_workspace_bytes(d, w.B, w.n, chunks)
         ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
         ws_ptr = (ws.data_ptr() + 255) // 256 * 256
@@ -809,7 +834,7 @@ def measure_e2e(lm, torch, chain, w, prm, device, steps: int, chunks: int = 0) -
         pb = lm.LmProblem(w.B, w.n, tp.data_ptr(), tq.data_ptr(), 0, seeds.data_ptr(), lm.LM_MEM_HOST, ws_ptr, nbytes)
         st = lm.LmStats(res.data_ptr(), None, None, None, its.data_ptr(), None, sts.data_ptr(), None, None, 0, 0)
         if chunks > 0:  # one call: chunked, H2D / kernel / D2H pipelined over the library's streams
-            lm.lm_solve_host(cchain, pb, prm, w.max_iters, chunks, q_out.data_ptr(), st)
+            lm.lm_pipe_solve(pipe, cchain, pb, prm, w.max_iters, chunks, q_out.data_ptr(), st, int(stream.cuda_stream))
             return int(st.total_waypoint_iters)
         ctx = lm.lm_init(cchain, pb, prm, int(stream.cuda_stream))
         lm.lm_run(ctx, w.max_iters)
@@ -826,6 +851,8 @@ def measure_e2e(lm, torch, chain, w, prm, device, steps: int, chunks: int = 0) -
         units += once()
         times.append(time.perf_counter() - t0)
     dist_barrier()
+    if pipe is not None:
+        lm.lm_pipe_destroy(pipe)
     return {"ms_total": 1e3 * float(sum(times)), "units": float(units), "steps": steps, "h2d": h2d, "d2h": d2h}
 
 

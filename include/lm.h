@@ -131,7 +131,14 @@ int lm_default_params(lm_params *out);
 int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *problem, const lm_params *params,
             void *cuda_stream);
 
-/* Exactly one LM iteration for every waypoint that is not frozen and has iters < 64.  Async. */
+/* Exactly one LM iteration for every waypoint that is not frozen and has iters < 64.  Async.
+ * lm_step is the interleaving / teacher-forcing entry point (tests, lm_plan_run's bookkeeping between phases), NOT the
+ * tuned path: it is the lm_run kernel with an iteration limit of one, so per call every waypoint's state round-trips
+ * through HBM (4 (2 d + 18) bytes) and FK + the Jacobian are recomputed at entry (1878 instead of 1459 FLOP at d = 7).
+ * Keeping r, F and J in the state instead would move 4 (6 d + 7) more bytes each way -- at d = 7 that is 520 B per
+ * waypoint-iteration, 98 us per step on 4096 x 300 at the measured HBM peak, slower than the recomputation (92 us) -- so
+ * the recomputation stays; a caller that wants throughput calls lm_run (one launch for all iterations, 41 us per
+ * iteration on the same batch). */
 int lm_step(lm_ctx *ctx);
 
 /* On-device loop: every waypoint iterates until frozen or until its iters == max_iters (<= 64,
@@ -142,14 +149,30 @@ int lm_run(lm_ctx *ctx, int32_t max_iters);
 /* Synchronise the stream and copy out the current state.  q_out: [d][W] device or host, nullable. */
 int lm_fetch(lm_ctx *ctx, float *q_out, lm_stats *stats_out);
 
-/* One call for HOST data (the end-to-end path): refine all B*n waypoints from host arrays (pinned memory makes
- * the copies asynchronous) and write the results to host arrays.  The batch is split into `chunks` groups of
- * whole trajectories that are pipelined over internal streams (copies in, kernels, copies out), so that the host->device copy of chunk k+1,
- * the LM kernel of chunk k and the device->host copy of chunk k-1 overlap (waypoints are independent:
- * PAPER.md:L121, so the result does not depend on `chunks`).  problem->memory must be LM_MEM_HOST,
- * shared_targets 0, problem->workspace DEVICE scratch of >= lm_solve_host_workspace_bytes().  q_out [d][B*n]
- * and every non-null array of `stats` are HOST pointers.  Blocks until everything has arrived. */
+/* HOST data (the end-to-end path): refine all B*n waypoints from host arrays (pinned memory makes the copies
+ * asynchronous) and write the results to host arrays.  The batch is split into `chunks` groups of whole trajectories
+ * that are pipelined over the streams of an lm_pipe (copies in, kernels, copies out), so that the host->device copy of
+ * chunk k+1, the LM kernel of chunk k and the device->host copy of chunk k-1 overlap (waypoints are independent:
+ * PAPER.md:L121, so the result does not depend on `chunks`).
+ *
+ * lm_pipe_create: the handle owns 4 streams, 2 max_chunks + 5 events and 16 max_chunks bytes of pinned memory on the
+ *   device that is CURRENT at the call; nothing is process-global.  1 <= max_chunks <= LM_PIPE_MAX_CHUNKS.
+ * lm_pipe_solve: problem->memory must be LM_MEM_HOST, shared_targets 0, problem->workspace DEVICE scratch of
+ *   >= lm_solve_host_workspace_bytes() bytes on the handle's device, which must be the current one (else LM_EINVAL);
+ *   1 <= chunks <= min(B, max_chunks).  q_out [d][B*n] and every non-null array of `stats` are HOST pointers.  The
+ *   pipeline starts after everything enqueued on `cuda_stream` so far (cudaStream_t as void*, 0 = the default stream),
+ *   later work on that stream is ordered after it, and the call blocks the host until every output has arrived.  One
+ *   call at a time per handle; handles of different devices (or several of one device) are independent.
+ * lm_pipe_destroy: releases the streams, events and pinned memory (null is a no-op).
+ * lm_solve_host: lm_pipe_create + lm_pipe_solve on the default stream + lm_pipe_destroy -- the one-shot form; creating
+ *   the streams costs more than a whole step, so a caller that solves repeatedly keeps a handle. */
+#define LM_PIPE_MAX_CHUNKS 256
+typedef struct lm_pipe lm_pipe;
 size_t lm_solve_host_workspace_bytes(int32_t dof, int64_t B, int64_t n, int32_t chunks);
+int lm_pipe_create(lm_pipe **pipe_out, int32_t max_chunks);
+int lm_pipe_solve(lm_pipe *pipe, void *cuda_stream, const lm_chain *chain, const lm_problem *problem, const lm_params *params,
+                  int32_t max_iters, int32_t chunks, float *q_out, lm_stats *stats);
+void lm_pipe_destroy(lm_pipe *pipe);
 int lm_solve_host(const lm_chain *chain, const lm_problem *problem, const lm_params *params, int32_t max_iters,
                   int32_t chunks, float *q_out, lm_stats *stats);
 

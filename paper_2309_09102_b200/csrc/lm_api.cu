@@ -7,7 +7,6 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
-#include <mutex>
 #include <new>
 
 using namespace lmk;
@@ -561,46 +560,97 @@ size_t lm_solve_host_workspace_bytes(int32_t dof, int64_t B, int64_t n, int32_t 
     return total;
 }
 
+} // extern "C"
+
+// The streams, events and pinned totals of the host-data pipeline (include/lm.h: lm_pipe_*).  Owned by the handle, bound
+// to the device that was current at lm_pipe_create; one lm_pipe_solve at a time per handle.
+struct lm_pipe {
+    static constexpr int NS = 4;
+    int dev = -1;
+    int max_chunks = 0;
+    cudaStream_t st[NS] = {nullptr, nullptr, nullptr, nullptr}; // host->device copies, device->host copies, 2 x kernels
+    cudaEvent_t *ev_in = nullptr, *ev_done = nullptr;           // [max_chunks]
+    cudaEvent_t ev_entry = nullptr, ev_exit[NS] = {nullptr, nullptr, nullptr, nullptr};
+    unsigned long long *totals = nullptr;                       // pinned, [2 * max_chunks]
+};
+
+extern "C" {
+
+void lm_pipe_destroy(lm_pipe *p) {
+    if (!p) return;
+    for (int i = 0; i < lm_pipe::NS; ++i) {
+        if (p->st[i]) cudaStreamDestroy(p->st[i]);
+        if (p->ev_exit[i]) cudaEventDestroy(p->ev_exit[i]);
+    }
+    for (int i = 0; i < p->max_chunks; ++i) {
+        if (p->ev_in && p->ev_in[i]) cudaEventDestroy(p->ev_in[i]);
+        if (p->ev_done && p->ev_done[i]) cudaEventDestroy(p->ev_done[i]);
+    }
+    if (p->ev_entry) cudaEventDestroy(p->ev_entry);
+    if (p->totals) cudaFreeHost(p->totals);
+    delete[] p->ev_in;
+    delete[] p->ev_done;
+    delete p;
+}
+
+int lm_pipe_create(lm_pipe **out, int32_t max_chunks) {
+    if (!out || max_chunks < 1 || max_chunks > LM_PIPE_MAX_CHUNKS) return LM_EINVAL;
+    *out = nullptr;
+    lm_pipe *p = new (std::nothrow) lm_pipe();
+    if (!p) return LM_ENOMEM;
+    p->ev_in = new (std::nothrow) cudaEvent_t[max_chunks]();
+    p->ev_done = new (std::nothrow) cudaEvent_t[max_chunks]();
+    if (!p->ev_in || !p->ev_done) { lm_pipe_destroy(p); return LM_ENOMEM; }
+    p->max_chunks = max_chunks;
+    cudaError_t e = cudaGetDevice(&p->dev);
+    for (int i = 0; i < lm_pipe::NS && e == cudaSuccess; ++i) {
+        e = cudaStreamCreateWithFlags(&p->st[i], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_exit[i], cudaEventDisableTiming);
+    }
+    for (int i = 0; i < max_chunks && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_done[i], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_entry, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void **>(&p->totals), 16 * (size_t)max_chunks);
+    if (e != cudaSuccess) { lm_pipe_destroy(p); return cuda_fail(e); }
+    *out = p;
+    return LM_OK;
+}
+
 int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *prm, int32_t max_iters, int32_t chunks,
                   float *q_out, lm_stats *st) {
-    if (!chain || !pb || !prm || max_iters < 0 || max_iters > LM_MAX_ITERS) return LM_EINVAL;
+    if (chunks < 1 || chunks > LM_PIPE_MAX_CHUNKS) return LM_EINVAL;
+    lm_pipe *p = nullptr;
+    int rc = lm_pipe_create(&p, chunks);
+    if (rc != LM_OK) return rc;
+    rc = lm_pipe_solve(p, nullptr, chain, pb, prm, max_iters, chunks, q_out, st);
+    lm_pipe_destroy(p);
+    return rc;
+}
+
+int lm_pipe_solve(lm_pipe *pp, void *cuda_stream, const lm_chain *chain, const lm_problem *pb, const lm_params *prm, int32_t max_iters,
+                  int32_t chunks, float *q_out, lm_stats *st) {
+    if (!pp || !chain || !pb || !prm || max_iters < 0 || max_iters > LM_MAX_ITERS) return LM_EINVAL;
     if (pb->memory != LM_MEM_HOST || pb->shared_targets || pb->B <= 0 || pb->n <= 0 || chunks < 1 || chunks > pb->B) return LM_EINVAL;
     if (!pb->target_pos || !pb->target_quat || !pb->seeds || !pb->workspace) return LM_EINVAL;
     const int d = chain->dof;
     if (d < 1 || d > LM_MAX_DOF) return LM_EINVAL;
+    if (chunks > pp->max_chunks) return LM_EINVAL;
     if (pb->workspace_bytes < lm_solve_host_workspace_bytes(d, pb->B, pb->n, chunks)) return LM_ENOMEM;
     const size_t W = (size_t)pb->B * (size_t)pb->n;
-    constexpr int NS = 4, MAX_CHUNKS = 256;
-    if (chunks > MAX_CHUNKS) return LM_EINVAL;
-    // streams and the pinned totals buffer are created once per process and device and kept (creating
-    // them costs more than a whole step); calls are serialised by the mutex
-    struct Pipe {
-        int dev = -1;
-        cudaStream_t st[NS] = {nullptr, nullptr, nullptr, nullptr}; // host->device copies, device->host copies, 2 x kernels
-        cudaEvent_t ev_in[MAX_CHUNKS] = {}, ev_done[MAX_CHUNKS] = {};
-        unsigned long long *totals = nullptr;
-    };
-    static Pipe pipe;
-    static std::mutex pipe_mutex;
-    std::lock_guard<std::mutex> lock(pipe_mutex);
+    lm_pipe &pipe = *pp;
+    constexpr int NS = lm_pipe::NS;
     int rc = LM_OK;
     auto fail = [&](cudaError_t e) { rc = cuda_fail(e); };
     int dev = 0;
     LM_CUDA(cudaGetDevice(&dev));
-    if (pipe.dev != dev) {
-        for (int i = 0; i < NS; ++i) {
-            if (pipe.st[i]) cudaStreamDestroy(pipe.st[i]);
-            LM_CUDA(cudaStreamCreateWithFlags(&pipe.st[i], cudaStreamNonBlocking));
-        }
-        for (int i = 0; i < MAX_CHUNKS; ++i) {
-            if (pipe.ev_in[i]) cudaEventDestroy(pipe.ev_in[i]);
-            if (pipe.ev_done[i]) cudaEventDestroy(pipe.ev_done[i]);
-            LM_CUDA(cudaEventCreateWithFlags(&pipe.ev_in[i], cudaEventDisableTiming));
-            LM_CUDA(cudaEventCreateWithFlags(&pipe.ev_done[i], cudaEventDisableTiming));
-        }
-        if (!pipe.totals) LM_CUDA(cudaMallocHost(reinterpret_cast<void **>(&pipe.totals), 16 * (size_t)MAX_CHUNKS));
-        pipe.dev = dev;
-    }
+    if (dev != pipe.dev) return LM_EINVAL; // the handle belongs to the device that was current when it was created
+    // everything the caller has enqueued on its stream (e.g. the production of the host inputs by a device->host copy)
+    // precedes the pipeline
+    cudaStream_t caller = static_cast<cudaStream_t>(cuda_stream);
+    LM_CUDA(cudaEventRecord(pipe.ev_entry, caller));
+    for (int i = 0; i < NS; ++i) LM_CUDA(cudaStreamWaitEvent(pipe.st[i], pipe.ev_entry, 0));
     cudaStream_t s_in = pipe.st[0], s_out = pipe.st[1];
     cudaStream_t s_kk[2] = {pipe.st[2], pipe.st[3]}; // chunks alternate between two kernel streams: the tail of one
                                                      // chunk's last wave overlaps the head of the next chunk's kernel
@@ -700,8 +750,10 @@ int lm_solve_host(const lm_chain *chain, const lm_problem *pb, const lm_params *
             if (e != cudaSuccess) fail(e);
         }
     }
-    for (int i = 0; i < NS; ++i) {
-        cudaError_t e = cudaStreamSynchronize(pipe.st[i]);
+    for (int i = 0; i < NS; ++i) { // later work on the caller's stream is ordered after the pipeline; the host waits for it
+        cudaError_t e = cudaEventRecord(pipe.ev_exit[i], pipe.st[i]);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(caller, pipe.ev_exit[i], 0);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(pipe.st[i]);
         if (e != cudaSuccess && rc == LM_OK) fail(e);
     }
     if (st && rc == LM_OK) {

@@ -151,9 +151,8 @@ __device__ __forceinline__ float segment_box_closest(const float (&a)[3], const 
     return fminf(fmaxf(ts, tl), th);
 }
 
-// ---- the two halves of a pair's work.  *_qp: the closest-point problem (divergent, expensive; depends on the capsule
-// endpoints and the obstacle only, so ANY lane can run it for the owner: coll_rows_compact).  *_finish: distance, hinge
-// test and the row, with the frames of the owning lane.  coll_rows runs both halves back to back.
+// ---- the two halves of a pair's work.  *_qp: the closest-point problem (divergent, expensive; a pure function of the
+// capsule endpoints and the obstacle).  *_finish: distance, hinge test and the row, with the frames of the owning lane.
 struct EnvQp { float t, eb[3]; };  // parameter of the closest axis point, (axis point - box point) in the box frame
 __device__ __forceinline__ EnvQp env_qp(const KCaps &C, int ob, const float (&wa)[3], const float (&wb)[3]) {
     float ab[3], bb[3], pmin[3], pmax[3];
@@ -342,99 +341,9 @@ __device__ __forceinline__ void coll_rows(const KChain &ch, const KCaps &C, cons
     }
 }
 
-// ---- the same rows with the closest-point problems COMPACTED over the warp.  The 32 lanes of a warp are 32 different
-// trajectories: after the culling each lane keeps its own short list of pairs, and running the lists in step leaves a
-// handful of lanes active through the most expensive code of the step (ncu, round 2: 13.8 of 32 threads per instruction
-// over the whole cost kernel).  Here the surviving (lane, pair) items of the warp are written to shared memory with the
-// endpoints they need, every lane solves the QP of ONE item per round -- whoever owns it -- and each owner then finishes
-// its own items in its own order (ascending pair index, environment pairs first: the order of coll_rows, so the sums the
-// callback forms are bitwise the same; the QP is a pure function of the endpoints, so it does not matter which lane ran
-// it).  All 32 lanes must call (lanes without work pass live = false); `sc` is the calling warp's scratch.
-constexpr int COLL_CAP = 64; // items per round
-struct CollScratch {
-    float in[COLL_CAP][12];  // env: wa, wb; self: a1, b1, a2, b2
-    int32_t meta[COLL_CAP];  // pair index | kind << 8 (1 = robot-robot)
-    float out[COLL_CAP][4];  // env: t, eb; self: t1, t2
-};
-template <int D, typename SpecT, typename F>
-__device__ __forceinline__ void coll_rows_compact(const KChain &ch, const KCaps &C, const CapsWorld &W, const Pose<D> &Fr, bool live,
-                                                  CollScratch &sc, F &&f) {
-    const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
-    uint32_t need_env, need_self;
-    coll_cull(C, W, need_env, need_self);
-    if (!live) { need_env = 0u; need_self = 0u; }
-    const int cnt = __popc(need_env) + __popc(need_self);
-    int incl = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int v = __shfl_up_sync(full, incl, o);
-        if (lane >= o) incl += v;
-    }
-    const int total = __shfl_sync(full, incl, 31), off = incl - cnt; // this lane's items are off .. off + cnt - 1
-    for (int base = 0; base < total; base += COLL_CAP) {
-        { // owners: the items of this round
-            int idx = off;
-            for (uint32_t m = need_env; m; m &= m - 1u, ++idx) {
-                if (idx < base || idx >= base + COLL_CAP) continue;
-                const int p = __ffs(m) - 1, k = C.env_pair[p][0], sl = idx - base;
-                sc.meta[sl] = p;
-#pragma unroll
-                for (int i = 0; i < 3; ++i) { sc.in[sl][i] = W.wa[k][i]; sc.in[sl][3 + i] = W.wb[k][i]; }
-            }
-            for (uint32_t m = need_self; m; m &= m - 1u, ++idx) {
-                if (idx < base || idx >= base + COLL_CAP) continue;
-                const int p = __ffs(m) - 1, k1 = C.pair[p][0], k2 = C.pair[p][1], sl = idx - base;
-                sc.meta[sl] = p | (1 << 8);
-#pragma unroll
-                for (int i = 0; i < 3; ++i) {
-                    sc.in[sl][i] = W.wa[k1][i]; sc.in[sl][3 + i] = W.wb[k1][i];
-                    sc.in[sl][6 + i] = W.wa[k2][i]; sc.in[sl][9 + i] = W.wb[k2][i];
-                }
-            }
-        }
-        __syncwarp();
-        const int nround = min(COLL_CAP, total - base);
-        for (int sl = lane; sl < nround; sl += 32) { // workers: one closest-point problem each
-            const int mt = sc.meta[sl], p = mt & 0xff;
-            if (mt >> 8) {
-                float a1[3], b1[3], a2[3], b2[3], t1, t2;
-#pragma unroll
-                for (int i = 0; i < 3; ++i) { a1[i] = sc.in[sl][i]; b1[i] = sc.in[sl][3 + i]; a2[i] = sc.in[sl][6 + i]; b2[i] = sc.in[sl][9 + i]; }
-                segment_closest(a1, b1, a2, b2, t1, t2);
-                sc.out[sl][0] = t1; sc.out[sl][1] = t2;
-            } else {
-                float wa[3], wb[3];
-#pragma unroll
-                for (int i = 0; i < 3; ++i) { wa[i] = sc.in[sl][i]; wb[i] = sc.in[sl][3 + i]; }
-                const EnvQp qp = env_qp(C, C.env_pair[p][1], wa, wb);
-                sc.out[sl][0] = qp.t; sc.out[sl][1] = qp.eb[0]; sc.out[sl][2] = qp.eb[1]; sc.out[sl][3] = qp.eb[2];
-            }
-        }
-        __syncwarp();
-        { // owners: distance, hinge test and row of their items, in their order
-            int idx = off;
-            for (uint32_t m = need_env; m; m &= m - 1u, ++idx) {
-                if (idx < base || idx >= base + COLL_CAP) continue;
-                const int p = __ffs(m) - 1, k = C.env_pair[p][0], ob = C.env_pair[p][1], sl = idx - base;
-                float wa[3], wb[3];
-#pragma unroll
-                for (int i = 0; i < 3; ++i) { wa[i] = W.wa[k][i]; wb[i] = W.wb[k][i]; }
-                EnvQp qp;
-                qp.t = sc.out[sl][0]; qp.eb[0] = sc.out[sl][1]; qp.eb[1] = sc.out[sl][2]; qp.eb[2] = sc.out[sl][3];
-                env_finish<D, SpecT, false>(ch, C, k, ob, wa, wb, qp, Fr, f, nullptr);
-            }
-            for (uint32_t m = need_self; m; m &= m - 1u, ++idx) {
-                if (idx < base || idx >= base + COLL_CAP) continue;
-                const int p = __ffs(m) - 1, k1 = C.pair[p][0], k2 = C.pair[p][1], sl = idx - base;
-                float a1[3], b1[3], a2[3], b2[3];
-#pragma unroll
-                for (int i = 0; i < 3; ++i) { a1[i] = W.wa[k1][i]; b1[i] = W.wb[k1][i]; a2[i] = W.wa[k2][i]; b2[i] = W.wb[k2][i]; }
-                self_finish<D, SpecT, false>(ch, C, k1, k2, a1, b1, a2, b2, sc.out[sl][0], sc.out[sl][1], Fr, f, nullptr);
-            }
-        }
-        __syncwarp(); // the scratch is rewritten by the next round
-    }
-}
+// Tried and removed (round 2, commit "Collision rows: found once per point ..."): compacting the closest-point problems
+// over the warp (items in shared memory, every lane solves one per round, owners finish in their own order; bitwise the
+// same).  A warp holds only ~6 items per waypoint on the bench scene, so a round still runs with ~6 lanes: 223 M -> 190 M
+// warp instructions, 338 -> 328 us for the cost kernel with 19 pairs, and slower with 9 pairs (0.521 -> 0.551 ms per iteration).
 
 } // namespace lmk

@@ -819,9 +819,7 @@ __global__ void __launch_bounds__(TL_SOLVE_MAX_THREADS) tl_solve_kernel(const __
 template <int D, bool FAST, bool WEIGHTED, typename SpecT, bool COLL, bool INIT>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(const __grid_constant__ TArgs A) {
     const Slot s = slot_of_thread(A);
-    // With collision rows all 32 lanes of a warp stay (a lane without work still solves other lanes' closest-point
-    // problems, coll_rows_compact); `live` gates every store.  wid is the same for the whole warp.
-    if (COLL ? (s.wid >= A.Bt * A.n) : !s.valid) return;
+    if (!s.valid) return;
     // every load below is issued before the first use: the joint values of BOTH buffers are fetched and the
     // trajectory's `sel` picks afterwards (a dependent address would cost one more DRAM round trip)
     const uint32_t pk = A.its[s.b];
@@ -842,8 +840,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
     }
     float pt[3], Rt[3][3];
     tl_load_target(A, s, pt, Rt);
-    const bool live = s.valid && (INIT || !((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0)));
-    if (!COLL && !live) return;
+    if (!INIT && ((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[s.b] == 0))) return;
     float qt[D], qn[D];
     bool clamped = false;
     auto point_of = [&](int u, int j, bool &cl) {
@@ -860,18 +857,17 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
         bool dummy = false;
         qt[j] = point_of(0, j, clamped);
         qn[j] = (s.i + 1 < A.n) ? point_of(1, j, dummy) : 0.f;
-        if (!INIT && live) A.q[(int64_t)(1 - sel) * D * A.nS + toff<D>(s.wid, j, s.lane)] = qt[j];
+        if (!INIT) A.q[(int64_t)(1 - sel) * D * A.nS + toff<D>(s.wid, j, s.lane)] = qt[j];
         if (s.i + 1 < A.n) {
             const float t = sub(qn[j], qt[j]);
             fd = fma_(t, t, fd);
         }
     }
     // "a trial point of this trajectory was clamped": integer atomic (order-free), skipped once the bit is seen set
-    if (!INIT && live && clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
+    if (!INIT && clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
     float fc = 0.f;
     Pose<D> P;
     if (COLL) {
-        __shared__ CollScratch scratch[LM_MAX_THREADS / 32];
         CapsWorld W;
         CapsSink sink(A.caps, W);
         sink.base();
@@ -881,7 +877,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
         const int dst = INIT ? sel : 1 - sel;
         float *rw = A.rows + (int64_t)dst * RC * A.nS + toff<RC>(s.wid, 0, s.lane); // component c at rw[c * 32]
         int cnt = 0;
-        coll_rows_compact<D, SpecT>(A.ch, A.caps, W, P, live, scratch[threadIdx.x >> 5], [&](const float (&g)[D], float r) {
+        coll_rows<D, SpecT>(A.ch, A.caps, W, P, [&](const float (&g)[D], float r) {
             fc = fma_(r, r, fc);
             if (cnt < TL_RMAX) {
 #pragma unroll
@@ -891,7 +887,6 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
             }
             ++cnt;
         });
-        if (!live) return;
         A.rcnt[(int64_t)dst * A.nS + s.wid * 32 + s.lane] = cnt > TL_RMAX ? TL_ROWS_OVERFLOW : cnt;
     } else {
         eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);

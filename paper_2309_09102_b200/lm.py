@@ -31,7 +31,7 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_strerror", "lm_launch_count", "lm_fp32_peak_form",
            "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
            "lm_traj_fetch", "lm_traj_set_trace", "lm_traj_set_capsules", "lm_traj_set_obstacles",
-           "lm_solve_host_workspace_bytes", "lm_solve_host",
+           "lm_solve_host_workspace_bytes", "lm_solve_host", "lm_pipe_create", "lm_pipe_solve", "lm_pipe_destroy",
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch",
            "lm_search_workspace_bytes", "lm_search_default_params", "lm_search")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR, LM_FMA_FORM_RRS, LM_FMA_FORM_RSS, LM_FMA_FORM_MUL, LM_FMA_FORM_PPP, LM_FMA_FORM_PSP = range(7)
@@ -158,6 +158,11 @@ def lib() -> C.CDLL:
         L.lm_solve_host_workspace_bytes.restype = C.c_size_t
         L.lm_solve_host.argtypes = [C.POINTER(LmChain), C.POINTER(LmProblem), C.POINTER(LmParams), C.c_int32, C.c_int32,
                                     C.c_void_p, C.POINTER(LmStats)]
+        L.lm_pipe_create.argtypes = [C.POINTER(C.c_void_p), C.c_int32]
+        L.lm_pipe_solve.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(LmChain), C.POINTER(LmProblem), C.POINTER(LmParams), C.c_int32,
+                                    C.c_int32, C.c_void_p, C.POINTER(LmStats)]
+        L.lm_pipe_destroy.argtypes = [C.c_void_p]
+        L.lm_pipe_destroy.restype = None
         L.lm_plan_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64]
         L.lm_plan_workspace_bytes.restype = C.c_size_t
         L.lm_plan_default_params.argtypes = [C.POINTER(LmPlanParams)]
@@ -350,6 +355,23 @@ def lm_solve_host(chain: LmChain, problem: LmProblem, params: LmParams, max_iter
                   q_out_ptr: Optional[int], stats: Optional[LmStats]) -> None:
     _check(lib().lm_solve_host(C.byref(chain), C.byref(problem), C.byref(params), int(max_iters), int(chunks),
                                q_out_ptr, C.byref(stats) if stats is not None else None), "lm_solve_host")
+
+
+def lm_pipe_create(max_chunks: int) -> C.c_void_p:
+    """Streams / events / pinned totals of the host-data pipeline on the CURRENT device (include/lm.h)."""
+    out = C.c_void_p()
+    _check(lib().lm_pipe_create(C.byref(out), int(max_chunks)), "lm_pipe_create")
+    return out
+
+
+def lm_pipe_solve(pipe, chain: LmChain, problem: LmProblem, params: LmParams, max_iters: int, chunks: int,
+                  q_out_ptr: Optional[int], stats: Optional[LmStats], cuda_stream: int = 0) -> None:
+    _check(lib().lm_pipe_solve(pipe, C.c_void_p(cuda_stream), C.byref(chain), C.byref(problem), C.byref(params), int(max_iters),
+                               int(chunks), q_out_ptr, C.byref(stats) if stats is not None else None), "lm_pipe_solve")
+
+
+def lm_pipe_destroy(pipe) -> None:
+    lib().lm_pipe_destroy(pipe)
 
 
 def lm_plan_workspace_bytes(dof: int, B: int, n: int) -> int:

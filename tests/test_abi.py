@@ -104,6 +104,34 @@ def test_init_validation_without_gpu(L):
     L.lm_free(ctx)
 
 
+def test_pipe_handle_validation_without_a_device():
+    """lm_pipe_* (include/lm.h): argument checks come before any CUDA call, null handles are harmless, and a handle is an
+    independent object (two creations never share state: on a box without a GPU both fail in CUDA, not in the library)."""
+    import ctypes as C
+    L = lm.lib()
+    assert L.lm_pipe_create(None, 4) == lm.LM_EINVAL
+    h = C.c_void_p()
+    assert L.lm_pipe_create(C.byref(h), 0) == lm.LM_EINVAL and not h.value
+    assert L.lm_pipe_create(C.byref(h), 257) == lm.LM_EINVAL and not h.value
+    L.lm_pipe_destroy(None)
+    assert L.lm_pipe_solve(None, None, None, None, None, 1, 1, None, None) == lm.LM_EINVAL
+    import torch
+    handles = []
+    for _ in range(2):  # one per "device slot" of a multi-GPU process: independent objects, no process-global state
+        h = C.c_void_p()
+        rc = L.lm_pipe_create(C.byref(h), 8)
+        if torch.cuda.is_available():
+            assert rc == lm.LM_OK and h.value
+            handles.append(h)
+        else:
+            assert rc == lm.LM_ECUDA and not h.value
+    assert len({x.value for x in handles}) == len(handles)
+    for x in handles:
+        # a handle rejects malformed problems before touching its streams
+        assert L.lm_pipe_solve(x, None, None, None, None, 1, 1, None, None) == lm.LM_EINVAL
+        L.lm_pipe_destroy(x)
+
+
 def test_product_has_no_oracle_dependency():
     """The package never imports oracle/ (no CPU fallback): grep the sources."""
     pkg = os.path.join(ROOT, "paper_2309_09102_b200")

@@ -369,3 +369,18 @@ def test_solve_host_pipelined_equals_the_stepwise_path(chunks):
     assert st.converged_trajectories == ref["converged_trajectories"]
     with pytest.raises(lm.LmError):
         lm.lm_solve_host(cchain, pb, prm, w.max_iters, w.B + 1, q.data_ptr(), st)
+    # the same through a kept handle (lm_pipe_*), twice, on a caller's stream that still has the production of the host
+    # inputs queued: the pipeline must start after it and later work on the stream after the pipeline
+    pipe = lm.lm_pipe_create(8)
+    stream = torch.cuda.Stream()
+    dev_seeds = torch.from_numpy(np.ascontiguousarray(w.seeds.T)).cuda()
+    for rep in range(2):
+        q.zero_(); res.zero_(); seeds.zero_()
+        with torch.cuda.stream(stream):
+            seeds.copy_(dev_seeds, non_blocking=True)           # inputs arrive on the caller's stream
+            lm.lm_pipe_solve(pipe, cchain, pb, prm, w.max_iters, chunks, q.data_ptr(), st, int(stream.cuda_stream))
+        assert np.array_equal(q.numpy().T, ref["q"]) and np.array_equal(res.numpy(), ref["res_norm"])
+        assert st.total_waypoint_iters == ref["total_waypoint_iters"]
+    with pytest.raises(lm.LmError):                              # more chunks than the handle was created for
+        lm.lm_pipe_solve(pipe, cchain, pb, prm, w.max_iters, 9, q.data_ptr(), st)
+    lm.lm_pipe_destroy(pipe)
