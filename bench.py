@@ -402,12 +402,12 @@ def traj_step_alg_bytes(d: int, refine: int = 1, fused: bool = True) -> float:
       each refinement  q d + delta d + target 7 + -S^-1 NA in, z d out, NA + 2 d back in, delta d out = 2 NA + 6 d + 7
       trial cost       q d + delta d + target 7 in, candidate q d + 3 cost terms out               = 3 d + 10
       decision         3 cost terms in.
-    Unfused path (small batches, collision rows): + the round trip of w_p^2 J^T J, g (2 (NA + d)) and rho (2 d) and their
-    inputs a second time (d + 7)."""
+    Unfused path (small batches, collision rows): + the round trip of w_p^2 J^T J, g (2 (NA + d)) and of rho (2 d); the
+    inputs q, delta, target are then read by the per-waypoint kernels instead of the solve kernels."""
     na = d * (d + 1) // 2
     words = (2 * na + 4 * d + 7) + refine * (2 * na + 6 * d + 7) + (3 * d + 10) + 3
     if not fused:
-        words += (2 * (na + d) + d + 7) + refine * (2 * d)
+        words += 2 * (na + d) + refine * (2 * d)
     return 4.0 * words
 
 

@@ -121,6 +121,27 @@ def test_plan_is_repeatable_and_argument_errors():
         assert np.array_equal(outs[0][k], outs[1][k], equal_nan=True), k
 
 
+def test_schedule_is_the_same_on_the_fused_and_unfused_step():
+    """lm_plan_run gates the trajectory-level step per trajectory (P2): the gate reaches the producer warps of the fused
+    solve kernels as it reaches the per-waypoint kernels -- identical records, verdicts and latest-valid joints."""
+    from paper_2309_09102_b200 import lm
+    ch = wl.panda_chain()
+    _, w = build_problem(ch, 40, 90, 0.05, 47)
+    outs = []
+    for mode in (1, 2):
+        s = lm.Solver(ch, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=1e-5))
+        s.traj_attach(lm.lm_traj_default_params(w_diff=0.5))
+        s.traj_set_fused(mode)
+        s.plan_attach()
+        s.plan_run(3)
+        outs.append(s.plan_fetch())
+        s.close()
+    for k in ("q_valid", "length", "valid", "records", "mjac_rev", "first_valid_cycle"):
+        if k in outs[0]:
+            assert np.array_equal(outs[0][k], outs[1][k], equal_nan=True), k
+    assert outs[0]["valid_trajectories"] == outs[1]["valid_trajectories"]
+
+
 def test_schedule_with_capsules_requires_collision_free_trajectories():
     """validity includes "no collision"; with lm_traj_set_capsules the schedule checks the smallest
     capsule clearance of every waypoint and the trajectory-level step carries the collision rows."""

@@ -440,3 +440,35 @@ def test_fused_and_unfused_paths_return_the_same_bits(chain_name, shape):
             assert np.array_equal(g1[k], g2[k], equal_nan=g1[k].dtype.kind == "f"), (k, refine)
         assert np.array_equal(f1["q"], f2["q"]) and np.array_equal(f1["res_norm"], f2["res_norm"])
         assert l2 - l1 == 2 * (1 + refine), (l1, l2)   # per iteration: fused 3 + refine, unfused 4 + 2 refine
+
+
+def test_fused_path_with_shared_targets_and_weights_matches_the_oracle():
+    """The producer warps of the fused solve read the shared target list by waypoint index and carry the pose weights:
+    same bits as the unfused path, and one teacher-forced step within the bar of the oracle (several tiles, ragged)."""
+    L = lm()
+    ch = wl.panda_chain()
+    B, n = 70, 33
+    w1 = make_problem(ch, 1, n, 0.0, 28)
+    rng = np.random.default_rng(4)
+    seeds = np.clip(w1.truth[None] + 0.05 * rng.normal(size=(B, n, 7)), ch.q_lo, ch.q_hi).astype(np.float32)
+    prm = L.lm_default_params(tol=0.0, w_pos=2.0, w_rot=0.5)
+    outs = []
+    for mode in (1, 2):
+        s = L.Solver(ch, B, n, w1.target_pos, w1.target_quat, seeds.reshape(B * n, 7), params=prm, shared_targets=True)
+        s.traj_attach(L.lm_traj_default_params(w_pose=1.5, w_diff=0.3))
+        s.traj_set_fused(mode)
+        s.traj_enable_trace()
+        s.traj_run(1)
+        outs.append((s.traj_fetch(), s.fetch()))
+        s.close()
+    (g, f), (g2, f2) = outs
+    for k in ("cost", "lam", "mask", "trial_q", "F_trial"):
+        assert np.array_equal(g[k], g2[k], equal_nan=g[k].dtype.kind == "f"), k
+    assert np.array_equal(f["q"], f2["q"])
+    tprm = torc.TrajParams(w_pose=1.5, w_diff=0.3)
+    tp = np.repeat(w1.target_pos.astype(np.float64)[None], B, axis=0)
+    tq = np.repeat(w1.target_quat.astype(np.float64)[None], B, axis=0)
+    st = torc.init_state(seeds.astype(np.float64), tprm)
+    torc.advance(ch, orc.Params(w_pos=2.0, w_rot=0.5), tprm, tp, tq, st, 1)
+    assert np.abs(g["trial_q"].reshape(B, n, 7) - st.trial_q).max() <= 2e-5
+    assert np.allclose(g["F_trial"], st.F_trial, rtol=1e-4)
