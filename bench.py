@@ -350,6 +350,9 @@ def run_gpu(args) -> None:
     if args.workload == "C4" and full_size:
         # what an unregistered robot gets: the generic (run-time chain structure) kernel on the same workload
         extra["generic_kernel_C4"] = time_kernel_option(lm, torch, w, device, stream, peak_tf, lm.LM_OPT_GENERIC_KERNEL, 1)
+        # ... and after lm_specialize: the same kernel template compiled at run time (NVRTC) for the structure of a chain that
+        # has no ahead-of-time kernel -- here the Panda with a rotated flange tool on the same inputs
+        extra["jit_specialized_C4"] = time_jit(lm, torch, w, device, stream, peak_tf)
         # the lane-group alternative the north star names (2 / 4 lanes per waypoint), measured beside the product kernel
         extra["lane_group_variants"] = {f"{g}_lanes": time_kernel_option(lm, torch, w, device, stream, peak_tf, lm.LM_OPT_LANES_PER_WAYPOINT, g)
                                         for g in (2, 4)}
@@ -711,6 +714,29 @@ def time_kernel_option(lm, torch, w, device, stream, peak_tf: float, option: int
     tf = ALG_FLOP.get(d, 1459.0 * d / 7.0) * iters / (ms * 1e-3) / 1e12
     return {"kernel": name, "ms_per_step": ms, "waypoint_iterations_per_sec": iters / (ms * 1e-3), "achieved_tflops": tf,
             "frac_of_derived_peak": tf / peak_tf}
+
+
+def time_jit(lm, torch, w, device, stream, peak_tf: float, reps: int = 10) -> dict:
+    """lm_specialize on a chain whose structure is not registered (Panda + rotated tool; the headline's targets and seeds):
+    generic kernel, then the run-time specialised one; compile time of the first call."""
+    import copy
+    ch = copy.deepcopy(w.chain)
+    ch.name = "panda_rotated_tool"
+    ch.tool = np.array([0.01, -0.02, 0.107, 0.9238795325112867, 0.2, -0.1, 0.3104])
+    ch.tool[3:] /= np.linalg.norm(ch.tool[3:])
+    d = int(ch.dof)
+    prm = lm.lm_default_params(lambda0=w.lambda0, tol=w.tol)
+    s = lm.Solver(ch, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=prm, device=str(device), stream=stream)
+    out = {"chain": "Panda with a rotated flange tool (no ahead-of-time kernel for this structure)"}
+    ms, iters, _ = _time_runs(torch, s, stream, w.max_iters, reps)
+    out["generic"] = {"kernel": s.kernel_name, "ms_per_step": ms, "frac_of_derived_peak": ALG_FLOP[d] * iters / (ms * 1e-3) / 1e12 / peak_tf}
+    t0 = time.perf_counter()
+    s.specialize()
+    out["compile_s"] = time.perf_counter() - t0
+    ms, iters, _ = _time_runs(torch, s, stream, w.max_iters, reps)
+    out["specialized"] = {"kernel": s.kernel_name, "ms_per_step": ms, "frac_of_derived_peak": ALG_FLOP[d] * iters / (ms * 1e-3) / 1e12 / peak_tf}
+    s.close()
+    return out
 
 
 def time_c3(lm, torch, wl, device, stream, peak_tf: float, reps: int = 10) -> dict:

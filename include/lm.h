@@ -210,6 +210,17 @@ int lm_set_option(lm_ctx *ctx, int32_t option, int32_t value);
  * structure, csrc/lm_specs.cuh) or "generic".  Static string. */
 const char *lm_kernel_name(lm_ctx *ctx);
 
+/* Run-time specialisation (csrc/lm_jit.cu).  Only the benchmark's robots have an ahead-of-time kernel for their chain
+ * STRUCTURE (which joints are prismatic, which twists are 0 / +-pi/2, which offsets vanish; csrc/lm_specs.cuh); any other
+ * chain runs the generic kernel (same results, ~1.35 x the time).  lm_specialize compiles the same kernel template for
+ * this context's structure with NVRTC (about one second, once per structure, device and process; cached), and lm_step /
+ * lm_run of this context launch it from then on: lm_kernel_name() returns "jit".  The values are those of the generic
+ * kernel bit for bit (the specialisation only drops multiplications by exact 0 / +-1).  No-op (LM_OK) for a chain that
+ * already has a specialised kernel.  LM_ECUDA when libnvrtc.so.12 cannot be loaded, the compilation fails or a CUDA call
+ * fails: lm_strerror(LM_ECUDA) has the reason, and the context keeps the generic kernel.  LM_OPT_GENERIC_KERNEL = 1 still
+ * selects the generic kernel; the trajectory-level kernels are not specialised at run time. */
+int lm_specialize(lm_ctx *ctx);
+
 /* Forward kinematics on the device with the context's chain (S1 of the hot path):
  * q [d][count] -> pos [3][count], rot [9][count] (row-major R, SoA).  Device pointers.  Async. */
 int lm_fk(lm_ctx *ctx, const float *q, int64_t count, float *pos, float *rot);

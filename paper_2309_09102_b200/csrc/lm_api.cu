@@ -179,7 +179,9 @@ int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_
         k.tool_has_rot = ident ? 0u : 1u;
         for (int i = 0; i < 3; ++i) k.tool_p[i] = (float)chain->tool[i];
     }
-    c->spec_id = match_spec(chain_signature(d, k));
+    c->sig = chain_signature(d, k);
+    c->spec_id = match_spec(c->sig);
+    c->jit_fn = nullptr;
     c->use_generic = false;
     c->lanes = 1;
     a.lambda0 = prm->lambda0; a.nu_up = prm->nu_up; a.inv_nu_down = (float)(1.0 / (double)prm->nu_down);
@@ -228,6 +230,7 @@ cudaError_t launch_iterate(lm_ctx *c, const KArgs &a) {
         return launch_iterate_lanegroup(c->spec_id, c->lanes, grid_lg, c->block, c->stream, a);
     }
     const unsigned grid = (unsigned)((c->W + c->block - 1) / c->block);
+    if (c->jit_fn && !c->use_generic) return jit_launch(c->jit_fn, grid, c->block, c->stream, a); // lm_specialize
     if (c->spec_id != SPEC_GENERIC && !c->use_generic)
         return launch_iterate_spec(c->spec_id, c->fast, weighted, grid, c->block, c->stream, a);
     return c->dof <= 4 ? launch_iterate_generic_lo(c->dof, c->fast, weighted, grid, c->block, c->stream, a)
@@ -440,7 +443,19 @@ int lm_set_option(lm_ctx *c, int32_t option, int32_t value) {
 
 const char *lm_kernel_name(lm_ctx *c) {
     if (!c) return "";
+    if (c->jit_fn && !c->use_generic) return "jit";
     return (c->spec_id != SPEC_GENERIC && !c->use_generic) ? spec_name(c->spec_id) : "generic";
+}
+
+int lm_specialize(lm_ctx *c) {
+    if (!c) return LM_EINVAL;
+    if (c->spec_id != SPEC_GENERIC || c->jit_fn) return LM_OK; // an ahead-of-time kernel (or an earlier call) already serves this chain
+    void *fn = nullptr;
+    const int rc = jit_get_kernel(c->sig, c->fast, c->args.weighted != 0, c->args.variant, &fn);
+    if (rc == LM_EINVAL) snprintf(g_cuda_err, sizeof(g_cuda_err), "lm_specialize: %s", jit_last_log());
+    if (rc != LM_OK) return rc == LM_EINVAL ? LM_ECUDA : rc; // the reason is in lm_strerror(LM_ECUDA)
+    c->jit_fn = fn;
+    return LM_OK;
 }
 
 int lm_set_state(lm_ctx *c, const float *q, const float *lambda) {

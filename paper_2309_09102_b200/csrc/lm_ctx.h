@@ -39,6 +39,10 @@ struct PlanState { // non-stationary schedule + anytime bookkeeping (lm_plan_*),
 };
 
 int cuda_fail(cudaError_t e);              // records the error string for lm_strerror, returns LM_ECUDA
+// lm_jit.cu: the LM kernel compiled at run time for one chain structure (lm_specialize)
+int jit_get_kernel(const ChainSpec &s, bool fast, bool weighted, int var, void **fn_out);
+cudaError_t jit_launch(void *fn, unsigned grid, unsigned block, cudaStream_t s, const KArgs &a);
+const char *jit_last_log();
 std::atomic<long long> &launch_counter();  // lm_launch_count
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -60,6 +64,8 @@ struct lm_ctx {
     int spec_id;      // structure-matched specialised kernel (lm_specs.cuh) or SPEC_GENERIC
     bool use_generic; // LM_OPT_GENERIC_KERNEL
     int lanes;        // LM_OPT_LANES_PER_WAYPOINT: 1 (default), 2 or 4
+    lmk::ChainSpec sig; // structure of the chain (lm_api.cu: chain_signature)
+    void *jit_fn;     // lm_specialize: the kernel compiled for `sig` (a CUfunction), nullptr = none
     lmk::TrajState traj;
     lmk::PlanState plan;
 };

@@ -15,8 +15,18 @@
 //
 // Step names S1..S9 follow DESIGN.md section 2.
 #pragma once
+#ifndef __CUDACC_RTC__
 #include <cuda_runtime.h>
 #include <stdint.h>
+#else // run-time compilation (lm_jit.cu): NVRTC has the CUDA built-ins but no host headers
+typedef signed char int8_t;
+typedef unsigned char uint8_t;
+typedef unsigned short uint16_t;
+typedef int int32_t;
+typedef unsigned int uint32_t;
+typedef long long int64_t;
+typedef unsigned long long uint64_t;
+#endif
 
 namespace lmk {
 

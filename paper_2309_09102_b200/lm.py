@@ -31,7 +31,7 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_strerror", "lm_launch_count", "lm_fp32_peak_form",
            "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
            "lm_traj_fetch", "lm_traj_set_trace", "lm_traj_set_capsules", "lm_traj_set_obstacles",
-           "lm_solve_host_workspace_bytes", "lm_solve_host", "lm_pipe_create", "lm_pipe_solve", "lm_pipe_destroy",
+           "lm_solve_host_workspace_bytes", "lm_solve_host", "lm_pipe_create", "lm_pipe_solve", "lm_pipe_destroy", "lm_specialize",
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch",
            "lm_search_workspace_bytes", "lm_search_default_params", "lm_search")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR, LM_FMA_FORM_RRS, LM_FMA_FORM_RSS, LM_FMA_FORM_MUL, LM_FMA_FORM_PPP, LM_FMA_FORM_PSP = range(7)
@@ -134,6 +134,7 @@ def lib() -> C.CDLL:
         L.lm_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.lm_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.lm_set_option.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        L.lm_specialize.argtypes = [C.c_void_p]
         L.lm_kernel_name.argtypes = [C.c_void_p]
         L.lm_kernel_name.restype = C.c_char_p
         L.lm_fk.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
@@ -520,6 +521,10 @@ class Solver:
 
     def use_generic_kernel(self, on: bool = True) -> None:
         lm_set_option(self._ctx, LM_OPT_GENERIC_KERNEL, int(on))
+
+    def specialize(self) -> None:
+        """lm_specialize: compile (NVRTC, once per chain structure) and use a kernel specialised to this chain."""
+        _check(lib().lm_specialize(self._ctx), "lm_specialize")
 
     def set_lanes_per_waypoint(self, lanes: int) -> None:
         """1 (default), 2 or 4 lanes per waypoint block (the measured lane-group alternative, include/lm.h)."""

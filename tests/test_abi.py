@@ -89,6 +89,7 @@ def test_init_validation_without_gpu(L):
     assert init(params=lm.lm_default_params(refine_steps=3))[0] == lm.LM_EINVAL
     assert init(params=lm.lm_default_params(lambda0=0.0))[0] == lm.LM_EINVAL
     # null handles
+    assert L.lm_specialize(None) == lm.LM_EINVAL
     assert L.lm_step(None) == lm.LM_EINVAL and L.lm_run(None, 5) == lm.LM_EINVAL
     assert L.lm_fetch(None, None, None) == lm.LM_EINVAL and L.lm_reset(None) == lm.LM_EINVAL
     # a well-formed device-memory problem binds without touching the device; max_iters is checked

@@ -326,3 +326,65 @@ def test_lane_group_option_is_validated(lm):
     with pytest.raises(lm.LmError):      # nor of the disclosed variants
         s.set_lanes_per_waypoint(2)
     s.close()
+
+
+# ------------------------------------------------------------------ run-time specialisation (lm_specialize)
+
+def _unregistered_chains():
+    rot_tool = wl.panda_chain()
+    rot_tool.name = "panda_rot_tool"
+    rot_tool.tool = np.array([0.01, -0.02, 0.107, 0.9238795325112867, 0.2, -0.1, 0.3104])
+    rot_tool.tool[3:] /= np.linalg.norm(rot_tool.tool[3:])
+    p = wl.panda_chain()
+    six = wl.Chain("panda6", 6, p.joint_type[:6], p.a[:6], p.alpha[:6], p.d[:6], p.theta[:6], p.q_lo[:6], p.q_hi[:6], p.tool)
+    gen = wl.Chain("gen3", 3, np.array([0, 1, 0], np.int32), np.array([0.1, 0.2, -0.3]), np.array([0.3, -1.1, 2.0]),
+                   np.array([0.05, 0.1, 0.2]), np.array([0.4, -0.7, 1.3]), np.full(3, -2.0), np.full(3, 2.0),
+                   np.array([0.1, 0.0, 0.2, 1, 0, 0, 0.0]))
+    return [rot_tool, six, gen]
+
+
+@pytest.mark.parametrize("chain", _unregistered_chains(), ids=lambda c: c.name)
+def test_runtime_specialised_kernel_equals_the_generic_one(lm, chain):
+    """lm_specialize (include/lm.h): a chain without an ahead-of-time kernel gets the SAME kernel template compiled for
+    its structure with NVRTC.  Bit-identical to the generic kernel (joints, residuals, iteration counts, masks; also with
+    weights, with the dual solver and stepwise), and within the bars of the oracle."""
+    rng = np.random.default_rng(7)
+    B, n, d = 9, 41, chain.dof
+    truth = wl.smooth_joint_paths(chain, B, n, 3, 0.3, rng)
+    w = wl._from_truth("J", chain, truth, 0.05, rng, H.oracle_fk(chain), 1e-5, 30)
+    for kw in ({}, {"w_pos": 2.0, "w_rot": 0.5}, {"solver": lm.LM_SOLVER_DUAL}):
+        s = H.make_solver(w, **kw)
+        assert s.kernel_name == "generic"
+        s.run(w.max_iters)
+        g0 = s.fetch()
+        s.specialize()
+        assert s.kernel_name == "jit"
+        s.reset()
+        s.run(w.max_iters)
+        g1 = s.fetch()
+        s.reset()
+        for _ in range(3):
+            s.step()
+        s.run(w.max_iters)
+        g2 = s.fetch()
+        s.use_generic_kernel(True)
+        assert s.kernel_name == "generic"
+        s.close()
+        for k in ("q", "res_norm", "iters", "mask", "status", "lam"):
+            assert np.array_equal(g0[k], g1[k]) and np.array_equal(g0[k], g2[k]), (k, kw)
+    if chain.dof == 7:   # and against the oracle (the redundant arm; the truncated 6- and 3-joint chains of this list are
+        o = H.run_oracle(w)  # near-singular test articles for the code paths, graded by the bitwise comparison above)
+        s = H.make_solver(w)
+        s.specialize()
+        s.run(w.max_iters)
+        g = s.fetch()
+        s.close()
+        _check_free_running(w, g, o, check_pose=False)
+
+
+def test_specialize_is_a_no_op_for_registered_chains(lm):
+    w = wl.config1(H.oracle_fk(wl.panda_chain()))
+    s = H.make_solver(w)
+    s.specialize()
+    assert s.kernel_name == "panda7"
+    s.close()
