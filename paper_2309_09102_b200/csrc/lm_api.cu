@@ -182,6 +182,7 @@ int lm_init(lm_ctx **out, const lm_chain *chain, const lm_problem *pb, const lm_
     c->sig = chain_signature(d, k);
     c->spec_id = match_spec(c->sig);
     c->jit_fn = nullptr;
+    c->jit_hot = false;
     c->use_generic = false;
     c->lanes = 1;
     a.lambda0 = prm->lambda0; a.nu_up = prm->nu_up; a.inv_nu_down = (float)(1.0 / (double)prm->nu_down);
@@ -230,7 +231,8 @@ cudaError_t launch_iterate(lm_ctx *c, const KArgs &a) {
         return launch_iterate_lanegroup(c->spec_id, c->lanes, grid_lg, c->block, c->stream, a);
     }
     const unsigned grid = (unsigned)((c->W + c->block - 1) / c->block);
-    if (c->jit_fn && !c->use_generic) return jit_launch(c->jit_fn, grid, c->block, c->stream, a); // lm_specialize
+    if (c->jit_fn && !c->use_generic && (!c->jit_hot || (a.refine == 1 && a.trace_q == nullptr))) // lm_specialize
+        return jit_launch(c->jit_fn, grid, c->block, c->stream, a);
     if (c->spec_id != SPEC_GENERIC && !c->use_generic)
         return launch_iterate_spec(c->spec_id, c->fast, weighted, grid, c->block, c->stream, a);
     return c->dof <= 4 ? launch_iterate_generic_lo(c->dof, c->fast, weighted, grid, c->block, c->stream, a)
@@ -443,7 +445,7 @@ int lm_set_option(lm_ctx *c, int32_t option, int32_t value) {
 
 const char *lm_kernel_name(lm_ctx *c) {
     if (!c) return "";
-    if (c->jit_fn && !c->use_generic) return "jit";
+    if (c->jit_fn && !c->use_generic && (!c->jit_hot || (c->args.refine == 1 && c->args.trace_q == nullptr))) return "jit";
     return (c->spec_id != SPEC_GENERIC && !c->use_generic) ? spec_name(c->spec_id) : "generic";
 }
 
@@ -451,10 +453,12 @@ int lm_specialize(lm_ctx *c) {
     if (!c) return LM_EINVAL;
     if (c->spec_id != SPEC_GENERIC || c->jit_fn) return LM_OK; // an ahead-of-time kernel (or an earlier call) already serves this chain
     void *fn = nullptr;
-    const int rc = jit_get_kernel(c->sig, c->fast, c->args.weighted != 0, c->args.variant, &fn);
+    const bool hot = !c->fast && c->args.variant == 0 && c->args.refine == 1;
+    const int rc = jit_get_kernel(c->sig, c->fast, c->args.weighted != 0, c->args.variant, hot, &fn);
     if (rc == LM_EINVAL) snprintf(g_cuda_err, sizeof(g_cuda_err), "lm_specialize: %s", jit_last_log());
     if (rc != LM_OK) return rc == LM_EINVAL ? LM_ECUDA : rc; // the reason is in lm_strerror(LM_ECUDA)
     c->jit_fn = fn;
+    c->jit_hot = hot;
     return LM_OK;
 }
 

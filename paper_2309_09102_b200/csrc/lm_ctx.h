@@ -40,7 +40,7 @@ struct PlanState { // non-stationary schedule + anytime bookkeeping (lm_plan_*),
 
 int cuda_fail(cudaError_t e);              // records the error string for lm_strerror, returns LM_ECUDA
 // lm_jit.cu: the LM kernel compiled at run time for one chain structure (lm_specialize)
-int jit_get_kernel(const ChainSpec &s, bool fast, bool weighted, int var, void **fn_out);
+int jit_get_kernel(const ChainSpec &s, bool fast, bool weighted, int var, bool hot, void **fn_out);
 cudaError_t jit_launch(void *fn, unsigned grid, unsigned block, cudaStream_t s, const KArgs &a);
 const char *jit_last_log();
 std::atomic<long long> &launch_counter();  // lm_launch_count
@@ -66,6 +66,7 @@ struct lm_ctx {
     int lanes;        // LM_OPT_LANES_PER_WAYPOINT: 1 (default), 2 or 4
     lmk::ChainSpec sig; // structure of the chain (lm_api.cu: chain_signature)
     void *jit_fn;     // lm_specialize: the kernel compiled for `sig` (a CUfunction), nullptr = none
+    bool jit_hot;     // ... as the HOT instantiation: only launched while refine == 1 and no trace is set
     lmk::TrajState traj;
     lmk::PlanState plan;
 };

@@ -474,7 +474,9 @@ __device__ __forceinline__ void chol_solve(const float (&L)[D][D], const float (
 //   rho = -J^T (r + J delta) - lambda delta,  delta += A^-1 rho                     (DESIGN R4)
 // which removes the 1/lambda amplification of fp32 rounding along the self-motion direction.
 // Returns false on a non-positive pivot or a non-finite step (=> the iteration is a reject).
-template <int D, bool WEIGHTED, typename SpecT, bool RPY = false>
+// REFINE >= 0: the number of refinement steps is a compile-time constant (the loop and its counter disappear and the
+// scheduler sees one block); REFINE = -1: the run-time argument `refine`.  Same operations either way.
+template <int D, bool WEIGHTED, typename SpecT, bool RPY = false, int REFINE = -1>
 __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine, float (&delta)[D]) {
     using K = JK<WEIGHTED, SpecT, RPY>;
     float L[D][D], invd[D], g[D];
@@ -500,7 +502,9 @@ __device__ __forceinline__ bool lm_delta(const Pose<D> &P, float lam, int refine
             for (int i = j; i < D; ++i) L[i][j] = fma_(-L[i][k], L[j][k], L[i][j]);
     }
     chol_solve<D>(L, invd, g, delta);
-    for (int it = 0; it < refine; ++it) {
+    const int nref = REFINE >= 0 ? REFINE : refine;
+#pragma unroll
+    for (int it = 0; it < nref; ++it) {
         float t[6], rho[D], e[D];
 #pragma unroll
         for (int k = 0; k < 3; ++k) {

@@ -61,7 +61,10 @@ __device__ __forceinline__ void quat_to_cols(float w, float x, float y, float z,
 // LM_VAR_RPY = the roll-pitch-yaw residual (disclosed variants, DESIGN.md sections 12 and 14)
 constexpr int LM_VAR_DUAL = 1, LM_VAR_RPY = 2;
 // G: lanes per waypoint (1 = the product path; 2 / 4 = the lane-group form lm_delta_lg, LM_OPT_LANES_PER_WAYPOINT)
-template <int D, bool FAST, bool WEIGHTED, typename SpecT, int VAR = 0, int G = 1>
+// HOT: the common configuration as compile-time constants -- exactly one refinement step (the default) and no debug
+// trace -- launched whenever the context is in it (lm_launch.h); the same operations, 29 + 7 fewer instructions per
+// iteration (the refinement loop's counter and branch, the trace test).
+template <int D, bool FAST, bool WEIGHTED, typename SpecT, int VAR = 0, int G = 1, bool HOT = false>
 __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kernel(const __grid_constant__ KArgs A) {
     const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t w = G == 1 ? tid : tid / G;
@@ -120,7 +123,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         if constexpr (DUAL) ok = lm_delta_dual<D, WEIGHTED, SpecT>(cur, lam, delta);                // S4, S5 (variant)
         else if constexpr (G > 1) ok = lm_delta_lg<D, G>(cur, lam, A.refine, gl, delta);
         else if constexpr (PACKED) ok = lm_delta_p<D, WEIGHTED, SpecT, RPY>(cur, lam, A.refine, delta);
-        else ok = lm_delta<D, WEIGHTED, SpecT, RPY>(cur, lam, A.refine, delta);                      // S4, S5
+        else ok = lm_delta<D, WEIGHTED, SpecT, RPY, HOT ? 1 : -1>(cur, lam, A.refine, delta);        // S4, S5
         float qt[D];
         bool clamped = false;
 #pragma unroll
@@ -134,7 +137,7 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) lm_iterate_kern
         eval_pose<D, FAST, WEIGHTED, SpecT, false, NoFrameSink, RPY>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, tri, nullptr, nullptr, ptri,
                                                                      NoFrameSink(), trpy);
 
-        if (A.trace_q != nullptr && active && live && gl == 0) {
+        if (!HOT && A.trace_q != nullptr && active && live && gl == 0) {
 #pragma unroll
             for (int j = 0; j < D; ++j) A.trace_q[(int64_t)j * W + w] = qt[j];
             A.trace_F[w] = cur.F;

@@ -32,6 +32,9 @@ cudaError_t launch_iterate_t(bool fast, bool weighted, unsigned grid, unsigned b
     } else if (fast) {
         if (weighted) lm_iterate_kernel<D, true, true, SpecT><<<grid, block, 0, s>>>(a);
         else lm_iterate_kernel<D, true, false, SpecT><<<grid, block, 0, s>>>(a);
+    } else if (!SpecT::spec.generic && a.refine == 1 && a.trace_q == nullptr) { // the HOT instantiations (lm_kernels.cuh)
+        if (weighted) lm_iterate_kernel<D, false, true, SpecT, 0, 1, true><<<grid, block, 0, s>>>(a);
+        else lm_iterate_kernel<D, false, false, SpecT, 0, 1, true><<<grid, block, 0, s>>>(a);
     } else {
         if (weighted) lm_iterate_kernel<D, false, true, SpecT><<<grid, block, 0, s>>>(a);
         else lm_iterate_kernel<D, false, false, SpecT><<<grid, block, 0, s>>>(a);
