@@ -865,32 +865,10 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
     }
     // "a trial point of this trajectory was clamped": integer atomic (order-free), skipped once the bit is seen set
     if (!INIT && clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
-    float fc = 0.f;
+    static_assert(!COLL, "with collision rows the cost is evaluated by tl_cost_window_kernel");
+    const float fc = 0.f;
     Pose<D> P;
-    if (COLL) {
-        CapsWorld W;
-        CapsSink sink(A.caps, W);
-        sink.base();
-        eval_pose<D, FAST, WEIGHTED, SpecT, false, CapsSink>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr, nullptr, sink);
-        // the rows of this point, kept for the assembly and the refinement residual (tl_rows_fetch)
-        constexpr int RC = tl_row_comps<D>();
-        const int dst = INIT ? sel : 1 - sel;
-        float *rw = A.rows + (int64_t)dst * RC * A.nS + toff<RC>(s.wid, 0, s.lane); // component c at rw[c * 32]
-        int cnt = 0;
-        coll_rows<D, SpecT>(A.ch, A.caps, W, P, [&](const float (&g)[D], float r) {
-            fc = fma_(r, r, fc);
-            if (cnt < TL_RMAX) {
-#pragma unroll
-                for (int j = 0; j < D; ++j) rw[j * 32] = g[j];
-                rw[D * 32] = r;
-                rw += (D + 1) * 32;
-            }
-            ++cnt;
-        });
-        A.rcnt[(int64_t)dst * A.nS + s.wid * 32 + s.lane] = cnt > TL_RMAX ? TL_ROWS_OVERFLOW : cnt;
-    } else {
-        eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
-    }
+    eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
     A.cst[toff<3>(s.wid, 0, s.lane)] = P.F;
     A.cst[toff<3>(s.wid, 1, s.lane)] = fd;
     A.cst[toff<3>(s.wid, 2, s.lane)] = fc;
@@ -898,6 +876,162 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
         const int64_t W = A.B * A.n, w = s.b * A.n + s.i;
 #pragma unroll
         for (int j = 0; j < D; ++j) A.trace_q[(int64_t)j * W + w] = qt[j];
+    }
+}
+
+// ---- the same for the step WITH collision rows, lanes along the PATH.  In tile order the 32 lanes of a warp are 32
+// different trajectories at one waypoint index: their surviving pair lists are uncorrelated and the pair loops run with a
+// handful of lanes (ncu, round 2: 13.8 of 32 threads per instruction, 5800 warp-instructions per chunk).  Consecutive
+// waypoints of ONE trajectory are millimetres apart and see the same obstacles, so here a block takes a tile and a window
+// of 32 waypoints, transposes it through shared memory, and every warp walks 32 consecutive waypoints of one trajectory
+// (lane = waypoint): the lists of its lanes are nearly the same and the loops run full.  Same per-waypoint functions as
+// tl_cost_kernel, so every output has the same bits.
+//   phase 1 (lane = trajectory, coalesced): trial point of the window's 33 chunks -> shared memory (and the candidate
+//            joint buffer, the "clamped" bit), targets -> shared memory
+//   phase 2 (lane = waypoint): FK with the capsule sink, pair loops, rows -> HBM (sparse), cost terms and row count ->
+//            shared memory
+//   phase 3 (lane = trajectory, coalesced): cost terms and row counts -> HBM
+constexpr int TL_CW = 32;            // waypoints per window
+constexpr int TL_CW_THREADS = 256;   // 8 warps: 4 trajectories each in phase 2
+template <int D> __host__ __device__ constexpr size_t tl_cost_window_smem() {
+    return sizeof(float) * ((size_t)(TL_CW + 1) * D * 33 + (size_t)TL_CW * 7 * 33); // the outputs reuse the targets' columns
+}
+template <int D, bool WEIGHTED, typename SpecT, bool INIT>
+__global__ void __launch_bounds__(TL_CW_THREADS, 3) tl_cost_window_kernel(const __grid_constant__ TArgs A) {
+    extern __shared__ __align__(16) float smem_cw[];
+    float *qs = smem_cw;                                  // [TL_CW + 1][D][33]: trial point of waypoint i0 + l, joint j, trajectory b
+    float *tg = qs + (TL_CW + 1) * D * 33;                // [TL_CW][7][33]: targets
+    float *co = tg;                                       // [TL_CW][4][33]: F_pose, diff, coll, row count (as int bits) -- column b of the
+                                                          // targets is dead once the warp that owns trajectory b has read it
+    const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int nwin = (A.n + TL_CW - 1) / TL_CW;
+    const int64_t bt = blockIdx.x / nwin;
+    const int i0 = (int)(blockIdx.x - bt * nwin) * TL_CW;
+    const int n = A.n;
+    // ---- phase 1: lane = trajectory
+    {
+        const int64_t b = bt * 32 + lane;
+        const bool valid = b < A.B;
+        const uint32_t pk = valid ? A.its[b] : 0xffu;
+        const int sel = valid ? A.sel[b] : 0;
+        const bool ok = INIT ? false : (valid && A.ok[b] != 0);
+        const bool live = valid && (INIT || !((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[b] == 0)));
+        const float *qcur = A.q + (int64_t)sel * D * A.nS;
+        float *qcand = A.q + (int64_t)(1 - sel) * D * A.nS;
+        bool clamped = false;
+        for (int l = wp; l <= TL_CW; l += nw) {
+            const int i = i0 + l;
+            if (i >= n) continue;
+            const int64_t wid = bt * n + i;
+#pragma unroll
+            for (int j = 0; j < D; ++j) {
+                const float qv = qcur[toff<D>(wid, j, lane)];
+                float c = qv;
+                if (!INIT) {
+                    const float t = ok ? add(qv, A.delta[toff<D>(wid, j, lane)]) : qv;
+                    c = fminf(fmaxf(t, A.ch.lo[j]), A.ch.hi[j]);
+                    if (l < TL_CW) {
+                        clamped = clamped || (c != t);
+                        if (live) qcand[toff<D>(wid, j, lane)] = c;
+                    }
+                }
+                qs[(l * D + j) * 33 + lane] = c;
+            }
+            if (l < TL_CW) {
+                if (A.shared_targets) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) tg[(l * 7 + c) * 33 + lane] = __ldg(A.tp + (int64_t)c * n + i);
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) tg[(l * 7 + 3 + c) * 33 + lane] = __ldg(A.tq + (int64_t)c * n + i);
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) tg[(l * 7 + c) * 33 + lane] = __ldg(A.tp + toff<3>(wid, c, lane));
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) tg[(l * 7 + 3 + c) * 33 + lane] = __ldg(A.tq + toff<4>(wid, c, lane));
+                }
+            }
+        }
+        // "a trial point of this trajectory was clamped": integer atomic (order-free), skipped once the bit is seen set
+        if (!INIT && live && clamped && !((__ldcg(A.its + b) >> 8) & 32u)) atomicOr(A.its + b, 32u << 8);
+    }
+    __syncthreads();
+    // ---- phase 2: lane = waypoint i0 + lane of trajectory bb (warp-uniform)
+    for (int tb = wp; tb < 32; tb += nw) {
+        const int64_t bb = bt * 32 + tb;
+        if (bb >= A.B) break;
+        const uint32_t pk = A.its[bb];
+        if (!INIT && ((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[bb] == 0))) continue;
+        const int sel = A.sel[bb];
+        const int i = i0 + lane;
+        const bool have = i < n;
+        const int lc = have ? lane : 0; // lanes beyond the end of the path shadow the window's first waypoint, never store
+        float qt[D], qn[D], fd = 0.f;
+#pragma unroll
+        for (int j = 0; j < D; ++j) {
+            qt[j] = qs[(lc * D + j) * 33 + tb];
+            qn[j] = (have && i + 1 < n) ? qs[((lc + 1) * D + j) * 33 + tb] : 0.f;
+            if (have && i + 1 < n) {
+                const float t = sub(qn[j], qt[j]);
+                fd = fma_(t, t, fd);
+            }
+        }
+        const float pt[3] = {tg[(lc * 7 + 0) * 33 + tb], tg[(lc * 7 + 1) * 33 + tb], tg[(lc * 7 + 2) * 33 + tb]};
+        float Rt[3][3];
+        quat_to_cols(tg[(lc * 7 + 3) * 33 + tb], tg[(lc * 7 + 4) * 33 + tb], tg[(lc * 7 + 5) * 33 + tb], tg[(lc * 7 + 6) * 33 + tb], Rt);
+        Pose<D> P;
+        CapsWorld W;
+        CapsSink sink(A.caps, W);
+        sink.base();
+        eval_pose<D, false, WEIGHTED, SpecT, false, CapsSink>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr, nullptr, sink);
+        // the rows of this point, kept for the assembly and the refinement residual (tl_rows_fetch)
+        constexpr int RC = tl_row_comps<D>();
+        const int dst = INIT ? sel : 1 - sel;
+        const int64_t wid = bt * n + (have ? i : i0);
+        float *rw = A.rows + (int64_t)dst * RC * A.nS + toff<RC>(wid, 0, tb); // component c at rw[c * 32]
+        int cnt = 0;
+        float fc = 0.f;
+        coll_rows<D, SpecT>(A.ch, A.caps, W, P, [&](const float (&g)[D], float r) {
+            fc = fma_(r, r, fc);
+            if (cnt < TL_RMAX && have) {
+#pragma unroll
+                for (int j = 0; j < D; ++j) rw[j * 32] = g[j];
+                rw[D * 32] = r;
+                rw += (D + 1) * 32;
+            }
+            ++cnt;
+        });
+        __syncwarp(); // every lane of this warp has read its target from column tb: the column may be overwritten
+        if (have) {
+            co[(lane * 4 + 0) * 33 + tb] = P.F;
+            co[(lane * 4 + 1) * 33 + tb] = fd;
+            co[(lane * 4 + 2) * 33 + tb] = fc;
+            co[(lane * 4 + 3) * 33 + tb] = __int_as_float(cnt > TL_RMAX ? TL_ROWS_OVERFLOW : cnt);
+            if (!INIT && A.trace_q != nullptr) {
+                const int64_t Wn = A.B * n, w = bb * n + i;
+#pragma unroll
+                for (int j = 0; j < D; ++j) A.trace_q[(int64_t)j * Wn + w] = qt[j];
+            }
+        }
+    }
+    __syncthreads();
+    // ---- phase 3: lane = trajectory
+    {
+        const int64_t b = bt * 32 + lane;
+        const bool valid = b < A.B;
+        const uint32_t pk = valid ? A.its[b] : 0xffu;
+        const bool live = valid && (INIT || !((pk & 0xffu) >= (uint32_t)A.max_total || (A.gate != nullptr && A.gate[b] == 0)));
+        const int sel = valid ? A.sel[b] : 0;
+        const int dst = INIT ? sel : 1 - sel;
+        if (live) {
+            for (int l = wp; l < TL_CW; l += nw) {
+                const int i = i0 + l;
+                if (i >= n) break;
+                const int64_t wid = bt * n + i;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) A.cst[toff<3>(wid, c, lane)] = co[(l * 4 + c) * 33 + lane];
+                A.rcnt[(int64_t)dst * A.nS + wid * 32 + lane] = __float_as_int(co[(l * 4 + 3) * 33 + lane]);
+            }
+        }
     }
 }
 

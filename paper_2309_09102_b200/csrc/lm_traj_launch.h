@@ -42,8 +42,17 @@ cudaError_t launch_traj_pose_t(int which, bool weighted, unsigned grid, unsigned
         if (weighted) { if (coll) { CALL(true, true); } else { CALL(true, false); } }   \
         else { if (coll) { CALL(false, true); } else { CALL(false, false); } }          \
     } while (0)
-#define LM_TL_COST_INIT(W, C) tl_cost_kernel<D, false, W, SpecT, C, true><<<grid, block, 0, s>>>(a)
-#define LM_TL_COST(W, C) tl_cost_kernel<D, false, W, SpecT, C, false><<<grid, block, 0, s>>>(a)
+    // with collision rows: the window kernel (lanes along the path); its transposition buffers need more than 48 KB
+    const unsigned wgrid = (unsigned)(a.Bt * ((a.n + TL_CW - 1) / TL_CW));
+#define LM_TL_COST_WINDOW(W, I)                                                                                                    \
+    do {                                                                                                                           \
+        cudaError_t e_ = cudaFuncSetAttribute(tl_cost_window_kernel<D, W, SpecT, I>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+                                              (int)tl_cost_window_smem<D>());                                                      \
+        if (e_ != cudaSuccess) return e_;                                                                                          \
+        tl_cost_window_kernel<D, W, SpecT, I><<<wgrid, TL_CW_THREADS, tl_cost_window_smem<D>(), s>>>(a);                           \
+    } while (0)
+#define LM_TL_COST_INIT(W, C) do { if (C) LM_TL_COST_WINDOW(W, true); else tl_cost_kernel<D, false, W, SpecT, false, true><<<grid, block, 0, s>>>(a); } while (0)
+#define LM_TL_COST(W, C) do { if (C) LM_TL_COST_WINDOW(W, false); else tl_cost_kernel<D, false, W, SpecT, false, false><<<grid, block, 0, s>>>(a); } while (0)
 #define LM_TL_ASSEMBLE(W, C) tl_assemble_kernel<D, false, W, SpecT, C><<<grid, block, 0, s>>>(a)
 #define LM_TL_RHO(W, C) tl_rho_kernel<D, false, W, SpecT, C><<<grid, block, 0, s>>>(a)
     switch (which) {
@@ -63,6 +72,7 @@ cudaError_t launch_traj_pose_t(int which, bool weighted, unsigned grid, unsigned
 #undef LM_TL_DISPATCH
 #undef LM_TL_COST_INIT
 #undef LM_TL_COST
+#undef LM_TL_COST_WINDOW
 #undef LM_TL_ASSEMBLE
 #undef LM_TL_RHO
     return cudaGetLastError();
