@@ -564,6 +564,7 @@ def time_correlated_tiles(lm, torch, w, wl_, stream, iters: int, reps: int):
     s.traj_attach(lm.lm_traj_default_params(w_pose=1.0, w_diff=0.3))
     s.traj_set_capsules(wl_.panda_capsules(), 1.0, 0.05)
     s.traj_set_obstacles(wl_.panda_scene(), 1.0, 0.05)
+    s.traj_set_cost_lanes(1)  # the caller knows its tiles are candidates of one path: a warp takes one waypoint of 32 trajectories
     ts = []
     with torch.cuda.stream(stream):
         for i in range(reps + 1):

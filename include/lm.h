@@ -204,6 +204,12 @@ int lm_set_trace(lm_ctx *ctx, float *trial_q, float *trial_F);
  * per-waypoint kernels through HBM, 0 (default) = 1 when the batch has enough tiles of 32 trajectories to pay for it,
  * else 2.  With collision rows the step always takes path 2.  Both paths return the same bits. */
 #define LM_OPT_TRAJ_FUSED 4
+/* LM_OPT_TRAJ_COST_LANES (after lm_traj_attach; only matters with collision rows): which waypoints share a warp when the
+ * trial cost and its collision rows are evaluated.  The pair loops run well when the 32 lanes of a warp see the same
+ * obstacles.  2 = 32 consecutive waypoints of ONE trajectory (always alike; costs a transposition through shared memory),
+ * 1 = the same waypoint of 32 trajectories of a tile (alike only if those trajectories are candidates for one path -- the
+ * paper's use of the optimiser on K plans of one problem), 0 (default) = 1 with shared_targets, else 2.  Same bits. */
+#define LM_OPT_TRAJ_COST_LANES 5
 int lm_set_option(lm_ctx *ctx, int32_t option, int32_t value);
 
 /* Name of the LM kernel variant this context launches: "panda7", "rand8" (compile-time chain

@@ -428,6 +428,10 @@ int lm_set_option(lm_ctx *c, int32_t option, int32_t value) {
         if (value != 0 && c->lanes > 1) return LM_EINVAL;
         c->use_generic = value != 0;
         return LM_OK;
+    case LM_OPT_TRAJ_COST_LANES:
+        if (value < 0 || value > 2 || !c->traj.attached) return LM_EINVAL;
+        c->traj.cost_lanes = value;
+        return LM_OK;
     case LM_OPT_TRAJ_FUSED:
         if (value < 0 || value > 2 || !c->traj.attached) return LM_EINVAL;
         c->traj.fused_mode = value;

@@ -19,6 +19,7 @@ struct TrajState { // trajectory-level LM (lm_traj_*), bound by lm_traj_attach
     TArgs args{};
     float lambda0 = 1e-3f;
     int refine = 1;
+    int cost_lanes = 0; // LM_OPT_TRAJ_COST_LANES: 0 = by shared_targets, 1 = lanes are trajectories, 2 = lanes are waypoints
     int fused_mode = 0; // LM_OPT_TRAJ_FUSED: 0 = by tile count, 1 = fused solve kernels, 2 = unfused (HBM) path
     size_t bytes = 0;
     char *ws = nullptr;

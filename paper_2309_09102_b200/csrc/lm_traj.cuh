@@ -38,6 +38,7 @@ struct TArgs {
     int32_t n;
     int32_t shared_targets;
     int32_t max_total;             // iteration cap per trajectory (mask width)
+    int32_t cost_by_waypoints;     // collision rows: 1 = tl_cost_window_kernel (lanes along the path), 0 = tl_cost_kernel (tile order)
     const float *tp, *tq;          // targets: tile order [3], [4] comps; when shared: plain [3][n], [4][n]
     float *tp_w, *tq_w;            // the same arrays, writable (pack kernel)
     float *q;                      // [2] x D comps     current / candidate joint values (`sel` says which is current)
@@ -865,10 +866,32 @@ __global__ void __launch_bounds__(LM_MAX_THREADS, LM_MIN_BLOCKS) tl_cost_kernel(
     }
     // "a trial point of this trajectory was clamped": integer atomic (order-free), skipped once the bit is seen set
     if (!INIT && clamped && !((__ldcg(A.its + s.b) >> 8) & 32u)) atomicOr(A.its + s.b, 32u << 8);
-    static_assert(!COLL, "with collision rows the cost is evaluated by tl_cost_window_kernel");
-    const float fc = 0.f;
+    float fc = 0.f;
     Pose<D> P;
-    eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+    if (COLL) { // lanes = trajectories (tile order); tl_cost_window_kernel is the same with lanes = consecutive waypoints
+        CapsWorld W;
+        CapsSink sink(A.caps, W);
+        sink.base();
+        eval_pose<D, FAST, WEIGHTED, SpecT, false, CapsSink>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr, nullptr, sink);
+        // the rows of this point, kept for the assembly and the refinement residual (tl_rows_fetch)
+        constexpr int RC = tl_row_comps<D>();
+        const int dst = INIT ? sel : 1 - sel;
+        float *rw = A.rows + (int64_t)dst * RC * A.nS + toff<RC>(s.wid, 0, s.lane); // component c at rw[c * 32]
+        int cnt = 0;
+        coll_rows<D, SpecT>(A.ch, A.caps, W, P, [&](const float (&g)[D], float r) {
+            fc = fma_(r, r, fc);
+            if (cnt < TL_RMAX) {
+#pragma unroll
+                for (int j = 0; j < D; ++j) rw[j * 32] = g[j];
+                rw[D * 32] = r;
+                rw += (D + 1) * 32;
+            }
+            ++cnt;
+        });
+        A.rcnt[(int64_t)dst * A.nS + s.wid * 32 + s.lane] = cnt > TL_RMAX ? TL_ROWS_OVERFLOW : cnt;
+    } else {
+        eval_pose<D, FAST, WEIGHTED, SpecT, false>(A.ch, qt, pt, Rt, A.w_pos, A.w_rot, P, nullptr, nullptr);
+    }
     A.cst[toff<3>(s.wid, 0, s.lane)] = P.F;
     A.cst[toff<3>(s.wid, 1, s.lane)] = fd;
     A.cst[toff<3>(s.wid, 2, s.lane)] = fc;

@@ -51,8 +51,8 @@ cudaError_t launch_traj_pose_t(int which, bool weighted, unsigned grid, unsigned
         if (e_ != cudaSuccess) return e_;                                                                                          \
         tl_cost_window_kernel<D, W, SpecT, I><<<wgrid, TL_CW_THREADS, tl_cost_window_smem<D>(), s>>>(a);                           \
     } while (0)
-#define LM_TL_COST_INIT(W, C) do { if (C) LM_TL_COST_WINDOW(W, true); else tl_cost_kernel<D, false, W, SpecT, false, true><<<grid, block, 0, s>>>(a); } while (0)
-#define LM_TL_COST(W, C) do { if (C) LM_TL_COST_WINDOW(W, false); else tl_cost_kernel<D, false, W, SpecT, false, false><<<grid, block, 0, s>>>(a); } while (0)
+#define LM_TL_COST_INIT(W, C) do { if (C && a.cost_by_waypoints) LM_TL_COST_WINDOW(W, true); else tl_cost_kernel<D, false, W, SpecT, C, true><<<grid, block, 0, s>>>(a); } while (0)
+#define LM_TL_COST(W, C) do { if (C && a.cost_by_waypoints) LM_TL_COST_WINDOW(W, false); else tl_cost_kernel<D, false, W, SpecT, C, false><<<grid, block, 0, s>>>(a); } while (0)
 #define LM_TL_ASSEMBLE(W, C) tl_assemble_kernel<D, false, W, SpecT, C><<<grid, block, 0, s>>>(a)
 #define LM_TL_RHO(W, C) tl_rho_kernel<D, false, W, SpecT, C><<<grid, block, 0, s>>>(a)
     switch (which) {

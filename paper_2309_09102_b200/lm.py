@@ -22,7 +22,7 @@ LM_MAX_DOF = 8
 LM_MAX_ITERS = 64
 LM_OK, LM_EINVAL, LM_ENOMEM, LM_ECUDA = 0, -1, -2, -3
 LM_MEM_DEVICE, LM_MEM_HOST = 0, 1
-LM_OPT_BLOCK_THREADS, LM_OPT_GENERIC_KERNEL, LM_OPT_LANES_PER_WAYPOINT, LM_OPT_TRAJ_FUSED = 1, 2, 3, 4
+LM_OPT_BLOCK_THREADS, LM_OPT_GENERIC_KERNEL, LM_OPT_LANES_PER_WAYPOINT, LM_OPT_TRAJ_FUSED, LM_OPT_TRAJ_COST_LANES = 1, 2, 3, 4, 5
 LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1, 2, 4, 8, 16
 
 # every symbol include/lm.h declares (checked by tests/test_abi.py)
@@ -594,6 +594,10 @@ class Solver:
     def traj_set_fused(self, mode: int) -> None:
         """LM_OPT_TRAJ_FUSED: 0 = chosen by tile count, 1 = fused solve kernels, 2 = per-waypoint kernels through HBM."""
         lm_set_option(self._ctx, LM_OPT_TRAJ_FUSED, int(mode))
+
+    def traj_set_cost_lanes(self, mode: int) -> None:
+        """LM_OPT_TRAJ_COST_LANES: 0 = by shared_targets, 1 = a warp takes one waypoint of 32 trajectories, 2 = 32 waypoints of one."""
+        lm_set_option(self._ctx, LM_OPT_TRAJ_COST_LANES, int(mode))
 
     def traj_set_capsules(self, model, w_coll: float = 1.0, d_safe: float = 0.05) -> None:
         lm_traj_set_capsules(self._ctx, model, w_coll, d_safe)

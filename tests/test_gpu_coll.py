@@ -362,3 +362,33 @@ def test_full_size_sampled_with_all_rows():
     margin = clear & (np.abs(st.F_before - st.F_trial) > 1e-3 * st.F_before)
     acc = (g["mask"][pick] & np.uint64(1)).astype(bool)
     assert np.array_equal(acc[margin], (st.accepted == 1)[margin])
+
+
+# ------------------------------------------------------------------ LM_OPT_TRAJ_COST_LANES
+
+@pytest.mark.parametrize("shape", [(37, 45), (3, 1), (2, 70), (65, 33)])
+def test_cost_lane_layouts_return_the_same_bits(shape):
+    """The trial cost with collision rows is evaluated with a warp's lanes along the path (tl_cost_window_kernel: windows
+    of 32 waypoints transposed through shared memory) or across the trajectories of a tile (tl_cost_kernel): the same
+    per-waypoint functions, so costs, kept rows (through the next step), decisions and joints are bit-identical -- on
+    ragged tiles, windows that end inside the path, one-waypoint trajectories, with the schedule's gate and trace on."""
+    from paper_2309_09102_b200 import lm
+    ch, model, scene = wl.panda_chain(), wl.panda_capsules(), wl.panda_scene()
+    B, n = shape
+    w = folded_problem(ch, model, B, n, 91, PANDA_FOLDED)
+    outs = []
+    for mode in (1, 2):
+        s = lm.Solver(ch, B, n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0))
+        s.traj_attach(lm.lm_traj_default_params(w_pose=0.5, w_diff=0.3))
+        s.traj_set_capsules(model, 1.0, 0.25)
+        s.traj_set_obstacles(scene, 1.0, 0.25)
+        s.traj_set_cost_lanes(mode)
+        s.traj_enable_trace()
+        s.traj_run(3)
+        outs.append((s.traj_fetch(), s.fetch()))
+        s.close()
+    (g1, f1), (g2, f2) = outs
+    assert (g1["cost_coll"] > 0).any()
+    for k in ("cost", "cost_pose", "cost_diff", "cost_coll", "lam", "mask", "iters", "status", "trial_q"):
+        assert np.array_equal(g1[k], g2[k], equal_nan=g1[k].dtype.kind == "f"), k
+    assert np.array_equal(f1["q"], f2["q"])
