@@ -377,8 +377,8 @@ def run_gpu(args) -> None:
         extra["schedule_C2"] = time_plan(lm, torch, wl, fk, device, stream)
         # the global discrete search over K candidates of one path (NEXT-4 iii)
         extra["search_K175_n300"] = time_search(lm, torch, wl, fk, device, stream)
-    roofline["peak_measured_fma_rrr"] = lm.lm_fp32_peak_form(lm.LM_FMA_FORM_RRR, int(stream.cuda_stream))
-    roofline["frac_of_measured_fma_rrr"] = achieved_tf / roofline["peak_measured_fma_rrr"]
+    # (the rate of FFMAs with three new register operands is a calibration point of the register-file read model, not a
+    # roofline: it is reported with the other operand forms under fma_operand_forms_tflops)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms_all / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
