@@ -138,13 +138,20 @@ def test_results_do_not_depend_on_timing():
         t = s.traj_fetch()
         return s.fetch()["q"].copy(), t["trial_q"].copy(), t["cost"].copy()
 
-    quiet = one_traj()
-    for rep in range(25):
-        heavy.reset()
-        heavy.run(30 + rep)                      # asynchronous, on its own stream: varies what shares the SMs
-        got = one_traj()
-        for a, b in zip(quiet, got):
-            assert np.array_equal(a, b), f"trajectory-level step differs in repetition {rep}"
+    quiet = None
+    for mode in (2, 1):  # the copy-fed rings (unfused) and the rings the producer warps compute into (fused, round 2)
+        s.traj_set_fused(mode)
+        first = one_traj()
+        if quiet is None:
+            quiet = first
+        for a, b in zip(quiet, first):
+            assert np.array_equal(a, b), "fused and unfused trajectory-level step differ"
+        for rep in range(25):
+            heavy.reset()
+            heavy.run(30 + rep)                  # asynchronous, on its own stream: varies what shares the SMs
+            got = one_traj()
+            for a, b in zip(quiet, got):
+                assert np.array_equal(a, b), f"trajectory-level step differs in repetition {rep} (fused mode {mode})"
     s.close()
     for K, n in ((3, 40), (9, 40), (24, 60), (175, 80), (600, 180)):
         q = wl.search_candidates(ch, K, n, 730 + K, limit_frac=0.02)
