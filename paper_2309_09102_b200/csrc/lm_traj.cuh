@@ -385,14 +385,25 @@ __device__ __forceinline__ void tl_sum_cost(const TArgs &A, float (*part)[3][32]
     const int i0 = wp * seg, i1 = min(A.n, i0 + seg);
     float sm[3] = {0.f, 0.f, 0.f}, cm[3] = {0.f, 0.f, 0.f};
     int i = i0;
-    for (; i + 8 <= i1; i += 8) { // 24 independent loads in flight, then the sums in order
-        float a[8][3];
+    for (; i + 16 <= i1; i += 16) { // 48 independent loads in flight, then the sums in order
+        float a[16][3];
 #pragma unroll
-        for (int u = 0; u < 8; ++u)
+        for (int u = 0; u < 16; ++u)
 #pragma unroll
             for (int c = 0; c < 3; ++c) a[u][c] = cp[toff<3>(w0 + i + u, c, lane)];
 #pragma unroll
-        for (int u = 0; u < 8; ++u)
+        for (int u = 0; u < 16; ++u)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) kahan_add(sm[c], cm[c], a[u][c]);
+    }
+    for (; i + 4 <= i1; i += 4) {
+        float a[4][3];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) a[u][c] = cp[toff<3>(w0 + i + u, c, lane)];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
 #pragma unroll
             for (int c = 0; c < 3; ++c) kahan_add(sm[c], cm[c], a[u][c]);
     }
