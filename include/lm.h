@@ -46,7 +46,8 @@ typedef enum {
     LM_OK = 0,
     LM_EINVAL = -1, /* null pointer, dof outside 1..8, B*n == 0, misaligned pointer, lo > hi, max_iters > 64 ... */
     LM_ENOMEM = -2, /* workspace smaller than lm_workspace_bytes() */
-    LM_ECUDA = -3   /* a CUDA runtime call failed; lm_strerror() gives cudaGetErrorString */
+    LM_ECUDA = -3,  /* a CUDA runtime call failed; lm_strerror() gives cudaGetErrorString */
+    LM_ECAPACITY = -4 /* lm_search_static only: (dof, K, n) needs more scratch than the fixed LM_SEARCH_STATIC_BYTES */
 } lm_status;
 
 typedef struct lm_ctx lm_ctx; /* opaque, library-owned (host memory); lm_free() releases it */
@@ -417,6 +418,46 @@ int lm_search_default_params(lm_search_params *out);
  * use_clearance without a capsule model; LM_ENOMEM: workspace too small. */
 int lm_search(lm_ctx *ctx, const lm_search_params *params, void *workspace, size_t workspace_bytes,
               int32_t *choice_out, float *xi_out, float *result_out);
+
+/* ---- The same search for callers that cannot allocate device memory ------------------------------------------
+ * Who this is for.  lm_search, like every other call here, works in a device workspace the caller allocates.  Some
+ * users of a planner cannot do that at the point where they need the search:
+ *   - a re-planning loop with a deadline (the paper's planner is "anytime": it must hand back a trajectory inside a
+ *     time budget).  cudaMalloc / cudaFree take driver-wide locks, can wait for all work on the device
+ *     and have no bound on how long they take, so such a loop may launch kernels but must not allocate;
+ *   - a process in which something else owns the GPU's memory -- a simulator or a learning framework whose caching
+ *     pool has claimed nearly everything, or a deployment whose memory budget is fixed at start-up -- so a fresh
+ *     cudaMalloc fails or is forbidden by policy, and the owner's pool is not reachable from C.
+ * For them the scratch of the search is a fixed array inside the library image: LM_SEARCH_STATIC_BYTES (16 MiB) of
+ * device memory that EVERY GPU on which this library is loaded holds from load until the process exits, used or not.
+ * That is the price, and the reason the limit is modest.
+ *
+ * lm_search_static allocates nothing (no cudaMalloc, cudaFree, host allocation or allocating library call) and needs
+ * no lm_ctx.  The caller passes only inputs and outputs:
+ *   chain       HOST; only dof, joint_type, q_lo, q_hi are read (dh and tool may be anything); the fp64 limits become
+ *               fp32 exactly as in lm_init (rounded into the interval).
+ *   K, n        candidates and timesteps.
+ *   q           DEVICE memory of the current device, [dof][K * n] fp32, element (j, k * n + i) = joint j of candidate
+ *               k at timestep i -- the layout of lm_problem.seeds.  Read only.
+ *   params      as for lm_search; use_clearance must be 0 (the clearance needs a capsule model, i.e. a context).
+ *   cuda_stream a stream of the current device (NULL = the default stream).
+ *   choice_out [n], xi_out [dof][n], result_out [2]: device or host, each nullable; same meaning as in lm_search, and
+ *               bit for bit the values lm_search returns for the same q, limits and params.
+ * Limit: the intermediate arrays of (dof, K, n) -- lm_search_workspace_bytes(dof, K, n), dominated by the
+ * (n - 1) * K * Kpad edge costs -- must fit in LM_SEARCH_STATIC_BYTES: for 7 joints e.g. K = 175 up to n = 124,
+ * K = 64 up to n = 170, K = 32 up to n = 339.  lm_search_static_fits() answers for a given size (1 / 0); a size that does not fit
+ * returns LM_ECAPACITY ("exceeds the fixed scratch ...") and launches nothing.  Other errors: LM_EINVAL (null pointer,
+ * dof / K / n out of range, lo > hi, q not device memory of the current device, use_clearance != 0), LM_ECUDA.
+ * Set-up: the first call on each device looks up the device address of the array (cudaGetSymbolAddress, with that
+ * device current) and remembers it; make that first call during start-up, before any stream capture begins.
+ * Sharing: all calls on a device, from every thread and every stream, use the SAME array, and it keeps whatever the
+ * previous call left in it.  Nothing in it has to start at zero -- each call overwrites every element it later reads --
+ * but two calls whose kernels overlap on the GPU (different streams, or threads calling concurrently) race on it and
+ * return garbage: serialise them.  The call synchronises cuda_stream before it returns, as lm_search does. */
+#define LM_SEARCH_STATIC_BYTES (16u << 20)
+int lm_search_static_fits(int32_t dof, int64_t K, int64_t n);
+int lm_search_static(const lm_chain *chain, int64_t K, int64_t n, const float *q, const lm_search_params *params,
+                     void *cuda_stream, int32_t *choice_out, float *xi_out, float *result_out);
 
 /* Measure the FP32 FMA throughput of the current device with an FMA-only micro-kernel (16 independent
  * chains per thread, best of 5 timed launches, CUDA events on `cuda_stream`); blocks the host.

@@ -849,6 +849,7 @@ const char *lm_strerror(int code) {
     case LM_EINVAL: return "invalid argument";
     case LM_ENOMEM: return "workspace too small or out of host memory";
     case LM_ECUDA: return g_cuda_err;
+    case LM_ECAPACITY: return "problem exceeds the fixed scratch of lm_search_static (LM_SEARCH_STATIC_BYTES); use lm_search with a caller-allocated workspace";
     default: return "unknown lm_status";
     }
 }

@@ -11,7 +11,9 @@
 #include "lm_ctx.h"
 
 #include <cooperative_groups.h>
+#include <cmath>
 #include <cstring>
+#include <mutex>
 
 namespace cg = cooperative_groups;
 
@@ -405,6 +407,161 @@ int lm_search(lm_ctx *c, const lm_search_params *p, void *workspace, size_t byte
     if (xi_out) LM_CUDA(cudaMemcpyAsync(xi_out, a.xi, 4 * (size_t)c->n * d, cudaMemcpyDefault, c->stream));
     if (result_out) LM_CUDA(cudaMemcpyAsync(result_out, a.result, 8, cudaMemcpyDefault, c->stream));
     LM_CUDA(cudaStreamSynchronize(c->stream));
+    return LM_OK;
+}
+
+} // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// lm_search_static: the same two kernels, for callers that cannot obtain device memory at all (include/lm.h has the
+// user-facing description).  Every intermediate array of the search -- edge costs, penalties, predecessors, the chosen
+// path -- lives in ONE fixed array that is part of the library image, so the call path below contains no cudaMalloc,
+// no cudaFree, no host allocation and no library routine that allocates.
+//
+// g_search_static is a device variable.  In HOST code its name is only a handle for the runtime (a host-side shadow),
+// not an address the GPU can use: the device address is looked up with cudaGetSymbolAddress, once per device and with
+// that device current, and it is that looked-up pointer the kernels receive.
+namespace {
+
+static __device__ __align__(256) unsigned char g_search_static[LM_SEARCH_STATIC_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+char *g_static_ptr[STATIC_MAX_DEVICES];   // device address of g_search_static on device i, nullptr = not looked up yet
+std::mutex g_static_mutex;
+
+// Device address of the static scratch on the CURRENT device; the first call on a device performs the look-up.
+int static_scratch(char **out) {
+    int dev = -1;
+    LM_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return LM_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        void *p = nullptr;
+        LM_CUDA(cudaGetSymbolAddress(&p, g_search_static));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u) != 0) return LM_EINVAL;
+        g_static_ptr[dev] = static_cast<char *>(p);
+    }
+    *out = g_static_ptr[dev];
+    return LM_OK;
+}
+
+float limit_inward(double x, bool lower) { // the fp32 limit lm_init derives from an fp64 one: never outside it
+    float f = (float)x;
+    if (lower && (double)f < x) f = nextafterf(f, INFINITY);
+    if (!lower && (double)f > x) f = nextafterf(f, -INFINITY);
+    return f;
+}
+
+} // namespace
+
+extern "C" {
+
+int lm_search_static_fits(int32_t dof, int64_t K, int64_t n) {
+    if (dof < 1 || dof > LM_MAX_DOF || K <= 0 || K > LM_SEARCH_MAX_K || n <= 0 || n > 0x7fffffff) return 0;
+    // K * KP * 4 bytes per layer >= 4 bytes: n beyond the capacity cannot fit, and the product below cannot overflow
+    if ((uint64_t)n > (uint64_t)LM_SEARCH_STATIC_BYTES) return 0;
+    return make_slayout(dof, K, n).all <= (size_t)LM_SEARCH_STATIC_BYTES ? 1 : 0;
+}
+
+int lm_search_static(const lm_chain *chain, int64_t K, int64_t n, const float *q, const lm_search_params *p,
+                     void *cuda_stream, int32_t *choice_out, float *xi_out, float *result_out) {
+    if (!chain || !q || !p) return LM_EINVAL;
+    const int d = chain->dof;
+    if (d < 1 || d > LM_MAX_DOF || !chain->joint_type || !chain->q_lo || !chain->q_hi) return LM_EINVAL;
+    if (K <= 0 || K > LM_SEARCH_MAX_K || n <= 0 || n > 0x7fffffff) return LM_EINVAL;
+    if (!(p->margin_rev >= 0.f) || !(p->margin_pris >= 0.f) || !(p->pen_limit >= 0.f) || !(p->pen_collision >= 0.f)) return LM_EINVAL;
+    if (p->use_clearance) return LM_EINVAL; // the clearance needs a capsule model, i.e. a context
+    if (!lm_search_static_fits(d, K, n)) return LM_ECAPACITY;
+    char *ws = nullptr;
+    int rc = static_scratch(&ws);
+    if (rc != LM_OK) return rc;
+    { // q must be memory of the device whose copy of the scratch the kernels are about to use
+        int dev = -1;
+        LM_CUDA(cudaGetDevice(&dev));
+        cudaPointerAttributes at{};
+        if (cudaPointerGetAttributes(&at, q) != cudaSuccess) { (void)cudaGetLastError(); return LM_EINVAL; }
+        if (!(at.type == cudaMemoryTypeManaged || (at.type == cudaMemoryTypeDevice && at.device == dev))) return LM_EINVAL;
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const SLayout L = make_slayout(d, K, n);
+    SArgs a{};
+    a.dof = d; a.n = (int32_t)n; a.K = (int32_t)K; a.W = K * n;
+    const DpShape shp = dp_shape(K);
+    a.KC = shp.KC;
+    a.KP = shp.KP;
+    for (int j = 0; j < d; ++j) {
+        if (!(chain->q_lo[j] <= chain->q_hi[j]) || chain->joint_type[j] > 1) return LM_EINVAL;
+        a.lo[j] = limit_inward(chain->q_lo[j], true);
+        a.hi[j] = limit_inward(chain->q_hi[j], false);
+        if (a.lo[j] > a.hi[j]) a.lo[j] = a.hi[j] = (float)chain->q_lo[j];
+        if (chain->joint_type[j]) a.prismatic_mask |= 1u << j;
+    }
+    a.margin_rev = p->margin_rev; a.margin_pris = p->margin_pris; a.pen_limit = p->pen_limit; a.pen_collision = p->pen_collision;
+    a.use_clear = 0;
+    a.q = q;
+    // Nothing below needs the scratch to start at zero: each of these regions is written in full by this call's own
+    // kernels (edge rows including their +inf padding, all n * K penalties, the predecessors of layers 1 .. n-1, the
+    // path, xi, the two results) before anything reads it, so what an earlier call left behind is never seen.
+    a.clear = reinterpret_cast<float *>(ws + L.clear);
+    a.edges = reinterpret_cast<float *>(ws + L.edges);
+    a.pen = reinterpret_cast<float *>(ws + L.pen);
+    a.pred = reinterpret_cast<uint16_t *>(ws + L.pred);
+    a.choice = reinterpret_cast<int32_t *>(ws + L.choice);
+    a.xi = reinterpret_cast<float *>(ws + L.xi);
+    a.result = reinterpret_cast<float *>(ws + L.result);
+    const size_t edge_smem = 2 * sizeof(float) * (size_t)d * (size_t)K;
+    size_t dp_smem = 2 * sizeof(float) * (size_t)a.KP;
+    const size_t pred_bytes = 2 * (size_t)n * ((size_t)a.KC + (size_t)K);
+    a.pred_in_smem = (dp_smem + pred_bytes + 2048 <= SMEM_OPT_IN) ? 1 : 0;
+    if (a.pred_in_smem) dp_smem += pred_bytes;
+    launch_counter().fetch_add(2);
+    {
+        int split = (int)((4 * 148 + n - 1) / n);
+        if (split > (int)K) split = (int)K;
+        if (split < 1) split = 1;
+        const dim3 grid((unsigned)n, (unsigned)split);
+#define LM_EDGE_LAUNCH(DD)                                                                                                  \
+    case DD:                                                                                                                \
+        LM_CUDA(cudaFuncSetAttribute(search_edges_kernel<DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536));         \
+        search_edges_kernel<DD><<<grid, EDGE_THREADS, edge_smem, stream>>>(a);                                              \
+        break;
+        switch (d) {
+            LM_EDGE_LAUNCH(1) LM_EDGE_LAUNCH(2) LM_EDGE_LAUNCH(3) LM_EDGE_LAUNCH(4)
+            LM_EDGE_LAUNCH(5) LM_EDGE_LAUNCH(6) LM_EDGE_LAUNCH(7) LM_EDGE_LAUNCH(8)
+            default: return LM_EINVAL;
+        }
+#undef LM_EDGE_LAUNCH
+        LM_CUDA(cudaGetLastError());
+    }
+    {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(DP_CLUSTER);
+        cfg.blockDim = dim3((unsigned)shp.threads);
+        cfg.dynamicSmemBytes = dp_smem;
+        cfg.stream = stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = DP_CLUSTER;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        const int smem_max = (int)(SMEM_OPT_IN - 2048);
+#define LM_DP_LAUNCH(GG)                                                                                                      \
+    case GG:                                                                                                                  \
+        LM_CUDA(cudaFuncSetAttribute(search_dp_kernel<GG, DP_BATCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max)); \
+        LM_CUDA(cudaLaunchKernelEx(&cfg, search_dp_kernel<GG, DP_BATCH>, a));                                                 \
+        break;
+        switch (shp.G) {
+            LM_DP_LAUNCH(1) LM_DP_LAUNCH(2) LM_DP_LAUNCH(4) LM_DP_LAUNCH(8) LM_DP_LAUNCH(16) LM_DP_LAUNCH(32)
+            default: return LM_EINVAL;
+        }
+#undef LM_DP_LAUNCH
+    }
+    if (choice_out) LM_CUDA(cudaMemcpyAsync(choice_out, a.choice, 4 * (size_t)n, cudaMemcpyDefault, stream));
+    if (xi_out) LM_CUDA(cudaMemcpyAsync(xi_out, a.xi, 4 * (size_t)n * d, cudaMemcpyDefault, stream));
+    if (result_out) LM_CUDA(cudaMemcpyAsync(result_out, a.result, 8, cudaMemcpyDefault, stream));
+    LM_CUDA(cudaStreamSynchronize(stream));
     return LM_OK;
 }
 

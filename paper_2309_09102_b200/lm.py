@@ -20,7 +20,8 @@ from .build import LIB_PATH
 
 LM_MAX_DOF = 8
 LM_MAX_ITERS = 64
-LM_OK, LM_EINVAL, LM_ENOMEM, LM_ECUDA = 0, -1, -2, -3
+LM_OK, LM_EINVAL, LM_ENOMEM, LM_ECUDA, LM_ECAPACITY = 0, -1, -2, -3, -4
+LM_SEARCH_STATIC_BYTES = 16 << 20
 LM_MEM_DEVICE, LM_MEM_HOST = 0, 1
 LM_OPT_BLOCK_THREADS, LM_OPT_GENERIC_KERNEL, LM_OPT_LANES_PER_WAYPOINT, LM_OPT_TRAJ_FUSED, LM_OPT_TRAJ_COST_LANES = 1, 2, 3, 4, 5
 LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1, 2, 4, 8, 16
@@ -33,7 +34,8 @@ SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_
            "lm_traj_fetch", "lm_traj_set_trace", "lm_traj_set_capsules", "lm_traj_set_obstacles",
            "lm_solve_host_workspace_bytes", "lm_solve_host", "lm_pipe_create", "lm_pipe_solve", "lm_pipe_destroy", "lm_specialize",
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch",
-           "lm_search_workspace_bytes", "lm_search_default_params", "lm_search")
+           "lm_search_workspace_bytes", "lm_search_default_params", "lm_search",
+           "lm_search_static_fits", "lm_search_static")
 LM_FMA_FORM_RCC, LM_FMA_FORM_RRR, LM_FMA_FORM_RRS, LM_FMA_FORM_RSS, LM_FMA_FORM_MUL, LM_FMA_FORM_PPP, LM_FMA_FORM_PSP = range(7)
 LM_SOLVER_PRIMAL, LM_SOLVER_DUAL = 0, 1
 LM_ROT_LOG, LM_ROT_RPY = 0, 1
@@ -174,6 +176,9 @@ def lib() -> C.CDLL:
         L.lm_search_workspace_bytes.restype = C.c_size_t
         L.lm_search_default_params.argtypes = [C.POINTER(LmSearchParams)]
         L.lm_search.argtypes = [C.c_void_p, C.POINTER(LmSearchParams), C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.lm_search_static_fits.argtypes = [C.c_int32, C.c_int64, C.c_int64]
+        L.lm_search_static.argtypes = [C.POINTER(LmChain), C.c_int64, C.c_int64, C.c_void_p, C.POINTER(LmSearchParams), C.c_void_p,
+                                       C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -418,6 +423,22 @@ def lm_search_default_params(**overrides) -> LmSearchParams:
 def lm_search(ctx: int, params: LmSearchParams, workspace_ptr: int, workspace_bytes: int, choice_ptr: Optional[int],
               xi_ptr: Optional[int], result_ptr: Optional[int]) -> None:
     _check(lib().lm_search(ctx, C.byref(params), workspace_ptr, workspace_bytes, choice_ptr, xi_ptr, result_ptr), "lm_search")
+
+
+def lm_search_static_fits(dof: int, K: int, n: int) -> bool:
+    return bool(lib().lm_search_static_fits(dof, K, n))
+
+
+def lm_search_static(chain, K: int, n: int, q_ptr: int, params: LmSearchParams, cuda_stream: int, choice_ptr: Optional[int],
+                     xi_ptr: Optional[int], result_ptr: Optional[int]) -> None:
+    """include/lm.h, lm_search_static: the search for callers that cannot allocate device memory (a re-planning loop
+    with a deadline, a process whose GPU memory belongs to somebody else's pool).  Its scratch is a fixed 16 MiB array
+    inside the library, shared by all calls; nothing is allocated here either: `chain` is marshalled on the host,
+    q_ptr is the caller's device array [d][K * n], the three outputs are the caller's (device or host) buffers."""
+    cstruct, keep = make_chain(chain)
+    rc = lib().lm_search_static(C.byref(cstruct), K, n, q_ptr, C.byref(params), C.c_void_p(cuda_stream), choice_ptr, xi_ptr, result_ptr)
+    del keep
+    _check(rc, "lm_search_static")
 
 
 def lm_free(ctx: int) -> None:
