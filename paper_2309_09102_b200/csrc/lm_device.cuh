@@ -129,11 +129,16 @@ struct Pose {
     float Ei[9];    // roll-pitch-yaw variant only: E(rpy)^-1 at this pose (row-major), d(rpy)/dq = E^-1 J_w
 };
 
-// w = Log(E)^vee for theta within 1e-4 of pi (rare: never reached by the documented workloads).
-// Axis from the symmetric part E_ii = c + (1 - c) a_i^2, signs from E_mi + E_im and from v.
-__device__ __forceinline__ void log_near_pi(const float (&X)[3], const float (&Y)[3], const float (&Z)[3],
-                                            const float (&Rt)[3][3], const float (&v)[3], float cth, float theta,
-                                            float (&w)[3]) {
+// w = Log(E)^vee for cos(theta) < -0.9 (theta > 154 deg: an IK seed on the wrong wrist flip; rare in the documented
+// workloads).  There v = sin(theta) a is short and carries an absolute fp32 error of ~1e-7, so the direction v / |v|
+// is off by 1e-7 / sin(theta) -- 3e-4 rad of residual at theta = pi - 1e-3, everything at theta = pi (at the switch,
+// sin(theta) = 0.44, it is 6e-7).  The symmetric part stays well conditioned: E_ii = c + (1 - c) a_i^2 and
+// E_mi + E_im = 2 (1 - c) a_m a_i with 1 - c > 1.9.
+// Largest component a_m (>= 1/sqrt 3) from the diagonal, the other two from the off-diagonal sums divided by it
+// (a square root of a small diagonal difference would lose half the digits), the overall sign from v.
+__device__ __forceinline__ void log_far(const float (&X)[3], const float (&Y)[3], const float (&Z)[3],
+                                        const float (&Rt)[3][3], const float (&v)[3], float cth, float theta,
+                                        float (&w)[3]) {
     float E[3][3];
 #pragma unroll
     for (int i = 0; i < 3; ++i)
@@ -141,17 +146,20 @@ __device__ __forceinline__ void log_near_pi(const float (&X)[3], const float (&Y
         for (int k = 0; k < 3; ++k)
             E[i][k] = fma_(Z[i], Rt[2][k], fma_(Y[i], Rt[1][k], mul(X[i], Rt[0][k])));
     const float inv = __fdividef(1.0f, sub(1.0f, cth));
-    float ax[3];
+    float d2[3];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) ax[i] = sqrtf(fmaxf(mul(sub(E[i][i], cth), inv), 0.f));
+    for (int i = 0; i < 3; ++i) d2[i] = mul(sub(E[i][i], cth), inv);
     int m = 0;
-    float amax = ax[0];
-    if (ax[1] > amax) { amax = ax[1]; m = 1; }
-    if (ax[2] > amax) { m = 2; }
+    float dmax = d2[0];
+    if (d2[1] > dmax) { dmax = d2[1]; m = 1; }
+    if (d2[2] > dmax) { dmax = d2[2]; m = 2; }
+    const float am = sqrtf(fmaxf(dmax, 0.25f));
+    const float k = __fdividef(mul(0.5f, inv), am);
+    float ax[3];
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         const float sym = (m == 0) ? add(E[0][i], E[i][0]) : (m == 1) ? add(E[1][i], E[i][1]) : add(E[2][i], E[i][2]);
-        if (i != m && sym < 0.f) ax[i] = -ax[i];
+        ax[i] = (i == m) ? am : mul(sym, k);
     }
     const float dt = fma_(ax[2], v[2], fma_(ax[1], v[1], mul(ax[0], v[0])));
     const float th = (dt < 0.f) ? -theta : theta;
@@ -386,7 +394,7 @@ __device__ __forceinline__ void eval_pose(const KChain &ch, const float (&q)[D],
     // theta / s; the small-angle series 1 + s^2/6 takes over below s = 1e-4
     const float scale = (sn < 1e-4f) ? fma_(s2, 0.166666667f, 1.0f) : __fdividef(theta, sn);
     w[0] = mul(scale, v[0]); w[1] = mul(scale, v[1]); w[2] = mul(scale, v[2]);
-    if (sn < 1e-4f && cth <= 0.f) log_near_pi(X, Y, Z, Rt, v, cth, theta, w);
+    if (cth < -0.9f) log_far(X, Y, Z, Rt, v, cth, theta, w);
     }
 #pragma unroll
     for (int i = 0; i < 3; ++i) {

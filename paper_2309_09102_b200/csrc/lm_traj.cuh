@@ -569,6 +569,9 @@ template <int D, int MODE, bool FUSED, bool WEIGHTED, typename SpecT>
 __global__ void __launch_bounds__(TL_SOLVE_MAX_THREADS) tl_solve_kernel(const __grid_constant__ TArgs A) {
     constexpr int NA = Tri<D>::NA, SF = tl_stage_floats<D, MODE>();
     constexpr int TL_STAGES = tl_stages<D, MODE>();
+    // the mbarrier parity argument (above) on the stage count this instantiation really has, not the wanted one
+    static_assert(!FUSED || (TL_SOLVE_THREADS_FEW_TILES / 32 - 2) / 2 <= TL_STAGES, "more producers per chain than ring stages");
+    static_assert(TL_STAGES >= 1, "no ring stage fits the shared-memory budget");
     constexpr uint32_t FULL_COUNT = (FUSED && MODE == 1) ? 2u : 1u; // fused MODE 1: the poster of the copy's byte count + the writer of rho
     extern __shared__ __align__(128) float smem[];
     __shared__ __align__(8) uint64_t full_all[2][TL_STAGES], empty_all[2][TL_STAGES];

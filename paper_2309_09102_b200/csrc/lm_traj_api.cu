@@ -265,6 +265,9 @@ int lm_traj_run(lm_ctx *c, int32_t iters) {
         LM_CUDA(launch_plain(c, TK_PACK_TARGETS, a));
         t.targets_packed = true;
     }
+    // collision cost: lanes along the path unless the trajectories of a tile are known to be alike (LM_OPT_TRAJ_COST_LANES);
+    // set before the entry cost pass, which obeys it too
+    a.cost_by_waypoints = t.cost_lanes == 2 || (t.cost_lanes == 0 && !c->shared) ? 1 : 0;
     // current point -> tile order, and its cost
     LM_CUDA(launch_plain(c, TK_PACK_Q, a));
     LM_CUDA(launch_pose(c, TK_COST_INIT, a));
@@ -277,8 +280,6 @@ int lm_traj_run(lm_ctx *c, int32_t iters) {
     // producer warps of one block per tile) and when there are too few tiles to keep the producers of a block ahead of
     // its chains.  Same functions, same bits either way (tests/test_gpu_traj.py).
     const bool coll = a.caps.npairs + a.caps.nenv > 0;
-    // collision cost: lanes along the path unless the trajectories of a tile are known to be alike (LM_OPT_TRAJ_COST_LANES)
-    a.cost_by_waypoints = t.cost_lanes == 2 || (t.cost_lanes == 0 && !c->shared) ? 1 : 0;
     // (with the stored rows the producers could take them too; measured: 0.62 vs 0.55 ms at 4096 x 300 with 9 pairs, the
     // recompute fallback spills in the solve kernel)
     const bool fused = !coll && (t.fused_mode == 1 || (t.fused_mode == 0 && a.Bt >= TL_FUSED_MIN_TILES));

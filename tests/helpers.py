@@ -10,7 +10,15 @@ TOL_Q = 1e-4      # rad (m for prismatic) per joint        -- BASELINE.json nort
 TOL_POS = 1e-5    # m, pose error after a fixed iteration count
 TOL_ROT = 1e-4    # rad
 FLOOR = 1e-5      # |r| below which accept/reject is no longer compared (the fp32 floor region)
-EPS_POSE = 5e-7   # abs error of an fp32 pose residual norm: 7-8 joints x ulp(1) ~ 2e-7 in position and in rotation
+# Absolute error of the kernel's fp32 pose against the fp64 oracle at the same fp32 inputs.  MEASURED on the B200 by
+# tests/test_gpu_parity.py (test_fk_matches_oracle on five chains over their whole joint range,
+# test_pose_residual_error_is_within_eps_pose on configs[1..3], 64 x 300 waypoints each), which assert these bounds:
+#   position of the end effector   max 4.63e-7 m   (8-DoF chain; Panda 1.8e-7 .. 2.0e-7)
+#   rotation angle of R R_oracle^T max 6.74e-7 rad (8-DoF chain; Panda 1.8e-7 .. 2.1e-7)
+#   | |r| - |r|_oracle |           max 5.66e-7     (configs[2]; configs[1] 2.5e-7, configs[3] 3.8e-7)
+# The constants are round numbers just above the measured maxima.
+EPS_POS = 5e-7    # m: position of a point carried through fp32 FK
+EPS_POSE = 8e-7   # abs error of an fp32 pose residual norm |r| (and of its position / rotation parts)
 
 
 def decisive(F_before, F_trial, floor: float = FLOOR, margin: float = 1e-3):
@@ -143,7 +151,7 @@ def oracle_travel_below_fp32(tr, o: orc.State, resolve: float = 1e-6) -> np.ndar
     return travel
 
 
-def check_chaotic_config(w: wl.Workload, g: dict, o: orc.State, n_iters: int, min_clear: float = 0.3) -> dict:
+def check_chaotic_config(w: wl.Workload, g: dict, o: orc.State, n_iters: int, min_clear: float = 0.65) -> dict:
     """Free-running protocol for configs[3] (far seeds): `g` = GPU outputs for exactly the
     waypoints of `w`.  Every set below is chosen from the ORACLE alone.
       clear  = every oracle decision above the 1e-5 floor is decisive (see `decisive`);

@@ -273,7 +273,8 @@ def test_solver_variants(lm, w_small):
         g = H.run_gpu(w_small, **kw)
         dq = np.abs(g["q"] - o.q).max(axis=1)
         assert np.all((g["status"] & 1) == 1)
-        assert np.percentile(dq, 99) <= (H.TOL_Q if "fast_sincos" not in kw else 5e-4), kw
+        print("solver variant", kw, "max |dq|", dq.max())
+        assert dq.max() <= H.TOL_Q, kw     # every waypoint (measured: 5.2e-5 without refinement, 8e-7 with two steps, 6.1e-5 fast sincos)
 
 
 def test_api_errors_on_device(lm, w_small):
@@ -384,3 +385,46 @@ def test_solve_host_pipelined_equals_the_stepwise_path(chunks):
     with pytest.raises(lm.LmError):                              # more chunks than the handle was created for
         lm.lm_pipe_solve(pipe, cchain, pb, prm, w.max_iters, 9, q.data_ptr(), st)
     lm.lm_pipe_destroy(pipe)
+
+
+# ------------------------------------------------------------------ the iteration limit of the ABI (LM_MAX_ITERS = 64)
+
+def test_iteration_limit_64(lm):
+    """lm_run(ctx, 64) with tol = 0: iteration 63 is bit 63 of the 64-bit accept mask and the 8-bit counter packed next
+    to the frozen flag reaches 64.  (a) lambda0 = 100, nu_down = 1.01: 64 small damped steps, EVERY one a decisive
+    accept in the oracle (checked below from the oracle alone) -> iters == 64, mask == 2^64 - 1 bit for bit, status
+    MAXITER, joints within the bar.  (b) the default constants: the run reaches the fp32 floor long before 64, where
+    decisions are noise -> iters == 64 both sides, joints within the bar, decisive bits equal.  (c) 64 x lm_step
+    returns the bits of lm_run(64); 65 is rejected."""
+    ch = wl.panda_chain()
+    c1 = wl.config1(H.oracle_fk(ch))
+    wa = wl.Workload("lim64a", ch, c1.B, c1.n, c1.target_pos, c1.target_quat, c1.seeds, 0.0, 64, 100.0)
+    tr = H.oracle_trace(wa, 64, nu_down=1.01)
+    Fb, Ft = np.stack([a.F_before for _, a in tr], 1), np.stack([a.F_trial for _, a in tr], 1)
+    assert H.decisive(Fb, Ft).all() and all((a.accepted == 1).all() for _, a in tr)
+    o = H.run_oracle(wa, nu_down=1.01)
+    g = H.run_gpu(wa, nu_down=1.01)
+    assert np.all(o.iters == 64) and np.all(g["iters"] == 64)
+    assert np.all(o.mask == np.uint64(0xFFFFFFFFFFFFFFFF)) and np.array_equal(g["mask"], o.mask)
+    assert np.all(g["status"] & lm.LM_ST_MAXITER) and not np.any(g["status"] & lm.LM_ST_FROZEN)
+    assert np.array_equal(g["status"] & 3, o.status & 3)
+    assert np.abs(g["q"] - o.q).max() <= H.TOL_Q
+    assert np.abs(g["lam"] / o.lam - 1.0).max() <= 1e-5            # lambda0 / 1.01^64, 64 roundings
+    assert np.abs(g["res_norm"] - o.res_norm).max() <= 2e-6
+    # (c) on the same problem
+    s = H.make_solver(wa, nu_down=1.01)
+    for _ in range(64):
+        s.step()
+    same_bits(s.fetch(), g, keys=("q", "res_norm", "lam", "iters", "mask"))
+    s.step()                                                       # a 65th iteration has no mask bit: nothing executes
+    same_bits(s.fetch(), g, keys=("q", "res_norm", "lam", "iters", "mask"))
+    with pytest.raises(lm.LmError):
+        lm.lm_run(s._ctx, 65)
+    s.close()
+    # (b)
+    wb = wl.Workload("lim64b", ch, c1.B, c1.n, c1.target_pos, c1.target_quat, c1.seeds, 0.0, 64, c1.lambda0)
+    o, g = H.run_oracle(wb), H.run_gpu(wb)
+    assert np.all(o.iters == 64) and np.all(g["iters"] == 64) and np.all(g["status"] & lm.LM_ST_MAXITER)
+    assert np.abs(g["q"] - o.q).max() <= H.TOL_Q
+    compared, bad = H.decisive_mismatches(wb, g, 64)
+    assert compared >= 100 and bad == 0, (compared, bad)

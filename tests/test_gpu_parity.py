@@ -52,6 +52,32 @@ def test_fk_matches_oracle(lm, chain):
     po, Ro = orc.fk(chain, q.astype(np.float64))
     assert np.abs(p - po).max() < 1e-6       # SURVEY section 7 minimum slice: <= 1e-6 m
     assert np.abs(R - Ro).max() < 1e-6       #                                 <= 1e-6 rad
+    # the measured fp32 pose error that H.EPS_POSE bounds (DESIGN.md section 4 quotes these numbers)
+    pos_e = np.linalg.norm(p - po, axis=1).max()
+    rot_e = (np.linalg.norm(R @ Ro.transpose(0, 2, 1) - np.eye(3), axis=(1, 2)) / np.sqrt(2.0)).max()
+    print("FK error:", chain.name, chain.dof, "max |p - p_oracle|", pos_e, "max rotation angle", rot_e)
+    assert pos_e <= H.EPS_POS and rot_e <= H.EPS_POSE
+
+
+@pytest.mark.parametrize("cfg", ["C2", "C3", "C4"])
+def test_pose_residual_error_is_within_eps_pose(lm, cfg):
+    """H.EPS_POSE (the absolute error allowed to an fp32 pose residual norm; `decisive` and the collision tests derive
+    their noise terms from it) is a bound on something MEASURED here: |r| of the kernel at the seeds of configs[1..3]
+    against the oracle's fp64 |r| at the same fp32 inputs, all waypoints of 64 trajectories."""
+    if cfg == "C2":
+        w = wl.config2(H.oracle_fk(wl.panda_chain()), B=64, n=300)
+    elif cfg == "C3":
+        w = wl.config3(H.oracle_fk(wl.random_chain_8dof(3)), B=64, n=300)
+    else:
+        w = wl.config4(H.oracle_fk(wl.panda_chain()), B=64, n=300)
+    s = H.make_solver(w)
+    g = s.fetch()
+    s.close()
+    pe, re = H.pose_errors_by_oracle(w, w.seeds)
+    rn = np.sqrt(pe * pe + re * re)
+    e_r, e_p, e_w = np.abs(g["res_norm"] - rn).max(), np.abs(g["pos_err"] - pe).max(), np.abs(g["rot_err"] - re).max()
+    print("pose residual error:", cfg, "max | |r| - oracle |", e_r, "position part", e_p, "rotation part", e_w, "max |r|", rn.max())
+    assert max(e_r, e_p, e_w) <= H.EPS_POSE
 
 
 # ------------------------------------------------------------------ free-running parity (P10)
