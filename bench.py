@@ -166,6 +166,31 @@ def dist_max_sum(ms: float, units: float, device) -> tuple:
     return float(t.item()), float(u.item())
 
 
+def spawn_ranks(n: int, argv: list) -> int:
+    """Re-run this script as n ranks of one node under torch.distributed.run (one process per GPU, LOCAL_RANK = device
+    index), exactly as the driver launches the N > 1 bench; returns its exit code.  Rank 0's JSON line passes through."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+    return subprocess.call(cmd)
+
+
+def run_dist_selftest(args) -> None:
+    """The N > 1 plumbing without a GPU (tests/test_dist_cpu.py): process group over gloo, the barrier, the MAX of the
+    per-rank times and the SUM of the per-rank units -- everything that crosses ranks in run_gpu -- and rank 0's line."""
+    import torch
+    rank, world = dist_init("gloo")
+    dist_barrier()
+    ms, units = dist_max_sum(1.0 + rank, 1.0, torch.device("cpu"))
+    dist_barrier()
+    if rank == 0:
+        print(json.dumps({"selftest": "dist", "n_gpus": world, "requested": args.gpus, "ms_max": ms, "units_sum": units}), flush=True)
+
+
 def rank_seed_offset(rank: int) -> int:
     """Each rank draws its own batch (weak scaling): the workload seed is offset by 1000 * rank."""
     return 1000 * rank
@@ -361,11 +386,6 @@ def run_gpu(args) -> None:
         extra["c3_8dof"] = time_c3(lm, torch, wl, device, stream, peak_tf)
         # BASELINE.json configs[4], compact: B x n grid, exactly 20 iterations
         extra["sweep_C5"] = time_sweep_c5(lm, torch, wl, fk, device, stream)
-        # FFMA / FFMA2 operand forms (register-file read-bandwidth calibration, profiles/r2_rf_model.md)
-        extra["fma_operand_forms_tflops"] = {n: lm.lm_fp32_peak_form(f, int(stream.cuda_stream)) for n, f in
-                                             (("R,c,c", lm.LM_FMA_FORM_RCC), ("R,R,R", lm.LM_FMA_FORM_RRR), ("R,Rreuse,R", lm.LM_FMA_FORM_RRS),
-                                              ("R,Rreuse,Rreuse", lm.LM_FMA_FORM_RSS), ("FMUL R,R", lm.LM_FMA_FORM_MUL),
-                                              ("FFMA2 P,P,P", lm.LM_FMA_FORM_PPP), ("FFMA2 P,Rbcast,P", lm.LM_FMA_FORM_PSP))}
         # the "to convergence" statistic of the metric, on BASELINE.json configs[1] (512 x 300, tol 1e-5)
         extra["to_convergence_C2"] = time_to_convergence(lm, torch, wl, fk, device, stream)
         extra["variant_dual"] = time_dual_variant(lm, torch, w, device, stream, peak_tf)
@@ -377,8 +397,6 @@ def run_gpu(args) -> None:
         extra["schedule_C2"] = time_plan(lm, torch, wl, fk, device, stream)
         # the global discrete search over K candidates of one path (NEXT-4 iii)
         extra["search_K175_n300"] = time_search(lm, torch, wl, fk, device, stream)
-    # (the rate of FFMAs with three new register operands is a calibration point of the register-file read model, not a
-    # roofline: it is reported with the other operand forms under fma_operand_forms_tflops)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms_all / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": cfg,
@@ -895,9 +913,22 @@ def main() -> None:
     ap.add_argument("--block", type=int, default=0, help="threads per block override")
     ap.add_argument("--ref-traj", type=int, default=0,
                     help="trajectories in the oracle's timed sample (default 256 for cpu_baseline, 16 per step for --impl reference)")
+    ap.add_argument("--dist-selftest", action="store_true",
+                    help="no GPU work: start the ranks, run the two cross-rank reductions of the bench over gloo and print their line")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: start the N ranks ourselves (the torchrun path stays as it is)
+        if not args.dist_selftest:
+            import torch
+            have = torch.cuda.device_count()
+            if have < args.gpus:
+                sys.exit(f"bench.py: {args.gpus} GPUs requested, {have} visible")
+        sys.exit(spawn_ranks(args.gpus, sys.argv[1:]))
+    if args.dist_selftest:
+        run_dist_selftest(args)
     else:
         run_gpu(args)
 

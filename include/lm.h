@@ -464,28 +464,13 @@ int lm_search_static(const lm_chain *chain, int64_t K, int64_t n, const float *q
  * tflops_out: 2 * FFMA / s / 1e12.  The measured counterpart of the ALU roofline. */
 int lm_fp32_peak(void *cuda_stream, double *tflops_out);
 
-/* The same measurement for one operand form of FFMA: LM_FMA_FORM_RCC = one register operand, the
- * other two from the constant bank (what lm_fp32_peak reports: the pipe's ceiling), LM_FMA_FORM_RRR =
- * three distinct register operands (what dense in-register linear algebra issues; register-file
- * read bandwidth limits it well below the pipe's ceiling on sm_100a). */
-#define LM_FMA_FORM_RCC 0
-#define LM_FMA_FORM_RRR 1
-/* Calibration points of the register-file read model (profiles/r2_rf_model.md): RRS / RSS = one / two of the register
- * operands shared by consecutive FFMAs (operand-reuse cache), MUL = FMUL with two register operands, PPP / PSP = the
- * packed FFMA2 with three register pairs / pair, broadcast scalar, pair.  All report 2 x lane-operations / s / 1e12. */
-#define LM_FMA_FORM_RRS 2
-#define LM_FMA_FORM_RSS 3
-#define LM_FMA_FORM_MUL 4
-#define LM_FMA_FORM_PPP 5
-#define LM_FMA_FORM_PSP 6
-int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out);
-
 void lm_free(lm_ctx *ctx);
 
 /* Static string for a status code; for LM_ECUDA the last CUDA error string seen by this thread. */
 const char *lm_strerror(int code);
 
-/* Kernels launched by this library in this process so far (bench.py's gpu_launches). */
+/* Diagnostics, not part of the method: kernels launched by this library in this process so far (bench.py reports it
+ * as gpu_launches; the tests use it to check launch counts such as "lm_run is ONE launch"). */
 int64_t lm_launch_count(void);
 
 #ifdef __cplusplus

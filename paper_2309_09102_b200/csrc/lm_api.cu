@@ -313,64 +313,6 @@ __global__ void __launch_bounds__(256) lm_fma_peak_kernel(float *out, int iters,
     if (sum == 12345.678f) out[0] = sum; // never true: keeps the chains alive
 }
 
-// The same with three distinct REGISTER operands per FFMA (x = x * y + z), the form dense
-// in-register linear algebra issues: limited by register-file read bandwidth, not by the FMA pipe.
-__global__ void __launch_bounds__(256) lm_fma_rrr_kernel(float *out, int iters, const float *in) {
-    float x[16], y[16], z[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        x[i] = (float)(threadIdx.x + i) * 1e-3f;
-        y[i] = in[i + (threadIdx.x & 3)];      // lane-dependent addresses: keeps y, z in vector registers
-        z[i] = in[32 + i + (threadIdx.x & 3)];
-    }
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) x[i] = __fmaf_rn(x[i], y[i], z[i]);
-    }
-    float sum = 0.f;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) sum += x[i];
-    if (sum == 12345.678f) out[0] = sum;
-}
-
-// Further operand forms of the same loop (register-file read-bandwidth calibration, profiles/r2_rf_model.md):
-//   RRS  x = x * y0 + z[i]   (y0 shared by consecutive FFMAs: operand-reuse cache)      2 new register reads
-//   RSS  x = x * y0 + z0                                                                  1 new register read
-//   MUL  x = x * y[i]        (FMUL, two register operands)                                2
-//   PPP  (x, x') = (x, x') * (y, y') + (z, z')   FFMA2, three register pairs              6
-//   PSP  (x, x') = (x, x') * (y0, y0) + (z, z')  FFMA2, pair, broadcast scalar, pair      5
-template <int FORM>
-__global__ void __launch_bounds__(256) lm_fma_form_kernel(float *out, int iters, const float *in) {
-    float x[16], y[16], z[16];
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        x[i] = (float)(threadIdx.x + i) * 1e-3f;
-        y[i] = in[i + (threadIdx.x & 3)];
-        z[i] = in[32 + i + (threadIdx.x & 3)];
-    }
-    for (int it = 0; it < iters; ++it) {
-        if (FORM == LM_FMA_FORM_PPP || FORM == LM_FMA_FORM_PSP) {
-#pragma unroll
-            for (int i = 0; i < 16; i += 2) {
-                const float2 yy = FORM == LM_FMA_FORM_PPP ? make_float2(y[i], y[i + 1]) : make_float2(y[0], y[0]);
-                const float2 r = __ffma2_rn(make_float2(x[i], x[i + 1]), yy, make_float2(z[i], z[i + 1]));
-                x[i] = r.x;
-                x[i + 1] = r.y;
-            }
-        } else {
-#pragma unroll
-            for (int i = 0; i < 16; ++i)
-                x[i] = FORM == LM_FMA_FORM_RRS ? __fmaf_rn(x[i], y[0], z[i])
-                     : FORM == LM_FMA_FORM_RSS ? __fmaf_rn(x[i], y[0], z[0])
-                                               : __fmul_rn(x[i], y[i]);
-        }
-    }
-    float sum = 0.f;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) sum += x[i];
-    if (sum == 12345.678f) out[0] = sum;
-}
-
 __global__ void lm_unpack_kernel(const uint32_t *__restrict__ its, int64_t W, int32_t *__restrict__ iters,
                                  uint32_t *__restrict__ status) {
     const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -793,21 +735,14 @@ int lm_pipe_solve(lm_pipe *pp, void *cuda_stream, const lm_chain *chain, const l
     return rc;
 }
 
-int lm_fp32_peak(void *cuda_stream, double *tflops_out) { return lm_fp32_peak_form(cuda_stream, LM_FMA_FORM_RCC, tflops_out); }
-
-int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out) {
-    if (!tflops_out || form < LM_FMA_FORM_RCC || form > LM_FMA_FORM_PSP) return LM_EINVAL;
+int lm_fp32_peak(void *cuda_stream, double *tflops_out) {
+    if (!tflops_out) return LM_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int dev = 0, sms = 0;
     LM_CUDA(cudaGetDevice(&dev));
     LM_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    float *scratch = nullptr;
-    LM_CUDA(cudaMalloc(&scratch, 256));
-    {
-        float h[64];
-        for (int i = 0; i < 64; ++i) h[i] = (i < 32) ? 0.999f : 1e-3f; // y = 0.999 (words 0..18), z = 1e-3 (words 32..50)
-        LM_CUDA(cudaMemcpy(scratch, h, sizeof(h), cudaMemcpyHostToDevice));
-    }
+    float *sink = nullptr; // the kernel's never-taken store needs an address
+    LM_CUDA(cudaMalloc(&sink, 256));
     cudaEvent_t e0, e1;
     LM_CUDA(cudaEventCreate(&e0));
     LM_CUDA(cudaEventCreate(&e1));
@@ -816,27 +751,18 @@ int lm_fp32_peak_form(void *cuda_stream, int32_t form, double *tflops_out) {
     for (int rep = 0; rep < 6; ++rep) {
         cudaEventRecord(e0, st);
         g_launches.fetch_add(1);
-        switch (form) {
-        case LM_FMA_FORM_RCC: lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(scratch + 60, iters, 0.999f, 1e-3f); break;
-        case LM_FMA_FORM_RRR: lm_fma_rrr_kernel<<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
-        case LM_FMA_FORM_RRS: lm_fma_form_kernel<LM_FMA_FORM_RRS><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
-        case LM_FMA_FORM_RSS: lm_fma_form_kernel<LM_FMA_FORM_RSS><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
-        case LM_FMA_FORM_MUL: lm_fma_form_kernel<LM_FMA_FORM_MUL><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
-        case LM_FMA_FORM_PPP: lm_fma_form_kernel<LM_FMA_FORM_PPP><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
-        default: lm_fma_form_kernel<LM_FMA_FORM_PSP><<<blocks, threads, 0, st>>>(scratch + 60, iters, scratch); break;
-        }
+        lm_fma_peak_kernel<<<blocks, threads, 0, st>>>(sink, iters, 0.999f, 1e-3f);
         cudaEventRecord(e1, st);
         cudaError_t e = cudaEventSynchronize(e1);
-        if (e != cudaSuccess) { cudaFree(scratch); return cuda_fail(e); }
+        if (e != cudaSuccess) { cudaFree(sink); return cuda_fail(e); }
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
-        // 2 flop per lane-operation also for the FMUL form: the figure is "lane-operations / s x 2", comparable across forms
         const double tf = 2.0 * 16.0 * iters * (double)blocks * threads / (ms * 1e-3) / 1e12;
         if (rep > 0 && tf > best) best = tf;
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    cudaFree(scratch);
+    cudaFree(sink);
     *tflops_out = best;
     return LM_OK;
 }

@@ -29,14 +29,13 @@ LM_ST_FROZEN, LM_ST_MAXITER, LM_ST_BREAKDOWN, LM_ST_NONFINITE, LM_ST_CLAMPED = 1
 # every symbol include/lm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ("lm_workspace_bytes", "lm_default_params", "lm_init", "lm_step", "lm_run", "lm_fetch",
            "lm_reset", "lm_set_state", "lm_set_trace", "lm_set_option", "lm_kernel_name", "lm_fk", "lm_fp32_peak", "lm_free",
-           "lm_strerror", "lm_launch_count", "lm_fp32_peak_form",
+           "lm_strerror", "lm_launch_count",
            "lm_traj_workspace_bytes", "lm_traj_default_params", "lm_traj_attach", "lm_traj_run", "lm_traj_reset",
            "lm_traj_fetch", "lm_traj_set_trace", "lm_traj_set_capsules", "lm_traj_set_obstacles",
            "lm_solve_host_workspace_bytes", "lm_solve_host", "lm_pipe_create", "lm_pipe_solve", "lm_pipe_destroy", "lm_specialize",
            "lm_plan_workspace_bytes", "lm_plan_default_params", "lm_plan_attach", "lm_plan_run", "lm_plan_fetch",
            "lm_search_workspace_bytes", "lm_search_default_params", "lm_search",
            "lm_search_static_fits", "lm_search_static")
-LM_FMA_FORM_RCC, LM_FMA_FORM_RRR, LM_FMA_FORM_RRS, LM_FMA_FORM_RSS, LM_FMA_FORM_MUL, LM_FMA_FORM_PPP, LM_FMA_FORM_PSP = range(7)
 LM_SOLVER_PRIMAL, LM_SOLVER_DUAL = 0, 1
 LM_ROT_LOG, LM_ROT_RPY = 0, 1
 
@@ -146,7 +145,6 @@ def lib() -> C.CDLL:
         L.lm_strerror.argtypes = [C.c_int]
         L.lm_strerror.restype = C.c_char_p
         L.lm_launch_count.restype = C.c_int64
-        L.lm_fp32_peak_form.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
         L.lm_traj_workspace_bytes.argtypes = [C.c_int32, C.c_int64, C.c_int64]
         L.lm_traj_workspace_bytes.restype = C.c_size_t
         L.lm_traj_default_params.argtypes = [C.POINTER(LmTrajParams)]
@@ -280,12 +278,6 @@ def lm_fp32_peak(cuda_stream: int = 0) -> float:
     return float(out.value)
 
 
-def lm_fp32_peak_form(form: int, cuda_stream: int = 0) -> float:
-    out = C.c_double(0.0)
-    _check(lib().lm_fp32_peak_form(C.c_void_p(cuda_stream), int(form), C.byref(out)), "lm_fp32_peak_form")
-    return float(out.value)
-
-
 def lm_traj_workspace_bytes(dof: int, B: int, n: int) -> int:
     return int(lib().lm_traj_workspace_bytes(dof, B, n))
 
@@ -333,13 +325,12 @@ def lm_traj_set_capsules(ctx: int, model, w_coll: float = 1.0, d_safe: float = 0
 
 
 def lm_traj_set_obstacles(ctx: int, scene, w_env: float = 1.0, d_safe: float = 0.05) -> None:
-    """scene: a workloads.ObstacleScene-like object (R [M,3,3], t, pmin, pmax, pairs) or None to remove the rows."""
+    """scene: a workloads.ObstacleScene-like object (pose [M, 7] = xyz + unit quaternion w, x, y, z of each box frame, as
+    lm_obstacles takes it; pmin, pmax [M, 3]; pairs [Q, 2]) or None to remove the rows."""
     if scene is None:
         _check(lib().lm_traj_set_obstacles(ctx, None), "lm_traj_set_obstacles")
         return
-    from scipy.spatial.transform import Rotation
-    xyzw = Rotation.from_matrix(np.asarray(scene.R, dtype=np.float64)).as_quat()
-    pose = np.ascontiguousarray(np.concatenate([scene.t, xyzw[:, 3:4], xyzw[:, 0:3]], axis=1), dtype=np.float32)
+    pose = np.ascontiguousarray(scene.pose, dtype=np.float32)
     pmin = np.ascontiguousarray(scene.pmin, dtype=np.float32)
     pmax = np.ascontiguousarray(scene.pmax, dtype=np.float32)
     pairs = np.ascontiguousarray(scene.pairs, dtype=np.int32)
@@ -457,8 +448,7 @@ class Solver:
     """
 
     def __init__(self, chain, B: int, n: int, target_pos, target_quat, seeds, params: Optional[LmParams] = None,
-                 shared_targets: bool = False, host_inputs: bool = False, device: str = "cuda:0", stream=None,
-                 guarded: bool = False):
+                 shared_targets: bool = False, host_inputs: bool = False, device: str = "cuda:0", stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the batched-LM path has no CPU fallback")
@@ -470,8 +460,6 @@ class Solver:
         self.host_inputs = bool(host_inputs)
         self.stream = stream
         self._ctx = None
-        self.guarded = bool(guarded)      # test knob: guard bands around every workspace + poisoned interior
-        self._guards = []
         Wt = self.n if self.shared else self.W
         assert np.shape(target_pos) == (Wt, 3) and np.shape(target_quat) == (Wt, 4) and np.shape(seeds) == (self.W, self.d)
 
@@ -491,32 +479,10 @@ class Solver:
             self._stream_handle = int(s.cuda_stream)
             self._ctx = lm_init(self._cchain, pb, self.params, self._stream_handle)
 
-    GUARD_BYTES = 4096
-
     def _alloc_ws(self, nbytes: int):
-        """Device scratch of `nbytes` (256-byte aligned pointer).  guarded=True (tests/test_gpu_guards.py; the stand-in
-        for compute-sanitizer's memcheck / initcheck, which is closed on this pool): 4 KiB guard bands filled with 0xA5
-        on either side -- an out-of-bounds WRITE of any kernel shows up in guards_intact() -- and the interior
-        poisoned with 0xFF bytes (fp32 NaN, int -1) so that a read of memory no kernel has written ends up in the
-        outputs."""
-        torch = self.torch
-        if not self.guarded:
-            t = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-            return t, (t.data_ptr() + 255) // 256 * 256
-        G = self.GUARD_BYTES
-        t = torch.full((nbytes + 2 * G + 256,), 0xA5, dtype=torch.uint8, device=self.device)
-        ptr = (t.data_ptr() + G + 255) // 256 * 256
-        off = ptr - t.data_ptr()
-        t[off:off + nbytes] = 0xFF
-        self._guards.append((t, off, nbytes))
-        return t, ptr
-
-    def guards_intact(self) -> bool:
-        self.torch.cuda.synchronize(self.device)
-        ok = True
-        for t, off, nbytes in self._guards:
-            ok = ok and bool((t[:off] == 0xA5).all().item()) and bool((t[off + nbytes:] == 0xA5).all().item())
-        return ok
+        """Device scratch of `nbytes`: (the tensor that owns it, a 256-byte aligned pointer into it)."""
+        t = self.torch.empty(nbytes + 256, dtype=self.torch.uint8, device=self.device)
+        return t, (t.data_ptr() + 255) // 256 * 256
 
     def _on_stream(self):
         """Uploads and allocations happen on the stream the library launches on: with a caller-supplied

@@ -134,6 +134,11 @@ class ObstacleScene:
     pmax: np.ndarray   # [M, 3]
     pairs: np.ndarray  # [Q, 2] (capsule index, obstacle index)
 
+    @property
+    def pose(self) -> np.ndarray:
+        """[M, 7] xyz + unit quaternion (w, x, y, z) of every box frame: the form include/lm.h's lm_obstacles takes."""
+        return np.concatenate([np.asarray(self.t, dtype=np.float64), _R_to_quat_wxyz(np.asarray(self.R, dtype=np.float64))], axis=1)
+
 
 def panda_scene(seed: int = 7) -> ObstacleScene:
     """SYNTHETIC scene for the Panda capsule model (the paper's obstacle scenes are not available): a table slab in

@@ -81,3 +81,24 @@ def test_reference_arm_runs_on_rank0_only():
 def test_shard_seeds_are_rank_specific():
     import bench
     assert bench.rank_seed_offset(0) == 0 and bench.rank_seed_offset(3) == 3000
+
+
+@pytest.mark.timeout(300)
+def test_bench_starts_its_own_ranks():
+    """`python bench.py --gpus 2` with no launcher around it starts two ranks itself (torch.distributed.run, 127.0.0.1):
+    the self-test leg runs the bench's cross-rank reductions over gloo and rank 0's line says n_gpus = 2.  Without the
+    self-test flag, on a box with fewer GPUs than requested, it fails loudly instead of running one rank."""
+    bench = os.path.join(ROOT, "bench.py")
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    env["OMP_NUM_THREADS"] = "1"
+    r = subprocess.run([sys.executable, bench, "--gpus", "2", "--dist-selftest"], env=env, stdout=subprocess.PIPE,
+                       stderr=subprocess.PIPE, text=True, timeout=280, cwd=ROOT)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(x) for x in r.stdout.splitlines() if x.startswith("{")]
+    assert len(lines) == 1                                          # rank 0 alone prints
+    assert lines[0]["n_gpus"] == 2 and lines[0]["ms_max"] == 2.0 and lines[0]["units_sum"] == 2.0
+    import torch
+    if torch.cuda.device_count() < 2:
+        r = subprocess.run([sys.executable, bench, "--gpus", "2", "--steps", "1"], env=env, stdout=subprocess.PIPE,
+                           stderr=subprocess.PIPE, text=True, timeout=120, cwd=ROOT)
+        assert r.returncode != 0 and "2 GPUs requested" in r.stderr and r.stdout.strip() == ""

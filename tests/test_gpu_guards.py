@@ -4,7 +4,7 @@ compute-sanitizer is CLOSED on this GPU pool (gpurun answers "compute-sanitizer 
 closed: runs under it have left GPUs needing a reset", profiles/r2_sanitizers.md), so memcheck / initcheck / racecheck
 are replaced by what can be observed from outside the kernels:
 
-  * out-of-bounds WRITES: every workspace gets 4 KiB guard bands filled with 0xA5 (Solver(guarded=True)); after every
+  * out-of-bounds WRITES: every workspace gets 4 KiB guard bands filled with 0xA5 (GuardedSolver below); after every
     kernel of the library has run on ragged sizes the bands must be intact;
   * reads of UNWRITTEN scratch: the workspace interior is poisoned with 0xFF bytes (fp32 NaN / int -1) instead of
     whatever the allocator hands out; all outputs must be bit-identical to the unpoisoned run;
@@ -28,11 +28,45 @@ def problem(ch, B, n, seed, sigma=0.03):
     return wl._from_truth("G", ch, truth, sigma, rng, lambda q: orc.fk(ch, q), 0.0, 8)
 
 
+def guarded_solver_class():
+    """lm.Solver with every workspace it allocates wrapped in guard bands (the stand-in for compute-sanitizer's memcheck /
+    initcheck, which is closed on this pool): 4 KiB filled with 0xA5 on either side -- an out-of-bounds WRITE of any
+    kernel shows up in guards_intact() -- and the interior poisoned with 0xFF bytes (fp32 NaN, int -1) so that a read
+    of memory no kernel has written ends up in the outputs.  Test equipment: it lives here, not in the binding."""
+    from paper_2309_09102_b200 import lm
+
+    class GuardedSolver(lm.Solver):
+        GUARD_BYTES = 4096
+
+        def __init__(self, *a, **kw):
+            self._guards = []
+            super().__init__(*a, **kw)
+
+        def _alloc_ws(self, nbytes: int):
+            torch, G = self.torch, self.GUARD_BYTES
+            t = torch.full((nbytes + 2 * G + 256,), 0xA5, dtype=torch.uint8, device=self.device)
+            ptr = (t.data_ptr() + G + 255) // 256 * 256
+            off = ptr - t.data_ptr()
+            t[off:off + nbytes] = 0xFF
+            self._guards.append((t, off, nbytes))
+            return t, ptr
+
+        def guards_intact(self) -> bool:
+            self.torch.cuda.synchronize(self.device)
+            ok = True
+            for t, off, nbytes in self._guards:
+                ok = ok and bool((t[:off] == 0xA5).all().item()) and bool((t[off + nbytes:] == 0xA5).all().item())
+            return ok
+
+    return GuardedSolver
+
+
 def everything(ch, w, guarded, rows=True):
     """Every entry point of the library on one problem; returns all outputs (numpy) and the solver's guard verdict."""
     from paper_2309_09102_b200 import lm
     out = {}
-    s = lm.Solver(ch, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0), guarded=guarded)
+    cls = guarded_solver_class() if guarded else lm.Solver
+    s = cls(ch, w.B, w.n, w.target_pos, w.target_quat, w.seeds, params=lm.lm_default_params(tol=0.0))
     s.enable_trace()
     s.run(3)
     s.step()
