@@ -66,11 +66,13 @@ def ncu_constant(key: str, field: str, files):
 
 def load_peaks() -> dict:
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    d = {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "_source": "fallback"}
     if os.path.exists(p):
         d = json.load(open(p))
         d["_source"] = "measured"
-        return d
-    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "_source": "fallback"}
+    # FP32 pipe peak, derived: SMs x FP32 lanes x 2 x the maximum SM clock
+    d["alu_tflops"] = SM_COUNT * FP32_LANES * 2 * d["sm_max_mhz"] * 1e6 / 1e12
+    return d
 
 
 def alg_bytes_per_waypoint(d: int) -> float:
@@ -386,6 +388,8 @@ def run_gpu(args) -> None:
         extra["c3_8dof"] = time_c3(lm, torch, wl, device, stream, peak_tf)
         # BASELINE.json configs[4], compact: B x n grid, exactly 20 iterations
         extra["sweep_C5"] = time_sweep_c5(lm, torch, wl, fk, device, stream)
+        # the paper's own batch shape: K = 175 plans of one path
+        extra["paper_shape_K175_n300"] = time_paper_shape(lm, torch, wl, fk, device, stream)
         # the "to convergence" statistic of the metric, on BASELINE.json configs[1] (512 x 300, tol 1e-5)
         extra["to_convergence_C2"] = time_to_convergence(lm, torch, wl, fk, device, stream)
         extra["variant_dual"] = time_dual_variant(lm, torch, w, device, stream, peak_tf)
@@ -430,6 +434,30 @@ def traj_step_alg_bytes(d: int, refine: int = 1, fused: bool = True) -> float:
     if not fused:
         words += 2 * (na + d) + refine * (2 * d)
     return 4.0 * words
+
+
+def traj_step_alg_flop(d: int, refine: int = 1) -> dict:
+    """Counted FP32 work of ONE trajectory-level LM iteration per waypoint (FMA = 2; DESIGN.md section 10 has the table).
+    The per-waypoint pieces are those of the pose step (FK 48 d + 6, residual 77, Jacobian 12 d,
+    J^T J + lambda 7 d^2, J^T r 12 d at d = 7: 342 / 77 / 84 / 343 / 84); the block-tridiagonal pieces follow from the
+    elimination S_i = D_i - w^4 S_{i-1}^-1 with the off-diagonal block -w_diff^2 I."""
+    fk, res, jac, jtj, jtr = 48.0 * d + 6.0, 77.0, 12.0 * d, 7.0 * d * d, 12.0 * d
+    matvec = 2.0 * d * d                                     # symmetric d x d block times a vector
+    assemble = fk + res + jac + jtj + jtr + 4.0 * d          # + the differencing part of g_i and of the diagonal
+    eliminate = d ** 3 + matvec + d * (d + 1)                # Cholesky + inverse of S_i (d^3), z_i update, S update
+    substitute = matvec + 2.0 * d                            # x_i = -S_i^-1 (z_i - w^2 x_{i+1})
+    rho = fk + res + jac + 12.0 * d + jtr + 6.0 * d          # r + J delta, J^T(...), lambda delta and differencing terms
+    resolve = 2.0 * (matvec + 2.0 * d)                       # forward and backward pass on the stored -S^-1
+    cost = fk + res + 5.0 * d                                # trial point, its pose and differencing cost
+    parts = {"assemble": assemble, "eliminate": eliminate, "substitute": substitute, "refine_rho": refine * rho,
+             "refine_resolve": refine * resolve, "trial_cost": cost}
+    parts["total"] = float(sum(parts.values()))
+    return parts
+
+
+def traj_step_method_bytes(d: int) -> float:
+    """What the METHOD must move per waypoint-iteration whatever the data flow: q (4 d) + target (28) in, q (4 d) out."""
+    return 8.0 * d + 28.0
 
 
 def traj_step_alg_bytes_round1(d: int, refine: int = 1) -> float:
@@ -525,26 +553,38 @@ def time_traj_step(lm, torch, w, solver, stream, peaks, iters: int = 10, reps: i
     ms0 = float(min(t0_)) / iters
     fused = (w.B + 31) // 32 >= 96  # LM_TL_FUSED_MIN_TILES (csrc/lm_traj.cuh); no collision rows in this leg
     alg0 = traj_step_alg_bytes(d, 0, fused) * w.W
-    norefine = {"ms_per_iteration": ms0, "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, 0, fused),
-                "hbm_frac": alg0 / (ms0 * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    norefine = {"ms_per_iteration": ms0, "design_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, 0, fused),
+                "hbm_design_traffic_frac": alg0 / (ms0 * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                "alu_frac": traj_step_alg_flop(d, 0)["total"] * w.W / (ms0 * 1e-3) / 1e12 / peaks["alu_tflops"]}
     ms_iter = float(min(ts)) / iters
     alg = traj_step_alg_bytes(d, int(tp.refine_steps), fused) * w.W
     alg_r1 = traj_step_alg_bytes_round1(d, int(tp.refine_steps)) * w.W
+    flop = traj_step_alg_flop(d, int(tp.refine_steps))
     out = {"workload": f"{w.name}: {w.B} x {w.n}, after 4 pose-only iterations; w_pose=1, w_diff=0.3, refine=1, {iters} iterations",
            "ms_per_iteration": ms_iter, "waypoint_iterations_per_sec": w.W / (ms_iter * 1e-3),
            "trajectory_iterations_per_sec": w.B / (ms_iter * 1e-3), "gpu_launches_per_run": int(launches),
            "accepted_fraction": float(np.mean([bin(int(m)).count("1") for m in g["mask"]])) / iters,
            "cost_diff_mean": float(g["cost_diff"].mean()), "with_self_collision_rows": coll,
            "without_refinement": norefine,
-           "roofline": {"bound": "hbm", "achieved": alg / (ms_iter * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                        "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"],
+           # Three fractions, none of them near 1: the step is bound by issue slots and by the latency of the sequential
+           # block elimination (one block of 32 trajectories per SM), DESIGN.md section 10.
+           "roofline": {"bound": "alu", "binding_limit": "issue slots / latency of the sequential block elimination, one tile of 32 trajectories per SM",
+                        "achieved": flop["total"] * w.W / (ms_iter * 1e-3) / 1e12, "peak": peaks["alu_tflops"], "unit": "TFLOP/s",
+                        "frac": flop["total"] * w.W / (ms_iter * 1e-3) / 1e12 / peaks["alu_tflops"],
                         "traffic": ncu_constant("traj_iteration_C4", "dram_bytes_per_iteration", TRAJ_SOURCES) if (w.B, w.n) == (4096, 300) else None,
-                        "alg_bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps), fused),
+                        "alg_flop_per_waypoint_iteration": flop,
+                        "hbm_method": {"bytes_per_waypoint_iteration": traj_step_method_bytes(d),
+                                       "what": "q and target in, q out: the method's own input + output, whatever the data flow",
+                                       "achieved_gbs": traj_step_method_bytes(d) * w.W / (ms_iter * 1e-3) / 1e9,
+                                       "frac": traj_step_method_bytes(d) * w.W / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"]},
+                        "hbm_design_traffic": {"bytes_per_waypoint_iteration": traj_step_alg_bytes(d, int(tp.refine_steps), fused),
+                                               "what": "the bytes of THIS design's data flow (the factor -S^-1 and z spilled to HBM and read back); "
+                                                       "measured DRAM traffic matches it by construction",
+                                               "achieved_gbs": alg / (ms_iter * 1e-3) / 1e9, "peak_gbs": peaks["hbm_gbs"],
+                                               "frac": alg / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                               "frac_on_round1_bytes": alg_r1 / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                               "round1_bytes_per_waypoint_iteration": traj_step_alg_bytes_round1(d, int(tp.refine_steps))},
                         "path": "fused (producer warps assemble in shared memory)" if fused else "unfused (per-waypoint kernels through HBM)",
-                        "frac_on_round1_bytes": alg_r1 / (ms_iter * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                        "round1_alg_bytes_per_waypoint_iteration": traj_step_alg_bytes_round1(d, int(tp.refine_steps)),
-                        "note": "the fused step needs 23 % fewer bytes than round 1's data flow, so the same time is a lower fraction; "
-                                "its solve kernels are bound by the issue slots of one SM per tile, not by HBM (DESIGN.md section 10)",
                         "peak_source": peaks["_source"]}}
     try:
         from oracle import lm_oracle as orc, lm_traj_oracle as torc
@@ -793,6 +833,43 @@ def time_sweep_c5(lm, torch, wl, fk, device, stream, reps: int = 5) -> dict:
             ms, iters, _ = _time_runs(torch, s, stream, w.max_iters, reps, flush)
             s.close()
             out["points"].append({"B": B, "n": n, "ms": ms, "waypoint_iterations_per_sec": iters / (ms * 1e-3)})
+    return out
+
+
+def time_paper_shape(lm, torch, wl, fk, device, stream, reps: int = 7) -> dict:
+    """The paper's own batch: K = 175 candidate plans x n = 300 poses of ONE target path (shared_targets),
+    52 500 waypoints = 11 warps per SM, one wave -- the latency-bound regime.  Candidates = the
+    path's joint-space truth + N(0, 0.1) per joint (as configs[4]).  Exactly 20 iterations with every block size / lane
+    group the library offers, and to convergence (tol 1e-5) with the defaults; L2 flushed before every launch."""
+    K, n = 175, 300
+    w1 = wl.config5(fk, B=1, n=n)
+    ch, d = w1.chain, int(w1.chain.dof)
+    rng = np.random.default_rng(175)
+    seeds = np.clip(w1.truth.reshape(1, n, d) + 0.1 * rng.normal(size=(K, n, d)), ch.q_lo, ch.q_hi).astype(np.float32).reshape(K * n, d)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)
+    out = {"workload": f"{K} candidates x {n} waypoints of one path (shared targets), Panda", "exactly_20_iterations": []}
+    for lanes in (1, 2, 4):
+        for block in (32, 64, 128):
+            s = lm.Solver(ch, K, n, w1.target_pos, w1.target_quat, seeds, params=lm.lm_default_params(lambda0=w1.lambda0, tol=0.0),
+                          shared_targets=True, device=str(device), stream=stream)
+            s.set_launch(block)
+            try:
+                if lanes > 1:
+                    s.set_lanes_per_waypoint(lanes)
+                ms, iters, _ = _time_runs(torch, s, stream, 20, reps, flush)
+            except lm.LmError as e:
+                out["exactly_20_iterations"].append({"lanes_per_waypoint": lanes, "block_threads": block, "error": str(e)})
+                s.close()
+                continue
+            s.close()
+            out["exactly_20_iterations"].append({"lanes_per_waypoint": lanes, "block_threads": block, "ms": ms, "us_per_iteration": 1e3 * ms / 20,
+                                                 "waypoint_iterations_per_sec": iters / (ms * 1e-3)})
+    s = lm.Solver(ch, K, n, w1.target_pos, w1.target_quat, seeds, params=lm.lm_default_params(lambda0=w1.lambda0, tol=1e-5),
+                  shared_targets=True, device=str(device), stream=stream)
+    ms, iters, conv = _time_runs(torch, s, stream, 50, reps, flush)
+    s.close()
+    out["to_convergence"] = {"tol": 1e-5, "ms": ms, "waypoint_iterations": int(iters), "converged_trajectories": int(conv),
+                             "waypoint_iterations_per_sec": iters / (ms * 1e-3)}
     return out
 
 
